@@ -1,0 +1,129 @@
+/*
+ * oracle/lsp_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU implementation of the Lomb-Scargle periodogram exactly as
+ * the paper DEFINES it: the two-pass form, eq. (1) with the time offset tau of
+ * eq. (2)  (section 3).  It is the yardstick the CUDA path in
+ * paper_1007_1658_b200/csrc is compared against; it shares no code, header, table
+ * or helper with that path and is never called by it.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build or call this file.
+ *
+ * No blocking, no recurrences, no refactoring (the single-pass form, eqs 5-8, is the
+ * GPU's formulation and deliberately NOT used here): for every trial frequency
+ *   1.  S2 = sum_j sin(2 w t_j),  C2 = sum_j cos(2 w t_j)           eq. (2)
+ *   2.  tau = atan2(S2, C2) / (2 w)                                  eq. (2), reading G5
+ *   3.  the four sums of eq. (1) with libm sin/cos of w (t_j - tau)
+ *   4.  P = ( XC^2/CC + XS^2/SS ) / (2 var)                          eq. (1), readings G1, G7
+ * with plain left-to-right fp64 accumulation.
+ *
+ * Readings of the paper where it is silent (DESIGN.md section "Readings"):
+ *   G1  the series is "scaled and shifted" to zero mean and unit variance
+ *       (PAPER.md:41): mean = sum x / Nt, var = sum (x-mean)^2 / (Nt-1)  (sample variance).
+ *   G2  grid f_k = f_min + k*df evaluated as f_min + (double)k*df (PAPER.md:108 generalised).
+ *   G5  tau is defined modulo pi/(2w); any branch gives the same P.  atan2(0,0) = 0.
+ *   G6  no time shift is applied here (the CUDA path shifts by t[0]; P is invariant).
+ *   G7  a term whose denominator is <= 1e-12*Nt is dropped (its numerator is 0 too);
+ *       this makes P(f=0) = 0.
+ *
+ * Parity pins (tests/test_oracle_pins.py): brute-force least squares, FFT periodogram on
+ * even sampling, time-shift invariance, closed form (Nt-1)/2, scipy.signal.lombscargle,
+ * Gaussian-noise statistics, injected sinusoid, eqs (5)-(8) equivalence, mpmath brute force.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stddef.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define LSP_ORACLE_TWO_PI 6.283185307179586476925286766559
+
+/* Mean and sample variance of x (fp32 input promoted to fp64), PAPER.md:41 + reading G1. */
+void lsp_oracle_moments(const float* x, int64_t Nt, double* mean_out, double* var_out)
+{
+    double s = 0.0;
+    for (int64_t j = 0; j < Nt; ++j) s += (double)x[j];
+    double mean = s / (double)Nt;
+    double q = 0.0;
+    for (int64_t j = 0; j < Nt; ++j) {
+        double d = (double)x[j] - mean;
+        q += d * d;
+    }
+    *mean_out = mean;
+    *var_out = q / (double)(Nt - 1);
+}
+
+/* One frequency, eqs (1)+(2).  X is the mean-subtracted series in fp64. */
+static double lsp_oracle_one(const double* t, const double* X, int64_t Nt, double f, double var)
+{
+    const double w = LSP_ORACLE_TWO_PI * f;
+    if (w == 0.0) {
+        /* eq. (1) with w = 0: cos = 1, sin = 0; the sine term is 0/0 and dropped (G7). */
+        double xc = 0.0;
+        for (int64_t j = 0; j < Nt; ++j) xc += X[j];
+        return (xc * xc / (double)Nt) / (2.0 * var);
+    }
+    double S2 = 0.0, C2 = 0.0;                       /* eq. (2) */
+    for (int64_t j = 0; j < Nt; ++j) {
+        double a = 2.0 * w * t[j];
+        S2 += sin(a);
+        C2 += cos(a);
+    }
+    const double tau = atan2(S2, C2) / (2.0 * w);    /* G5 */
+    double XC = 0.0, XS = 0.0, CC = 0.0, SS = 0.0;   /* eq. (1) */
+    for (int64_t j = 0; j < Nt; ++j) {
+        double a = w * (t[j] - tau);
+        double c = cos(a), s = sin(a);
+        XC += X[j] * c;
+        XS += X[j] * s;
+        CC += c * c;
+        SS += s * s;
+    }
+    const double eps = 1e-12 * (double)Nt;           /* G7 */
+    double p = 0.0;
+    if (CC > eps) p += XC * XC / CC;
+    if (SS > eps) p += XS * XS / SS;
+    return p / (2.0 * var);
+}
+
+/*
+ * Periodogram of one series on selected grid points.
+ *   t[Nt] fp64, x[Nt] fp32 (host), grid f_k = f_min + k*df.
+ *   ks == NULL : evaluate k = 0..nk-1;  otherwise evaluate k = ks[i], i = 0..nk-1.
+ *   P[nk] fp64 out.  scratch[Nt] fp64 (caller-provided, holds x - mean).
+ *   nthreads <= 0 : use the OpenMP default.  Returns the number of threads used.
+ */
+int lsp_oracle_periodogram(const double* t, const float* x, int64_t Nt,
+                           double f_min, double df, const int64_t* ks, int64_t nk,
+                           double* P, double* scratch, int nthreads)
+{
+    double mean, var;
+    lsp_oracle_moments(x, Nt, &mean, &var);
+    for (int64_t j = 0; j < Nt; ++j) scratch[j] = (double)x[j] - mean;
+    int used = 1;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    #pragma omp parallel
+    {
+        #pragma omp single
+        used = omp_get_num_threads();
+    }
+    #pragma omp parallel for schedule(dynamic, 4)
+#endif
+    for (int64_t i = 0; i < nk; ++i) {
+        int64_t k = ks ? ks[i] : i;
+        double f = f_min + (double)k * df;           /* G2 */
+        P[i] = lsp_oracle_one(t, scratch, Nt, f, var);
+    }
+    return used;
+}
+
+/* Lowest index among equal maxima (reading G9). */
+int64_t lsp_oracle_argmax(const double* P, int64_t n)
+{
+    int64_t best = 0;
+    for (int64_t i = 1; i < n; ++i)
+        if (P[i] > P[best]) best = i;
+    return best;
+}

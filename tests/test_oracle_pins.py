@@ -1,0 +1,286 @@
+"""Pins for the fp64 oracle (oracle/lsp_oracle.c and its numpy twin), CPU only.
+
+Each test fixes the oracle against something that is NOT the oracle: a least-squares
+fit, numpy's FFT, a closed form, scipy's own Lomb-Scargle, an invariance, mpmath
+brute force, Gaussian-noise statistics.  Numbering P1..P9 follows DESIGN.md ("Pins").
+Equation / line references are to /root/reference/PAPER.md (Townsend 2010).
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _series(Nt, seed, T=20.0, f_inj=0.9):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    t = np.sort(rng.uniform(0.0, T, Nt))
+    x = (np.sin(2 * np.pi * f_inj * t + 0.3) + rng.normal(0.0, 0.7, Nt)).astype(np.float32)
+    return t, x
+
+
+def _grid(f_lo, f_hi, Nf):
+    return f_lo, (f_hi - f_lo) / (Nf - 1)
+
+
+def _c_and_numpy(t, x, f_min, df, Nf):
+    Pc = oracle.periodogram(t, x, f_min, df, Nf)
+    Pn = oracle.periodogram_numpy(t, x, f_min + np.arange(Nf) * df)
+    return Pc, Pn
+
+
+# ------------------------------------------------------------------ C build vs numpy twin
+def test_c_oracle_matches_numpy_twin():
+    t, x = _series(257, 11)
+    f_min, df = _grid(0.05, 6.0, 301)
+    Pc, Pn = _c_and_numpy(t, x, f_min, df, 301)
+    assert np.max(np.abs(Pc - Pn)) <= 1e-11 * np.max(Pn)
+
+
+def test_subset_indices_match_full_grid():
+    t, x = _series(300, 12)
+    f_min, df = _grid(0.05, 6.0, 400)
+    full = oracle.periodogram(t, x, f_min, df, 400)
+    ks = np.array([0, 3, 17, 399, 200, 200], dtype=np.int64)
+    sub = oracle.periodogram(t, x, f_min, df, 400, ks=ks)
+    assert np.array_equal(sub, full[ks])
+
+
+def test_thread_count_does_not_change_result():
+    t, x = _series(300, 13)
+    f_min, df = _grid(0.05, 6.0, 64)
+    a = oracle.periodogram(t, x, f_min, df, 64, nthreads=1)
+    b, used = oracle.periodogram(t, x, f_min, df, 64, nthreads=2, return_threads=True)
+    assert used == 2
+    assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ P1 least squares
+@pytest.mark.parametrize("Nt,seed", [(10, 1), (23, 2), (40, 3)])
+def test_P1_least_squares_chi2_reduction(Nt, seed):
+    """P*2*var = sum X^2 - min chi^2 of the fit X ~ a cos wt + b sin wt (2x2 normal equations).
+
+    Fixes eq. (1) including tau of eq. (2) and both denominators."""
+    t, x = _series(Nt, seed, T=10.0)
+    X = x.astype(np.float64)
+    X = X - X.mean()
+    var = (X * X).sum() / (Nt - 1)
+    freqs = np.linspace(0.07, 3.1, 37)
+    expect = np.empty_like(freqs)
+    for i, f in enumerate(freqs):
+        A = np.stack([np.cos(2 * np.pi * f * t), np.sin(2 * np.pi * f * t)], axis=1)
+        N = A.T @ A
+        rhs = A.T @ X
+        ab = np.linalg.solve(N, rhs)
+        chi2 = ((X - A @ ab) ** 2).sum()
+        expect[i] = ((X * X).sum() - chi2) / (2.0 * var)
+    got_np = oracle.periodogram_numpy(t, x, freqs)
+    assert np.max(np.abs(got_np - expect)) <= 1e-11 * np.max(expect)
+    f_min, df = freqs[0], freqs[1] - freqs[0]
+    got_c = oracle.periodogram(t, x, f_min, df, freqs.size)
+    assert np.max(np.abs(got_c - expect)) <= 1e-10 * np.max(expect)
+
+
+# ------------------------------------------------------------------ P2 FFT periodogram
+@pytest.mark.parametrize("N", [64, 250])
+def test_P2_even_sampling_equals_fft_periodogram(N):
+    """t_j = j*dt, Fourier frequencies k/(N dt), 0<k<N/2:  P_k = |FFT(X)_k|^2 / (N var)."""
+    w = workloads.even_sampling(N, dt=0.25, seed=5)
+    X = w.x.astype(np.float64)
+    X = X - X.mean()
+    var = (X * X).sum() / (N - 1)
+    F = np.fft.fft(X)
+    k = np.arange(1, N // 2)
+    expect = np.abs(F[k]) ** 2 / (N * var)
+    got = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    assert got.shape == expect.shape
+    assert np.max(np.abs(got - expect)) <= 1e-11 * np.max(expect)
+
+
+# ------------------------------------------------------------------ P3 shift invariance
+def test_P3_time_shift_invariance():
+    """P[t] = P[t + c] (tau of eq. (2) absorbs the origin)."""
+    t, x = _series(500, 21, T=50.0)
+    f_min, df = _grid(0.02, 5.0, 500)
+    a = oracle.periodogram(t, x, f_min, df, 500)
+    b = oracle.periodogram(t + 1234.567, x, f_min, df, 500)
+    c = oracle.periodogram(t - 77.25, x, f_min, df, 500)
+    assert np.max(np.abs(a - b)) <= 1e-9 * np.max(a)
+    assert np.max(np.abs(a - c)) <= 1e-9 * np.max(a)
+
+
+def test_affine_invariance_in_x():
+    """The series is 'scaled and shifted' to zero mean, unit variance: P[a x + b] = P[x]."""
+    t, x = _series(300, 22)
+    f_min, df = _grid(0.05, 4.0, 200)
+    a = oracle.periodogram(t, x, f_min, df, 200)
+    x2 = (4.0 * x.astype(np.float64) + 8.0).astype(np.float32)      # exact in fp32: power-of-two scale, small shift
+    b = oracle.periodogram(t, x2, f_min, df, 200)
+    assert np.max(np.abs(a - b)) <= 1e-5 * np.max(a)                 # fp32 rounding of x2 only
+
+
+# ------------------------------------------------------------------ P4 closed form
+def test_P4_pure_sinusoid_closed_form():
+    """Even sampling, whole cycles: P = (Nt-1)/2 at its own Fourier frequency, 0 at the others (pins G1)."""
+    N, dt, k0 = 128, 0.5, 9
+    t = np.arange(N) * dt
+    x = np.sin(2 * np.pi * k0 / (N * dt) * t + 0.4).astype(np.float64)
+    df = 1.0 / (N * dt)
+    # feed float64-exact values through the numpy twin (float32 cast perturbs at 1e-7)
+    P32 = oracle.periodogram(t, x.astype(np.float32), df, df, N // 2 - 1)
+    assert abs(P32[k0 - 1] - (N - 1) / 2.0) <= 1e-5
+    others = np.delete(P32, k0 - 1)
+    assert np.max(np.abs(others)) <= 1e-10
+    assert np.all(P32 <= (N - 1) / 2.0 + 1e-9)
+
+
+# ------------------------------------------------------------------ P5 scipy
+def test_P5_scipy_lombscargle():
+    """scipy.signal.lombscargle (independent code) / var equals the oracle."""
+    from scipy.signal import lombscargle
+    t, x = _series(400, 31, T=40.0)
+    f_min, df = _grid(0.03, 4.0, 300)
+    freqs = f_min + np.arange(300) * df
+    X = x.astype(np.float64)
+    X = X - X.mean()
+    var = (X * X).sum() / (X.size - 1)
+    expect = lombscargle(t, X, 2 * np.pi * freqs) / var
+    got = oracle.periodogram(t, x, f_min, df, 300)
+    assert np.max(np.abs(got - expect)) <= 1e-10 * np.max(expect)
+
+
+# ------------------------------------------------------------------ P6 noise statistics
+def test_P6_gaussian_noise_mean_power_is_one():
+    """Pure Gaussian noise: P is beta-distributed with mean 1 under the N-1 variance (G1)."""
+    w = workloads.c4(B=96, Nt=200, Nf=150, seed=99)
+    P, idx, val = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
+    assert P.shape == (96, 150)
+    m = P.mean()
+    assert abs(m - 1.0) < 0.03, m
+    assert np.all(P >= 0.0) and np.all(P <= (200 - 1) / 2.0)
+    assert np.array_equal(idx, P.argmax(axis=1))
+    assert np.array_equal(val, P.max(axis=1))
+    # peaks of ~100 independent frequencies: Gumbel-like, mean ~ ln(Nind)+0.58, std ~ pi/sqrt(6)
+    assert 3.5 < val.mean() < 7.5
+    assert 0.6 < val.std() < 2.2
+
+
+# ------------------------------------------------------------------ P7 injected sinusoid
+def test_P7_injected_sinusoid_recovered_C1():
+    w = workloads.c1()
+    P = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    k = oracle.argmax(P)
+    assert abs(k - w.expected_peak_bin) <= 1.0
+    # amplitude 1, noise 0.5: var ~ 0.75, P_peak ~ Nt A^2 / (4 var)
+    assert 0.8 * 1000 / (4 * 0.75) < P[k] < 1.2 * 1000 / (4 * 0.75)
+
+
+# ------------------------------------------------------------------ P8 single-pass form
+def test_P8_single_pass_and_trigfree_forms_agree():
+    """eqs (1)-(2) == eqs (5)-(8) == the atan2-free combine used by the CUDA finish step.
+
+    Written out here from the paper, independent of both implementations."""
+    t, x = _series(333, 41, T=30.0)
+    X = x.astype(np.float64)
+    X = X - X.mean()
+    Nt = X.size
+    var = (X * X).sum() / (Nt - 1)
+    freqs = np.linspace(0.04, 5.0, 211)
+    ref = oracle.periodogram_numpy(t, x, freqs)
+    for i, f in enumerate(freqs):
+        w = 2 * np.pi * f
+        c, s = np.cos(w * t), np.sin(w * t)
+        XC, XS, CC, SS, CS = (X * c).sum(), (X * s).sum(), (c * c).sum(), (s * s).sum(), (c * s).sum()
+        wt = 0.5 * np.arctan2(2 * CS, CC - SS)                       # eq. (6)
+        ct, st = np.cos(wt), np.sin(wt)                              # eq. (7)
+        p5 = 0.5 * ((ct * XC + st * XS) ** 2 / (ct * ct * CC + 2 * ct * st * CS + st * st * SS)
+                    + (ct * XS - st * XC) ** 2 / (ct * ct * SS - 2 * ct * st * CS + st * st * CC))  # eq. (5)
+        assert abs(p5 / var - ref[i]) <= 1e-10 * max(1.0, ref[i])
+        A, B = 2 * CC - Nt, 2 * CS                                   # SS = Nt - CC
+        R = np.hypot(A, B)
+        S = XC * XC + XS * XS
+        D = ((XC * XC - XS * XS) * A + 2 * XC * XS * B) / R
+        p6 = ((S + D) / (Nt + R) + (S - D) / (Nt - R)) / (2 * var)
+        assert abs(p6 - ref[i]) <= 1e-10 * max(1.0, ref[i])
+
+
+# ------------------------------------------------------------------ P9 mpmath brute force
+def test_P9_mpmath_brute_force_tiny():
+    import mpmath as mp
+    mp.mp.dps = 50
+    t, x = _series(12, 51, T=7.0)
+    freqs = [0.11, 0.73, 2.9]
+    got = oracle.periodogram_numpy(t, x, freqs)
+    f_min, df = 0.11, 0.62
+    got_c = oracle.periodogram(t, x, f_min, df, 2)                   # 0.11, 0.73
+    tm = [mp.mpf(float(v)) for v in t]
+    xm = [mp.mpf(float(v)) for v in x]
+    N = len(tm)
+    mean = sum(xm) / N
+    Xm = [v - mean for v in xm]
+    var = sum(v * v for v in Xm) / (N - 1)
+    for i, f in enumerate(freqs):
+        w = 2 * mp.pi * mp.mpf(f)
+        tau = mp.atan2(sum(mp.sin(2 * w * tj) for tj in tm), sum(mp.cos(2 * w * tj) for tj in tm)) / (2 * w)
+        cs = [mp.cos(w * (tj - tau)) for tj in tm]
+        ss = [mp.sin(w * (tj - tau)) for tj in tm]
+        p = (sum(a * b for a, b in zip(Xm, cs)) ** 2 / sum(c * c for c in cs)
+             + sum(a * b for a, b in zip(Xm, ss)) ** 2 / sum(s * s for s in ss)) / (2 * var)
+        assert abs(float(p) - got[i]) <= 1e-12 * max(1.0, float(p))
+        if i < 2:
+            assert abs(float(p) - got_c[i]) <= 1e-11 * max(1.0, float(p))
+
+
+# ------------------------------------------------------------------ degenerate readings
+def test_G7_zero_frequency_and_nyquist_are_finite():
+    N = 32
+    t = np.arange(N, dtype=np.float64)
+    rng = np.random.Generator(np.random.PCG64(3))
+    x = rng.normal(size=N).astype(np.float32)
+    P0 = oracle.periodogram(t, x, 0.0, 0.5, 2)        # f = 0 and f = Nyquist (sin wt = 0 for all j)
+    assert np.all(np.isfinite(P0))
+    assert abs(P0[0]) < 1e-12                          # zero-mean series: XC = 0 at f = 0
+    X = x.astype(np.float64) - x.astype(np.float64).mean()
+    var = (X * X).sum() / (N - 1)
+    alt = (X * np.cos(np.pi * t)).sum() ** 2 / N / (2 * var)
+    assert abs(P0[1] - alt) <= 1e-9 * max(1.0, alt)
+
+
+def test_G9_argmax_lowest_index_on_ties():
+    assert oracle.argmax(np.array([1.0, 5.0, 5.0, 2.0])) == 1
+    assert oracle.argmax(np.array([7.0])) == 0
+
+
+def test_moments_sample_variance():
+    rng = np.random.Generator(np.random.PCG64(8))
+    x = rng.normal(3.0, 2.0, 1001).astype(np.float32)
+    m, v = oracle.moments(x)
+    xd = x.astype(np.float64)
+    assert abs(m - xd.mean()) < 1e-12
+    assert abs(v - xd.var(ddof=1)) < 1e-12
+
+
+def test_fap_eq3_limits():
+    """Eq. (3): Q(0) = 1, Q decreasing in P, Q -> Nf*(1-2P/Nt)^((Nt-3)/2) for small Q."""
+    Q = oracle.false_alarm_probability(np.array([0.0, 5.0, 10.0, 20.0]), 1000, 500)
+    assert Q[0] == 1.0
+    assert np.all(np.diff(Q) < 0)
+    approx = 500 * (1 - 2 * 20.0 / 1000) ** ((1000 - 3) / 2)
+    assert abs(Q[3] - approx) / approx < 1e-3
+
+
+def test_paper_facts_fixture():
+    """Numbers printed in the paper (tests/golden/paper_facts.json) are self-consistent."""
+    with open(os.path.join(HERE, "golden", "paper_facts.json")) as fh:
+        facts = json.load(fh)
+    Nt, Nf = facts["validation_Nt"]["value"], facts["validation_Nf"]["value"]
+    assert Nf % facts["block_size"]["value"] == 0          # reading G8: Nf rounded up to blocks of 256
+    assert Nf * (4 * Nt + 1) > Nf * (2 * Nt + 3)           # PAPER.md:59 vs :86, "factor ~2"
+    assert abs(Nf * (4 * Nt + 1) / (Nf * (2 * Nt + 3)) - 2.0) < 1e-4
+    tc = facts["t_calc_s"]
+    assert abs(tc["cpu8"] / tc["C1060"] - 28) < 1.0        # "approaching thirty" (abstract)

@@ -1,0 +1,185 @@
+"""Seeded synthetic input generators shared by the oracle side and the CUDA side.
+
+This module holds NONE of the method's arithmetic (no trig sums, no periodogram,
+no normalisation): it only draws time stamps and measurement values with numpy's
+counter-free PCG64 generator and states the frequency grid of each configuration.
+Both `oracle/` (through the tests) and the CUDA path (through the tests and
+`bench.py`) read their inputs from here; neither side imports the other.
+
+The recipes stand in for the workloads the paper describes and are the five
+`BASELINE.json` configs:
+
+  C1  small single series, uniform-random times                (sec. 3)
+  C2  gappy ground-based survey sampling                        (sec. 6.2)
+  C3  satellite-like photometry with periodic gaps
+  C4  Monte-Carlo batch of pure-noise series                    (sec. 6.2)
+  C5  large survey, Nt = Nf = 1e6
+  P0  paper-shaped: Nt=382,003 over 150 d, Nf=1,528,064
+
+The paper's only dataset (CoRoT photometry of V1449 Aql) is not available and is
+not reproduced; P0 only copies its *shape* (counts, span, grid).
+
+All times are float64 days, values float32, frequencies cycles/day.  The grid is
+f_k = f_min + k*df, k = 0..Nf-1, both ends of the stated range included
+(df = (f_max - f_min)/(Nf - 1)), reading G2.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+BASE_SEED = 1007165800          # seed_i = BASE_SEED + i (+ bump, see SEED_BUMP)
+
+# Seed qualification (reading G9): if the oracle finds the two largest
+# powers of a config closer than 1e-5*max(P), the seed is bumped by one and the
+# bump recorded here.  `tests/golden/qualify_seeds.py` (oracle only) re-derives it.
+SEED_BUMP = {1: 0, 2: 0, 3: 0, 4: 0, 5: 0, 0: 0}
+
+
+@dataclass
+class Workload:
+    name: str
+    t: np.ndarray                 # float64 [Nt] or [B, Nt]
+    x: np.ndarray                 # float32 [Nt] or [B, Nt]
+    f_min: float
+    df: float
+    Nf: int
+    B: int = 1                    # number of independent series (batched when > 1)
+    T: float = 0.0                # nominal span used for the grid
+    expected_peak_bin: Optional[float] = None   # fractional bin of the injected signal
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def Nt(self) -> int:
+        return int(self.t.shape[-1])
+
+    @property
+    def terms(self) -> int:
+        return int(self.B) * self.Nt * int(self.Nf)
+
+    def freqs(self) -> np.ndarray:
+        return self.f_min + np.arange(self.Nf, dtype=np.float64) * self.df
+
+
+def _seed(i: int) -> int:
+    return BASE_SEED + i + SEED_BUMP.get(i, 0)
+
+
+def _grid(f_lo: float, f_hi: float, Nf: int):
+    df = (f_hi - f_lo) / (Nf - 1) if Nf > 1 else 0.0
+    return float(f_lo), float(df)
+
+
+def c1(Nt: int = 1000, Nf: int = 1000, seed: Optional[int] = None) -> Workload:
+    """C1: Nt uniform-random sorted times on [0,100) d; x = sin(2 pi 0.37 t) + N(0, 0.5^2)."""
+    rng = np.random.Generator(np.random.PCG64(_seed(1) if seed is None else seed))
+    T = 100.0
+    t = np.sort(rng.uniform(0.0, T, Nt))
+    x = np.sin(2.0 * np.pi * 0.37 * t) + rng.normal(0.0, 0.5, Nt)
+    f_min, df = _grid(1.0 / T, Nt / (2.0 * T), Nf)
+    return Workload("C1", t, x.astype(np.float32), f_min, df, Nf, T=T,
+                    expected_peak_bin=(0.37 - f_min) / df if df > 0 else None)
+
+
+def c2(Nt: int = 10000, Nf: int = 10000, seed: Optional[int] = None) -> Workload:
+    """C2: 365 nights, 30 % dropped, 8 h windows, jittered; 3 sinusoids + N(0,1)."""
+    rng = np.random.Generator(np.random.PCG64(_seed(2) if seed is None else seed))
+    n_nights, n_drop = 365, 110
+    kept = np.sort(rng.permutation(n_nights)[n_drop:])           # 255 nights kept
+    n_kept = kept.size
+    slots = 40
+    i = np.arange(Nt)
+    night = kept[i % n_kept]
+    slot = (i // n_kept) % slots
+    wrap = i // (n_kept * slots)                                  # only when Nt > 255*40
+    t = night + (slot + rng.uniform(0.0, 1.0, Nt) + wrap * 1e-3) / slots * (8.0 / 24.0)
+    t = np.sort(t)
+    g = rng.uniform(0.1, 5.0, 3)
+    a = rng.uniform(0.2, 1.0, 3)
+    ph = rng.uniform(0.0, 2.0 * np.pi, 3)
+    x = rng.normal(0.0, 1.0, Nt)
+    for m in range(3):
+        x = x + a[m] * np.sin(2.0 * np.pi * g[m] * t + ph[m])
+    T = 365.0
+    f_min, df = _grid(1.0 / T, 10.0, Nf)
+    return Workload("C2", t, x.astype(np.float32), f_min, df, Nf, T=T,
+                    meta={"freqs": g.tolist(), "amps": a.tolist(), "phases": ph.tolist()})
+
+
+def c3(Nt: int = 100000, Nf: int = 1000000, seed: Optional[int] = None) -> Workload:
+    """C3: 30-min cadence, 3-d gap every 90 d; 1e-3 sinusoid at 0.731 c/d + AR(1) red noise + white."""
+    rng = np.random.Generator(np.random.PCG64(_seed(3) if seed is None else seed))
+    n_cand = int(Nt * 90.0 / 87.0) + 4800
+    tc = np.arange(n_cand, dtype=np.float64) / 48.0
+    tc = tc[np.mod(tc, 90.0) < 87.0][:Nt]
+    assert tc.size == Nt
+    amp = 1e-3
+    eps = rng.normal(0.0, amp * np.sqrt(1.0 - 0.81), Nt)
+    r = np.empty(Nt)
+    acc = 0.0
+    for j in range(Nt):                                           # AR(1), phi = 0.9, by sample index
+        acc = 0.9 * acc + eps[j]
+        r[j] = acc
+    x = amp * np.sin(2.0 * np.pi * 0.731 * tc) + r + rng.normal(0.0, amp, Nt)
+    T = Nt / 48.0
+    f_min, df = _grid(1.0 / T, 24.0, Nf)
+    return Workload("C3", tc, x.astype(np.float32), f_min, df, Nf, T=T,
+                    expected_peak_bin=(0.731 - f_min) / df)
+
+
+def c4(B: int = 4096, Nt: int = 1000, Nf: int = 2000, seed: Optional[int] = None) -> Workload:
+    """C4: B independent white-noise series, each with its own uniform-random times on [0,50) d."""
+    ss = np.random.SeedSequence(_seed(4) if seed is None else seed)
+    children = ss.spawn(B)
+    T = 50.0
+    t = np.empty((B, Nt), dtype=np.float64)
+    x = np.empty((B, Nt), dtype=np.float32)
+    for b in range(B):
+        rng = np.random.Generator(np.random.PCG64(children[b]))
+        t[b] = np.sort(rng.uniform(0.0, T, Nt))
+        x[b] = rng.normal(0.0, 1.0, Nt).astype(np.float32)
+    f_min, df = _grid(1.0 / T, Nt / (2.0 * T), Nf)
+    return Workload("C4", t, x, f_min, df, Nf, B=B, T=T)
+
+
+def c5(Nt: int = 1000000, Nf: int = 1000000, seed: Optional[int] = None) -> Workload:
+    """C5: Nt uniform-random sorted times on [0,3650) d; x = 0.05 sin(2 pi 1.2345 t) + N(0,1)."""
+    rng = np.random.Generator(np.random.PCG64(_seed(5) if seed is None else seed))
+    T = 3650.0
+    t = np.sort(rng.uniform(0.0, T, Nt))
+    x = 0.05 * np.sin(2.0 * np.pi * 1.2345 * t) + rng.normal(0.0, 1.0, Nt)
+    f_min, df = _grid(1.0 / T, 50.0, Nf)
+    return Workload("C5", t, x.astype(np.float32), f_min, df, Nf, T=T,
+                    expected_peak_bin=(1.2345 - f_min) / df)
+
+
+def p0(Nt: int = 382003, Nf: int = 1528064, seed: Optional[int] = None) -> Workload:
+    """P0: paper-shaped run: 150 d, mean spacing ~34 s, grid f_i = i*df."""
+    rng = np.random.Generator(np.random.PCG64(_seed(0) if seed is None else seed))
+    T = 150.0
+    jit = 8.0 / 86400.0
+    t = np.sort(np.arange(Nt) * (T / Nt) + rng.uniform(-jit, jit, Nt))
+    f_inj = 1.0 / 0.18
+    x = np.sin(2.0 * np.pi * f_inj * t) + rng.normal(0.0, 1.0, Nt)
+    df = 1.0 / (4.0 * T)                                          # F_over = 4 (reading G11)
+    return Workload("P0", t, x.astype(np.float32), df, df, Nf, T=T,
+                    expected_peak_bin=f_inj / df - 1.0)
+
+
+_FACTORY = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "C5": c5, "P0": p0}
+
+
+def make(name: str, **kw) -> Workload:
+    """Build a configuration by name ('C1'..'C5', 'P0'); kwargs override the sizes."""
+    return _FACTORY[name.upper()](**kw)
+
+
+def even_sampling(N: int, dt: float = 1.0, seed: int = 7) -> Workload:
+    """Evenly sampled white noise + grid of Fourier frequencies k/(N dt), k = 1..N/2-1 (test helper)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    t = np.arange(N, dtype=np.float64) * dt
+    x = rng.normal(0.0, 1.0, N).astype(np.float32)
+    df = 1.0 / (N * dt)
+    return Workload("EVEN", t, x, df, df, N // 2 - 1, T=N * dt)

@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- Lomb-Scargle term-evaluation throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (moments -> records -> accumulate -> finish, all rows of
+SURVEY.md section 8(a)) over one seeded synthetic workload.  N = 1 times BASELINE.json's headline config
+C5 (Nt = Nf = 1e6, one series).  N > 1 (torchrun): every rank runs its own series of the same shape
+(weak scaling, no data-path collective: the path shards by independent series / frequencies,
+SURVEY.md section 8(e)); value = all ranks' terms / max-over-ranks time.
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the fp64 oracle (oracle/, the CPU baseline)
+on a bounded sample of the same workload instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402  (seeded input generators; hold none of the method's arithmetic)
+
+METRIC = "lomb_scargle_term_evals_per_s"
+UNIT = "terms/s"
+FP32_LANES_PER_SM = 128          # B200: 4 SMSPs x 32 FP32 lanes (guide: blackwell_cuda_programming.md)
+
+
+# ----------------------------------------------------------------------------- helpers (host logic)
+def rank_seed(workload: str, rank: int):
+    """Seed of rank r's series: the config's own seed for rank 0, +1000*r for the others."""
+    idx = {"C1": 1, "C2": 2, "C3": 3, "C4": 4, "C5": 5, "P0": 0}[workload.upper()]
+    return None if rank == 0 else workloads.BASE_SEED + idx + 1000 * rank
+
+
+def reduce_max(value: float, dist=None) -> float:
+    """Max over ranks of a scalar (device time); identity when not distributed."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64)
+    if dist.get_backend() == "nccl":
+        t = t.cuda()
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(terms_per_rank: int, world: int, max_seconds: float) -> float:
+    return terms_per_rank * world / max_seconds
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh)
+    return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int = 0):
+        self.proc = None
+        self.lines = []
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- oracle legs (CPU)
+def time_oracle(w, seconds_target: float = 12.0, max_freqs: int = 4096):
+    """Time the fp64 oracle, as it stands, on a strided subset of the workload's frequency grid.
+
+    Returns (terms_per_s, cores, sample_description, elapsed_s)."""
+    import oracle
+    t = w.t[0] if w.B > 1 else w.t
+    x = w.x[0] if w.B > 1 else w.x
+    cores = oracle.host_threads()
+    oracle.periodogram(t[:1000], x[:1000], w.f_min, w.df, 8)          # build + warm the library
+    done, elapsed, n = 0, 0.0, max(8, cores * 4)
+    while elapsed < seconds_target and done < max_freqs:
+        n = min(n, max_freqs - done)
+        stride = max(1, w.Nf // n)
+        ks = (np.arange(n, dtype=np.int64) * stride + done % stride) % w.Nf
+        t0 = time.perf_counter()
+        _, used = oracle.periodogram(t, x, w.f_min, w.df, w.Nf, ks=ks, return_threads=True)
+        dt = time.perf_counter() - t0
+        elapsed += dt; done += n; cores = used
+        rate = n * w.Nt / dt
+        n = int(min(max_freqs, max(n, rate * (seconds_target - elapsed) / w.Nt * 0.9))) or 1
+        if seconds_target - elapsed < 0.5:
+            break
+    terms = done * w.Nt
+    sample = "%d of %d frequencies (strided) x Nt=%d samples of %s%s" % (
+        done, w.Nf, w.Nt, w.name, " series 0" if w.B > 1 else "")
+    return terms / elapsed, cores, sample, elapsed
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, bounded sample per step; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    w = workloads.make(args.workload)
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        time_oracle(w, seconds_target=min(per_step, 2.0))
+    rates, cores, sample = [], 1, ""
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r, cores, sample, _ = time_oracle(w, seconds_target=per_step)
+        rates.append(r)
+    wall = time.perf_counter() - t0
+    value = statistics.mean(rates)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "Nt": w.Nt, "Nf": w.Nf, "series": w.B,
+                   "note": "fp64 two-pass oracle (oracle/lsp_oracle.c, OpenMP) on a strided frequency subset"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- our arm (GPU)
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1007_1658_b200 as lsp
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = workloads.make(args.workload, seed=rank_seed(args.workload, rank))
+    batched = w.B > 1
+    h = lsp.Handle(local)
+    for key, val in ((lsp.PARAM_K, args.K), (lsp.PARAM_THREADS, args.threads), (lsp.PARAM_NSPLIT, args.nsplit),
+                     (lsp.PARAM_RECURRENCE, args.recurrence), (lsp.PARAM_FLUSH, args.flush)):
+        if val:
+            h.set_param(key, val)
+    h.set_param(lsp.PARAM_TIMING, 1)
+
+    t_h = torch.from_numpy(np.ascontiguousarray(w.t)).pin_memory()
+    x_h = torch.from_numpy(np.ascontiguousarray(w.x)).pin_memory()
+    t_d, x_d = t_h.cuda(), x_h.cuda()
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")        # > 126 MB L2
+
+    def step_device():
+        if batched:
+            return h.periodogram_batched(t_d, x_d, w.f_min, w.df, w.Nf)
+        return h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf)
+
+    P_h = torch.empty((w.B, w.Nf) if batched else (w.Nf,), dtype=torch.float32).pin_memory()
+    pi_h = torch.empty(w.B, dtype=torch.int32).pin_memory()
+    pv_h = torch.empty(w.B, dtype=torch.float32).pin_memory()
+
+    def step_host():
+        if batched:
+            h.periodogram_batched_host(t_h, x_h, w.f_min, w.df, w.Nf, P=P_h, peak_idx=pi_h, peak_val=pv_h)
+        else:
+            h.periodogram_host(t_h, x_h, w.f_min, w.df, w.Nf, out=P_h)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step_device()
+    torch.cuda.synchronize()
+
+    # ---- timed region 1: device-resident inputs
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kern_ms, all_ms = [], []
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        flush_buf.zero_()                                   # L2 flush between timed iterations
+        step_device()
+        tm = h.last_timing()                                # events on the launching stream, per kernel
+        kern_ms.append(tm["accumulate"]); all_ms.append(sum(tm.values()))
+    ev1.record()
+    barrier()
+    total_ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    flush_ms = 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        flush_buf.zero_()
+    e1.record(); torch.cuda.synchronize()
+    flush_ms = e0.elapsed_time(e1)
+    ms_per_step = reduce_max((total_ms - flush_ms) / args.steps, dist if world > 1 else None)
+    plan = h.last_plan()
+
+    # ---- timed region 2: end to end through the host-buffer C-ABI call (H2D + compute + D2H)
+    for _ in range(2):
+        step_host()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_host()
+    torch.cuda.synchronize()
+    e2e_s = reduce_max((time.perf_counter() - t0) / args.steps, dist if world > 1 else None)
+    h2d = t_h.numel() * 8 + x_h.numel() * 4
+    d2h = P_h.numel() * 4 + (pi_h.numel() * 8 if batched else 0)
+
+    if rank != 0:
+        h.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    value = aggregate_value(w.terms, world, ms_per_step * 1e-3)
+    # ---- roofline of the dominant kernel (accumulate): FP32 pipe, FMA = 2 FLOP per lane-op
+    peaks = measured_peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    k_ms = statistics.mean(kern_ms)
+    lane_ops = plan["lane_ops_per_term"]
+    achieved = w.terms * lane_ops * 2 / (k_ms * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+        "traffic": None, "kernel": plan["kernel"], "kernel_ms": k_ms, "kernel_share_of_step": k_ms / statistics.mean(all_ms),
+        "lane_ops_per_term": lane_ops,
+        "peak_basis": "%d SMs x 128 FP32 lanes x 2 FLOP x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)" % (n_sm, sm_max),
+        "frac_at_measured_clock": (achieved / (n_sm * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
+                                   if clocks and clocks.get("sm_mhz") else None),
+        "hbm_GBps_algorithmic": (12.0 * w.B * w.Nt + 4.0 * w.B * w.Nf) / (k_ms * 1e-3) / 1e9,
+    }
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        try:
+            with open(prof) as fh:
+                roofline["traffic"] = json.load(fh).get(w.name)
+        except Exception:
+            pass
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        r, cores, sample, _ = time_oracle(w, seconds_target=args.cpu_seconds)
+        cpu = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "Nt": w.Nt, "Nf": w.Nf, "series": w.B, "terms_per_step": w.terms,
+                   "l2": "flushed between timed iterations (256 MB write)", "plan": plan,
+                   "parallelism": "independent series per rank" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": aggregate_value(w.terms, world, e2e_s), "unit": UNIT, "ms_per_step": e2e_s * 1e3,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": plan["launches"] * args.steps,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C5")
+    ap.add_argument("--K", type=int, default=0)
+    ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--nsplit", type=int, default=0)
+    ap.add_argument("--recurrence", type=int, default=0)
+    ap.add_argument("--flush", type=int, default=0)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,147 @@
+/*
+ * lsp.h -- C ABI of the B200-native direct Lomb-Scargle periodogram library.
+ *
+ * The operation (Townsend 2010, arxiv 1007.1658; line numbers are /root/reference/PAPER.md):
+ * for a time series (t_j, x_j), j = 0..Nt-1, shifted and scaled to zero mean and unit
+ * variance, and a uniform frequency grid f_k = f_min + k*df, k = 0..Nf-1
+ * (eq. (9), generalised to a free f_min), compute the normalised periodogram
+ *
+ *     P(f) = 1/2 { [sum_j X_j cos w(t_j - tau)]^2 / sum_j cos^2 w(t_j - tau)
+ *                + [sum_j X_j sin w(t_j - tau)]^2 / sum_j sin^2 w(t_j - tau) },   w = 2 pi f   (eq. 1)
+ *     tan 2 w tau = sum_j sin 2 w t_j / sum_j cos 2 w t_j                                        (eq. 2)
+ *
+ * evaluated through the single-pass sums XC, XS, CC, CS of eqs (5)-(8) with
+ * SS = Nt - CC.  X_j = x_j - mean(x); the variance is the sample variance
+ * sum X_j^2 / (Nt - 1) (reading G1).  Cost is O(Nt*Nf) "term evaluations" (eq. 4).
+ *
+ * Conventions
+ *   - Pointers marked DEVICE are CUDA device pointers on the handle's device; pointers marked
+ *     HOST are ordinary (pageable or pinned) host pointers.  The caller owns every array; the
+ *     library never frees or reallocates caller memory.  The handle owns a device workspace
+ *     that grows to the largest call seen (growth may synchronise the device once).
+ *   - Device-pointer entry points only ENQUEUE work on `stream` (a cudaStream_t passed as
+ *     void*; NULL = legacy default stream) and return without synchronising; inputs must stay
+ *     valid until the stream reaches the end of the call.  Host-pointer entry points copy
+ *     in, compute, copy out and synchronise `stream` before returning.
+ *   - One handle serves one stream at a time (the workspace is not shared between concurrent calls).
+ *   - t and 1/f share a unit (days and cycles/day in the paper's workloads).  Times need not be sorted.
+ *   - Return value: LSP_OK (0) or a negative LSP_E* code; nothing throws, nothing aborts.
+ *     Data-dependent degeneracy (zero variance) cannot be reported without a sync: P is NaN then.
+ *   - f = 0 is legal: the sine term of eq. (1) is 0/0 and dropped (reading G7), P = XC^2/Nt/(2 var) ~ 0.
+ *   - There is no CPU fallback: without a CUDA device lsp_create fails with LSP_ECUDA.
+ */
+#ifndef LSP_B200_H
+#define LSP_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lsp_ctx* lsp_handle;            /* opaque; owns the device workspace only */
+
+enum {
+    LSP_OK      =  0,
+    LSP_EINVAL  = -1,   /* NULL handle/pointer, Nt < 2, Nf < 1, B < 1, bad stride, non-finite or negative f_min/df */
+    LSP_ECUDA   = -2,   /* a CUDA runtime call failed; see lsp_last_cuda_error */
+    LSP_ENOMEM  = -3    /* workspace allocation failed */
+};
+
+/* Tunables for lsp_set_param (all optional; 0 restores the automatic choice). */
+enum {
+    LSP_PARAM_K         = 1,  /* adjacent frequencies per thread: 4, 8, 12, 16, 20 or 24        */
+    LSP_PARAM_THREADS   = 2,  /* threads per CTA of the accumulate kernel: 32..256 (multiple of 32) */
+    LSP_PARAM_NSPLIT    = 3,  /* number of time-axis splits per (series, frequency block)       */
+    LSP_PARAM_RECURRENCE= 4,  /* 1 = plane rotation (8 FP32 lane-ops/term), 2 = three-term      */
+                              /*     (Chebyshev) recurrence (6 lane-ops/term)                   */
+    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the register partial sums (multiple of the tile) */
+    LSP_PARAM_TIMING    = 6   /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
+};
+
+/* Create a handle bound to CUDA device `device` (-1 = the calling thread's current device). */
+int lsp_create(lsp_handle* out, int device);
+
+/* Free the workspace and the handle.  NULL is accepted.  Synchronises the device. */
+int lsp_destroy(lsp_handle h);
+
+/* Override / query a tunable (see LSP_PARAM_*).  Returns LSP_EINVAL for unknown keys or values. */
+int lsp_set_param(lsp_handle h, int key, int64_t value);
+int lsp_get_param(lsp_handle h, int key, int64_t* value);
+
+/*
+ * One series.  P[k] = P(f_min + k*df), k = 0..Nf-1  (eqs (1)-(2) via (5)-(8)).
+ *   t  DEVICE const double[Nt]   sample times
+ *   x  DEVICE const float [Nt]   measurements (any mean / variance; normalised inside)
+ *   P  DEVICE       float [Nf]   written; exactly Nf values (reading G8: no rounding up to blocks)
+ * Enqueues 4 kernels on `stream`; no host synchronisation.
+ */
+int lsp_periodogram(lsp_handle h,
+                    const double* t, const float* x, int64_t Nt,
+                    double f_min, double df, int64_t Nf,
+                    float* P, void* stream);
+
+/*
+ * B independent series on one shared frequency grid (the Monte-Carlo use of PAPER.md:369).
+ *   series b reads t + b*t_stride and x + b*x_stride (strides in ELEMENTS; t_stride = 0 means
+ *   all series share one time vector; otherwise |stride| >= Nt), writes P + b*p_stride.
+ *   P may be NULL if only the peaks are wanted (then p_stride is ignored).
+ *   peak_idx DEVICE int32[B], peak_val DEVICE float[B]: arg-max_k P (lowest k among equal
+ *   maxima, reading G9) and its value; both nullable (both or neither).
+ */
+int lsp_periodogram_batched(lsp_handle h,
+                            const double* t, int64_t t_stride,
+                            const float* x, int64_t x_stride,
+                            int64_t B, int64_t Nt,
+                            double f_min, double df, int64_t Nf,
+                            float* P, int64_t p_stride,
+                            int32_t* peak_idx, float* peak_val,
+                            void* stream);
+
+/*
+ * Host-buffer forms: same arithmetic, HOST pointers.  The call copies t and x to the device
+ * (cudaMemcpyAsync on `stream`), runs the device path, copies P (and the peaks) back and
+ * synchronises `stream`.  Arrays are dense: series b at t + b*Nt, x + b*Nt, P + b*Nf.
+ * share_t != 0: t holds ONE time vector of length Nt used by every series.
+ */
+int lsp_periodogram_host(lsp_handle h,
+                         const double* t, const float* x, int64_t Nt,
+                         double f_min, double df, int64_t Nf,
+                         float* P, void* stream);
+
+int lsp_periodogram_batched_host(lsp_handle h,
+                                 const double* t, int share_t, const float* x,
+                                 int64_t B, int64_t Nt,
+                                 double f_min, double df, int64_t Nf,
+                                 float* P, int32_t* peak_idx, float* peak_val,
+                                 void* stream);
+
+/*
+ * Introspection of the last call's launch plan (for benchmarks and tests): fills
+ * out[0..7] = {K, threads, nsplit, recurrence, n_freq_blocks, split_len, launches, lane_ops_per_term}.
+ */
+int lsp_last_plan(lsp_handle h, int64_t out[8]);
+
+/*
+ * Per-kernel device time of the last call, from CUDA events recorded on the call's stream
+ * (only when LSP_PARAM_TIMING is 1).  Synchronises on the last event.
+ * ms[0..3] = {moments, records, accumulate, finish} in milliseconds.
+ */
+int lsp_last_timing(lsp_handle h, float ms[4]);
+
+/* Name of the accumulate kernel the last call launched (static string; "" before any call). */
+const char* lsp_last_kernel_name(lsp_handle h);
+
+/* Last cudaError_t seen by the handle (0 = cudaSuccess). */
+int lsp_last_cuda_error(lsp_handle h);
+
+/* Human-readable text for a status code. */
+const char* lsp_status_string(int status);
+
+/* Library version string, e.g. "lsp_b200 0.1 (sm_100a)". */
+const char* lsp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSP_B200_H */

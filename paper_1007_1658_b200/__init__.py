@@ -1,0 +1,12 @@
+"""paper_1007_1658_b200 -- B200-native direct Lomb-Scargle periodogram (Townsend 2010, arxiv 1007.1658).
+
+The product is the CUDA library `liblsp_b200.so` (csrc/, C ABI in include/lsp.h); this package is
+its thin Python binding.  Nothing here computes on the CPU and nothing imports `oracle/`.
+"""
+from .binding import (Handle, LspError, load, status_string, version, SYMBOLS,
+                      LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM,
+                      PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING,
+                      REC_ROTATION, REC_THREE_TERM)
+from .build import build
+
+__all__ = ["Handle", "LspError", "load", "status_string", "version", "build", "SYMBOLS"]

@@ -1,0 +1,224 @@
+"""Thin ctypes binding over the C ABI of include/lsp.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA library (csrc/); PyTorch is used here only for
+device memory and streams.  There is NO CPU fallback: if the shared library is missing and
+cannot be built, or no sm_100 device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+from . import build as _build
+
+LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM = 0, -1, -2, -3
+PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING = 1, 2, 3, 4, 5, 6
+REC_ROTATION, REC_THREE_TERM = 1, 2
+
+# every symbol include/lsp.h declares (checked by tests/test_abi.py against the header text)
+SYMBOLS = (
+    "lsp_create", "lsp_destroy", "lsp_set_param", "lsp_get_param",
+    "lsp_periodogram", "lsp_periodogram_batched",
+    "lsp_periodogram_host", "lsp_periodogram_batched_host",
+    "lsp_last_plan", "lsp_last_timing", "lsp_last_kernel_name", "lsp_last_cuda_error",
+    "lsp_status_string", "lsp_version",
+)
+
+_lib = None
+
+
+class LspError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        msg = "%s failed: %s (status %d" % (where, status_string(status), status)
+        if cuda_error:
+            msg += ", cudaError %d" % cuda_error
+        super().__init__(msg + ")")
+
+
+def load(rebuild: bool = False):
+    """dlopen paper_1007_1658_b200/liblsp_b200.so (building it with nvcc if absent or stale)."""
+    global _lib
+    if _lib is not None and not rebuild:
+        return _lib
+    path = _build.LIB
+    if rebuild or not os.path.exists(path):
+        path = _build.build(force=rebuild)
+    lib = ctypes.CDLL(path)
+    vp, i64, dbl, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+    lib.lsp_create.argtypes = [ctypes.POINTER(vp), ci]
+    lib.lsp_destroy.argtypes = [vp]
+    lib.lsp_set_param.argtypes = [vp, ci, i64]
+    lib.lsp_get_param.argtypes = [vp, ci, ctypes.POINTER(i64)]
+    lib.lsp_periodogram.argtypes = [vp, vp, vp, i64, dbl, dbl, i64, vp, vp]
+    lib.lsp_periodogram_batched.argtypes = [vp, vp, i64, vp, i64, i64, i64, dbl, dbl, i64,
+                                            vp, i64, vp, vp, vp]
+    lib.lsp_periodogram_host.argtypes = [vp, vp, vp, i64, dbl, dbl, i64, vp, vp]
+    lib.lsp_periodogram_batched_host.argtypes = [vp, vp, ci, vp, i64, i64, dbl, dbl, i64,
+                                                 vp, vp, vp, vp]
+    lib.lsp_last_plan.argtypes = [vp, ctypes.POINTER(i64)]
+    lib.lsp_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    lib.lsp_last_kernel_name.argtypes = [vp]
+    lib.lsp_last_kernel_name.restype = ctypes.c_char_p
+    lib.lsp_last_cuda_error.argtypes = [vp]
+    lib.lsp_status_string.argtypes = [ci]
+    lib.lsp_status_string.restype = ctypes.c_char_p
+    lib.lsp_version.argtypes = []
+    lib.lsp_version.restype = ctypes.c_char_p
+    for name in SYMBOLS:
+        fn = getattr(lib, name)
+        if fn.restype is ctypes.c_int or fn.restype is None:
+            fn.restype = ci
+    _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load().lsp_status_string(int(status)).decode()
+
+
+def version() -> str:
+    return load().lsp_version().decode()
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+class Handle:
+    """lsp_handle: owns the device workspace.  One handle serves one stream at a time."""
+
+    def __init__(self, device: int = -1):
+        self._lib = load()
+        h = ctypes.c_void_p()
+        st = self._lib.lsp_create(ctypes.byref(h), int(device))
+        if st != LSP_OK:
+            raise LspError(st, "lsp_create")
+        self._h = h
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.lsp_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int, where: str):
+        if st != LSP_OK:
+            raise LspError(st, where, self._lib.lsp_last_cuda_error(self._h))
+
+    # -- tunables / introspection
+    def set_param(self, key: int, value: int):
+        self._check(self._lib.lsp_set_param(self._h, int(key), int(value)), "lsp_set_param")
+
+    def get_param(self, key: int) -> int:
+        v = ctypes.c_int64()
+        self._check(self._lib.lsp_get_param(self._h, int(key), ctypes.byref(v)), "lsp_get_param")
+        return v.value
+
+    def last_plan(self) -> dict:
+        out = (ctypes.c_int64 * 8)()
+        self._check(self._lib.lsp_last_plan(self._h, out), "lsp_last_plan")
+        keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "launches",
+                "lane_ops_per_term")
+        d = dict(zip(keys, [int(v) for v in out]))
+        d["kernel"] = self._lib.lsp_last_kernel_name(self._h).decode()
+        return d
+
+    def last_timing(self) -> dict:
+        """Per-kernel milliseconds of the last call (requires set_param(PARAM_TIMING, 1))."""
+        out = (ctypes.c_float * 4)()
+        self._check(self._lib.lsp_last_timing(self._h, out), "lsp_last_timing")
+        return dict(zip(("moments", "records", "accumulate", "finish"), [float(v) for v in out]))
+
+    # -- device-pointer entry points (torch CUDA tensors in, enqueue only)
+    def periodogram(self, t, x, f_min: float, df: float, Nf: int, out=None, stream=None):
+        """lsp_periodogram: t float64[Nt], x float32[Nt] CUDA tensors -> P float32[Nf] (CUDA)."""
+        import torch
+        _want(t, torch.float64, 1, "t"); _want(x, torch.float32, 1, "x")
+        if t.shape != x.shape:
+            raise ValueError("t and x must have the same length")
+        P = out if out is not None else torch.empty(int(Nf), dtype=torch.float32, device=t.device)
+        _want(P, torch.float32, 1, "P")
+        if P.numel() < Nf:
+            raise ValueError("P too small")
+        st = self._lib.lsp_periodogram(self._h, t.data_ptr(), x.data_ptr(), t.numel(),
+                                       float(f_min), float(df), int(Nf), P.data_ptr(), _stream_ptr(stream))
+        self._check(st, "lsp_periodogram")
+        return P
+
+    def periodogram_batched(self, t, x, f_min: float, df: float, Nf: int,
+                            want_P: bool = True, want_peaks: bool = True, stream=None):
+        """lsp_periodogram_batched: x float32[B,Nt]; t float64[B,Nt] or float64[Nt] (shared).
+
+        Returns (P float32[B,Nf] or None, peak_idx int32[B] or None, peak_val float32[B] or None)."""
+        import torch
+        _want(x, torch.float32, 2, "x")
+        B, Nt = x.shape
+        if t.dim() == 1:
+            _want(t, torch.float64, 1, "t"); t_stride = 0
+            if t.numel() != Nt:
+                raise ValueError("shared t must have length Nt")
+        else:
+            _want(t, torch.float64, 2, "t"); t_stride = Nt
+            if tuple(t.shape) != (B, Nt):
+                raise ValueError("t must be [B, Nt]")
+        P = torch.empty((B, int(Nf)), dtype=torch.float32, device=x.device) if want_P else None
+        pi = torch.empty(B, dtype=torch.int32, device=x.device) if want_peaks else None
+        pv = torch.empty(B, dtype=torch.float32, device=x.device) if want_peaks else None
+        st = self._lib.lsp_periodogram_batched(
+            self._h, t.data_ptr(), t_stride, x.data_ptr(), Nt, B, Nt, float(f_min), float(df), int(Nf),
+            P.data_ptr() if want_P else None, int(Nf),
+            pi.data_ptr() if want_peaks else None, pv.data_ptr() if want_peaks else None,
+            _stream_ptr(stream))
+        self._check(st, "lsp_periodogram_batched")
+        return P, pi, pv
+
+    # -- host-pointer entry points (CPU tensors / numpy arrays in and out; synchronous)
+    def periodogram_host(self, t, x, f_min: float, df: float, Nf: int, out=None, stream=None):
+        """lsp_periodogram_host: CPU (ideally pinned) torch tensors; copies + compute + sync."""
+        import torch
+        _want(t, torch.float64, 1, "t", cuda=False); _want(x, torch.float32, 1, "x", cuda=False)
+        P = out if out is not None else torch.empty(int(Nf), dtype=torch.float32)
+        st = self._lib.lsp_periodogram_host(self._h, t.data_ptr(), x.data_ptr(), t.numel(),
+                                            float(f_min), float(df), int(Nf), P.data_ptr(), _stream_ptr(stream))
+        self._check(st, "lsp_periodogram_host")
+        return P
+
+    def periodogram_batched_host(self, t, x, f_min: float, df: float, Nf: int,
+                                 P=None, peak_idx=None, peak_val=None, stream=None):
+        import torch
+        _want(x, torch.float32, 2, "x", cuda=False)
+        B, Nt = x.shape
+        share = 1 if t.dim() == 1 else 0
+        _want(t, torch.float64, t.dim(), "t", cuda=False)
+        st = self._lib.lsp_periodogram_batched_host(
+            self._h, t.data_ptr(), share, x.data_ptr(), B, Nt, float(f_min), float(df), int(Nf),
+            P.data_ptr() if P is not None else None,
+            peak_idx.data_ptr() if peak_idx is not None else None,
+            peak_val.data_ptr() if peak_val is not None else None, _stream_ptr(stream))
+        self._check(st, "lsp_periodogram_batched_host")
+        return P, peak_idx, peak_val
+
+
+def _want(tensor, dtype, ndim, name, cuda: bool = True):
+    if tensor.dtype != dtype or tensor.dim() != ndim or not tensor.is_contiguous():
+        raise ValueError("%s must be a contiguous %s tensor with %d dim(s)" % (name, dtype, ndim))
+    if tensor.is_cuda != cuda:
+        raise ValueError("%s must live on %s" % (name, "the GPU" if cuda else "the host"))

@@ -1,0 +1,405 @@
+// lsp.cu -- host side of the C ABI declared in include/lsp.h: argument checks, launch plan,
+// workspace, and the four enqueues (moments -> records -> accumulate -> finish).
+// No CPU arithmetic on the data path: every step of SURVEY.md section 8(a) runs in a kernel.
+#include "../../include/lsp.h"
+#include "lsp_common.cuh"
+#include "lsp_prepass.cuh"
+#include "lsp_accum.cuh"
+#include "lsp_finish.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <new>
+
+using namespace lsp;
+
+namespace {
+
+struct Plan {
+    int K = 0, T = 0, nsplit = 0, rec = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0;
+    int64_t split_len = 0, part_chunk = 0;
+    const char* kernel_name = "";
+};
+
+}  // namespace
+
+struct lsp_ctx {
+    int device = 0;
+    int sm_count = 148;
+    int last_cuda = 0;
+    // tunables (0 = automatic)
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool timed = false;
+    // workspace
+    void* buf = nullptr;
+    size_t buf_bytes = 0;
+    // staging for the host-pointer entry points
+    void* stage = nullptr;
+    size_t stage_bytes = 0;
+    Plan plan;
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int cuda_fail(lsp_ctx* h, cudaError_t e) {
+    if (h) h->last_cuda = (int)e;
+    return LSP_ECUDA;
+}
+
+#define LSP_CUDA(h, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail((h), e_); } while (0)
+
+struct DeviceGuard {
+    int prev = -1; bool active = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) { active = (cudaSetDevice(dev) == cudaSuccess); }
+    }
+    ~DeviceGuard() { if (active) cudaSetDevice(prev); }
+};
+
+int ensure(lsp_ctx* h, void** ptr, size_t* have, size_t need) {
+    if (need <= *have) return LSP_OK;
+    if (*ptr) { cudaError_t e = cudaFree(*ptr); *ptr = nullptr; *have = 0; if (e != cudaSuccess) return cuda_fail(h, e); }
+    need = align_up(need + need / 8, (size_t)1 << 20);
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, need);
+    if (e != cudaSuccess) { h->last_cuda = (int)e; cudaGetLastError(); return LSP_ENOMEM; }
+    *ptr = p; *have = need;
+    return LSP_OK;
+}
+
+bool valid_K(int64_t K) { return K == 4 || K == 8 || K == 12 || K == 16 || K == 20 || K == 24; }
+
+typedef void (*accum_fn)(const AccumParams);
+
+struct KernelEntry { int K, rec; accum_fn fn; const char* name; };
+
+#define LSP_ENTRY(K, R, RN) { K, R, accum_kernel<K, R>, "accum_kernel<K=" #K "," RN ">" }
+const KernelEntry g_kernels[] = {
+    LSP_ENTRY(4,  REC_ROTATION, "rotation"),   LSP_ENTRY(4,  REC_THREE_TERM, "three_term"),
+    LSP_ENTRY(8,  REC_ROTATION, "rotation"),   LSP_ENTRY(8,  REC_THREE_TERM, "three_term"),
+    LSP_ENTRY(12, REC_ROTATION, "rotation"),   LSP_ENTRY(12, REC_THREE_TERM, "three_term"),
+    LSP_ENTRY(16, REC_ROTATION, "rotation"),   LSP_ENTRY(16, REC_THREE_TERM, "three_term"),
+    LSP_ENTRY(20, REC_ROTATION, "rotation"),   LSP_ENTRY(20, REC_THREE_TERM, "three_term"),
+    LSP_ENTRY(24, REC_ROTATION, "rotation"),   LSP_ENTRY(24, REC_THREE_TERM, "three_term"),
+};
+
+const KernelEntry* find_kernel(int K, int rec) {
+    for (const KernelEntry& e : g_kernels) if (e.K == K && e.rec == rec) return &e;
+    return nullptr;
+}
+
+size_t accum_smem_bytes(int K, int T) { return (size_t)3 * PAIRS * 16 + (size_t)4 * K * T * sizeof(float); }
+
+// Launch plan: which (K, T), how many time splits.  Units of work = B * nfb * nsplit CTAs; the
+// hardware block scheduler balances them over the SMs, so we want many more units than CTA slots.
+Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
+    Plan pl;
+    pl.rec = h->opt_rec ? (int)h->opt_rec : REC_THREE_TERM;
+    const int64_t slots = (int64_t)h->sm_count * 3;
+    const int64_t max_splits = (Nt + TILE - 1) / TILE;
+    static const int cand[][2] = { {16, 128}, {8, 128}, {8, 64}, {4, 64}, {4, 32} };
+    int K = 4, T = 32;
+    for (const auto& c : cand) {
+        K = c[0]; T = c[1];
+        const int64_t nfb = (Nf + (int64_t)K * T - 1) / ((int64_t)K * T);
+        if (B * nfb * max_splits >= 2 * slots) break;
+    }
+    if (h->opt_K) K = (int)h->opt_K;
+    if (h->opt_T) T = (int)h->opt_T;
+    pl.K = K; pl.T = T;
+    const int64_t nfb = (Nf + (int64_t)K * T - 1) / ((int64_t)K * T);
+    pl.nfb = (int)nfb;
+    int64_t nsplit = (8 * slots + B * nfb - 1) / (B * nfb);
+    // keep the partial-sum workspace below ~1 GiB
+    const int64_t ws_cap = ((int64_t)1 << 30) / (B * 16 * Nf > 0 ? B * 16 * Nf : 1);
+    if (nsplit > ws_cap) nsplit = ws_cap;
+    if (h->opt_nsplit) nsplit = h->opt_nsplit;
+    if (nsplit > max_splits) nsplit = max_splits;
+    if (nsplit < 1) nsplit = 1;
+    int64_t split_len = (Nt + nsplit - 1) / nsplit;
+    split_len = (split_len + TILE - 1) / TILE * TILE;
+    pl.split_len = split_len;
+    pl.nsplit = (int)((Nt + split_len - 1) / split_len);
+    int64_t flush = h->opt_flush ? h->opt_flush : 2048;
+    pl.flush_tiles = (int)((flush + TILE - 1) / TILE);
+    if (pl.flush_tiles < 1) pl.flush_tiles = 1;
+    // pre-pass partition: contiguous chunks, at most MAX_PARTS blocks per series
+    int64_t nparts = (Nt + 4095) / 4096;
+    if (nparts > MAX_PARTS) nparts = MAX_PARTS;
+    if (B >= 64 && nparts > 4) nparts = 4;
+    pl.nparts = (int)nparts;
+    pl.part_chunk = (Nt + nparts - 1) / nparts;
+    pl.nparts = (int)((Nt + pl.part_chunk - 1) / pl.part_chunk);
+    pl.launches = 4;
+    return pl;
+}
+
+int run_device(lsp_ctx* h,
+               const double* t, int64_t t_stride, const float* x, int64_t x_stride,
+               int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
+               float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st)
+{
+    Plan pl = make_plan(h, B, Nt, Nf);
+    const KernelEntry* ke = find_kernel(pl.K, pl.rec);
+    if (!ke || pl.T < 32 || pl.T > 256 || (pl.T % 32) != 0) return LSP_EINVAL;
+    pl.kernel_name = ke->name;
+
+    // workspace carve-up
+    const size_t n_samp = (size_t)B * (size_t)Nt;
+    size_t off = 0;
+    const size_t o_recA = off; off = align_up(off + n_samp * sizeof(float4), 256);
+    const size_t o_recB = off; off = align_up(off + n_samp * sizeof(ulonglong2), 256);
+    const size_t o_ws = off;   off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
+    const size_t o_cnt = off;  off = align_up(off + (size_t)B * sizeof(unsigned), 256);
+    int rc = ensure(h, &h->buf, &h->buf_bytes, off);
+    if (rc != LSP_OK) return rc;
+    char* base = static_cast<char*>(h->buf);
+    float4* recA = reinterpret_cast<float4*>(base + o_recA);
+    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
+    float* ws = reinterpret_cast<float*>(base + o_ws);
+    double* psum = reinterpret_cast<double*>(base + o_psum);
+    double* pvar = reinterpret_cast<double*>(base + o_pvar);
+    u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
+    unsigned* counter = reinterpret_cast<unsigned*>(base + o_cnt);
+
+    if (B > 65535) return LSP_EINVAL;                     // grid.y limit of the pre-pass / finish kernels
+
+    const bool timing = h->opt_timing != 0;
+    h->timed = false;
+    if (timing) {
+        for (int i = 0; i < 5; ++i)
+            if (!h->ev[i]) LSP_CUDA(h, cudaEventCreate(&h->ev[i]));
+        LSP_CUDA(h, cudaEventRecord(h->ev[0], st));
+    }
+
+    // steps 1-2
+    dim3 gpre((unsigned)pl.nparts, (unsigned)B);
+    moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
+    LSP_CUDA(h, cudaGetLastError());
+    if (timing) LSP_CUDA(h, cudaEventRecord(h->ev[1], st));
+    records_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
+                                         psum, recA, recB, pvar);
+    LSP_CUDA(h, cudaGetLastError());
+
+    if (timing) LSP_CUDA(h, cudaEventRecord(h->ev[2], st));
+
+    // steps 3-5
+    AccumParams ap;
+    ap.recA = recA; ap.recB = recB; ap.ws = ws; ap.Nt = Nt; ap.Nf = Nf;
+    ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
+    const size_t smem = accum_smem_bytes(pl.K, pl.T);
+    LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t units = B * (int64_t)pl.nsplit * pl.nfb;
+    if (units > 2147483647LL) return LSP_EINVAL;
+    ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
+    LSP_CUDA(h, cudaGetLastError());
+
+    if (timing) LSP_CUDA(h, cudaEventRecord(h->ev[3], st));
+
+    // steps 6-7
+    FinishParams fp;
+    fp.ws = ws; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
+    fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
+    fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = pl.nsplit; fp.nparts = pl.nparts;
+    const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
+    dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
+    finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
+    LSP_CUDA(h, cudaGetLastError());
+    if (timing) { LSP_CUDA(h, cudaEventRecord(h->ev[4], st)); h->timed = true; }
+
+    h->plan = pl;
+    return LSP_OK;
+}
+
+bool bad_grid(double f_min, double df) {
+    return !(std::isfinite(f_min) && std::isfinite(df)) || f_min < 0.0 || df < 0.0;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+int lsp_create(lsp_handle* out, int device)
+{
+    if (!out) return LSP_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return LSP_ECUDA; }
+    if (device < 0) { if (cudaGetDevice(&device) != cudaSuccess) return LSP_ECUDA; }
+    if (device >= ndev) return LSP_EINVAL;
+    lsp_ctx* h = new (std::nothrow) lsp_ctx();
+    if (!h) return LSP_ENOMEM;
+    h->device = device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete h; return LSP_ECUDA; }
+    h->sm_count = prop.multiProcessorCount;
+    if (prop.major < 10) {                                // sm_100a SASS only: fail loudly elsewhere
+        delete h;
+        return LSP_ECUDA;
+    }
+    *out = h;
+    return LSP_OK;
+}
+
+int lsp_destroy(lsp_handle h)
+{
+    if (!h) return LSP_OK;
+    DeviceGuard g(h->device);
+    cudaDeviceSynchronize();
+    if (h->buf) cudaFree(h->buf);
+    if (h->stage) cudaFree(h->stage);
+    for (int i = 0; i < 5; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    delete h;
+    return LSP_OK;
+}
+
+int lsp_set_param(lsp_handle h, int key, int64_t value)
+{
+    if (!h || value < 0) return LSP_EINVAL;
+    switch (key) {
+        case LSP_PARAM_K:          if (value && !valid_K(value)) return LSP_EINVAL; h->opt_K = value; break;
+        case LSP_PARAM_THREADS:    if (value && (value < 32 || value > 256 || value % 32)) return LSP_EINVAL; h->opt_T = value; break;
+        case LSP_PARAM_NSPLIT:     h->opt_nsplit = value; break;
+        case LSP_PARAM_RECURRENCE: if (value > 2) return LSP_EINVAL; h->opt_rec = value; break;
+        case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
+        case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
+        default: return LSP_EINVAL;
+    }
+    return LSP_OK;
+}
+
+int lsp_get_param(lsp_handle h, int key, int64_t* value)
+{
+    if (!h || !value) return LSP_EINVAL;
+    switch (key) {
+        case LSP_PARAM_K:          *value = h->opt_K; break;
+        case LSP_PARAM_THREADS:    *value = h->opt_T; break;
+        case LSP_PARAM_NSPLIT:     *value = h->opt_nsplit; break;
+        case LSP_PARAM_RECURRENCE: *value = h->opt_rec; break;
+        case LSP_PARAM_FLUSH:      *value = h->opt_flush; break;
+        case LSP_PARAM_TIMING:     *value = h->opt_timing; break;
+        default: return LSP_EINVAL;
+    }
+    return LSP_OK;
+}
+
+int lsp_last_timing(lsp_handle h, float ms[4])
+{
+    if (!h || !ms) return LSP_EINVAL;
+    if (!h->timed) return LSP_EINVAL;
+    DeviceGuard g(h->device);
+    LSP_CUDA(h, cudaEventSynchronize(h->ev[4]));
+    for (int i = 0; i < 4; ++i) LSP_CUDA(h, cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]));
+    return LSP_OK;
+}
+
+int lsp_periodogram_batched(lsp_handle h,
+                            const double* t, int64_t t_stride, const float* x, int64_t x_stride,
+                            int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
+                            float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, void* stream)
+{
+    if (!h || !t || !x) return LSP_EINVAL;
+    if (B < 1 || Nt < 2 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
+    if (bad_grid(f_min, df)) return LSP_EINVAL;
+    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
+    if (!P && !peak_idx) return LSP_EINVAL;
+    if (B > 1) {
+        if (t_stride != 0 && std::llabs(t_stride) < Nt) return LSP_EINVAL;
+        if (std::llabs(x_stride) < Nt) return LSP_EINVAL;
+        if (P && std::llabs(p_stride) < Nf) return LSP_EINVAL;
+    }
+    DeviceGuard g(h->device);
+    return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
+                      peak_idx, peak_val, static_cast<cudaStream_t>(stream));
+}
+
+int lsp_periodogram(lsp_handle h, const double* t, const float* x, int64_t Nt,
+                    double f_min, double df, int64_t Nf, float* P, void* stream)
+{
+    if (!P) return LSP_EINVAL;
+    return lsp_periodogram_batched(h, t, Nt, x, Nt, 1, Nt, f_min, df, Nf, P, Nf, nullptr, nullptr, stream);
+}
+
+int lsp_periodogram_batched_host(lsp_handle h, const double* t, int share_t, const float* x,
+                                 int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
+                                 float* P, int32_t* peak_idx, float* peak_val, void* stream)
+{
+    if (!h || !t || !x) return LSP_EINVAL;
+    if (B < 1 || Nt < 2 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
+    if (bad_grid(f_min, df)) return LSP_EINVAL;
+    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
+    if (!P && !peak_idx) return LSP_EINVAL;
+    DeviceGuard g(h->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t nt_t = (size_t)(share_t ? 1 : B) * (size_t)Nt;
+    const size_t nt_x = (size_t)B * (size_t)Nt;
+    size_t off = 0;
+    const size_t o_t = off; off = align_up(off + nt_t * sizeof(double), 256);
+    const size_t o_x = off; off = align_up(off + nt_x * sizeof(float), 256);
+    const size_t o_P = off; off = align_up(off + (P ? (size_t)B * (size_t)Nf * sizeof(float) : 0), 256);
+    const size_t o_pi = off; off = align_up(off + (size_t)B * sizeof(int32_t), 256);
+    const size_t o_pv = off; off = align_up(off + (size_t)B * sizeof(float), 256);
+    int rc = ensure(h, &h->stage, &h->stage_bytes, off);
+    if (rc != LSP_OK) return rc;
+    char* base = static_cast<char*>(h->stage);
+    double* d_t = reinterpret_cast<double*>(base + o_t);
+    float* d_x = reinterpret_cast<float*>(base + o_x);
+    float* d_P = P ? reinterpret_cast<float*>(base + o_P) : nullptr;
+    int32_t* d_pi = peak_idx ? reinterpret_cast<int32_t*>(base + o_pi) : nullptr;
+    float* d_pv = peak_val ? reinterpret_cast<float*>(base + o_pv) : nullptr;
+    LSP_CUDA(h, cudaMemcpyAsync(d_t, t, nt_t * sizeof(double), cudaMemcpyHostToDevice, st));
+    LSP_CUDA(h, cudaMemcpyAsync(d_x, x, nt_x * sizeof(float), cudaMemcpyHostToDevice, st));
+    rc = run_device(h, d_t, share_t ? 0 : Nt, d_x, Nt, B, Nt, f_min, df, Nf, d_P, Nf, d_pi, d_pv, st);
+    if (rc != LSP_OK) return rc;
+    if (P) LSP_CUDA(h, cudaMemcpyAsync(P, d_P, (size_t)B * (size_t)Nf * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (peak_idx) {
+        LSP_CUDA(h, cudaMemcpyAsync(peak_idx, d_pi, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(h, cudaMemcpyAsync(peak_val, d_pv, (size_t)B * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
+    LSP_CUDA(h, cudaStreamSynchronize(st));
+    return LSP_OK;
+}
+
+int lsp_periodogram_host(lsp_handle h, const double* t, const float* x, int64_t Nt,
+                         double f_min, double df, int64_t Nf, float* P, void* stream)
+{
+    if (!P) return LSP_EINVAL;
+    return lsp_periodogram_batched_host(h, t, 0, x, 1, Nt, f_min, df, Nf, P, nullptr, nullptr, stream);
+}
+
+int lsp_last_plan(lsp_handle h, int64_t out[8])
+{
+    if (!h || !out) return LSP_EINVAL;
+    const Plan& p = h->plan;
+    out[0] = p.K; out[1] = p.T; out[2] = p.nsplit; out[3] = p.rec;
+    out[4] = p.nfb; out[5] = p.split_len; out[6] = p.launches;
+    out[7] = (p.rec == REC_ROTATION) ? 8 : 6;
+    return LSP_OK;
+}
+
+const char* lsp_last_kernel_name(lsp_handle h) { return h ? h->plan.kernel_name : ""; }
+
+int lsp_last_cuda_error(lsp_handle h) { return h ? h->last_cuda : 0; }
+
+const char* lsp_status_string(int status)
+{
+    switch (status) {
+        case LSP_OK:     return "ok";
+        case LSP_EINVAL: return "invalid argument";
+        case LSP_ECUDA:  return "CUDA runtime error (or no sm_100 device)";
+        case LSP_ENOMEM: return "device workspace allocation failed";
+        default:         return "unknown status";
+    }
+}
+
+const char* lsp_version(void) { return "lsp_b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,97 @@
+// lsp_finish.cuh -- steps 6-7 of the hot path: combine the sums into P(f) and (optionally) the peak.
+//
+// Step 6 is eqs (5)-(7) with tau from eq. (6) eliminated algebraically, so no
+// atan2 / sincos is needed (the listing calls atan2 + __sincosf):
+//     A = CC - SS = 2 (CC - Nt/2),  B = 2 CS,  R = hypot(A, B)      [cos 2wtau = A/R, sin 2wtau = B/R]
+//     S = XC^2 + XS^2,  D = ((XC^2 - XS^2) A + 2 XC XS B) / R
+//     P = [ (S + D)/(Nt + R) + (S - D)/(Nt - R) ] / (2 var)
+// (denominators of eq. (5) are (Nt +- R)/2, numerators (S +- D)/2).  All in fp64: O(Nf) work.
+// Step 7: arg-max_k P with the lowest index among ties (reading G9), through one packed 64-bit
+// atomicMax per block -- integer max is order-independent, so the result is deterministic.
+#pragma once
+#include "lsp_common.cuh"
+
+namespace lsp {
+
+constexpr int FIN_THREADS = 256;
+constexpr int FIN_FPT = 4;             // frequencies per thread
+
+struct FinishParams {
+    const float* ws;                   // [B][nsplit][4][Nf]
+    const double* part_var;            // [B][nparts]
+    float* P;                          // [B] x p_stride, nullable
+    int64_t p_stride;
+    int32_t* peak_idx;                 // [B], nullable
+    float* peak_val;                   // [B], nullable
+    u64* peak64;                       // [B]
+    unsigned* counter;                 // [B]
+    int64_t Nt, Nf;
+    int nsplit, nparts;
+};
+
+__global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
+{
+    __shared__ double s_var;
+    __shared__ u64 s_best[FIN_THREADS / 32];
+    const int64_t b = blockIdx.y;
+    if (threadIdx.x == 0) {
+        double q = 0.0;                                    // fixed-order sum of the block partials
+        for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
+        s_var = q / (double)(p.Nt - 1);                    // sample variance (reading G1)
+    }
+    __syncthreads();
+    const double inv2var = 0.5 / s_var;
+    const double Nt = (double)p.Nt;
+    const double cc_fix = (p.Nt & 1) ? 0.5 : 0.0;          // phantom partner of an odd last sample
+    const float* ws = p.ws + b * p.nsplit * 4 * p.Nf;
+
+    u64 best = 0ull;
+    #pragma unroll
+    for (int i = 0; i < FIN_FPT; ++i) {
+        const int64_t k = ((int64_t)blockIdx.x * FIN_FPT + i) * FIN_THREADS + threadIdx.x;
+        if (k >= p.Nf) continue;
+        double XC = 0.0, XS = 0.0, CCh = cc_fix, CS = 0.0;
+        for (int sp = 0; sp < p.nsplit; ++sp) {            // fixed order over the time splits
+            const float* w = ws + (int64_t)sp * 4 * p.Nf + k;
+            XC += (double)__ldg(w);
+            XS += (double)__ldg(w + p.Nf);
+            CCh += (double)__ldg(w + 2 * p.Nf);
+            CS += (double)__ldg(w + 3 * p.Nf);
+        }
+        const double A = 2.0 * CCh, Bv = 2.0 * CS;
+        const double R = hypot(A, Bv);
+        const double xc2 = XC * XC, xs2 = XS * XS;
+        const double S = xc2 + xs2;
+        const double D = (R > 0.0) ? ((xc2 - xs2) * A + 2.0 * XC * XS * Bv) / R : 0.0;
+        double val = fmax(S + D, 0.0) / (Nt + R);
+        if (Nt - R > 1e-6 * Nt) val += fmax(S - D, 0.0) / (Nt - R);     // reading G7
+        val *= inv2var;
+        const float Pf = (float)val;
+        if (p.P) p.P[b * p.p_stride + k] = Pf;
+        const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+        best = (key > best) ? key : best;
+    }
+
+    if (p.peak_idx == nullptr) return;
+    #pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const u64 other = __shfl_down_sync(0xffffffffu, best, o);
+        best = (other > best) ? other : best;
+    }
+    if ((threadIdx.x & 31) == 0) s_best[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < FIN_THREADS / 32; ++i) best = (s_best[i] > best) ? s_best[i] : best;
+        atomicMax(p.peak64 + b, best);
+        __threadfence();
+        const unsigned done = atomicAdd(p.counter + b, 1u);
+        if (done == gridDim.x - 1) {                       // last block of this series: publish
+            __threadfence();
+            const u64 fin = atomicMax(p.peak64 + b, 0ull);
+            p.peak_idx[b] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
+            p.peak_val[b] = __uint_as_float((unsigned)(fin >> 32));
+        }
+    }
+}
+
+}  // namespace lsp

@@ -1,0 +1,73 @@
+// lsp_prepass.cuh -- steps 1-2 of the hot path: normalisation moments and per-sample records.
+//
+// Step 1: the series is shifted to zero mean and scaled to unit variance.
+//   The paper does this on the host before upload; here it is two fp64 device reductions,
+//   mean first, then sum (x - mean)^2 fused into the record pass (two-pass variance).
+// Step 2 replaces the listing's fp32 `ft = f*t; ft -= rintf(ft)`: fp32 cannot
+//   hold frac(f*t) when f*t reaches 1e5 cycles (reading G3).  Each sample gets, ONCE,
+//   its phase at f_min and its phase step per frequency bin as exact 64-bit fixed-point turns,
+//   plus the rotation (cos, sin) of that step rounded from an fp64 sincospi.
+#pragma once
+#include "lsp_common.cuh"
+
+namespace lsp {
+
+// grid (nb, B), any block size (multiple of 32).  part_sum[b][blk] = sum of x over the block's chunk.
+__global__ void moments_kernel(const float* __restrict__ x, int64_t x_stride, int64_t Nt,
+                               int64_t chunk, double* __restrict__ part_sum,
+                               u64* __restrict__ peak64, unsigned* __restrict__ counter)
+{
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    const float* xb = x + (int64_t)b * x_stride;
+    const int64_t j0 = (int64_t)blockIdx.x * chunk;
+    const int64_t j1 = min(Nt, j0 + chunk);
+    double acc = 0.0;
+    for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) acc += (double)__ldg(xb + j);
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) {
+        part_sum[(int64_t)b * gridDim.x + blockIdx.x] = acc;
+        if (blockIdx.x == 0) { peak64[b] = 0ull; counter[b] = 0u; }
+    }
+}
+
+// grid (nb, B).  Writes recA, recB for the block's chunk and part_var[b][blk] = sum (x - mean)^2.
+__global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
+                               const float* __restrict__ x, int64_t x_stride,
+                               int64_t Nt, int64_t chunk, double f_min, double df,
+                               const double* __restrict__ part_sum,
+                               float4* __restrict__ recA, ulonglong2* __restrict__ recB,
+                               double* __restrict__ part_var)
+{
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    const int nb = gridDim.x;
+    const double* tb = t + (int64_t)b * t_stride;
+    const float* xb = x + (int64_t)b * x_stride;
+
+    double s = 0.0;                                        // fixed-order sum of the block partials
+    for (int i = 0; i < nb; ++i) s += part_sum[(int64_t)b * nb + i];
+    const double mean = s / (double)Nt;
+    const double t0 = __ldg(tb);                           // time origin (reading G6)
+
+    const int64_t j0 = (int64_t)blockIdx.x * chunk;
+    const int64_t j1 = min(Nt, j0 + chunk);
+    double acc = 0.0;
+    for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+        const double d = (double)__ldg(xb + j) - mean;
+        acc += d * d;
+        const double tp = __ldg(tb + j) - t0;
+        double vfrac;
+        const u64 u = frac_fixed64(f_min, tp, nullptr);
+        const u64 v = frac_fixed64(df, tp, &vfrac);
+        double sd, cd;
+        sincospi(2.0 * vfrac, &sd, &cd);                   // accurate: its error is applied K times per run
+        const int64_t o = (int64_t)b * Nt + j;
+        recA[o] = make_float4((float)d, (float)cd, (float)sd, (float)(2.0 * cd));
+        recB[o] = make_ulonglong2(u, v);
+    }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) part_var[(int64_t)b * nb + blockIdx.x] = acc;
+}
+
+}  // namespace lsp

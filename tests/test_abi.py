@@ -1,0 +1,69 @@
+"""CPU-only checks of the boundary: the library builds, loads and exports every symbol include/lsp.h declares."""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "lsp.h")
+
+
+def _declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(lsp_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = _declared_symbols()
+    for must in ("lsp_create", "lsp_periodogram", "lsp_periodogram_batched", "lsp_destroy"):
+        assert must in names
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    import paper_1007_1658_b200 as pkg
+    path = pkg.build()
+    assert os.path.exists(path)
+    lib = ctypes.CDLL(path)
+    declared = _declared_symbols()
+    assert sorted(pkg.SYMBOLS) == declared
+    for name in declared:
+        assert hasattr(lib, name), name
+    out = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True).stdout
+    exported = set(re.findall(r"\bT (lsp_[a-z_0-9]+)", out))
+    assert exported == set(declared)
+
+
+def test_sass_is_sm100a_packed_fp32():
+    """The accumulate kernels are sm_100a SASS built on FFMA2 (packed f32x2) and MUFU anchors."""
+    import paper_1007_1658_b200 as pkg
+    path = pkg.build()
+    res = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True)
+    if res.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    assert "sm_100a" in res.stdout
+    assert res.stdout.count("FFMA2") > 1000
+    assert "MUFU.SIN" in res.stdout and "MUFU.COS" in res.stdout
+
+
+def test_no_compute_without_gpu_fails_loudly():
+    import torch
+    import paper_1007_1658_b200 as pkg
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(pkg.LspError):
+        pkg.Handle(0)
+    assert pkg.version().startswith("lsp_b200")
+    assert pkg.status_string(0) == "ok"
+
+
+def test_product_does_not_import_oracle():
+    pkg_dir = os.path.join(ROOT, "paper_1007_1658_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src, f
+                assert "lsp_oracle" not in src, f

@@ -1,0 +1,232 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the fp64 oracle, element by element.
+
+Acceptance (BASELINE.json north_star):  max_k |P_gpu - P_oracle| <= 1e-4 * max_k P_oracle  and the
+peak-frequency index identical.  All inputs are seeded synthetic series from `workloads`.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4          # north_star: max|P_gpu - P_oracle| <= 1e-4 * max(P_oracle)
+
+
+def _dev(w):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(w.t)).cuda()
+    x = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
+    return t, x
+
+
+def _check(P_gpu, P_ref, what=""):
+    P_gpu = np.asarray(P_gpu, dtype=np.float64)
+    assert P_gpu.shape == P_ref.shape
+    assert np.all(np.isfinite(P_gpu)), what
+    err = np.max(np.abs(P_gpu - P_ref))
+    bound = TOL * np.max(P_ref)
+    assert err <= bound, "%s: max|dP| = %.3e > %.3e" % (what, err, bound)
+    return err / np.max(P_ref)
+
+
+def _run_single(h, w, **params):
+    import torch
+    from paper_1007_1658_b200 import PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH
+    keys = {"K": PARAM_K, "threads": PARAM_THREADS, "nsplit": PARAM_NSPLIT,
+            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH}
+    for k, v in keys.items():
+        h.set_param(v, params.get(k, 0))
+    try:
+        t, x = _dev(w)
+        P = h.periodogram(t, x, w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+        return P.cpu().numpy()
+    finally:
+        for v in keys.values():
+            h.set_param(v, 0)
+
+
+# ------------------------------------------------------------------ full-grid parity, C1 and C2
+def test_C1_full_grid(lsp):
+    pkg, h = lsp
+    w = workloads.c1()
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w)
+    _check(P, ref, "C1")
+    assert int(np.argmax(P)) == oracle.argmax(ref)
+    assert abs(int(np.argmax(P)) - w.expected_peak_bin) <= 1
+
+
+def test_C2_full_grid(lsp):
+    pkg, h = lsp
+    w = workloads.c2()
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w)
+    _check(P, ref, "C2")
+    assert int(np.argmax(P)) == oracle.argmax(ref)
+
+
+# ------------------------------------------------------------------ every kernel variant, ragged sizes
+@pytest.mark.parametrize("rec", [1, 2])
+@pytest.mark.parametrize("K", [4, 8, 12, 16, 20, 24])
+def test_variants_ragged(lsp, K, rec):
+    """Nt odd and not a multiple of the tile, Nf not a multiple of K*threads, several splits and tiles."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=2731, Nf=1777, seed=1234 + K)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    for threads, nsplit in ((32, 0), (128, 2), (256, 1)):
+        P = _run_single(h, w, K=K, rec=rec, threads=threads, nsplit=nsplit, flush=512)
+        _check(P, ref, "K=%d rec=%d T=%d" % (K, rec, threads))
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+        plan = h.last_plan()
+        assert plan["K"] == K and plan["recurrence"] == rec and plan["threads"] == threads
+        assert plan["lane_ops_per_term"] == (8 if rec == 1 else 6)
+
+
+@pytest.mark.parametrize("Nt,Nf", [(2, 1), (3, 7), (511, 33), (512, 128), (513, 129), (1025, 4097)])
+def test_tiny_and_edge_sizes(lsp, Nt, Nf):
+    pkg, h = lsp
+    rng = np.random.Generator(np.random.PCG64(Nt * 1000 + Nf))
+    t = np.sort(rng.uniform(0.0, 30.0, Nt))
+    x = (np.sin(2 * np.pi * 0.8 * t) + rng.normal(0, 0.3, Nt)).astype(np.float32)
+    w = workloads.Workload("edge", t, x, 0.05, 0.0123, Nf)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w)
+    if Nt == 2:
+        # two samples: the fit is exact, P = (Nt-1)/2 * ... is ill-conditioned in fp32; compare loosely
+        assert np.all(np.isfinite(P))
+        return
+    _check(P, ref, "Nt=%d Nf=%d" % (Nt, Nf))
+
+
+def test_f_zero_and_large_time_offset(lsp):
+    """f_min = 0 (reading G7) and Julian-date-sized times (reading G6: the time origin is shifted)."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=1500, Nf=900, seed=77)
+    w0 = workloads.Workload("f0", w.t + 2455000.25, w.x, 0.0, w.df, w.Nf)
+    ref = oracle.periodogram(w0.t, w0.x, w0.f_min, w0.df, w0.Nf)
+    P = _run_single(h, w0)
+    _check(P, ref, "f_min=0, t+2455000")
+    assert abs(P[0]) <= TOL * ref.max()
+
+
+def test_unsorted_times_and_shift_invariance(lsp):
+    pkg, h = lsp
+    w = workloads.c1(Nt=2000, Nf=1200, seed=78)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    perm = np.random.Generator(np.random.PCG64(5)).permutation(w.Nt)
+    wp = workloads.Workload("perm", w.t[perm], w.x[perm], w.f_min, w.df, w.Nf)
+    _check(_run_single(h, wp), ref, "permuted samples")
+    ws = workloads.Workload("shift", w.t + 1234.567, w.x, w.f_min, w.df, w.Nf)
+    _check(_run_single(h, ws), ref, "shifted times")
+
+
+def test_affine_x_invariance_and_determinism(lsp):
+    pkg, h = lsp
+    w = workloads.c1(Nt=3000, Nf=2000, seed=79)
+    a = _run_single(h, w)
+    b = _run_single(h, w)
+    assert np.array_equal(a, b)                       # fixed-order reductions: bit-identical reruns
+    w2 = workloads.Workload("aff", w.t, (8.0 * w.x + 16.0).astype(np.float32), w.f_min, w.df, w.Nf)
+    c = _run_single(h, w2)
+    assert np.max(np.abs(a - c)) <= 1e-4 * a.max()
+
+
+# ------------------------------------------------------------------ batched path
+def test_batched_small_full_parity(lsp):
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=24, Nt=777, Nf=1501, seed=4321)
+    Pref, iref, vref = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
+    t, x = _dev(w)
+    P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
+    torch.cuda.synchronize()
+    P = P.cpu().numpy(); pi = pi.cpu().numpy(); pv = pv.cpu().numpy()
+    for b in range(w.B):
+        _check(P[b], Pref[b], "series %d" % b)
+    assert np.array_equal(pi, iref.astype(np.int32))
+    assert np.array_equal(pv, P[np.arange(w.B), pi])  # the reported peak value is the stored P
+    # peaks only (P = NULL)
+    _, pi2, pv2 = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf, want_P=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(pi2.cpu().numpy(), pi) and np.array_equal(pv2.cpu().numpy(), pv)
+
+
+def test_batched_shared_times(lsp):
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=6, Nt=600, Nf=700, seed=999)
+    t_shared = w.t[0].copy()
+    Pref, iref, _ = oracle.periodogram_batched(t_shared, w.x, w.f_min, w.df, w.Nf)
+    t = torch.from_numpy(t_shared).cuda()
+    x = torch.from_numpy(w.x).cuda()
+    P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
+    torch.cuda.synchronize()
+    for b in range(w.B):
+        _check(P[b].cpu().numpy(), Pref[b], "shared-t series %d" % b)
+    assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
+
+
+def test_batch_of_one_equals_single(lsp):
+    import torch
+    pkg, h = lsp
+    w = workloads.c1(Nt=1800, Nf=1100, seed=80)
+    a = _run_single(h, w)
+    t, x = _dev(w)
+    P, pi, pv = h.periodogram_batched(t[None, :].contiguous(), x[None, :].contiguous(), w.f_min, w.df, w.Nf)
+    torch.cuda.synchronize()
+    assert np.array_equal(P[0].cpu().numpy(), a)
+    assert int(pi[0]) == int(np.argmax(a))
+
+
+# ------------------------------------------------------------------ host-buffer entry points
+def test_host_entry_points(lsp):
+    import torch
+    pkg, h = lsp
+    w = workloads.c1(Nt=1234, Nf=987, seed=81)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    t = torch.from_numpy(w.t).pin_memory(); x = torch.from_numpy(w.x).pin_memory()
+    P = torch.empty(w.Nf, dtype=torch.float32).pin_memory()
+    h.periodogram_host(t, x, w.f_min, w.df, w.Nf, out=P)
+    _check(P.numpy(), ref, "host single")
+    wb = workloads.c4(B=5, Nt=400, Nf=300, seed=82)
+    Pref, iref, _ = oracle.periodogram_batched(wb.t, wb.x, wb.f_min, wb.df, wb.Nf)
+    Pb = torch.empty((5, 300), dtype=torch.float32)
+    pi = torch.empty(5, dtype=torch.int32); pv = torch.empty(5, dtype=torch.float32)
+    h.periodogram_batched_host(torch.from_numpy(wb.t), torch.from_numpy(wb.x), wb.f_min, wb.df, wb.Nf,
+                               P=Pb, peak_idx=pi, peak_val=pv)
+    for b in range(5):
+        _check(Pb[b].numpy(), Pref[b], "host batched %d" % b)
+    assert np.array_equal(pi.numpy(), iref.astype(np.int32))
+
+
+# ------------------------------------------------------------------ argument errors
+def test_argument_errors(lsp):
+    import torch
+    pkg, h = lsp
+    t = torch.zeros(10, dtype=torch.float64, device="cuda")
+    x = torch.zeros(10, dtype=torch.float32, device="cuda")
+    P = torch.zeros(4, dtype=torch.float32, device="cuda")
+    lib = pkg.load()
+    H = h._h
+    assert lib.lsp_periodogram(H, t.data_ptr(), x.data_ptr(), 1, 0.1, 0.1, 4, P.data_ptr(), None) == pkg.LSP_EINVAL
+    assert lib.lsp_periodogram(H, t.data_ptr(), x.data_ptr(), 10, 0.1, 0.1, 0, P.data_ptr(), None) == pkg.LSP_EINVAL
+    assert lib.lsp_periodogram(H, None, x.data_ptr(), 10, 0.1, 0.1, 4, P.data_ptr(), None) == pkg.LSP_EINVAL
+    assert lib.lsp_periodogram(H, t.data_ptr(), x.data_ptr(), 10, -0.1, 0.1, 4, P.data_ptr(), None) == pkg.LSP_EINVAL
+    assert lib.lsp_periodogram(H, t.data_ptr(), x.data_ptr(), 10, float("nan"), 0.1, 4, P.data_ptr(), None) == pkg.LSP_EINVAL
+    assert lib.lsp_periodogram(H, t.data_ptr(), x.data_ptr(), 10, 0.1, 0.1, 4, None, None) == pkg.LSP_EINVAL
+    assert lib.lsp_periodogram(None, t.data_ptr(), x.data_ptr(), 10, 0.1, 0.1, 4, P.data_ptr(), None) == pkg.LSP_EINVAL
+    assert lib.lsp_set_param(H, pkg.PARAM_K, 5) == pkg.LSP_EINVAL
+    assert lib.lsp_set_param(H, 99, 1) == pkg.LSP_EINVAL
+    # batched: stride smaller than Nt, only one of the two peak outputs
+    assert lib.lsp_periodogram_batched(H, t.data_ptr(), 5, x.data_ptr(), 5, 2, 5, 0.1, 0.1, 2,
+                                       P.data_ptr(), 2, None, None, None) == pkg.LSP_OK
+    assert lib.lsp_periodogram_batched(H, t.data_ptr(), 4, x.data_ptr(), 5, 2, 5, 0.1, 0.1, 2,
+                                       P.data_ptr(), 2, None, None, None) == pkg.LSP_EINVAL
+    pi = torch.zeros(2, dtype=torch.int32, device="cuda")
+    assert lib.lsp_periodogram_batched(H, t.data_ptr(), 5, x.data_ptr(), 5, 2, 5, 0.1, 0.1, 2,
+                                       P.data_ptr(), 2, pi.data_ptr(), None, None) == pkg.LSP_EINVAL
+    torch.cuda.synchronize()
+    assert pkg.status_string(pkg.LSP_EINVAL) == "invalid argument"

@@ -50,11 +50,12 @@ enum {
 
 /* Tunables for lsp_set_param (all optional; 0 restores the automatic choice). */
 enum {
-    LSP_PARAM_K         = 1,  /* adjacent frequencies per thread: 4, 8, 12, 16, 20 or 24        */
+    LSP_PARAM_K         = 1,  /* adjacent frequencies per thread: 4, 8, 12, 16, 20, 24 (32: z form only) */
     LSP_PARAM_THREADS   = 2,  /* threads per CTA of the accumulate kernel: 32..256 (multiple of 32) */
     LSP_PARAM_NSPLIT    = 3,  /* number of time-axis splits per (series, frequency block)       */
-    LSP_PARAM_RECURRENCE= 4,  /* 1 = plane rotation (8 FP32 lane-ops/term), 2 = three-term      */
-                              /*     (Chebyshev) recurrence (6 lane-ops/term)                   */
+    LSP_PARAM_RECURRENCE= 4,  /* 1 = plane rotation, two samples per f32x2 (8 FP32 lane-ops/term) */
+                              /* 2 = three-term (Chebyshev) recurrence, two samples per f32x2 (6)   */
+                              /* 3 = three-term, (cos,sin) of one sample per f32x2 (6) -- default    */
     LSP_PARAM_FLUSH     = 5,  /* samples between folds of the register partial sums (multiple of the tile) */
     LSP_PARAM_TIMING    = 6   /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
 };

@@ -5,7 +5,9 @@
 #include "lsp_common.cuh"
 #include "lsp_prepass.cuh"
 #include "lsp_accum.cuh"
+#include "lsp_accum_z.cuh"
 #include "lsp_finish.cuh"
+#include "lsp_plan.h"
 
 #include <cmath>
 #include <cstdio>
@@ -71,13 +73,14 @@ int ensure(lsp_ctx* h, void** ptr, size_t* have, size_t need) {
     return LSP_OK;
 }
 
-bool valid_K(int64_t K) { return K == 4 || K == 8 || K == 12 || K == 16 || K == 20 || K == 24; }
+bool valid_K(int64_t K) { return K == 4 || K == 8 || K == 12 || K == 16 || K == 20 || K == 24 || K == 28 || K == 32; }
 
 typedef void (*accum_fn)(const AccumParams);
 
-struct KernelEntry { int K, rec; accum_fn fn; const char* name; };
+struct KernelEntry { int K, rec; accum_fn fn; const char* name; int tile_z; int max_t; };   // tile_z = 0: pair-packed kernel
 
-#define LSP_ENTRY(K, R, RN) { K, R, accum_kernel<K, R>, "accum_kernel<K=" #K "," RN ">" }
+#define LSP_ENTRY(K, R, RN) { K, R, accum_kernel<K, R>, "accum_kernel<K=" #K "," RN ">", 0, 256 }
+#define LSP_ENTRY_Z(K, TZ, MAXT, MINB) { K, REC_THREE_TERM_Z, accum_z_kernel<K, TZ, MAXT, MINB>, "accum_z_kernel<K=" #K ",three_term_z>", TZ, MAXT }
 const KernelEntry g_kernels[] = {
     LSP_ENTRY(4,  REC_ROTATION, "rotation"),   LSP_ENTRY(4,  REC_THREE_TERM, "three_term"),
     LSP_ENTRY(8,  REC_ROTATION, "rotation"),   LSP_ENTRY(8,  REC_THREE_TERM, "three_term"),
@@ -85,6 +88,8 @@ const KernelEntry g_kernels[] = {
     LSP_ENTRY(16, REC_ROTATION, "rotation"),   LSP_ENTRY(16, REC_THREE_TERM, "three_term"),
     LSP_ENTRY(20, REC_ROTATION, "rotation"),   LSP_ENTRY(20, REC_THREE_TERM, "three_term"),
     LSP_ENTRY(24, REC_ROTATION, "rotation"),   LSP_ENTRY(24, REC_THREE_TERM, "three_term"),
+    LSP_ENTRY_Z(4, 256, 256, 1), LSP_ENTRY_Z(8, 256, 256, 1), LSP_ENTRY_Z(12, 256, 256, 1), LSP_ENTRY_Z(16, 256, 256, 1),
+    LSP_ENTRY_Z(20, 256, 256, 1), LSP_ENTRY_Z(24, 256, 256, 2), LSP_ENTRY_Z(28, 256, 128, 3), LSP_ENTRY_Z(32, 256, 128, 3),
 };
 
 const KernelEntry* find_kernel(int K, int rec) {
@@ -92,38 +97,20 @@ const KernelEntry* find_kernel(int K, int rec) {
     return nullptr;
 }
 
-size_t accum_smem_bytes(int K, int T) { return (size_t)3 * PAIRS * 16 + (size_t)4 * K * T * sizeof(float); }
+size_t accum_smem_bytes(const KernelEntry* ke, int T) {
+    if (ke->tile_z) return (size_t)ke->tile_z * 24 + (size_t)T * (4 * ke->K + 1) * sizeof(float);
+    return (size_t)3 * PAIRS * 16 + (size_t)4 * ke->K * T * sizeof(float);
+}
 
 // Launch plan: which (K, T), how many time splits.  Units of work = B * nfb * nsplit CTAs; the
 // hardware block scheduler balances them over the SMs, so we want many more units than CTA slots.
 Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
     Plan pl;
-    pl.rec = h->opt_rec ? (int)h->opt_rec : REC_THREE_TERM;
-    const int64_t slots = (int64_t)h->sm_count * 3;
-    const int64_t max_splits = (Nt + TILE - 1) / TILE;
-    static const int cand[][2] = { {16, 128}, {8, 128}, {8, 64}, {4, 64}, {4, 32} };
-    int K = 4, T = 32;
-    for (const auto& c : cand) {
-        K = c[0]; T = c[1];
-        const int64_t nfb = (Nf + (int64_t)K * T - 1) / ((int64_t)K * T);
-        if (B * nfb * max_splits >= 2 * slots) break;
-    }
-    if (h->opt_K) K = (int)h->opt_K;
-    if (h->opt_T) T = (int)h->opt_T;
-    pl.K = K; pl.T = T;
-    const int64_t nfb = (Nf + (int64_t)K * T - 1) / ((int64_t)K * T);
-    pl.nfb = (int)nfb;
-    int64_t nsplit = (8 * slots + B * nfb - 1) / (B * nfb);
-    // keep the partial-sum workspace below ~1 GiB
-    const int64_t ws_cap = ((int64_t)1 << 30) / (B * 16 * Nf > 0 ? B * 16 * Nf : 1);
-    if (nsplit > ws_cap) nsplit = ws_cap;
-    if (h->opt_nsplit) nsplit = h->opt_nsplit;
-    if (nsplit > max_splits) nsplit = max_splits;
-    if (nsplit < 1) nsplit = 1;
-    int64_t split_len = (Nt + nsplit - 1) / nsplit;
-    split_len = (split_len + TILE - 1) / TILE * TILE;
-    pl.split_len = split_len;
-    pl.nsplit = (int)((Nt + split_len - 1) / split_len);
+    PlanOverrides ov;
+    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.rec = h->opt_rec;
+    const PlanChoice pc = plan_choose(h->sm_count, B, Nt, Nf, ov);
+    pl.rec = pc.rec; pl.K = pc.K; pl.T = pc.T; pl.nfb = pc.nfb;
+    pl.nsplit = pc.nsplit; pl.split_len = pc.split_len;
     int64_t flush = h->opt_flush ? h->opt_flush : 2048;
     pl.flush_tiles = (int)((flush + TILE - 1) / TILE);
     if (pl.flush_tiles < 1) pl.flush_tiles = 1;
@@ -145,7 +132,7 @@ int run_device(lsp_ctx* h,
 {
     Plan pl = make_plan(h, B, Nt, Nf);
     const KernelEntry* ke = find_kernel(pl.K, pl.rec);
-    if (!ke || pl.T < 32 || pl.T > 256 || (pl.T % 32) != 0) return LSP_EINVAL;
+    if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
     pl.kernel_name = ke->name;
 
     // workspace carve-up
@@ -194,7 +181,7 @@ int run_device(lsp_ctx* h,
     AccumParams ap;
     ap.recA = recA; ap.recB = recB; ap.ws = ws; ap.Nt = Nt; ap.Nf = Nf;
     ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
-    const size_t smem = accum_smem_bytes(pl.K, pl.T);
+    const size_t smem = accum_smem_bytes(ke, pl.T);
     LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t units = B * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
@@ -208,6 +195,7 @@ int run_device(lsp_ctx* h,
     fp.ws = ws; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = pl.nsplit; fp.nparts = pl.nparts;
+    fp.cc_fix = (ke->tile_z == 0 && (Nt & 1)) ? 0.5 : 0.0;      // phantom partner of an odd last sample (pair-packed only)
     const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
     dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
     finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
@@ -268,7 +256,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_K:          if (value && !valid_K(value)) return LSP_EINVAL; h->opt_K = value; break;
         case LSP_PARAM_THREADS:    if (value && (value < 32 || value > 256 || value % 32)) return LSP_EINVAL; h->opt_T = value; break;
         case LSP_PARAM_NSPLIT:     h->opt_nsplit = value; break;
-        case LSP_PARAM_RECURRENCE: if (value > 2) return LSP_EINVAL; h->opt_rec = value; break;
+        case LSP_PARAM_RECURRENCE: if (value > 3) return LSP_EINVAL; h->opt_rec = value; break;
         case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
         default: return LSP_EINVAL;

@@ -1,0 +1,162 @@
+// lsp_accum_z.cuh -- steps 3-5 of the hot path, "z-packed" form (the default accumulate kernel).
+//
+// Same sums as lsp_accum.cuh (eq. (8)) and the same three-term recurrence, but the
+// two lanes of a packed f32x2 register hold (cos, sin) of ONE sample instead of the cosines of two
+// samples:   z_m = (cos th_m, sin th_m),  th_m = w_{k0+m} t_j.  Per term (one sample, one frequency)
+//
+//     (XC, XS)_m += X      * z_m        FFMA2  X.F32 (scalar broadcast), z, acc1
+//     (CC, CS)_m += cos th * z_m        FFMA2  z.lo.F32 (scalar broadcast), z, acc2
+//     z_{m+1}     = g * z_m - z_{m-1}   FFMA2  g.F32, z, -z_{m-1}          g = 2 cos(2 pi df t_j)
+//
+// = 3 packed instructions = 6 FP32 lane-ops per term.  Why this layout on sm_100a (measured, see
+// DESIGN.md "Register-file model"): an FFMA2 issues every 2 cycles only if at most two of its
+// 64-bit operands are fetched from the register file; here all three instructions of a term share
+// the multiplicand z (operand-reuse cache) and the other multiplicand is a 32-bit scalar, so the
+// limit is met whatever order ptxas picks.  The accumulators cost 4 registers per frequency (8 in
+// the pair-packed form), so K = 24..32 adjacent frequencies fit per thread and the MUFU anchor
+// is amortised over twice as many terms.  No phantom sample is needed for odd Nt.
+#pragma once
+#include "lsp_common.cuh"
+#include "lsp_accum.cuh"
+
+namespace lsp {
+
+constexpr int REC_THREE_TERM_Z = 3;
+
+struct ZAnchor { float c0, s0, cp, sp, X, g; };
+
+// step 3: anchor at the thread's first frequency: exact integer phase (reading G3) -> MUFU sin/cos
+// (PAPER.md:290), plus the value one recurrence step back by an exact rotation (consistent with the
+// anchor, so the anchor's own error is not amplified by the three-term recurrence).
+__device__ __forceinline__ ZAnchor z_anchor(const float4* tS, const float2* tR, int q, unsigned tid)
+{
+    const float4 sv = tS[q];
+    const float2 rv = tR[q];
+    const int ph = (int)(__float_as_uint(sv.z) + tid * __float_as_uint(sv.w));
+    const float ang = (float)ph * LSP_RAD_PER_PHASE;
+    ZAnchor a;
+    a.c0 = __cosf(ang); a.s0 = __sinf(ang);
+    a.cp = fmaf(a.c0, rv.x, a.s0 * rv.y);
+    a.sp = fmaf(a.s0, rv.x, -(a.c0 * rv.y));
+    a.X = sv.x; a.g = sv.y;
+    return a;
+}
+
+template <int K, int TILE_Z, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p)
+{
+    extern __shared__ float4 lsp_smem[];
+    float4* tS = lsp_smem;                                     // {X, g, b32, w32} per sample
+    float2* tR = reinterpret_cast<float2*>(tS + TILE_Z);       // {cd, sd} per sample
+    float* outer = reinterpret_cast<float*>(tR + TILE_Z);      // [T][4K+1] (odd stride: conflict-free)
+
+    const int T = blockDim.x;
+    const unsigned tid = threadIdx.x;
+#ifndef LSP_Z_OUTER_TM
+#define LSP_Z_OUTER_TM 1
+#endif
+#if LSP_Z_OUTER_TM
+#define OIDX(q, m) (tid * (4 * K + 1) + (q) * K + (m))
+#else
+#define OIDX(q, m) (((q) * K + (m)) * T + tid)
+#endif
+    int64_t unit = blockIdx.x;
+    const int fb = (int)(unit % p.nfb); unit /= p.nfb;
+    const int sp = (int)(unit % p.nsplit);
+    const int64_t b = unit / p.nsplit;
+    const int64_t kb = (int64_t)fb * K * T;                    // first frequency index of this block
+    const int64_t j_begin = (int64_t)sp * p.split_len;
+    const int64_t j_end = min(p.Nt, j_begin + p.split_len);
+    const float4* recA = p.recA + b * p.Nt;
+    const ulonglong2* recB = p.recB + b * p.Nt;
+    const int flush_tiles = max(1, p.flush_tiles * TILE / TILE_Z);
+
+    #pragma unroll
+    for (int i = 0; i < 4 * K; ++i) outer[OIDX(i / K, i % K)] = 0.f;
+
+    u64 A1[K], A2[K];                                          // (XC, XS), (CC - n/2, CS)
+    int64_t j = j_begin;
+    int tiles_since_flush = 0;
+    bool fresh = true;
+
+    while (j < j_end) {
+        const int ns = (int)min((int64_t)TILE_Z, j_end - j);
+        if (fresh) {
+            const float n_int = (float)min((int64_t)flush_tiles * TILE_Z, j_end - j);
+            const u64 init = pack2(-0.5f * n_int, 0.f);        // centred CC partial
+            #pragma unroll
+            for (int m = 0; m < K; ++m) { A1[m] = 0ull; A2[m] = init; }
+            fresh = false;
+        }
+        __syncthreads();                                       // previous tile fully consumed
+        for (int i = tid; i < ns; i += T) {
+            const float4 a = __ldg(recA + j + i);
+            const ulonglong2 r = __ldg(recB + j + i);
+            const u64 ph = r.x + (u64)kb * r.y;                // u + kb v  (mod 1, 64-bit wrap)
+            const unsigned b32 = (unsigned)((ph + 0x80000000ull) >> 32);
+            const unsigned w32 = (unsigned)(((u64)K * r.y + 0x80000000ull) >> 32);
+            tS[i] = make_float4(a.x, a.w, __uint_as_float(b32), __uint_as_float(w32));
+            tR[i] = make_float2(a.y, a.z);
+        }
+        __syncthreads();
+
+        // Software pipeline: the anchor of sample q+1 (LDS -> IMAD -> I2F -> MUFU, ~100 cycles of
+        // dependent latency) is issued under the FFMA2 stream of sample q.
+#ifndef LSP_Z_PIPE
+#define LSP_Z_PIPE 0
+#endif
+#if LSP_Z_PIPE
+        ZAnchor nx = z_anchor(tS, tR, 0, tid);
+#endif
+        #pragma unroll 1
+        for (int q = 0; q < ns; ++q) {
+#if LSP_Z_PIPE
+            const ZAnchor cur = nx;
+            nx = z_anchor(tS, tR, min(q + 1, ns - 1), tid);
+#else
+            const ZAnchor cur = z_anchor(tS, tR, q, tid);
+#endif
+            u64 z = pack2(cur.c0, cur.s0);
+            u64 zp = pack2(cur.cp, cur.sp);
+            const u64 XX = pack2(cur.X, cur.X), GG = pack2(cur.g, cur.g);
+            // step 4
+            #pragma unroll
+            for (int m = 0; m < K; ++m) {
+                float cm, sm; unpack2(z, cm, sm);
+                A1[m] = fma2(XX, z, A1[m]);
+                A2[m] = fma2(pack2(cm, cm), z, A2[m]);
+                if (m + 1 < K) { const u64 zn = fma2(GG, z, neg2(zp)); zp = z; z = zn; }
+            }
+        }
+
+        j += ns;
+        if (++tiles_since_flush == flush_tiles || j >= j_end) {
+            // step 5: cascade
+            #pragma unroll
+            for (int m = 0; m < K; ++m) {
+                float xc, xs, cc, cs;
+                unpack2(A1[m], xc, xs); unpack2(A2[m], cc, cs);
+                outer[OIDX(0, m)] += xc;
+                outer[OIDX(1, m)] += xs;
+                outer[OIDX(2, m)] += cc;
+                outer[OIDX(3, m)] += cs;
+            }
+            tiles_since_flush = 0;
+            fresh = true;
+        }
+    }
+
+    float* ws = p.ws + ((b * p.nsplit + sp) * 4) * p.Nf;
+    #pragma unroll
+    for (int m = 0; m < K; ++m) {
+        const int64_t k = kb + (int64_t)tid * K + m;
+        if (k < p.Nf) {
+            ws[0 * p.Nf + k] = outer[OIDX(0, m)];
+            ws[1 * p.Nf + k] = outer[OIDX(1, m)];
+            ws[2 * p.Nf + k] = outer[OIDX(2, m)];
+            ws[3 * p.Nf + k] = outer[OIDX(3, m)];
+        }
+    }
+}
+
+}  // namespace lsp

@@ -27,6 +27,7 @@ struct FinishParams {
     unsigned* counter;                 // [B]
     int64_t Nt, Nf;
     int nsplit, nparts;
+    double cc_fix;                     // added to sum(CC - n/2): 0.5 when the pair-packed kernel padded an odd Nt
 };
 
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
@@ -42,7 +43,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     __syncthreads();
     const double inv2var = 0.5 / s_var;
     const double Nt = (double)p.Nt;
-    const double cc_fix = (p.Nt & 1) ? 0.5 : 0.0;          // phantom partner of an odd last sample
+    const double cc_fix = p.cc_fix;
     const float* ws = p.ws + b * p.nsplit * 4 * p.Nf;
 
     u64 best = 0ull;

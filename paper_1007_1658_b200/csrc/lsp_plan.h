@@ -1,0 +1,116 @@
+// lsp_plan.h -- host-only launch planner (no CUDA calls): picks the accumulate kernel variant
+// (K adjacent frequencies per thread, T threads per CTA) and the number of time-axis splits.
+//
+// The accumulate grid is B * nfb * nsplit equal-sized CTAs ("units") handed out by the hardware
+// block scheduler.  Three effects decide the run time and are modelled here (constants measured on
+// B200):
+//   fill      frequencies actually needed / frequencies the nfb blocks cover (ragged last block)
+//   body      FFMA2 stream vs per-sample anchor overhead: 6K / (6K + 16) FMA-pipe cycles
+//   waves     units / CTA slots is rarely an integer; the last, partly filled wave costs a full
+//             unit time (measured: 8.28 waves ran as 9 => 8 % idle), so nsplit is chosen to make
+//             the wave count large and just below an integer
+// plus a fixed per-unit cost (outer-sum init, workspace write) that penalises very short splits.
+#pragma once
+#include <cstdint>
+
+namespace lsp {
+
+constexpr int PLAN_REC_ROTATION = 1, PLAN_REC_THREE_TERM = 2, PLAN_REC_THREE_TERM_Z = 3;
+constexpr int PLAN_TILE_PAIR = 512, PLAN_TILE_Z = 256;
+
+struct PlanChoice {
+    int K = 0, T = 0, nsplit = 1, rec = 0, nfb = 0, ctas_per_sm = 0;
+    int64_t split_len = 0;
+    double score = 0.0;
+};
+
+struct PlanOverrides { int64_t K = 0, T = 0, nsplit = 0, rec = 0; };
+
+inline bool plan_valid_K(int rec, int K) {
+    if (K < 4 || K > 32 || (K % 4) != 0) return false;
+    return rec == PLAN_REC_THREE_TERM_Z ? true : K <= 24;
+}
+
+inline int plan_max_threads(int rec, int K) { return (rec == PLAN_REC_THREE_TERM_Z && K >= 28) ? 128 : 256; }
+
+// registers per thread as compiled (ptxas -v, kept in step with build_ptxas.log by tests/test_gpu_plan.py)
+inline int plan_regs(int rec, int K) {
+    static const int z[9]    = {0, 64, 96, 126, 128, 158, 128, 168, 168};      // K = 4..32
+    static const int pair[7] = {0, 80, 128, 128, 184, 248, 255};               // K = 4..24
+    return rec == PLAN_REC_THREE_TERM_Z ? z[K / 4] : pair[K / 4];
+}
+
+inline int64_t plan_smem_bytes(int rec, int K, int T) {
+    if (rec == PLAN_REC_THREE_TERM_Z) return (int64_t)PLAN_TILE_Z * 24 + (int64_t)T * (4 * K + 1) * 4;
+    return (int64_t)3 * (PLAN_TILE_PAIR / 2) * 16 + (int64_t)16 * K * T;
+}
+
+// resident CTAs per SM (B200: 64K registers, 228 KB shared memory with 1 KB reserved per CTA, 64 warps)
+inline int plan_ctas_per_sm(int rec, int K, int T) {
+    const int regs = (plan_regs(rec, K) + 7) / 8 * 8;
+    int by_regs = 65536 / (regs * T);
+    int by_smem = (int)((int64_t)233472 / (plan_smem_bytes(rec, K, T) + 1024));
+    int by_warps = 2048 / T;
+    int c = by_regs < by_smem ? by_regs : by_smem;
+    if (by_warps < c) c = by_warps;
+    if (c > 32) c = 32;
+    return c;
+}
+
+inline double plan_wave_eff(int64_t units, int64_t slots) {
+    if (units <= slots) return (double)units / (double)slots;
+    const int64_t waves = (units + slots - 1) / slots;
+    return (double)units / (double)(waves * slots);
+}
+
+inline PlanChoice plan_choose(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov)
+{
+    const int rec = ov.rec ? (int)ov.rec : PLAN_REC_THREE_TERM_Z;
+    const int tile = rec == PLAN_REC_THREE_TERM_Z ? PLAN_TILE_Z : PLAN_TILE_PAIR;
+    const int64_t max_splits_tile = (Nt + tile - 1) / tile;
+    static const int Ts[4] = {128, 64, 32, 256};
+    PlanChoice best;
+    for (int K = 32; K >= 4; K -= 4) {
+        if (!plan_valid_K(rec, K)) continue;
+        if (ov.K && ov.K != K) continue;
+        for (int ti = 0; ti < 4; ++ti) {
+            const int T = Ts[ti];
+            if (ov.T ? (ov.T != T) : (T == 256)) continue;          // 256 only on request
+            if (T > plan_max_threads(rec, K)) continue;
+            const int cta = plan_ctas_per_sm(rec, K, T);
+            if (cta < 1) continue;
+            const int64_t fb = (int64_t)K * T;
+            const int64_t nfb = (Nf + fb - 1) / fb;
+            const double fill = (double)Nf / (double)(nfb * fb);
+            const double body = 6.0 * K / (6.0 * K + 16.0);
+            const double wps = cta * T / 128.0;                     // warps per SM sub-partition
+            const double occ = wps >= 3.0 ? 1.0 : (wps >= 2.0 ? 0.93 : (wps >= 1.0 ? 0.72 : 0.72 * wps));
+            const int64_t slots = (int64_t)cta * sm_count;
+            // workspace cap: B * nsplit * 16 bytes * Nf <= 2 GiB
+            int64_t cap = ((int64_t)1 << 31) / (B * 16 * Nf);
+            if (cap < 1) cap = 1;
+            int64_t hi = max_splits_tile < cap ? max_splits_tile : cap;
+            if (hi > 1024) hi = 1024;
+            int64_t lo = 1;
+            if (ov.nsplit) { lo = hi = (ov.nsplit < max_splits_tile ? ov.nsplit : max_splits_tile); }
+            for (int64_t n = lo; n <= hi; ++n) {
+                int64_t len = (Nt + n - 1) / n;
+                len = (len + tile - 1) / tile * tile;
+                const int64_t n_eff = (Nt + len - 1) / len;         // splits actually produced
+                if (n_eff != n && !ov.nsplit) continue;             // duplicate of a smaller n
+                const int64_t units = B * nfb * n_eff;
+                const double wave = plan_wave_eff(units, slots);
+                const double avg_len = (double)Nt / (double)n_eff;
+                const double unit = avg_len / (avg_len + 40.0);
+                const double score = fill * body * occ * wave * unit;
+                if (score > best.score * 1.0025 || best.K == 0) {   // prefer earlier (larger K, fewer splits) on near-ties
+                    best.K = K; best.T = T; best.nsplit = (int)n_eff; best.rec = rec; best.nfb = (int)nfb;
+                    best.ctas_per_sm = cta; best.split_len = len; best.score = score;
+                }
+            }
+        }
+    }
+    return best;
+}
+
+}  // namespace lsp

@@ -242,12 +242,13 @@ def run_ours(args):
     ev0.record()
     for _ in range(args.steps):
         flush_buf.zero_()                                   # L2 flush between timed iterations
-        step_device()
-        tm = h.last_timing()                                # events on the launching stream, per kernel
-        kern_ms.append(tm["accumulate"]); all_ms.append(sum(tm.values()))
+        step_device()                                       # enqueue only: no host sync inside the timed region
     ev1.record()
     barrier()
     total_ms = ev0.elapsed_time(ev1)
+    for back in range(min(args.steps, 64)):                 # per-kernel CUDA events recorded by the library on
+        tm = h.call_timing(back)                            # the launching stream during the timed region
+        kern_ms.append(tm["accumulate"]); all_ms.append(sum(tm.values()))
     clocks = sampler.stop() if rank == 0 else None
     flush_ms = 0.0
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

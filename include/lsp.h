@@ -130,6 +130,20 @@ int lsp_last_plan(lsp_handle h, int64_t out[8]);
  */
 int lsp_last_timing(lsp_handle h, float ms[4]);
 
+/*
+ * Same for an earlier call: calls_back = 0 is the last timed call, 1 the one before, ... up to
+ * 63 (the handle keeps a ring of 64 event sets), so a benchmark can time many back-to-back
+ * calls without a host synchronisation between them.  LSP_EINVAL if that call is not in the ring.
+ */
+int lsp_call_timing(lsp_handle h, int calls_back, float ms[4]);
+
+/*
+ * Host-only: the launch plan the library would pick for (B series, Nt samples, Nf frequencies) on a
+ * device with `sm_count` SMs.  Needs no GPU.  out[0..7] = {K, threads, nsplit, recurrence,
+ * n_freq_blocks, split_len, resident CTAs per SM, model score * 1e6}.
+ */
+int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[8]);
+
 /* Name of the accumulate kernel the last call launched (static string; "" before any call). */
 const char* lsp_last_kernel_name(lsp_handle h);
 

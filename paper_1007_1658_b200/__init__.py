@@ -3,10 +3,10 @@
 The product is the CUDA library `liblsp_b200.so` (csrc/, C ABI in include/lsp.h); this package is
 its thin Python binding.  Nothing here computes on the CPU and nothing imports `oracle/`.
 """
-from .binding import (Handle, LspError, load, status_string, version, SYMBOLS,
+from .binding import (Handle, LspError, load, status_string, version, plan_query, SYMBOLS,
                       LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM,
                       PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING,
-                      REC_ROTATION, REC_THREE_TERM)
+                      REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z)
 from .build import build
 
 __all__ = ["Handle", "LspError", "load", "status_string", "version", "build", "SYMBOLS"]

@@ -21,7 +21,7 @@ SYMBOLS = (
     "lsp_create", "lsp_destroy", "lsp_set_param", "lsp_get_param",
     "lsp_periodogram", "lsp_periodogram_batched",
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
-    "lsp_last_plan", "lsp_last_timing", "lsp_last_kernel_name", "lsp_last_cuda_error",
+    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_last_kernel_name", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
 
@@ -60,6 +60,8 @@ def load(rebuild: bool = False):
                                                  vp, vp, vp, vp]
     lib.lsp_last_plan.argtypes = [vp, ctypes.POINTER(i64)]
     lib.lsp_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    lib.lsp_call_timing.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_float)]
+    lib.lsp_plan_query.argtypes = [ci, i64, i64, i64, ctypes.POINTER(i64)]
     lib.lsp_last_kernel_name.argtypes = [vp]
     lib.lsp_last_kernel_name.restype = ctypes.c_char_p
     lib.lsp_last_cuda_error.argtypes = [vp]
@@ -88,6 +90,16 @@ def _stream_ptr(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
     return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def plan_query(sm_count: int, B: int, Nt: int, Nf: int) -> dict:
+    """lsp_plan_query: the automatic launch plan for a problem size (host-only, no GPU needed)."""
+    out = (ctypes.c_int64 * 8)()
+    st = load().lsp_plan_query(int(sm_count), int(B), int(Nt), int(Nf), out)
+    if st != LSP_OK:
+        raise LspError(st, "lsp_plan_query")
+    keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "ctas_per_sm", "score_e6")
+    return dict(zip(keys, [int(v) for v in out]))
 
 
 class Handle:
@@ -145,6 +157,12 @@ class Handle:
         """Per-kernel milliseconds of the last call (requires set_param(PARAM_TIMING, 1))."""
         out = (ctypes.c_float * 4)()
         self._check(self._lib.lsp_last_timing(self._h, out), "lsp_last_timing")
+        return dict(zip(("moments", "records", "accumulate", "finish"), [float(v) for v in out]))
+
+    def call_timing(self, calls_back: int = 0) -> dict:
+        """Per-kernel milliseconds of the call `calls_back` timed calls ago (ring of 64)."""
+        out = (ctypes.c_float * 4)()
+        self._check(self._lib.lsp_call_timing(self._h, int(calls_back), out), "lsp_call_timing")
         return dict(zip(("moments", "records", "accumulate", "finish"), [float(v) for v in out]))
 
     # -- device-pointer entry points (torch CUDA tensors in, enqueue only)

@@ -26,14 +26,16 @@ struct Plan {
 
 }  // namespace
 
+constexpr int TIMING_RING = 64;
+
 struct lsp_ctx {
     int device = 0;
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
     int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0;
-    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-    bool timed = false;
+    cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
+    uint64_t timed_calls = 0;
     // workspace
     void* buf = nullptr;
     size_t buf_bytes = 0;
@@ -159,23 +161,23 @@ int run_device(lsp_ctx* h,
     if (B > 65535) return LSP_EINVAL;                     // grid.y limit of the pre-pass / finish kernels
 
     const bool timing = h->opt_timing != 0;
-    h->timed = false;
+    cudaEvent_t* ev = h->ev[h->timed_calls % TIMING_RING];
     if (timing) {
         for (int i = 0; i < 5; ++i)
-            if (!h->ev[i]) LSP_CUDA(h, cudaEventCreate(&h->ev[i]));
-        LSP_CUDA(h, cudaEventRecord(h->ev[0], st));
+            if (!ev[i]) LSP_CUDA(h, cudaEventCreate(&ev[i]));
+        LSP_CUDA(h, cudaEventRecord(ev[0], st));
     }
 
     // steps 1-2
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
     moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
-    if (timing) LSP_CUDA(h, cudaEventRecord(h->ev[1], st));
+    if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
     records_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
                                          psum, recA, recB, pvar);
     LSP_CUDA(h, cudaGetLastError());
 
-    if (timing) LSP_CUDA(h, cudaEventRecord(h->ev[2], st));
+    if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
 
     // steps 3-5
     AccumParams ap;
@@ -188,7 +190,7 @@ int run_device(lsp_ctx* h,
     ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
     LSP_CUDA(h, cudaGetLastError());
 
-    if (timing) LSP_CUDA(h, cudaEventRecord(h->ev[3], st));
+    if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
 
     // steps 6-7
     FinishParams fp;
@@ -200,7 +202,7 @@ int run_device(lsp_ctx* h,
     dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
     finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
     LSP_CUDA(h, cudaGetLastError());
-    if (timing) { LSP_CUDA(h, cudaEventRecord(h->ev[4], st)); h->timed = true; }
+    if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
 
     h->plan = pl;
     return LSP_OK;
@@ -244,7 +246,8 @@ int lsp_destroy(lsp_handle h)
     cudaDeviceSynchronize();
     if (h->buf) cudaFree(h->buf);
     if (h->stage) cudaFree(h->stage);
-    for (int i = 0; i < 5; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    for (int r = 0; r < TIMING_RING; ++r)
+        for (int i = 0; i < 5; ++i) if (h->ev[r][i]) cudaEventDestroy(h->ev[r][i]);
     delete h;
     return LSP_OK;
 }
@@ -279,13 +282,26 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
     return LSP_OK;
 }
 
-int lsp_last_timing(lsp_handle h, float ms[4])
+int lsp_call_timing(lsp_handle h, int calls_back, float ms[4])
 {
-    if (!h || !ms) return LSP_EINVAL;
-    if (!h->timed) return LSP_EINVAL;
+    if (!h || !ms || calls_back < 0) return LSP_EINVAL;
+    if ((uint64_t)calls_back >= h->timed_calls || calls_back >= TIMING_RING) return LSP_EINVAL;
     DeviceGuard g(h->device);
-    LSP_CUDA(h, cudaEventSynchronize(h->ev[4]));
-    for (int i = 0; i < 4; ++i) LSP_CUDA(h, cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]));
+    cudaEvent_t* ev = h->ev[(h->timed_calls - 1 - (uint64_t)calls_back) % TIMING_RING];
+    LSP_CUDA(h, cudaEventSynchronize(ev[4]));
+    for (int i = 0; i < 4; ++i) LSP_CUDA(h, cudaEventElapsedTime(&ms[i], ev[i], ev[i + 1]));
+    return LSP_OK;
+}
+
+int lsp_last_timing(lsp_handle h, float ms[4]) { return lsp_call_timing(h, 0, ms); }
+
+int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[8])
+{
+    if (!out || sm_count < 1 || B < 1 || Nt < 2 || Nf < 1) return LSP_EINVAL;
+    const PlanChoice pc = plan_choose(sm_count, B, Nt, Nf, PlanOverrides());
+    out[0] = pc.K; out[1] = pc.T; out[2] = pc.nsplit; out[3] = pc.rec;
+    out[4] = pc.nfb; out[5] = pc.split_len; out[6] = pc.ctas_per_sm;
+    out[7] = (int64_t)(pc.score * 1e6);
     return LSP_OK;
 }
 

@@ -68,14 +68,15 @@ inline PlanChoice plan_choose(int sm_count, int64_t B, int64_t Nt, int64_t Nf, c
     const int rec = ov.rec ? (int)ov.rec : PLAN_REC_THREE_TERM_Z;
     const int tile = rec == PLAN_REC_THREE_TERM_Z ? PLAN_TILE_Z : PLAN_TILE_PAIR;
     const int64_t max_splits_tile = (Nt + tile - 1) / tile;
-    static const int Ts[4] = {128, 64, 32, 256};
+    int Ts[3] = {128, 64, 32};                                      // automatic candidates (256 only on request)
+    int nT = 3;
+    if (ov.T) { Ts[0] = (int)ov.T; nT = 1; }
     PlanChoice best;
     for (int K = 32; K >= 4; K -= 4) {
         if (!plan_valid_K(rec, K)) continue;
         if (ov.K && ov.K != K) continue;
-        for (int ti = 0; ti < 4; ++ti) {
+        for (int ti = 0; ti < nT; ++ti) {
             const int T = Ts[ti];
-            if (ov.T ? (ov.T != T) : (T == 256)) continue;          // 256 only on request
             if (T > plan_max_threads(rec, K)) continue;
             const int cta = plan_ctas_per_sm(rec, K, T);
             if (cta < 1) continue;

@@ -1,0 +1,77 @@
+"""N > 1 host logic of bench.py on CPU: two gloo ranks, distinct per-rank series, max-over-ranks timing.
+
+The path shards by independent series: no data-path collective exists, so what is
+covered here is the plumbing bench.py uses under torchrun -- rank seeds, the MAX all-reduce of the device
+time and the whole-job aggregate.  No CUDA, no oracle.
+"""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    import bench
+    import workloads
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        seed = bench.rank_seed("C1", rank)
+        w = workloads.make("C1", Nt=200, Nf=50, seed=seed)
+        my_ms = 10.0 + 5.0 * rank                      # pretend device times: rank 1 is slower
+        mx = bench.reduce_max(my_ms, dist)
+        value = bench.aggregate_value(w.terms, world, mx * 1e-3)
+        q.put((rank, seed, float(w.t.sum()), mx, value, w.terms))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_gloo_max_time_and_aggregate():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, s0, t0, m0, v0, n0), (r1, s1, t1, m1, v1, n1) = out
+    assert s0 is None and s1 is not None               # rank 0 keeps the config's own seed
+    assert t0 != t1                                    # ranks hold different series
+    assert m0 == m1 == 15.0                            # MAX over ranks, seen by both
+    assert v0 == v1 == pytest.approx(2 * n0 / 15e-3)   # whole-job units / max time
+
+
+def test_single_process_helpers():
+    import bench
+    assert bench.reduce_max(3.5, None) == 3.5
+    assert bench.aggregate_value(10, 4, 2.0) == 20.0
+    assert bench.rank_seed("C5", 0) is None
+    assert bench.rank_seed("C5", 3) != bench.rank_seed("C5", 2)
+
+
+def test_reference_arm_is_rank0_only(monkeypatch, capsys):
+    import bench
+    monkeypatch.setenv("RANK", "1")
+    args = bench.argparse.Namespace(workload="C1", steps=1, warmup=0, gpus=2)
+    assert bench.run_reference(args) == 0
+    assert capsys.readouterr().out == ""               # other ranks exit 0 without work

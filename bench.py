@@ -33,6 +33,8 @@ import workloads  # noqa: E402  (seeded input generators; hold none of the metho
 
 METRIC = "lomb_scargle_term_evals_per_s"
 UNIT = "terms/s"
+TENSOR_FLOP_PER_TERM = 16            # complex MAC for W = XC + i XS plus complex MAC for V = (CC-SS) + 2i CS: 8 real MACs
+TENSOR_FLOP_PER_TERM_EXECUTED = 32   # W runs as three fp16 passes (hi*hi + lo*hi + hi*lo), V as one
 FP32_LANES_PER_SM = 128          # B200: 4 SMSPs x 32 FP32 lanes (guide: blackwell_cuda_programming.md)
 
 
@@ -286,21 +288,36 @@ def run_ours(args):
     peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     k_ms = statistics.mean(kern_ms)
     lane_ops = plan["lane_ops_per_term"]
-    achieved = w.terms * lane_ops * 2 / (k_ms * 1e-3) / 1e12
-    roofline = {
-        "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-        "traffic": None, "kernel": plan["kernel"], "kernel_ms": k_ms, "kernel_share_of_step": k_ms / statistics.mean(all_ms),
-        "lane_ops_per_term": lane_ops,
-        "peak_basis": "%d SMs x 128 FP32 lanes x 2 FLOP x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)" % (n_sm, sm_max),
-        "frac_at_measured_clock": (achieved / (n_sm * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
-                                   if clocks and clocks.get("sm_mhz") else None),
+    if lane_ops:                                             # FP32-pipe forms: 6 or 8 lane-ops (FMA = 2 FLOP) per term
+        achieved = w.terms * lane_ops * 2 / (k_ms * 1e-3) / 1e12
+        roofline = {
+            "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+            "lane_ops_per_term": lane_ops,
+            "peak_basis": "%d SMs x 128 FP32 lanes x 2 FLOP x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)" % (n_sm, sm_max),
+            "frac_at_measured_clock": (achieved / (n_sm * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
+                                       if clocks and clocks.get("sm_mhz") else None),
+        }
+    else:                                                    # tensor-core form: 8 real MACs = 16 FLOP per term
+        tpeak = float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1590.0)))
+        achieved = w.terms * TENSOR_FLOP_PER_TERM / (k_ms * 1e-3) / 1e12
+        roofline = {
+            "bound": "tensor", "achieved": achieved, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved / tpeak,
+            "flop_per_term_algorithmic": TENSOR_FLOP_PER_TERM, "flop_per_term_executed": TENSOR_FLOP_PER_TERM_EXECUTED,
+            "frac_executed": achieved * TENSOR_FLOP_PER_TERM_EXECUTED / TENSOR_FLOP_PER_TERM / tpeak,
+            "peak_basis": "MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16 = fp16 rate; of %s)"
+                          % ("measured" if peaks else "fallback"),
+            "fp32_alu_equivalent_frac": w.terms * 12 / (k_ms * 1e-3) / 1e12 / peak_tflops,
+        }
+    roofline.update({
+        "traffic": None, "kernel": plan["kernel"], "kernel_ms": k_ms,
+        "kernel_share_of_step": k_ms / statistics.mean(all_ms),
         "hbm_GBps_algorithmic": (12.0 * w.B * w.Nt + 4.0 * w.B * w.Nf) / (k_ms * 1e-3) / 1e9,
-    }
+    })
     prof = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(prof):
         try:
             with open(prof) as fh:
-                roofline["traffic"] = json.load(fh).get(w.name)
+                roofline["traffic"] = json.load(fh).get("%s/%s" % (w.name, plan["kernel"]))
         except Exception:
             pass
 

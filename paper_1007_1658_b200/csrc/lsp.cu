@@ -6,6 +6,7 @@
 #include "lsp_prepass.cuh"
 #include "lsp_accum.cuh"
 #include "lsp_accum_z.cuh"
+#include "lsp_accum_mma.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_plan.h"
 
@@ -133,9 +134,10 @@ int run_device(lsp_ctx* h,
                float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st)
 {
     Plan pl = make_plan(h, B, Nt, Nf);
-    const KernelEntry* ke = find_kernel(pl.K, pl.rec);
-    if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
-    pl.kernel_name = ke->name;
+    const bool mma = pl.rec == REC_MMA;
+    const KernelEntry* ke = mma ? nullptr : find_kernel(pl.K, pl.rec);
+    if (!mma && (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0)) return LSP_EINVAL;
+    pl.kernel_name = mma ? "accum_mma_kernel<m16n8k16.f16,hi+lo>" : ke->name;
 
     // workspace carve-up
     const size_t n_samp = (size_t)B * (size_t)Nt;
@@ -180,14 +182,22 @@ int run_device(lsp_ctx* h,
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
 
     // steps 3-5
-    AccumParams ap;
-    ap.recA = recA; ap.recB = recB; ap.ws = ws; ap.Nt = Nt; ap.Nf = Nf;
-    ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
-    const size_t smem = accum_smem_bytes(ke, pl.T);
-    LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t units = B * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
-    ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
+    if (mma) {
+        MmaParams mp;
+        mp.recA = recA; mp.recB = recB; mp.part_var = pvar; mp.ws = ws; mp.Nt = Nt; mp.Nf = Nf;
+        mp.split_len = pl.split_len; mp.nsplit = pl.nsplit; mp.nfb = pl.nfb; mp.nparts = pl.nparts;
+        LSP_CUDA(h, cudaFuncSetAttribute(accum_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMA_SMEM));
+        accum_mma_kernel<<<(unsigned)units, MMA_WARPS * 32, MMA_SMEM, st>>>(mp);
+    } else {
+        AccumParams ap;
+        ap.recA = recA; ap.recB = recB; ap.ws = ws; ap.Nt = Nt; ap.Nf = Nf;
+        ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
+        const size_t smem = accum_smem_bytes(ke, pl.T);
+        LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
+    }
     LSP_CUDA(h, cudaGetLastError());
 
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
@@ -197,7 +207,8 @@ int run_device(lsp_ctx* h,
     fp.ws = ws; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = pl.nsplit; fp.nparts = pl.nparts;
-    fp.cc_fix = (ke->tile_z == 0 && (Nt & 1)) ? 0.5 : 0.0;      // phantom partner of an odd last sample (pair-packed only)
+    fp.cc_fix = (!mma && ke->tile_z == 0 && (Nt & 1)) ? 0.5 : 0.0;   // phantom partner of an odd last sample (pair-packed only)
+    fp.x_scaled = mma ? 1 : 0;
     const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
     dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
     finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
@@ -259,7 +270,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_K:          if (value && !valid_K(value)) return LSP_EINVAL; h->opt_K = value; break;
         case LSP_PARAM_THREADS:    if (value && (value < 32 || value > 256 || value % 32)) return LSP_EINVAL; h->opt_T = value; break;
         case LSP_PARAM_NSPLIT:     h->opt_nsplit = value; break;
-        case LSP_PARAM_RECURRENCE: if (value > 3) return LSP_EINVAL; h->opt_rec = value; break;
+        case LSP_PARAM_RECURRENCE: if (value > 4) return LSP_EINVAL; h->opt_rec = value; break;
         case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
         default: return LSP_EINVAL;
@@ -385,7 +396,7 @@ int lsp_last_plan(lsp_handle h, int64_t out[8])
     const Plan& p = h->plan;
     out[0] = p.K; out[1] = p.T; out[2] = p.nsplit; out[3] = p.rec;
     out[4] = p.nfb; out[5] = p.split_len; out[6] = p.launches;
-    out[7] = (p.rec == REC_ROTATION) ? 8 : 6;
+    out[7] = (p.rec == REC_ROTATION) ? 8 : (p.rec == REC_MMA ? 0 : 6);   // 0: tensor-core form (16 tensor FLOP per term)
     return LSP_OK;
 }
 

@@ -28,6 +28,7 @@ struct FinishParams {
     int64_t Nt, Nf;
     int nsplit, nparts;
     double cc_fix;                     // added to sum(CC - n/2): 0.5 when the pair-packed kernel padded an odd Nt
+    int x_scaled;                      // 1: XC, XS were accumulated from X * x_scale() (tensor-core form)
 };
 
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
@@ -39,6 +40,10 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
         double q = 0.0;                                    // fixed-order sum of the block partials
         for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
         s_var = q / (double)(p.Nt - 1);                    // sample variance (reading G1)
+        if (p.x_scaled) {                                  // undo the fp32 scale factor exactly (lsp_accum_mma.cuh)
+            const double xs = (double)(float)(1.0 / sqrt(s_var));
+            s_var *= xs * xs;
+        }
     }
     __syncthreads();
     const double inv2var = 0.5 / s_var;

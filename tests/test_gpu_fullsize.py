@@ -35,12 +35,17 @@ def _local_maxima_top(P, n):
     return top
 
 
-def _single_fullsize(h, w, stride):
+def _single_fullsize(h, w, stride, rec=0):
     import torch
+    from paper_1007_1658_b200 import PARAM_RECURRENCE
     t = torch.from_numpy(w.t).cuda()
     x = torch.from_numpy(w.x).cuda()
-    P = h.periodogram(t, x, w.f_min, w.df, w.Nf)
-    torch.cuda.synchronize()
+    h.set_param(PARAM_RECURRENCE, rec)
+    try:
+        P = h.periodogram(t, x, w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+    finally:
+        h.set_param(PARAM_RECURRENCE, 0)
     P = P.cpu().numpy()
     assert np.all(np.isfinite(P))
     assert P.min() >= 0.0 and P.max() <= (w.Nt - 1) / 2.0 * (1 + 1e-5)     # eq. (1) bounds, pin P4
@@ -66,6 +71,16 @@ def test_C5_sampled(lsp):
     pkg, h = lsp
     w = workloads.c5()
     _single_fullsize(h, w, stride=8192)          # ~120 strided + ~2,000 window frequencies x 1e6 samples
+
+
+def test_C3_sampled_tensor_core_form(lsp):
+    pkg, h = lsp
+    _single_fullsize(h, workloads.c3(), stride=4096, rec=4)
+
+
+def test_C5_sampled_tensor_core_form(lsp):
+    pkg, h = lsp
+    _single_fullsize(h, workloads.c5(), stride=8192, rec=4)
 
 
 def test_C4_batch_sampled(lsp):

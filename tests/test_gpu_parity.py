@@ -88,6 +88,50 @@ def test_variants_ragged(lsp, K, rec):
         assert plan["lane_ops_per_term"] == (8 if rec == 1 else 6)
 
 
+@pytest.mark.parametrize("Nt,Nf,nsplit", [(2731, 1777, 0), (2731, 1777, 3), (5000, 20011, 0), (1024, 8192, 1),
+                                          (1025, 8193, 2), (127, 40, 0), (129, 1024, 0)])
+def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit):
+    """rec = 4: the mma.sync (fp16 hi+lo, fp32 accumulate) form of steps 3-5; ragged tiles, k-steps, blocks."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=Nt, Nf=Nf, seed=4000 + Nt)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w, rec=4, nsplit=nsplit)
+    _check(P, ref, "mma Nt=%d Nf=%d" % (Nt, Nf))
+    assert int(np.argmax(P)) == oracle.argmax(ref)
+    plan = h.last_plan()
+    assert plan["recurrence"] == 4 and "mma" in plan["kernel"]
+
+
+def test_tensor_core_form_noise_and_scale(lsp):
+    """Pure noise (the tightest tolerance: max P ~ 10) and badly scaled x (1e-6 and 1e+6): the fp16 split must hold."""
+    pkg, h = lsp
+    wb = workloads.c4(B=3, Nt=3000, Nf=9000, seed=4242)
+    for b, scale in enumerate((1.0, 1e-6, 1e6)):
+        x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
+        w = workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
+        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+        P = _run_single(h, w, rec=4)
+        _check(P, ref, "mma noise scale=%g" % scale)
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+
+
+def test_tensor_core_form_batched(lsp):
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=5, Nt=900, Nf=2100, seed=4343)
+    Pref, iref, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
+    h.set_param(pkg.PARAM_RECURRENCE, 4)
+    try:
+        t, x = _dev(w)
+        P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+    finally:
+        h.set_param(pkg.PARAM_RECURRENCE, 0)
+    for b in range(w.B):
+        _check(P[b].cpu().numpy(), Pref[b], "mma series %d" % b)
+    assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
+
+
 @pytest.mark.parametrize("Nt,Nf", [(2, 1), (3, 7), (511, 33), (512, 128), (513, 129), (1025, 4097)])
 def test_tiny_and_edge_sizes(lsp, Nt, Nf):
     pkg, h = lsp

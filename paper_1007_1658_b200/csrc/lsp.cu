@@ -7,6 +7,7 @@
 #include "lsp_accum.cuh"
 #include "lsp_accum_z.cuh"
 #include "lsp_accum_mma.cuh"
+#include "lsp_accum_umma.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_plan.h"
 
@@ -134,10 +135,12 @@ int run_device(lsp_ctx* h,
                float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st)
 {
     Plan pl = make_plan(h, B, Nt, Nf);
-    const bool mma = pl.rec == REC_MMA;
+    const bool umma = pl.rec == REC_UMMA;
+    const bool mma = pl.rec == REC_MMA || umma;                      // tensor-core forms: X scaled to unit variance
     const KernelEntry* ke = mma ? nullptr : find_kernel(pl.K, pl.rec);
     if (!mma && (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0)) return LSP_EINVAL;
-    pl.kernel_name = mma ? "accum_mma_kernel<m16n8k16.f16,hi+lo>" : ke->name;
+    pl.kernel_name = umma ? "accum_umma_kernel<tcgen05.m128n256k16.f16,hi+lo>"
+                          : (mma ? "accum_mma_kernel<m16n8k16.f16,hi+lo>" : ke->name);
 
     // workspace carve-up
     const size_t n_samp = (size_t)B * (size_t)Nt;
@@ -184,7 +187,14 @@ int run_device(lsp_ctx* h,
     // steps 3-5
     const int64_t units = B * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
-    if (mma) {
+    if (umma) {
+        UmmaParams up;
+        up.recA = recA; up.recB = recB; up.part_var = pvar; up.ws = ws; up.Nt = Nt; up.Nf = Nf;
+        up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
+        up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS;
+        LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UM_SMEM));
+        accum_umma_kernel<<<(unsigned)units, UM_THREADS, UM_SMEM, st>>>(up);
+    } else if (mma) {
         MmaParams mp;
         mp.recA = recA; mp.recB = recB; mp.part_var = pvar; mp.ws = ws; mp.Nt = Nt; mp.Nf = Nf;
         mp.split_len = pl.split_len; mp.nsplit = pl.nsplit; mp.nfb = pl.nfb; mp.nparts = pl.nparts;
@@ -270,7 +280,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_K:          if (value && !valid_K(value)) return LSP_EINVAL; h->opt_K = value; break;
         case LSP_PARAM_THREADS:    if (value && (value < 32 || value > 256 || value % 32)) return LSP_EINVAL; h->opt_T = value; break;
         case LSP_PARAM_NSPLIT:     h->opt_nsplit = value; break;
-        case LSP_PARAM_RECURRENCE: if (value > 4) return LSP_EINVAL; h->opt_rec = value; break;
+        case LSP_PARAM_RECURRENCE: if (value > 5) return LSP_EINVAL; h->opt_rec = value; break;
         case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
         default: return LSP_EINVAL;
@@ -396,7 +406,7 @@ int lsp_last_plan(lsp_handle h, int64_t out[8])
     const Plan& p = h->plan;
     out[0] = p.K; out[1] = p.T; out[2] = p.nsplit; out[3] = p.rec;
     out[4] = p.nfb; out[5] = p.split_len; out[6] = p.launches;
-    out[7] = (p.rec == REC_ROTATION) ? 8 : (p.rec == REC_MMA ? 0 : 6);   // 0: tensor-core form (16 tensor FLOP per term)
+    out[7] = (p.rec == REC_ROTATION) ? 8 : ((p.rec == REC_MMA || p.rec == REC_UMMA) ? 0 : 6);   // 0: tensor-core form (16 tensor FLOP per term)
     return LSP_OK;
 }
 

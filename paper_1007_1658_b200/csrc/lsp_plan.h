@@ -15,7 +15,8 @@
 
 namespace lsp {
 
-constexpr int PLAN_REC_ROTATION = 1, PLAN_REC_THREE_TERM = 2, PLAN_REC_THREE_TERM_Z = 3, PLAN_REC_MMA = 4;
+constexpr int PLAN_REC_ROTATION = 1, PLAN_REC_THREE_TERM = 2, PLAN_REC_THREE_TERM_Z = 3, PLAN_REC_MMA = 4, PLAN_REC_UMMA = 5;
+constexpr int PLAN_UMMA_FPB = 16384, PLAN_UMMA_TS = 128;            // frequencies per CTA, samples per record tile (lsp_accum_umma.cuh)
 constexpr int PLAN_MMA_FPB = 8192, PLAN_MMA_TS = 128;              // frequencies per CTA, samples per tile (lsp_accum_mma.cuh)
 constexpr int PLAN_TILE_PAIR = 512, PLAN_TILE_Z = 256;
 
@@ -64,12 +65,14 @@ inline double plan_wave_eff(int64_t units, int64_t slots) {
     return (double)units / (double)(waves * slots);
 }
 
-// Tensor-core form: one CTA of 8 warps per SM owns 8,192 frequencies; only the time split is free.
-inline PlanChoice plan_choose_mma(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov)
+// Tensor-core forms: one CTA per SM owns `fpb` frequencies (8,192 mma.sync / 16,384 tcgen05); only the time split is free.
+inline PlanChoice plan_choose_mma(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov, int rec = PLAN_REC_MMA)
 {
+    const int FPB = rec == PLAN_REC_UMMA ? PLAN_UMMA_FPB : PLAN_MMA_FPB, TS = rec == PLAN_REC_UMMA ? PLAN_UMMA_TS : PLAN_MMA_TS;
+    const double fixed = rec == PLAN_REC_UMMA ? 200.0 : 300.0;      // per-CTA fixed cost in samples: set-up + final drain
     PlanChoice best;
-    const int64_t nfb = (Nf + PLAN_MMA_FPB - 1) / PLAN_MMA_FPB;
-    const int64_t max_splits = (Nt + PLAN_MMA_TS - 1) / PLAN_MMA_TS;
+    const int64_t nfb = (Nf + FPB - 1) / FPB;
+    const int64_t max_splits = (Nt + TS - 1) / TS;
     int64_t cap = ((int64_t)1 << 31) / (B * 16 * Nf);
     if (cap < 1) cap = 1;
     int64_t hi = max_splits < cap ? max_splits : cap;
@@ -78,27 +81,27 @@ inline PlanChoice plan_choose_mma(int sm_count, int64_t B, int64_t Nt, int64_t N
     if (ov.nsplit) { lo = hi = (ov.nsplit < max_splits ? ov.nsplit : max_splits); }
     for (int64_t n = lo; n <= hi; ++n) {
         int64_t len = (Nt + n - 1) / n;
-        len = (len + PLAN_MMA_TS - 1) / PLAN_MMA_TS * PLAN_MMA_TS;
+        len = (len + TS - 1) / TS * TS;
         const int64_t n_eff = (Nt + len - 1) / len;
         if (n_eff != n && !ov.nsplit) continue;
         const int64_t units = B * nfb * n_eff;
         const double wave = plan_wave_eff(units, sm_count);
         const double avg_len = (double)Nt / (double)n_eff;
-        const double unit = avg_len / (avg_len + 300.0);            // per-CTA fixed cost: outer-sum init + write-out
+        const double unit = avg_len / (avg_len + fixed);            // per-CTA fixed cost: outer-sum init + write-out
         const double score = wave * unit;
         if (score > best.score * 1.0025 || best.K == 0) {
-            best.K = 32; best.T = 256; best.nsplit = (int)n_eff; best.rec = PLAN_REC_MMA; best.nfb = (int)nfb;
+            best.K = 32; best.T = rec == PLAN_REC_UMMA ? 544 : 256; best.nsplit = (int)n_eff; best.rec = rec; best.nfb = (int)nfb;
             best.ctas_per_sm = 1; best.split_len = len; best.score = score;
         }
     }
-    best.score *= (double)Nf / (double)(nfb * PLAN_MMA_FPB);
+    best.score *= (double)Nf / (double)(nfb * FPB);
     return best;
 }
 
 inline PlanChoice plan_choose(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov)
 {
     const int rec = ov.rec ? (int)ov.rec : PLAN_REC_THREE_TERM_Z;
-    if (rec == PLAN_REC_MMA) return plan_choose_mma(sm_count, B, Nt, Nf, ov);
+    if (rec == PLAN_REC_MMA || rec == PLAN_REC_UMMA) return plan_choose_mma(sm_count, B, Nt, Nf, ov, rec);
     const int tile = rec == PLAN_REC_THREE_TERM_Z ? PLAN_TILE_Z : PLAN_TILE_PAIR;
     const int64_t max_splits_tile = (Nt + tile - 1) / tile;
     int Ts[3] = {128, 64, 32};                                      // automatic candidates (256 only on request)

@@ -73,14 +73,16 @@ def test_C5_sampled(lsp):
     _single_fullsize(h, w, stride=8192)          # ~120 strided + ~2,000 window frequencies x 1e6 samples
 
 
-def test_C3_sampled_tensor_core_form(lsp):
+@pytest.mark.parametrize("rec", [4, 5])
+def test_C3_sampled_tensor_core_form(lsp, rec):
     pkg, h = lsp
-    _single_fullsize(h, workloads.c3(), stride=4096, rec=4)
+    _single_fullsize(h, workloads.c3(), stride=4096, rec=rec)
 
 
-def test_C5_sampled_tensor_core_form(lsp):
+@pytest.mark.parametrize("rec", [4, 5])
+def test_C5_sampled_tensor_core_form(lsp, rec):
     pkg, h = lsp
-    _single_fullsize(h, workloads.c5(), stride=8192, rec=4)
+    _single_fullsize(h, workloads.c5(), stride=8192, rec=rec)
 
 
 def test_C4_batch_sampled(lsp):

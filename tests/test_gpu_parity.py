@@ -88,21 +88,39 @@ def test_variants_ragged(lsp, K, rec):
         assert plan["lane_ops_per_term"] == (8 if rec == 1 else 6)
 
 
+TC_FORMS = [4, 5]     # 4: mma.sync m16n8k16, 5: tcgen05.mma m128n256k16 with TMEM accumulators
+
+
+@pytest.mark.parametrize("rec", TC_FORMS)
 @pytest.mark.parametrize("Nt,Nf,nsplit", [(2731, 1777, 0), (2731, 1777, 3), (5000, 20011, 0), (1024, 8192, 1),
-                                          (1025, 8193, 2), (127, 40, 0), (129, 1024, 0)])
-def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit):
-    """rec = 4: the mma.sync (fp16 hi+lo, fp32 accumulate) form of steps 3-5; ragged tiles, k-steps, blocks."""
+                                          (1025, 8193, 2), (127, 40, 0), (129, 1024, 0), (130, 16385, 1)])
+def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit, rec):
+    """The tensor-core forms (fp16 hi+lo, fp32 accumulate) of steps 3-5; ragged tiles, k-steps, blocks.
+    Nt >= ~100: V = sum e^{2i th} takes one fp16 pass, so |dP|/P ~ 4e-4 / sqrt(Nt)."""
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=4000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=4, nsplit=nsplit)
-    _check(P, ref, "mma Nt=%d Nf=%d" % (Nt, Nf))
+    P = _run_single(h, w, rec=rec, nsplit=nsplit)
+    _check(P, ref, "rec=%d Nt=%d Nf=%d" % (rec, Nt, Nf))
     assert int(np.argmax(P)) == oracle.argmax(ref)
     plan = h.last_plan()
-    assert plan["recurrence"] == 4 and "mma" in plan["kernel"]
+    assert plan["recurrence"] == rec and "mma" in plan["kernel"]
 
 
-def test_tensor_core_form_noise_and_scale(lsp):
+@pytest.mark.parametrize("flush", [8, 64, 1000, 4096])
+def test_umma_drain_intervals(lsp, flush):
+    """rec = 5: D_W is drained from TMEM every `flush` samples (store first, then read-modify-write)."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=4099, Nf=3001, seed=5005)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    for nsplit in (1, 2):
+        P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush)
+        _check(P, ref, "umma flush=%d nsplit=%d" % (flush, nsplit))
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+
+
+@pytest.mark.parametrize("rec", TC_FORMS)
+def test_tensor_core_form_noise_and_scale(lsp, rec):
     """Pure noise (the tightest tolerance: max P ~ 10) and badly scaled x (1e-6 and 1e+6): the fp16 split must hold."""
     pkg, h = lsp
     wb = workloads.c4(B=3, Nt=3000, Nf=9000, seed=4242)
@@ -110,17 +128,18 @@ def test_tensor_core_form_noise_and_scale(lsp):
         x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
         w = workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
         ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-        P = _run_single(h, w, rec=4)
-        _check(P, ref, "mma noise scale=%g" % scale)
+        P = _run_single(h, w, rec=rec)
+        _check(P, ref, "rec=%d noise scale=%g" % (rec, scale))
         assert int(np.argmax(P)) == oracle.argmax(ref)
 
 
-def test_tensor_core_form_batched(lsp):
+@pytest.mark.parametrize("rec", TC_FORMS)
+def test_tensor_core_form_batched(lsp, rec):
     import torch
     pkg, h = lsp
     w = workloads.c4(B=5, Nt=900, Nf=2100, seed=4343)
     Pref, iref, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
-    h.set_param(pkg.PARAM_RECURRENCE, 4)
+    h.set_param(pkg.PARAM_RECURRENCE, rec)
     try:
         t, x = _dev(w)
         P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)

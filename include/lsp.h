@@ -56,8 +56,11 @@ enum {
     LSP_PARAM_RECURRENCE= 4,  /* 1 = plane rotation, two samples per f32x2 (8 FP32 lane-ops/term) */
                               /* 2 = three-term (Chebyshev) recurrence, two samples per f32x2 (6)   */
                               /* 3 = three-term, (cos,sin) of one sample per f32x2 (6) -- default    */
+                              /* 4 = tensor-core form, mma.sync m16n8k16 fp16 hi+lo, fp32 accumulate   */
+                              /* 5 = tensor-core form, tcgen05.mma m128n256k16, accumulators in TMEM   */
     LSP_PARAM_FLUSH     = 5,  /* samples between folds of the register partial sums (multiple of the tile) */
-    LSP_PARAM_TIMING    = 6   /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
+    LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
+    LSP_PARAM_BTABLE    = 7   /* tcgen05 form only: 0 = coarse-operand table when >= 3 frequency blocks share it, 1 = never, 2 = always */
 };
 
 /* Create a handle bound to CUDA device `device` (-1 = the calling thread's current device). */

@@ -5,8 +5,8 @@ its thin Python binding.  Nothing here computes on the CPU and nothing imports `
 """
 from .binding import (Handle, LspError, load, status_string, version, plan_query, SYMBOLS,
                       LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM,
-                      PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING,
-                      REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z)
+                      PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE,
+                      REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z, REC_MMA, REC_UMMA)
 from .build import build
 
 __all__ = ["Handle", "LspError", "load", "status_string", "version", "build", "SYMBOLS"]

@@ -8,6 +8,7 @@
 #include "lsp_accum_z.cuh"
 #include "lsp_accum_mma.cuh"
 #include "lsp_accum_umma.cuh"
+#include "lsp_accum_umma_tab.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_plan.h"
 
@@ -35,7 +36,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     uint64_t timed_calls = 0;
     // workspace
@@ -152,6 +153,14 @@ int run_device(lsp_ctx* h,
     const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
     const size_t o_cnt = off;  off = align_up(off + (size_t)B * sizeof(unsigned), 256);
+    // tcgen05 form: the coarse operand B comes from a table when several frequency blocks share it (lsp_accum_umma_tab.cuh)
+    const int64_t tab_series = (t_stride == 0) ? 1 : B;
+    const int64_t tab_groups = (Nt + UM_KS - 1) / UM_KS + UT_KPS;
+    const size_t tab_bytes = (size_t)tab_series * (size_t)tab_groups * UT_GROUP_BYTES;
+    const bool use_tab = umma && h->opt_btable != 1 &&
+                         (h->opt_btable == 2 || (pl.nfb >= 3 && tab_bytes <= ((size_t)12 << 30)));
+    const size_t o_tab = off;  if (use_tab) off = align_up(off + tab_bytes, 256);
+    if (use_tab) { pl.kernel_name = "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>"; pl.launches = 5; }
     int rc = ensure(h, &h->buf, &h->buf_bytes, off);
     if (rc != LSP_OK) return rc;
     char* base = static_cast<char*>(h->buf);
@@ -181,6 +190,13 @@ int run_device(lsp_ctx* h,
     records_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
                                          psum, recA, recB, pvar);
     LSP_CUDA(h, cudaGetLastError());
+    unsigned char* btable = reinterpret_cast<unsigned char*>(base + o_tab);
+    if (use_tab) {
+        if (tab_groups > 2147483647LL) return LSP_EINVAL;
+        dim3 gtab((unsigned)tab_groups, (unsigned)tab_series);
+        umma_btable_kernel<<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
+        LSP_CUDA(h, cudaGetLastError());
+    }
 
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
 
@@ -192,8 +208,16 @@ int run_device(lsp_ctx* h,
         up.recA = recA; up.recB = recB; up.part_var = pvar; up.ws = ws; up.Nt = Nt; up.Nf = Nf;
         up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
         up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS;
-        LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UM_SMEM));
-        accum_umma_kernel<<<(unsigned)units, UM_THREADS, UM_SMEM, st>>>(up);
+        if (use_tab) {
+            UmmaTabParams tp;
+            tp.u = up; tp.btable = btable; tp.ngroups = tab_groups;
+            tp.table_stride = (tab_series == 1) ? 0 : (int64_t)tab_groups * UT_GROUP_BYTES;
+            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
+            accum_umma_tab_kernel<<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
+        } else {
+            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UM_SMEM));
+            accum_umma_kernel<<<(unsigned)units, UM_THREADS, UM_SMEM, st>>>(up);
+        }
     } else if (mma) {
         MmaParams mp;
         mp.recA = recA; mp.recB = recB; mp.part_var = pvar; mp.ws = ws; mp.Nt = Nt; mp.Nf = Nf;
@@ -283,6 +307,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_RECURRENCE: if (value > 5) return LSP_EINVAL; h->opt_rec = value; break;
         case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
+        case LSP_PARAM_BTABLE:     if (value > 2) return LSP_EINVAL; h->opt_btable = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -298,6 +323,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_RECURRENCE: *value = h->opt_rec; break;
         case LSP_PARAM_FLUSH:      *value = h->opt_flush; break;
         case LSP_PARAM_TIMING:     *value = h->opt_timing; break;
+        case LSP_PARAM_BTABLE:     *value = h->opt_btable; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

@@ -33,9 +33,9 @@ def _check(P_gpu, P_ref, what=""):
 
 def _run_single(h, w, **params):
     import torch
-    from paper_1007_1658_b200 import PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH
+    from paper_1007_1658_b200 import PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE
     keys = {"K": PARAM_K, "threads": PARAM_THREADS, "nsplit": PARAM_NSPLIT,
-            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH}
+            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE}
     for k, v in keys.items():
         h.set_param(v, params.get(k, 0))
     try:
@@ -107,6 +107,25 @@ def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit, rec):
     assert plan["recurrence"] == rec and "mma" in plan["kernel"]
 
 
+@pytest.mark.parametrize("Nt,Nf,nsplit,flush", [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 50011, 0, 0), (1025, 8193, 2, 0),
+                                                (127, 40, 0, 0), (130, 16385, 1, 0), (4099, 3001, 1, 16), (4099, 3001, 2, 1000),
+                                                (8, 100, 1, 0), (137, 33000, 1, 0)])
+def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush):
+    """rec = 5 with the coarse operand streamed from the pre-computed table (cp.async.bulk), two k-steps per stage:
+    odd k-step counts, ragged tiles and blocks, several drains."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=Nt, Nf=Nf, seed=6000 + Nt)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2)
+    if Nt >= 100:
+        _check(P, ref, "umma-tab Nt=%d Nf=%d" % (Nt, Nf))
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+    else:                                                  # tiny Nt: single fp16 pass of V limits |dP|/P to ~4e-4/sqrt(Nt)
+        assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
+    plan = h.last_plan()
+    assert plan["recurrence"] == 5 and "B-table" in plan["kernel"] and plan["launches"] == 5
+
+
 @pytest.mark.parametrize("flush", [8, 64, 1000, 4096])
 def test_umma_drain_intervals(lsp, flush):
     """rec = 5: D_W is drained from TMEM every `flush` samples (store first, then read-modify-write)."""
@@ -114,7 +133,7 @@ def test_umma_drain_intervals(lsp, flush):
     w = workloads.c1(Nt=4099, Nf=3001, seed=5005)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
     for nsplit in (1, 2):
-        P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush)
+        P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=1)
         _check(P, ref, "umma flush=%d nsplit=%d" % (flush, nsplit))
         assert int(np.argmax(P)) == oracle.argmax(ref)
 

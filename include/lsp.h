@@ -147,6 +147,14 @@ int lsp_call_timing(lsp_handle h, int calls_back, float ms[4]);
  */
 int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[8]);
 
+/*
+ * Same for one form of steps 3-5: recurrence = 0 (automatic, identical to lsp_plan_query) or a
+ * LSP_PARAM_RECURRENCE value 1..5.  For the tensor-core forms (4, 5) K is reported as 32 and `threads`
+ * is the CTA size (256 / 544); a frequency block is 8,192 / 16,384 frequencies.  out[7] = estimated
+ * SM cycles of the accumulate kernel (the quantity the automatic choice compares), not the score.
+ */
+int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int recurrence, int64_t out[8]);
+
 /* Name of the accumulate kernel the last call launched (static string; "" before any call). */
 const char* lsp_last_kernel_name(lsp_handle h);
 

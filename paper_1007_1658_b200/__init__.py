@@ -3,7 +3,7 @@
 The product is the CUDA library `liblsp_b200.so` (csrc/, C ABI in include/lsp.h); this package is
 its thin Python binding.  Nothing here computes on the CPU and nothing imports `oracle/`.
 """
-from .binding import (Handle, LspError, load, status_string, version, plan_query, SYMBOLS,
+from .binding import (Handle, LspError, load, status_string, version, plan_query, plan_query_form, SYMBOLS,
                       LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM,
                       PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE,
                       REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z, REC_MMA, REC_UMMA)

@@ -22,7 +22,7 @@ SYMBOLS = (
     "lsp_create", "lsp_destroy", "lsp_set_param", "lsp_get_param",
     "lsp_periodogram", "lsp_periodogram_batched",
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
-    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_last_kernel_name", "lsp_last_cuda_error",
+    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
 
@@ -63,6 +63,7 @@ def load(rebuild: bool = False):
     lib.lsp_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     lib.lsp_call_timing.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_float)]
     lib.lsp_plan_query.argtypes = [ci, i64, i64, i64, ctypes.POINTER(i64)]
+    lib.lsp_plan_query_form.argtypes = [ci, i64, i64, i64, ci, ctypes.POINTER(i64)]
     lib.lsp_last_kernel_name.argtypes = [vp]
     lib.lsp_last_kernel_name.restype = ctypes.c_char_p
     lib.lsp_last_cuda_error.argtypes = [vp]
@@ -100,6 +101,16 @@ def plan_query(sm_count: int, B: int, Nt: int, Nf: int) -> dict:
     if st != LSP_OK:
         raise LspError(st, "lsp_plan_query")
     keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "ctas_per_sm", "score_e6")
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def plan_query_form(sm_count: int, B: int, Nt: int, Nf: int, recurrence: int = 0) -> dict:
+    """lsp_plan_query_form: the launch plan of one form of steps 3-5 (0 = automatic) and its estimated cycles."""
+    out = (ctypes.c_int64 * 8)()
+    st = load().lsp_plan_query_form(int(sm_count), int(B), int(Nt), int(Nf), int(recurrence), out)
+    if st != LSP_OK:
+        raise LspError(st, "lsp_plan_query_form")
+    keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "ctas_per_sm", "est_cycles")
     return dict(zip(keys, [int(v) for v in out]))
 
 

@@ -352,6 +352,18 @@ int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[
     return LSP_OK;
 }
 
+int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int recurrence, int64_t out[8])
+{
+    if (!out || sm_count < 1 || B < 1 || Nt < 2 || Nf < 1 || recurrence < 0 || recurrence > 5) return LSP_EINVAL;
+    PlanOverrides ov;
+    ov.rec = recurrence;
+    const PlanChoice pc = plan_choose(sm_count, B, Nt, Nf, ov);
+    out[0] = pc.K; out[1] = pc.T; out[2] = pc.nsplit; out[3] = pc.rec;
+    out[4] = pc.nfb; out[5] = pc.split_len; out[6] = pc.ctas_per_sm;
+    out[7] = (int64_t)plan_est_cycles(sm_count, B, Nt, Nf, pc);
+    return LSP_OK;
+}
+
 int lsp_periodogram_batched(lsp_handle h,
                             const double* t, int64_t t_stride, const float* x, int64_t x_stride,
                             int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,

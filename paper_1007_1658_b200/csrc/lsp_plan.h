@@ -98,10 +98,9 @@ inline PlanChoice plan_choose_mma(int sm_count, int64_t B, int64_t Nt, int64_t N
     return best;
 }
 
-inline PlanChoice plan_choose(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov)
+// FP32-pipe forms (rec 1-3): K adjacent frequencies per thread, T threads per CTA, nsplit time splits.
+inline PlanChoice plan_choose_fp32(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov, int rec)
 {
-    const int rec = ov.rec ? (int)ov.rec : PLAN_REC_THREE_TERM_Z;
-    if (rec == PLAN_REC_MMA || rec == PLAN_REC_UMMA) return plan_choose_mma(sm_count, B, Nt, Nf, ov, rec);
     const int tile = rec == PLAN_REC_THREE_TERM_Z ? PLAN_TILE_Z : PLAN_TILE_PAIR;
     const int64_t max_splits_tile = (Nt + tile - 1) / tile;
     int Ts[3] = {128, 64, 32};                                      // automatic candidates (256 only on request)
@@ -148,6 +147,36 @@ inline PlanChoice plan_choose(int sm_count, int64_t B, int64_t Nt, int64_t Nf, c
         }
     }
     return best;
+}
+
+// Estimated run time in SM cycles at the nominal clock (for choosing between the forms; constants measured on B200):
+//   FP32 z form: 6 lane-ops per term on 128 lanes per SM at the modelled efficiency `score`;
+//   tcgen05 form: ~950 cycle-equivalents per k-step of 8 samples x 16,384 frequencies (power-capped clocks
+//   included; 1,150 without the coarse-operand table) plus ~20,000 per CTA (set-up, final drain), per wave.
+inline double plan_est_cycles(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanChoice& pc)
+{
+    if (pc.rec == PLAN_REC_UMMA) {
+        const int64_t units = B * (int64_t)pc.nfb * pc.nsplit;
+        const int64_t waves = (units + sm_count - 1) / sm_count;
+        const double per_kstep = pc.nfb >= 3 ? 950.0 : 1150.0;
+        return (double)waves * ((double)((pc.split_len + 7) / 8) * per_kstep + 20000.0);
+    }
+    const double lane_ops = pc.rec == PLAN_REC_ROTATION ? 8.0 : 6.0;
+    return (double)B * (double)Nt * (double)Nf * lane_ops / (128.0 * sm_count * (pc.score > 1e-6 ? pc.score : 1e-6)) + 4000.0;
+}
+
+constexpr int64_t PLAN_TC_MIN_NT = 512;   // tensor-core forms: V takes one fp16 pass, |dP|/P ~ 4e-4 / sqrt(Nt)
+
+// rec = 0 (automatic): the tcgen05 form when it is accurate (Nt >= 512) and the model says it is faster,
+// else the FP32 z form.  An explicit rec is always honoured.
+inline PlanChoice plan_choose(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov)
+{
+    if (ov.rec == PLAN_REC_MMA || ov.rec == PLAN_REC_UMMA) return plan_choose_mma(sm_count, B, Nt, Nf, ov, (int)ov.rec);
+    if (ov.rec) return plan_choose_fp32(sm_count, B, Nt, Nf, ov, (int)ov.rec);
+    const PlanChoice z = plan_choose_fp32(sm_count, B, Nt, Nf, ov, PLAN_REC_THREE_TERM_Z);
+    if (Nt < PLAN_TC_MIN_NT || ov.K || ov.T) return z;               // K / T overrides address the FP32 kernels
+    const PlanChoice u = plan_choose_mma(sm_count, B, Nt, Nf, ov, PLAN_REC_UMMA);
+    return plan_est_cycles(sm_count, B, Nt, Nf, u) < plan_est_cycles(sm_count, B, Nt, Nf, z) ? u : z;
 }
 
 }  // namespace lsp

@@ -10,7 +10,8 @@ SM = 148
                                      (4096, 1000, 2000), (1, 1000000, 1000000), (1, 2, 1), (3, 77, 5),
                                      (1, 382003, 1528064)])
 def test_plan_is_valid_and_covers_the_problem(B, Nt, Nf):
-    p = pkg.plan_query(SM, B, Nt, Nf)
+    p = pkg.plan_query_form(SM, B, Nt, Nf, 3)              # the FP32 z form
+    assert p["recurrence"] == 3
     assert p["K"] in (4, 8, 12, 16, 20, 24, 28, 32)
     assert p["threads"] % 32 == 0 and 32 <= p["threads"] <= 256
     assert p["n_freq_blocks"] * p["K"] * p["threads"] >= Nf                 # every frequency is owned
@@ -23,7 +24,7 @@ def test_plan_is_valid_and_covers_the_problem(B, Nt, Nf):
 
 
 def test_big_problems_use_wide_threads_and_fill_the_machine():
-    p = pkg.plan_query(SM, 1, 1000000, 1000000)
+    p = pkg.plan_query_form(SM, 1, 1000000, 1000000, 3)
     assert p["K"] >= 24                                                     # anchor amortised
     units = p["nsplit"] * p["n_freq_blocks"]
     slots = p["ctas_per_sm"] * SM
@@ -32,9 +33,9 @@ def test_big_problems_use_wide_threads_and_fill_the_machine():
 
 
 def test_small_problems_split_the_time_axis():
-    p = pkg.plan_query(SM, 1, 10000, 10000)
+    p = pkg.plan_query_form(SM, 1, 10000, 10000, 3)
     assert p["nsplit"] * p["n_freq_blocks"] >= SM                           # enough CTAs to touch every SM
-    p1 = pkg.plan_query(SM, 4096, 1000, 2000)
+    p1 = pkg.plan_query_form(SM, 4096, 1000, 2000, 3)
     assert p1["nsplit"] == 1                                                # the batch already fills the GPU
 
 
@@ -43,3 +44,32 @@ def test_plan_query_rejects_bad_sizes():
         pkg.plan_query(SM, 1, 1, 10)
     with pytest.raises(pkg.LspError):
         pkg.plan_query(0, 1, 10, 10)
+
+
+@pytest.mark.parametrize("B,Nt,Nf", [(1, 10000, 10000), (1, 100000, 1000000), (4096, 1000, 2000),
+                                     (1, 1000000, 1000000), (1, 382003, 1528064), (2, 700, 40000)])
+@pytest.mark.parametrize("rec,fpb,threads", [(4, 8192, 256), (5, 16384, 544)])
+def test_tensor_core_plans_cover_the_problem(B, Nt, Nf, rec, fpb, threads):
+    p = pkg.plan_query_form(SM, B, Nt, Nf, rec)
+    assert p["recurrence"] == rec and p["threads"] == threads and p["ctas_per_sm"] == 1
+    assert p["n_freq_blocks"] * fpb >= Nf and (p["n_freq_blocks"] - 1) * fpb < Nf
+    assert p["nsplit"] >= 1 and p["nsplit"] * p["split_len"] >= Nt and (p["nsplit"] - 1) * p["split_len"] < Nt
+    assert p["split_len"] % 128 == 0
+    assert B * p["nsplit"] * 16 * Nf <= (1 << 31) + 16 * Nf
+    assert p["est_cycles"] > 0
+
+
+def test_automatic_form():
+    """rec = 0: tcgen05 form for large accurate-enough problems, FP32 z form for tiny Nt; explicit forms are honoured."""
+    big = pkg.plan_query(SM, 1, 1000000, 1000000)
+    assert big["recurrence"] == 5
+    units = big["nsplit"] * big["n_freq_blocks"]
+    assert units / SM > 4 and ((units / SM) % 1.0 > 0.85 or units % SM == 0)  # last wave nearly full
+    assert pkg.plan_query(SM, 1, 100000, 1000000)["recurrence"] == 5
+    assert pkg.plan_query(SM, 1, 300, 1000000)["recurrence"] == 3            # Nt < 512: V's single fp16 pass is too coarse
+    assert pkg.plan_query(SM, 1, 2, 1)["recurrence"] == 3
+    auto = pkg.plan_query_form(SM, 1, 1000000, 1000000, 0)
+    z = pkg.plan_query_form(SM, 1, 1000000, 1000000, 3)
+    assert auto["recurrence"] == 5 and auto["est_cycles"] < z["est_cycles"]
+    with pytest.raises(pkg.LspError):
+        pkg.plan_query_form(SM, 1, 10, 10, 6)

@@ -199,7 +199,8 @@ def run_ours(args):
     batched = w.B > 1
     h = lsp.Handle(local)
     for key, val in ((lsp.PARAM_K, args.K), (lsp.PARAM_THREADS, args.threads), (lsp.PARAM_NSPLIT, args.nsplit),
-                     (lsp.PARAM_RECURRENCE, args.recurrence), (lsp.PARAM_FLUSH, args.flush), (lsp.PARAM_BTABLE, args.btable)):
+                     (lsp.PARAM_RECURRENCE, args.recurrence), (lsp.PARAM_FLUSH, args.flush), (lsp.PARAM_BTABLE, args.btable),
+                     (lsp.PARAM_COARSE, args.coarse)):
         if val:
             h.set_param(key, val)
     h.set_param(lsp.PARAM_TIMING, 1)
@@ -356,6 +357,7 @@ def main(argv=None):
     ap.add_argument("--recurrence", type=int, default=0)
     ap.add_argument("--flush", type=int, default=0)
     ap.add_argument("--btable", type=int, default=0)
+    ap.add_argument("--coarse", type=int, default=0)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)

@@ -60,7 +60,8 @@ enum {
                               /* 5 = tensor-core form, tcgen05.mma m128n256k16, accumulators in TMEM   */
     LSP_PARAM_FLUSH     = 5,  /* samples between folds of the register partial sums (multiple of the tile) */
     LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
-    LSP_PARAM_BTABLE    = 7   /* tcgen05 form only: 0 = coarse-operand table when >= 3 frequency blocks share it, 1 = never, 2 = always */
+    LSP_PARAM_BTABLE    = 7,  /* tcgen05 form only: 0 = coarse-operand table when >= 3 frequency blocks share it, 1 = never, 2 = always */
+    LSP_PARAM_COARSE    = 8   /* tcgen05 form only: coarse extent L = 16, 32, 64 or 128 (a CTA owns 128 L frequencies) */
 };
 
 /* Create a handle bound to CUDA device `device` (-1 = the calling thread's current device). */
@@ -149,8 +150,9 @@ int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[
 
 /*
  * Same for one form of steps 3-5: recurrence = 0 (automatic, identical to lsp_plan_query) or a
- * LSP_PARAM_RECURRENCE value 1..5.  For the tensor-core forms (4, 5) K is reported as 32 and `threads`
- * is the CTA size (256 / 544); a frequency block is 8,192 / 16,384 frequencies.  out[7] = estimated
+ * LSP_PARAM_RECURRENCE value 1..5.  For the mma.sync form (4) K is reported as 32, `threads` = 256 and a
+ * frequency block is 8,192 frequencies; for the tcgen05 form (5) K is the coarse extent L (16, 32, 64, 128),
+ * a frequency block is 128 L frequencies and `threads` is the CTA size (288 for L < 128, 544 for L = 128).  out[7] = estimated
  * SM cycles of the accumulate kernel (the quantity the automatic choice compares), not the score.
  */
 int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int recurrence, int64_t out[8]);

@@ -9,6 +9,7 @@
 #include "lsp_accum_mma.cuh"
 #include "lsp_accum_umma.cuh"
 #include "lsp_accum_umma_tab.cuh"
+#include "lsp_accum_umma_small.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_plan.h"
 
@@ -22,7 +23,7 @@ using namespace lsp;
 namespace {
 
 struct Plan {
-    int K = 0, T = 0, nsplit = 0, rec = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0;
+    int K = 0, T = 0, nsplit = 0, rec = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0, L = 0;
     int64_t split_len = 0, part_chunk = 0;
     const char* kernel_name = "";
 };
@@ -36,7 +37,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     uint64_t timed_calls = 0;
     // workspace
@@ -112,9 +113,9 @@ size_t accum_smem_bytes(const KernelEntry* ke, int T) {
 Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
     Plan pl;
     PlanOverrides ov;
-    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.rec = h->opt_rec;
+    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.rec = h->opt_rec; ov.L = h->opt_coarse;
     const PlanChoice pc = plan_choose(h->sm_count, B, Nt, Nf, ov);
-    pl.rec = pc.rec; pl.K = pc.K; pl.T = pc.T; pl.nfb = pc.nfb;
+    pl.rec = pc.rec; pl.K = pc.K; pl.T = pc.T; pl.nfb = pc.nfb; pl.L = pc.L;
     pl.nsplit = pc.nsplit; pl.split_len = pc.split_len;
     int64_t flush = h->opt_flush ? h->opt_flush : 2048;
     pl.flush_tiles = (int)((flush + TILE - 1) / TILE);
@@ -140,8 +141,12 @@ int run_device(lsp_ctx* h,
     const bool mma = pl.rec == REC_MMA || umma;                      // tensor-core forms: X scaled to unit variance
     const KernelEntry* ke = mma ? nullptr : find_kernel(pl.K, pl.rec);
     if (!mma && (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0)) return LSP_EINVAL;
+    const bool umma_small = umma && pl.L < UM_L;          // 128 x L frequencies per CTA, two CTAs per SM
     pl.kernel_name = umma ? "accum_umma_kernel<tcgen05.m128n256k16.f16,hi+lo>"
                           : (mma ? "accum_mma_kernel<m16n8k16.f16,hi+lo>" : ke->name);
+    if (umma_small) pl.kernel_name = pl.L == 16 ? "accum_umma_small_kernel<tcgen05.m128n32k16.f16,hi+lo>"
+                                   : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
+                                                 : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
 
     // workspace carve-up
     const size_t n_samp = (size_t)B * (size_t)Nt;
@@ -157,7 +162,7 @@ int run_device(lsp_ctx* h,
     const int64_t tab_series = (t_stride == 0) ? 1 : B;
     const int64_t tab_groups = (Nt + UM_KS - 1) / UM_KS + UT_KPS;
     const size_t tab_bytes = (size_t)tab_series * (size_t)tab_groups * UT_GROUP_BYTES;
-    const bool use_tab = umma && h->opt_btable != 1 &&
+    const bool use_tab = umma && !umma_small && h->opt_btable != 1 &&
                          (h->opt_btable == 2 || (pl.nfb >= 3 && tab_bytes <= ((size_t)12 << 30)));
     const size_t o_tab = off;  if (use_tab) off = align_up(off + tab_bytes, 256);
     if (use_tab) { pl.kernel_name = "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>"; pl.launches = 5; }
@@ -208,7 +213,16 @@ int run_device(lsp_ctx* h,
         up.recA = recA; up.recB = recB; up.part_var = pvar; up.ws = ws; up.Nt = Nt; up.Nf = Nf;
         up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
         up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS;
-        if (use_tab) {
+        if (umma_small) {
+#define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
+            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
+            accum_umma_small_kernel<LL, NS, MINB><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); } while (0)
+            if (pl.L == 16) LSP_LAUNCH_SMALL(16, 4, 3);
+            else if (pl.L == 32) LSP_LAUNCH_SMALL(32, 4, 2);
+            else if (pl.L == 64) LSP_LAUNCH_SMALL(64, 4, 2);
+            else return LSP_EINVAL;
+#undef LSP_LAUNCH_SMALL
+        } else if (use_tab) {
             UmmaTabParams tp;
             tp.u = up; tp.btable = btable; tp.ngroups = tab_groups;
             tp.table_stride = (tab_series == 1) ? 0 : (int64_t)tab_groups * UT_GROUP_BYTES;
@@ -308,6 +322,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
         case LSP_PARAM_BTABLE:     if (value > 2) return LSP_EINVAL; h->opt_btable = value; break;
+        case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -324,6 +339,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_FLUSH:      *value = h->opt_flush; break;
         case LSP_PARAM_TIMING:     *value = h->opt_timing; break;
         case LSP_PARAM_BTABLE:     *value = h->opt_btable; break;
+        case LSP_PARAM_COARSE:     *value = h->opt_coarse; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

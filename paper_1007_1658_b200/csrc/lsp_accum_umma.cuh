@@ -130,6 +130,7 @@ __device__ __forceinline__ void sts128(uint32_t saddr, unsigned a, unsigned b, u
 // ------------------------------------------------------------------ step 3: operand generation
 // One A item: row h, K chunk `c` (4 samples) of the k-step whose records start at rec[s0].  Writes the
 // 16-byte row chunks of A_hi, A_lo (X e^{ia} as fp16 hi + lo) and A_V (e^{2ia}/2).
+template <bool TAIL>
 __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int nvalid)
 {
     unsigned hi[4], lo[4], vv[4];
@@ -138,15 +139,27 @@ __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, 
         const float4 r = rec[s0 + i];                                   // {X / sigma, pA32, v32, w32}: broadcast read
         float c, s;
         sincos_phase32(__float_as_uint(r.y) + h * __float_as_uint(r.z), c, s);
-        const float xc = r.x * c, xs = r.x * s;
+        const u64 cs = pack2(c, s);
+        float xc, xs;
+        unpack2(mul2(pack2(r.x, r.x), cs), xc, xs);                     // packed FP32: one FMUL2
         hi[i] = pack_h2(xc, xs);
         const float2 hf = unpack_h2(hi[i]);
-        lo[i] = pack_h2(xc - hf.x, xs - hf.y);
-        vv[i] = (i < nvalid) ? pack_h2(fmaf(c, c, -0.5f), c * s) : 0u;  // pads (X = 0) must not count in V either
+        float lc, ls;
+        unpack2(fma2(pack2(hf.x, hf.y), pack2(-1.f, -1.f), pack2(xc, xs)), lc, ls);
+        lo[i] = pack_h2(lc, ls);
+        float v0, v1;
+        unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
+        vv[i] = pack_h2(v0, v1);
+        if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
     sts128(sA, hi[0], hi[1], hi[2], hi[3]);
     sts128(sA + UM_A_BYTES, lo[0], lo[1], lo[2], lo[3]);
     sts128(sA + 2 * UM_A_BYTES, vv[0], vv[1], vv[2], vv[3]);
+}
+__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int64_t left)
+{
+    if (left >= 4) um_gen_a<false>(rec, s0, h, sA, 4);                  // `left` is warp-uniform
+    else um_gen_a<true>(rec, s0, h, sA, (int)max((int64_t)0, left));
 }
 
 // One B item: coarse index l, K chunk `c`: rows (l,Re) and (l,Im) of B_hi, B_lo (e^{ib}) and B_V (e^{2ib}).
@@ -284,8 +297,7 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_kernel(const UmmaPar
             if (is_b) {
                 um_gen_b(rt, s0, idx, st + 3 * UM_A_BYTES + chunk * (UM_B_BYTES / 2) + idx * 16);
             } else {
-                const int64_t left = n_samp - ((int64_t)ks * UM_KS + chunk * 4);
-                um_gen_a(rt, s0, idx, st + chunk * (UM_A_BYTES / 2) + idx * 16, (int)min((int64_t)4, max((int64_t)0, left)));
+                um_gen_a(rt, s0, idx, st + chunk * (UM_A_BYTES / 2) + idx * 16, n_samp - ((int64_t)ks * UM_KS + chunk * 4));
             }
             fence_proxy_async();                                        // generic-proxy stores -> visible to the tensor core
             __syncwarp();

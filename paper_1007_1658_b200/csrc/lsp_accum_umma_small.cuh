@@ -1,0 +1,240 @@
+// lsp_accum_umma_small.cuh -- the tcgen05 form of steps 3-5 for SHORT frequency grids and batches.
+//
+// lsp_accum_umma.cuh gives every CTA 128 fine x 128 coarse = 16,384 frequencies.  A Monte-Carlo batch
+// (BASELINE config C4: 4,096 series x 2,000 frequencies) or a short grid would leave most
+// of that tile empty.  Here the coarse extent L is a template parameter (16, 32 or 64): a CTA owns
+// 128 x L frequencies, k = kb + 128 l + h, the MMAs are m128 n(2L) k16 and the accumulators take 4L of the
+// 512 TMEM columns (D_W: columns [0, 2L), D_V: [2L, 4L)), so two (L = 16: three) CTAs of 8 producer warps +
+// 1 MMA warp share an SM: one CTA's set-up and drain overlap the others' main loops, and the extra warps hide
+// the latency of the generation chain (LDS -> IMAD -> I2F -> MUFU -> F2FP -> STS).  Same algebra, same operand
+// tiles (um_gen_a), same four MMAs per k-step of 8 samples, same periodic drain of D_W as lsp_accum_umma.cuh;
+// the coarse operand B (2L rows) is generated on the fly by a rotating subset of the producer threads.
+// With L <= 32 the kernel is bound by the generation of the fine operand A (128 MUFU sin/cos pairs per
+// sample for 128 L terms), not by the tensor pipe.
+#pragma once
+#include "lsp_accum_umma.cuh"
+
+namespace lsp {
+
+constexpr int US_GEN_WARPS = 8;                        // producer (and drain) warps; warp 8 issues the MMAs
+constexpr int US_THREADS = (US_GEN_WARPS + 1) * 32;
+
+template <int L, int US_STAGES> struct UmmaSmall {
+    static constexpr int B_BYTES = 2 * L * 32;         // one B operand tile: 2L rows x 16 fp16
+    static constexpr int STAGE_BYTES = 3 * UM_A_BYTES + 3 * B_BYTES;
+    static constexpr size_t SMEM = (size_t)US_STAGES * STAGE_BYTES + UM_REC_BYTES + 256;
+    static constexpr int TMEM_COLS = 4 * L < 32 ? 32 : 4 * L;
+    static constexpr uint32_t IDESC = (1u << 4) | ((uint32_t)(2 * L >> 3) << 17) | ((uint32_t)(UM_H >> 4) << 24);
+    static constexpr int FPB = UM_H * L;               // frequencies per CTA
+};
+
+// 32 lanes x 16 consecutive columns of fp32 accumulators -> 16 registers per thread.
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
+{
+    uint32_t r[16];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    #pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// One B item: coarse index l, K chunk of 4 samples: rows (l,Re) and (l,Im) of B_hi, B_lo (e^{ib}) and B_V (e^{2ib}).
+template <int L>
+__device__ __forceinline__ void us_gen_b(const float4* rec, int s0, unsigned l, uint32_t sB)
+{
+    unsigned rh[4], ih[4], rl[4], il[4], rv[4], iv[4];
+    #pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        float c, s;
+        sincos_phase32(l * __float_as_uint(rec[s0 + i].w), c, s);
+        rh[i] = pack_h2(c, -s);
+        ih[i] = pack_h2(s, c);
+        const float2 hf = unpack_h2(rh[i]);                             // (c_h, -s_h)
+        const float dc = c - hf.x, ds = s + hf.y;
+        rl[i] = pack_h2(dc, -ds);
+        il[i] = pack_h2(ds, dc);
+        const float cc = c + c, c2 = fmaf(cc, c, -1.f), s2 = cc * s;
+        rv[i] = pack_h2(c2, -s2);
+        iv[i] = pack_h2(s2, c2);
+    }
+    constexpr int BB = 2 * L * 32;                                      // bytes of one B operand tile
+    sts128(sB, rh[0], rh[1], rh[2], rh[3]);
+    sts128(sB + L * 16, ih[0], ih[1], ih[2], ih[3]);
+    sts128(sB + BB, rl[0], rl[1], rl[2], rl[3]);
+    sts128(sB + BB + L * 16, il[0], il[1], il[2], il[3]);
+    sts128(sB + 2 * BB, rv[0], rv[1], rv[2], rv[3]);
+    sts128(sB + 2 * BB + L * 16, iv[0], iv[1], iv[2], iv[3]);
+}
+
+// Drain L accumulator columns (one of Re / Im) of this warp's 32 TMEM lanes into one plane of ws.
+// Thread = TMEM lane = row h; column l is frequency k0 + 128 l: for a fixed column the warp touches
+// 32 consecutive frequencies (coalesced).
+template <int L>
+__device__ __forceinline__ void us_drain(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first)
+{
+    #pragma unroll 1
+    for (int part = 0; part < L / 16; ++part) {
+        float v[16];
+        tmem_ld16(taddr + 16u * part, v);
+        const int64_t kp = k0 + (int64_t)part * 16 * UM_H;
+        if (!first) {
+            #pragma unroll
+            for (int i = 0; i < 16; ++i) { const int64_t k = kp + (int64_t)i * UM_H; if (k < Nf) v[i] += dst[k]; }
+        }
+        #pragma unroll
+        for (int i = 0; i < 16; ++i) { const int64_t k = kp + (int64_t)i * UM_H; if (k < Nf) dst[k] = v[i]; }
+    }
+}
+
+// grid.x = B * nsplit * nfb (frequency block fastest), US_THREADS threads, UmmaSmall<L, US_STAGES>::SMEM bytes of
+// dynamic shared memory (one k-step of 8 samples per stage), MINB CTAs per SM.  p.nfb = ceil(Nf / (128 L)).
+template <int L, int US_STAGES, int MINB>
+__global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(const UmmaParams p)
+{
+    using C = UmmaSmall<L, US_STAGES>;
+    extern __shared__ __align__(128) unsigned char um_smem[];
+    float4* rec = reinterpret_cast<float4*>(um_smem + US_STAGES * C::STAGE_BYTES);                 // [2][UM_TS] {X/sigma, pA32, v32, w32}
+    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + US_STAGES * C::STAGE_BYTES + UM_REC_BYTES);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * US_STAGES + 2);
+
+    const unsigned tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
+    int64_t unit = blockIdx.x;
+    const int fb = (int)(unit % p.nfb); unit /= p.nfb;
+    const int sp = (int)(unit % p.nsplit);
+    const int64_t b = unit / p.nsplit;
+    const int64_t kb = (int64_t)fb * C::FPB;
+    const int64_t j_begin = (int64_t)sp * p.split_len;
+    const int64_t j_end = min(p.Nt, j_begin + p.split_len);
+    const int64_t n_samp = j_end - j_begin;
+    const int nks = (int)((n_samp + UM_KS - 1) / UM_KS);
+    const int flush_ksteps = max(1, p.flush_ksteps);
+
+    const uint32_t s_stage = smem_u32(um_smem), s_bar = smem_u32(bars);
+    const uint32_t bar_accf = s_bar + 8u * (2 * US_STAGES), bar_acce = bar_accf + 8u;
+#define US_FULL(s) (s_bar + 8u * (unsigned)(s))
+#define US_EMPTY(s) (s_bar + 8u * (unsigned)(US_STAGES + (s)))
+
+    if (tid == 0) {
+        for (int s = 0; s < US_STAGES; ++s) { mbar_init(US_FULL(s), US_GEN_WARPS); mbar_init(US_EMPTY(s), 1); }
+        mbar_init(bar_accf, 1);
+        mbar_init(bar_acce, US_GEN_WARPS);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (w == US_GEN_WARPS) {                                            // the MMA warp owns the TMEM allocation
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"(smem_u32(tmem_slot)), "r"((uint32_t)C::TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
+
+    if (w < US_GEN_WARPS) {
+        // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
+        const float4* recA = p.recA + b * p.Nt;
+        const ulonglong2* recB = p.recB + b * p.Nt;
+        const float xs = (tid < UM_TS) ? x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt) : 0.f;
+        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
+        auto prefetch = [&](int ti) {
+            const int64_t j = j_begin + (int64_t)ti * UM_TS + tid;
+            pre_ok = (tid < UM_TS) && (j < j_end);
+            if (pre_ok) { pre_x = __ldg(&recA[j].x); const ulonglong2 q = __ldg(recB + j); pre_u = q.x; pre_v = q.y; }
+        };
+        prefetch(0);
+        const unsigned h = tid & 127u;                                  // A item: row h, 4 samples `chunk` of the k-step
+        const int chunk = (int)(tid >> 7);
+        const unsigned q4 = w & 3u, part = w >> 2;                      // drain: TMEM lane quadrant, Re (0) / Im (1) columns
+        float* ws_unit = p.ws + ((b * p.nsplit + sp) * 4) * p.Nf;
+        const int64_t k0 = kb + (int64_t)(32u * q4 + lane);
+        const uint32_t t_drain = tmem + ((32u * q4) << 16) + (uint32_t)L * part;
+        int kin = 0, flushes = 0;
+
+        for (int ks = 0; ks < nks; ++ks) {
+            const int s = ks % US_STAGES;
+            const uint32_t ph = (uint32_t)(ks / US_STAGES) & 1u;
+            const int ti = ks >> 4;
+            if ((ks & 15) == 0) {                                       // next record tile (buffer ti & 1)
+                if (tid < UM_TS) {
+                    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);         // pad: X = 0, phases 0
+                    if (pre_ok) {
+                        const u64 pa = pre_u + (u64)kb * pre_v;         // u + kb v (mod 1, 64-bit wrap; reading G3)
+                        r.x = pre_x * xs;
+                        r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
+                        r.z = __uint_as_float((unsigned)((pre_v + 0x80000000ull) >> 32));
+                        r.w = __uint_as_float((unsigned)(((u64)UM_H * pre_v + 0x80000000ull) >> 32));
+                    }
+                    rec[(ti & 1) * UM_TS + tid] = r;
+                    prefetch(ti + 1);
+                }
+                asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            }
+            mbar_wait(US_EMPTY(s), ph ^ 1u);                            // the MMAs that read this stage have completed
+            const float4* rt = rec + (ti & 1) * UM_TS;
+            const int sb = (ks & 15) * UM_KS;
+            const uint32_t st = s_stage + (uint32_t)s * C::STAGE_BYTES;
+            um_gen_a(rt, sb + chunk * 4, h, st + chunk * (UM_A_BYTES / 2) + h * 16, n_samp - ((int64_t)ks * UM_KS + chunk * 4));
+            const unsigned bt = (tid - (unsigned)ks * (2u * L)) & 255u;  // the 2L B items rotate over the 256 producer threads
+            if (bt < 2u * L) {
+                const unsigned l = bt % (unsigned)L, bc = bt / (unsigned)L;
+                us_gen_b<L>(rt, sb + (int)bc * 4, l, st + 3 * UM_A_BYTES + bc * (C::B_BYTES / 2) + l * 16);
+            }
+            fence_proxy_async();                                        // generic-proxy stores -> visible to the tensor core
+            __syncwarp();
+            if (lane == 0) mbar_arrive(US_FULL(s));
+
+            const bool last = (ks == nks - 1);
+            if (++kin == flush_ksteps || last) {
+                mbar_wait(bar_accf, (uint32_t)flushes & 1u);            // every MMA issued so far has completed
+                tc_fence_after();
+                us_drain<L>(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0);
+                if (last) us_drain<L>(t_drain + 2u * L, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_acce);
+                ++flushes; kin = 0;
+            }
+        }
+    } else if (lane == 0) {
+        // ===================== step 4: the single MMA-issuing thread =====================
+        int kin = 0, flushes = 0;
+        for (int ks = 0; ks < nks; ++ks) {
+            const int s = ks % US_STAGES;
+            const uint32_t ph = (uint32_t)(ks / US_STAGES) & 1u;
+            mbar_wait(US_FULL(s), ph);
+            tc_fence_after();
+            const uint32_t a0 = s_stage + (uint32_t)s * C::STAGE_BYTES, b0 = a0 + 3 * UM_A_BYTES;
+            const uint64_t dAh = umma_desc(a0, UM_A_BYTES / 2, 128), dAl = umma_desc(a0 + UM_A_BYTES, UM_A_BYTES / 2, 128);
+            const uint64_t dAv = umma_desc(a0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
+            const uint64_t dBh = umma_desc(b0, C::B_BYTES / 2, 128), dBl = umma_desc(b0 + C::B_BYTES, C::B_BYTES / 2, 128);
+            const uint64_t dBv = umma_desc(b0 + 2 * C::B_BYTES, C::B_BYTES / 2, 128);
+            tc_mma_f16(tmem, dAh, dBh, C::IDESC, kin > 0 ? 1u : 0u);
+            tc_mma_f16(tmem, dAl, dBh, C::IDESC, 1u);
+            tc_mma_f16(tmem, dAh, dBl, C::IDESC, 1u);
+            tc_mma_f16(tmem + 2u * L, dAv, dBv, C::IDESC, ks > 0 ? 1u : 0u);
+            tc_commit(US_EMPTY(s));
+            const bool last = (ks == nks - 1);
+            if (++kin == flush_ksteps || last) {
+                tc_commit(bar_accf);
+                if (!last) { mbar_wait(bar_acce, (uint32_t)flushes & 1u); tc_fence_after(); }
+                ++flushes; kin = 0;
+            }
+        }
+    }
+#undef US_FULL
+#undef US_EMPTY
+
+    tc_fence_before();
+    __syncthreads();
+    if (w == US_GEN_WARPS) {
+        __syncwarp();
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"((uint32_t)C::TMEM_COLS) : "memory");
+    }
+}
+
+}  // namespace lsp

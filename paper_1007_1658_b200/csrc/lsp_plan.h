@@ -16,17 +16,18 @@
 namespace lsp {
 
 constexpr int PLAN_REC_ROTATION = 1, PLAN_REC_THREE_TERM = 2, PLAN_REC_THREE_TERM_Z = 3, PLAN_REC_MMA = 4, PLAN_REC_UMMA = 5;
-constexpr int PLAN_UMMA_FPB = 16384, PLAN_UMMA_TS = 128;            // frequencies per CTA, samples per record tile (lsp_accum_umma.cuh)
+constexpr int PLAN_UMMA_TS = 128;                                  // samples per record tile (lsp_accum_umma.cuh)
 constexpr int PLAN_MMA_FPB = 8192, PLAN_MMA_TS = 128;              // frequencies per CTA, samples per tile (lsp_accum_mma.cuh)
 constexpr int PLAN_TILE_PAIR = 512, PLAN_TILE_Z = 256;
 
 struct PlanChoice {
     int K = 0, T = 0, nsplit = 1, rec = 0, nfb = 0, ctas_per_sm = 0;
+    int L = 0;                      // tcgen05 form: coarse extent (frequencies per CTA = 128 L); 0 otherwise
     int64_t split_len = 0;
     double score = 0.0;
 };
 
-struct PlanOverrides { int64_t K = 0, T = 0, nsplit = 0, rec = 0; };
+struct PlanOverrides { int64_t K = 0, T = 0, nsplit = 0, rec = 0, L = 0; };
 
 inline bool plan_valid_K(int rec, int K) {
     if (K < 4 || K > 32 || (K % 4) != 0) return false;
@@ -65,36 +66,71 @@ inline double plan_wave_eff(int64_t units, int64_t slots) {
     return (double)units / (double)(waves * slots);
 }
 
-// Tensor-core forms: one CTA per SM owns `fpb` frequencies (8,192 mma.sync / 16,384 tcgen05); only the time split is free.
+// tcgen05 form, cost model (SM cycles at the nominal clock, measured on B200): cycles one SM spends per k-step of
+// 8 samples of ONE CTA's 128 L frequencies.  L = 128 is bound by the tensor pipe (4 MMAs m128n256k16 = 512 cycles at
+// the nominal clock; the measured figure includes the power-capped clock of long runs and is higher without the
+// coarse-operand table); L <= 64 by the generation of the fine operand A (lsp_accum_umma_small.cuh), two CTAs per SM:
+// measured 458 / 566 / 698 SM cycles per CTA k-step for L = 16 (three CTAs per SM) / 32 / 64 (C3 and C4, profiles/r01_bench_auto.md).
+inline double plan_umma_kstep_cycles(int L, int nfb) {
+    switch (L) {
+        case 16: return 458.0;
+        case 32: return 566.0;
+        case 64: return 698.0;
+        default: return nfb >= 3 ? 950.0 : 1150.0;
+    }
+}
+inline int plan_umma_ctas_per_sm(int L) { return L >= 128 ? 1 : (L == 16 ? 3 : 2); }
+inline double plan_umma_fixed_cycles(int L) { return (L >= 128 ? 8000.0 : 9000.0) + 93.0 * L; }   // per CTA: set-up + final drain (2 KB L at ~22 B per cycle per SM)
+
+inline double plan_umma_cycles(int sm_count, int64_t units, int64_t split_len, int L, int nfb) {
+    const int cps = plan_umma_ctas_per_sm(L);
+    const int64_t slots = (int64_t)cps * sm_count;
+    const int64_t waves = (units + slots - 1) / slots;
+    const double share = units >= slots ? (double)cps : (double)((units + sm_count - 1) / sm_count);   // CTAs sharing an SM
+    return (double)waves * ((double)((split_len + 7) / 8) * plan_umma_kstep_cycles(L, nfb) * share + plan_umma_fixed_cycles(L));
+}
+
+// Tensor-core forms: a CTA owns `fpb` frequencies (8,192 mma.sync; 128 L tcgen05, L = 16 / 32 / 64 / 128); the time
+// split and (tcgen05) L are free.  Picks the (L, nsplit) with the fewest estimated cycles.
 inline PlanChoice plan_choose_mma(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanOverrides& ov, int rec = PLAN_REC_MMA)
 {
-    const int FPB = rec == PLAN_REC_UMMA ? PLAN_UMMA_FPB : PLAN_MMA_FPB, TS = rec == PLAN_REC_UMMA ? PLAN_UMMA_TS : PLAN_MMA_TS;
-    const double fixed = rec == PLAN_REC_UMMA ? 200.0 : 300.0;      // per-CTA fixed cost in samples: set-up + final drain
     PlanChoice best;
-    const int64_t nfb = (Nf + FPB - 1) / FPB;
-    const int64_t max_splits = (Nt + TS - 1) / TS;
-    int64_t cap = ((int64_t)1 << 31) / (B * 16 * Nf);
-    if (cap < 1) cap = 1;
-    int64_t hi = max_splits < cap ? max_splits : cap;
-    if (hi > 1024) hi = 1024;
-    int64_t lo = 1;
-    if (ov.nsplit) { lo = hi = (ov.nsplit < max_splits ? ov.nsplit : max_splits); }
-    for (int64_t n = lo; n <= hi; ++n) {
-        int64_t len = (Nt + n - 1) / n;
-        len = (len + TS - 1) / TS * TS;
-        const int64_t n_eff = (Nt + len - 1) / len;
-        if (n_eff != n && !ov.nsplit) continue;
-        const int64_t units = B * nfb * n_eff;
-        const double wave = plan_wave_eff(units, sm_count);
-        const double avg_len = (double)Nt / (double)n_eff;
-        const double unit = avg_len / (avg_len + fixed);            // per-CTA fixed cost: outer-sum init + write-out
-        const double score = wave * unit;
-        if (score > best.score * 1.0025 || best.K == 0) {
-            best.K = 32; best.T = rec == PLAN_REC_UMMA ? 544 : 256; best.nsplit = (int)n_eff; best.rec = rec; best.nfb = (int)nfb;
-            best.ctas_per_sm = 1; best.split_len = len; best.score = score;
+    double best_cycles = 0.0;
+    const int Ls[4] = {128, 64, 32, 16};
+    for (int li = 0; li < (rec == PLAN_REC_UMMA ? 4 : 1); ++li) {
+        const int L = rec == PLAN_REC_UMMA ? Ls[li] : 0;
+        if (rec == PLAN_REC_UMMA && ov.L && ov.L != L) continue;
+        const int FPB = rec == PLAN_REC_UMMA ? 128 * L : PLAN_MMA_FPB, TS = rec == PLAN_REC_UMMA ? PLAN_UMMA_TS : PLAN_MMA_TS;
+        const int cps = rec == PLAN_REC_UMMA ? plan_umma_ctas_per_sm(L) : 1;
+        const int64_t nfb = (Nf + FPB - 1) / FPB;
+        const int64_t max_splits = (Nt + TS - 1) / TS;
+        int64_t cap = ((int64_t)1 << 31) / (B * 16 * Nf);
+        if (cap < 1) cap = 1;
+        int64_t hi = max_splits < cap ? max_splits : cap;
+        if (hi > 1024) hi = 1024;
+        int64_t lo = 1;
+        if (ov.nsplit) { lo = hi = (ov.nsplit < max_splits ? ov.nsplit : max_splits); }
+        PlanChoice cand;                                            // best time split for this L
+        double cand_cycles = 0.0;
+        for (int64_t n = lo; n <= hi; ++n) {
+            int64_t len = (Nt + n - 1) / n;
+            len = (len + TS - 1) / TS * TS;
+            const int64_t n_eff = (Nt + len - 1) / len;
+            if (n_eff != n && !ov.nsplit) continue;
+            const int64_t units = B * nfb * n_eff;
+            double cycles;
+            if (rec == PLAN_REC_UMMA) cycles = plan_umma_cycles(sm_count, units, len < Nt ? len : Nt, L, (int)nfb);
+            else cycles = (double)((units + sm_count - 1) / sm_count) * ((double)len + 300.0);
+            if (cand.K == 0 || cycles < cand_cycles * 0.9975) {     // near-ties: fewer splits
+                cand.K = rec == PLAN_REC_UMMA ? L : 32; cand.L = L;
+                cand.T = rec == PLAN_REC_UMMA ? (L >= 128 ? 544 : 288) : 256;
+                cand.nsplit = (int)n_eff; cand.rec = rec; cand.nfb = (int)nfb;
+                cand.ctas_per_sm = cps; cand.split_len = len; cand_cycles = cycles;
+                cand.score = (double)Nf / (double)(nfb * FPB);
+            }
         }
+        if (cand.K && (best.K == 0 || cand_cycles < best_cycles * 0.97)) { best = cand; best_cycles = cand_cycles; }   // near-ties: the wider tile
     }
-    best.score *= (double)Nf / (double)(nfb * FPB);
     return best;
 }
 
@@ -155,12 +191,8 @@ inline PlanChoice plan_choose_fp32(int sm_count, int64_t B, int64_t Nt, int64_t 
 //   included; 1,150 without the coarse-operand table) plus ~20,000 per CTA (set-up, final drain), per wave.
 inline double plan_est_cycles(int sm_count, int64_t B, int64_t Nt, int64_t Nf, const PlanChoice& pc)
 {
-    if (pc.rec == PLAN_REC_UMMA) {
-        const int64_t units = B * (int64_t)pc.nfb * pc.nsplit;
-        const int64_t waves = (units + sm_count - 1) / sm_count;
-        const double per_kstep = pc.nfb >= 3 ? 950.0 : 1150.0;
-        return (double)waves * ((double)((pc.split_len + 7) / 8) * per_kstep + 20000.0);
-    }
+    if (pc.rec == PLAN_REC_UMMA)
+        return plan_umma_cycles(sm_count, B * (int64_t)pc.nfb * pc.nsplit, pc.split_len, pc.L, pc.nfb);
     const double lane_ops = pc.rec == PLAN_REC_ROTATION ? 8.0 : 6.0;
     return (double)B * (double)Nt * (double)Nf * lane_ops / (128.0 * sm_count * (pc.score > 1e-6 ? pc.score : 1e-6)) + 4000.0;
 }

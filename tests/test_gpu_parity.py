@@ -31,11 +31,18 @@ def _check(P_gpu, P_ref, what=""):
     return err / np.max(P_ref)
 
 
+def _same_peak(P_gpu, P_ref):
+    """Reading G9: the arg-max must be bit-exact on seed-QUALIFIED inputs (top-two gap >= 1e-5 max P).  The ad-hoc
+    ragged-size inputs of this file are not qualified; on a near-tie below that gap either bin is a valid peak."""
+    i_gpu, i_ref = int(np.argmax(P_gpu)), oracle.argmax(P_ref)
+    return i_gpu == i_ref or (P_ref[i_ref] - P_ref[i_gpu]) < 1e-5 * P_ref[i_ref]
+
+
 def _run_single(h, w, **params):
     import torch
-    from paper_1007_1658_b200 import PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE
+    from paper_1007_1658_b200 import PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE, PARAM_COARSE
     keys = {"K": PARAM_K, "threads": PARAM_THREADS, "nsplit": PARAM_NSPLIT,
-            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE}
+            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE, "coarse": PARAM_COARSE}
     for k, v in keys.items():
         h.set_param(v, params.get(k, 0))
     try:
@@ -100,7 +107,7 @@ def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit, rec):
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=4000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=rec, nsplit=nsplit)
+    P = _run_single(h, w, rec=rec, nsplit=nsplit, coarse=128 if rec == 5 else 0)
     _check(P, ref, "rec=%d Nt=%d Nf=%d" % (rec, Nt, Nf))
     assert int(np.argmax(P)) == oracle.argmax(ref)
     plan = h.last_plan()
@@ -116,7 +123,7 @@ def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush):
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=6000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2)
+    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2, coarse=128)
     if Nt >= 100:
         _check(P, ref, "umma-tab Nt=%d Nf=%d" % (Nt, Nf))
         assert int(np.argmax(P)) == oracle.argmax(ref)
@@ -126,6 +133,48 @@ def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush):
     assert plan["recurrence"] == 5 and "B-table" in plan["kernel"] and plan["launches"] == 5
 
 
+@pytest.mark.parametrize("coarse", [16, 32, 64])
+@pytest.mark.parametrize("Nt,Nf,nsplit,flush", [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 20011, 0, 0), (1025, 8193, 2, 0),
+                                                (127, 40, 0, 0), (130, 16385, 1, 0), (4099, 3001, 1, 16), (4099, 3001, 2, 1000),
+                                                (8, 100, 1, 0), (1000, 2000, 1, 0)])
+def test_umma_small_form_ragged(lsp, Nt, Nf, nsplit, flush, coarse):
+    """rec = 5 with a narrow coarse extent (128 x L frequencies per CTA, MMA N = 2L, two CTAs per SM):
+    ragged tiles, k-steps and frequency blocks, several drains, every L."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=Nt, Nf=Nf, seed=7000 + Nt)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, coarse=coarse)
+    if Nt >= 100:
+        _check(P, ref, "umma-small L=%d Nt=%d Nf=%d" % (coarse, Nt, Nf))
+        if Nt >= 512:                                      # below the automatic form's threshold (PLAN_TC_MIN_NT) only the tolerance is promised
+            assert _same_peak(P, ref)
+    else:                                                  # tiny Nt: single fp16 pass of V limits |dP|/P to ~4e-4/sqrt(Nt)
+        assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
+    plan = h.last_plan()
+    assert plan["recurrence"] == 5 and plan["K"] == coarse and "small" in plan["kernel"]
+    assert plan["n_freq_blocks"] == -(-Nf // (128 * coarse))
+
+
+@pytest.mark.parametrize("coarse", [16, 32, 64])
+def test_umma_small_form_batched_noise(lsp, coarse):
+    """Batched pure noise (the tightest tolerance) through the narrow tcgen05 tiles, with per-series peaks."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=37, Nt=1000, Nf=2000, seed=4747)
+    Pref, iref, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
+    h.set_param(pkg.PARAM_RECURRENCE, 5); h.set_param(pkg.PARAM_COARSE, coarse)
+    try:
+        t, x = _dev(w)
+        P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+        assert h.last_plan()["K"] == coarse
+    finally:
+        h.set_param(pkg.PARAM_RECURRENCE, 0); h.set_param(pkg.PARAM_COARSE, 0)
+    for b in range(w.B):
+        _check(P[b].cpu().numpy(), Pref[b], "umma-small L=%d series %d" % (coarse, b))
+    assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
+
+
 @pytest.mark.parametrize("flush", [8, 64, 1000, 4096])
 def test_umma_drain_intervals(lsp, flush):
     """rec = 5: D_W is drained from TMEM every `flush` samples (store first, then read-modify-write)."""
@@ -133,7 +182,7 @@ def test_umma_drain_intervals(lsp, flush):
     w = workloads.c1(Nt=4099, Nf=3001, seed=5005)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
     for nsplit in (1, 2):
-        P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=1)
+        P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=1, coarse=128)
         _check(P, ref, "umma flush=%d nsplit=%d" % (flush, nsplit))
         assert int(np.argmax(P)) == oracle.argmax(ref)
 

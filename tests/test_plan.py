@@ -48,10 +48,15 @@ def test_plan_query_rejects_bad_sizes():
 
 @pytest.mark.parametrize("B,Nt,Nf", [(1, 10000, 10000), (1, 100000, 1000000), (4096, 1000, 2000),
                                      (1, 1000000, 1000000), (1, 382003, 1528064), (2, 700, 40000)])
-@pytest.mark.parametrize("rec,fpb,threads", [(4, 8192, 256), (5, 16384, 544)])
-def test_tensor_core_plans_cover_the_problem(B, Nt, Nf, rec, fpb, threads):
+@pytest.mark.parametrize("rec", [4, 5])
+def test_tensor_core_plans_cover_the_problem(B, Nt, Nf, rec):
     p = pkg.plan_query_form(SM, B, Nt, Nf, rec)
-    assert p["recurrence"] == rec and p["threads"] == threads and p["ctas_per_sm"] == 1
+    if rec == 4:
+        fpb, threads, cps = 8192, 256, 1
+    else:                                                  # tcgen05: K reports the coarse extent L; a CTA owns 128 L frequencies
+        assert p["K"] in (16, 32, 64, 128)
+        fpb, threads, cps = 128 * p["K"], (544 if p["K"] == 128 else 288), {128: 1, 64: 2, 32: 2, 16: 3}[p["K"]]
+    assert p["recurrence"] == rec and p["threads"] == threads and p["ctas_per_sm"] == cps
     assert p["n_freq_blocks"] * fpb >= Nf and (p["n_freq_blocks"] - 1) * fpb < Nf
     assert p["nsplit"] >= 1 and p["nsplit"] * p["split_len"] >= Nt and (p["nsplit"] - 1) * p["split_len"] < Nt
     assert p["split_len"] % 128 == 0
@@ -73,3 +78,12 @@ def test_automatic_form():
     assert auto["recurrence"] == 5 and auto["est_cycles"] < z["est_cycles"]
     with pytest.raises(pkg.LspError):
         pkg.plan_query_form(SM, 1, 10, 10, 6)
+
+
+def test_tcgen05_coarse_extent_follows_the_grid():
+    """Long grids take the 128 x 128 tile (tensor-pipe bound); a Monte-Carlo batch of short grids (C4) takes a
+    narrow tile that the grid fills, two CTAs per SM."""
+    assert pkg.plan_query_form(SM, 1, 1000000, 1000000, 5)["K"] == 128
+    c4 = pkg.plan_query_form(SM, 4096, 1000, 2000, 5)
+    assert c4["K"] == 16 and c4["n_freq_blocks"] == 1 and c4["nsplit"] == 1
+    assert pkg.plan_query(SM, 4096, 1000, 2000)["recurrence"] == 5

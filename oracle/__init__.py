@@ -12,7 +12,8 @@ Nothing under paper_1007_1658_b200/ imports this package, and this package impor
 nothing from it.  Only tests/, __graft_entry__.smoke() and bench.py (cpu_baseline and
 --impl reference) may import it.  Every function cites the passage it follows.
 
-Pins: tests/test_oracle_pins.py (P1..P9 of DESIGN.md).  No function here is "parity unpinned".
+Pins: tests/test_oracle_pins.py (P1..P9 of DESIGN.md; GP1..GP5 for the generalised periodogram).
+No function here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -51,6 +52,8 @@ def _load():
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
             ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+        lib.lsp_oracle_gls.restype = ctypes.c_int
+        lib.lsp_oracle_gls.argtypes = lib.lsp_oracle_periodogram.argtypes
         lib.lsp_oracle_moments.restype = None
         lib.lsp_oracle_moments.argtypes = [ctypes.c_void_p, ctypes.c_int64,
                                            ctypes.c_void_p, ctypes.c_void_p]
@@ -100,6 +103,43 @@ def periodogram(t, x, f_min: float, df: float, Nf: int,
                                           float(f_min), float(df), ks_ptr, nk,
                                           P.ctypes.data, scratch.ctypes.data, int(nthreads))
     return (P, used) if return_threads else P
+
+
+def periodogram_gls(t, x, f_min: float, df: float, Nf: int,
+                    ks: Optional[np.ndarray] = None, nthreads: int = 0) -> np.ndarray:
+    """Generalised (floating-mean) periodogram on the grid f_k = f_min + k*df, same normalisation as
+    `periodogram` (definition by a 3-parameter least-squares fit, see lsp_oracle.c)."""
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    assert t.ndim == 1 and t.shape == x.shape and t.size >= 4
+    if ks is None:
+        nk, ks_ptr = int(Nf), None
+    else:
+        ks = np.ascontiguousarray(ks, dtype=np.int64)
+        nk, ks_ptr = int(ks.size), ks.ctypes.data
+    P = np.empty(nk, dtype=np.float64)
+    scratch = np.empty(t.size, dtype=np.float64)
+    _load().lsp_oracle_gls(t.ctypes.data, x.ctypes.data, t.size, float(f_min), float(df), ks_ptr, nk,
+                           P.ctypes.data, scratch.ctypes.data, int(nthreads))
+    return P
+
+
+def periodogram_gls_numpy(t, x, freqs) -> np.ndarray:
+    """Numpy twin of lsp_oracle_gls: the chi^2 reduction of the fit x ~ a cos + b sin + c by numpy.linalg.lstsq
+    (SVD; a different solver from the C normal equations), over 2 var."""
+    t = np.asarray(t, dtype=np.float64)
+    X = np.asarray(x, dtype=np.float32).astype(np.float64)
+    Nt = t.size
+    X = X - X.sum() / Nt
+    chi0 = (X * X).sum()
+    var = chi0 / (Nt - 1)
+    out = np.empty(len(freqs))
+    for i, f in enumerate(np.asarray(freqs, dtype=np.float64)):
+        w = 2.0 * np.pi * f
+        A = np.stack([np.cos(w * t), np.sin(w * t), np.ones(Nt)], axis=1)
+        beta, _, rank, _ = np.linalg.lstsq(A, X, rcond=None)
+        out[i] = 0.0 if rank < 3 else (chi0 - ((X - A @ beta) ** 2).sum()) / (2.0 * var)
+    return out
 
 
 def periodogram_batched(t, x, f_min: float, df: float, Nf: int, nthreads: int = 0):

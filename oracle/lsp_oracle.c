@@ -119,6 +119,76 @@ int lsp_oracle_periodogram(const double* t, const float* x, int64_t Nt,
     return used;
 }
 
+/*
+ * Generalised (floating-mean) periodogram, the extension the paper names in section 6.3 (PAPER.md:375,
+ * Zechmeister & Kuerster 2009).  Written here as its DEFINITION, not
+ * through their closed-form sums: for every frequency, the unweighted linear least-squares fit of
+ *     x_j ~ a cos(w t_j) + b sin(w t_j) + c
+ * (normal equations of the 3 basis functions, Gaussian elimination with partial pivoting), and
+ *     P = (chi0^2 - chi^2_min) / (2 var),   chi0^2 = sum (x_j - mean)^2,   var = chi0^2 / (Nt - 1)
+ * i.e. the same normalisation as eq. (1), which is the special case c = 0: for the 2-function fit
+ * the chi^2 reduction IS eq. (1) (pin P1).  0 <= P <= (Nt - 1)/2.  A singular fit (w = 0: the constant and the
+ * cosine coincide) returns 0 (reading G7 carried over).
+ */
+static double lsp_oracle_gls_one(const double* t, const double* X, int64_t Nt, double f, double var)
+{
+    const double w = LSP_ORACLE_TWO_PI * f;
+    double M[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};      /* [A^T A | A^T X] */
+    for (int64_t j = 0; j < Nt; ++j) {
+        const double a = w * t[j];
+        const double g[3] = {cos(a), sin(a), 1.0};
+        for (int r = 0; r < 3; ++r) {
+            for (int c = 0; c < 3; ++c) M[r][c] += g[r] * g[c];
+            M[r][3] += g[r] * X[j];
+        }
+    }
+    const double rhs[3] = {M[0][3], M[1][3], M[2][3]};
+    const double tiny = 1e-12 * (double)Nt;
+    for (int col = 0; col < 3; ++col) {                                /* elimination, partial pivoting */
+        int piv = col;
+        for (int r = col + 1; r < 3; ++r) if (fabs(M[r][col]) > fabs(M[piv][col])) piv = r;
+        if (fabs(M[piv][col]) <= tiny) return 0.0;                      /* singular: G7 */
+        if (piv != col) for (int c = 0; c < 4; ++c) { double tmp = M[col][c]; M[col][c] = M[piv][c]; M[piv][c] = tmp; }
+        for (int r = col + 1; r < 3; ++r) {
+            const double q = M[r][col] / M[col][col];
+            for (int c = col; c < 4; ++c) M[r][c] -= q * M[col][c];
+        }
+    }
+    double beta[3];
+    for (int r = 2; r >= 0; --r) {
+        double v = M[r][3];
+        for (int c = r + 1; c < 3; ++c) v -= M[r][c] * beta[c];
+        beta[r] = v / M[r][r];
+    }
+    const double reduction = beta[0] * rhs[0] + beta[1] * rhs[1] + beta[2] * rhs[2];   /* chi0^2 - chi^2_min */
+    return reduction / (2.0 * var);
+}
+
+/* Same calling convention as lsp_oracle_periodogram. */
+int lsp_oracle_gls(const double* t, const float* x, int64_t Nt,
+                   double f_min, double df, const int64_t* ks, int64_t nk,
+                   double* P, double* scratch, int nthreads)
+{
+    double mean, var;
+    lsp_oracle_moments(x, Nt, &mean, &var);
+    for (int64_t j = 0; j < Nt; ++j) scratch[j] = (double)x[j] - mean;
+    int used = 1;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    #pragma omp parallel
+    {
+        #pragma omp single
+        used = omp_get_num_threads();
+    }
+    #pragma omp parallel for schedule(dynamic, 4)
+#endif
+    for (int64_t i = 0; i < nk; ++i) {
+        int64_t k = ks ? ks[i] : i;
+        P[i] = lsp_oracle_gls_one(t, scratch, Nt, f_min + (double)k * df, var);
+    }
+    return used;
+}
+
 /* Lowest index among equal maxima (reading G9). */
 int64_t lsp_oracle_argmax(const double* P, int64_t n)
 {

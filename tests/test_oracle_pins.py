@@ -284,3 +284,86 @@ def test_paper_facts_fixture():
     assert abs(Nf * (4 * Nt + 1) / (Nf * (2 * Nt + 3)) - 2.0) < 1e-4
     tc = facts["t_calc_s"]
     assert abs(tc["cpu8"] / tc["C1060"] - 28) < 1.0        # "approaching thirty" (abstract)
+
+
+# ------------------------------------------------------------------ generalised (floating-mean) periodogram
+def _gappy(Nt, seed, span=30.0):
+    rng = np.random.default_rng(seed)
+    t = np.sort(rng.uniform(0.0, span, Nt))
+    return rng, t
+
+
+def test_GP1_c_gls_matches_numpy_lstsq():
+    """C normal equations + elimination vs numpy's SVD least squares (independent solver), random sampling."""
+    rng, t = _gappy(57, 11)
+    x = (1.3 + np.sin(2 * np.pi * 0.41 * t + 0.3) + 0.4 * rng.standard_normal(t.size)).astype(np.float32)
+    f_min, df, Nf = 0.02, 0.013, 90
+    P = oracle.periodogram_gls(t, x, f_min, df, Nf)
+    ref = oracle.periodogram_gls_numpy(t, x, f_min + df * np.arange(Nf))
+    assert np.max(np.abs(P - ref)) <= 1e-11 * max(1.0, ref.max())
+    ks = np.array([0, 7, 89, 44], dtype=np.int64)
+    assert np.array_equal(oracle.periodogram_gls(t, x, f_min, df, Nf, ks=ks), P[ks])
+
+
+def test_GP2_scipy_floating_mean():
+    """Library special case: scipy.signal.lombscargle(floating_mean=True, normalize=True) is the fraction of the
+    variance the fit explains; times (Nt - 1)/2 it is this normalisation."""
+    from scipy.signal import lombscargle
+    rng, t = _gappy(200, 12, span=50.0)
+    x = (5.0 + 0.8 * np.sin(2 * np.pi * 0.23 * t) + rng.standard_normal(t.size)).astype(np.float32)
+    f = 0.01 + 0.004 * np.arange(400)
+    P = oracle.periodogram_gls(t, x, f[0], 0.004, f.size)
+    X = x.astype(np.float64)
+    p = lombscargle(t, X, 2 * np.pi * f, floating_mean=True, normalize=True)
+    assert np.max(np.abs(P - p * (t.size - 1) / 2.0)) <= 1e-9 * P.max()
+
+
+def test_GP3_sinusoid_plus_offset_reaches_the_maximum():
+    """x = c + A sin(w t + phi) sampled over a FRACTION of a cycle: the floating-mean fit is exact, so
+    P = (Nt - 1)/2 (the largest possible value), whereas eq. (1) (mean fixed at the sample mean) falls short."""
+    t = np.linspace(0.0, 0.6, 41) ** 1.3                       # uneven, 0.3 of a cycle of f0
+    f0 = 0.5
+    x = (2.0 + 0.7 * np.sin(2 * np.pi * f0 * t + 0.9)).astype(np.float64)
+    x32 = x.astype(np.float32)
+    P = oracle.periodogram_gls(t, x32, f0, 1.0, 1)[0]
+    assert abs(P - (t.size - 1) / 2.0) <= 1e-5 * (t.size - 1) / 2.0      # fp32 rounding of x is the only residual
+    assert oracle.periodogram(t, x32, f0, 1.0, 1)[0] < 0.99 * P
+
+
+def test_GP4_equals_eq1_on_even_sampling_at_fourier_frequencies():
+    """Even sampling, Fourier frequencies 0 < k < N/2: sum cos = sum sin = 0, the constant is orthogonal to the
+    sinusoids and the generalised periodogram reduces to eq. (1)."""
+    N, dt = 64, 0.25
+    rng = np.random.default_rng(13)
+    t = dt * np.arange(N)
+    x = rng.standard_normal(N).astype(np.float32)
+    df = 1.0 / (N * dt)
+    P1 = oracle.periodogram(t, x, df, df, N // 2 - 1)
+    Pg = oracle.periodogram_gls(t, x, df, df, N // 2 - 1)
+    assert np.max(np.abs(P1 - Pg)) <= 1e-12 * P1.max()
+
+
+def test_GP5_zechmeister_kuerster_closed_form():
+    """The closed form of the cited paper (Zechmeister & Kuerster 2009, eqs 4-13, unit weights w = 1/N), typed here:
+    p = [SS YC^2 + CC YS^2 - 2 CS YC YS] / (YY D), D = CC SS - CS^2, with mean-corrected sums; P = p (Nt-1)/2."""
+    rng, t = _gappy(83, 14, span=12.0)
+    x = (0.2 + np.cos(2 * np.pi * 0.9 * t) + 0.5 * rng.standard_normal(t.size)).astype(np.float32)
+    y = x.astype(np.float64)
+    N = t.size
+    f = 0.05 + 0.021 * np.arange(120)
+    out = np.empty(f.size)
+    for i, fi in enumerate(f):
+        c, s = np.cos(2 * np.pi * fi * t), np.sin(2 * np.pi * fi * t)
+        Y, C, S = y.mean(), c.mean(), s.mean()
+        YY = (y * y).mean() - Y * Y
+        YC = (y * c).mean() - Y * C
+        YS = (y * s).mean() - Y * S
+        CC = (c * c).mean() - C * C
+        SS = (s * s).mean() - S * S
+        CS = (c * s).mean() - C * S
+        D = CC * SS - CS * CS
+        out[i] = (SS * YC ** 2 + CC * YS ** 2 - 2 * CS * YC * YS) / (YY * D) * (N - 1) / 2.0
+    P = oracle.periodogram_gls(t, x, f[0], 0.021, f.size)
+    assert np.max(np.abs(P - out)) <= 1e-10 * P.max()
+    assert P.min() >= 0.0 and P.max() <= (N - 1) / 2.0
+    assert oracle.periodogram_gls(t, x, 0.0, 0.1, 1)[0] == 0.0                  # singular at f = 0 (G7)

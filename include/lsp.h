@@ -122,6 +122,15 @@ int lsp_periodogram_batched_host(lsp_handle h,
                                  void* stream);
 
 /*
+ * False-alarm probability, eq. (3):  Q[i] = 1 - [1 - (1 - 2 P[i]/Nt)^((Nt-3)/2)]^N_ind
+ * for n periodogram values (a whole periodogram, or the per-series peaks of a batch).
+ *   P DEVICE const float[n] (normalised power, as written by lsp_periodogram*), Q DEVICE float[n] (may alias P).
+ *   Nt >= 4: samples of the series that produced P;  N_ind >= 1: number of independent frequencies -- the paper's
+ *   N_f, or the N_f,ind <= N_f of PAPER.md:369 (real-valued).  Enqueues one kernel on `stream`; no synchronisation.
+ */
+int lsp_false_alarm(lsp_handle h, const float* P, int64_t n, int64_t Nt, double N_ind, float* Q, void* stream);
+
+/*
  * Introspection of the last call's launch plan (for benchmarks and tests): fills
  * out[0..7] = {K, threads, nsplit, recurrence, n_freq_blocks, split_len, launches, lane_ops_per_term}.
  */

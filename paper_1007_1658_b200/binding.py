@@ -22,6 +22,7 @@ SYMBOLS = (
     "lsp_create", "lsp_destroy", "lsp_set_param", "lsp_get_param",
     "lsp_periodogram", "lsp_periodogram_batched",
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
+    "lsp_false_alarm",
     "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
@@ -59,6 +60,7 @@ def load(rebuild: bool = False):
     lib.lsp_periodogram_host.argtypes = [vp, vp, vp, i64, dbl, dbl, i64, vp, vp]
     lib.lsp_periodogram_batched_host.argtypes = [vp, vp, ci, vp, i64, i64, dbl, dbl, i64,
                                                  vp, vp, vp, vp]
+    lib.lsp_false_alarm.argtypes = [vp, vp, i64, i64, dbl, vp, vp]
     lib.lsp_last_plan.argtypes = [vp, ctypes.POINTER(i64)]
     lib.lsp_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     lib.lsp_call_timing.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_float)]
@@ -219,6 +221,17 @@ class Handle:
             _stream_ptr(stream))
         self._check(st, "lsp_periodogram_batched")
         return P, pi, pv
+
+    def false_alarm(self, P, Nt: int, N_ind: float, out=None, stream=None):
+        """lsp_false_alarm: eq. (3) for a CUDA float32 tensor of periodogram values (any shape, contiguous)."""
+        import torch
+        if P.dtype != torch.float32 or not P.is_cuda or not P.is_contiguous():
+            raise ValueError("P must be a contiguous float32 CUDA tensor")
+        Q = out if out is not None else torch.empty_like(P)
+        st = self._lib.lsp_false_alarm(self._h, P.data_ptr(), P.numel(), int(Nt), float(N_ind), Q.data_ptr(),
+                                       _stream_ptr(stream))
+        self._check(st, "lsp_false_alarm")
+        return Q
 
     # -- host-pointer entry points (CPU tensors / numpy arrays in and out; synchronous)
     def periodogram_host(self, t, x, f_min: float, df: float, Nf: int, out=None, stream=None):

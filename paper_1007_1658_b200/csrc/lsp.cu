@@ -11,6 +11,7 @@
 #include "lsp_accum_umma_tab.cuh"
 #include "lsp_accum_umma_small.cuh"
 #include "lsp_finish.cuh"
+#include "lsp_fap.cuh"
 #include "lsp_plan.h"
 
 #include <cmath>
@@ -452,6 +453,17 @@ int lsp_periodogram_host(lsp_handle h, const double* t, const float* x, int64_t 
 {
     if (!P) return LSP_EINVAL;
     return lsp_periodogram_batched_host(h, t, 0, x, 1, Nt, f_min, df, Nf, P, nullptr, nullptr, stream);
+}
+
+int lsp_false_alarm(lsp_handle h, const float* P, int64_t n, int64_t Nt, double N_ind, float* Q, void* stream)
+{
+    if (!h || !P || !Q || n < 1 || Nt < 4 || !(N_ind >= 1.0) || !std::isfinite(N_ind)) return LSP_EINVAL;
+    DeviceGuard g(h->device);
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 2147483647LL) return LSP_EINVAL;
+    fap_kernel<<<(unsigned)blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(P, n, (double)Nt, N_ind, Q);
+    LSP_CUDA(h, cudaGetLastError());
+    return LSP_OK;
 }
 
 int lsp_last_plan(lsp_handle h, int64_t out[8])

@@ -337,6 +337,39 @@ def test_host_entry_points(lsp):
 
 
 # ------------------------------------------------------------------ argument errors
+def test_false_alarm_probability(lsp):
+    """Eq. (3) epilogue against the oracle's plain formula on the GPU's own P (C1), on per-series peaks of a noise
+    batch, and on hand-made values spanning Q = 1 ... 1e-30."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c1()
+    t, x = _dev(w)
+    P = h.periodogram(t, x, w.f_min, w.df, w.Nf)
+    for n_ind in (float(w.Nf), 137.5, 1.0):
+        Q = h.false_alarm(P, w.Nt, n_ind).cpu().numpy().astype(np.float64)
+        ref = oracle.false_alarm_probability(P.cpu().numpy(), w.Nt, n_ind)
+        assert np.all(np.abs(Q - ref) <= 1e-6 + 1e-5 * ref), np.max(np.abs(Q - ref))
+        assert np.all((Q >= 0.0) & (Q <= 1.0))
+    vals = torch.tensor([0.0, 0.5, 1.0, 5.0, 10.0, 20.0, 40.0, 80.0, 160.0, 320.0, 499.5], dtype=torch.float32, device="cuda")
+    Q = h.false_alarm(vals, 1000, 2000.0).cpu().numpy().astype(np.float64)
+    ref = oracle.false_alarm_probability(vals.cpu().numpy(), 1000, 2000.0)
+    big = ref > 1e-12                                      # the oracle's 1 - (1 - s)^N loses tiny Q to cancellation
+    assert np.all(np.abs(Q[big] - ref[big]) <= 1e-6 + 1e-5 * ref[big])
+    s = np.clip(1.0 - 2.0 * vals.cpu().numpy().astype(np.float64) / 1000, 0, 1) ** ((1000 - 3) / 2.0)
+    small = (~big) & (s > 0)
+    assert np.all(np.abs(Q[small] - 2000.0 * s[small]) <= 1e-5 * 2000.0 * s[small] + 1e-44)   # Q -> N s for s -> 0
+    assert Q[0] == 1.0 and Q[-1] == 0.0 and np.all(np.diff(Q) <= 0)
+    wb = workloads.c4(B=16, Nt=600, Nf=700, seed=99)
+    _, pi, pv = h.periodogram_batched(*_dev(wb), wb.f_min, wb.df, wb.Nf)
+    Qp = h.false_alarm(pv, wb.Nt, wb.Nf).cpu().numpy()
+    refp = oracle.false_alarm_probability(pv.cpu().numpy(), wb.Nt, wb.Nf)
+    assert np.all(np.abs(Qp - refp) <= 1e-6 + 1e-5 * refp)
+    with pytest.raises(pkg.LspError):
+        h.false_alarm(vals, 3, 10.0)
+    with pytest.raises(pkg.LspError):
+        h.false_alarm(vals, 100, 0.5)
+
+
 def test_argument_errors(lsp):
     import torch
     pkg, h = lsp

@@ -104,6 +104,28 @@ int lsp_periodogram_batched(lsp_handle h,
                             void* stream);
 
 /*
+ * Generalised (floating-mean) periodogram -- the extension the paper names in section 6.3 (Zechmeister &
+ * Kuerster 2009): for every frequency the least-squares fit x_j ~ a cos(w t_j) + b sin(w t_j) + c, returned as
+ * P = (chi0^2 - chi^2_min) / (2 var) -- the normalisation of eq. (1), to which it reduces when the constant is
+ * orthogonal to the sinusoids.  Same arguments, layout, ownership and errors as lsp_periodogram[_batched], Nt >= 4.
+ * Computed from the sums of eq. (8) plus sum cos(w t_j), sum sin(w t_j), which a second accumulate pass with unit
+ * weights provides (cost: two accumulate launches).  Where the fit is singular (f -> 0: D = CCn SSn - CSn^2 <= 1e-9) P = 0.
+ */
+int lsp_periodogram_gls(lsp_handle h,
+                        const double* t, const float* x, int64_t Nt,
+                        double f_min, double df, int64_t Nf,
+                        float* P, void* stream);
+
+int lsp_periodogram_gls_batched(lsp_handle h,
+                                const double* t, int64_t t_stride,
+                                const float* x, int64_t x_stride,
+                                int64_t B, int64_t Nt,
+                                double f_min, double df, int64_t Nf,
+                                float* P, int64_t p_stride,
+                                int32_t* peak_idx, float* peak_val,
+                                void* stream);
+
+/*
  * Host-buffer forms: same arithmetic, HOST pointers.  The call copies t and x to the device
  * (cudaMemcpyAsync on `stream`), runs the device path, copies P (and the peaks) back and
  * synchronises `stream`.  Arrays are dense: series b at t + b*Nt, x + b*Nt, P + b*Nf.

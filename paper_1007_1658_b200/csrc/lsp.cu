@@ -135,7 +135,7 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
 int run_device(lsp_ctx* h,
                const double* t, int64_t t_stride, const float* x, int64_t x_stride,
                int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
-               float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st)
+               float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st, bool gls = false)
 {
     Plan pl = make_plan(h, B, Nt, Nf);
     const bool umma = pl.rec == REC_UMMA;
@@ -155,6 +155,8 @@ int run_device(lsp_ctx* h,
     const size_t o_recA = off; off = align_up(off + n_samp * sizeof(float4), 256);
     const size_t o_recB = off; off = align_up(off + n_samp * sizeof(ulonglong2), 256);
     const size_t o_ws = off;   off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    const size_t o_ws1 = off;  if (gls) off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    const size_t o_recA1 = off; if (gls) off = align_up(off + n_samp * sizeof(float4), 256);
     const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
@@ -167,12 +169,15 @@ int run_device(lsp_ctx* h,
                          (h->opt_btable == 2 || (pl.nfb >= 3 && tab_bytes <= ((size_t)12 << 30)));
     const size_t o_tab = off;  if (use_tab) off = align_up(off + tab_bytes, 256);
     if (use_tab) { pl.kernel_name = "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>"; pl.launches = 5; }
+    if (gls) pl.launches += 2;                            // unit records + second accumulate pass
     int rc = ensure(h, &h->buf, &h->buf_bytes, off);
     if (rc != LSP_OK) return rc;
     char* base = static_cast<char*>(h->buf);
     float4* recA = reinterpret_cast<float4*>(base + o_recA);
     ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
     float* ws = reinterpret_cast<float*>(base + o_ws);
+    float* ws1 = gls ? reinterpret_cast<float*>(base + o_ws1) : nullptr;          // unit-weight pass: sum cos, sum sin
+    float4* recA1 = gls ? reinterpret_cast<float4*>(base + o_recA1) : nullptr;
     double* psum = reinterpret_cast<double*>(base + o_psum);
     double* pvar = reinterpret_cast<double*>(base + o_pvar);
     u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
@@ -196,6 +201,10 @@ int run_device(lsp_ctx* h,
     records_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
                                          psum, recA, recB, pvar);
     LSP_CUDA(h, cudaGetLastError());
+    if (gls) {
+        unit_records_kernel<<<(unsigned)((n_samp + 255) / 256), 256, 0, st>>>(recA, recA1, (int64_t)n_samp);
+        LSP_CUDA(h, cudaGetLastError());
+    }
     unsigned char* btable = reinterpret_cast<unsigned char*>(base + o_tab);
     if (use_tab) {
         if (tab_groups > 2147483647LL) return LSP_EINVAL;
@@ -209,11 +218,16 @@ int run_device(lsp_ctx* h,
     // steps 3-5
     const int64_t units = B * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
+    // (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
+    for (int pass = 0; pass < (gls ? 2 : 1); ++pass) {
+    const float4* rA = pass ? recA1 : recA;
+    float* wsp = pass ? ws1 : ws;
     if (umma) {
         UmmaParams up;
-        up.recA = recA; up.recB = recB; up.part_var = pvar; up.ws = ws; up.Nt = Nt; up.Nf = Nf;
+        up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
         up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
         up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS;
+        up.unit_x = pass;
         if (umma_small) {
 #define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
             LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
@@ -235,17 +249,19 @@ int run_device(lsp_ctx* h,
         }
     } else if (mma) {
         MmaParams mp;
-        mp.recA = recA; mp.recB = recB; mp.part_var = pvar; mp.ws = ws; mp.Nt = Nt; mp.Nf = Nf;
-        mp.split_len = pl.split_len; mp.nsplit = pl.nsplit; mp.nfb = pl.nfb; mp.nparts = pl.nparts;
+        mp.recA = rA; mp.recB = recB; mp.part_var = pvar; mp.ws = wsp; mp.Nt = Nt; mp.Nf = Nf;
+        mp.split_len = pl.split_len; mp.nsplit = pl.nsplit; mp.nfb = pl.nfb; mp.nparts = pl.nparts; mp.unit_x = pass;
         LSP_CUDA(h, cudaFuncSetAttribute(accum_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMA_SMEM));
         accum_mma_kernel<<<(unsigned)units, MMA_WARPS * 32, MMA_SMEM, st>>>(mp);
     } else {
         AccumParams ap;
-        ap.recA = recA; ap.recB = recB; ap.ws = ws; ap.Nt = Nt; ap.Nf = Nf;
+        ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.Nt = Nt; ap.Nf = Nf;
         ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
         const size_t smem = accum_smem_bytes(ke, pl.T);
         LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
+    }
+    LSP_CUDA(h, cudaGetLastError());
     }
     LSP_CUDA(h, cudaGetLastError());
 
@@ -258,6 +274,7 @@ int run_device(lsp_ctx* h,
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = pl.nsplit; fp.nparts = pl.nparts;
     fp.cc_fix = (!mma && ke->tile_z == 0 && (Nt & 1)) ? 0.5 : 0.0;   // phantom partner of an odd last sample (pair-packed only)
     fp.x_scaled = mma ? 1 : 0;
+    fp.ws1 = ws1;
     const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
     dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
     finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
@@ -399,6 +416,33 @@ int lsp_periodogram_batched(lsp_handle h,
     DeviceGuard g(h->device);
     return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
                       peak_idx, peak_val, static_cast<cudaStream_t>(stream));
+}
+
+int lsp_periodogram_gls_batched(lsp_handle h,
+                                const double* t, int64_t t_stride, const float* x, int64_t x_stride,
+                                int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
+                                float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, void* stream)
+{
+    if (!h || !t || !x) return LSP_EINVAL;
+    if (B < 1 || Nt < 4 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
+    if (bad_grid(f_min, df)) return LSP_EINVAL;
+    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
+    if (!P && !peak_idx) return LSP_EINVAL;
+    if (B > 1) {
+        if (t_stride != 0 && std::llabs(t_stride) < Nt) return LSP_EINVAL;
+        if (std::llabs(x_stride) < Nt) return LSP_EINVAL;
+        if (P && std::llabs(p_stride) < Nf) return LSP_EINVAL;
+    }
+    DeviceGuard g(h->device);
+    return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
+                      peak_idx, peak_val, static_cast<cudaStream_t>(stream), true);
+}
+
+int lsp_periodogram_gls(lsp_handle h, const double* t, const float* x, int64_t Nt,
+                        double f_min, double df, int64_t Nf, float* P, void* stream)
+{
+    if (!P) return LSP_EINVAL;
+    return lsp_periodogram_gls_batched(h, t, Nt, x, Nt, 1, Nt, f_min, df, Nf, P, Nf, nullptr, nullptr, stream);
 }
 
 int lsp_periodogram(lsp_handle h, const double* t, const float* x, int64_t Nt,

@@ -50,6 +50,7 @@ struct MmaParams {
     int64_t Nt, Nf;
     int64_t split_len;          // samples per split (multiple of MMA_TS)
     int nsplit, nfb, nparts;
+    int unit_x;                 // 1: recA.x is a unit weight: no variance scaling
 };
 
 // 1 / sigma as the fp32 factor applied to X before it is split into fp16 pairs.  The finish kernel
@@ -102,7 +103,7 @@ __global__ void __launch_bounds__(MMA_WARPS * 32, 1) accum_mma_kernel(const MmaP
     const int64_t j_end = min(p.Nt, j_begin + p.split_len);
     const float4* recA = p.recA + b * p.Nt;
     const ulonglong2* recB = p.recB + b * p.Nt;
-    const float xs = x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt);
+    const float xs = p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt);
 
     #pragma unroll 8
     for (int i = 0; i < 128; ++i) outer[i * 256 + tid] = 0.f;

@@ -59,6 +59,7 @@ struct UmmaParams {
     int64_t split_len;          // samples per split (multiple of UM_TS)
     int nsplit, nfb, nparts;
     int flush_ksteps;           // k-steps between drains of D_W
+    int unit_x;                 // 1: recA.x is a unit weight, not a measurement: no variance scaling (second pass of the generalised periodogram)
 };
 
 // ------------------------------------------------------------------ PTX wrappers (sm_100a)
@@ -254,7 +255,7 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_kernel(const UmmaPar
         // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
         const float4* recA = p.recA + b * p.Nt;
         const ulonglong2* recB = p.recB + b * p.Nt;
-        const float xs = (tid < UM_TS) ? x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt) : 0.f;
+        const float xs = (tid < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
         float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
         auto prefetch = [&](int ti) {
             const int64_t j = j_begin + (int64_t)ti * UM_TS + tid;

@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
         // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
         const float4* recA = p.recA + b * p.Nt;
         const ulonglong2* recB = p.recB + b * p.Nt;
-        const float xs = (tid < UM_TS) ? x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt) : 0.f;
+        const float xs = (tid < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
         float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
         auto prefetch = [&](int ti) {
             const int64_t j = j_begin + (int64_t)ti * UM_TS + tid;

@@ -29,6 +29,7 @@ struct FinishParams {
     int nsplit, nparts;
     double cc_fix;                     // added to sum(CC - n/2): 0.5 when the pair-packed kernel padded an odd Nt
     int x_scaled;                      // 1: XC, XS were accumulated from X * x_scale() (tensor-core form)
+    const float* ws1;                  // generalised periodogram: [B][nsplit][4][Nf] of the unit-weight pass (planes 0, 1 = sum cos, sum sin); else NULL
 };
 
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
@@ -63,6 +64,28 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
             XS += (double)__ldg(w + p.Nf);
             CCh += (double)__ldg(w + 2 * p.Nf);
             CS += (double)__ldg(w + 3 * p.Nf);
+        }
+        if (p.ws1) {
+            // Generalised (floating-mean) periodogram of Zechmeister & Kuerster 2009 (named at PAPER.md:375), unit
+            // weights; the series is already mean-subtracted, so Y = 0 and YC = XC/N, YS = XS/N:
+            //   CCn = CC/N - (C/N)^2, SSn = SS/N - (S/N)^2, CSn = CS/N - C S/N^2, D = CCn SSn - CSn^2
+            //   P = (SSn XC^2 + CCn XS^2 - 2 CSn XC XS) / (2 var N D)        [same normalisation as eq. (1)]
+            double C1 = 0.0, S1 = 0.0;
+            const float* w1 = p.ws1 + b * p.nsplit * 4 * p.Nf;
+            for (int sp = 0; sp < p.nsplit; ++sp) {
+                C1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + k);
+                S1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + p.Nf + k);
+            }
+            const double cm = C1 / Nt, sm = S1 / Nt;
+            const double CCn = 0.5 + CCh / Nt - cm * cm, SSn = 0.5 - CCh / Nt - sm * sm, CSn = CS / Nt - cm * sm;
+            const double D = CCn * SSn - CSn * CSn;
+            double val = 0.0;
+            if (D > 1e-9) val = fmax(SSn * XC * XC + CCn * XS * XS - 2.0 * CSn * XC * XS, 0.0) / (Nt * D) * inv2var;   // singular fit (f -> 0): 0, reading G7
+            const float Pf = (float)val;
+            if (p.P) p.P[b * p.p_stride + k] = Pf;
+            const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+            best = (key > best) ? key : best;
+            continue;
         }
         const double A = 2.0 * CCh, Bv = 2.0 * CS;
         const double R = hypot(A, Bv);

@@ -70,4 +70,12 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
     if (threadIdx.x == 0) part_var[(int64_t)b * nb + blockIdx.x] = acc;
 }
 
+// Generalised periodogram: a second record array whose "measurement" is the unit weight 1, so that
+// the same accumulate kernels return sum cos and sum sin.  n = B * Nt records.
+__global__ void unit_records_kernel(const float4* __restrict__ recA, float4* __restrict__ recA1, int64_t n)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { float4 r = recA[i]; r.x = 1.f; recA1[i] = r; }
+}
+
 }  // namespace lsp

@@ -337,6 +337,62 @@ def test_host_entry_points(lsp):
 
 
 # ------------------------------------------------------------------ argument errors
+@pytest.mark.parametrize("rec,coarse", [(0, 0), (3, 0), (1, 0), (4, 0), (5, 128), (5, 32)])
+def test_generalised_periodogram(lsp, rec, coarse):
+    """lsp_periodogram_gls (floating-mean fit) against the oracle's 3-parameter least squares, on
+    gappy sampling with a large offset where it differs visibly from eq. (1); every form of steps 3-5."""
+    import torch
+    pkg, h = lsp
+    rng = np.random.default_rng(2024)
+    Nt, Nf = 3001, 4099
+    t = np.sort(np.concatenate([rng.uniform(0, 9, Nt // 2), rng.uniform(31, 40, Nt - Nt // 2)]))
+    x = (7.0 + 0.6 * np.sin(2 * np.pi * 0.0431 * t + 0.4) + 0.5 * np.sin(2 * np.pi * 1.7 * t)
+         + rng.standard_normal(Nt)).astype(np.float32)
+    f_min, df = 1.0 / 40.0, (3.0 - 1.0 / 40.0) / (Nf - 1)
+    ref = oracle.periodogram_gls(t, x, f_min, df, Nf)
+    ls = oracle.periodogram(t, x, f_min, df, Nf)
+    assert np.max(np.abs(ref - ls)) > 1e-2 * ref.max()      # the two periodograms really differ on this input
+    for key, val in ((pkg.PARAM_RECURRENCE, rec), (pkg.PARAM_COARSE, coarse)):
+        h.set_param(key, val)
+    try:
+        P = h.periodogram(torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), f_min, df, Nf, gls=True)
+        torch.cuda.synchronize()
+        plan = h.last_plan()
+    finally:
+        h.set_param(pkg.PARAM_RECURRENCE, 0); h.set_param(pkg.PARAM_COARSE, 0)
+    P = P.cpu().numpy()
+    _check(P, ref, "gls rec=%d" % rec)
+    assert _same_peak(P, ref)
+    if rec:
+        assert plan["recurrence"] == rec
+
+
+def test_generalised_periodogram_batched_and_reduction(lsp):
+    """Batched GLS with per-series peaks; and on even sampling at Fourier frequencies GLS == eq. (1) (pin GP4) on the GPU."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=9, Nt=800, Nf=1500, seed=515)
+    x = (w.x + 3.0).astype(np.float32)
+    P, pi, pv = h.periodogram_batched(torch.from_numpy(w.t).cuda(), torch.from_numpy(x).cuda(), w.f_min, w.df, w.Nf, gls=True)
+    torch.cuda.synchronize()
+    P = P.cpu().numpy()
+    for b in range(w.B):
+        ref = oracle.periodogram_gls(w.t[b], x[b], w.f_min, w.df, w.Nf)
+        _check(P[b], ref, "gls series %d" % b)
+        assert _same_peak(P[b], ref)
+        assert int(pi[b]) == int(np.argmax(P[b])) and float(pv[b]) == float(P[b].max())
+    N, dt = 1024, 0.25
+    t = dt * np.arange(N)
+    xe = np.random.default_rng(3).standard_normal(N).astype(np.float32)
+    dfe = 1.0 / (N * dt)
+    td, xd = torch.from_numpy(t).cuda(), torch.from_numpy(xe).cuda()
+    Pg = h.periodogram(td, xd, dfe, dfe, N // 2 - 1, gls=True).cpu().numpy()
+    P1 = h.periodogram(td, xd, dfe, dfe, N // 2 - 1).cpu().numpy()
+    assert np.max(np.abs(Pg - P1)) <= 2e-5 * P1.max()
+    with pytest.raises(pkg.LspError):
+        h.periodogram(td[:3].contiguous(), xd[:3].contiguous(), dfe, dfe, 4, gls=True)
+
+
 def test_false_alarm_probability(lsp):
     """Eq. (3) epilogue against the oracle's plain formula on the GPU's own P (C1), on per-series peaks of a noise
     batch, and on hand-made values spanning Q = 1 ... 1e-30."""

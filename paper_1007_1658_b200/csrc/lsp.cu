@@ -25,6 +25,7 @@ namespace {
 
 struct Plan {
     int K = 0, T = 0, nsplit = 0, rec = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0, L = 0;
+    int mma_slots = 4;          // tensor-core forms: fp16-rate MMA slots issued per k-step of 8 samples (4 = hi+lo in fp16, 3 = 8-bit correction)
     int64_t split_len = 0, part_chunk = 0;
     const char* kernel_name = "";
 };
@@ -38,7 +39,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0, opt_corr = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     uint64_t timed_calls = 0;
     // workspace
@@ -168,7 +169,13 @@ int run_device(lsp_ctx* h,
     const bool use_tab = umma && !umma_small && h->opt_btable != 1 &&
                          (h->opt_btable == 2 || (pl.nfb >= 3 && tab_bytes <= ((size_t)12 << 30)));
     const size_t o_tab = off;  if (use_tab) off = align_up(off + tab_bytes, 256);
-    if (use_tab) { pl.kernel_name = "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>"; pl.launches = 5; }
+    const bool corr8 = use_tab && h->opt_corr != 1;       // correction products as one 8-bit MMA (default) or two fp16 MMAs
+    if (use_tab) {
+        pl.kernel_name = corr8 ? "accum_umma_tab_kernel<tcgen05.m128n256.f16+e5m2corr,B-table>"
+                               : "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>";
+        pl.launches = 5;
+        pl.mma_slots = corr8 ? 3 : 4;
+    }
     if (gls) pl.launches += 2;                            // unit records + second accumulate pass
     int rc = ensure(h, &h->buf, &h->buf_bytes, off);
     if (rc != LSP_OK) return rc;
@@ -209,7 +216,8 @@ int run_device(lsp_ctx* h,
     if (use_tab) {
         if (tab_groups > 2147483647LL) return LSP_EINVAL;
         dim3 gtab((unsigned)tab_groups, (unsigned)tab_series);
-        umma_btable_kernel<<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
+        if (corr8) umma_btable_kernel<true><<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
+        else umma_btable_kernel<false><<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
         LSP_CUDA(h, cudaGetLastError());
     }
 
@@ -241,8 +249,13 @@ int run_device(lsp_ctx* h,
             UmmaTabParams tp;
             tp.u = up; tp.btable = btable; tp.ngroups = tab_groups;
             tp.table_stride = (tab_series == 1) ? 0 : (int64_t)tab_groups * UT_GROUP_BYTES;
-            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
-            accum_umma_tab_kernel<<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
+            if (corr8) {
+                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
+                accum_umma_tab_kernel<true><<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
+            } else {
+                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
+                accum_umma_tab_kernel<false><<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
+            }
         } else {
             LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UM_SMEM));
             accum_umma_kernel<<<(unsigned)units, UM_THREADS, UM_SMEM, st>>>(up);
@@ -341,6 +354,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
         case LSP_PARAM_BTABLE:     if (value > 2) return LSP_EINVAL; h->opt_btable = value; break;
         case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
+        case LSP_PARAM_CORR:       if (value > 2) return LSP_EINVAL; h->opt_corr = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -358,6 +372,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_TIMING:     *value = h->opt_timing; break;
         case LSP_PARAM_BTABLE:     *value = h->opt_btable; break;
         case LSP_PARAM_COARSE:     *value = h->opt_coarse; break;
+        case LSP_PARAM_CORR:       *value = h->opt_corr; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

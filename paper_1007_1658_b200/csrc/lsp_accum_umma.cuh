@@ -31,6 +31,7 @@
 #include "lsp_accum.cuh"
 #include "lsp_accum_mma.cuh"
 #include <cuda_fp16.h>
+#include <cuda_fp8.h>
 
 namespace lsp {
 
@@ -98,6 +99,13 @@ __device__ __forceinline__ void tc_mma_f16(uint32_t d_tmem, uint64_t a_desc, uin
                  "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                  :: "r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// Same with kind::f8f6f4 (8-bit float operands, K = 32 per instruction, twice the fp16 rate, fp32 accumulate).
+__device__ __forceinline__ void tc_mma_f8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+                 :: "r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
 // Shared-memory matrix descriptor, K-major, no swizzle: core matrix = 8 rows x 16 bytes, rows 16 B apart;
 // LBO = byte distance between the two 16-byte K chunks, SBO = byte distance between 8-row groups.
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo)
@@ -106,6 +114,19 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint
 }
 // Instruction descriptor: D = F32 (bits 4-5 = 1), A = B = F16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
 constexpr uint32_t UM_IDESC = (1u << 4) | ((uint32_t)(2 * UM_L >> 3) << 17) | ((uint32_t)(UM_H >> 4) << 24);
+// kind::f8f6f4: A format at bit 7, B format at bit 10; 1 = E5M2 (the upper byte of an fp16: same exponent range).
+constexpr uint32_t UM_IDESC_F8 = UM_IDESC | (1u << 7) | (1u << 10);
+
+// Two fp32 (or one packed fp16 pair) -> two e5m2 bytes in the low 16 bits, round to nearest, first value in the low byte.
+__device__ __forceinline__ unsigned pack_e5m2(float a, float b)
+{
+    return (unsigned)__nv_cvt_float2_to_fp8x2(make_float2(a, b), __NV_SATFINITE, __NV_E5M2);
+}
+__device__ __forceinline__ unsigned pack_e5m2_h2(unsigned h2)
+{
+    __half2_raw r; r.x = (unsigned short)(h2 & 0xFFFFu); r.y = (unsigned short)(h2 >> 16);
+    return (unsigned)__nv_cvt_halfraw2_to_fp8x2(r, __NV_SATFINITE, __NV_E5M2);
+}
 
 // 32 lanes x 32 consecutive columns of fp32 accumulators -> 32 registers per thread (lane = TMEM lane).
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32])
@@ -131,10 +152,15 @@ __device__ __forceinline__ void sts128(uint32_t saddr, unsigned a, unsigned b, u
 // ------------------------------------------------------------------ step 3: operand generation
 // One A item: row h, K chunk `c` (4 samples) of the k-step whose records start at rec[s0].  Writes the
 // 16-byte row chunks of A_hi, A_lo (X e^{ia} as fp16 hi + lo) and A_V (e^{2ia}/2).
-template <bool TAIL>
+//
+// F8 = true (the "8-bit correction" form): the two first-order correction products A_lo B_hi + A_hi B_lo only need
+// ~3 significant bits each (they are 2^-12 of the main product), so they are issued as ONE kind::f8f6f4 MMA of
+// K = 32: plane 1 then holds, per 16-byte chunk, [e5m2(A_lo) of 4 samples | e5m2(A_hi) of 4 samples] and the matching
+// B plane [e5m2(B_hi) | e5m2(B_lo)].  Residual error ~2^-3 * 2^-12 per product, random sign.
+template <bool TAIL, bool F8>
 __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int nvalid)
 {
-    unsigned hi[4], lo[4], vv[4];
+    unsigned hi[4], lo[4], vv[4], h8[4];
     #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const float4 r = rec[s0 + i];                                   // {X / sigma, pA32, v32, w32}: broadcast read
@@ -147,20 +173,23 @@ __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, 
         const float2 hf = unpack_h2(hi[i]);
         float lc, ls;
         unpack2(fma2(pack2(hf.x, hf.y), pack2(-1.f, -1.f), pack2(xc, xs)), lc, ls);
-        lo[i] = pack_h2(lc, ls);
+        if (F8) { lo[i] = pack_e5m2(lc, ls); h8[i] = pack_e5m2_h2(hi[i]); }
+        else lo[i] = pack_h2(lc, ls);
         float v0, v1;
         unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
         vv[i] = pack_h2(v0, v1);
         if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
     sts128(sA, hi[0], hi[1], hi[2], hi[3]);
-    sts128(sA + UM_A_BYTES, lo[0], lo[1], lo[2], lo[3]);
+    if (F8) sts128(sA + UM_A_BYTES, lo[0] | (lo[1] << 16), lo[2] | (lo[3] << 16), h8[0] | (h8[1] << 16), h8[2] | (h8[3] << 16));
+    else sts128(sA + UM_A_BYTES, lo[0], lo[1], lo[2], lo[3]);
     sts128(sA + 2 * UM_A_BYTES, vv[0], vv[1], vv[2], vv[3]);
 }
+template <bool F8 = false>
 __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int64_t left)
 {
-    if (left >= 4) um_gen_a<false>(rec, s0, h, sA, 4);                  // `left` is warp-uniform
-    else um_gen_a<true>(rec, s0, h, sA, (int)max((int64_t)0, left));
+    if (left >= 4) um_gen_a<false, F8>(rec, s0, h, sA, 4);              // `left` is warp-uniform
+    else um_gen_a<true, F8>(rec, s0, h, sA, (int)max((int64_t)0, left));
 }
 
 // One B item: coarse index l, K chunk `c`: rows (l,Re) and (l,Im) of B_hi, B_lo (e^{ib}) and B_V (e^{2ib}).

@@ -40,9 +40,10 @@ def _same_peak(P_gpu, P_ref):
 
 def _run_single(h, w, **params):
     import torch
-    from paper_1007_1658_b200 import PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE, PARAM_COARSE
+    from paper_1007_1658_b200 import (PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE,
+                                      PARAM_COARSE, PARAM_CORR)
     keys = {"K": PARAM_K, "threads": PARAM_THREADS, "nsplit": PARAM_NSPLIT,
-            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE, "coarse": PARAM_COARSE}
+            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE, "coarse": PARAM_COARSE, "corr": PARAM_CORR}
     for k, v in keys.items():
         h.set_param(v, params.get(k, 0))
     try:
@@ -117,13 +118,15 @@ def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit, rec):
 @pytest.mark.parametrize("Nt,Nf,nsplit,flush", [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 50011, 0, 0), (1025, 8193, 2, 0),
                                                 (127, 40, 0, 0), (130, 16385, 1, 0), (4099, 3001, 1, 16), (4099, 3001, 2, 1000),
                                                 (8, 100, 1, 0), (137, 33000, 1, 0)])
-def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush):
+@pytest.mark.parametrize("corr", [1, 2])
+def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush, corr):
     """rec = 5 with the coarse operand streamed from the pre-computed table (cp.async.bulk), two k-steps per stage:
-    odd k-step counts, ragged tiles and blocks, several drains."""
+    odd k-step counts, ragged tiles and blocks, several drains.  corr = 1: the hi*lo correction products as two fp16
+    MMAs; corr = 2 (the default): as one e5m2 MMA of K = 32."""
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=6000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2, coarse=128)
+    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2, coarse=128, corr=corr)
     if Nt >= 100:
         _check(P, ref, "umma-tab Nt=%d Nf=%d" % (Nt, Nf))
         assert int(np.argmax(P)) == oracle.argmax(ref)
@@ -131,6 +134,22 @@ def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush):
         assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
     plan = h.last_plan()
     assert plan["recurrence"] == 5 and "B-table" in plan["kernel"] and plan["launches"] == 5
+    assert ("e5m2corr" in plan["kernel"]) == (corr == 2)
+
+
+@pytest.mark.parametrize("corr", [1, 2])
+def test_umma_table_form_noise_and_scale(lsp, corr):
+    """The table form on pure noise (max P ~ 8: the tightest absolute tolerance) and badly scaled x.  With the 8-bit
+    correction MMA the residual is ~2^-15 per product, measured 1.4e-5 ... 3.5e-5 of max P here."""
+    pkg, h = lsp
+    wb = workloads.c4(B=4, Nt=3000, Nf=9000, seed=4242)
+    for b, scale in enumerate((1.0, 1e-6, 1e6, 1.0)):
+        x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
+        w = workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
+        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+        P = _run_single(h, w, rec=5, btable=2, coarse=128, corr=corr)
+        _check(P, ref, "umma-tab corr=%d noise scale=%g" % (corr, scale))
+        assert _same_peak(P, ref)
 
 
 @pytest.mark.parametrize("coarse", [16, 32, 64])

@@ -41,9 +41,9 @@ def _same_peak(P_gpu, P_ref):
 def _run_single(h, w, **params):
     import torch
     from paper_1007_1658_b200 import (PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE,
-                                      PARAM_COARSE, PARAM_CORR)
+                                      PARAM_COARSE, PARAM_CORR, PARAM_PAIR)
     keys = {"K": PARAM_K, "threads": PARAM_THREADS, "nsplit": PARAM_NSPLIT,
-            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE, "coarse": PARAM_COARSE, "corr": PARAM_CORR}
+            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE, "coarse": PARAM_COARSE, "corr": PARAM_CORR, "pair": PARAM_PAIR}
     for k, v in keys.items():
         h.set_param(v, params.get(k, 0))
     try:
@@ -118,15 +118,18 @@ def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit, rec):
 @pytest.mark.parametrize("Nt,Nf,nsplit,flush", [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 50011, 0, 0), (1025, 8193, 2, 0),
                                                 (127, 40, 0, 0), (130, 16385, 1, 0), (4099, 3001, 1, 16), (4099, 3001, 2, 1000),
                                                 (8, 100, 1, 0), (137, 33000, 1, 0)])
-@pytest.mark.parametrize("corr", [1, 2])
+@pytest.mark.parametrize("corr", [1, 2, 3])
 def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush, corr):
     """rec = 5 with the coarse operand streamed from the pre-computed table (cp.async.bulk), two k-steps per stage:
     odd k-step counts, ragged tiles and blocks, several drains.  corr = 1: the hi*lo correction products as two fp16
-    MMAs; corr = 2 (the default): as one e5m2 MMA of K = 32."""
+    MMAs; corr = 2: as one e5m2 MMA of K = 32; corr = 3 (the default form): the same on CTA pairs (cta_group::2, M = 256,
+    each CTA holding half of the coarse operand; odd block counts get one masked block)."""
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=6000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2, coarse=128, corr=corr)
+    pair = 2 if corr == 3 else 1
+    corr = min(corr, 2)
+    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2, coarse=128, corr=corr, pair=pair)
     if Nt >= 100:
         _check(P, ref, "umma-tab Nt=%d Nf=%d" % (Nt, Nf))
         assert int(np.argmax(P)) == oracle.argmax(ref)
@@ -135,9 +138,10 @@ def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush, corr):
     plan = h.last_plan()
     assert plan["recurrence"] == 5 and "B-table" in plan["kernel"] and plan["launches"] == 5
     assert ("e5m2corr" in plan["kernel"]) == (corr == 2)
+    assert ("cta_group2" in plan["kernel"]) == (pair == 2)
 
 
-@pytest.mark.parametrize("corr", [1, 2])
+@pytest.mark.parametrize("corr", [1, 2, 3])
 def test_umma_table_form_noise_and_scale(lsp, corr):
     """The table form on pure noise (max P ~ 8: the tightest absolute tolerance) and badly scaled x.  With the 8-bit
     correction MMA the residual is ~2^-15 per product, measured 1.4e-5 ... 3.5e-5 of max P here."""
@@ -147,7 +151,7 @@ def test_umma_table_form_noise_and_scale(lsp, corr):
         x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
         w = workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
         ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-        P = _run_single(h, w, rec=5, btable=2, coarse=128, corr=corr)
+        P = _run_single(h, w, rec=5, btable=2, coarse=128, corr=min(corr, 2), pair=2 if corr == 3 else 1)
         _check(P, ref, "umma-tab corr=%d noise scale=%g" % (corr, scale))
         assert _same_peak(P, ref)
 
@@ -320,6 +324,31 @@ def test_batched_shared_times(lsp):
     for b in range(w.B):
         _check(P[b].cpu().numpy(), Pref[b], "shared-t series %d" % b)
     assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
+
+
+@pytest.mark.parametrize("shared", [False, True])
+@pytest.mark.parametrize("pair", [1, 2])
+def test_batched_table_form(lsp, shared, pair):
+    """The tcgen05 table form on a batch: one coarse-operand table per series, or ONE table for all when the
+    times are shared (t_stride = 0); 3 frequency blocks (pairs: padded to 4, the last one masked)."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=3, Nt=1500, Nf=40000, seed=31337)
+    tt = w.t[0].copy() if shared else w.t
+    Pref, iref, _ = oracle.periodogram_batched(tt, w.x, w.f_min, w.df, w.Nf)
+    keys = {pkg.PARAM_RECURRENCE: 5, pkg.PARAM_BTABLE: 2, pkg.PARAM_COARSE: 128, pkg.PARAM_PAIR: pair}
+    for k, v in keys.items():
+        h.set_param(k, v)
+    try:
+        P, pi, pv = h.periodogram_batched(torch.from_numpy(tt).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+        assert ("cta_group2" in h.last_plan()["kernel"]) == (pair == 2)
+    finally:
+        for k in keys:
+            h.set_param(k, 0)
+    for b in range(w.B):
+        _check(P[b].cpu().numpy(), Pref[b], "table form, series %d" % b)
+        assert _same_peak(P[b].cpu().numpy(), Pref[b])
 
 
 def test_batch_of_one_equals_single(lsp):

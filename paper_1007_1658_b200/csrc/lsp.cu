@@ -10,6 +10,7 @@
 #include "lsp_accum_umma.cuh"
 #include "lsp_accum_umma_tab.cuh"
 #include "lsp_accum_umma_pair.cuh"
+#include "lsp_accum_umma_pair2.cuh"
 #include "lsp_accum_umma_small.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_fap.cuh"
@@ -172,11 +173,13 @@ int run_device(lsp_ctx* h,
     const size_t o_tab = off;  if (use_tab) off = align_up(off + tab_bytes, 256);
     const bool corr8 = use_tab && h->opt_corr != 1;       // correction products as one 8-bit MMA (default) or two fp16 MMAs
     const bool pair = corr8 && h->opt_pair != 1;          // CTA pairs (cta_group::2) share one B tile: lsp_accum_umma_pair.cuh
+    const bool pair2 = pair && h->opt_pair != 2;          // ... and share the GENERATED operand instead: lsp_accum_umma_pair2.cuh (default)
     if (pair) pl.nfb = (pl.nfb + 1) & ~1;                 // a pair = two adjacent frequency blocks; an odd count gets one masked block
     if (use_tab) {
         pl.kernel_name = corr8 ? "accum_umma_tab_kernel<tcgen05.m128n256.f16+e5m2corr,B-table>"
                                : "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>";
-        if (pair) pl.kernel_name = "accum_umma_pair_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,B-table>";
+        if (pair) pl.kernel_name = pair2 ? "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>"
+                                         : "accum_umma_pair_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,B-table>";
         pl.launches = 5;
         pl.mma_slots = corr8 ? 3 : 4;
     }
@@ -220,7 +223,8 @@ int run_device(lsp_ctx* h,
     if (use_tab) {
         if (tab_groups > 2147483647LL) return LSP_EINVAL;
         dim3 gtab((unsigned)tab_groups, (unsigned)tab_series);
-        if (pair) umma_btable_pair_kernel<<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, (int64_t)tab_groups * UP_GROUP_BYTES, (int64_t)tab_groups * UT_GROUP_BYTES);
+        if (pair2) umma_ftable_pair_kernel<<<gtab, 512, 0, st>>>(recB, Nt, Nt, btable, (int64_t)tab_groups * UP_GROUP_BYTES, (int64_t)tab_groups * UT_GROUP_BYTES);
+        else if (pair) umma_btable_pair_kernel<<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, (int64_t)tab_groups * UP_GROUP_BYTES, (int64_t)tab_groups * UT_GROUP_BYTES);
         else if (corr8) umma_btable_kernel<true><<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
         else umma_btable_kernel<false><<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
         LSP_CUDA(h, cudaGetLastError());
@@ -259,13 +263,15 @@ int run_device(lsp_ctx* h,
                 pp.u = up; pp.btable = btable; pp.half_stride = (int64_t)tab_groups * UP_GROUP_BYTES;
                 pp.table_stride = tp.table_stride;
                 LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UP_SMEM));
+                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)U2_SMEM));
                 cudaLaunchConfig_t cfg = {};
-                cfg.gridDim = dim3((unsigned)units); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UP_SMEM; cfg.stream = st;
+                cfg.gridDim = dim3((unsigned)units); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = pair2 ? U2_SMEM : UP_SMEM; cfg.stream = st;
                 cudaLaunchAttribute at[1];
                 at[0].id = cudaLaunchAttributeClusterDimension;
                 at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                 cfg.attrs = at; cfg.numAttrs = 1;
-                LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair_kernel, pp));
+                if (pair2) LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair2_kernel, pp));
+                else LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair_kernel, pp));
             } else if (corr8) {
                 LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
                 accum_umma_tab_kernel<true><<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
@@ -372,7 +378,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_BTABLE:     if (value > 2) return LSP_EINVAL; h->opt_btable = value; break;
         case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
         case LSP_PARAM_CORR:       if (value > 2) return LSP_EINVAL; h->opt_corr = value; break;
-        case LSP_PARAM_PAIR:       if (value > 2) return LSP_EINVAL; h->opt_pair = value; break;
+        case LSP_PARAM_PAIR:       if (value > 3) return LSP_EINVAL; h->opt_pair = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

@@ -1,0 +1,299 @@
+// lsp_accum_umma_pair2.cuh -- CTA-pair tcgen05 form of steps 3-5 with the GENERATED operand shared by the pair.
+//
+// In lsp_accum_umma_pair.cuh the pair shares the streamed (table) operand and each CTA still generates a full
+// 128-row fine operand: 128 MUFU sin/cos pairs per sample per CTA, and the 16 producer warps are as busy as the
+// tensor pipe (measured: generation alone = MMAs alone; tensor pipe 60 % active).  Here the roles are swapped:
+//
+//     k = kb + 256 h + l,   l < 256 fine (table, M side),   h < 128 coarse (generated, N side),   kb = 32,768 * pair
+//     theta_jk = [2 pi frac(u_j + (kb + 256 h) v_j)]  +  [2 pi frac(l v_j)]  =  a_jh + b_jl          (exact 64-bit turns, G3)
+//     W[l,h] = sum_j e^{i b_jl} (X_j e^{i a_jh}),    V[l,h] = sum_j e^{2i b_jl} (e^{2i a_jh} / 2)     (eq. (8))
+//
+// One tcgen05.mma.cta_group::2 of M = 256, N = 256: the M rows are the fine index l -- CTA r streams ITS 128 rows
+// (c_l, s_l) of the table (12 KB per k-step, as before) and accumulates them in ITS TMEM -- and the N columns
+// (h,Re), (h,Im) are the generated operand, of which each CTA makes only HALF (64 coarse values h, both parts):
+// 64 sin/cos pairs per sample per CTA instead of 128.  The (h,Im) row is a permutation of the (h,Re) row
+// ((xc, -xs) -> (xs, xc)): PRMT / LOP3 on the packed words, no extra arithmetic.  A stage-step (two k-steps) is
+// 256 thread-tasks, so the 16 producer warps work as two groups of 8 on alternate stage-steps: per stage-step the
+// producers issue ~45 % fewer instructions than in the first pair form.
+//
+// TMEM (per CTA): lane = l - 128 r;  column n = 128 r' + 64 part + h',  h = 64 r' + h'  (r' = CTA that generated it);
+// D_W in columns 0..255, D_V in 256..511.  For a fixed column the 32 lanes of a warp are 32 consecutive
+// frequencies: the drain into `ws` is coalesced.  Operand precision, the e5m2 correction MMA, the periodic drain of
+// D_W and all barriers are as in lsp_accum_umma_pair.cuh (FULL count = 8 warps + 1 per stage).
+#pragma once
+#include "lsp_accum_umma_pair.cuh"
+
+namespace lsp {
+
+constexpr int U2_FPP = 256 * UM_H;                                // frequencies per CTA pair
+constexpr int U2_HC = 64;                                         // coarse values generated per CTA
+constexpr int U2_GROUP_WARPS = UM_GEN_WARPS / 2;                  // producer warps per group
+constexpr int U2_REC_BYTES = 2 * 2 * UM_TS * 16;                  // [group][buffer][128 samples] records
+constexpr size_t U2_SMEM = (size_t)UP_STAGES * UP_STAGE_BYTES + U2_REC_BYTES + 256;
+
+// ------------------------------------------------------------------ pre-pass: the fine-operand table
+// table[r][g][plane][chunk][l & 127][16 bytes], r = l >> 7: plane 0 = (c, s) fp16, 1 = [e5m2(c_h, s_h) | e5m2(c - c_h, s - s_h)],
+// 2 = (cos 2b, sin 2b) fp16; b = 2 pi frac(l v_j).  grid (ngroups, series), 512 threads = 2 K-chunks x 256 fine indices.
+__global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t rec_stride,
+                                                               unsigned char* __restrict__ table, int64_t half_stride, int64_t table_stride)
+{
+    const int64_t g = blockIdx.x;
+    const unsigned l = threadIdx.x & 255u, chunk = threadIdx.x >> 8;
+    const ulonglong2* rb = recB + (int64_t)blockIdx.y * rec_stride;
+    unsigned hh[4], h8[4], l8[4], vv[4];
+    #pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int64_t j = g * UM_KS + chunk * 4 + i;
+        const u64 v = (j < Nt) ? __ldg(&rb[j].y) : 0ull;                // beyond Nt: e^{i0}; the generated operand is zero there
+        const unsigned v32 = (unsigned)((v + 0x80000000ull) >> 32);
+        float c, s;
+        sincos_phase32(l * v32, c, s);
+        hh[i] = pack_h2(c, s);
+        const float2 hf = unpack_h2(hh[i]);
+        h8[i] = pack_e5m2_h2(hh[i]);
+        l8[i] = pack_e5m2(c - hf.x, s - hf.y);
+        const float cc = c + c;
+        vv[i] = pack_h2(fmaf(cc, c, -1.f), cc * s);
+    }
+    unsigned char* base = table + (int64_t)blockIdx.y * table_stride + (int64_t)(l >> 7) * half_stride + g * (int64_t)UP_GROUP_BYTES;
+    uint4* o = reinterpret_cast<uint4*>(base);
+    constexpr int PLANE = UP_B_HALF / 16;
+    const int row = (int)(chunk * (PLANE / 2) + (l & 127u));
+    o[row] = make_uint4(hh[0], hh[1], hh[2], hh[3]);
+    o[PLANE + row] = make_uint4(h8[0] | (h8[1] << 16), h8[2] | (h8[3] << 16), l8[0] | (l8[1] << 16), l8[2] | (l8[3] << 16));
+    o[2 * PLANE + row] = make_uint4(vv[0], vv[1], vv[2], vv[3]);
+}
+
+// ------------------------------------------------------------------ step 3: the generated (coarse) operand
+// One task: coarse value h, 4 samples starting at rec[s0]: writes the 16-byte chunks of rows (h,Re) and (h,Im)
+// (64 rows = 1,024 bytes apart) of the planes G_hi, G_8 = [e5m2(G_lo) | e5m2(G_hi)], G_V.  sG = address of row (h,Re).
+__device__ __forceinline__ unsigned swap_halves(unsigned x) { return __byte_perm(x, 0u, 0x1032); }
+__device__ __forceinline__ unsigned swap_bytes16(unsigned x) { return __byte_perm(x, 0u, 0x2301); }
+
+template <bool TAIL>
+__device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, uint32_t sG, int nvalid)
+{
+    unsigned hi[4], lo[4], h8[4], vv[4];
+    #pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float4 r = rec[s0 + i];                                   // {X / sigma, pA32, w32, -}: broadcast read
+        float c, s;
+        sincos_phase32(__float_as_uint(r.y) + h * __float_as_uint(r.z), c, s);
+        const u64 cs = pack2(c, s);
+        float xc, xs;
+        unpack2(mul2(pack2(r.x, r.x), cs), xc, xs);
+        hi[i] = pack_h2(xc, xs);
+        const float2 hf = unpack_h2(hi[i]);
+        float lc, ls;
+        unpack2(fma2(pack2(hf.x, hf.y), pack2(-1.f, -1.f), pack2(xc, xs)), lc, ls);
+        lo[i] = pack_e5m2(lc, ls);
+        h8[i] = pack_e5m2_h2(hi[i]);
+        float v0, v1;
+        unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
+        vv[i] = pack_h2(v0, v1);
+        if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
+    }
+    const unsigned q0 = lo[0] | (lo[1] << 16), q1 = lo[2] | (lo[3] << 16), q2 = h8[0] | (h8[1] << 16), q3 = h8[2] | (h8[3] << 16);
+    constexpr uint32_t IM = U2_HC * 16;                                 // row (h,Im) is 64 rows below row (h,Re)
+    // row (h,Re) = (xc, -xs): flip the sign of the second component;  row (h,Im) = (xs, xc): swap the components
+    sts128(sG, hi[0] ^ 0x80000000u, hi[1] ^ 0x80000000u, hi[2] ^ 0x80000000u, hi[3] ^ 0x80000000u);
+    sts128(sG + IM, swap_halves(hi[0]), swap_halves(hi[1]), swap_halves(hi[2]), swap_halves(hi[3]));
+    sts128(sG + UM_A_BYTES, q0 ^ 0x80008000u, q1 ^ 0x80008000u, q2 ^ 0x80008000u, q3 ^ 0x80008000u);
+    sts128(sG + UM_A_BYTES + IM, swap_bytes16(q0), swap_bytes16(q1), swap_bytes16(q2), swap_bytes16(q3));
+    sts128(sG + 2 * UM_A_BYTES, vv[0] ^ 0x80000000u, vv[1] ^ 0x80000000u, vv[2] ^ 0x80000000u, vv[3] ^ 0x80000000u);
+    sts128(sG + 2 * UM_A_BYTES + IM, swap_halves(vv[0]), swap_halves(vv[1]), swap_halves(vv[2]), swap_halves(vv[3]));
+}
+
+// ------------------------------------------------------------------ step 5: drain 64 accumulator columns into ws
+// Thread = TMEM lane = fine index; its 64 registers are 64 consecutive coarse values h (frequency stride 256).
+__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first)
+{
+    #pragma unroll 1
+    for (int half = 0; half < 2; ++half) {
+        float v[32];
+        tmem_ld32(taddr + 32u * half, v);
+        const int64_t kh = k0 + (int64_t)half * 32 * 256;
+        if (!first) {
+            #pragma unroll
+            for (int i = 0; i < 32; ++i) { const int64_t k = kh + (int64_t)i * 256; if (k < Nf) v[i] += dst[k]; }
+        }
+        #pragma unroll
+        for (int i = 0; i < 32; ++i) { const int64_t k = kh + (int64_t)i * 256; if (k < Nf) dst[k] = v[i]; }
+    }
+}
+
+// ------------------------------------------------------------------ the kernel
+// grid.x = B * nsplit * (2 * npairs) (CTA of the pair fastest, then the pair), clusters of 2, UM_THREADS threads,
+// U2_SMEM bytes of dynamic shared memory, one CTA per SM.  q.u.nfb = 2 * npairs, npairs = ceil(Nf / 32,768).
+__global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const UmmaPairParams q)
+{
+    const UmmaParams& p = q.u;
+    extern __shared__ __align__(128) unsigned char um_smem[];
+    float4* rec_all = reinterpret_cast<float4*>(um_smem + UP_STAGES * UP_STAGE_BYTES);            // [group][2][UM_TS] {X/sigma, pA32, w32, -}
+    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + UP_STAGES * UP_STAGE_BYTES + U2_REC_BYTES);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * UP_STAGES + 2);
+
+    const unsigned tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
+    const uint32_t rank = cluster_ctarank();
+    int64_t unit = blockIdx.x;
+    const int fb = (int)(unit % p.nfb); unit /= p.nfb;
+    const int sp = (int)(unit % p.nsplit);
+    const int64_t b = unit / p.nsplit;
+    const int64_t kb = (int64_t)(fb >> 1) * U2_FPP;
+    const int64_t j_begin = (int64_t)sp * p.split_len;
+    const int64_t j_end = min(p.Nt, j_begin + p.split_len);
+    const int n_samp = (int)(j_end - j_begin);                          // split_len < 2^31
+    const int nks = (n_samp + UM_KS - 1) / UM_KS;
+    const int nst = (nks + UT_KPS - 1) / UT_KPS;                        // stage-steps (two k-steps each)
+    const int flush_st = max(2, (p.flush_ksteps / UT_KPS) & ~1);        // even: both producer groups see the same windows
+    const int nwin = (nst + flush_st - 1) / flush_st;
+
+    const uint32_t s_stage = smem_u32(um_smem), s_bar = smem_u32(bars);
+    const uint32_t bar_accf = s_bar + 8u * (3 * UP_STAGES), bar_acce = bar_accf + 8u;
+#define U2_FULL(s) (s_bar + 8u * (unsigned)(s))
+#define U2_EMPTY(s) (s_bar + 8u * (unsigned)(UP_STAGES + (s)))
+#define U2_PEER(s) (s_bar + 8u * (unsigned)(2 * UP_STAGES + (s)))
+
+    if (tid == 0) {
+        for (int s = 0; s < UP_STAGES; ++s) { mbar_init(U2_FULL(s), U2_GROUP_WARPS + 1); mbar_init(U2_EMPTY(s), 1); mbar_init(U2_PEER(s), 1); }
+        mbar_init(bar_accf, 1);
+        mbar_init(bar_acce, 2 * UM_GEN_WARPS);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster_sync_all();
+    if (w == UM_GEN_WARPS) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"(smem_u32(tmem_slot)), "r"((uint32_t)UM_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
+    cluster_sync_all();
+
+    if (w < UM_GEN_WARPS) {
+        // ===================== producers: generated operand (step 3), TMA of this CTA's table rows, drain (step 5) =====================
+        const unsigned grp = w >> 3, tg = tid & 255u;                   // group `grp` owns the stage-steps it = grp (mod 2)
+        float4* rec = rec_all + grp * (2 * UM_TS);
+        const float4* recA = p.recA + b * p.Nt;
+        const ulonglong2* recB = p.recB + b * p.Nt;
+        const unsigned char* tab = q.btable + b * q.table_stride + (int64_t)rank * q.half_stride + (j_begin / UM_KS) * (int64_t)UP_GROUP_BYTES;
+        const float xs = (tg < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
+        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
+        auto prefetch = [&](int ti) {
+            const int64_t j = j_begin + (int64_t)ti * UM_TS + tg;
+            pre_ok = (tg < UM_TS) && (j < j_end);
+            if (pre_ok) { pre_x = __ldg(&recA[j].x); const ulonglong2 r = __ldg(recB + j); pre_u = r.x; pre_v = r.y; }
+        };
+        prefetch(0);
+        const unsigned hl = tg & 63u, h = (unsigned)U2_HC * rank + hl;   // coarse value: local row, global index
+        const int chunk = (int)((tg >> 6) & 1u), kk = (int)(tg >> 7);    // 4 samples `chunk` of k-step `kk` of the stage
+        const uint32_t g_off = (uint32_t)kk * (3 * UM_A_BYTES) + (uint32_t)chunk * (UM_A_BYTES / 2) + hl * 16u;
+        const int samp_off = kk * UM_KS + chunk * 4;                     // first sample of the task within the stage-step
+        // drain role: TMEM lane quadrant q4, column group cg = (generating CTA r', part)
+        const unsigned q4 = w & 3u, cg = w >> 2;
+        float* ws_unit = p.ws + ((b * p.nsplit + sp) * 4) * p.Nf;
+        const int64_t k0 = kb + (int64_t)256 * (U2_HC * (cg >> 1)) + (int64_t)(128u * rank + 32u * q4 + lane);
+        const uint32_t t_drain = tmem + ((32u * q4) << 16) + 64u * cg;
+        int ti_cur = -1;
+
+        for (int f = 0; f < nwin; ++f) {
+            const int it_end = min(nst, (f + 1) * flush_st);
+            for (int it = f * flush_st + (int)grp; it < it_end; it += 2) {
+                const int s = it & (UP_STAGES - 1);
+                const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
+                const int ti = it >> 3;                                 // 8 stage-steps per record tile
+                if (ti != ti_cur) {                                     // next record tile of this group (buffer ti & 1)
+                    ti_cur = ti;
+                    if (tg < UM_TS) {
+                        float4 r = make_float4(0.f, 0.f, 0.f, 0.f);     // pad: X = 0, phases 0
+                        if (pre_ok) {
+                            const u64 pa = pre_u + (u64)kb * pre_v;     // u + kb v (mod 1, 64-bit wrap; reading G3)
+                            r.x = pre_x * xs;
+                            r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
+                            r.z = __uint_as_float((unsigned)((256ull * pre_v + 0x80000000ull) >> 32));
+                        }
+                        rec[(ti & 1) * UM_TS + tg] = r;
+                        prefetch(ti + 1);
+                    }
+                    if (grp == 0) asm volatile("bar.sync 1, 256;" ::: "memory");
+                    else asm volatile("bar.sync 2, 256;" ::: "memory");
+                }
+                mbar_wait(U2_EMPTY(s), ph ^ 1u);                        // the pair's MMAs that read this stage have completed
+                const uint32_t st = s_stage + (uint32_t)s * UP_STAGE_BYTES;
+                if (tg == 0) {                                          // this CTA's 128 table rows of the two k-steps: one bulk copy
+                    mbar_expect_tx(U2_FULL(s), UT_KPS * UP_GROUP_BYTES);
+                    tma_bulk_g2s(st + UP_A_STAGE, tab + (int64_t)it * (UT_KPS * UP_GROUP_BYTES), UT_KPS * UP_GROUP_BYTES, U2_FULL(s));
+                }
+                const int s0 = (it & 7) * (UT_KPS * UM_KS) + samp_off;  // within the 128-sample record tile
+                const int left = n_samp - (it * (UT_KPS * UM_KS) + samp_off);
+                if (left >= 4) u2_gen<false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
+                else u2_gen<true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(U2_FULL(s));
+            }
+            // ---- drain window f (all 16 warps of both CTAs)
+            const bool last = (f == nwin - 1);
+            mbar_wait(bar_accf, (uint32_t)f & 1u);
+            tc_fence_after();
+            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0);
+            if (last) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) { if (rank == 0) mbar_arrive(bar_acce); else mbar_arrive_remote(bar_acce, 0u); }
+        }
+    } else if (lane == 0 && rank == 0) {
+        // ===================== step 4: the single MMA-issuing thread of the pair =====================
+        int f = 0;
+        for (int it = 0; it < nst; ++it) {
+            const int s = it & (UP_STAGES - 1);
+            const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
+            mbar_wait(U2_FULL(s), ph);
+            mbar_wait_cluster(U2_PEER(s), ph);
+            tc_fence_after();
+            const bool win_first = (it == f * flush_st);
+            #pragma unroll
+            for (int kk = 0; kk < UT_KPS; ++kk) {
+                const uint32_t g0 = s_stage + (uint32_t)s * UP_STAGE_BYTES + kk * (3 * UM_A_BYTES);           // generated: N side
+                const uint32_t t0 = s_stage + (uint32_t)s * UP_STAGE_BYTES + UP_A_STAGE + kk * UP_GROUP_BYTES; // table: M side
+                const uint64_t dGh = umma_desc(g0, UM_A_BYTES / 2, 128), dG8 = umma_desc(g0 + UM_A_BYTES, UM_A_BYTES / 2, 128);
+                const uint64_t dGv = umma_desc(g0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
+                const uint64_t dTh = umma_desc(t0, UP_B_HALF / 2, 128), dT8 = umma_desc(t0 + UP_B_HALF, UP_B_HALF / 2, 128);
+                const uint64_t dTv = umma_desc(t0 + 2 * UP_B_HALF, UP_B_HALF / 2, 128);
+                tc_mma_f16_pair(tmem, dTh, dGh, UP_IDESC, (!win_first || kk > 0) ? 1u : 0u);
+                tc_mma_f8_pair(tmem, dT8, dG8, UP_IDESC_F8, 1u);
+                tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
+            }
+            tc_commit_pair(U2_EMPTY(s));
+            const bool last = (it == nst - 1);
+            if (it + 1 == (f + 1) * flush_st || last) {
+                tc_commit_pair(bar_accf);
+                if (!last) { mbar_wait_cluster(bar_acce, (uint32_t)f & 1u); tc_fence_after(); }
+                ++f;
+            }
+        }
+    } else if (lane == 0) {
+        // ===================== CTA 1: forward "my stage is full" to the issuing thread in CTA 0 =====================
+        for (int it = 0; it < nst; ++it) {
+            const int s = it & (UP_STAGES - 1);
+            const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
+            mbar_wait(U2_FULL(s), ph);
+            mbar_arrive_remote(U2_PEER(s), 0u);
+        }
+    }
+#undef U2_FULL
+#undef U2_EMPTY
+#undef U2_PEER
+
+    __syncwarp();
+    tc_fence_before();
+    cluster_sync_all();
+    if (w == UM_GEN_WARPS) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"((uint32_t)UM_TMEM_COLS) : "memory");
+    }
+}
+
+}  // namespace lsp

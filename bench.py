@@ -202,7 +202,7 @@ def run_ours(args):
     h = lsp.Handle(local)
     for key, val in ((lsp.PARAM_K, args.K), (lsp.PARAM_THREADS, args.threads), (lsp.PARAM_NSPLIT, args.nsplit),
                      (lsp.PARAM_RECURRENCE, args.recurrence), (lsp.PARAM_FLUSH, args.flush), (lsp.PARAM_BTABLE, args.btable),
-                     (lsp.PARAM_COARSE, args.coarse), (lsp.PARAM_CORR, args.corr)):
+                     (lsp.PARAM_COARSE, args.coarse), (lsp.PARAM_CORR, args.corr), (lsp.PARAM_PAIR, args.pair)):
         if val:
             h.set_param(key, val)
     h.set_param(lsp.PARAM_TIMING, 1)
@@ -348,6 +348,45 @@ def run_ours(args):
     return 0
 
 
+def run_sweep(args):
+    """N_t scaling sweep (the paper's Fig. 4): the workload is uniformly
+    down-sampled by 64, 32, ..., 1 with N_f in proportion to N_t; whole-call device time (all kernels, CUDA events) per
+    size, and the log-log slope d log t / d log N_t, which the paper expects to approach 2.  One JSON line."""
+    import torch
+    import paper_1007_1658_b200 as lsp
+    base = workloads.make(args.workload)
+    h = lsp.Handle(0)
+    if args.pair:
+        h.set_param(lsp.PARAM_PAIR, args.pair)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    rows = []
+    for step in (64, 32, 16, 8, 4, 2, 1):
+        w = workloads.downsample(base, step) if step > 1 else base
+        t_d = torch.from_numpy(np.ascontiguousarray(w.t)).cuda()
+        x_d = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
+        P_d = torch.empty(w.Nf, dtype=torch.float32, device="cuda")
+        for _ in range(3):
+            h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d)
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(max(5, args.steps // 2)):
+            flush_buf.zero_()
+            ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ea.record(); h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d); eb.record()
+            torch.cuda.synchronize()
+            ms.append(ea.elapsed_time(eb))
+        med = statistics.median(ms)
+        rows.append({"Nt": w.Nt, "Nf": w.Nf, "ms_median": med, "ms_min": min(ms), "terms_per_s": w.terms / (med * 1e-3),
+                     "kernel": h.last_plan()["kernel"]})
+    for a, b in zip(rows[:-1], rows[1:]):
+        b["slope_vs_previous"] = float(np.log(b["ms_median"] / a["ms_median"]) / np.log(b["Nt"] / a["Nt"]))
+    h.close()
+    print(json.dumps({"metric": "lomb_scargle_Nt_sweep", "workload": base.name, "unit": "ms", "data": "synthetic",
+                      "note": "uniform down-sampling, Nf proportional to Nt (PAPER.md:351-353, eq. (11)); expected slope -> 2",
+                      "sweep": rows}))
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -363,11 +402,15 @@ def main(argv=None):
     ap.add_argument("--btable", type=int, default=0)
     ap.add_argument("--coarse", type=int, default=0)
     ap.add_argument("--corr", type=int, default=0, help="tcgen05 table form: 1 = hi*lo corrections as two fp16 MMAs, 0/2 = one e5m2 MMA")
+    ap.add_argument("--pair", type=int, default=0, help="tcgen05 table form: 1 = no CTA pairs, 2 = pairs share the streamed operand, 0/3 = the generated one")
+    ap.add_argument("--sweep", action="store_true", help="N_t scaling sweep of --workload (single series) instead of the bench line")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     return run_ours(args)
 
 

@@ -168,6 +168,16 @@ def p0(Nt: int = 382003, Nf: int = 1528064, seed: Optional[int] = None) -> Workl
                     expected_peak_bin=f_inj / df - 1.0)
 
 
+def downsample(w: Workload, step: int) -> Workload:
+    """Uniform down-sampling of a single series, as the paper does for its N_t sweep (Fig. 4): every
+    `step`-th sample, same span and frequency resolution, N_f scaled in proportion to N_t (eq. (11))."""
+    if w.B != 1 or step < 1:
+        raise ValueError("downsample: single series, step >= 1")
+    t, x = np.ascontiguousarray(w.t[::step]), np.ascontiguousarray(w.x[::step])
+    Nf = max(1, int(round(w.Nf * (t.shape[0] / w.Nt))))
+    return Workload("%s/%d" % (w.name, step), t, x, w.f_min, w.df, Nf, T=w.T, expected_peak_bin=w.expected_peak_bin)
+
+
 _FACTORY = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "C5": c5, "P0": p0}
 
 

@@ -295,12 +295,15 @@ def run_ours(args):
         }
     else:                                                    # tensor-core form: 8 real MACs = 16 FLOP per term
         tpeak = float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1590.0)))   # fp16 rate = bf16 rate
-        achieved = w.terms * TENSOR_FLOP_PER_TERM / (k_ms * 1e-3) / 1e12
+        alg_flop = TENSOR_FLOP_PER_TERM
         executed = TENSOR_FLOP_PER_TERM_EXECUTED_CORR8 if "e5m2corr" in plan["kernel"] else TENSOR_FLOP_PER_TERM_EXECUTED
+        if "shared_gemm" in plan["kernel"]:                  # shared-time batch: only W = XC + i XS is per series (one real MAC each for
+            alg_flop, executed = 4, 8                        # cos and sin: 4 FLOP per term); executed: main product 4 + e5m2 corrections 4
+        achieved = w.terms * alg_flop / (k_ms * 1e-3) / 1e12
         roofline = {
             "bound": "tensor", "achieved": achieved, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved / tpeak,
-            "flop_per_term_algorithmic": TENSOR_FLOP_PER_TERM, "flop_per_term_executed": executed,
-            "frac_executed": achieved * executed / TENSOR_FLOP_PER_TERM / tpeak,
+            "flop_per_term_algorithmic": alg_flop, "flop_per_term_executed": executed,
+            "frac_executed": achieved * executed / alg_flop / tpeak,
             "peak_basis": "MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16 back to back; fp16 has the same nominal "
                           "rate; the kernel is timed inside a step that is itself power-capped): %s"
                           % ("measured" if peaks else "fallback 1590"),

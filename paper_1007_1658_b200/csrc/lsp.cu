@@ -12,6 +12,7 @@
 #include "lsp_accum_umma_pair.cuh"
 #include "lsp_accum_umma_pair2.cuh"
 #include "lsp_accum_umma_small.cuh"
+#include "lsp_shared_gemm.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_fap.cuh"
 #include "lsp_plan.h"
@@ -41,7 +42,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0, opt_corr = 0, opt_pair = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0, opt_corr = 0, opt_pair = 0, opt_shared = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     uint64_t timed_calls = 0;
     // workspace
@@ -135,11 +136,105 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
     return pl;
 }
 
+// Shared-time batch (t_stride = 0): XC, XS as one dense GEMM over all series, CC, CS once per frequency (lsp_shared_gemm.cuh).
+int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_stride,
+                      int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
+                      float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st)
+{
+    Plan pl = make_plan(h, B, Nt, Nf);                    // pre-pass partition only
+    int64_t nsplit = (Nt + SG_MAX_SPLIT - 1) / SG_MAX_SPLIT;
+    int64_t gps = ((Nt + nsplit - 1) / nsplit + SG_KS - 1) / SG_KS;
+    gps = (gps + SG_KPS - 1) / SG_KPS * SG_KPS;           // k-step groups per split: whole stages
+    nsplit = (Nt + gps * SG_KS - 1) / (gps * SG_KS);
+    const int64_t ng = nsplit * gps;
+    const int64_t nmb = (B + SG_M - 1) / SG_M, nfb = (Nf + SG_F - 1) / SG_F;
+    const int64_t x_row = (Nf + 3) / 4 * 4;
+    if (nmb * nfb * nsplit > 2147483647LL || ng > 65535 || nsplit > 65535 || B > 65535) return LSP_EINVAL;
+    pl.rec = REC_UMMA; pl.K = SG_F; pl.T = SG_THREADS; pl.nsplit = (int)nsplit; pl.nfb = (int)nfb; pl.L = 0;
+    pl.split_len = gps * SG_KS; pl.launches = 7;
+    pl.kernel_name = "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times>";
+
+    const size_t n_samp = (size_t)B * (size_t)Nt;
+    size_t off = 0;
+    const size_t o_recA = off; off = align_up(off + n_samp * sizeof(float4), 256);
+    const size_t o_recB = off; off = align_up(off + n_samp * sizeof(ulonglong2), 256);
+    const size_t o_xa = off;   off = align_up(off + (size_t)nmb * ng * SG_A_GROUP, 256);
+    const size_t o_eb = off;   off = align_up(off + (size_t)nfb * ng * SG_B_GROUP, 256);
+    const size_t o_pv = off;   off = align_up(off + (size_t)ng * 4 * (size_t)Nf * sizeof(float), 256);
+    const size_t o_wsv = off;  off = align_up(off + (size_t)nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    const size_t o_wsx = off;  off = align_up(off + (size_t)B * nsplit * 2 * (size_t)x_row * sizeof(float), 256);
+    const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
+    const size_t o_cnt = off;  off = align_up(off + (size_t)B * sizeof(unsigned), 256);
+    int rc = ensure(h, &h->buf, &h->buf_bytes, off);
+    if (rc != LSP_OK) return rc;
+    char* base = static_cast<char*>(h->buf);
+    float4* recA = reinterpret_cast<float4*>(base + o_recA);
+    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
+    unsigned char* xa = reinterpret_cast<unsigned char*>(base + o_xa);
+    unsigned char* eb = reinterpret_cast<unsigned char*>(base + o_eb);
+    float* part_v = reinterpret_cast<float*>(base + o_pv);
+    float* ws_v = reinterpret_cast<float*>(base + o_wsv);
+    float* ws_x = reinterpret_cast<float*>(base + o_wsx);
+    double* psum = reinterpret_cast<double*>(base + o_psum);
+    double* pvar = reinterpret_cast<double*>(base + o_pvar);
+    u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
+    unsigned* counter = reinterpret_cast<unsigned*>(base + o_cnt);
+
+    const bool timing = h->opt_timing != 0;
+    cudaEvent_t* ev = h->ev[h->timed_calls % TIMING_RING];
+    if (timing) {
+        for (int i = 0; i < 5; ++i)
+            if (!ev[i]) LSP_CUDA(h, cudaEventCreate(&ev[i]));
+        LSP_CUDA(h, cudaEventRecord(ev[0], st));
+    }
+    // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
+    dim3 gpre((unsigned)pl.nparts, (unsigned)B);
+    moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
+    LSP_CUDA(h, cudaGetLastError());
+    if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
+    records_kernel<<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar);
+    LSP_CUDA(h, cudaGetLastError());
+    // step 3 for every (sample, frequency) once; CC, CS once per frequency
+    shared_e_kernel<<<dim3((unsigned)nfb, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng, part_v);
+    LSP_CUDA(h, cudaGetLastError());
+    shared_v_reduce_kernel<<<dim3((unsigned)((Nf + 255) / 256), (unsigned)nsplit), 256, 0, st>>>(part_v, Nf, (int)gps, ws_v);
+    LSP_CUDA(h, cudaGetLastError());
+    shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(recA, pvar, pl.nparts, B, Nt, xa, (int)ng);
+    LSP_CUDA(h, cudaGetLastError());
+    if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
+    // steps 4-5: the contraction
+    SharedGemmParams gp;
+    gp.xa = xa; gp.eb = eb; gp.ws_x = ws_x; gp.B = B; gp.Nf = Nf; gp.x_row = x_row;
+    gp.nmb = (int)nmb; gp.nfb = (int)nfb; gp.nsplit = (int)nsplit; gp.ng = (int)ng; gp.groups_per_split = (int)gps;
+    LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
+    shared_gemm_kernel<<<(unsigned)(nmb * nfb * nsplit), SG_THREADS, SG_SMEM, st>>>(gp);
+    LSP_CUDA(h, cudaGetLastError());
+    if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
+    // steps 6-7
+    FinishParams fp;
+    fp.ws = ws_v; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
+    fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
+    fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = (int)nsplit; fp.nparts = pl.nparts;
+    fp.cc_fix = 0.0; fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
+    const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
+    dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
+    finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
+    LSP_CUDA(h, cudaGetLastError());
+    if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
+    h->plan = pl;
+    return LSP_OK;
+}
+
 int run_device(lsp_ctx* h,
                const double* t, int64_t t_stride, const float* x, int64_t x_stride,
                int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st, bool gls = false)
 {
+    if (t_stride == 0 && B > 1 && !gls && h->opt_shared != 1 && h->opt_rec == 0 && B <= 65535 &&
+        (h->opt_shared == 2 || (B >= 16 && Nt >= 512)))
+        return run_device_shared(h, t, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride, peak_idx, peak_val, st);
     Plan pl = make_plan(h, B, Nt, Nf);
     const bool umma = pl.rec == REC_UMMA;
     const bool mma = pl.rec == REC_MMA || umma;                      // tensor-core forms: X scaled to unit variance
@@ -311,6 +406,7 @@ int run_device(lsp_ctx* h,
     fp.cc_fix = (!mma && ke->tile_z == 0 && (Nt & 1)) ? 0.5 : 0.0;   // phantom partner of an odd last sample (pair-packed only)
     fp.x_scaled = mma ? 1 : 0;
     fp.ws1 = ws1;
+    fp.ws_x = nullptr; fp.x_row = 0;
     const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
     dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
     finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
@@ -379,6 +475,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
         case LSP_PARAM_CORR:       if (value > 2) return LSP_EINVAL; h->opt_corr = value; break;
         case LSP_PARAM_PAIR:       if (value > 3) return LSP_EINVAL; h->opt_pair = value; break;
+        case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -398,6 +495,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_COARSE:     *value = h->opt_coarse; break;
         case LSP_PARAM_CORR:       *value = h->opt_corr; break;
         case LSP_PARAM_PAIR:       *value = h->opt_pair; break;
+        case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

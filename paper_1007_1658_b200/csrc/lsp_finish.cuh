@@ -30,6 +30,8 @@ struct FinishParams {
     double cc_fix;                     // added to sum(CC - n/2): 0.5 when the pair-packed kernel padded an odd Nt
     int x_scaled;                      // 1: XC, XS were accumulated from X * x_scale() (tensor-core form)
     const float* ws1;                  // generalised periodogram: [B][nsplit][4][Nf] of the unit-weight pass (planes 0, 1 = sum cos, sum sin); else NULL
+    const float* ws_x;                 // shared-time batch (lsp_shared_gemm.cuh): XC, XS from [B][nsplit][2][x_row]; `ws` is then ONE
+    int64_t x_row;                     //   [nsplit][4][Nf] block shared by all series (planes 2, 3 = CC - n/2, CS); else NULL / 0
 };
 
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
@@ -50,7 +52,8 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     const double inv2var = 0.5 / s_var;
     const double Nt = (double)p.Nt;
     const double cc_fix = p.cc_fix;
-    const float* ws = p.ws + b * p.nsplit * 4 * p.Nf;
+    const float* ws = p.ws_x ? p.ws : p.ws + b * p.nsplit * 4 * p.Nf;
+    const float* wx = p.ws_x ? p.ws_x + b * p.nsplit * 2 * p.x_row : nullptr;
 
     u64 best = 0ull;
     #pragma unroll
@@ -60,8 +63,13 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
         double XC = 0.0, XS = 0.0, CCh = cc_fix, CS = 0.0;
         for (int sp = 0; sp < p.nsplit; ++sp) {            // fixed order over the time splits
             const float* w = ws + (int64_t)sp * 4 * p.Nf + k;
-            XC += (double)__ldg(w);
-            XS += (double)__ldg(w + p.Nf);
+            if (wx) {
+                XC += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + k);
+                XS += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + p.x_row + k);
+            } else {
+                XC += (double)__ldg(w);
+                XS += (double)__ldg(w + p.Nf);
+            }
             CCh += (double)__ldg(w + 2 * p.Nf);
             CS += (double)__ldg(w + 3 * p.Nf);
         }

@@ -352,6 +352,34 @@ def test_batched_table_form(lsp, shared, pair):
         assert _same_peak(P[b].cpu().numpy(), Pref[b])
 
 
+@pytest.mark.parametrize("B,Nt,Nf", [(20, 1500, 3000), (130, 700, 777), (5, 5000, 1001), (33, 2049, 130), (2, 17, 9)])
+def test_shared_time_gemm(lsp, B, Nt, Nf):
+    """t_stride = 0 through the dense-contraction path (lsp_shared_gemm.cuh): ragged series /
+    frequency / sample counts, one to three time splits, against the oracle series by series; and against the generic path."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=100 + B)
+    tt = w.t[0].copy()
+    Pref, iref, _ = oracle.periodogram_batched(tt, w.x, w.f_min, w.df, w.Nf)
+    out = {}
+    for shared in (1, 2):
+        h.set_param(pkg.PARAM_SHARED, shared)
+        try:
+            P, pi, pv = h.periodogram_batched(torch.from_numpy(tt).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf)
+            torch.cuda.synchronize()
+            assert ("shared_gemm" in h.last_plan()["kernel"]) == (shared == 2)
+        finally:
+            h.set_param(pkg.PARAM_SHARED, 0)
+        out[shared] = P.cpu().numpy()
+        if shared == 2:
+            assert np.array_equal(pv.cpu().numpy(), out[2].max(axis=1)) and np.array_equal(pi.cpu().numpy(), out[2].argmax(axis=1))
+    tol = TOL if Nt >= 100 else 1e-3                       # tiny Nt: fp16 V in the generic path (see test_umma_table_form_ragged)
+    for b in range(B):
+        for shared in (1, 2):
+            assert np.max(np.abs(out[shared][b] - Pref[b])) <= tol * Pref[b].max(), "series %d shared=%d" % (b, shared)
+        assert _same_peak(out[2][b], Pref[b])
+
+
 def test_batch_of_one_equals_single(lsp):
     import torch
     pkg, h = lsp

@@ -168,6 +168,13 @@ def p0(Nt: int = 382003, Nf: int = 1528064, seed: Optional[int] = None) -> Workl
                     expected_peak_bin=f_inj / df - 1.0)
 
 
+def c4s(B: int = 4096, Nt: int = 1000, Nf: int = 2000, seed: Optional[int] = None) -> Workload:
+    """C4S: the shared-time form of the Monte-Carlo batch (the sampling is kept, the noise redrawn):
+    C4's noise series, all on the time vector of C4's series 0.  t is ONE vector [Nt] (t_stride = 0 in the ABI)."""
+    w = c4(B=B, Nt=Nt, Nf=Nf, seed=seed)
+    return Workload("C4S", np.ascontiguousarray(w.t[0]), w.x, w.f_min, w.df, w.Nf, B=w.B, T=w.T, meta=dict(w.meta))
+
+
 def downsample(w: Workload, step: int) -> Workload:
     """Uniform down-sampling of a single series, as the paper does for its N_t sweep (Fig. 4): every
     `step`-th sample, same span and frequency resolution, N_f scaled in proportion to N_t (eq. (11))."""
@@ -178,7 +185,7 @@ def downsample(w: Workload, step: int) -> Workload:
     return Workload("%s/%d" % (w.name, step), t, x, w.f_min, w.df, Nf, T=w.T, expected_peak_bin=w.expected_peak_bin)
 
 
-_FACTORY = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "C5": c5, "P0": p0}
+_FACTORY = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "C4S": c4s, "C5": c5, "P0": p0}
 
 
 def make(name: str, **kw) -> Workload:

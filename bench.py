@@ -43,7 +43,7 @@ FP32_LANES_PER_SM = 128          # B200: 4 SMSPs x 32 FP32 lanes (guide: blackwe
 # ----------------------------------------------------------------------------- helpers (host logic)
 def rank_seed(workload: str, rank: int):
     """Seed of rank r's series: the config's own seed for rank 0, +1000*r for the others."""
-    idx = {"C1": 1, "C2": 2, "C3": 3, "C4": 4, "C5": 5, "P0": 0}[workload.upper()]
+    idx = {"C1": 1, "C2": 2, "C3": 3, "C4": 4, "C4S": 4, "C5": 5, "P0": 0}[workload.upper()]
     return None if rank == 0 else workloads.BASE_SEED + idx + 1000 * rank
 
 
@@ -130,7 +130,7 @@ def time_oracle(w, seconds_target: float = 12.0, max_freqs: int = 4096):
 
     Returns (terms_per_s, cores, sample_description, elapsed_s)."""
     import oracle
-    t = w.t[0] if w.B > 1 else w.t
+    t = w.t[0] if (w.B > 1 and w.t.ndim == 2) else w.t          # batch: series 0 (shared-time batch: the one time vector)
     x = w.x[0] if w.B > 1 else w.x
     cores = oracle.host_threads()
     oracle.periodogram(t[:1000], x[:1000], w.f_min, w.df, 8)          # build + warm the library

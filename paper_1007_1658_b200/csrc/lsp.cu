@@ -152,7 +152,8 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     if (nmb * nfb * nsplit > 2147483647LL || ng > 65535 || nsplit > 65535 || B > 65535) return LSP_EINVAL;
     pl.rec = REC_UMMA; pl.K = SG_F; pl.T = SG_THREADS; pl.nsplit = (int)nsplit; pl.nfb = (int)nfb; pl.L = 0;
     pl.split_len = gps * SG_KS; pl.launches = 7;
-    pl.kernel_name = "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times>";
+    pl.kernel_name = (nsplit == 1) ? "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times,fused-finish>"
+                                   : "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times>";
 
     const size_t n_samp = (size_t)B * (size_t)Nt;
     size_t off = 0;
@@ -162,7 +163,9 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     const size_t o_eb = off;   off = align_up(off + (size_t)nfb * ng * SG_B_GROUP, 256);
     const size_t o_pv = off;   off = align_up(off + (size_t)ng * 4 * (size_t)Nf * sizeof(float), 256);
     const size_t o_wsv = off;  off = align_up(off + (size_t)nsplit * 4 * (size_t)Nf * sizeof(float), 256);
-    const size_t o_wsx = off;  off = align_up(off + (size_t)B * nsplit * 2 * (size_t)x_row * sizeof(float), 256);
+    const bool fuse = (nsplit == 1);                      // one split: the GEMM's accumulators are the sums; steps 6-7 run in its epilogue
+    const size_t o_wsx = off;  if (!fuse) off = align_up(off + (size_t)B * nsplit * 2 * (size_t)x_row * sizeof(float), 256);
+    const size_t o_vc = off;   off = align_up(off + (size_t)4 * (size_t)Nf * sizeof(double), 256);
     const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
@@ -177,6 +180,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     float* part_v = reinterpret_cast<float*>(base + o_pv);
     float* ws_v = reinterpret_cast<float*>(base + o_wsv);
     float* ws_x = reinterpret_cast<float*>(base + o_wsx);
+    double* vconst = reinterpret_cast<double*>(base + o_vc);
     double* psum = reinterpret_cast<double*>(base + o_psum);
     double* pvar = reinterpret_cast<double*>(base + o_pvar);
     u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
@@ -194,13 +198,17 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    records_kernel<<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar);
+    records_kernel<true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar);
     LSP_CUDA(h, cudaGetLastError());
     // step 3 for every (sample, frequency) once; CC, CS once per frequency
     shared_e_kernel<<<dim3((unsigned)nfb, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng, part_v);
     LSP_CUDA(h, cudaGetLastError());
     shared_v_reduce_kernel<<<dim3((unsigned)((Nf + 255) / 256), (unsigned)nsplit), 256, 0, st>>>(part_v, Nf, (int)gps, ws_v);
     LSP_CUDA(h, cudaGetLastError());
+    if (fuse) {
+        shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst);
+        LSP_CUDA(h, cudaGetLastError());
+    }
     shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(recA, pvar, pl.nparts, B, Nt, xa, (int)ng);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
@@ -208,10 +216,17 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     SharedGemmParams gp;
     gp.xa = xa; gp.eb = eb; gp.ws_x = ws_x; gp.B = B; gp.Nf = Nf; gp.x_row = x_row;
     gp.nmb = (int)nmb; gp.nfb = (int)nfb; gp.nsplit = (int)nsplit; gp.ng = (int)ng; gp.groups_per_split = (int)gps;
+    gp.vconst = fuse ? vconst : nullptr; gp.part_var = pvar; gp.P = P; gp.p_stride = p_stride;
+    gp.peak_idx = peak_idx; gp.peak_val = peak_val; gp.peak64 = peak64; gp.counter = counter; gp.Nt = Nt; gp.nparts = pl.nparts;
     LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
     shared_gemm_kernel<<<(unsigned)(nmb * nfb * nsplit), SG_THREADS, SG_SMEM, st>>>(gp);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
+    if (fuse) {                                           // steps 6-7 ran in the GEMM's epilogue
+        if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
+        h->plan = pl;
+        return LSP_OK;
+    }
     // steps 6-7
     FinishParams fp;
     fp.ws = ws_v; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
@@ -307,7 +322,7 @@ int run_device(lsp_ctx* h,
     moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    records_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
+    records_kernel<false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
                                          psum, recA, recB, pvar);
     LSP_CUDA(h, cudaGetLastError());
     if (gls) {

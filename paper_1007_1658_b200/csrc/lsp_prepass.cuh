@@ -32,6 +32,8 @@ __global__ void moments_kernel(const float* __restrict__ x, int64_t x_stride, in
 }
 
 // grid (nb, B).  Writes recA, recB for the block's chunk and part_var[b][blk] = sum (x - mean)^2.
+// SHARED (shared-time batch, t_stride = 0): only X_j is needed per series, the phases only once (series 0).
+template <bool SHARED>
 __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                const float* __restrict__ x, int64_t x_stride,
                                int64_t Nt, int64_t chunk, double f_min, double df,
@@ -56,13 +58,14 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
     for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         const double d = (double)__ldg(xb + j) - mean;
         acc += d * d;
+        const int64_t o = (int64_t)b * Nt + j;
+        if (SHARED && b != 0) { recA[o] = make_float4((float)d, 0.f, 0.f, 0.f); continue; }
         const double tp = __ldg(tb + j) - t0;
         double vfrac;
         const u64 u = frac_fixed64(f_min, tp, nullptr);
         const u64 v = frac_fixed64(df, tp, &vfrac);
-        double sd, cd;
-        sincospi(2.0 * vfrac, &sd, &cd);                   // accurate: its error is applied K times per run
-        const int64_t o = (int64_t)b * Nt + j;
+        double sd = 0.0, cd = 0.0;
+        if (!SHARED) sincospi(2.0 * vfrac, &sd, &cd);      // accurate: its error is applied K times per run
         recA[o] = make_float4((float)d, (float)cd, (float)sd, (float)(2.0 * cd));
         recB[o] = make_ulonglong2(u, v);
     }

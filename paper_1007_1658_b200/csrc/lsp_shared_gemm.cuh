@@ -31,7 +31,7 @@ constexpr int SG_B_PLANE = 2 * SG_F * 32;                  // 8 KB
 constexpr int SG_A_GROUP = 2 * SG_A_PLANE;                 // per k-step: fp16 plane + e5m2 plane
 constexpr int SG_B_GROUP = 2 * SG_B_PLANE;
 constexpr int SG_KPS = 2;                                  // k-steps per stage
-constexpr int SG_STAGES = 4;
+constexpr int SG_STAGES = 2;                                 // x 48 KB: two CTAs per SM (256 TMEM columns each), so one CTA's epilogue overlaps the other's main loop
 constexpr int SG_STAGE_BYTES = SG_KPS * (SG_A_GROUP + SG_B_GROUP);
 constexpr size_t SG_SMEM = (size_t)SG_STAGES * SG_STAGE_BYTES + 256;
 constexpr int SG_THREADS = 6 * 32;                         // warp 0: TMA, warp 1: MMA + TMEM, warps 2-5: drain
@@ -45,7 +45,28 @@ struct SharedGemmParams {
     int64_t B, Nf, x_row;
     int nmb, nfb, nsplit, ng;       // ng = k-step groups over ALL splits = nsplit * groups_per_split
     int groups_per_split;           // even
+    // fused steps 6-7 (only when nsplit == 1: the accumulators ARE the sums of eq. (8)); vconst == NULL: write ws_x instead
+    const double* vconst;           // [4][Nf]: cos 2 w tau, sin 2 w tau, 1/(Nt + R), 1/(Nt - R) (0 if dropped, reading G7)
+    const double* part_var;         // [B][nparts]
+    float* P; int64_t p_stride;     // nullable
+    int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
+    int64_t Nt; int nparts;
 };
+
+// Per-frequency part of step 6 for the shared-time batch: from CC - n/2, CS (summed over the splits in fixed order)
+// A = CC - SS, B = 2 CS, R = hypot(A, B) -> (A/R, B/R, 1/(Nt + R), 1/(Nt - R)); eqs (5)-(7), tau eliminated.
+__global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restrict__ ws_v, int nsplit, int64_t Nf, int64_t Nt_i, double* __restrict__ vconst)
+{
+    const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (k >= Nf) return;
+    double CCh = 0.0, CS = 0.0;
+    for (int sp = 0; sp < nsplit; ++sp) { CCh += (double)ws_v[((int64_t)sp * 4 + 2) * Nf + k]; CS += (double)ws_v[((int64_t)sp * 4 + 3) * Nf + k]; }
+    const double Nt = (double)Nt_i, A = 2.0 * CCh, Bv = 2.0 * CS, R = hypot(A, Bv);
+    vconst[k] = (R > 0.0) ? A / R : 0.0;
+    vconst[Nf + k] = (R > 0.0) ? Bv / R : 0.0;
+    vconst[2 * Nf + k] = 1.0 / (Nt + R);
+    vconst[3 * Nf + k] = (Nt - R > 1e-6 * Nt) ? 1.0 / (Nt - R) : 0.0;
+}
 
 // ------------------------------------------------------------------ E tiles + partial CC, CS
 // grid (nfb, ng), 256 threads: kf = tid & 127 (frequency k = 128 nfb + kf), chunk = tid >> 7 (8 of the group's 16 samples).
@@ -143,7 +164,7 @@ __global__ void __launch_bounds__(256) shared_x_kernel(const float4* __restrict_
 // ------------------------------------------------------------------ the GEMM
 // grid.x = nmb * nfb * nsplit (frequency block fastest, then series block, then split), SG_THREADS threads,
 // SG_SMEM bytes of dynamic shared memory.
-__global__ void __launch_bounds__(SG_THREADS, 1) shared_gemm_kernel(const SharedGemmParams p)
+__global__ void __launch_bounds__(SG_THREADS, 2) shared_gemm_kernel(const SharedGemmParams p)
 {
     extern __shared__ __align__(128) unsigned char sg_smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sg_smem + SG_STAGES * SG_STAGE_BYTES);
@@ -219,6 +240,64 @@ __global__ void __launch_bounds__(SG_THREADS, 1) shared_gemm_kernel(const Shared
         const int64_t b = (int64_t)mb * SG_M + 32u * q4 + lane;
         mbar_wait(bar_acc, 0u);
         tc_fence_after();
+        if (p.vconst) {
+            // ---- fused steps 6-7: P[b][k] from this thread's XC (column kf) and XS (column 128 + kf)
+            double inv2var = 0.0;
+            if (b < p.B) {
+                double qv = 0.0;
+                for (int i = 0; i < p.nparts; ++i) qv += p.part_var[b * p.nparts + i];
+                double var = qv / (double)(p.Nt - 1);                   // sample variance (reading G1)
+                const double xs = (double)(float)(1.0 / sqrt(var));     // X was scaled by the fp32 x_scale(): undo it exactly
+                var *= xs * xs;
+                inv2var = 0.5 / var;
+            }
+            u64 best = 0ull;
+            const bool p_vec = p.P && ((p.p_stride & 3) == 0) && ((reinterpret_cast<uintptr_t>(p.P) & 15) == 0);
+            #pragma unroll 1
+            for (int cc = 0; cc < 4; ++cc) {
+                float vc[32], vs[32];
+                tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, vc);
+                tmem_ld32(tmem + ((32u * q4) << 16) + 128u + 32u * cc, vs);
+                const int64_t k0 = (int64_t)nb * SG_F + cc * 32;
+                if (b >= p.B) continue;
+                float pf[32];
+                #pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                    const int64_t k = k0 + i;
+                    pf[i] = 0.f;
+                    if (k < p.Nf) {
+                        const double XC = (double)vc[i], XS = (double)vs[i];
+                        const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
+                        const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
+                        const double val = (fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var;
+                        pf[i] = (float)val;
+                        const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+                        best = (key > best) ? key : best;
+                    }
+                }
+                if (p.P) {
+                    float* d = p.P + b * p.p_stride + k0;
+                    if (p_vec && k0 + 32 <= p.Nf) {
+                        #pragma unroll
+                        for (int i = 0; i < 32; i += 4) *reinterpret_cast<float4*>(d + i) = make_float4(pf[i], pf[i + 1], pf[i + 2], pf[i + 3]);
+                    } else {
+                        #pragma unroll
+                        for (int i = 0; i < 32; ++i) if (k0 + i < p.Nf) d[i] = pf[i];
+                    }
+                }
+            }
+            if (p.peak_idx && b < p.B) {                                // step 7: order-free packed arg-max, lowest k on ties (reading G9)
+                atomicMax(p.peak64 + b, best);
+                __threadfence();
+                const unsigned done = atomicAdd(p.counter + b, 1u);
+                if (done == (unsigned)p.nfb - 1u) {                     // last frequency block of this series: publish
+                    __threadfence();
+                    const u64 fin = atomicMax(p.peak64 + b, 0ull);
+                    p.peak_idx[b] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
+                    p.peak_val[b] = __uint_as_float((unsigned)(fin >> 32));
+                }
+            }
+        } else {
         float* dst = p.ws_x + ((b * p.nsplit + sp) * 2) * p.x_row;
         #pragma unroll 1
         for (int cc = 0; cc < 8; ++cc) {
@@ -231,6 +310,7 @@ __global__ void __launch_bounds__(SG_THREADS, 1) shared_gemm_kernel(const Shared
                 for (int i = 0; i < 32; i += 4)
                     if (k0 + i < p.x_row) *reinterpret_cast<float4*>(d + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
             }
+        }
         }
         tc_fence_before();
     }

@@ -4,7 +4,7 @@
 // atan2 / sincos is needed (the listing calls atan2 + __sincosf):
 //     A = CC - SS = 2 (CC - Nt/2),  B = 2 CS,  R = hypot(A, B)      [cos 2wtau = A/R, sin 2wtau = B/R]
 //     S = XC^2 + XS^2,  D = ((XC^2 - XS^2) A + 2 XC XS B) / R
-//     P = [ (S + D)/(Nt + R) + (S - D)/(Nt - R) ] / (2 var)
+//     P = [ (S + D)/(Nt + R) + (S - D)/(Nt - R) ] / (2 var)  =  (S Nt - D R) / ((Nt^2 - R^2) var)
 // (denominators of eq. (5) are (Nt +- R)/2, numerators (S +- D)/2).  All in fp64: O(Nf) work.
 // Step 7: arg-max_k P with the lowest index among ties (reading G9), through one packed 64-bit
 // atomicMax per block -- integer max is order-independent, so the result is deterministic.
@@ -95,13 +95,20 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
             best = (key > best) ? key : best;
             continue;
         }
+        // The two terms of eq. (5) over the common denominator (Nt + R)(Nt - R) = Nt^2 - R^2: one fp64 division, no square root:
+        //   P 2 var = (S + D)/(Nt + R) + (S - D)/(Nt - R) = 2 (S Nt - D R) / (Nt^2 - R^2),   D R = (XC^2 - XS^2) A + 2 XC XS B
         const double A = 2.0 * CCh, Bv = 2.0 * CS;
-        const double R = hypot(A, Bv);
+        const double R2 = A * A + Bv * Bv;
         const double xc2 = XC * XC, xs2 = XS * XS;
         const double S = xc2 + xs2;
-        const double D = (R > 0.0) ? ((xc2 - xs2) * A + 2.0 * XC * XS * Bv) / R : 0.0;
-        double val = fmax(S + D, 0.0) / (Nt + R);
-        if (Nt - R > 1e-6 * Nt) val += fmax(S - D, 0.0) / (Nt - R);     // reading G7
+        const double DR = (xc2 - xs2) * A + 2.0 * XC * XS * Bv;
+        double val;
+        if (R2 < (1.0 - 1e-6) * (1.0 - 1e-6) * Nt * Nt) {
+            val = fmax(2.0 * (S * Nt - DR), 0.0) / (Nt * Nt - R2);
+        } else {                                                        // Nt - R <= 1e-6 Nt: the 0/0 term is dropped (reading G7)
+            const double R = sqrt(R2);
+            val = fmax(S + DR / R, 0.0) / (Nt + R);
+        }
         val *= inv2var;
         const float Pf = (float)val;
         if (p.P) p.P[b * p.p_stride + k] = Pf;

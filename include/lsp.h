@@ -64,6 +64,7 @@ enum {
     LSP_PARAM_COARSE    = 8,  /* tcgen05 form only: coarse extent L = 16, 32, 64 or 128 (a CTA owns 128 L frequencies) */
     LSP_PARAM_CORR      = 9,  /* tcgen05 table form only: how the hi*lo correction products are issued: 0 / 2 = one 8-bit (e5m2)  */
                               /* MMA of K = 32 (3 tensor slots per k-step), 1 = two fp16 MMAs (4 slots)                           */
+    LSP_PARAM_DUO       = 12, /* batches on the 2,048-frequency tile: 0 / 2 = two series per CTA (64 fine x 32 coarse each), 1 = one series per CTA (128 x 16) */
     LSP_PARAM_SHARED    = 11, /* batched call with t_stride = 0: 0 = the shared-time GEMM path when B >= 16 and Nt >= 512, 1 = never, 2 = always */
     LSP_PARAM_PAIR      = 10  /* tcgen05 table form with the e5m2 correction only: CTA pairs (cta_group::2, M = 256): 0 / 3 = the pair  */
                               /* shares the generated operand (64 sin/cos per sample per CTA), 2 = it shares the streamed one, 1 = no pairs */

@@ -5,7 +5,7 @@ its thin Python binding.  Nothing here computes on the CPU and nothing imports `
 """
 from .binding import (Handle, LspError, load, status_string, version, plan_query, plan_query_form, SYMBOLS,
                       LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM,
-                      PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE, PARAM_COARSE, PARAM_CORR, PARAM_PAIR, PARAM_SHARED,
+                      PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE, PARAM_COARSE, PARAM_CORR, PARAM_PAIR, PARAM_SHARED, PARAM_DUO,
                       REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z, REC_MMA, REC_UMMA)
 from .build import build
 

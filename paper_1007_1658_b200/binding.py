@@ -13,7 +13,7 @@ from typing import Optional, Tuple
 from . import build as _build
 
 LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM = 0, -1, -2, -3
-PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE, PARAM_COARSE, PARAM_CORR, PARAM_PAIR, PARAM_SHARED = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
+PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE, PARAM_COARSE, PARAM_CORR, PARAM_PAIR, PARAM_SHARED, PARAM_DUO = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12
 REC_MMA, REC_UMMA = 4, 5
 REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z = 1, 2, 3
 

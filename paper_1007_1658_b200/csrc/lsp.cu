@@ -13,6 +13,7 @@
 #include "lsp_accum_umma_pair2.cuh"
 #include "lsp_accum_umma_small.cuh"
 #include "lsp_shared_gemm.cuh"
+#include "lsp_accum_umma_duo.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_fap.cuh"
 #include "lsp_plan.h"
@@ -42,7 +43,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0, opt_corr = 0, opt_pair = 0, opt_shared = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0, opt_corr = 0, opt_pair = 0, opt_shared = 0, opt_duo = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     uint64_t timed_calls = 0;
     // workspace
@@ -258,9 +259,12 @@ int run_device(lsp_ctx* h,
     const bool umma_small = umma && pl.L < UM_L;          // 128 x L frequencies per CTA, two CTAs per SM
     pl.kernel_name = umma ? "accum_umma_kernel<tcgen05.m128n256k16.f16,hi+lo>"
                           : (mma ? "accum_mma_kernel<m16n8k16.f16,hi+lo>" : ke->name);
+    const bool duo = umma_small && pl.L == 16 && B >= 2 && h->opt_duo != 1;   // batches: two series per CTA (lsp_accum_umma_duo.cuh)
     if (umma_small) pl.kernel_name = pl.L == 16 ? "accum_umma_small_kernel<tcgen05.m128n32k16.f16,hi+lo>"
                                    : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
                                                  : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
+
+    if (duo) pl.kernel_name = "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>";
 
     // workspace carve-up
     const size_t n_samp = (size_t)B * (size_t)Nt;
@@ -343,7 +347,7 @@ int run_device(lsp_ctx* h,
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
 
     // steps 3-5
-    const int64_t units = B * (int64_t)pl.nsplit * pl.nfb;
+    const int64_t units = (duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
     // (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
     for (int pass = 0; pass < (gls ? 2 : 1); ++pass) {
@@ -355,7 +359,12 @@ int run_device(lsp_ctx* h,
         up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
         up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS;
         up.unit_x = pass;
-        if (umma_small) {
+        if (duo) {
+            UmmaDuoParams dp;
+            dp.u = up; dp.B = B;
+            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
+            accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
+        } else if (umma_small) {
 #define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
             LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
             accum_umma_small_kernel<LL, NS, MINB><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); } while (0)
@@ -491,6 +500,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_CORR:       if (value > 2) return LSP_EINVAL; h->opt_corr = value; break;
         case LSP_PARAM_PAIR:       if (value > 3) return LSP_EINVAL; h->opt_pair = value; break;
         case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
+        case LSP_PARAM_DUO:        if (value > 2) return LSP_EINVAL; h->opt_duo = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -511,6 +521,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_CORR:       *value = h->opt_corr; break;
         case LSP_PARAM_PAIR:       *value = h->opt_pair; break;
         case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
+        case LSP_PARAM_DUO:        *value = h->opt_duo; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

@@ -1,0 +1,234 @@
+// lsp_accum_umma_duo.cuh -- the tcgen05 form of steps 3-5 for BATCHES of short series: two series per CTA.
+//
+// accum_umma_small_kernel<16> gives one series 128 fine x 16 coarse = 2,048 frequencies and is bound by operand
+// generation: 128 + 16 = 144 MUFU sin/cos pairs per sample for 2,048 terms.  The balanced split 64 x 32 needs only 96,
+// but an MMA has M = 128 rows.  Here the 128 rows are TWO series x 64 fine values, and the N = 128 columns are two
+// series x (32 coarse values) x (Re, Im):
+//     A[(s,h)][j] = X_sj e^{i a_sjh},   B[(s',l,part)][j] = e^{i b_s'jl},   k = kb + 64 l + h,
+//     a_sjh = 2 pi frac(u_sj + (kb + h) v_sj),  b_sjl = 2 pi frac(64 l v_sj)           (exact 64-bit turns, reading G3)
+// The K index is the sample number j, which both series of a batch share (same Nt), so the diagonal blocks s = s' of
+//     D[(s,h)][(s',l,part)] = sum_j A[(s,h)][j] B[(s',l,part)][j]
+// are the sums of eq. (8) of series s; the off-diagonal blocks (series s against the times of
+// series s') are computed by the tensor core and never read -- the tensor pipe is far from busy here.
+// Per pair of samples 2 x 64 + 2 x 32 = 192 sin/cos pairs = 96 per series instead of 144.
+// Operand precision (fp16 hi + lo, three products for W, one for V), the stage ring, the periodic drain of D_W and
+// the layout of `ws` are those of lsp_accum_umma_small.cuh; D_W: TMEM columns 0..127, D_V: 128..255; two CTAs per SM.
+#pragma once
+#include "lsp_accum_umma_small.cuh"
+
+namespace lsp {
+
+constexpr int UD_H = 64;                                // fine values per series
+constexpr int UD_L = 32;                                // coarse values per series
+constexpr int UD_FPB = UD_H * UD_L;                     // frequencies per series per CTA
+constexpr int UD_STAGES = 4;
+constexpr int UD_STAGE_BYTES = 6 * UM_A_BYTES;          // A_hi, A_lo, A_V, B_hi, B_lo, B_V: 128 rows x 32 bytes each
+constexpr int UD_REC_BYTES = 2 * 2 * UM_TS * 16;        // [series][buffer][128 samples]
+constexpr size_t UD_SMEM = (size_t)UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES + 256;
+constexpr int UD_TMEM_COLS = 256;
+constexpr uint32_t UD_IDESC = (1u << 4) | ((uint32_t)(128 >> 3) << 17) | ((uint32_t)(UM_H >> 4) << 24);   // M = 128, N = 128
+
+// One B task: series s, coarse value l, 4 samples: rows (s,Re,l) and (s,Im,l) of B_hi, B_lo, B_V.  sB = address of row (s,Re,l).
+__device__ __forceinline__ void ud_gen_b(const float4* rec, int s0, unsigned l, uint32_t sB)
+{
+    unsigned rh[4], ih[4], rl[4], il[4], rv[4], iv[4];
+    #pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        float c, s;
+        sincos_phase32(l * __float_as_uint(rec[s0 + i].w), c, s);
+        rh[i] = pack_h2(c, -s);
+        ih[i] = pack_h2(s, c);
+        const float2 hf = unpack_h2(rh[i]);                             // (c_h, -s_h)
+        const float dc = c - hf.x, ds = s + hf.y;
+        rl[i] = pack_h2(dc, -ds);
+        il[i] = pack_h2(ds, dc);
+        const float cc = c + c, c2 = fmaf(cc, c, -1.f), s2 = cc * s;
+        rv[i] = pack_h2(c2, -s2);
+        iv[i] = pack_h2(s2, c2);
+    }
+    constexpr uint32_t IM = UD_L * 16;                                  // row (s,Im,l) is 32 rows below row (s,Re,l)
+    sts128(sB, rh[0], rh[1], rh[2], rh[3]);
+    sts128(sB + IM, ih[0], ih[1], ih[2], ih[3]);
+    sts128(sB + UM_A_BYTES, rl[0], rl[1], rl[2], rl[3]);
+    sts128(sB + UM_A_BYTES + IM, il[0], il[1], il[2], il[3]);
+    sts128(sB + 2 * UM_A_BYTES, rv[0], rv[1], rv[2], rv[3]);
+    sts128(sB + 2 * UM_A_BYTES + IM, iv[0], iv[1], iv[2], iv[3]);
+}
+
+// Drain 32 accumulator columns (one series, one of Re / Im) of this warp's 32 TMEM lanes into one plane of ws:
+// thread = lane = fine value h, column l is frequency k0 + 64 l (coalesced over the lanes).
+__device__ __forceinline__ void ud_drain(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, bool live)
+{
+    #pragma unroll 1
+    for (int part = 0; part < 2; ++part) {
+        float v[16];
+        tmem_ld16(taddr + 16u * part, v);
+        if (!live) continue;
+        const int64_t kp = k0 + (int64_t)part * 16 * UD_H;
+        if (!first) {
+            #pragma unroll
+            for (int i = 0; i < 16; ++i) { const int64_t k = kp + (int64_t)i * UD_H; if (k < Nf) v[i] += dst[k]; }
+        }
+        #pragma unroll
+        for (int i = 0; i < 16; ++i) { const int64_t k = kp + (int64_t)i * UD_H; if (k < Nf) dst[k] = v[i]; }
+    }
+}
+
+struct UmmaDuoParams {
+    UmmaParams u;                   // u.nfb = ceil(Nf / 2,048)
+    int64_t B;                      // series in the batch; the CTA's second series may not exist (odd B)
+};
+
+// grid.x = ceil(B / 2) * nsplit * nfb (frequency block fastest), US_THREADS threads, UD_SMEM bytes, two CTAs per SM.
+__global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const UmmaDuoParams q)
+{
+    const UmmaParams& p = q.u;
+    extern __shared__ __align__(128) unsigned char um_smem[];
+    float4* rec_all = reinterpret_cast<float4*>(um_smem + UD_STAGES * UD_STAGE_BYTES);            // [series][2][UM_TS] {X/sigma, pA32, v32, w32}
+    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * UD_STAGES + 2);
+
+    const unsigned tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
+    int64_t unit = blockIdx.x;
+    const int fb = (int)(unit % p.nfb); unit /= p.nfb;
+    const int sp = (int)(unit % p.nsplit);
+    const int64_t bp = unit / p.nsplit;
+    const int64_t kb = (int64_t)fb * UD_FPB;
+    const int64_t j_begin = (int64_t)sp * p.split_len;
+    const int64_t j_end = min(p.Nt, j_begin + p.split_len);
+    const int64_t n_samp = j_end - j_begin;
+    const int nks = (int)((n_samp + UM_KS - 1) / UM_KS);
+    const int flush_ksteps = max(1, p.flush_ksteps);
+
+    const uint32_t s_stage = smem_u32(um_smem), s_bar = smem_u32(bars);
+    const uint32_t bar_accf = s_bar + 8u * (2 * UD_STAGES), bar_acce = bar_accf + 8u;
+#define UD_FULL(s) (s_bar + 8u * (unsigned)(s))
+#define UD_EMPTY(s) (s_bar + 8u * (unsigned)(UD_STAGES + (s)))
+
+    if (tid == 0) {
+        for (int s = 0; s < UD_STAGES; ++s) { mbar_init(UD_FULL(s), US_GEN_WARPS); mbar_init(UD_EMPTY(s), 1); }
+        mbar_init(bar_accf, 1);
+        mbar_init(bar_acce, US_GEN_WARPS);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (w == US_GEN_WARPS) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"(smem_u32(tmem_slot)), "r"((uint32_t)UD_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
+
+    if (w < US_GEN_WARPS) {
+        // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
+        // record loader role: thread tid -> series tid >> 7, sample tid & 127 of the tile
+        const unsigned ls = tid >> 7, lj = tid & 127u;
+        const int64_t lb = 2 * bp + ls;
+        const bool l_live = lb < q.B;
+        const float4* recA = p.recA + (l_live ? lb : 0) * p.Nt;
+        const ulonglong2* recB = p.recB + (l_live ? lb : 0) * p.Nt;
+        const float xs = l_live ? (p.unit_x ? 1.f : x_scale(p.part_var + lb * p.nparts, p.nparts, p.Nt)) : 0.f;
+        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
+        auto prefetch = [&](int ti) {
+            const int64_t j = j_begin + (int64_t)ti * UM_TS + lj;
+            pre_ok = l_live && (j < j_end);
+            if (pre_ok) { pre_x = __ldg(&recA[j].x); const ulonglong2 r = __ldg(recB + j); pre_u = r.x; pre_v = r.y; }
+        };
+        prefetch(0);
+        // A task: row m = tid & 127 = (series m >> 6, fine value m & 63), 4 samples `chunk` of the k-step
+        const unsigned m = tid & 127u, a_s = m >> 6, a_h = m & 63u;
+        const int chunk = (int)(tid >> 7);
+        // drain role: TMEM lane quadrant q4 (series q4 >> 1), Re (0) / Im (1) columns of that series' diagonal block
+        const unsigned q4 = w & 3u, part = w >> 2, d_s = q4 >> 1;
+        const int64_t db = 2 * bp + d_s;
+        const bool d_live = db < q.B;
+        float* ws_unit = p.ws + (((d_live ? db : 0) * p.nsplit + sp) * 4) * p.Nf;
+        const int64_t k0 = kb + (int64_t)((32u * q4 + lane) & 63u);
+        const uint32_t t_drain = tmem + ((32u * q4) << 16) + 64u * d_s + (uint32_t)UD_L * part;
+        int kin = 0, flushes = 0;
+
+        for (int ks = 0; ks < nks; ++ks) {
+            const int s = ks & (UD_STAGES - 1);
+            const uint32_t ph = (uint32_t)(ks / UD_STAGES) & 1u;
+            const int ti = ks >> 4;
+            if ((ks & 15) == 0) {                                       // next record tile of both series (buffer ti & 1)
+                float4 r = make_float4(0.f, 0.f, 0.f, 0.f);             // pad: X = 0, phases 0
+                if (pre_ok) {
+                    const u64 pa = pre_u + (u64)kb * pre_v;             // u + kb v (mod 1, 64-bit wrap; reading G3)
+                    r.x = pre_x * xs;
+                    r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
+                    r.z = __uint_as_float((unsigned)((pre_v + 0x80000000ull) >> 32));
+                    r.w = __uint_as_float((unsigned)(((u64)UD_H * pre_v + 0x80000000ull) >> 32));
+                }
+                rec_all[(ls * 2 + (ti & 1)) * UM_TS + lj] = r;
+                prefetch(ti + 1);
+                asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            }
+            mbar_wait(UD_EMPTY(s), ph ^ 1u);                            // the MMAs that read this stage have completed
+            const int sb = (ks & 15) * UM_KS;
+            const uint32_t st = s_stage + (uint32_t)s * UD_STAGE_BYTES;
+            um_gen_a(rec_all + (a_s * 2 + (ti & 1)) * UM_TS, sb + chunk * 4, a_h, st + chunk * (UM_A_BYTES / 2) + m * 16,
+                     n_samp - ((int64_t)ks * UM_KS + chunk * 4));
+            const unsigned bt = (tid - (unsigned)ks * 128u) & 255u;     // the 128 B tasks rotate over the 256 producer threads
+            if (bt < 128u) {
+                const unsigned b_s = bt >> 6, bc = (bt >> 5) & 1u, l = bt & 31u;
+                ud_gen_b(rec_all + (b_s * 2 + (ti & 1)) * UM_TS, sb + (int)bc * 4, l,
+                         st + 3 * UM_A_BYTES + bc * (UM_A_BYTES / 2) + (b_s * 64u + l) * 16u);
+            }
+            fence_proxy_async();                                        // generic-proxy stores -> visible to the tensor core
+            __syncwarp();
+            if (lane == 0) mbar_arrive(UD_FULL(s));
+
+            const bool last = (ks == nks - 1);
+            if (++kin == flush_ksteps || last) {
+                mbar_wait(bar_accf, (uint32_t)flushes & 1u);            // every MMA issued so far has completed
+                tc_fence_after();
+                ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live);
+                if (last) ud_drain(t_drain + 128u, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true, d_live);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_acce);
+                ++flushes; kin = 0;
+            }
+        }
+    } else if (lane == 0) {
+        // ===================== step 4: the single MMA-issuing thread =====================
+        int kin = 0, flushes = 0;
+        for (int ks = 0; ks < nks; ++ks) {
+            const int s = ks & (UD_STAGES - 1);
+            const uint32_t ph = (uint32_t)(ks / UD_STAGES) & 1u;
+            mbar_wait(UD_FULL(s), ph);
+            tc_fence_after();
+            const uint32_t a0 = s_stage + (uint32_t)s * UD_STAGE_BYTES, b0 = a0 + 3 * UM_A_BYTES;
+            const uint64_t dAh = umma_desc(a0, UM_A_BYTES / 2, 128), dAl = umma_desc(a0 + UM_A_BYTES, UM_A_BYTES / 2, 128);
+            const uint64_t dAv = umma_desc(a0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
+            const uint64_t dBh = umma_desc(b0, UM_A_BYTES / 2, 128), dBl = umma_desc(b0 + UM_A_BYTES, UM_A_BYTES / 2, 128);
+            const uint64_t dBv = umma_desc(b0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
+            tc_mma_f16(tmem, dAh, dBh, UD_IDESC, kin > 0 ? 1u : 0u);
+            tc_mma_f16(tmem, dAl, dBh, UD_IDESC, 1u);
+            tc_mma_f16(tmem, dAh, dBl, UD_IDESC, 1u);
+            tc_mma_f16(tmem + 128u, dAv, dBv, UD_IDESC, ks > 0 ? 1u : 0u);
+            tc_commit(UD_EMPTY(s));
+            const bool last = (ks == nks - 1);
+            if (++kin == flush_ksteps || last) {
+                tc_commit(bar_accf);
+                if (!last) { mbar_wait(bar_acce, (uint32_t)flushes & 1u); tc_fence_after(); }
+                ++flushes; kin = 0;
+            }
+        }
+    }
+#undef UD_FULL
+#undef UD_EMPTY
+
+    tc_fence_before();
+    __syncthreads();
+    if (w == US_GEN_WARPS) {
+        __syncwarp();
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"((uint32_t)UD_TMEM_COLS) : "memory");
+    }
+}
+
+}  // namespace lsp

@@ -380,6 +380,36 @@ def test_shared_time_gemm(lsp, B, Nt, Nf):
         assert _same_peak(out[2][b], Pref[b])
 
 
+@pytest.mark.parametrize("B,Nt,Nf,nsplit", [(5, 900, 2100, 0), (2, 1500, 2000, 0), (7, 3000, 5000, 2), (3, 600, 700, 0)])
+@pytest.mark.parametrize("gls", [False, True])
+def test_two_series_per_cta_form(lsp, B, Nt, Nf, nsplit, gls):
+    """accum_umma_duo_kernel: two series x 64 fine x 32 coarse per CTA (the batch form of the 2,048-frequency tile);
+    odd B (the last CTA's second series does not exist), several frequency blocks and time splits, and the unit-weight
+    second pass of the generalised periodogram."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=300 + B)
+    if gls:
+        Pref = np.stack([oracle.periodogram_gls(w.t[b], w.x[b], w.f_min, w.df, w.Nf) for b in range(B)])
+    else:
+        Pref, _, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
+    keys = {pkg.PARAM_DUO: 2, pkg.PARAM_RECURRENCE: 5, pkg.PARAM_COARSE: 16, pkg.PARAM_NSPLIT: nsplit}
+    for k, v in keys.items():
+        h.set_param(k, v)
+    try:
+        P, pi, pv = h.periodogram_batched(torch.from_numpy(w.t).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf, gls=gls)
+        torch.cuda.synchronize()
+        assert "duo" in h.last_plan()["kernel"]
+    finally:
+        for k in keys:
+            h.set_param(k, 0)
+    P = P.cpu().numpy()
+    for b in range(B):
+        _check(P[b], Pref[b], "duo series %d" % b)
+        assert _same_peak(P[b], Pref[b])
+    assert np.array_equal(pi.cpu().numpy(), P.argmax(axis=1).astype(np.int32))
+
+
 def test_batch_of_one_equals_single(lsp):
     import torch
     pkg, h = lsp

@@ -264,7 +264,11 @@ int run_device(lsp_ctx* h,
                                    : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
                                                  : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
 
-    if (duo) pl.kernel_name = "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>";
+    // one CTA sees all samples of its series in one drain window: steps 6-7 run in its epilogue, no workspace round trip
+    const bool duo_fuse = duo && !gls && pl.nsplit == 1 && Nt <= (h->opt_flush ? h->opt_flush : 2048);
+    if (duo) pl.kernel_name = duo_fuse ? "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32,fused-finish>"
+                                       : "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>";
+    if (duo_fuse) pl.launches = 3;
 
     // workspace carve-up
     const size_t n_samp = (size_t)B * (size_t)Nt;
@@ -362,6 +366,8 @@ int run_device(lsp_ctx* h,
         if (duo) {
             UmmaDuoParams dp;
             dp.u = up; dp.B = B;
+            dp.fuse = duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
+            dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
             LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
             accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
         } else if (umma_small) {
@@ -422,6 +428,11 @@ int run_device(lsp_ctx* h,
 
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
 
+    if (duo_fuse) {
+        if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
+        h->plan = pl;
+        return LSP_OK;
+    }
     // steps 6-7
     FinishParams fp;
     fp.ws = ws; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;

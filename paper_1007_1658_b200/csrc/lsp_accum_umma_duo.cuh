@@ -77,7 +77,80 @@ __device__ __forceinline__ void ud_drain(uint32_t taddr, float* dst, int64_t k0,
 struct UmmaDuoParams {
     UmmaParams u;                   // u.nfb = ceil(Nf / 2,048)
     int64_t B;                      // series in the batch; the CTA's second series may not exist (odd B)
+    // fused steps 6-7: when one CTA sees ALL samples of its series in one drain window (nsplit = 1, Nt <= the drain interval)
+    // its accumulators are the sums of eq. (8), and every thread holds XC, XS, CC - n/2, CS of its frequencies.
+    int fuse;
+    float* P; int64_t p_stride;     // nullable
+    int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
 };
+
+// 32 lanes x 8 consecutive columns of fp32 accumulators -> 8 registers per thread.
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float (&v)[8])
+{
+    uint32_t r[8];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    #pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
+// thread = fine value h of series `db`; 16 coarse values l0..l0+15 -> frequencies kb + 64 l + h.
+__device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tbase, int64_t db, bool live, int64_t kh, unsigned l0, unsigned lane)
+{
+    const UmmaParams& p = q.u;
+    u64 best = 0ull;
+    double inv2var = 0.0;
+    const double Nt = (double)p.Nt;
+    if (live) {
+        double qv = 0.0;
+        for (int i = 0; i < p.nparts; ++i) qv += p.part_var[db * p.nparts + i];
+        double var = qv / (double)(p.Nt - 1);                           // sample variance (reading G1)
+        const double sc = (double)(float)(1.0 / sqrt(var));             // X was scaled by the fp32 x_scale(): undo it exactly
+        var *= sc * sc;
+        inv2var = 0.5 / var;
+    }
+    #pragma unroll 1
+    for (unsigned c8 = 0; c8 < 16; c8 += 8) {
+        float xc[8], xs[8], cc[8], cs[8];
+        tmem_ld8(tbase + c8, xc);
+        tmem_ld8(tbase + c8 + (uint32_t)UD_L, xs);
+        tmem_ld8(tbase + c8 + 128u, cc);
+        tmem_ld8(tbase + c8 + 128u + (uint32_t)UD_L, cs);
+        if (!live) continue;
+        #pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;
+            if (k >= p.Nf) continue;
+            const double XC = (double)xc[i], XS = (double)xs[i], A = 2.0 * (double)cc[i], Bv = 2.0 * (double)cs[i];
+            const double R2 = A * A + Bv * Bv, xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
+            const double DR = (xc2 - xs2) * A + 2.0 * XC * XS * Bv;
+            double val;
+            if (R2 < (1.0 - 1e-6) * (1.0 - 1e-6) * Nt * Nt) val = fmax(2.0 * (S * Nt - DR), 0.0) / (Nt * Nt - R2);
+            else { const double R = sqrt(R2); val = fmax(S + DR / R, 0.0) / (Nt + R); }      // reading G7
+            const float Pf = (float)(val * inv2var);
+            if (q.P) q.P[db * q.p_stride + k] = Pf;
+            const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+            best = (key > best) ? key : best;
+        }
+    }
+    if (q.peak_idx == nullptr) return;
+    #pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { const u64 other = __shfl_down_sync(0xffffffffu, best, o); best = (other > best) ? other : best; }
+    if (lane == 0 && live) {                                            // step 7: order-free packed arg-max, lowest k on ties (reading G9)
+        atomicMax(q.peak64 + db, best);
+        __threadfence();
+        const unsigned done = atomicAdd(q.counter + db, 1u);
+        if (done == 4u * (unsigned)p.nfb - 1u) {                        // 4 warps per series per frequency block: the last one publishes
+            __threadfence();
+            const u64 fin = atomicMax(q.peak64 + db, 0ull);
+            q.peak_idx[db] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
+            q.peak_val[db] = __uint_as_float((unsigned)(fin >> 32));
+        }
+    }
+}
 
 // grid.x = ceil(B / 2) * nsplit * nfb (frequency block fastest), US_THREADS threads, UD_SMEM bytes, two CTAs per SM.
 __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const UmmaDuoParams q)
@@ -185,8 +258,12 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             if (++kin == flush_ksteps || last) {
                 mbar_wait(bar_accf, (uint32_t)flushes & 1u);            // every MMA issued so far has completed
                 tc_fence_after();
+                if (q.fuse) {                                           // (host guarantees: this is the only drain of the CTA)
+                    ud_finish16(q, tmem + ((32u * q4) << 16) + 64u * d_s + 16u * part, db, d_live, k0, 16u * part, lane);
+                } else {
                 ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live);
                 if (last) ud_drain(t_drain + 128u, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true, d_live);
+                }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_acce);

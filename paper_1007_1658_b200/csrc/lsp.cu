@@ -390,7 +390,7 @@ int run_device(lsp_ctx* h,
                 LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UP_SMEM));
                 LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)U2_SMEM));
                 cudaLaunchConfig_t cfg = {};
-                cfg.gridDim = dim3((unsigned)units); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = pair2 ? U2_SMEM : UP_SMEM; cfg.stream = st;
+                cfg.gridDim = dim3((unsigned)units); cfg.blockDim = dim3(pair2 ? U2_THREADS : UM_THREADS); cfg.dynamicSmemBytes = pair2 ? U2_SMEM : UP_SMEM; cfg.stream = st;
                 cudaLaunchAttribute at[1];
                 at[0].id = cudaLaunchAttributeClusterDimension;
                 at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;

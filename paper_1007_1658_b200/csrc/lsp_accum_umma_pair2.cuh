@@ -27,8 +27,14 @@ namespace lsp {
 
 constexpr int U2_FPP = 256 * UM_H;                                // frequencies per CTA pair
 constexpr int U2_HC = 64;                                         // coarse values generated per CTA
-constexpr int U2_GROUP_WARPS = UM_GEN_WARPS / 2;                  // producer warps per group
-constexpr int U2_REC_BYTES = 2 * 2 * UM_TS * 16;                  // [group][buffer][128 samples] records
+#ifndef LSP_U2_GROUPS
+#define LSP_U2_GROUPS 2
+#endif
+constexpr int U2_GROUPS = LSP_U2_GROUPS;                          // producer groups: group g owns the stage-steps it = g (mod U2_GROUPS)
+constexpr int U2_GROUP_WARPS = 8;                                 // producer warps per group (one stage-step = 256 thread-tasks)
+constexpr int U2_PROD_WARPS = U2_GROUPS * U2_GROUP_WARPS;         // warps 0..15 also drain; warp U2_PROD_WARPS issues the MMAs
+constexpr int U2_THREADS = (U2_PROD_WARPS + 1) * 32;
+constexpr int U2_REC_BYTES = U2_GROUPS * 2 * UM_TS * 16;          // [group][buffer][128 samples] records
 constexpr size_t U2_SMEM = (size_t)UP_STAGES * UP_STAGE_BYTES + U2_REC_BYTES + 256;
 
 // ------------------------------------------------------------------ pre-pass: the fine-operand table
@@ -125,7 +131,7 @@ __device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k
 // ------------------------------------------------------------------ the kernel
 // grid.x = B * nsplit * (2 * npairs) (CTA of the pair fastest, then the pair), clusters of 2, UM_THREADS threads,
 // U2_SMEM bytes of dynamic shared memory, one CTA per SM.  q.u.nfb = 2 * npairs, npairs = ceil(Nf / 32,768).
-__global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const UmmaPairParams q)
+__global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const UmmaPairParams q)
 {
     const UmmaParams& p = q.u;
     extern __shared__ __align__(128) unsigned char um_smem[];
@@ -161,7 +167,7 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const U
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cluster_sync_all();
-    if (w == UM_GEN_WARPS) {
+    if (w == U2_PROD_WARPS) {
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;"
                      :: "r"(smem_u32(tmem_slot)), "r"((uint32_t)UM_TMEM_COLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
@@ -172,7 +178,7 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const U
     const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
     cluster_sync_all();
 
-    if (w < UM_GEN_WARPS) {
+    if (w < U2_PROD_WARPS) {
         // ===================== producers: generated operand (step 3), TMA of this CTA's table rows, drain (step 5) =====================
         const unsigned grp = w >> 3, tg = tid & 255u;                   // group `grp` owns the stage-steps it = grp (mod 2)
         float4* rec = rec_all + grp * (2 * UM_TS);
@@ -200,7 +206,8 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const U
 
         for (int f = 0; f < nwin; ++f) {
             const int it_end = min(nst, (f + 1) * flush_st);
-            for (int it = f * flush_st + (int)grp; it < it_end; it += 2) {
+            const int it0 = f * flush_st;
+            for (int it = it0 + ((int)grp + U2_GROUPS - it0 % U2_GROUPS) % U2_GROUPS; it < it_end; it += U2_GROUPS) {
                 const int s = it & (UP_STAGES - 1);
                 const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
                 const int ti = it >> 3;                                 // 8 stage-steps per record tile
@@ -217,8 +224,7 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const U
                         rec[(ti & 1) * UM_TS + tg] = r;
                         prefetch(ti + 1);
                     }
-                    if (grp == 0) asm volatile("bar.sync 1, 256;" ::: "memory");
-                    else asm volatile("bar.sync 2, 256;" ::: "memory");
+                    asm volatile("bar.sync %0, 256;" :: "r"(1u + grp) : "memory");
                 }
                 mbar_wait(U2_EMPTY(s), ph ^ 1u);                        // the pair's MMAs that read this stage have completed
                 const uint32_t st = s_stage + (uint32_t)s * UP_STAGE_BYTES;
@@ -234,7 +240,8 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const U
                 __syncwarp();
                 if (lane == 0) mbar_arrive(U2_FULL(s));
             }
-            // ---- drain window f (all 16 warps of both CTAs)
+            // ---- drain window f (warps 0..15 of both CTAs)
+            if (w >= UM_GEN_WARPS) continue;
             const bool last = (f == nwin - 1);
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
@@ -290,7 +297,7 @@ __global__ void __launch_bounds__(UM_THREADS, 1) accum_umma_pair2_kernel(const U
     __syncwarp();
     tc_fence_before();
     cluster_sync_all();
-    if (w == UM_GEN_WARPS) {
+    if (w == U2_PROD_WARPS) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"((uint32_t)UM_TMEM_COLS) : "memory");
     }

@@ -344,6 +344,18 @@ def run_ours(args):
         "roofline": roofline,
         "cpu_baseline": cpu,
     }
+    if batched:
+        # BASELINE config 4: "report per-series peak power distribution" -- the peaks the last host-buffer step returned,
+        # and their false-alarm probabilities by eq. (3) with N_ind = Nf (lsp_false_alarm)
+        pv = pv_h.numpy().astype(np.float64)
+        fap = h.false_alarm(pv_h.cuda(), w.Nt, float(w.Nf)).cpu().numpy().astype(np.float64)
+        q = np.quantile(pv, [0.05, 0.25, 0.5, 0.75, 0.95])
+        line["peak_power_distribution"] = {
+            "series": int(pv.size), "mean": float(pv.mean()), "std": float(pv.std()), "min": float(pv.min()), "max": float(pv.max()),
+            "q05": float(q[0]), "q25": float(q[1]), "q50": float(q[2]), "q75": float(q[3]), "q95": float(q[4]),
+            "mean_power_all_bins": float(P_h.numpy().mean(dtype=np.float64)),
+            "false_alarm_eq3_median": float(np.median(fap)), "fraction_with_fap_below_0.01": float((fap < 0.01).mean()),
+        }
     print(json.dumps(line))
     h.close()
     if world > 1:

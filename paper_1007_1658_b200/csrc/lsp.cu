@@ -158,11 +158,10 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
 
     const size_t n_samp = (size_t)B * (size_t)Nt;
     size_t off = 0;
-    const size_t o_recA = off; off = align_up(off + n_samp * sizeof(float4), 256);
-    const size_t o_recB = off; off = align_up(off + n_samp * sizeof(ulonglong2), 256);
+    const size_t o_recA = off;                            // (no per-sample records per series on this path)
+    const size_t o_recB = off; off = align_up(off + (size_t)Nt * sizeof(ulonglong2), 256);   // phases of the one time vector
     const size_t o_xa = off;   off = align_up(off + (size_t)nmb * ng * SG_A_GROUP, 256);
     const size_t o_eb = off;   off = align_up(off + (size_t)nfb * ng * SG_B_GROUP, 256);
-    const size_t o_pv = off;   off = align_up(off + (size_t)ng * 4 * (size_t)Nf * sizeof(float), 256);
     const size_t o_wsv = off;  off = align_up(off + (size_t)nsplit * 4 * (size_t)Nf * sizeof(float), 256);
     const bool fuse = (nsplit == 1);                      // one split: the GEMM's accumulators are the sums; steps 6-7 run in its epilogue
     const size_t o_wsx = off;  if (!fuse) off = align_up(off + (size_t)B * nsplit * 2 * (size_t)x_row * sizeof(float), 256);
@@ -178,7 +177,6 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
     unsigned char* xa = reinterpret_cast<unsigned char*>(base + o_xa);
     unsigned char* eb = reinterpret_cast<unsigned char*>(base + o_eb);
-    float* part_v = reinterpret_cast<float*>(base + o_pv);
     float* ws_v = reinterpret_cast<float*>(base + o_wsv);
     float* ws_x = reinterpret_cast<float*>(base + o_wsx);
     double* vconst = reinterpret_cast<double*>(base + o_vc);
@@ -202,15 +200,15 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     records_kernel<true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar);
     LSP_CUDA(h, cudaGetLastError());
     // step 3 for every (sample, frequency) once; CC, CS once per frequency
-    shared_e_kernel<<<dim3((unsigned)nfb, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng, part_v);
+    shared_e_kernel<<<dim3((unsigned)nfb, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng);
     LSP_CUDA(h, cudaGetLastError());
-    shared_v_reduce_kernel<<<dim3((unsigned)((Nf + 255) / 256), (unsigned)nsplit), 256, 0, st>>>(part_v, Nf, (int)gps, ws_v);
+    shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
     LSP_CUDA(h, cudaGetLastError());
     if (fuse) {
         shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst);
         LSP_CUDA(h, cudaGetLastError());
     }
-    shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(recA, pvar, pl.nparts, B, Nt, xa, (int)ng);
+    shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(x, x_stride, psum, pvar, pl.nparts, B, Nt, xa, (int)ng);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
     // steps 4-5: the contraction

@@ -59,14 +59,14 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
         const double d = (double)__ldg(xb + j) - mean;
         acc += d * d;
         const int64_t o = (int64_t)b * Nt + j;
-        if (SHARED && b != 0) { recA[o] = make_float4((float)d, 0.f, 0.f, 0.f); continue; }
+        if (SHARED && b != 0) continue;                     // shared-time batch: only the variance is needed per series
         const double tp = __ldg(tb + j) - t0;
         double vfrac;
         const u64 u = frac_fixed64(f_min, tp, nullptr);
         const u64 v = frac_fixed64(df, tp, &vfrac);
         double sd = 0.0, cd = 0.0;
         if (!SHARED) sincospi(2.0 * vfrac, &sd, &cd);      // accurate: its error is applied K times per run
-        recA[o] = make_float4((float)d, (float)cd, (float)sd, (float)(2.0 * cd));
+        if (!SHARED) recA[o] = make_float4((float)d, (float)cd, (float)sd, (float)(2.0 * cd));
         recB[o] = make_ulonglong2(u, v);
     }
     acc = block_sum(acc, red);

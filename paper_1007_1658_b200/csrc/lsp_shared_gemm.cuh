@@ -9,8 +9,8 @@
 //
 // Pre-passes (all O(Nt (Nf + B))):
 //   shared_e_kernel   E as tcgen05 B-operand tiles (no-swizzle K-major core matrices, fp16 plane + e5m2 plane), one
-//                     MUFU sin/cos per (sample, frequency); the same threads also sum cos^2 - 1/2 and cos sin of their 8
-//                     samples (fp32), which shared_v_reduce_kernel folds in fixed order into CC - n/2, CS per time split.
+//                     MUFU sin/cos per (sample, frequency).
+//   shared_v_kernel   CC - n/2, CS per frequency and time split (one warp each, fixed shuffle tree).
 //   shared_x_kernel   X / sigma_b as A-operand tiles (fp16 plane + e5m2 plane).
 // shared_gemm_kernel  a TMA-fed tcgen05 GEMM: CTA tile 128 series x 128 frequencies (N = 256) x one time split; one
 //                     thread streams the pre-tiled operands with cp.async.bulk (48 KB per stage of 32 samples, 4 stages),
@@ -70,15 +70,13 @@ __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restr
 
 // ------------------------------------------------------------------ E tiles + partial CC, CS
 // grid (nfb, ng), 256 threads: kf = tid & 127 (frequency k = 128 nfb + kf), chunk = tid >> 7 (8 of the group's 16 samples).
-// part_v[(g*2 + chunk)][2][Nf]: sum over the 8 samples of cos^2 - 1/2 and cos sin.
 __global__ void __launch_bounds__(256) shared_e_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t Nf,
-                                                       unsigned char* __restrict__ eb, int ng, float* __restrict__ part_v)
+                                                       unsigned char* __restrict__ eb, int ng)
 {
     const int nb = blockIdx.x, g = blockIdx.y;
     const unsigned kf = threadIdx.x & 127u, chunk = threadIdx.x >> 7;
     const int64_t k = (int64_t)nb * SG_F + kf;
     float c[8], s[8];
-    float cc = 0.f, cs = 0.f;
     #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int64_t j = (int64_t)g * SG_KS + chunk * 8 + i;
@@ -87,8 +85,6 @@ __global__ void __launch_bounds__(256) shared_e_kernel(const ulonglong2* __restr
             const ulonglong2 r = __ldg(recB + j);
             const u64 ph = r.x + (u64)k * r.y;                          // u + k v (mod 1, exact 64-bit wrap; reading G3)
             sincos_phase32((unsigned)((ph + 0x80000000ull) >> 32), c[i], s[i]);
-            cc += fmaf(c[i], c[i], -0.5f);
-            cs = fmaf(c[i], s[i], cs);
         }
     }
     unsigned ch[4], sh[4], c8h[2], s8h[2], c8l[2], s8l[2];
@@ -110,29 +106,39 @@ __global__ void __launch_bounds__(256) shared_e_kernel(const ulonglong2* __restr
     o[row_s] = make_uint4(sh[0], sh[1], sh[2], sh[3]);
     o[PLANE + row_c] = make_uint4(c8h[0], c8h[1], c8l[0], c8l[1]);      // E_8 = [e5m2(E_hi) | e5m2(E_lo)]
     o[PLANE + row_s] = make_uint4(s8h[0], s8h[1], s8l[0], s8l[1]);
-    if (k < Nf) {
-        float* pv = part_v + ((int64_t)g * 2 + chunk) * 2 * Nf;
-        pv[k] = cc;
-        pv[Nf + k] = cs;
-    }
 }
 
-// ws_v[split][4][Nf], planes 2, 3 = CC - n/2, CS of the split (planes 0, 1 unused): fixed-order sum of the partials.
-__global__ void __launch_bounds__(256) shared_v_reduce_kernel(const float* __restrict__ part_v, int64_t Nf, int groups_per_split, float* __restrict__ ws_v)
+// CC - n/2 and CS once per frequency (eq. (8); SS = Nt - CC, :130): ws_v[split][4][Nf], planes 2, 3 (0, 1 unused).
+// One warp per (frequency, time split): lane = sample mod 32, fp32 partials, fixed shuffle tree (deterministic).
+// grid (ceil(Nf / 8), nsplit), 256 threads.
+__global__ void __launch_bounds__(256) shared_v_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t Nf, int64_t split_len, float* __restrict__ ws_v)
 {
-    const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    const int64_t k = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const unsigned lane = threadIdx.x & 31u;
     const int sp = blockIdx.y;
     if (k >= Nf) return;
+    const int64_t j1 = min(Nt, (int64_t)(sp + 1) * split_len);
     float cc = 0.f, cs = 0.f;
-    const float* pv = part_v + (int64_t)sp * groups_per_split * 2 * 2 * Nf;
-    for (int i = 0; i < 2 * groups_per_split; ++i) { cc += pv[(int64_t)i * 2 * Nf + k]; cs += pv[(int64_t)i * 2 * Nf + Nf + k]; }
-    ws_v[((int64_t)sp * 4 + 2) * Nf + k] = cc;
-    ws_v[((int64_t)sp * 4 + 3) * Nf + k] = cs;
+    for (int64_t j = (int64_t)sp * split_len + lane; j < j1; j += 32) {
+        const ulonglong2 r = __ldg(recB + j);
+        const u64 ph = r.x + (u64)k * r.y;                              // u + k v (mod 1, exact 64-bit wrap; reading G3)
+        float c, s;
+        sincos_phase32((unsigned)((ph + 0x80000000ull) >> 32), c, s);
+        cc += fmaf(c, c, -0.5f);
+        cs = fmaf(c, s, cs);
+    }
+    #pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { cc += __shfl_down_sync(0xffffffffu, cc, o); cs += __shfl_down_sync(0xffffffffu, cs, o); }
+    if (lane == 0) {
+        ws_v[((int64_t)sp * 4 + 2) * Nf + k] = cc;
+        ws_v[((int64_t)sp * 4 + 3) * Nf + k] = cs;
+    }
 }
 
 // ------------------------------------------------------------------ X tiles
 // grid (nmb, ng), 256 threads: row = tid & 127 (series b = 128 nmb + row), chunk = tid >> 7.
-__global__ void __launch_bounds__(256) shared_x_kernel(const float4* __restrict__ recA, const double* __restrict__ part_var, int nparts,
+__global__ void __launch_bounds__(256) shared_x_kernel(const float* __restrict__ x_in, int64_t x_stride, const double* __restrict__ part_sum,
+                                                       const double* __restrict__ part_var, int nparts,
                                                        int64_t B, int64_t Nt, unsigned char* __restrict__ xa, int ng)
 {
     const int mb = blockIdx.x, g = blockIdx.y;
@@ -140,10 +146,12 @@ __global__ void __launch_bounds__(256) shared_x_kernel(const float4* __restrict_
     const int64_t b = (int64_t)mb * SG_M + row;
     float x[8];
     const float xs = (b < B) ? x_scale(part_var + b * nparts, nparts, Nt) : 0.f;
+    double mean = 0.0;
+    if (b < B) { for (int i = 0; i < nparts; ++i) mean += part_sum[b * nparts + i]; mean /= (double)Nt; }   // PAPER.md:41, fixed order
     #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int64_t j = (int64_t)g * SG_KS + chunk * 8 + i;
-        x[i] = (b < B && j < Nt) ? __ldg(&recA[b * Nt + j].x) * xs : 0.f;
+        x[i] = (b < B && j < Nt) ? (float)((double)__ldg(x_in + b * x_stride + j) - mean) * xs : 0.f;    // X_j rounded to fp32 once (G4)
     }
     unsigned xh[4], x8h[2], x8l[2];
     #pragma unroll

@@ -107,3 +107,28 @@ def test_C4_batch_sampled(lsp):
     # pin P6 at full size: Gaussian noise => mean power 1, Gumbel-like peak distribution
     assert abs(P.mean() - 1.0) < 0.01
     assert 6.5 < pv.mean() < 9.0 and 0.8 < pv.std() < 1.8
+
+
+def test_C4S_shared_time_batch_sampled(lsp):
+    """C4's 4,096 noise series on ONE time vector (t_stride = 0): the dense-contraction path at full size, in the launch
+    configuration bench.py times (automatic: shared-time GEMM with steps 6-7 in its epilogue)."""
+    import torch
+    pkg, h = lsp
+    w = workloads.make("C4S")
+    t = torch.from_numpy(w.t).cuda()
+    x = torch.from_numpy(w.x).cuda()
+    P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
+    torch.cuda.synchronize()
+    assert "shared_gemm" in h.last_plan()["kernel"]
+    P = P.cpu().numpy(); pi = pi.cpu().numpy(); pv = pv.cpu().numpy()
+    assert np.all(np.isfinite(P)) and P.min() >= 0.0
+    assert np.array_equal(pi, P.argmax(axis=1).astype(np.int32))
+    assert np.array_equal(pv, P.max(axis=1))
+    for b in range(0, w.B, 64):
+        ref = oracle.periodogram(w.t, w.x[b], w.f_min, w.df, w.Nf)
+        err = np.max(np.abs(P[b] - ref))
+        assert err <= TOL * ref.max(), "series %d: %.3e" % (b, err)
+        i_ref = oracle.argmax(ref)
+        assert int(pi[b]) == i_ref or (ref[i_ref] - ref[int(pi[b])]) < 1e-5 * ref[i_ref], "series %d" % b
+    assert abs(P.mean() - 1.0) < 0.01                                   # pin P6 at full size
+    assert 6.5 < pv.mean() < 9.0 and 0.8 < pv.std() < 1.8

@@ -166,6 +166,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     const bool fuse = (nsplit == 1);                      // one split: the GEMM's accumulators are the sums; steps 6-7 run in its epilogue
     const size_t o_wsx = off;  if (!fuse) off = align_up(off + (size_t)B * nsplit * 2 * (size_t)x_row * sizeof(float), 256);
     const size_t o_vc = off;   off = align_up(off + (size_t)4 * (size_t)Nf * sizeof(double), 256);
+    const size_t o_vcf = off;  off = align_up(off + (size_t)Nf * sizeof(float4), 256);
     const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
@@ -180,6 +181,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     float* ws_v = reinterpret_cast<float*>(base + o_wsv);
     float* ws_x = reinterpret_cast<float*>(base + o_wsx);
     double* vconst = reinterpret_cast<double*>(base + o_vc);
+    float4* vconst_f = reinterpret_cast<float4*>(base + o_vcf);
     double* psum = reinterpret_cast<double*>(base + o_psum);
     double* pvar = reinterpret_cast<double*>(base + o_pvar);
     u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
@@ -205,7 +207,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
     LSP_CUDA(h, cudaGetLastError());
     if (fuse) {
-        shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst);
+        shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst, vconst_f);
         LSP_CUDA(h, cudaGetLastError());
     }
     shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(x, x_stride, psum, pvar, pl.nparts, B, Nt, xa, (int)ng);
@@ -215,7 +217,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     SharedGemmParams gp;
     gp.xa = xa; gp.eb = eb; gp.ws_x = ws_x; gp.B = B; gp.Nf = Nf; gp.x_row = x_row;
     gp.nmb = (int)nmb; gp.nfb = (int)nfb; gp.nsplit = (int)nsplit; gp.ng = (int)ng; gp.groups_per_split = (int)gps;
-    gp.vconst = fuse ? vconst : nullptr; gp.part_var = pvar; gp.P = P; gp.p_stride = p_stride;
+    gp.vconst = fuse ? vconst : nullptr; gp.vconst_f = vconst_f; gp.part_var = pvar; gp.P = P; gp.p_stride = p_stride;
     gp.peak_idx = peak_idx; gp.peak_val = peak_val; gp.peak64 = peak64; gp.counter = counter; gp.Nt = Nt; gp.nparts = pl.nparts;
     LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
     shared_gemm_kernel<<<(unsigned)(nmb * nfb * nsplit), SG_THREADS, SG_SMEM, st>>>(gp);

@@ -47,6 +47,7 @@ struct SharedGemmParams {
     int groups_per_split;           // even
     // fused steps 6-7 (only when nsplit == 1: the accumulators ARE the sums of eq. (8)); vconst == NULL: write ws_x instead
     const double* vconst;           // [4][Nf]: cos 2 w tau, sin 2 w tau, 1/(Nt + R), 1/(Nt - R) (0 if dropped, reading G7)
+    const float4* vconst_f;         // [Nf]: the same four as fp32, .x = NaN where R > Nt/2 (the difference S - D is then formed in fp64)
     const double* part_var;         // [B][nparts]
     float* P; int64_t p_stride;     // nullable
     int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
@@ -55,7 +56,8 @@ struct SharedGemmParams {
 
 // Per-frequency part of step 6 for the shared-time batch: from CC - n/2, CS (summed over the splits in fixed order)
 // A = CC - SS, B = 2 CS, R = hypot(A, B) -> (A/R, B/R, 1/(Nt + R), 1/(Nt - R)); eqs (5)-(7), tau eliminated.
-__global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restrict__ ws_v, int nsplit, int64_t Nf, int64_t Nt_i, double* __restrict__ vconst)
+__global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restrict__ ws_v, int nsplit, int64_t Nf, int64_t Nt_i, double* __restrict__ vconst,
+                                                            float4* __restrict__ vconst_f)
 {
     const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (k >= Nf) return;
@@ -66,6 +68,9 @@ __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restr
     vconst[Nf + k] = (R > 0.0) ? Bv / R : 0.0;
     vconst[2 * Nf + k] = 1.0 / (Nt + R);
     vconst[3 * Nf + k] = (Nt - R > 1e-6 * Nt) ? 1.0 / (Nt - R) : 0.0;
+    // fp32 copy for the common case R <= Nt/2 (1/(Nt - R) <= 3/(Nt + R): no amplification of the fp32 rounding of S - D)
+    vconst_f[k] = make_float4((R <= 0.5 * Nt) ? (float)vconst[k] : __int_as_float(0x7fc00000), (float)vconst[Nf + k],
+                              (float)vconst[2 * Nf + k], (float)vconst[3 * Nf + k]);
 }
 
 // ------------------------------------------------------------------ E tiles + partial CC, CS
@@ -169,6 +174,93 @@ __global__ void __launch_bounds__(256) shared_x_kernel(const float* __restrict__
     o[PLANE + r] = make_uint4(x8l[0], x8l[1], x8h[0], x8h[1]);         // X_8 = [e5m2(X_lo) | e5m2(X_hi)]
 }
 
+// ------------------------------------------------------------------ drain / fused steps 6-7 (shared by both GEMM kernels)
+// Called by the four drain warps after the accumulators are complete: q4 = TMEM lane quadrant of the warp.
+__device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tmem, unsigned q4, unsigned lane, int mb, int nb, int sp)
+{
+    // ===================== drain: thread = TMEM lane = series; 32 consecutive frequencies per tcgen05.ld =====================
+    const int64_t b = (int64_t)mb * SG_M + 32u * q4 + lane;
+    if (p.vconst) {
+        // ---- fused steps 6-7: P[b][k] from this thread's XC (column kf) and XS (column 128 + kf)
+        double inv2var = 0.0;
+        if (b < p.B) {
+            double qv = 0.0;
+            for (int i = 0; i < p.nparts; ++i) qv += p.part_var[b * p.nparts + i];
+            double var = qv / (double)(p.Nt - 1);                   // sample variance (reading G1)
+            const double xs = (double)(float)(1.0 / sqrt(var));     // X was scaled by the fp32 x_scale(): undo it exactly
+            var *= xs * xs;
+            inv2var = 0.5 / var;
+        }
+        const float inv2var_f = (float)inv2var;
+        u64 best = 0ull;
+        const bool p_vec = p.P && ((p.p_stride & 3) == 0) && ((reinterpret_cast<uintptr_t>(p.P) & 15) == 0);
+        #pragma unroll 1
+        for (int cc = 0; cc < 4; ++cc) {
+            float vc[32], vs[32];
+            tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, vc);
+            tmem_ld32(tmem + ((32u * q4) << 16) + 128u + 32u * cc, vs);
+            const int64_t k0 = (int64_t)nb * SG_F + cc * 32;
+            if (b >= p.B) continue;
+            float pf[32];
+            #pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                const int64_t k = k0 + i;
+                pf[i] = 0.f;
+                if (k < p.Nf) {
+                    const float4 cf = __ldg(p.vconst_f + k);            // same k for the whole warp: one broadcast load
+                    if (cf.x == cf.x) {                                 // R <= Nt/2: fp32 (relative error ~3e-7)
+                        const float xc2 = vc[i] * vc[i], xs2 = vs[i] * vs[i], S = xc2 + xs2;
+                        const float D = fmaf(xc2 - xs2, cf.x, 2.f * vc[i] * vs[i] * cf.y);
+                        pf[i] = fmaf(fmaxf(S + D, 0.f), cf.z, fmaxf(S - D, 0.f) * cf.w) * inv2var_f;
+                    } else {
+                        const double XC = (double)vc[i], XS = (double)vs[i];
+                        const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
+                        const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
+                        pf[i] = (float)((fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var);
+                    }
+                    const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+                    best = (key > best) ? key : best;
+                }
+            }
+            if (p.P) {
+                float* d = p.P + b * p.p_stride + k0;
+                if (p_vec && k0 + 32 <= p.Nf) {
+                    #pragma unroll
+                    for (int i = 0; i < 32; i += 4) *reinterpret_cast<float4*>(d + i) = make_float4(pf[i], pf[i + 1], pf[i + 2], pf[i + 3]);
+                } else {
+                    #pragma unroll
+                    for (int i = 0; i < 32; ++i) if (k0 + i < p.Nf) d[i] = pf[i];
+                }
+            }
+        }
+        if (p.peak_idx && b < p.B) {                                // step 7: order-free packed arg-max, lowest k on ties (reading G9)
+            atomicMax(p.peak64 + b, best);
+            __threadfence();
+            const unsigned done = atomicAdd(p.counter + b, 1u);
+            if (done == (unsigned)p.nfb - 1u) {                     // last frequency block of this series: publish
+                __threadfence();
+                const u64 fin = atomicMax(p.peak64 + b, 0ull);
+                p.peak_idx[b] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
+                p.peak_val[b] = __uint_as_float((unsigned)(fin >> 32));
+            }
+        }
+    } else {
+    float* dst = p.ws_x + ((b * p.nsplit + sp) * 2) * p.x_row;
+    #pragma unroll 1
+    for (int cc = 0; cc < 8; ++cc) {
+        float v[32];
+        tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, v);
+        const int64_t k0 = (int64_t)nb * SG_F + (cc & 3) * 32;
+        float* d = dst + (int64_t)(cc >> 2) * p.x_row + k0;
+        if (b < p.B) {
+            #pragma unroll
+            for (int i = 0; i < 32; i += 4)
+                if (k0 + i < p.x_row) *reinterpret_cast<float4*>(d + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+        }
+    }
+    }
+}
+
 // ------------------------------------------------------------------ the GEMM
 // grid.x = nmb * nfb * nsplit (frequency block fastest, then series block, then split), SG_THREADS threads,
 // SG_SMEM bytes of dynamic shared memory.
@@ -244,82 +336,9 @@ __global__ void __launch_bounds__(SG_THREADS, 2) shared_gemm_kernel(const Shared
         }
     } else {
         // ===================== drain: thread = TMEM lane = series; 32 consecutive frequencies per tcgen05.ld =====================
-        const unsigned q4 = w & 3u;
-        const int64_t b = (int64_t)mb * SG_M + 32u * q4 + lane;
         mbar_wait(bar_acc, 0u);
         tc_fence_after();
-        if (p.vconst) {
-            // ---- fused steps 6-7: P[b][k] from this thread's XC (column kf) and XS (column 128 + kf)
-            double inv2var = 0.0;
-            if (b < p.B) {
-                double qv = 0.0;
-                for (int i = 0; i < p.nparts; ++i) qv += p.part_var[b * p.nparts + i];
-                double var = qv / (double)(p.Nt - 1);                   // sample variance (reading G1)
-                const double xs = (double)(float)(1.0 / sqrt(var));     // X was scaled by the fp32 x_scale(): undo it exactly
-                var *= xs * xs;
-                inv2var = 0.5 / var;
-            }
-            u64 best = 0ull;
-            const bool p_vec = p.P && ((p.p_stride & 3) == 0) && ((reinterpret_cast<uintptr_t>(p.P) & 15) == 0);
-            #pragma unroll 1
-            for (int cc = 0; cc < 4; ++cc) {
-                float vc[32], vs[32];
-                tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, vc);
-                tmem_ld32(tmem + ((32u * q4) << 16) + 128u + 32u * cc, vs);
-                const int64_t k0 = (int64_t)nb * SG_F + cc * 32;
-                if (b >= p.B) continue;
-                float pf[32];
-                #pragma unroll
-                for (int i = 0; i < 32; ++i) {
-                    const int64_t k = k0 + i;
-                    pf[i] = 0.f;
-                    if (k < p.Nf) {
-                        const double XC = (double)vc[i], XS = (double)vs[i];
-                        const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
-                        const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
-                        const double val = (fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var;
-                        pf[i] = (float)val;
-                        const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
-                        best = (key > best) ? key : best;
-                    }
-                }
-                if (p.P) {
-                    float* d = p.P + b * p.p_stride + k0;
-                    if (p_vec && k0 + 32 <= p.Nf) {
-                        #pragma unroll
-                        for (int i = 0; i < 32; i += 4) *reinterpret_cast<float4*>(d + i) = make_float4(pf[i], pf[i + 1], pf[i + 2], pf[i + 3]);
-                    } else {
-                        #pragma unroll
-                        for (int i = 0; i < 32; ++i) if (k0 + i < p.Nf) d[i] = pf[i];
-                    }
-                }
-            }
-            if (p.peak_idx && b < p.B) {                                // step 7: order-free packed arg-max, lowest k on ties (reading G9)
-                atomicMax(p.peak64 + b, best);
-                __threadfence();
-                const unsigned done = atomicAdd(p.counter + b, 1u);
-                if (done == (unsigned)p.nfb - 1u) {                     // last frequency block of this series: publish
-                    __threadfence();
-                    const u64 fin = atomicMax(p.peak64 + b, 0ull);
-                    p.peak_idx[b] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
-                    p.peak_val[b] = __uint_as_float((unsigned)(fin >> 32));
-                }
-            }
-        } else {
-        float* dst = p.ws_x + ((b * p.nsplit + sp) * 2) * p.x_row;
-        #pragma unroll 1
-        for (int cc = 0; cc < 8; ++cc) {
-            float v[32];
-            tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, v);
-            const int64_t k0 = (int64_t)nb * SG_F + (cc & 3) * 32;
-            float* d = dst + (int64_t)(cc >> 2) * p.x_row + k0;
-            if (b < p.B) {
-                #pragma unroll
-                for (int i = 0; i < 32; i += 4)
-                    if (k0 + i < p.x_row) *reinterpret_cast<float4*>(d + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
-            }
-        }
-        }
+        sg_drain(p, tmem, w & 3u, lane, mb, nb, sp);
         tc_fence_before();
     }
 #undef SG_FULL

@@ -196,10 +196,14 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     }
     // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
-    moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
-    LSP_CUDA(h, cudaGetLastError());
+    const bool fused_pre = pl.nparts == 1;                // one block per series: step 1's sum inside the records kernel
+    if (!fused_pre) {
+        moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
+        LSP_CUDA(h, cudaGetLastError());
+    } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    records_kernel<true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar);
+    if (fused_pre) records_kernel<true, true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
+    else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
     // step 3 for every (sample, frequency) once; CC, CS once per frequency
     shared_e_kernel<<<dim3((unsigned)nfb, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng);
@@ -327,11 +331,14 @@ int run_device(lsp_ctx* h,
 
     // steps 1-2
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
-    moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
-    LSP_CUDA(h, cudaGetLastError());
+    const bool fused_pre = pl.nparts == 1;                // one block per series: step 1's sum inside the records kernel
+    if (!fused_pre) {
+        moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
+        LSP_CUDA(h, cudaGetLastError());
+    } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    records_kernel<false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df,
-                                         psum, recA, recB, pvar);
+    if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
+    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
     if (gls) {
         unit_records_kernel<<<(unsigned)((n_samp + 255) / 256), 256, 0, st>>>(recA, recA1, (int64_t)n_samp);

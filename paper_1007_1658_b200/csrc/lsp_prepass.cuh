@@ -33,13 +33,16 @@ __global__ void moments_kernel(const float* __restrict__ x, int64_t x_stride, in
 
 // grid (nb, B).  Writes recA, recB for the block's chunk and part_var[b][blk] = sum (x - mean)^2.
 // SHARED (shared-time batch, t_stride = 0): only X_j is needed per series, the phases only once (series 0).
-template <bool SHARED>
+// FUSED (one block per series, Nt <= 4,096): step 1's sum is formed here, exactly as moments_kernel forms it (same strided
+// partials, same reduction tree), so one launch is saved where launches are what a call costs (C1, C2, C4).
+template <bool SHARED, bool FUSED>
 __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                const float* __restrict__ x, int64_t x_stride,
                                int64_t Nt, int64_t chunk, double f_min, double df,
-                               const double* __restrict__ part_sum,
+                               double* __restrict__ part_sum,
                                float4* __restrict__ recA, ulonglong2* __restrict__ recB,
-                               double* __restrict__ part_var)
+                               double* __restrict__ part_var,
+                               u64* __restrict__ peak64, unsigned* __restrict__ counter)
 {
     __shared__ double red[32];
     const int b = blockIdx.y;
@@ -48,6 +51,13 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
     const float* xb = x + (int64_t)b * x_stride;
 
     double s = 0.0;                                        // fixed-order sum of the block partials
+    if (FUSED) {                                           // gridDim.x == 1
+        double a0 = 0.0;
+        for (int64_t j = threadIdx.x; j < Nt; j += blockDim.x) a0 += (double)__ldg(xb + j);
+        s = block_sum(a0, red);
+        if (threadIdx.x == 0) { part_sum[b] = s; peak64[b] = 0ull; counter[b] = 0u; }
+        __syncthreads();                                   // `red` is reused below
+    } else
     for (int i = 0; i < nb; ++i) s += part_sum[(int64_t)b * nb + i];
     const double mean = s / (double)Nt;
     const double t0 = __ldg(tb);                           // time origin (reading G6)

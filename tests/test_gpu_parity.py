@@ -137,7 +137,7 @@ def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush, corr):
     else:                                                  # tiny Nt: single fp16 pass of V limits |dP|/P to ~4e-4/sqrt(Nt)
         assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
     plan = h.last_plan()
-    assert plan["recurrence"] == 5 and "table" in plan["kernel"] and plan["launches"] == 5
+    assert plan["recurrence"] == 5 and "table" in plan["kernel"] and plan["launches"] == (4 if Nt <= 4096 else 5)   # one-block series: step 1 fused into the records kernel
     assert ("e5m2corr" in plan["kernel"]) == (corr == 2)
     assert ("cta_group2" in plan["kernel"]) == (pair >= 2) and ("pair2" in plan["kernel"]) == (pair == 3)
 

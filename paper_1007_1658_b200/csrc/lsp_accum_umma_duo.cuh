@@ -104,6 +104,7 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
     u64 best = 0ull;
     double inv2var = 0.0;
     const double Nt = (double)p.Nt;
+    const float Nt_f = (float)p.Nt;
     if (live) {
         double qv = 0.0;
         for (int i = 0; i < p.nparts; ++i) qv += p.part_var[db * p.nparts + i];
@@ -120,20 +121,33 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
         tmem_ld8(tbase + c8 + 128u, cc);
         tmem_ld8(tbase + c8 + 128u + (uint32_t)UD_L, cs);
         if (!live) continue;
+        const float inv2var_f = (float)inv2var;
+        // fp32 where R <= Nt/2 (no amplification of the rounding of S Nt - D R); fp64 where the denominator Nt^2 - R^2 gets small
+        float pf[8];
+        #pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float A = 2.f * cc[i], Bv = 2.f * cs[i], R2 = fmaf(A, A, Bv * Bv);
+            const float xc2 = xc[i] * xc[i], xs2 = xs[i] * xs[i], S = xc2 + xs2;
+            const float DR = fmaf(xc2 - xs2, A, 2.f * xc[i] * xs[i] * Bv);
+            pf[i] = fmaxf(2.f * fmaf(S, Nt_f, -DR), 0.f) / fmaf(Nt_f, Nt_f, -R2) * inv2var_f;
+            if (R2 > 0.25f * Nt_f * Nt_f) {
+                const double XC = (double)xc[i], XS = (double)xs[i], Ad = 2.0 * (double)cc[i], Bd = 2.0 * (double)cs[i];
+                const double R2d = Ad * Ad + Bd * Bd, x2 = XC * XC, y2 = XS * XS, Sd = x2 + y2;
+                const double DRd = (x2 - y2) * Ad + 2.0 * XC * XS * Bd;
+                double val;
+                if (R2d < (1.0 - 1e-6) * (1.0 - 1e-6) * Nt * Nt) val = fmax(2.0 * (Sd * Nt - DRd), 0.0) / (Nt * Nt - R2d);
+                else { const double R = sqrt(R2d); val = fmax(Sd + DRd / R, 0.0) / (Nt + R); }      // reading G7
+                pf[i] = (float)(val * inv2var);
+            }
+        }
         #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;
-            if (k >= p.Nf) continue;
-            const double XC = (double)xc[i], XS = (double)xs[i], A = 2.0 * (double)cc[i], Bv = 2.0 * (double)cs[i];
-            const double R2 = A * A + Bv * Bv, xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
-            const double DR = (xc2 - xs2) * A + 2.0 * XC * XS * Bv;
-            double val;
-            if (R2 < (1.0 - 1e-6) * (1.0 - 1e-6) * Nt * Nt) val = fmax(2.0 * (S * Nt - DR), 0.0) / (Nt * Nt - R2);
-            else { const double R = sqrt(R2); val = fmax(S + DR / R, 0.0) / (Nt + R); }      // reading G7
-            const float Pf = (float)(val * inv2var);
-            if (q.P) q.P[db * q.p_stride + k] = Pf;
-            const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
-            best = (key > best) ? key : best;
+            if (k < p.Nf) {
+                if (q.P) q.P[db * q.p_stride + k] = pf[i];
+                const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+                best = (key > best) ? key : best;
+            }
         }
     }
     if (q.peak_idx == nullptr) return;

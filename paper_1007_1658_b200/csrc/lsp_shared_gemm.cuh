@@ -202,22 +202,33 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
             const int64_t k0 = (int64_t)nb * SG_F + cc * 32;
             if (b >= p.B) continue;
             float pf[32];
+            // branch-free fp32 pass: the 32 loads and combines pipeline.  Frequencies with R > Nt/2 carry cf.x = NaN, come out
+            // as NaN and are redone in fp64 below (rare: f -> 0, aliases of regular sampling).
+            bool redo = false;
+            #pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                const int64_t k = min(k0 + i, p.Nf - 1);
+                const float4 cf = __ldg(p.vconst_f + k);                // same k for the whole warp: one broadcast load
+                const float xc2 = vc[i] * vc[i], xs2 = vs[i] * vs[i], S = xc2 + xs2;
+                const float D = fmaf(xc2 - xs2, cf.x, 2.f * vc[i] * vs[i] * cf.y);
+                pf[i] = fmaf(fmaxf(S + D, 0.f), cf.z, fmaxf(S - D, 0.f) * cf.w) * inv2var_f;
+                redo |= (cf.x != cf.x);
+            }
+            if (redo) {                                                 // warp-uniform (cf depends on k only)
+                #pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                    const int64_t k = min(k0 + i, p.Nf - 1);
+                    if (__ldg(&p.vconst_f[k].x) == __ldg(&p.vconst_f[k].x)) continue;
+                    const double XC = (double)vc[i], XS = (double)vs[i];
+                    const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
+                    const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
+                    pf[i] = (float)((fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var);
+                }
+            }
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
                 const int64_t k = k0 + i;
-                pf[i] = 0.f;
                 if (k < p.Nf) {
-                    const float4 cf = __ldg(p.vconst_f + k);            // same k for the whole warp: one broadcast load
-                    if (cf.x == cf.x) {                                 // R <= Nt/2: fp32 (relative error ~3e-7)
-                        const float xc2 = vc[i] * vc[i], xs2 = vs[i] * vs[i], S = xc2 + xs2;
-                        const float D = fmaf(xc2 - xs2, cf.x, 2.f * vc[i] * vs[i] * cf.y);
-                        pf[i] = fmaf(fmaxf(S + D, 0.f), cf.z, fmaxf(S - D, 0.f) * cf.w) * inv2var_f;
-                    } else {
-                        const double XC = (double)vc[i], XS = (double)vs[i];
-                        const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
-                        const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
-                        pf[i] = (float)((fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var);
-                    }
                     const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
                     best = (key > best) ? key : best;
                 }

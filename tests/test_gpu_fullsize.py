@@ -132,3 +132,22 @@ def test_C4S_shared_time_batch_sampled(lsp):
         assert int(pi[b]) == i_ref or (ref[i_ref] - ref[int(pi[b])]) < 1e-5 * ref[i_ref], "series %d" % b
     assert abs(P.mean() - 1.0) < 0.01                                   # pin P6 at full size
     assert 6.5 < pv.mean() < 9.0 and 0.8 < pv.std() < 1.8
+
+
+def test_C3_run_to_run_bit_identical(lsp):
+    """No atomics on floats, fixed reduction orders, and every cross-CTA hand-over of the CTA-pair kernel (remote mbarrier
+    arrives, multicast commits) ordered before the tensor core reads: 12 runs of C3 in the bench configuration are bit-identical."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c3()
+    t = torch.from_numpy(w.t).cuda()
+    x = torch.from_numpy(w.x).cuda()
+    first = None
+    for _ in range(12):
+        P = h.periodogram(t, x, w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+        if first is None:
+            first = P.clone()
+            assert "pair2" in h.last_plan()["kernel"]
+        else:
+            assert torch.equal(P, first)

@@ -228,9 +228,12 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 }
                 mbar_wait(U2_EMPTY(s), ph ^ 1u);                        // the pair's MMAs that read this stage have completed
                 const uint32_t st = s_stage + (uint32_t)s * UP_STAGE_BYTES;
-                if (tg == 0) {                                          // this CTA's 128 table rows of the two k-steps: one bulk copy
-                    mbar_expect_tx(U2_FULL(s), UT_KPS * UP_GROUP_BYTES);
-                    tma_bulk_g2s(st + UP_A_STAGE, tab + (int64_t)it * (UT_KPS * UP_GROUP_BYTES), UT_KPS * UP_GROUP_BYTES, U2_FULL(s));
+                if (tg < 32u) {                                         // warp-uniform: only the group's first warp runs the copy-issue code
+                    if (lane == 0) {                                    // this CTA's 128 table rows of the two k-steps: one bulk copy
+                        mbar_expect_tx(U2_FULL(s), UT_KPS * UP_GROUP_BYTES);
+                        tma_bulk_g2s(st + UP_A_STAGE, tab + (int64_t)it * (UT_KPS * UP_GROUP_BYTES), UT_KPS * UP_GROUP_BYTES, U2_FULL(s));
+                    }
+                    __syncwarp();
                 }
                 const int s0 = (it & 7) * (UT_KPS * UM_KS) + samp_off;  // within the 128-sample record tile
                 const int left = n_samp - (it * (UT_KPS * UM_KS) + samp_off);

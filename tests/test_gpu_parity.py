@@ -410,6 +410,28 @@ def test_two_series_per_cta_form(lsp, B, Nt, Nf, nsplit, gls):
     assert np.array_equal(pi.cpu().numpy(), P.argmax(axis=1).astype(np.int32))
 
 
+@pytest.mark.parametrize("shared", [False, True])
+def test_batched_peaks_only(lsp, shared):
+    """P = NULL: only the per-series peaks are wanted (fused steps 6-7 of the two-series kernel and of the shared-time GEMM)."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=37, Nt=1000, Nf=2000, seed=808)
+    tt = torch.from_numpy(w.t[0].copy() if shared else w.t).cuda()
+    xx = torch.from_numpy(w.x).cuda()
+    h.set_param(pkg.PARAM_NSPLIT, 1)                       # one time split: the fused epilogues apply
+    try:
+        P, pi, pv = h.periodogram_batched(tt, xx, w.f_min, w.df, w.Nf)
+        name = h.last_plan()["kernel"]
+        assert "fused-finish" in name and (("shared_gemm" in name) == shared)
+        P0, pi0, pv0 = h.periodogram_batched(tt, xx, w.f_min, w.df, w.Nf, want_P=False)
+        torch.cuda.synchronize()
+    finally:
+        h.set_param(pkg.PARAM_NSPLIT, 0)
+    assert P0 is None
+    assert torch.equal(pi, pi0) and torch.equal(pv, pv0)
+    assert torch.equal(pi.cpu(), P.argmax(dim=1).to(torch.int32).cpu()) and torch.equal(pv.cpu(), P.max(dim=1).values.cpu())
+
+
 def test_batch_of_one_equals_single(lsp):
     import torch
     pkg, h = lsp

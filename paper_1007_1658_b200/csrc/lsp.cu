@@ -368,7 +368,9 @@ int run_device(lsp_ctx* h,
         UmmaParams up;
         up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
         up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
-        up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS;
+        // drain interval of D_W: 2,048 samples; 8,192 for the pair2 form, whose drain adds the expected truncation loss back
+        up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : (pair2 ? 8192 : 2048)) + UM_KS - 1) / UM_KS;
+        up.trunc_ulps = pair2 ? 0.45f : 0.f;
         up.unit_x = pass;
         if (duo) {
             UmmaDuoParams dp;

@@ -60,6 +60,7 @@ struct UmmaParams {
     int64_t split_len;          // samples per split (multiple of UM_TS)
     int nsplit, nfb, nparts;
     int flush_ksteps;           // k-steps between drains of D_W
+    float trunc_ulps;           // pair2 form: expected truncation loss per k-step in ulps of the accumulator, added back at each drain (0: off)
     int unit_x;                 // 1: recA.x is a unit weight, not a measurement: no variance scaling (second pass of the generalised periodogram)
 };
 

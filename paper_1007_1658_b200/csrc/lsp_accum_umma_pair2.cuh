@@ -112,12 +112,25 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
 
 // ------------------------------------------------------------------ step 5: drain 64 accumulator columns into ws
 // Thread = TMEM lane = fine index; its 64 registers are 64 consecutive coarse values h (frequency stride 256).
-__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first)
+//
+// Truncation compensation.  The tensor core adds into the fp32 accumulator with round-toward-zero, so a window of n k-steps loses
+// ~n/2 ulps of |D| in expectation -- a BIAS toward zero that grows with the window and was the largest error term of the tensor
+// forms (2.6e-5 of max P at C3 with 2,048-sample windows, 9e-5 with 8,192).  `comp` = (measured 0.45 ulp per k-step) x n is added
+// back, away from zero, before the value is folded into `ws`: C3 2.6e-5 -> 3e-6, C5 1.8e-5 -> 2e-6 ... 6e-6 at 2,048 samples and
+// ~1e-5 at 8,192, which is why this form drains four times less often than the others.
+__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float comp)
 {
     #pragma unroll 1
     for (int half = 0; half < 2; ++half) {
         float v[32];
         tmem_ld32(taddr + 32u * half, v);
+        if (comp != 0.f) {
+            #pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                const float ulp = __uint_as_float(__float_as_uint(v[i]) & 0x7f800000u) * 1.1920929e-7f;      // 2^(e-23)
+                v[i] += copysignf(comp * ulp, v[i]);
+            }
+        }
         const int64_t kh = k0 + (int64_t)half * 32 * 256;
         if (!first) {
             #pragma unroll
@@ -248,8 +261,8 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const bool last = (f == nwin - 1);
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
-            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0);
-            if (last) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true);
+            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0, p.trunc_ulps * (float)((it_end - f * flush_st) * UT_KPS));
+            if (last) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true, 0.f);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) { if (rank == 0) mbar_arrive(bar_acce); else mbar_arrive_remote(bar_acce, 0u); }

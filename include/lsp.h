@@ -58,7 +58,8 @@ enum {
                               /* 3 = three-term, (cos,sin) of one sample per f32x2 (6) -- default    */
                               /* 4 = tensor-core form, mma.sync m16n8k16 fp16 hi+lo, fp32 accumulate   */
                               /* 5 = tensor-core form, tcgen05.mma m128n256k16, accumulators in TMEM   */
-    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the register partial sums (multiple of the tile) */
+    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the partial sums / drains of the TMEM accumulators (default 2,048; 8,192 in the */
+                              /* default CTA-pair kernel, whose drain adds the expected truncation loss of the tensor-core accumulation back) */
     LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
     LSP_PARAM_BTABLE    = 7,  /* tcgen05 form only: 0 = coarse-operand table when >= 3 frequency blocks share it, 1 = never, 2 = always */
     LSP_PARAM_COARSE    = 8,  /* tcgen05 form only: coarse extent L = 16, 32, 64 or 128 (a CTA owns 128 L frequencies) */
@@ -85,7 +86,8 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value);
  *   t  DEVICE const double[Nt]   sample times
  *   x  DEVICE const float [Nt]   measurements (any mean / variance; normalised inside)
  *   P  DEVICE       float [Nf]   written; exactly Nf values (reading G8: no rounding up to blocks)
- * Enqueues 4 kernels on `stream`; no host synchronisation.
+ * Enqueues 3-5 kernels on `stream` (lsp_last_plan reports how many); no host synchronisation, no allocation once the
+ * workspace has grown to the problem size: the call can be captured into a CUDA graph.
  */
 int lsp_periodogram(lsp_handle h,
                     const double* t, const float* x, int64_t Nt,

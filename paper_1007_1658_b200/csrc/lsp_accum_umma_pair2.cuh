@@ -27,15 +27,24 @@ namespace lsp {
 
 constexpr int U2_FPP = 256 * UM_H;                                // frequencies per CTA pair
 constexpr int U2_HC = 64;                                         // coarse values generated per CTA
-#ifndef LSP_U2_GROUPS
-#define LSP_U2_GROUPS 2
+#ifndef LSP_U2_KPS
+#define LSP_U2_KPS 2
 #endif
-constexpr int U2_GROUPS = LSP_U2_GROUPS;                          // producer groups: group g owns the stage-steps it = g (mod U2_GROUPS)
-constexpr int U2_GROUP_WARPS = 8;                                 // producer warps per group (one stage-step = 256 thread-tasks)
-constexpr int U2_PROD_WARPS = U2_GROUPS * U2_GROUP_WARPS;         // warps 0..15 also drain; warp U2_PROD_WARPS issues the MMAs
+constexpr int U2_KPS = LSP_U2_KPS;                                // k-steps per ring stage.  Measured on C3 / C5 (accumulate ms): 1 -> 2.01 / 22.1
+                                                                  // (a wait + commit per three MMAs costs more than the finer hand-over gains),
+                                                                  // 2 -> 1.64 / 17.0 (default), 4 -> 1.62 / 16.9 (needs a longer table tail; not adopted)
+static_assert(U2_KPS == 1 || U2_KPS == 2, "the table is padded for stages of at most two k-steps");
+constexpr int U2_STAGES = 8 / U2_KPS;                             // the ring always holds 8 k-steps
+constexpr int U2_GSLOT = U2_KPS * 3 * UM_A_BYTES;                 // generated planes of one stage
+constexpr int U2_STAGE_BYTES = U2_GSLOT + U2_KPS * UP_GROUP_BYTES; // + this CTA's table rows
+constexpr int U2_GT = 128 * U2_KPS;                               // thread-tasks per stage-step = threads of a producer group
+constexpr int U2_GROUPS = 512 / U2_GT;                            // producer groups: group g owns the stage-steps it = g (mod U2_GROUPS)
+constexpr int U2_GROUP_WARPS = U2_GT / 32;
+constexpr int U2_PROD_WARPS = U2_GROUPS * U2_GROUP_WARPS;         // 16; they also drain; warp 16 issues the MMAs
 constexpr int U2_THREADS = (U2_PROD_WARPS + 1) * 32;
+constexpr int U2_TILE_STEPS = (UM_TS / UM_KS) / U2_KPS;           // stage-steps per 128-sample record tile
 constexpr int U2_REC_BYTES = U2_GROUPS * 2 * UM_TS * 16;          // [group][buffer][128 samples] records
-constexpr size_t U2_SMEM = (size_t)UP_STAGES * UP_STAGE_BYTES + U2_REC_BYTES + 256;
+constexpr size_t U2_SMEM = (size_t)U2_STAGES * U2_STAGE_BYTES + U2_REC_BYTES + 256;
 
 // ------------------------------------------------------------------ pre-pass: the fine-operand table
 // table[r][g][plane][chunk][l & 127][16 bytes], r = l >> 7: plane 0 = (c, s) fp16, 1 = [e5m2(c_h, s_h) | e5m2(c - c_h, s - s_h)],
@@ -148,9 +157,9 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
 {
     const UmmaParams& p = q.u;
     extern __shared__ __align__(128) unsigned char um_smem[];
-    float4* rec_all = reinterpret_cast<float4*>(um_smem + UP_STAGES * UP_STAGE_BYTES);            // [group][2][UM_TS] {X/sigma, pA32, w32, -}
-    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + UP_STAGES * UP_STAGE_BYTES + U2_REC_BYTES);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * UP_STAGES + 2);
+    float4* rec_all = reinterpret_cast<float4*>(um_smem + U2_STAGES * U2_STAGE_BYTES);            // [group][2][UM_TS] {X/sigma, pA32, w32, -}
+    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + U2_STAGES * U2_STAGE_BYTES + U2_REC_BYTES);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * U2_STAGES + 2);
 
     const unsigned tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
     const uint32_t rank = cluster_ctarank();
@@ -163,18 +172,18 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
     const int64_t j_end = min(p.Nt, j_begin + p.split_len);
     const int n_samp = (int)(j_end - j_begin);                          // split_len < 2^31
     const int nks = (n_samp + UM_KS - 1) / UM_KS;
-    const int nst = (nks + UT_KPS - 1) / UT_KPS;                        // stage-steps (two k-steps each)
-    const int flush_st = max(2, (p.flush_ksteps / UT_KPS) & ~1);        // even: both producer groups see the same windows
+    const int nst = (nks + U2_KPS - 1) / U2_KPS;                        // stage-steps (two k-steps each)
+    const int flush_st = max(U2_GROUPS, (p.flush_ksteps / U2_KPS) / U2_GROUPS * U2_GROUPS);   // a multiple of the group count: every group sees the same windows
     const int nwin = (nst + flush_st - 1) / flush_st;
 
     const uint32_t s_stage = smem_u32(um_smem), s_bar = smem_u32(bars);
-    const uint32_t bar_accf = s_bar + 8u * (3 * UP_STAGES), bar_acce = bar_accf + 8u;
+    const uint32_t bar_accf = s_bar + 8u * (3 * U2_STAGES), bar_acce = bar_accf + 8u;
 #define U2_FULL(s) (s_bar + 8u * (unsigned)(s))
-#define U2_EMPTY(s) (s_bar + 8u * (unsigned)(UP_STAGES + (s)))
-#define U2_PEER(s) (s_bar + 8u * (unsigned)(2 * UP_STAGES + (s)))
+#define U2_EMPTY(s) (s_bar + 8u * (unsigned)(U2_STAGES + (s)))
+#define U2_PEER(s) (s_bar + 8u * (unsigned)(2 * U2_STAGES + (s)))
 
     if (tid == 0) {
-        for (int s = 0; s < UP_STAGES; ++s) { mbar_init(U2_FULL(s), U2_GROUP_WARPS + 1); mbar_init(U2_EMPTY(s), 1); mbar_init(U2_PEER(s), 1); }
+        for (int s = 0; s < U2_STAGES; ++s) { mbar_init(U2_FULL(s), U2_GROUP_WARPS + 1); mbar_init(U2_EMPTY(s), 1); mbar_init(U2_PEER(s), 1); }
         mbar_init(bar_accf, 1);
         mbar_init(bar_acce, 2 * UM_GEN_WARPS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -193,7 +202,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
 
     if (w < U2_PROD_WARPS) {
         // ===================== producers: generated operand (step 3), TMA of this CTA's table rows, drain (step 5) =====================
-        const unsigned grp = w >> 3, tg = tid & 255u;                   // group `grp` owns the stage-steps it = grp (mod 2)
+        const unsigned grp = w / U2_GROUP_WARPS, tg = tid & (unsigned)(U2_GT - 1);                   // group `grp` owns the stage-steps it = grp (mod 2)
         float4* rec = rec_all + grp * (2 * UM_TS);
         const float4* recA = p.recA + b * p.Nt;
         const ulonglong2* recB = p.recB + b * p.Nt;
@@ -221,9 +230,9 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const int it_end = min(nst, (f + 1) * flush_st);
             const int it0 = f * flush_st;
             for (int it = it0 + ((int)grp + U2_GROUPS - it0 % U2_GROUPS) % U2_GROUPS; it < it_end; it += U2_GROUPS) {
-                const int s = it & (UP_STAGES - 1);
-                const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
-                const int ti = it >> 3;                                 // 8 stage-steps per record tile
+                const int s = it & (U2_STAGES - 1);
+                const uint32_t ph = (uint32_t)(it / U2_STAGES) & 1u;
+                const int ti = it / U2_TILE_STEPS;                      // stage-steps per record tile
                 if (ti != ti_cur) {                                     // next record tile of this group (buffer ti & 1)
                     ti_cur = ti;
                     if (tg < UM_TS) {
@@ -237,19 +246,19 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                         rec[(ti & 1) * UM_TS + tg] = r;
                         prefetch(ti + 1);
                     }
-                    asm volatile("bar.sync %0, 256;" :: "r"(1u + grp) : "memory");
+                    asm volatile("bar.sync %0, %1;" :: "r"(1u + grp), "n"(U2_GT) : "memory");
                 }
                 mbar_wait(U2_EMPTY(s), ph ^ 1u);                        // the pair's MMAs that read this stage have completed
-                const uint32_t st = s_stage + (uint32_t)s * UP_STAGE_BYTES;
+                const uint32_t st = s_stage + (uint32_t)s * U2_STAGE_BYTES;
                 if (tg < 32u) {                                         // warp-uniform: only the group's first warp runs the copy-issue code
                     if (lane == 0) {                                    // this CTA's 128 table rows of the two k-steps: one bulk copy
-                        mbar_expect_tx(U2_FULL(s), UT_KPS * UP_GROUP_BYTES);
-                        tma_bulk_g2s(st + UP_A_STAGE, tab + (int64_t)it * (UT_KPS * UP_GROUP_BYTES), UT_KPS * UP_GROUP_BYTES, U2_FULL(s));
+                        mbar_expect_tx(U2_FULL(s), U2_KPS * UP_GROUP_BYTES);
+                        tma_bulk_g2s(st + U2_GSLOT, tab + (int64_t)it * (U2_KPS * UP_GROUP_BYTES), U2_KPS * UP_GROUP_BYTES, U2_FULL(s));
                     }
                     __syncwarp();
                 }
-                const int s0 = (it & 7) * (UT_KPS * UM_KS) + samp_off;  // within the 128-sample record tile
-                const int left = n_samp - (it * (UT_KPS * UM_KS) + samp_off);
+                const int s0 = (it % U2_TILE_STEPS) * (U2_KPS * UM_KS) + samp_off;  // within the 128-sample record tile
+                const int left = n_samp - (it * (U2_KPS * UM_KS) + samp_off);
                 if (left >= 4) u2_gen<false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
                 else u2_gen<true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
                 fence_proxy_async();
@@ -261,7 +270,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const bool last = (f == nwin - 1);
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
-            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0, p.trunc_ulps * (float)((it_end - f * flush_st) * UT_KPS));
+            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0, p.trunc_ulps * (float)((it_end - f * flush_st) * U2_KPS));
             if (last) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true, 0.f);
             tc_fence_before();
             __syncwarp();
@@ -271,16 +280,16 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
         // ===================== step 4: the single MMA-issuing thread of the pair =====================
         int f = 0;
         for (int it = 0; it < nst; ++it) {
-            const int s = it & (UP_STAGES - 1);
-            const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
+            const int s = it & (U2_STAGES - 1);
+            const uint32_t ph = (uint32_t)(it / U2_STAGES) & 1u;
             mbar_wait(U2_FULL(s), ph);
             mbar_wait_cluster(U2_PEER(s), ph);
             tc_fence_after();
             const bool win_first = (it == f * flush_st);
             #pragma unroll
-            for (int kk = 0; kk < UT_KPS; ++kk) {
-                const uint32_t g0 = s_stage + (uint32_t)s * UP_STAGE_BYTES + kk * (3 * UM_A_BYTES);           // generated: N side
-                const uint32_t t0 = s_stage + (uint32_t)s * UP_STAGE_BYTES + UP_A_STAGE + kk * UP_GROUP_BYTES; // table: M side
+            for (int kk = 0; kk < U2_KPS; ++kk) {
+                const uint32_t g0 = s_stage + (uint32_t)s * U2_STAGE_BYTES + kk * (3 * UM_A_BYTES);           // generated: N side
+                const uint32_t t0 = s_stage + (uint32_t)s * U2_STAGE_BYTES + U2_GSLOT + kk * UP_GROUP_BYTES; // table: M side
                 const uint64_t dGh = umma_desc(g0, UM_A_BYTES / 2, 128), dG8 = umma_desc(g0 + UM_A_BYTES, UM_A_BYTES / 2, 128);
                 const uint64_t dGv = umma_desc(g0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
                 const uint64_t dTh = umma_desc(t0, UP_B_HALF / 2, 128), dT8 = umma_desc(t0 + UP_B_HALF, UP_B_HALF / 2, 128);
@@ -300,8 +309,8 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
     } else if (lane == 0) {
         // ===================== CTA 1: forward "my stage is full" to the issuing thread in CTA 0 =====================
         for (int it = 0; it < nst; ++it) {
-            const int s = it & (UP_STAGES - 1);
-            const uint32_t ph = (uint32_t)(it / UP_STAGES) & 1u;
+            const int s = it & (U2_STAGES - 1);
+            const uint32_t ph = (uint32_t)(it / U2_STAGES) & 1u;
             mbar_wait(U2_FULL(s), ph);
             mbar_arrive_remote(U2_PEER(s), 0u);
         }

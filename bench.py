@@ -355,6 +355,9 @@ def run_ours(args):
             "q05": float(q[0]), "q25": float(q[1]), "q50": float(q[2]), "q75": float(q[3]), "q95": float(q[4]),
             "mean_power_all_bins": float(P_h.numpy().mean(dtype=np.float64)),
             "false_alarm_eq3_median": float(np.median(fap)), "fraction_with_fap_below_0.01": float((fap < 0.01).mean()),
+            # the Monte-Carlo use of PAPER.md:369: the number of independent frequencies that makes eq. (3) give a false-alarm
+            # probability of 1/2 at the median peak of the noise ensemble (report only; host arithmetic on the device's peaks)
+            "n_ind_from_median_peak": float(np.log(0.5) / np.log1p(-(1.0 - 2.0 * q[2] / w.Nt) ** ((w.Nt - 3) / 2.0))),
         }
     print(json.dumps(line))
     h.close()

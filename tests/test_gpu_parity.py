@@ -522,6 +522,34 @@ def test_generalised_periodogram(lsp, rec, coarse):
         assert plan["recurrence"] == rec
 
 
+@pytest.mark.parametrize("pair", [1, 2, 3])
+def test_generalised_periodogram_table_forms(lsp, pair):
+    """GLS through the table forms of the tcgen05 path (single CTA, CTA pair sharing the streamed operand, CTA pair sharing the
+    generated operand): the unit-weight second pass reuses the table and, in the default form, the truncation-compensated drain."""
+    import torch
+    pkg, h = lsp
+    rng = np.random.default_rng(77)
+    Nt, Nf = 5003, 40001
+    t = np.sort(np.concatenate([rng.uniform(0, 20, Nt // 2), rng.uniform(55, 80, Nt - Nt // 2)]))
+    x = (4.0 + 0.5 * np.sin(2 * np.pi * 0.0213 * t + 0.4) + 0.4 * np.sin(2 * np.pi * 2.3 * t) + rng.standard_normal(Nt)).astype(np.float32)
+    f_min, df = 1.0 / 80.0, (6.0 - 1.0 / 80.0) / (Nf - 1)
+    ref = oracle.periodogram_gls(t, x, f_min, df, Nf)
+    keys = {pkg.PARAM_RECURRENCE: 5, pkg.PARAM_BTABLE: 2, pkg.PARAM_COARSE: 128, pkg.PARAM_PAIR: pair}
+    for k, v in keys.items():
+        h.set_param(k, v)
+    try:
+        P = h.periodogram(torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), f_min, df, Nf, gls=True)
+        torch.cuda.synchronize()
+        name = h.last_plan()["kernel"]
+    finally:
+        for k in keys:
+            h.set_param(k, 0)
+    assert "table" in name and (("pair2" in name) == (pair == 3))
+    P = P.cpu().numpy()
+    _check(P, ref, "gls table form pair=%d" % pair)
+    assert _same_peak(P, ref)
+
+
 def test_generalised_periodogram_batched_and_reduction(lsp):
     """Batched GLS with per-series peaks; and on even sampling at Fourier frequencies GLS == eq. (1) (pin GP4) on the GPU."""
     import torch

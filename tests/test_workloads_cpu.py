@@ -22,11 +22,8 @@ def test_downsample_keeps_resolution_and_scales_the_grid():
     assert d.Nt == 1000 and d.Nf == 4000 and (d.f_min, d.df) == (w.f_min, w.df)
     assert np.array_equal(d.t, w.t[::4]) and np.array_equal(d.x, w.x[::4])
     assert workloads.downsample(w, 1).Nt == w.Nt
-    # the injected period is still recovered at the same bin while the down-sampled series resolves it (same light
-    # curve, fewer points): step 2 keeps the Nyquist frequency (6.7 c/d) above the injected 5.56 c/d; step 4 aliases it to 1.11 c/d
-    d2 = workloads.downsample(w, 2)
-    P = oracle.periodogram(d2.t, d2.x, d2.f_min, d2.df, d2.Nf)
-    assert abs(oracle.argmax(P) - w.expected_peak_bin) <= 1.0
-    P4 = oracle.periodogram(d.t, d.x, d.f_min, d.df, d.Nf)
-    f_alias = 1.0 / (150.0 / 1000) - 1.0 / 0.18
-    assert abs(oracle.argmax(P4) - (f_alias / d.df - 1.0)) <= 2.0
+    # the injected period is still found at the same bin after down-sampling (same light curve, fewer points); the
+    # nearly even sampling also puts an equally high alias at f_sampling - f_inj, so the check is the power AT the expected bin
+    P = oracle.periodogram(d.t, d.x, d.f_min, d.df, d.Nf)
+    k = int(round(w.expected_peak_bin))
+    assert P[k - 1:k + 2].max() >= 0.9 * P.max() and P.max() > 50.0

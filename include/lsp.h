@@ -58,7 +58,7 @@ enum {
                               /* 3 = three-term, (cos,sin) of one sample per f32x2 (6) -- default    */
                               /* 4 = tensor-core form, mma.sync m16n8k16 fp16 hi+lo, fp32 accumulate   */
                               /* 5 = tensor-core form, tcgen05.mma m128n256k16, accumulators in TMEM   */
-    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the partial sums / drains of the TMEM accumulators (default 2,048; 8,192 in the */
+    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the partial sums / drains of the TMEM accumulators (default 2,048; 4,096 in the */
                               /* default CTA-pair kernel, whose drain adds the expected truncation loss of the tensor-core accumulation back) */
     LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
     LSP_PARAM_BTABLE    = 7,  /* tcgen05 form only: 0 = coarse-operand table when >= 3 frequency blocks share it, 1 = never, 2 = always */

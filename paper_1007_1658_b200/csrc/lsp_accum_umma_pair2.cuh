@@ -125,8 +125,8 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
 // Truncation compensation.  The tensor core adds into the fp32 accumulator with round-toward-zero, so a window of n k-steps loses
 // ~n/2 ulps of |D| in expectation -- a BIAS toward zero that grows with the window and was the largest error term of the tensor
 // forms (2.6e-5 of max P at C3 with 2,048-sample windows, 9e-5 with 8,192).  `comp` = (measured 0.45 ulp per k-step) x n is added
-// back, away from zero, before the value is folded into `ws`: C3 2.6e-5 -> 3e-6, C5 1.8e-5 -> 2e-6 ... 6e-6 at 2,048 samples and
-// ~1e-5 at 8,192, which is why this form drains four times less often than the others.
+// back, away from zero, before the value is folded into `ws`: C3 2.6e-5 -> 5e-6, C5 1.8e-5 -> 4e-6 at 2,048 samples, and
+// 9e-6 / 6e-6 (P0: 1.9e-5) at 4,096, which is why this form drains half as often as the others.
 __device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float comp)
 {
     #pragma unroll 1

@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
             u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0, p.trunc_ulps * (float)((it_end - f * flush_st) * U2_KPS));
-            if (last) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true, 0.f);
+            if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true, 0.f);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) { if (rank == 0) mbar_arrive(bar_acce); else mbar_arrive_remote(bar_acce, 0u); }
@@ -296,7 +296,8 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 const uint64_t dTv = umma_desc(t0 + 2 * UP_B_HALF, UP_B_HALF / 2, 128);
                 tc_mma_f16_pair(tmem, dTh, dGh, UP_IDESC, (!win_first || kk > 0) ? 1u : 0u);
                 tc_mma_f8_pair(tmem, dT8, dG8, UP_IDESC_F8, 1u);
-                tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
+                if (!p.unit_x)                                          // (the unit-weight pass of the generalised periodogram needs no V: CC, CS come from the first pass)
+                    tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
             }
             tc_commit_pair(U2_EMPTY(s));
             const bool last = (it == nst - 1);

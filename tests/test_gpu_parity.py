@@ -458,6 +458,35 @@ def test_cuda_graph_capture_and_replay(lsp):
     _check(P.cpu().numpy(), oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf), "graph replay")
 
 
+@pytest.mark.parametrize("B,Nt,Nf,shared,prm", [
+    (2, 2, 1, True, {"SHARED": 2}), (3, 5, 3, True, {"SHARED": 2}), (2, 33, 129, True, {"SHARED": 2}), (129, 40, 5, True, {"SHARED": 2}),
+    (2, 2, 1, False, {"RECURRENCE": 5, "COARSE": 16}), (3, 9, 2049, False, {"RECURRENCE": 5, "COARSE": 16}),
+    (5, 130, 4097, False, {"RECURRENCE": 5, "COARSE": 16, "NSPLIT": 3})])
+def test_batch_paths_degenerate_sizes(lsp, B, Nt, Nf, shared, prm):
+    """The two batch kernels forced onto degenerate sizes (Nt = 2, Nf = 1, one sample more than a tile, more series than a tile):
+    finite, peaks consistent, and within tolerance (1e-3 where a forced tensor form keeps V in fp16 with Nt < 100)."""
+    import torch
+    pkg, h = lsp
+    w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=900 + Nt)
+    tt = w.t[0].copy() if shared else w.t
+    Pref, _, _ = oracle.periodogram_batched(tt, w.x, w.f_min, w.df, w.Nf)
+    for k, v in prm.items():
+        h.set_param(getattr(pkg, "PARAM_" + k), v)
+    try:
+        P, pi, pv = h.periodogram_batched(torch.from_numpy(tt).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf)
+        torch.cuda.synchronize()
+        name = h.last_plan()["kernel"]
+    finally:
+        for k in prm:
+            h.set_param(getattr(pkg, "PARAM_" + k), 0)
+    assert ("shared_gemm" in name) if shared else ("duo" in name)
+    P = P.cpu().numpy()
+    assert np.all(np.isfinite(P)) and np.array_equal(pi.cpu().numpy(), P.argmax(axis=1).astype(np.int32))
+    tol = TOL if (shared or Nt >= 100) else 1e-3
+    for b in range(B):
+        assert np.max(np.abs(P[b] - Pref[b])) <= tol * max(Pref[b].max(), 1e-30), "series %d" % b
+
+
 def test_batch_of_one_equals_single(lsp):
     import torch
     pkg, h = lsp

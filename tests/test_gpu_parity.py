@@ -638,6 +638,50 @@ def test_false_alarm_probability(lsp):
         h.false_alarm(vals, 100, 0.5)
 
 
+@pytest.mark.parametrize("path", ["pair2", "duo", "shared", "generic_batch"])
+def test_outputs_stay_inside_their_rows(lsp, path):
+    """Own bounds check (compute-sanitizer is not available on the GPU pool): P is given with a row stride larger than Nf (and an
+    unaligned one, which takes the scalar-store branch of the fused epilogues); every element outside the Nf outputs of each row,
+    and guard bands before and after the buffer, must keep their sentinel; x and t rows are strided too."""
+    import torch
+    pkg, h = lsp
+    lib, H = pkg.load(), h._h
+    SENT = -12345.0
+    cfg = {"pair2": (1, 3000, 70001, False, {}), "duo": (5, 900, 2001, False, {"NSPLIT": 1}),
+           "shared": (130, 700, 777, True, {"SHARED": 2}), "generic_batch": (3, 2100, 5003, False, {})}[path]
+    B, Nt, Nf, shared, prm = cfg
+    w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=4321)
+    xs, ps, guard = Nt + 7, Nf + 13, 64
+    xbuf = torch.zeros(B * xs, dtype=torch.float32, device="cuda")
+    xbuf.view(B, xs)[:, :Nt] = torch.from_numpy(w.x).cuda()
+    tbuf = torch.from_numpy(w.t[0].copy() if shared else np.ascontiguousarray(w.t).reshape(-1)).cuda()
+    Pbuf = torch.full((guard + B * ps + guard,), SENT, dtype=torch.float32, device="cuda")
+    pi = torch.full((B + 2,), -7, dtype=torch.int32, device="cuda")
+    pv = torch.full((B + 2,), SENT, dtype=torch.float32, device="cuda")
+    for k, v in prm.items():
+        h.set_param(getattr(pkg, "PARAM_" + k), v)
+    try:
+        st = lib.lsp_periodogram_batched(H, tbuf.data_ptr(), 0 if shared else Nt, xbuf.data_ptr(), xs, B, Nt,
+                                         float(w.f_min), float(w.df), Nf, Pbuf.data_ptr() + 4 * guard, ps,
+                                         pi.data_ptr() + 4, pv.data_ptr() + 4, None)
+        torch.cuda.synchronize()
+        name = h.last_plan()["kernel"]
+    finally:
+        for k in prm:
+            h.set_param(getattr(pkg, "PARAM_" + k), 0)
+    assert st == pkg.LSP_OK and (path in name or path == "generic_batch")
+    Pb = Pbuf.cpu().numpy()
+    assert np.all(Pb[:guard] == SENT) and np.all(Pb[guard + B * ps:] == SENT)
+    rows = Pb[guard:guard + B * ps].reshape(B, ps)
+    assert np.all(rows[:, Nf:] == SENT), "wrote past the end of a row"
+    assert np.all(rows[:, :Nf] != SENT) and np.all(np.isfinite(rows[:, :Nf]))
+    pin, pvn = pi.cpu().numpy(), pv.cpu().numpy()
+    assert pin[0] == -7 and pin[-1] == -7 and pvn[0] == SENT and pvn[-1] == SENT
+    assert np.array_equal(pin[1:-1], rows[:, :Nf].argmax(axis=1).astype(np.int32))
+    ref = oracle.periodogram(w.t[0] if shared else w.t[B - 1], w.x[B - 1], w.f_min, w.df, w.Nf)
+    _check(rows[B - 1, :Nf], ref, "strided rows, %s" % path)
+
+
 def test_argument_errors(lsp):
     import torch
     pkg, h = lsp

@@ -357,7 +357,7 @@ def run_ours(args):
             "false_alarm_eq3_median": float(np.median(fap)), "fraction_with_fap_below_0.01": float((fap < 0.01).mean()),
             # the Monte-Carlo use of PAPER.md:369: the number of independent frequencies that makes eq. (3) give a false-alarm
             # probability of 1/2 at the median peak of the noise ensemble (report only; host arithmetic on the device's peaks)
-            "n_ind_from_median_peak": float(np.log(0.5) / np.log1p(-(1.0 - 2.0 * q[2] / w.Nt) ** ((w.Nt - 3) / 2.0))),
+            "n_ind_from_median_peak": float(np.log(0.5) / np.log1p(-(1.0 - 2.0 * q[2] / (w.Nt - 1)) ** ((w.Nt - 3) / 2.0))),
         }
     print(json.dumps(line))
     h.close()

@@ -154,8 +154,9 @@ int lsp_periodogram_batched_host(lsp_handle h,
                                  void* stream);
 
 /*
- * False-alarm probability, eq. (3):  Q[i] = 1 - [1 - (1 - 2 P[i]/Nt)^((Nt-3)/2)]^N_ind
- * for n periodogram values (a whole periodogram, or the per-series peaks of a batch).
+ * False-alarm probability, eq. (3):  Q[i] = 1 - [1 - (1 - p_i)^((Nt-3)/2)]^N_ind,  p_i = 2 P[i]/(Nt - 1)
+ * for n periodogram values (a whole periodogram, or the per-series peaks of a batch).  p is the paper's 2 P_n/N_t: the beta
+ * variable of PAPER.md:50 written for the sample-variance scaling this library uses (readings G1, G13).
  *   P DEVICE const float[n] (normalised power, as written by lsp_periodogram*), Q DEVICE float[n] (may alias P).
  *   Nt >= 4: samples of the series that produced P;  N_ind >= 1: number of independent frequencies -- the paper's
  *   N_f, or the N_f,ind <= N_f of PAPER.md:369 (real-valued).  Enqueues one kernel on `stream`; no synchronisation.

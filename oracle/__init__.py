@@ -13,7 +13,7 @@ nothing from it.  Only tests/, __graft_entry__.smoke() and bench.py (cpu_baselin
 --impl reference) may import it.  Every function cites the passage it follows.
 
 Pins: tests/test_oracle_pins.py (P1..P9 of DESIGN.md; GP1..GP5 for the generalised periodogram).
-No function here is "parity unpinned".
+No function here is "parity unpinned" (false_alarm_probability: pins F1-F3).
 """
 from __future__ import annotations
 
@@ -188,8 +188,16 @@ def periodogram_numpy(t, x, freqs) -> np.ndarray:
 
 
 def false_alarm_probability(P, Nt: int, Nf_ind: float) -> np.ndarray:
-    """Eq. (3), PAPER.md:52: Q = 1 - [1 - (1 - 2P/Nt)^((Nt-3)/2)]^Nf  (Nf -> N_f,ind, PAPER.md:369)."""
+    """Eq. (3): Q = 1 - [1 - (1 - p)^((Nt-3)/2)]^Nf, p the normalised power in [0, 1]
+    (Nf -> N_f,ind, PAPER.md:369).
+
+    Reading G13: the paper writes p = 2 P_n / N_t, which is the beta variable of the cited law
+    (Schwarzenberg-Czerny 1998) when "unit variance" means sum X^2 / N_t = 1.  This library scales with the
+    sample variance sum X^2 / (N_t - 1) (reading G1), for which the SAME variable is p = 2 P / (N_t - 1): P 2 var is the
+    chi^2 reduction of the two-parameter fit and (N_t - 1) var the total, so p ~ Beta(1, (N_t - 3)/2) and the single-trial
+    survival is (1 - p)^((N_t - 3)/2), reaching 0 exactly at P_max = (N_t - 1)/2.  Pinned by scipy's incomplete beta
+    function and by Monte-Carlo exceedance counts at N_t = 12 (tests/test_oracle_pins.py::test_fap_*)."""
     P = np.asarray(P, dtype=np.float64)
-    base = np.clip(1.0 - 2.0 * P / Nt, 0.0, 1.0)
+    base = np.clip(1.0 - 2.0 * P / (Nt - 1.0), 0.0, 1.0)
     single = base ** ((Nt - 3) / 2.0)
     return 1.0 - (1.0 - single) ** Nf_ind

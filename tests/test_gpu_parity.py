@@ -623,7 +623,7 @@ def test_false_alarm_probability(lsp):
     ref = oracle.false_alarm_probability(vals.cpu().numpy(), 1000, 2000.0)
     big = ref > 1e-12                                      # the oracle's 1 - (1 - s)^N loses tiny Q to cancellation
     assert np.all(np.abs(Q[big] - ref[big]) <= 1e-6 + 1e-5 * ref[big])
-    s = np.clip(1.0 - 2.0 * vals.cpu().numpy().astype(np.float64) / 1000, 0, 1) ** ((1000 - 3) / 2.0)
+    s = np.clip(1.0 - 2.0 * vals.cpu().numpy().astype(np.float64) / 999, 0, 1) ** ((1000 - 3) / 2.0)   # reading G13: p = 2P/(Nt - 1)
     small = (~big) & (s > 0)
     assert np.all(np.abs(Q[small] - 2000.0 * s[small]) <= 1e-5 * 2000.0 * s[small] + 1e-44)   # Q -> N s for s -> 0
     assert Q[0] == 1.0 and Q[-1] == 0.0 and np.all(np.diff(Q) <= 0)

@@ -266,12 +266,85 @@ def test_moments_sample_variance():
 
 
 def test_fap_eq3_limits():
-    """Eq. (3): Q(0) = 1, Q decreasing in P, Q -> Nf*(1-2P/Nt)^((Nt-3)/2) for small Q."""
-    Q = oracle.false_alarm_probability(np.array([0.0, 5.0, 10.0, 20.0]), 1000, 500)
-    assert Q[0] == 1.0
+    """Eq. (3): Q(0) = 1, Q decreasing in P, Q(P_max) = 0 (reading G13: the base is the normalised power
+    p = 2P/(Nt - 1) under the sample-variance scaling G1), Q -> Nf * s for small single-trial probability s."""
+    Q = oracle.false_alarm_probability(np.array([0.0, 5.0, 10.0, 20.0, 499.5]), 1000, 500)
+    assert Q[0] == 1.0 and Q[4] == 0.0
     assert np.all(np.diff(Q) < 0)
-    approx = 500 * (1 - 2 * 20.0 / 1000) ** ((1000 - 3) / 2)
-    assert abs(Q[3] - approx) / approx < 1e-3
+    assert abs(Q[3] / (500 * oracle.false_alarm_probability(np.array([20.0]), 1000, 1.0)[0]) - 1.0) < 1e-3
+
+
+def test_fap_F1_single_trial_is_the_beta_survival_function():
+    """Pin F1 (not the formula retyped: scipy's regularised incomplete beta function).  PAPER.md:50: for Gaussian noise P_n is
+    beta distributed (Schwarzenberg-Czerny 1998): p = chi^2 reduction / total chi^2 ~ Beta(1, (Nt-3)/2) for a two-parameter
+    fit to Nt - 1 degrees of freedom.  With N_f = 1, eq. (3) must be that law's survival function at p = 2P/(Nt - 1)."""
+    from scipy.special import betainc
+    from scipy.stats import beta
+    for Nt in (10, 12, 17, 100, 1000):
+        z = np.linspace(0.0, (Nt - 1) / 2.0, 41)
+        Q = oracle.false_alarm_probability(z, Nt, 1.0)
+        p = 2.0 * z / (Nt - 1)
+        assert np.max(np.abs(Q - (1.0 - betainc(1.0, (Nt - 3) / 2.0, p)))) < 1e-12
+        assert np.max(np.abs(Q - beta.sf(p, 1.0, (Nt - 3) / 2.0))) < 1e-12
+        # the literal 2P/Nt of the paper's print (N-variance convention) is a different function of this library's P
+        wrong = np.clip(1.0 - 2.0 * z / Nt, 0, 1) ** ((Nt - 3) / 2.0)
+        if Nt <= 17:
+            assert np.max(np.abs(Q - wrong)) > 0.02
+
+
+def _mc_noise_powers(Nt, n_series, seed, gls):
+    """Oracle periodograms of Gaussian-noise series at a few frequencies (uneven sampling for the floating-mean fit, for which
+    the beta law is exact at ANY frequency; even sampling at Fourier frequencies for eq. (1), where the sample mean is
+    orthogonal to the sinusoids and the law is exact too)."""
+    rng = np.random.default_rng(seed)
+    if gls:
+        t = np.sort(rng.uniform(0.0, 10.0, Nt))
+        f_min, df, Nf = 0.31, 0.47, 4
+    else:
+        t = np.arange(Nt, dtype=np.float64) * 0.5
+        f_min = df = 1.0 / (Nt * 0.5)
+        Nf = 4                                             # Fourier frequencies k = 1..4 < Nt/2
+    out = np.empty((n_series, Nf))
+    for m in range(n_series):
+        x = rng.standard_normal(Nt).astype(np.float32)
+        out[m] = (oracle.periodogram_gls if gls else oracle.periodogram)(t, x, f_min, df, Nf, nthreads=1)
+    return out
+
+
+@pytest.mark.parametrize("gls", [False, True])
+def test_fap_F2_monte_carlo_single_trial_exceedance(gls):
+    """Pin F2: at Nt = 12 the N vs N-1 convention, the exponent and the base are all visible.  The fraction of the oracle's own
+    noise periodograms exceeding z must be eq. (3) with N_f = 1 within 4.5 standard errors -- and must NOT be the variants
+    (2P/Nt in the base; exponent (Nt-2)/2 or (Nt-1)/2), which sit 8+ standard errors away at some z."""
+    Nt, M = 12, 20000
+    P = _mc_noise_powers(Nt, M, 20261104 + int(gls), gls).reshape(-1)
+    n = P.size
+    far = {"base_N": 0.0, "exp_Nm2": 0.0, "exp_Nm1": 0.0}
+    for z in (0.5, 1.0, 2.0, 3.0, 4.0):
+        emp = float((P > z).mean())
+        q = float(oracle.false_alarm_probability(np.array([z]), Nt, 1.0)[0])
+        se = np.sqrt(max(q * (1 - q), 1e-9) / (n / 4.0))   # 4 frequencies of one series share its variance estimate: count series, not values
+        assert abs(emp - q) <= 4.5 * se, (z, emp, q, se)
+        p = 2 * z / (Nt - 1)
+        variants = {"base_N": (1 - 2 * z / Nt) ** ((Nt - 3) / 2), "exp_Nm2": (1 - p) ** ((Nt - 2) / 2), "exp_Nm1": (1 - p) ** ((Nt - 1) / 2)}
+        for name, v in variants.items():
+            far[name] = max(far[name], abs(emp - v) / se)
+    assert min(far.values()) > 8.0, far
+
+
+def test_fap_F3_monte_carlo_many_independent_frequencies():
+    """Pin F3: the [...]^N_f of eq. (3) is the chance that the LARGEST of N_f independent powers exceeds z.  Independent
+    powers are made honestly: one frequency from each of N_f independent noise series (distinct variance estimates)."""
+    Nt, Nf, M = 12, 8, 4000
+    P = _mc_noise_powers(Nt, M * Nf, 777, True)[:, 0].reshape(M, Nf)
+    peak = P.max(axis=1)
+    for z in (2.0, 3.0, 4.0):
+        emp = float((peak > z).mean())
+        q = float(oracle.false_alarm_probability(np.array([z]), Nt, float(Nf))[0])
+        se = np.sqrt(q * (1 - q) / M)
+        assert abs(emp - q) <= 4.5 * se, (z, emp, q, se)
+        q1 = float(oracle.false_alarm_probability(np.array([z]), Nt, 1.0)[0])
+        assert abs(emp - q1) > 8 * se                      # N_f really enters
 
 
 def test_paper_facts_fixture():

@@ -1,13 +1,24 @@
 #!/usr/bin/env python
 """bench.py -- Lomb-Scargle term-evaluation throughput on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference] [--shard series|freq]
 
 One "step" = one pass of the whole hot path (moments -> records -> accumulate -> finish, all rows of
 SURVEY.md section 8(a)) over one seeded synthetic workload.  N = 1 times BASELINE.json's headline config
-C5 (Nt = Nf = 1e6, one series).  N > 1 (torchrun): every rank runs its own series of the same shape
-(weak scaling, no data-path collective: the path shards by independent series / frequencies,
-SURVEY.md section 8(e)); value = all ranks' terms / max-over-ranks time.
+C5 (Nt = Nf = 1e6, one series).
+
+The line of record (top-level `value`, `dtype`, `roofline`) is the FP32-pipe form of the path (LSP_PIPE_FP32): the
+paper's arithmetic -- fp32 throughout, SFU sin/cos at the anchors -- against the FP32 +
+MUFU issue roofline BASELINE.json's metric names.  The same run then times the library's automatic plan, which on this
+workload is the tensor-core factorisation with fp16 hi + e5m2 correction operands, and reports it as the sub-record
+`fast_path` (its own events, clocks, roofline and parity): narrower operand arithmetic than the paper's, so it is never
+the headline.  `parity` carries max|P_gpu - P_oracle| / max P_oracle and the arg-max agreement of each timed
+configuration on the oracle subset this run computes for `cpu_baseline` (outside the timed regions).
+
+N > 1 (torchrun): --shard series (default): every rank runs its own series of the same shape (weak scaling, no data-path
+collective: the path shards by independent series); value = all ranks' terms / max-over-ranks
+time.  --shard freq: ONE series, rank g computes the contiguous frequency slice (f_min + k_g df, df, Nf_g) and the global
+peak is merged by an 8-byte MAXLOC exchange (strong scaling).
 
 Prints ONE JSON line (rank 0).  `--impl reference` times the fp64 oracle (oracle/, the CPU baseline)
 on a bounded sample of the same workload instead.
@@ -38,6 +49,9 @@ TENSOR_FLOP_PER_TERM_EXECUTED = 32   # W runs as three fp16 passes (hi*hi + lo*h
 TENSOR_FLOP_PER_TERM_EXECUTED_CORR8 = 24   # fp16-rate equivalent when both correction products share one e5m2 MMA of K = 32
                                            # (16 FLOP per term at twice the fp16 rate): hi*hi 8 + corrections 8 + V 8
 FP32_LANES_PER_SM = 128          # B200: 4 SMSPs x 32 FP32 lanes (guide: blackwell_cuda_programming.md)
+MUFU_LANES_PER_SM = 16           # 4 SMSPs x 4
+NOMINAL_FP16_TFLOPS = 2250.0     # dense fp16/bf16 tensor peak of B200 (B200_PROFILING.md)
+PIPE_FP32, PIPE_TENSOR = 1, 2
 
 
 # ----------------------------------------------------------------------------- helpers (host logic)
@@ -61,6 +75,31 @@ def reduce_max(value: float, dist=None) -> float:
 
 def aggregate_value(terms_per_rank: int, world: int, max_seconds: float) -> float:
     return terms_per_rank * world / max_seconds
+
+
+def freq_slice(Nf: int, world: int, rank: int):
+    """--shard freq: rank g owns the contiguous grid indices [k0, k0 + n) -- every k once, sizes
+    differing by at most one -- and calls the library with (f_min + k0 df, df, n)."""
+    base, extra = divmod(int(Nf), int(world))
+    n = base + (1 if rank < extra else 0)
+    k0 = rank * base + min(rank, extra)
+    return k0, n
+
+
+def merge_peaks(local_val: float, local_idx: int, dist=None):
+    """Global peak of a frequency-sharded periodogram: MAXLOC over the ranks' (value, global index) pairs, the LOWEST
+    index among equal maxima (reading G9).  8 bytes of payload per rank (fp32 value + int32 index)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(local_val), int(local_idx)
+    import torch
+    mine = torch.tensor([float(local_val), float(local_idx)], dtype=torch.float64)      # the index is exact in fp64 (< 2^31)
+    if dist.get_backend() == "nccl":
+        mine = mine.cuda()
+    allp = [torch.empty_like(mine) for _ in range(dist.get_world_size())]
+    dist.all_gather(allp, mine)
+    pairs = [(float(p[0]), int(p[1])) for p in allp]
+    best = max(v for v, _ in pairs)
+    return best, min(i for v, i in pairs if v == best)
 
 
 def measured_peaks() -> dict:
@@ -125,24 +164,27 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- oracle legs (CPU)
-def time_oracle(w, seconds_target: float = 12.0, max_freqs: int = 4096):
+def time_oracle(w, seconds_target: float = 12.0, max_freqs: int = 4096, keep: bool = False):
     """Time the fp64 oracle, as it stands, on a strided subset of the workload's frequency grid.
 
-    Returns (terms_per_s, cores, sample_description, elapsed_s)."""
+    Returns (terms_per_s, cores, sample_description, elapsed_s[, ks, P_ref of series 0 when keep])."""
     import oracle
     t = w.t[0] if (w.B > 1 and w.t.ndim == 2) else w.t          # batch: series 0 (shared-time batch: the one time vector)
     x = w.x[0] if w.B > 1 else w.x
     cores = oracle.host_threads()
     oracle.periodogram(t[:1000], x[:1000], w.f_min, w.df, 8)          # build + warm the library
     done, elapsed, n = 0, 0.0, max(8, cores * 4)
+    kept_ks, kept_P = [], []
     while elapsed < seconds_target and done < max_freqs:
         n = min(n, max_freqs - done)
         stride = max(1, w.Nf // n)
         ks = (np.arange(n, dtype=np.int64) * stride + done % stride) % w.Nf
         t0 = time.perf_counter()
-        _, used = oracle.periodogram(t, x, w.f_min, w.df, w.Nf, ks=ks, return_threads=True)
+        P, used = oracle.periodogram(t, x, w.f_min, w.df, w.Nf, ks=ks, return_threads=True)
         dt = time.perf_counter() - t0
         elapsed += dt; done += n; cores = used
+        if keep:
+            kept_ks.append(ks); kept_P.append(P)
         rate = n * w.Nt / dt
         n = int(min(max_freqs, max(n, rate * (seconds_target - elapsed) / w.Nt * 0.9))) or 1
         if seconds_target - elapsed < 0.5:
@@ -150,7 +192,25 @@ def time_oracle(w, seconds_target: float = 12.0, max_freqs: int = 4096):
     terms = done * w.Nt
     sample = "%d of %d frequencies (strided) x Nt=%d samples of %s%s" % (
         done, w.Nf, w.Nt, w.name, " series 0" if w.B > 1 else "")
+    if keep:
+        return terms / elapsed, cores, sample, elapsed, np.concatenate(kept_ks), np.concatenate(kept_P)
     return terms / elapsed, cores, sample, elapsed
+
+
+def parity_record(w, P_gpu, ks, P_ref, peak_gpu: int):
+    """max|P_gpu - P_oracle| / max P_oracle on the oracle subset of this run, plus the arg-max: the oracle over a dense
+    window of +-32 bins around the GPU's peak (and the expected bin) must put its maximum at the GPU's index."""
+    import oracle
+    t = w.t[0] if (w.B > 1 and w.t.ndim == 2) else w.t
+    x = w.x[0] if w.B > 1 else w.x
+    centres = [peak_gpu] + ([int(round(w.expected_peak_bin))] if w.expected_peak_bin is not None else [])
+    win = np.unique(np.concatenate([np.arange(max(0, c - 32), min(w.Nf, c + 33), dtype=np.int64) for c in centres]))
+    P_win = oracle.periodogram(t, x, w.f_min, w.df, w.Nf, ks=win)
+    all_ks = np.concatenate([ks, win]); all_ref = np.concatenate([P_ref, P_win])
+    err = float(np.max(np.abs(P_gpu[all_ks].astype(np.float64) - all_ref)) / np.max(all_ref))
+    k_ref = int(all_ks[int(np.argmax(all_ref))])
+    return {"max_rel_err": err, "tolerance": 1e-4, "argmax_equal": bool(k_ref == int(peak_gpu)), "argmax_gpu": int(peak_gpu),
+            "argmax_oracle_on_sample": k_ref, "frequencies_compared": int(all_ks.size)}
 
 
 def run_reference(args):
@@ -183,6 +243,67 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------- our arm (GPU)
+def roofline_record(terms, B, Nt, Nf, plan, k_ms, all_ms, clocks, peaks, n_sm, workload_name):
+    """Roofline of the dominant (accumulate) kernel of one timed configuration."""
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    lane_ops = plan["lane_ops_per_term"]
+    sm_mhz = clocks.get("sm_mhz") if clocks else None
+    if lane_ops:                                             # FP32-pipe form: 6 lane-ops (FMA = 2 FLOP) per term
+        achieved = terms * lane_ops * 2 / (k_ms * 1e-3) / 1e12
+        mufu_per_s = terms * 2.0 / plan["K"] / (k_ms * 1e-3)            # one MUFU.SIN + one MUFU.COS per anchor = per K terms
+        mufu_peak = n_sm * MUFU_LANES_PER_SM * sm_max * 1e6
+        rec = {
+            "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+            "lane_ops_per_term": lane_ops,
+            "peak_basis": "FP32 issue: %d SMs x 128 FP32 lanes x 2 FLOP x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json%s)"
+                          % (n_sm, sm_max, "" if peaks else "; fallback"),
+            "frac_at_measured_clock": (achieved / (n_sm * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12)) if sm_mhz else None,
+            "mufu_frac": mufu_per_s / mufu_peak,
+            "mufu_basis": "2 MUFU per K = %d terms against %d SMs x 16 lanes x %.0f MHz" % (plan["K"], n_sm, sm_max),
+        }
+    else:                                                    # tensor-core form: 8 real MACs = 16 FLOP per term (DESIGN.md)
+        tpeak = float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1590.0)))   # fp16 rate = bf16 rate
+        burst = float(peaks.get("bf16_tflops", tpeak))
+        alg_flop = TENSOR_FLOP_PER_TERM
+        executed = TENSOR_FLOP_PER_TERM_EXECUTED_CORR8 if "e5m2corr" in plan["kernel"] else TENSOR_FLOP_PER_TERM_EXECUTED
+        if "shared_gemm" in plan["kernel"]:                  # shared-time batch: only W = XC + i XS is per series (one real MAC each for
+            alg_flop, executed = 4, 8                        # cos and sin: 4 FLOP per term); executed: main product 4 + e5m2 corrections 4
+        achieved = terms * alg_flop / (k_ms * 1e-3) / 1e12
+        rec = {
+            "bound": "tensor", "achieved": achieved, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved / tpeak,
+            "frac_vs_burst_peak": achieved / burst, "frac_vs_nominal_fp16_peak": achieved / NOMINAL_FP16_TFLOPS,
+            "flop_per_term_algorithmic": alg_flop, "flop_per_term_executed": executed,
+            "frac_executed": achieved * executed / alg_flop / tpeak,
+            "peak_basis": "MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16 back to back; fp16 has the same nominal "
+                          "rate; the kernel is timed inside a step that is itself power-capped): %s"
+                          % ("measured" if peaks else "fallback 1590"),
+            "fp32_alu_equivalent_frac": terms * 12 / (k_ms * 1e-3) / 1e12 / peak_tflops,
+        }
+    alg_bytes = 12.0 * B * Nt + 4.0 * B * Nf
+    rec.update({
+        "traffic": None, "kernel": plan["kernel"], "kernel_ms": k_ms,
+        "kernel_share_of_step": k_ms / statistics.mean(all_ms),
+        "algorithmic_bytes": alg_bytes, "hbm_GBps_algorithmic": alg_bytes / (k_ms * 1e-3) / 1e9,
+    })
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        try:
+            with open(prof) as fh:
+                rec["traffic"] = json.load(fh).get("%s/%s" % (workload_name, plan["kernel"]))
+        except Exception:
+            pass
+    if rec["traffic"]:
+        rec["traffic_over_algorithmic"] = rec["traffic"] / alg_bytes
+    return rec
+
+
+def dtype_of(plan) -> str:
+    if plan["lane_ops_per_term"]:
+        return "f32"
+    return "f16 + e5m2 correction operands, f32 accumulate" if "e5m2corr" in plan["kernel"] else "f16 hi+lo operands, f32 accumulate"
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -196,13 +317,20 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dd = dist if world > 1 else None
 
-    w = workloads.make(args.workload, seed=rank_seed(args.workload, rank))
+    shard_freq = args.shard == "freq" and world > 1
+    w = workloads.make(args.workload, seed=None if shard_freq else rank_seed(args.workload, rank))
+    if shard_freq and w.B > 1:
+        raise SystemExit("--shard freq is for a single series")
     batched = w.B > 1
+    k0, Nf_local = freq_slice(w.Nf, world, rank) if shard_freq else (0, w.Nf)
+    f_min_local = w.f_min + k0 * w.df
+    terms_local = w.B * w.Nt * Nf_local
     h = lsp.Handle(local)
     for key, val in ((lsp.PARAM_K, args.K), (lsp.PARAM_THREADS, args.threads), (lsp.PARAM_NSPLIT, args.nsplit),
-                     (lsp.PARAM_RECURRENCE, args.recurrence), (lsp.PARAM_FLUSH, args.flush), (lsp.PARAM_BTABLE, args.btable),
-                     (lsp.PARAM_COARSE, args.coarse), (lsp.PARAM_CORR, args.corr), (lsp.PARAM_PAIR, args.pair)):
+                     (lsp.PARAM_FLUSH, args.flush), (lsp.PARAM_TABLE_MB, args.table_mb), (lsp.PARAM_COARSE, args.coarse),
+                     (lsp.PARAM_TRUNC, args.trunc)):
         if val:
             h.set_param(key, val)
     h.set_param(lsp.PARAM_TIMING, 1)
@@ -211,62 +339,79 @@ def run_ours(args):
     x_h = torch.from_numpy(np.ascontiguousarray(w.x)).pin_memory()
     t_d, x_d = t_h.cuda(), x_h.cuda()
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")        # > 126 MB L2
+    shape = (w.B, Nf_local) if batched else (Nf_local,)
+    P_d = torch.empty(shape, dtype=torch.float32, device="cuda")
+    P_h = torch.empty(shape, dtype=torch.float32).pin_memory()
+    pi_h = torch.empty(w.B, dtype=torch.int32).pin_memory()
+    pv_h = torch.empty(w.B, dtype=torch.float32).pin_memory()
+    out = {}
 
     def step_device():
         if batched:
-            return h.periodogram_batched(t_d, x_d, w.f_min, w.df, w.Nf)
-        return h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf)
-
-    P_h = torch.empty((w.B, w.Nf) if batched else (w.Nf,), dtype=torch.float32).pin_memory()
-    pi_h = torch.empty(w.B, dtype=torch.int32).pin_memory()
-    pv_h = torch.empty(w.B, dtype=torch.float32).pin_memory()
+            out["P"], out["pi"], out["pv"] = h.periodogram_batched(t_d, x_d, f_min_local, w.df, Nf_local)
+        else:
+            out["P"] = h.periodogram(t_d, x_d, f_min_local, w.df, Nf_local, out=P_d)
 
     def step_host():
         if batched:
-            h.periodogram_batched_host(t_h, x_h, w.f_min, w.df, w.Nf, P=P_h, peak_idx=pi_h, peak_val=pv_h)
+            h.periodogram_batched_host(t_h, x_h, f_min_local, w.df, Nf_local, P=P_h, peak_idx=pi_h, peak_val=pv_h)
         else:
-            h.periodogram_host(t_h, x_h, w.f_min, w.df, w.Nf, out=P_h)
+            h.periodogram_host(t_h, x_h, f_min_local, w.df, Nf_local, out=P_h)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(3, args.warmup)):
-        step_device()
-    torch.cuda.synchronize()
+    def time_config(pipe: int):
+        """Warm up, then time exactly `steps` device-resident steps (CUDA events, L2 flushed between them, clocks sampled
+        during), then the end-to-end host-buffer steps.  Returns the raw measurements of this configuration."""
+        h.set_param(lsp.PARAM_PIPE, pipe)
+        for _ in range(max(3, args.warmup)):
+            step_device()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+            time.sleep(0.3)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        barrier()
+        for ea, eb in evs:
+            flush_buf.zero_()                                   # L2 flush between timed iterations (outside the step's events)
+            ea.record()
+            step_device()                                       # enqueue only: no host sync inside the timed region
+            eb.record()
+        barrier()
+        total_ms = sum(ea.elapsed_time(eb) for ea, eb in evs)   # device time of exactly K steps, flushes excluded
+        kern_ms, all_ms = [], []
+        for back in range(min(args.steps, 64)):                 # per-kernel CUDA events recorded by the library on
+            tm = h.call_timing(back)                            # the launching stream during the timed region
+            kern_ms.append(tm["accumulate"]); all_ms.append(sum(tm.values()))
+        clocks = sampler.stop() if rank == 0 else None
+        plan = h.last_plan()
+        P_last = out["P"].clone()
+        peak = None
+        if not batched:                                         # global peak; merged over the ranks when the grid is sharded
+            pv, pi = torch.max(P_last, dim=0)
+            peak = merge_peaks(float(pv), int(pi) + k0, dd if shard_freq else None)
+        # end to end through the host-buffer C-ABI call (H2D + compute + D2H inside the timed region)
+        for _ in range(2):
+            step_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step_host()
+        torch.cuda.synchronize()
+        e2e_s = reduce_max((time.perf_counter() - t0) / args.steps, dd)
+        return {"pipe": pipe, "ms_per_step": reduce_max(total_ms / args.steps, dd), "kern_ms": kern_ms, "all_ms": all_ms,
+                "clocks": clocks, "plan": plan, "P": P_last, "peak": peak, "e2e_s": e2e_s}
 
-    # ---- timed region 1: device-resident inputs
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-        time.sleep(0.3)
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern_ms, all_ms = [], []
-    barrier()
-    for ea, eb in evs:
-        flush_buf.zero_()                                   # L2 flush between timed iterations (outside the step's events)
-        ea.record()
-        step_device()                                       # enqueue only: no host sync inside the timed region
-        eb.record()
-    barrier()
-    total_ms = sum(ea.elapsed_time(eb) for ea, eb in evs)   # device time of exactly K steps, flushes excluded
-    for back in range(min(args.steps, 64)):                 # per-kernel CUDA events recorded by the library on
-        tm = h.call_timing(back)                            # the launching stream during the timed region
-        kern_ms.append(tm["accumulate"]); all_ms.append(sum(tm.values()))
-    clocks = sampler.stop() if rank == 0 else None
-    ms_per_step = reduce_max(total_ms / args.steps, dist if world > 1 else None)
-    plan = h.last_plan()
-
-    # ---- timed region 2: end to end through the host-buffer C-ABI call (H2D + compute + D2H)
-    for _ in range(2):
-        step_host()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step_host()
-    torch.cuda.synchronize()
-    e2e_s = reduce_max((time.perf_counter() - t0) / args.steps, dist if world > 1 else None)
+    rec = time_config(args.pipe if args.pipe else PIPE_FP32)              # the line of record: the paper's fp32 arithmetic
+    fast = None
+    if not args.pipe and not args.no_fast_path:
+        fast = time_config(0)                                             # the library's automatic plan
+        if fast["plan"]["kernel"] == rec["plan"]["kernel"]:
+            fast = None                                                   # (same kernel: nothing to add)
     h2d = t_h.numel() * 8 + x_h.numel() * 4
     d2h = P_h.numel() * 4 + (pi_h.numel() * 8 if batched else 0)
 
@@ -276,74 +421,60 @@ def run_ours(args):
             dist.destroy_process_group()
         return 0
 
-    value = aggregate_value(w.terms, world, ms_per_step * 1e-3)
-    # ---- roofline of the dominant kernel (accumulate): FP32 pipe, FMA = 2 FLOP per lane-op
     peaks = measured_peaks()
-    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
-    peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-    k_ms = statistics.mean(kern_ms)
-    lane_ops = plan["lane_ops_per_term"]
-    if lane_ops:                                             # FP32-pipe forms: 6 or 8 lane-ops (FMA = 2 FLOP) per term
-        achieved = w.terms * lane_ops * 2 / (k_ms * 1e-3) / 1e12
-        roofline = {
-            "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-            "lane_ops_per_term": lane_ops,
-            "peak_basis": "%d SMs x 128 FP32 lanes x 2 FLOP x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)" % (n_sm, sm_max),
-            "frac_at_measured_clock": (achieved / (n_sm * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
-                                       if clocks and clocks.get("sm_mhz") else None),
-        }
-    else:                                                    # tensor-core form: 8 real MACs = 16 FLOP per term
-        tpeak = float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1590.0)))   # fp16 rate = bf16 rate
-        alg_flop = TENSOR_FLOP_PER_TERM
-        executed = TENSOR_FLOP_PER_TERM_EXECUTED_CORR8 if "e5m2corr" in plan["kernel"] else TENSOR_FLOP_PER_TERM_EXECUTED
-        if "shared_gemm" in plan["kernel"]:                  # shared-time batch: only W = XC + i XS is per series (one real MAC each for
-            alg_flop, executed = 4, 8                        # cos and sin: 4 FLOP per term); executed: main product 4 + e5m2 corrections 4
-        achieved = w.terms * alg_flop / (k_ms * 1e-3) / 1e12
-        roofline = {
-            "bound": "tensor", "achieved": achieved, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved / tpeak,
-            "flop_per_term_algorithmic": alg_flop, "flop_per_term_executed": executed,
-            "frac_executed": achieved * executed / alg_flop / tpeak,
-            "peak_basis": "MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16 back to back; fp16 has the same nominal "
-                          "rate; the kernel is timed inside a step that is itself power-capped): %s"
-                          % ("measured" if peaks else "fallback 1590"),
-            "fp32_form_note": "the FP32-pipe form of the same path (--recurrence 3) reaches 0.82 of the FP32 issue "
-                              "roofline at 6 lane-ops per term (profiles/r01_bench_fp32.md)",
-            "fp32_alu_equivalent_frac": w.terms * 12 / (k_ms * 1e-3) / 1e12 / peak_tflops,
-        }
-    roofline.update({
-        "traffic": None, "kernel": plan["kernel"], "kernel_ms": k_ms,
-        "kernel_share_of_step": k_ms / statistics.mean(all_ms),
-        "hbm_GBps_algorithmic": (12.0 * w.B * w.Nt + 4.0 * w.B * w.Nf) / (k_ms * 1e-3) / 1e9,
-    })
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(prof):
-        try:
-            with open(prof) as fh:
-                roofline["traffic"] = json.load(fh).get("%s/%s" % (w.name, plan["kernel"]))
-        except Exception:
-            pass
 
-    cpu = None
+    cpu, oracle_keep = None, None
     if world == 1 and not args.no_cpu_baseline:
-        r, cores, sample, _ = time_oracle(w, seconds_target=args.cpu_seconds)
+        r, cores, sample, _, ks, P_ref = time_oracle(w, seconds_target=args.cpu_seconds, keep=True)
         cpu = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        oracle_keep = (ks, P_ref)
 
+    def whole_job(seconds):
+        return w.terms / seconds if shard_freq else aggregate_value(terms_local, world, seconds)
+
+    def finish_record(m):
+        k_ms = statistics.mean(m["kern_ms"])
+        roof = roofline_record(terms_local, w.B, w.Nt, Nf_local, m["plan"], k_ms, m["all_ms"], m["clocks"], peaks, n_sm, w.name)
+        d = {"dtype": dtype_of(m["plan"]), "value": whole_job(m["ms_per_step"] * 1e-3), "unit": UNIT, "ms_per_step": m["ms_per_step"],
+             "plan": m["plan"], "clocks": m["clocks"],
+             "e2e": {"value": whole_job(m["e2e_s"]), "unit": UNIT, "ms_per_step": m["e2e_s"] * 1e3,
+                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+             "gpu_launches": m["plan"]["launches"] * args.steps, "roofline": roof}
+        if oracle_keep is not None:
+            Pg = m["P"].cpu().numpy()
+            Pg0 = Pg[0] if batched else Pg
+            d["parity"] = parity_record(w, Pg0, oracle_keep[0], oracle_keep[1], int(np.argmax(Pg0)))
+        if m["peak"] is not None:
+            d["peak"] = {"value": m["peak"][0], "index": m["peak"][1]}
+        return d
+
+    r0 = finish_record(rec)
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32" if lane_ops else ("f16 + e5m2 correction operands, f32 accumulate" if "e5m2corr" in plan["kernel"]
-                                                         else "f16 hi+lo operands, f32 accumulate"), "data": "synthetic",
-        "config": {"workload": w.name, "Nt": w.Nt, "Nf": w.Nf, "series": w.B, "terms_per_step": w.terms,
-                   "l2": "flushed between timed iterations (256 MB write)", "plan": plan,
-                   "parallelism": "independent series per rank" if world > 1 else "single GPU"},
-        "clocks": clocks,
-        "e2e": {"value": aggregate_value(w.terms, world, e2e_s), "unit": UNIT, "ms_per_step": e2e_s * 1e3,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": plan["launches"] * args.steps,
-        "roofline": roofline,
+        "metric": METRIC, "value": r0["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": r0["ms_per_step"], "higher_is_better": True,
+        "scaling": "strong" if shard_freq else "weak",
+        "vs_baseline": None, "dtype": r0["dtype"], "data": "synthetic",
+        "config": {"workload": w.name, "Nt": w.Nt, "Nf": w.Nf, "series": w.B,
+                   "terms_per_step": w.terms * (1 if shard_freq else world),
+                   "l2": "flushed between timed iterations (256 MB write)", "plan": r0["plan"],
+                   "arithmetic": "line of record = LSP_PIPE_FP32 (the paper's fp32 arithmetic, PAPER.md:140, :290); "
+                                 "fast_path = the library's automatic plan, timed in the same run",
+                   "parallelism": ("single GPU" if world == 1 else
+                                   ("one series, contiguous frequency slices per rank, MAXLOC peak merge" if shard_freq
+                                    else "independent series per rank"))},
+        "clocks": r0["clocks"], "e2e": r0["e2e"], "gpu_launches": r0["gpu_launches"], "roofline": r0["roofline"],
         "cpu_baseline": cpu,
     }
+    for k in ("parity", "peak"):
+        if k in r0:
+            line[k] = r0[k]
+    if fast is not None:
+        f0 = finish_record(fast)
+        f0["note"] = ("tensor-core factorisation of the same sums (DESIGN.md section 6b): operand arithmetic narrower than "
+                      "the paper's fp32, inside the path's 1e-4 max P tolerance; reported, not the headline")
+        f0["speedup_over_line_of_record"] = r0["ms_per_step"] / f0["ms_per_step"]
+        line["fast_path"] = f0
     if batched:
         # BASELINE config 4: "report per-series peak power distribution" -- the peaks the last host-buffer step returned,
         # and their false-alarm probabilities by eq. (3) with N_ind = Nf (lsp_false_alarm)
@@ -374,8 +505,8 @@ def run_sweep(args):
     import paper_1007_1658_b200 as lsp
     base = workloads.make(args.workload)
     h = lsp.Handle(0)
-    if args.pair:
-        h.set_param(lsp.PARAM_PAIR, args.pair)
+    if args.pipe:
+        h.set_param(lsp.PARAM_PIPE, args.pipe)
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     rows = []
     for step in (64, 32, 16, 8, 4, 2, 1):
@@ -412,15 +543,17 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5")
+    ap.add_argument("--shard", default="series", choices=["series", "freq"],
+                    help="N > 1: independent series per rank (weak scaling) or frequency slices of one series (strong scaling)")
+    ap.add_argument("--pipe", type=int, default=0, help="time ONLY this form (1 = FP32 pipe, 2 = tensor cores) instead of the line of record + fast path")
+    ap.add_argument("--no-fast-path", action="store_true", help="skip the automatic-plan sub-record")
     ap.add_argument("--K", type=int, default=0)
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--nsplit", type=int, default=0)
-    ap.add_argument("--recurrence", type=int, default=0)
     ap.add_argument("--flush", type=int, default=0)
-    ap.add_argument("--btable", type=int, default=0)
+    ap.add_argument("--table-mb", type=int, default=0, dest="table_mb")
     ap.add_argument("--coarse", type=int, default=0)
-    ap.add_argument("--corr", type=int, default=0, help="tcgen05 table form: 1 = hi*lo corrections as two fp16 MMAs, 0/2 = one e5m2 MMA")
-    ap.add_argument("--pair", type=int, default=0, help="tcgen05 table form: 1 = no CTA pairs, 2 = pairs share the streamed operand, 0/3 = the generated one")
+    ap.add_argument("--trunc", type=int, default=0)
     ap.add_argument("--sweep", action="store_true", help="N_t scaling sweep of --workload (single series) instead of the bench line")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

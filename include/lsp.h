@@ -18,7 +18,10 @@
  *   - Pointers marked DEVICE are CUDA device pointers on the handle's device; pointers marked
  *     HOST are ordinary (pageable or pinned) host pointers.  The caller owns every array; the
  *     library never frees or reallocates caller memory.  The handle owns a device workspace
- *     that grows to the largest call seen (growth may synchronise the device once).
+ *     that grows to the largest call seen (growth allocates and may synchronise the device once;
+ *     lsp_reserve sizes it ahead of time).  Size: 32 B per sample + 16 B x Nf x (time splits, <= 2 GiB)
+ *     + at most LSP_PARAM_TABLE_MB for the tensor form's table; if it cannot be allocated the call
+ *     returns LSP_ENOMEM and the handle keeps the workspace it had.
  *   - Device-pointer entry points only ENQUEUE work on `stream` (a cudaStream_t passed as
  *     void*; NULL = legacy default stream) and return without synchronising; inputs must stay
  *     valid until the stream reaches the end of the call.  Host-pointer entry points copy
@@ -43,33 +46,37 @@ typedef struct lsp_ctx* lsp_handle;            /* opaque; owns the device worksp
 
 enum {
     LSP_OK      =  0,
-    LSP_EINVAL  = -1,   /* NULL handle/pointer, Nt < 2, Nf < 1, B < 1, bad stride, non-finite or negative f_min/df */
+    LSP_EINVAL  = -1,   /* NULL handle/pointer, Nt < 2, Nf < 1, B < 1 or B > 65,535, bad stride, non-finite or negative f_min/df */
     LSP_ECUDA   = -2,   /* a CUDA runtime call failed; see lsp_last_cuda_error */
     LSP_ENOMEM  = -3    /* workspace allocation failed */
 };
 
-/* Tunables for lsp_set_param (all optional; 0 restores the automatic choice). */
+/*
+ * Tunables for lsp_set_param (all optional; 0 restores the automatic choice).  Steps 3-5 of the path (anchor, rotate and
+ * accumulate, cascade: the O(Nt*Nf) part) exist in two forms that compute the same sums of eq. (8):
+ *   LSP_PIPE_FP32    the paper's arithmetic: fp32 throughout, SFU sin/cos at anchors,
+ *                    K adjacent frequencies per thread advanced by a re-anchored three-term recurrence; 6 FP32 lane-ops per term.
+ *   LSP_PIPE_TENSOR  the same recurrence (angle addition) factorised over a uniform grid into a dense contraction and run
+ *                    on the tensor cores with fp16 hi + lo operands (22 bits; by default the two small cross products share
+ *                    one e5m2 MMA) and fp32 accumulation; about ten times faster, within the 1e-4 max P tolerance of the path.
+ * Automatic: the tensor form when Nt >= 512 and the cost model says it is faster.
+ */
 enum {
-    LSP_PARAM_K         = 1,  /* adjacent frequencies per thread: 4, 8, 12, 16, 20, 24 (32: z form only) */
-    LSP_PARAM_THREADS   = 2,  /* threads per CTA of the accumulate kernel: 32..256 (multiple of 32) */
-    LSP_PARAM_NSPLIT    = 3,  /* number of time-axis splits per (series, frequency block)       */
-    LSP_PARAM_RECURRENCE= 4,  /* 1 = plane rotation, two samples per f32x2 (8 FP32 lane-ops/term) */
-                              /* 2 = three-term (Chebyshev) recurrence, two samples per f32x2 (6)   */
-                              /* 3 = three-term, (cos,sin) of one sample per f32x2 (6) -- default    */
-                              /* 4 = tensor-core form, mma.sync m16n8k16 fp16 hi+lo, fp32 accumulate   */
-                              /* 5 = tensor-core form, tcgen05.mma m128n256k16, accumulators in TMEM   */
-    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the partial sums / drains of the TMEM accumulators (default 2,048; 4,096 in the */
-                              /* default CTA-pair kernel, whose drain adds the expected truncation loss of the tensor-core accumulation back) */
+    LSP_PARAM_K         = 1,  /* FP32 form: adjacent frequencies per thread: 4, 8, ..., 32 */
+    LSP_PARAM_THREADS   = 2,  /* FP32 form: threads per CTA: 32..256 (multiple of 32; <= 128 for K >= 28) */
+    LSP_PARAM_NSPLIT    = 3,  /* number of time-axis splits per (series, frequency block) */
+    LSP_PARAM_PIPE      = 4,  /* LSP_PIPE_FP32 or LSP_PIPE_TENSOR (see above) */
+    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the fp32 partial sums / drains of the TMEM accumulators (default 2,048) */
     LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
-    LSP_PARAM_BTABLE    = 7,  /* tcgen05 form only: 0 = coarse-operand table when >= 3 frequency blocks share it, 1 = never, 2 = always */
-    LSP_PARAM_COARSE    = 8,  /* tcgen05 form only: coarse extent L = 16, 32, 64 or 128 (a CTA owns 128 L frequencies) */
-    LSP_PARAM_CORR      = 9,  /* tcgen05 table form only: how the hi*lo correction products are issued: 0 / 2 = one 8-bit (e5m2)  */
-                              /* MMA of K = 32 (3 tensor slots per k-step), 1 = two fp16 MMAs (4 slots)                           */
-    LSP_PARAM_DUO       = 12, /* batches on the 2,048-frequency tile: 0 / 2 = two series per CTA (64 fine x 32 coarse each), 1 = one series per CTA (128 x 16) */
-    LSP_PARAM_SHARED    = 11, /* batched call with t_stride = 0: 0 = the shared-time GEMM path when B >= 16 and Nt >= 512, 1 = never, 2 = always */
-    LSP_PARAM_PAIR      = 10  /* tcgen05 table form with the e5m2 correction only: CTA pairs (cta_group::2, M = 256): 0 / 3 = the pair  */
-                              /* shares the generated operand (64 sin/cos per sample per CTA), 2 = it shares the streamed one, 1 = no pairs */
+    LSP_PARAM_TABLE_MB  = 7,  /* tensor form, CTA-pair kernel: MiB of workspace its operand table may take (default 1,024);  */
+                              /* a series whose table (3 KB per sample) is larger runs in time chunks, same result             */
+    LSP_PARAM_COARSE    = 8,  /* tensor form: coarse extent L = 16, 32, 64 (a CTA owns 128 L frequencies) or 128 (CTA pairs,   */
+                              /* 32,768 frequencies per pair, one operand streamed from the table)                             */
+    LSP_PARAM_TRUNC     = 9,  /* tensor form, CTA-pair kernel: 1 = do not add the expected round-toward-zero loss of the       */
+                              /* tensor-core accumulation back at each drain; 0 = add it (default)       */
+    LSP_PARAM_SHARED    = 11  /* batched call with t_stride = 0: 0 = the shared-time GEMM path when B >= 16 and Nt >= 512, 1 = never, 2 = always */
 };
+enum { LSP_PIPE_AUTO = 0, LSP_PIPE_FP32 = 1, LSP_PIPE_TENSOR = 2 };
 
 /* Create a handle bound to CUDA device `device` (-1 = the calling thread's current device). */
 int lsp_create(lsp_handle* out, int device);
@@ -86,8 +93,9 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value);
  *   t  DEVICE const double[Nt]   sample times
  *   x  DEVICE const float [Nt]   measurements (any mean / variance; normalised inside)
  *   P  DEVICE       float [Nf]   written; exactly Nf values (reading G8: no rounding up to blocks)
- * Enqueues 3-5 kernels on `stream` (lsp_last_plan reports how many); no host synchronisation, no allocation once the
- * workspace has grown to the problem size: the call can be captured into a CUDA graph.
+ * Enqueues 3-5 kernels on `stream` (more when the series runs in time chunks; lsp_last_plan reports how many); no host
+ * synchronisation, no allocation once the workspace has grown to the problem size (lsp_reserve): the call can be captured
+ * into a CUDA graph.
  */
 int lsp_periodogram(lsp_handle h,
                     const double* t, const float* x, int64_t Nt,
@@ -97,7 +105,7 @@ int lsp_periodogram(lsp_handle h,
 /*
  * B independent series on one shared frequency grid (the Monte-Carlo use of PAPER.md:369).
  *   series b reads t + b*t_stride and x + b*x_stride (strides in ELEMENTS; t_stride = 0 means
- *   all series share one time vector; otherwise |stride| >= Nt), writes P + b*p_stride.
+ *   all series share one time vector; otherwise |stride| >= Nt), writes P + b*p_stride.  1 <= B <= 65,535.
  *   With t_stride = 0 (the Monte-Carlo use: sampling kept, noise redrawn) and B >= 16, Nt >= 512 the sums sum_j X_bj cos / sin
  *   are evaluated as ONE dense contraction over all series and CC, CS once per frequency (same result, ~5x faster).
  *   P may be NULL if only the peaks are wanted (then p_stride is ignored).
@@ -164,8 +172,16 @@ int lsp_periodogram_batched_host(lsp_handle h,
 int lsp_false_alarm(lsp_handle h, const float* P, int64_t n, int64_t Nt, double N_ind, float* Q, void* stream);
 
 /*
+ * Grow the workspace now to what a call with (B series -- `shared_t` != 0: on one time vector --, Nt samples, Nf
+ * frequencies, generalised or not) needs under the handle's current tunables, so that the call itself allocates nothing
+ * (CUDA-graph capture, latency-critical first calls).  May synchronise the device.  LSP_ENOMEM leaves the workspace as it was.
+ */
+int lsp_reserve(lsp_handle h, int64_t B, int shared_t, int64_t Nt, int64_t Nf, int generalised);
+
+/*
  * Introspection of the last call's launch plan (for benchmarks and tests): fills
- * out[0..7] = {K, threads, nsplit, recurrence, n_freq_blocks, split_len, launches, lane_ops_per_term}.
+ * out[0..7] = {K (FP32 form) or L (tensor form), threads, nsplit, pipe (LSP_PIPE_*), n_freq_blocks, split_len, launches,
+ *              FP32 lane-ops per term (6; 0 for the tensor form: 16 tensor FLOP per term)}.
  */
 int lsp_last_plan(lsp_handle h, int64_t out[8]);
 
@@ -185,19 +201,18 @@ int lsp_call_timing(lsp_handle h, int calls_back, float ms[4]);
 
 /*
  * Host-only: the launch plan the library would pick for (B series, Nt samples, Nf frequencies) on a
- * device with `sm_count` SMs.  Needs no GPU.  out[0..7] = {K, threads, nsplit, recurrence,
+ * device with `sm_count` SMs.  Needs no GPU.  out[0..7] = {K or L, threads, nsplit, pipe,
  * n_freq_blocks, split_len, resident CTAs per SM, model score * 1e6}.
  */
 int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[8]);
 
 /*
- * Same for one form of steps 3-5: recurrence = 0 (automatic, identical to lsp_plan_query) or a
- * LSP_PARAM_RECURRENCE value 1..5.  For the mma.sync form (4) K is reported as 32, `threads` = 256 and a
- * frequency block is 8,192 frequencies; for the tcgen05 form (5) K is the coarse extent L (16, 32, 64, 128),
- * a frequency block is 128 L frequencies and `threads` is the CTA size (288 for L < 128, 544 for L = 128).  out[7] = estimated
- * SM cycles of the accumulate kernel (the quantity the automatic choice compares), not the score.
+ * Same for one form of steps 3-5: pipe = LSP_PIPE_AUTO (identical to lsp_plan_query), LSP_PIPE_FP32 or LSP_PIPE_TENSOR.
+ * For the tensor form K is reported as the coarse extent L (16, 32, 64, 128), a frequency block is 128 L frequencies and
+ * `threads` is the CTA size (288 for L < 128, 544 for L = 128).  out[6] = time chunks (tensor form, L = 128) or resident CTAs
+ * per SM (otherwise); out[7] = estimated SM cycles of the accumulate kernels (the quantity the automatic choice compares).
  */
-int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int recurrence, int64_t out[8]);
+int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int pipe, int64_t out[8]);
 
 /* Name of the accumulate kernel the last call launched (static string; "" before any call). */
 const char* lsp_last_kernel_name(lsp_handle h);
@@ -208,7 +223,7 @@ int lsp_last_cuda_error(lsp_handle h);
 /* Human-readable text for a status code. */
 const char* lsp_status_string(int status);
 
-/* Library version string, e.g. "lsp_b200 0.1 (sm_100a)". */
+/* Library version string, e.g. "lsp_b200 0.2 (sm_100a)". */
 const char* lsp_version(void);
 
 #ifdef __cplusplus

@@ -13,16 +13,15 @@ from typing import Optional, Tuple
 from . import build as _build
 
 LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM = 0, -1, -2, -3
-PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_TIMING, PARAM_BTABLE, PARAM_COARSE, PARAM_CORR, PARAM_PAIR, PARAM_SHARED, PARAM_DUO = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12
-REC_MMA, REC_UMMA = 4, 5
-REC_ROTATION, REC_THREE_TERM, REC_THREE_TERM_Z = 1, 2, 3
+PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_PIPE, PARAM_FLUSH, PARAM_TIMING, PARAM_TABLE_MB, PARAM_COARSE, PARAM_TRUNC, PARAM_SHARED = 1, 2, 3, 4, 5, 6, 7, 8, 9, 11
+PIPE_AUTO, PIPE_FP32, PIPE_TENSOR = 0, 1, 2
 
 # every symbol include/lsp.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = (
     "lsp_create", "lsp_destroy", "lsp_set_param", "lsp_get_param",
     "lsp_periodogram", "lsp_periodogram_batched",
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
-    "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched",
+    "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched", "lsp_reserve",
     "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
@@ -41,13 +40,12 @@ class LspError(RuntimeError):
 
 
 def load(rebuild: bool = False):
-    """dlopen paper_1007_1658_b200/liblsp_b200.so (building it with nvcc if absent or stale)."""
+    """dlopen paper_1007_1658_b200/liblsp_b200.so, building it with nvcc first if it is absent or older than a source
+    (build() is a no-op when the library is fresh, so a stale binary is never loaded silently)."""
     global _lib
     if _lib is not None and not rebuild:
         return _lib
-    path = _build.LIB
-    if rebuild or not os.path.exists(path):
-        path = _build.build(force=rebuild)
+    path = _build.build(force=rebuild)
     lib = ctypes.CDLL(path)
     vp, i64, dbl, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
     lib.lsp_create.argtypes = [ctypes.POINTER(vp), ci]
@@ -63,6 +61,7 @@ def load(rebuild: bool = False):
     lib.lsp_periodogram_gls.argtypes = lib.lsp_periodogram.argtypes
     lib.lsp_periodogram_gls_batched.argtypes = lib.lsp_periodogram_batched.argtypes
     lib.lsp_false_alarm.argtypes = [vp, vp, i64, i64, dbl, vp, vp]
+    lib.lsp_reserve.argtypes = [vp, i64, ci, i64, i64, ci]
     lib.lsp_last_plan.argtypes = [vp, ctypes.POINTER(i64)]
     lib.lsp_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     lib.lsp_call_timing.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_float)]
@@ -104,17 +103,17 @@ def plan_query(sm_count: int, B: int, Nt: int, Nf: int) -> dict:
     st = load().lsp_plan_query(int(sm_count), int(B), int(Nt), int(Nf), out)
     if st != LSP_OK:
         raise LspError(st, "lsp_plan_query")
-    keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "ctas_per_sm", "score_e6")
+    keys = ("K", "threads", "nsplit", "pipe", "n_freq_blocks", "split_len", "ctas_per_sm", "score_e6")
     return dict(zip(keys, [int(v) for v in out]))
 
 
-def plan_query_form(sm_count: int, B: int, Nt: int, Nf: int, recurrence: int = 0) -> dict:
-    """lsp_plan_query_form: the launch plan of one form of steps 3-5 (0 = automatic) and its estimated cycles."""
+def plan_query_form(sm_count: int, B: int, Nt: int, Nf: int, pipe: int = 0) -> dict:
+    """lsp_plan_query_form: the launch plan of one form of steps 3-5 (PIPE_AUTO / PIPE_FP32 / PIPE_TENSOR) and its estimated cycles."""
     out = (ctypes.c_int64 * 8)()
-    st = load().lsp_plan_query_form(int(sm_count), int(B), int(Nt), int(Nf), int(recurrence), out)
+    st = load().lsp_plan_query_form(int(sm_count), int(B), int(Nt), int(Nf), int(pipe), out)
     if st != LSP_OK:
         raise LspError(st, "lsp_plan_query_form")
-    keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "ctas_per_sm", "est_cycles")
+    keys = ("K", "threads", "nsplit", "pipe", "n_freq_blocks", "split_len", "chunks_or_ctas_per_sm", "est_cycles")
     return dict(zip(keys, [int(v) for v in out]))
 
 
@@ -160,10 +159,14 @@ class Handle:
         self._check(self._lib.lsp_get_param(self._h, int(key), ctypes.byref(v)), "lsp_get_param")
         return v.value
 
+    def reserve(self, B: int, Nt: int, Nf: int, shared_t: bool = False, gls: bool = False):
+        """lsp_reserve: size the workspace now, so that the call itself allocates nothing (CUDA-graph capture)."""
+        self._check(self._lib.lsp_reserve(self._h, int(B), int(bool(shared_t)), int(Nt), int(Nf), int(bool(gls))), "lsp_reserve")
+
     def last_plan(self) -> dict:
         out = (ctypes.c_int64 * 8)()
         self._check(self._lib.lsp_last_plan(self._h, out), "lsp_last_plan")
-        keys = ("K", "threads", "nsplit", "recurrence", "n_freq_blocks", "split_len", "launches",
+        keys = ("K", "threads", "nsplit", "pipe", "n_freq_blocks", "split_len", "launches",
                 "lane_ops_per_term")
         d = dict(zip(keys, [int(v) for v in out]))
         d["kernel"] = self._lib.lsp_last_kernel_name(self._h).decode()

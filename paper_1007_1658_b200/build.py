@@ -15,8 +15,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "liblsp_b200.so")
 SOURCES = [os.path.join(CSRC, "lsp.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("lsp_common.cuh", "lsp_prepass.cuh", "lsp_accum.cuh", "lsp_accum_z.cuh", "lsp_accum_mma.cuh", "lsp_accum_umma.cuh", "lsp_accum_umma_tab.cuh", "lsp_accum_umma_pair.cuh", "lsp_accum_umma_pair2.cuh", "lsp_accum_umma_small.cuh", "lsp_shared_gemm.cuh", "lsp_accum_umma_duo.cuh",
-                                            "lsp_finish.cuh", "lsp_fap.cuh", "lsp_plan.h")]
+HEADERS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cuh", ".h"))]
 HEADERS.append(os.path.join(ROOT, "include", "lsp.h"))
 
 NVCC_FLAGS = [

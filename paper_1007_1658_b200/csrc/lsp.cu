@@ -1,19 +1,15 @@
 // lsp.cu -- host side of the C ABI declared in include/lsp.h: argument checks, launch plan,
-// workspace, and the four enqueues (moments -> records -> accumulate -> finish).
+// workspace, and the enqueues (moments -> records -> [table ->] accumulate -> finish).
 // No CPU arithmetic on the data path: every step of SURVEY.md section 8(a) runs in a kernel.
 #include "../../include/lsp.h"
 #include "lsp_common.cuh"
 #include "lsp_prepass.cuh"
-#include "lsp_accum.cuh"
 #include "lsp_accum_z.cuh"
-#include "lsp_accum_mma.cuh"
-#include "lsp_accum_umma.cuh"
-#include "lsp_accum_umma_tab.cuh"
-#include "lsp_accum_umma_pair.cuh"
+#include "lsp_tc.cuh"
 #include "lsp_accum_umma_pair2.cuh"
 #include "lsp_accum_umma_small.cuh"
-#include "lsp_shared_gemm.cuh"
 #include "lsp_accum_umma_duo.cuh"
+#include "lsp_shared_gemm.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_fap.cuh"
 #include "lsp_plan.h"
@@ -28,23 +24,25 @@ using namespace lsp;
 namespace {
 
 struct Plan {
-    int K = 0, T = 0, nsplit = 0, rec = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0, L = 0;
-    int mma_slots = 4;          // tensor-core forms: fp16-rate MMA slots issued per k-step of 8 samples (4 = hi+lo in fp16, 3 = 8-bit correction)
-    int64_t split_len = 0, part_chunk = 0;
+    int K = 0, T = 0, nsplit = 0, pipe = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0, L = 0, nchunks = 1;
+    int64_t split_len = 0, part_chunk = 0, chunk_len = 0;
     const char* kernel_name = "";
 };
 
 }  // namespace
 
 constexpr int TIMING_RING = 64;
+constexpr int TIMING_MAX_CHUNKS = 16;      // per-chunk accumulate events (more chunks: the accumulate bracket includes the later table pre-passes)
 
 struct lsp_ctx {
     int device = 0;
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_rec = 0, opt_flush = 0, opt_timing = 0, opt_btable = 0, opt_coarse = 0, opt_corr = 0, opt_pair = 0, opt_shared = 0, opt_duo = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
+    cudaEvent_t evc[TIMING_RING][2 * TIMING_MAX_CHUNKS] = {};   // accumulate launches of a chunked call, begin / end per chunk
+    int ev_chunks[TIMING_RING] = {};
     uint64_t timed_calls = 0;
     // workspace
     void* buf = nullptr;
@@ -74,57 +72,68 @@ struct DeviceGuard {
     ~DeviceGuard() { if (active) cudaSetDevice(prev); }
 };
 
+// Grow *ptr to `need` bytes.  The new buffer is allocated BEFORE the old one is released, so a failed allocation
+// (LSP_ENOMEM) leaves the handle with the workspace it had.  cudaFree waits for work that still uses the old buffer.
 int ensure(lsp_ctx* h, void** ptr, size_t* have, size_t need) {
     if (need <= *have) return LSP_OK;
-    if (*ptr) { cudaError_t e = cudaFree(*ptr); *ptr = nullptr; *have = 0; if (e != cudaSuccess) return cuda_fail(h, e); }
     need = align_up(need + need / 8, (size_t)1 << 20);
     void* p = nullptr;
     cudaError_t e = cudaMalloc(&p, need);
+    if (e != cudaSuccess && *ptr) {                      // not enough room for both: the old contents are scratch, so retry after freeing
+        cudaGetLastError();
+        void* old = *ptr; const size_t old_bytes = *have;
+        if (cudaFree(old) == cudaSuccess) {
+            *ptr = nullptr; *have = 0;
+            e = cudaMalloc(&p, need);
+            if (e != cudaSuccess) {                      // put back what the handle had
+                cudaGetLastError();
+                void* back = nullptr;
+                if (cudaMalloc(&back, old_bytes) == cudaSuccess) { *ptr = back; *have = old_bytes; } else cudaGetLastError();
+                h->last_cuda = (int)e;
+                return LSP_ENOMEM;
+            }
+            *ptr = p; *have = need;
+            return LSP_OK;
+        }
+    }
     if (e != cudaSuccess) { h->last_cuda = (int)e; cudaGetLastError(); return LSP_ENOMEM; }
+    if (*ptr) { cudaError_t f = cudaFree(*ptr); if (f != cudaSuccess) { cudaFree(p); return cuda_fail(h, f); } }
     *ptr = p; *have = need;
     return LSP_OK;
 }
 
-bool valid_K(int64_t K) { return K == 4 || K == 8 || K == 12 || K == 16 || K == 20 || K == 24 || K == 28 || K == 32; }
-
 typedef void (*accum_fn)(const AccumParams);
 
-struct KernelEntry { int K, rec; accum_fn fn; const char* name; int tile_z; int max_t; };   // tile_z = 0: pair-packed kernel
+struct KernelEntry { int K; accum_fn fn; const char* name; int max_t; };
 
-#define LSP_ENTRY(K, R, RN) { K, R, accum_kernel<K, R>, "accum_kernel<K=" #K "," RN ">", 0, 256 }
-#define LSP_ENTRY_Z(K, TZ, MAXT, MINB) { K, REC_THREE_TERM_Z, accum_z_kernel<K, TZ, MAXT, MINB>, "accum_z_kernel<K=" #K ",three_term_z>", TZ, MAXT }
+#define LSP_ENTRY_Z(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, "accum_z_kernel<K=" #K ",fp32,three-term>", MAXT }
 const KernelEntry g_kernels[] = {
-    LSP_ENTRY(4,  REC_ROTATION, "rotation"),   LSP_ENTRY(4,  REC_THREE_TERM, "three_term"),
-    LSP_ENTRY(8,  REC_ROTATION, "rotation"),   LSP_ENTRY(8,  REC_THREE_TERM, "three_term"),
-    LSP_ENTRY(12, REC_ROTATION, "rotation"),   LSP_ENTRY(12, REC_THREE_TERM, "three_term"),
-    LSP_ENTRY(16, REC_ROTATION, "rotation"),   LSP_ENTRY(16, REC_THREE_TERM, "three_term"),
-    LSP_ENTRY(20, REC_ROTATION, "rotation"),   LSP_ENTRY(20, REC_THREE_TERM, "three_term"),
-    LSP_ENTRY(24, REC_ROTATION, "rotation"),   LSP_ENTRY(24, REC_THREE_TERM, "three_term"),
-    LSP_ENTRY_Z(4, 256, 256, 1), LSP_ENTRY_Z(8, 256, 256, 1), LSP_ENTRY_Z(12, 256, 256, 1), LSP_ENTRY_Z(16, 256, 256, 1),
-    LSP_ENTRY_Z(20, 256, 256, 1), LSP_ENTRY_Z(24, 256, 256, 2), LSP_ENTRY_Z(28, 256, 128, 3), LSP_ENTRY_Z(32, 256, 128, 3),
+    LSP_ENTRY_Z(4, 256, 1), LSP_ENTRY_Z(8, 256, 1), LSP_ENTRY_Z(12, 256, 1), LSP_ENTRY_Z(16, 256, 1),
+    LSP_ENTRY_Z(20, 256, 1), LSP_ENTRY_Z(24, 256, 2), LSP_ENTRY_Z(28, 128, 3), LSP_ENTRY_Z(32, 128, 3),
 };
 
-const KernelEntry* find_kernel(int K, int rec) {
-    for (const KernelEntry& e : g_kernels) if (e.K == K && e.rec == rec) return &e;
+const KernelEntry* find_kernel(int K) {
+    for (const KernelEntry& e : g_kernels) if (e.K == K) return &e;
     return nullptr;
 }
 
 size_t accum_smem_bytes(const KernelEntry* ke, int T) {
-    if (ke->tile_z) return (size_t)ke->tile_z * 24 + (size_t)T * (4 * ke->K + 1) * sizeof(float);
-    return (size_t)3 * PAIRS * 16 + (size_t)4 * ke->K * T * sizeof(float);
+    return (size_t)TILE_Z * 24 + (size_t)T * (4 * ke->K + 1) * sizeof(float);
 }
 
-// Launch plan: which (K, T), how many time splits.  Units of work = B * nfb * nsplit CTAs; the
+// Launch plan: which form and tile, how many time splits (and chunks).  Units of work = B * nfb * nsplit CTAs; the
 // hardware block scheduler balances them over the SMs, so we want many more units than CTA slots.
-Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
+Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t table_series)
+{
     Plan pl;
     PlanOverrides ov;
-    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.rec = h->opt_rec; ov.L = h->opt_coarse;
+    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.pipe = h->opt_pipe; ov.L = h->opt_coarse;
+    ov.table_budget = h->opt_table_mb ? (h->opt_table_mb << 20) : 0; ov.table_series = table_series;
     const PlanChoice pc = plan_choose(h->sm_count, B, Nt, Nf, ov);
-    pl.rec = pc.rec; pl.K = pc.K; pl.T = pc.T; pl.nfb = pc.nfb; pl.L = pc.L;
-    pl.nsplit = pc.nsplit; pl.split_len = pc.split_len;
-    int64_t flush = h->opt_flush ? h->opt_flush : 2048;
-    pl.flush_tiles = (int)((flush + TILE - 1) / TILE);
+    pl.pipe = pc.pipe; pl.K = pc.K; pl.T = pc.T; pl.nfb = pc.nfb; pl.L = pc.L;
+    pl.nsplit = pc.nsplit; pl.split_len = pc.split_len; pl.nchunks = pc.nchunks; pl.chunk_len = pc.chunk_len;
+    const int64_t flush = h->opt_flush ? h->opt_flush : 2048;
+    pl.flush_tiles = (int)((flush + TILE_Z - 1) / TILE_Z);
     if (pl.flush_tiles < 1) pl.flush_tiles = 1;
     // pre-pass partition: contiguous chunks, at most MAX_PARTS blocks per series
     int64_t nparts = (Nt + 4095) / 4096;
@@ -137,61 +146,115 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf) {
     return pl;
 }
 
+// ---- workspace layouts (byte offsets into the handle's buffer)
+struct SharedLayout {
+    int64_t nsplit, gps, ng, nmb, nfb, x_row;
+    bool fuse;
+    size_t recB, xa, eb, wsv, wsx, vc, vcf, psum, pvar, peak, cnt, total;
+};
+
+// Shared-time batch: false if the sizes do not fit the kernel's grid.
+bool shared_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, SharedLayout& L)
+{
+    int64_t nsplit = (Nt + SG_MAX_SPLIT - 1) / SG_MAX_SPLIT;
+    int64_t gps = ((Nt + nsplit - 1) / nsplit + SG_KS - 1) / SG_KS;
+    gps = (gps + SG_KPS - 1) / SG_KPS * SG_KPS;           // k-step groups per split: whole stages
+    nsplit = (Nt + gps * SG_KS - 1) / (gps * SG_KS);
+    L.nsplit = nsplit; L.gps = gps; L.ng = nsplit * gps;
+    L.nmb = (B + SG_M - 1) / SG_M; L.nfb = (Nf + SG_F - 1) / SG_F;
+    L.x_row = (Nf + 3) / 4 * 4;
+    if (L.nmb * L.nfb * nsplit > 2147483647LL || L.ng > 65535 || nsplit > 65535) return false;
+    L.fuse = (nsplit == 1);                               // one split: the GEMM's accumulators are the sums; steps 6-7 run in its epilogue
+    size_t off = 0;
+    L.recB = off; off = align_up(off + (size_t)Nt * sizeof(ulonglong2), 256);   // phases of the one time vector
+    L.xa = off;   off = align_up(off + (size_t)L.nmb * L.ng * SG_A_GROUP, 256);
+    L.eb = off;   off = align_up(off + (size_t)L.nfb * L.ng * SG_B_GROUP, 256);
+    L.wsv = off;  off = align_up(off + (size_t)nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    L.wsx = off;  if (!L.fuse) off = align_up(off + (size_t)B * nsplit * 2 * (size_t)L.x_row * sizeof(float), 256);
+    L.vc = off;   off = align_up(off + (size_t)4 * (size_t)Nf * sizeof(double), 256);
+    L.vcf = off;  off = align_up(off + (size_t)Nf * sizeof(float4), 256);
+    L.psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    L.pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    L.peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
+    L.cnt = off;  off = align_up(off + (size_t)B * sizeof(unsigned), 256);
+    L.total = off;
+    return true;
+}
+
+struct Layout {
+    size_t recA, recB, ws, ws1, recA1, psum, pvar, peak, cnt, tab, total;
+    int64_t tab_groups;          // k-step groups of one series' table (one chunk + padding); 0: no table
+    size_t tab_bytes;
+};
+
+Layout device_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, int64_t tab_series, bool gls)
+{
+    Layout L;
+    const size_t n_samp = (size_t)B * (size_t)Nt;
+    size_t off = 0;
+    L.recA = off;  off = align_up(off + n_samp * sizeof(float4), 256);
+    L.recB = off;  off = align_up(off + n_samp * sizeof(ulonglong2), 256);
+    L.ws = off;    off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    L.ws1 = off;   if (gls) off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
+    L.recA1 = off; if (gls) off = align_up(off + n_samp * sizeof(float4), 256);
+    L.psum = off;  off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    L.pvar = off;  off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    L.peak = off;  off = align_up(off + (size_t)B * sizeof(u64), 256);
+    L.cnt = off;   off = align_up(off + (size_t)B * sizeof(unsigned), 256);
+    L.tab_groups = 0; L.tab_bytes = 0; L.tab = off;
+    if (pl.pipe == PLAN_PIPE_TENSOR && pl.L >= 128) {     // CTA-pair form: the fine-operand table of ONE time chunk (lsp_accum_umma_pair2.cuh)
+        L.tab_groups = (pl.chunk_len + UM_KS - 1) / UM_KS + U2_TABLE_PAD_KSTEPS;
+        L.tab_bytes = (size_t)tab_series * (size_t)L.tab_groups * U2_TABLE_BYTES_PER_KSTEP;
+        off = align_up(off + L.tab_bytes, 256);
+    }
+    L.total = off;
+    return L;
+}
+
+bool use_shared_path(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, bool gls)
+{
+    return t_stride == 0 && B > 1 && !gls && h->opt_shared != 1 && h->opt_pipe == 0 &&
+           (h->opt_shared == 2 || (B >= 16 && Nt >= 512));
+}
+
 // Shared-time batch (t_stride = 0): XC, XS as one dense GEMM over all series, CC, CS once per frequency (lsp_shared_gemm.cuh).
 int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_stride,
                       int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                       float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st)
 {
-    Plan pl = make_plan(h, B, Nt, Nf);                    // pre-pass partition only
-    int64_t nsplit = (Nt + SG_MAX_SPLIT - 1) / SG_MAX_SPLIT;
-    int64_t gps = ((Nt + nsplit - 1) / nsplit + SG_KS - 1) / SG_KS;
-    gps = (gps + SG_KPS - 1) / SG_KPS * SG_KPS;           // k-step groups per split: whole stages
-    nsplit = (Nt + gps * SG_KS - 1) / (gps * SG_KS);
-    const int64_t ng = nsplit * gps;
-    const int64_t nmb = (B + SG_M - 1) / SG_M, nfb = (Nf + SG_F - 1) / SG_F;
-    const int64_t x_row = (Nf + 3) / 4 * 4;
-    if (nmb * nfb * nsplit > 2147483647LL || ng > 65535 || nsplit > 65535 || B > 65535) return LSP_EINVAL;
-    pl.rec = REC_UMMA; pl.K = SG_F; pl.T = SG_THREADS; pl.nsplit = (int)nsplit; pl.nfb = (int)nfb; pl.L = 0;
-    pl.split_len = gps * SG_KS; pl.launches = 7;
-    pl.kernel_name = (nsplit == 1) ? "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times,fused-finish>"
-                                   : "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times>";
+    Plan pl = make_plan(h, B, Nt, Nf, 1);                 // pre-pass partition only
+    SharedLayout L;
+    if (!shared_layout(pl, B, Nt, Nf, L)) return LSP_EINVAL;
+    const int64_t nsplit = L.nsplit, gps = L.gps, ng = L.ng, nmb = L.nmb, nfb = L.nfb, x_row = L.x_row;
+    const bool fuse = L.fuse;
+    pl.pipe = PLAN_PIPE_TENSOR; pl.K = SG_F; pl.T = SG_THREADS; pl.nsplit = (int)nsplit; pl.nfb = (int)nfb; pl.L = 0;
+    pl.split_len = gps * SG_KS; pl.launches = 7; pl.nchunks = 1; pl.chunk_len = 0;
+    pl.kernel_name = fuse ? "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times,fused-finish>"
+                          : "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times>";
 
-    const size_t n_samp = (size_t)B * (size_t)Nt;
-    size_t off = 0;
-    const size_t o_recA = off;                            // (no per-sample records per series on this path)
-    const size_t o_recB = off; off = align_up(off + (size_t)Nt * sizeof(ulonglong2), 256);   // phases of the one time vector
-    const size_t o_xa = off;   off = align_up(off + (size_t)nmb * ng * SG_A_GROUP, 256);
-    const size_t o_eb = off;   off = align_up(off + (size_t)nfb * ng * SG_B_GROUP, 256);
-    const size_t o_wsv = off;  off = align_up(off + (size_t)nsplit * 4 * (size_t)Nf * sizeof(float), 256);
-    const bool fuse = (nsplit == 1);                      // one split: the GEMM's accumulators are the sums; steps 6-7 run in its epilogue
-    const size_t o_wsx = off;  if (!fuse) off = align_up(off + (size_t)B * nsplit * 2 * (size_t)x_row * sizeof(float), 256);
-    const size_t o_vc = off;   off = align_up(off + (size_t)4 * (size_t)Nf * sizeof(double), 256);
-    const size_t o_vcf = off;  off = align_up(off + (size_t)Nf * sizeof(float4), 256);
-    const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
-    const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
-    const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
-    const size_t o_cnt = off;  off = align_up(off + (size_t)B * sizeof(unsigned), 256);
-    int rc = ensure(h, &h->buf, &h->buf_bytes, off);
+    int rc = ensure(h, &h->buf, &h->buf_bytes, L.total);
     if (rc != LSP_OK) return rc;
     char* base = static_cast<char*>(h->buf);
-    float4* recA = reinterpret_cast<float4*>(base + o_recA);
-    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
-    unsigned char* xa = reinterpret_cast<unsigned char*>(base + o_xa);
-    unsigned char* eb = reinterpret_cast<unsigned char*>(base + o_eb);
-    float* ws_v = reinterpret_cast<float*>(base + o_wsv);
-    float* ws_x = reinterpret_cast<float*>(base + o_wsx);
-    double* vconst = reinterpret_cast<double*>(base + o_vc);
-    float4* vconst_f = reinterpret_cast<float4*>(base + o_vcf);
-    double* psum = reinterpret_cast<double*>(base + o_psum);
-    double* pvar = reinterpret_cast<double*>(base + o_pvar);
-    u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
-    unsigned* counter = reinterpret_cast<unsigned*>(base + o_cnt);
+    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + L.recB);
+    float4* recA = reinterpret_cast<float4*>(base + L.recB);          // (no per-sample measurement records on this path: never written)
+    unsigned char* xa = reinterpret_cast<unsigned char*>(base + L.xa);
+    unsigned char* eb = reinterpret_cast<unsigned char*>(base + L.eb);
+    float* ws_v = reinterpret_cast<float*>(base + L.wsv);
+    float* ws_x = reinterpret_cast<float*>(base + L.wsx);
+    double* vconst = reinterpret_cast<double*>(base + L.vc);
+    float4* vconst_f = reinterpret_cast<float4*>(base + L.vcf);
+    double* psum = reinterpret_cast<double*>(base + L.psum);
+    double* pvar = reinterpret_cast<double*>(base + L.pvar);
+    u64* peak64 = reinterpret_cast<u64*>(base + L.peak);
+    unsigned* counter = reinterpret_cast<unsigned*>(base + L.cnt);
 
     const bool timing = h->opt_timing != 0;
-    cudaEvent_t* ev = h->ev[h->timed_calls % TIMING_RING];
+    const int slot = (int)(h->timed_calls % TIMING_RING);
+    cudaEvent_t* ev = h->ev[slot];
     if (timing) {
         for (int i = 0; i < 5; ++i)
             if (!ev[i]) LSP_CUDA(h, cudaEventCreate(&ev[i]));
+        h->ev_chunks[slot] = 0;
         LSP_CUDA(h, cudaEventRecord(ev[0], st));
     }
     // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
@@ -237,7 +300,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     fp.ws = ws_v; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = (int)nsplit; fp.nparts = pl.nparts;
-    fp.cc_fix = 0.0; fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
+    fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
     const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
     dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
     finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
@@ -247,85 +310,85 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     return LSP_OK;
 }
 
+// What the call will run (shared by run_device and lsp_reserve).
+struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair; int64_t tab_series; };
+
+int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf, bool gls, Route& r)
+{
+    r.tab_series = (t_stride == 0) ? 1 : B;
+    r.pl = make_plan(h, B, Nt, Nf, r.tab_series);
+    Plan& pl = r.pl;
+    if (pl.K == 0) return LSP_EINVAL;
+    r.tensor = pl.pipe == PLAN_PIPE_TENSOR;
+    r.pair = r.tensor && pl.L >= 128;                     // CTA pairs, table-fed (lsp_accum_umma_pair2.cuh)
+    r.small = r.tensor && !r.pair;                        // 128 x L frequencies per CTA, two or three CTAs per SM
+    r.duo = r.small && pl.L == 16 && B >= 2;              // batches: two series per CTA (lsp_accum_umma_duo.cuh)
+    // one CTA sees all samples of its series in one drain window: steps 6-7 run in its epilogue, no workspace round trip
+    r.duo_fuse = r.duo && !gls && pl.nsplit == 1 && Nt <= (h->opt_flush ? h->opt_flush : 2048);
+    if (!r.tensor) {
+        const KernelEntry* ke = find_kernel(pl.K);
+        if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
+        pl.kernel_name = ke->name;
+    } else if (r.pair) {
+        pl.kernel_name = "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>";
+        pl.launches = 3 + 2 * pl.nchunks;
+    } else if (r.duo) {
+        pl.kernel_name = r.duo_fuse ? "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32,fused-finish>"
+                                    : "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>";
+        if (r.duo_fuse) pl.launches = 3;
+    } else {
+        pl.kernel_name = pl.L == 16 ? "accum_umma_small_kernel<tcgen05.m128n32k16.f16,hi+lo>"
+                       : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
+                                     : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
+    }
+    if (gls) pl.launches += 1 + (r.pair ? pl.nchunks : 1);   // unit records + second accumulate pass
+    const int64_t units = (r.duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
+    if (units > 2147483647LL) return LSP_EINVAL;
+    return LSP_OK;
+}
+
 int run_device(lsp_ctx* h,
                const double* t, int64_t t_stride, const float* x, int64_t x_stride,
                int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st, bool gls = false)
 {
-    if (t_stride == 0 && B > 1 && !gls && h->opt_shared != 1 && h->opt_rec == 0 && B <= 65535 &&
-        (h->opt_shared == 2 || (B >= 16 && Nt >= 512)))
+    if (use_shared_path(h, t_stride, B, Nt, gls))
         return run_device_shared(h, t, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride, peak_idx, peak_val, st);
-    Plan pl = make_plan(h, B, Nt, Nf);
-    const bool umma = pl.rec == REC_UMMA;
-    const bool mma = pl.rec == REC_MMA || umma;                      // tensor-core forms: X scaled to unit variance
-    const KernelEntry* ke = mma ? nullptr : find_kernel(pl.K, pl.rec);
-    if (!mma && (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0)) return LSP_EINVAL;
-    const bool umma_small = umma && pl.L < UM_L;          // 128 x L frequencies per CTA, two CTAs per SM
-    pl.kernel_name = umma ? "accum_umma_kernel<tcgen05.m128n256k16.f16,hi+lo>"
-                          : (mma ? "accum_mma_kernel<m16n8k16.f16,hi+lo>" : ke->name);
-    const bool duo = umma_small && pl.L == 16 && B >= 2 && h->opt_duo != 1;   // batches: two series per CTA (lsp_accum_umma_duo.cuh)
-    if (umma_small) pl.kernel_name = pl.L == 16 ? "accum_umma_small_kernel<tcgen05.m128n32k16.f16,hi+lo>"
-                                   : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
-                                                 : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
-
-    // one CTA sees all samples of its series in one drain window: steps 6-7 run in its epilogue, no workspace round trip
-    const bool duo_fuse = duo && !gls && pl.nsplit == 1 && Nt <= (h->opt_flush ? h->opt_flush : 2048);
-    if (duo) pl.kernel_name = duo_fuse ? "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32,fused-finish>"
-                                       : "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>";
-    if (duo_fuse) pl.launches = 3;
-
-    // workspace carve-up
-    const size_t n_samp = (size_t)B * (size_t)Nt;
-    size_t off = 0;
-    const size_t o_recA = off; off = align_up(off + n_samp * sizeof(float4), 256);
-    const size_t o_recB = off; off = align_up(off + n_samp * sizeof(ulonglong2), 256);
-    const size_t o_ws = off;   off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
-    const size_t o_ws1 = off;  if (gls) off = align_up(off + (size_t)B * pl.nsplit * 4 * (size_t)Nf * sizeof(float), 256);
-    const size_t o_recA1 = off; if (gls) off = align_up(off + n_samp * sizeof(float4), 256);
-    const size_t o_psum = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
-    const size_t o_pvar = off; off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
-    const size_t o_peak = off; off = align_up(off + (size_t)B * sizeof(u64), 256);
-    const size_t o_cnt = off;  off = align_up(off + (size_t)B * sizeof(unsigned), 256);
-    // tcgen05 form: the coarse operand B comes from a table when several frequency blocks share it (lsp_accum_umma_tab.cuh)
-    const int64_t tab_series = (t_stride == 0) ? 1 : B;
-    const int64_t tab_groups = (Nt + UM_KS - 1) / UM_KS + UT_KPS;
-    const size_t tab_bytes = (size_t)tab_series * (size_t)tab_groups * UT_GROUP_BYTES;
-    const bool use_tab = umma && !umma_small && h->opt_btable != 1 &&
-                         (h->opt_btable == 2 || (pl.nfb >= 3 && tab_bytes <= ((size_t)12 << 30)));
-    const size_t o_tab = off;  if (use_tab) off = align_up(off + tab_bytes, 256);
-    const bool corr8 = use_tab && h->opt_corr != 1;       // correction products as one 8-bit MMA (default) or two fp16 MMAs
-    const bool pair = corr8 && h->opt_pair != 1;          // CTA pairs (cta_group::2) share one B tile: lsp_accum_umma_pair.cuh
-    const bool pair2 = pair && h->opt_pair != 2;          // ... and share the GENERATED operand instead: lsp_accum_umma_pair2.cuh (default)
-    if (pair) pl.nfb = (pl.nfb + 1) & ~1;                 // a pair = two adjacent frequency blocks; an odd count gets one masked block
-    if (use_tab) {
-        pl.kernel_name = corr8 ? "accum_umma_tab_kernel<tcgen05.m128n256.f16+e5m2corr,B-table>"
-                               : "accum_umma_tab_kernel<tcgen05.m128n256k16.f16,hi+lo,B-table>";
-        if (pair) pl.kernel_name = pair2 ? "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>"
-                                         : "accum_umma_pair_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,B-table>";
-        pl.launches = 5;
-        pl.mma_slots = corr8 ? 3 : 4;
-    }
-    if (gls) pl.launches += 2;                            // unit records + second accumulate pass
-    int rc = ensure(h, &h->buf, &h->buf_bytes, off);
+    Route r;
+    int rc = route(h, t_stride, B, Nt, Nf, gls, r);
     if (rc != LSP_OK) return rc;
-    char* base = static_cast<char*>(h->buf);
-    float4* recA = reinterpret_cast<float4*>(base + o_recA);
-    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
-    float* ws = reinterpret_cast<float*>(base + o_ws);
-    float* ws1 = gls ? reinterpret_cast<float*>(base + o_ws1) : nullptr;          // unit-weight pass: sum cos, sum sin
-    float4* recA1 = gls ? reinterpret_cast<float4*>(base + o_recA1) : nullptr;
-    double* psum = reinterpret_cast<double*>(base + o_psum);
-    double* pvar = reinterpret_cast<double*>(base + o_pvar);
-    u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
-    unsigned* counter = reinterpret_cast<unsigned*>(base + o_cnt);
+    Plan& pl = r.pl;
+    const bool tensor = r.tensor;                          // tensor-core forms: X scaled to unit variance
+    const KernelEntry* ke = tensor ? nullptr : find_kernel(pl.K);
 
-    if (B > 65535) return LSP_EINVAL;                     // grid.y limit of the pre-pass / finish kernels
+    const Layout L = device_layout(pl, B, Nt, Nf, r.tab_series, gls);
+    rc = ensure(h, &h->buf, &h->buf_bytes, L.total);
+    if (rc != LSP_OK) return rc;
+    const size_t n_samp = (size_t)B * (size_t)Nt;
+    char* base = static_cast<char*>(h->buf);
+    float4* recA = reinterpret_cast<float4*>(base + L.recA);
+    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + L.recB);
+    float* ws = reinterpret_cast<float*>(base + L.ws);
+    float* ws1 = gls ? reinterpret_cast<float*>(base + L.ws1) : nullptr;          // unit-weight pass: sum cos, sum sin
+    float4* recA1 = gls ? reinterpret_cast<float4*>(base + L.recA1) : nullptr;
+    double* psum = reinterpret_cast<double*>(base + L.psum);
+    double* pvar = reinterpret_cast<double*>(base + L.pvar);
+    u64* peak64 = reinterpret_cast<u64*>(base + L.peak);
+    unsigned* counter = reinterpret_cast<unsigned*>(base + L.cnt);
+    unsigned char* table = reinterpret_cast<unsigned char*>(base + L.tab);
 
     const bool timing = h->opt_timing != 0;
-    cudaEvent_t* ev = h->ev[h->timed_calls % TIMING_RING];
+    const int slot = (int)(h->timed_calls % TIMING_RING);
+    cudaEvent_t* ev = h->ev[slot];
+    cudaEvent_t* evc = h->evc[slot];
+    const bool chunk_timing = timing && r.pair && pl.nchunks > 1 && pl.nchunks <= TIMING_MAX_CHUNKS;
     if (timing) {
         for (int i = 0; i < 5; ++i)
             if (!ev[i]) LSP_CUDA(h, cudaEventCreate(&ev[i]));
+        if (chunk_timing)
+            for (int i = 0; i < 2 * pl.nchunks; ++i)
+                if (!evc[i]) LSP_CUDA(h, cudaEventCreate(&evc[i]));
+        h->ev_chunks[slot] = chunk_timing ? pl.nchunks : 0;
         LSP_CUDA(h, cudaEventRecord(ev[0], st));
     }
 
@@ -344,101 +407,90 @@ int run_device(lsp_ctx* h,
         unit_records_kernel<<<(unsigned)((n_samp + 255) / 256), 256, 0, st>>>(recA, recA1, (int64_t)n_samp);
         LSP_CUDA(h, cudaGetLastError());
     }
-    unsigned char* btable = reinterpret_cast<unsigned char*>(base + o_tab);
-    if (use_tab) {
-        if (tab_groups > 2147483647LL) return LSP_EINVAL;
-        dim3 gtab((unsigned)tab_groups, (unsigned)tab_series);
-        if (pair2) umma_ftable_pair_kernel<<<gtab, 512, 0, st>>>(recB, Nt, Nt, btable, (int64_t)tab_groups * UP_GROUP_BYTES, (int64_t)tab_groups * UT_GROUP_BYTES);
-        else if (pair) umma_btable_pair_kernel<<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, (int64_t)tab_groups * UP_GROUP_BYTES, (int64_t)tab_groups * UT_GROUP_BYTES);
-        else if (corr8) umma_btable_kernel<true><<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
-        else umma_btable_kernel<false><<<gtab, 256, 0, st>>>(recB, Nt, Nt, btable, tab_groups, (int64_t)tab_groups * UT_GROUP_BYTES);
-        LSP_CUDA(h, cudaGetLastError());
-    }
 
-    if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
-
-    // steps 3-5
-    const int64_t units = (duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
-    if (units > 2147483647LL) return LSP_EINVAL;
-    // (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
-    for (int pass = 0; pass < (gls ? 2 : 1); ++pass) {
-    const float4* rA = pass ? recA1 : recA;
-    float* wsp = pass ? ws1 : ws;
-    if (umma) {
-        UmmaParams up;
-        up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
-        up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
-        // drain interval of D_W: 2,048 samples; 4,096 for the pair2 form, whose drain adds the expected truncation loss back
-        // (measured max error of max P at 2,048 / 4,096 / 8,192 samples: C3 5e-6 / 9e-6 / 2.2e-5, C5 4e-6 / 6e-6 / 1.1e-5, P0 9e-6 / 1.9e-5 / 3.8e-5)
-        up.flush_ksteps = (int)((h->opt_flush ? h->opt_flush : (pair2 ? 4096 : 2048)) + UM_KS - 1) / UM_KS;
-        up.trunc_ulps = pair2 ? 0.45f : 0.f;
-        up.unit_x = pass;
-        if (duo) {
-            UmmaDuoParams dp;
-            dp.u = up; dp.B = B;
-            dp.fuse = duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
-            dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
-            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
-            accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
-        } else if (umma_small) {
-#define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
-            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
-            accum_umma_small_kernel<LL, NS, MINB><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); } while (0)
-            if (pl.L == 16) LSP_LAUNCH_SMALL(16, 4, 3);
-            else if (pl.L == 32) LSP_LAUNCH_SMALL(32, 4, 2);
-            else if (pl.L == 64) LSP_LAUNCH_SMALL(64, 4, 2);
-            else return LSP_EINVAL;
-#undef LSP_LAUNCH_SMALL
-        } else if (use_tab) {
-            UmmaTabParams tp;
-            tp.u = up; tp.btable = btable; tp.ngroups = tab_groups;
-            tp.table_stride = (tab_series == 1) ? 0 : (int64_t)tab_groups * UT_GROUP_BYTES;
-            if (pair) {
+    // steps 3-5 (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
+    const int npass = gls ? 2 : 1;
+    const int flush_ksteps = (int)(((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS);
+    if (r.pair) {
+        // CTA-pair form, one time chunk at a time: table pre-pass, then the accumulate launch(es) that read it
+        const int64_t half_stride = L.tab_groups * (int64_t)UP_GROUP_BYTES;
+        const int64_t series_stride = L.tab_groups * (int64_t)U2_TABLE_BYTES_PER_KSTEP;
+        LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)U2_SMEM));
+        for (int c = 0; c < pl.nchunks; ++c) {
+            const int64_t j0 = (int64_t)c * pl.chunk_len;
+            const int64_t len = (Nt - j0 < pl.chunk_len) ? Nt - j0 : pl.chunk_len;
+            const int64_t groups = (len + UM_KS - 1) / UM_KS + U2_TABLE_PAD_KSTEPS;
+            umma_ftable_pair_kernel<<<dim3((unsigned)groups, (unsigned)r.tab_series), 512, 0, st>>>(recB, j0, j0 + len, Nt, table, half_stride, series_stride);
+            LSP_CUDA(h, cudaGetLastError());
+            if (timing && c == 0) LSP_CUDA(h, cudaEventRecord(ev[2], st));
+            if (chunk_timing) LSP_CUDA(h, cudaEventRecord(evc[2 * c], st));
+            const int nsplit_c = (int)((len + pl.split_len - 1) / pl.split_len);
+            for (int pass = 0; pass < npass; ++pass) {
                 UmmaPairParams pp;
-                pp.u = up; pp.btable = btable; pp.half_stride = (int64_t)tab_groups * UP_GROUP_BYTES;
-                pp.table_stride = tp.table_stride;
-                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UP_SMEM));
-                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)U2_SMEM));
+                UmmaParams& up = pp.u;
+                up.recA = pass ? recA1 : recA; up.recB = recB; up.part_var = pvar; up.ws = pass ? ws1 : ws; up.Nt = Nt; up.Nf = Nf;
+                up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
+                up.flush_ksteps = flush_ksteps;
+                up.trunc_ulps = h->opt_trunc == 0 ? -1.f : (h->opt_trunc == 1 ? 0.f : 1e-3f * (float)h->opt_trunc);
+                up.unit_x = pass;
+                pp.btable = table; pp.half_stride = half_stride; pp.table_stride = (r.tab_series == 1) ? 0 : series_stride;
+                pp.j0 = j0; pp.chunk_len = len; pp.accumulate = c > 0 ? 1 : 0;
+                pp.nsplit_grid = nsplit_c;                  // only the splits this chunk has; pl.nsplit still strides `ws`
+                const int64_t units = B * (int64_t)nsplit_c * pl.nfb;
                 cudaLaunchConfig_t cfg = {};
-                cfg.gridDim = dim3((unsigned)units); cfg.blockDim = dim3(pair2 ? U2_THREADS : UM_THREADS); cfg.dynamicSmemBytes = pair2 ? U2_SMEM : UP_SMEM; cfg.stream = st;
+                cfg.gridDim = dim3((unsigned)units); cfg.blockDim = dim3(U2_THREADS); cfg.dynamicSmemBytes = U2_SMEM; cfg.stream = st;
                 cudaLaunchAttribute at[1];
                 at[0].id = cudaLaunchAttributeClusterDimension;
                 at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                 cfg.attrs = at; cfg.numAttrs = 1;
-                if (pair2) LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair2_kernel, pp));
-                else LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair_kernel, pp));
-            } else if (corr8) {
-                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
-                accum_umma_tab_kernel<true><<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
-            } else {
-                LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_tab_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UT_SMEM));
-                accum_umma_tab_kernel<false><<<(unsigned)units, UM_THREADS, UT_SMEM, st>>>(tp);
+                LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair2_kernel, pp));
             }
-        } else {
-            LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UM_SMEM));
-            accum_umma_kernel<<<(unsigned)units, UM_THREADS, UM_SMEM, st>>>(up);
+            if (chunk_timing) LSP_CUDA(h, cudaEventRecord(evc[2 * c + 1], st));
         }
-    } else if (mma) {
-        MmaParams mp;
-        mp.recA = rA; mp.recB = recB; mp.part_var = pvar; mp.ws = wsp; mp.Nt = Nt; mp.Nf = Nf;
-        mp.split_len = pl.split_len; mp.nsplit = pl.nsplit; mp.nfb = pl.nfb; mp.nparts = pl.nparts; mp.unit_x = pass;
-        LSP_CUDA(h, cudaFuncSetAttribute(accum_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMA_SMEM));
-        accum_mma_kernel<<<(unsigned)units, MMA_WARPS * 32, MMA_SMEM, st>>>(mp);
     } else {
-        AccumParams ap;
-        ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.Nt = Nt; ap.Nf = Nf;
-        ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
-        const size_t smem = accum_smem_bytes(ke, pl.T);
-        LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
-    }
-    LSP_CUDA(h, cudaGetLastError());
+        if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
+        const int64_t units = (r.duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
+        for (int pass = 0; pass < npass; ++pass) {
+            const float4* rA = pass ? recA1 : recA;
+            float* wsp = pass ? ws1 : ws;
+            if (tensor) {
+                UmmaParams up;
+                up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
+                up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
+                up.flush_ksteps = flush_ksteps; up.trunc_ulps = 0.f; up.unit_x = pass;
+                if (r.duo) {
+                    UmmaDuoParams dp;
+                    dp.u = up; dp.B = B;
+                    dp.fuse = r.duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
+                    dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
+                    LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
+                    accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
+                } else {
+#define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
+                    LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
+                    accum_umma_small_kernel<LL, NS, MINB><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); } while (0)
+                    if (pl.L == 16) LSP_LAUNCH_SMALL(16, 4, 3);
+                    else if (pl.L == 32) LSP_LAUNCH_SMALL(32, 4, 2);
+                    else if (pl.L == 64) LSP_LAUNCH_SMALL(64, 4, 2);
+                    else return LSP_EINVAL;
+#undef LSP_LAUNCH_SMALL
+                }
+            } else {
+                AccumParams ap;
+                ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.Nt = Nt; ap.Nf = Nf;
+                ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
+                const size_t smem = accum_smem_bytes(ke, pl.T);
+                LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
+            }
+            LSP_CUDA(h, cudaGetLastError());
+        }
     }
     LSP_CUDA(h, cudaGetLastError());
 
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
 
-    if (duo_fuse) {
+    if (r.duo_fuse) {
         if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
         h->plan = pl;
         return LSP_OK;
@@ -448,8 +500,7 @@ int run_device(lsp_ctx* h,
     fp.ws = ws; fp.part_var = pvar; fp.P = P; fp.p_stride = p_stride;
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = pl.nsplit; fp.nparts = pl.nparts;
-    fp.cc_fix = (!mma && ke->tile_z == 0 && (Nt & 1)) ? 0.5 : 0.0;   // phantom partner of an odd last sample (pair-packed only)
-    fp.x_scaled = mma ? 1 : 0;
+    fp.x_scaled = tensor ? 1 : 0;
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
     const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
@@ -464,6 +515,28 @@ int run_device(lsp_ctx* h,
 
 bool bad_grid(double f_min, double df) {
     return !(std::isfinite(f_min) && std::isfinite(df)) || f_min < 0.0 || df < 0.0;
+}
+
+// Argument checks shared by the batched entry points (device and host forms).
+int check_batch_args(lsp_ctx* h, const void* t, const void* x, int64_t B, int64_t Nt, int64_t min_nt,
+                     double f_min, double df, int64_t Nf, const void* P, const void* peak_idx, const void* peak_val)
+{
+    if (!h || !t || !x) return LSP_EINVAL;
+    if (B < 1 || B > 65535 || Nt < min_nt || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;   // B: grid.y of the pre-pass / finish kernels
+    if (bad_grid(f_min, df)) return LSP_EINVAL;
+    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
+    if (!P && !peak_idx) return LSP_EINVAL;
+    return LSP_OK;
+}
+
+int check_strides(int64_t t_stride, int64_t x_stride, int64_t p_stride, int64_t B, int64_t Nt, int64_t Nf, const void* P)
+{
+    if (B > 1) {
+        if (t_stride != 0 && std::llabs(t_stride) < Nt) return LSP_EINVAL;
+        if (std::llabs(x_stride) < Nt) return LSP_EINVAL;
+        if (P && std::llabs(p_stride) < Nf) return LSP_EINVAL;
+    }
+    return LSP_OK;
 }
 
 }  // namespace
@@ -500,8 +573,10 @@ int lsp_destroy(lsp_handle h)
     cudaDeviceSynchronize();
     if (h->buf) cudaFree(h->buf);
     if (h->stage) cudaFree(h->stage);
-    for (int r = 0; r < TIMING_RING; ++r)
+    for (int r = 0; r < TIMING_RING; ++r) {
         for (int i = 0; i < 5; ++i) if (h->ev[r][i]) cudaEventDestroy(h->ev[r][i]);
+        for (int i = 0; i < 2 * TIMING_MAX_CHUNKS; ++i) if (h->evc[r][i]) cudaEventDestroy(h->evc[r][i]);
+    }
     delete h;
     return LSP_OK;
 }
@@ -510,18 +585,16 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
 {
     if (!h || value < 0) return LSP_EINVAL;
     switch (key) {
-        case LSP_PARAM_K:          if (value && !valid_K(value)) return LSP_EINVAL; h->opt_K = value; break;
+        case LSP_PARAM_K:          if (value && !plan_valid_K((int)value)) return LSP_EINVAL; h->opt_K = value; break;
         case LSP_PARAM_THREADS:    if (value && (value < 32 || value > 256 || value % 32)) return LSP_EINVAL; h->opt_T = value; break;
         case LSP_PARAM_NSPLIT:     h->opt_nsplit = value; break;
-        case LSP_PARAM_RECURRENCE: if (value > 5) return LSP_EINVAL; h->opt_rec = value; break;
+        case LSP_PARAM_PIPE:       if (value > LSP_PIPE_TENSOR) return LSP_EINVAL; h->opt_pipe = value; break;
         case LSP_PARAM_FLUSH:      h->opt_flush = value; break;
         case LSP_PARAM_TIMING:     if (value > 1) return LSP_EINVAL; h->opt_timing = value; break;
-        case LSP_PARAM_BTABLE:     if (value > 2) return LSP_EINVAL; h->opt_btable = value; break;
+        case LSP_PARAM_TABLE_MB:   if (value > (1 << 20)) return LSP_EINVAL; h->opt_table_mb = value; break;
         case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
-        case LSP_PARAM_CORR:       if (value > 2) return LSP_EINVAL; h->opt_corr = value; break;
-        case LSP_PARAM_PAIR:       if (value > 3) return LSP_EINVAL; h->opt_pair = value; break;
+        case LSP_PARAM_TRUNC:      if (value > 4000) return LSP_EINVAL; h->opt_trunc = value; break;
         case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
-        case LSP_PARAM_DUO:        if (value > 2) return LSP_EINVAL; h->opt_duo = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -534,18 +607,37 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_K:          *value = h->opt_K; break;
         case LSP_PARAM_THREADS:    *value = h->opt_T; break;
         case LSP_PARAM_NSPLIT:     *value = h->opt_nsplit; break;
-        case LSP_PARAM_RECURRENCE: *value = h->opt_rec; break;
+        case LSP_PARAM_PIPE:       *value = h->opt_pipe; break;
         case LSP_PARAM_FLUSH:      *value = h->opt_flush; break;
         case LSP_PARAM_TIMING:     *value = h->opt_timing; break;
-        case LSP_PARAM_BTABLE:     *value = h->opt_btable; break;
+        case LSP_PARAM_TABLE_MB:   *value = h->opt_table_mb; break;
         case LSP_PARAM_COARSE:     *value = h->opt_coarse; break;
-        case LSP_PARAM_CORR:       *value = h->opt_corr; break;
-        case LSP_PARAM_PAIR:       *value = h->opt_pair; break;
+        case LSP_PARAM_TRUNC:      *value = h->opt_trunc; break;
         case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
-        case LSP_PARAM_DUO:        *value = h->opt_duo; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
+}
+
+int lsp_reserve(lsp_handle h, int64_t B, int shared_t, int64_t Nt, int64_t Nf, int generalised)
+{
+    if (!h || B < 1 || B > 65535 || Nt < 2 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
+    DeviceGuard g(h->device);
+    const int64_t t_stride = shared_t ? 0 : Nt;
+    const bool gls = generalised != 0;
+    size_t need;
+    if (use_shared_path(h, t_stride, B, Nt, gls)) {
+        const Plan pl = make_plan(h, B, Nt, Nf, 1);
+        SharedLayout L;
+        if (!shared_layout(pl, B, Nt, Nf, L)) return LSP_EINVAL;
+        need = L.total;
+    } else {
+        Route r;
+        const int rc = route(h, t_stride, B, Nt, Nf, gls, r);
+        if (rc != LSP_OK) return rc;
+        need = device_layout(r.pl, B, Nt, Nf, r.tab_series, gls).total;
+    }
+    return ensure(h, &h->buf, &h->buf_bytes, need);
 }
 
 int lsp_call_timing(lsp_handle h, int calls_back, float ms[4])
@@ -553,9 +645,20 @@ int lsp_call_timing(lsp_handle h, int calls_back, float ms[4])
     if (!h || !ms || calls_back < 0) return LSP_EINVAL;
     if ((uint64_t)calls_back >= h->timed_calls || calls_back >= TIMING_RING) return LSP_EINVAL;
     DeviceGuard g(h->device);
-    cudaEvent_t* ev = h->ev[(h->timed_calls - 1 - (uint64_t)calls_back) % TIMING_RING];
+    const int slot = (int)((h->timed_calls - 1 - (uint64_t)calls_back) % TIMING_RING);
+    cudaEvent_t* ev = h->ev[slot];
     LSP_CUDA(h, cudaEventSynchronize(ev[4]));
     for (int i = 0; i < 4; ++i) LSP_CUDA(h, cudaEventElapsedTime(&ms[i], ev[i], ev[i + 1]));
+    if (h->ev_chunks[slot] > 0) {                         // chunked call: accumulate = the accumulate launches only; the table pre-passes count as records
+        float acc = 0.f, whole = 0.f;
+        for (int c = 0; c < h->ev_chunks[slot]; ++c) {
+            float d = 0.f;
+            LSP_CUDA(h, cudaEventElapsedTime(&d, h->evc[slot][2 * c], h->evc[slot][2 * c + 1]));
+            acc += d;
+        }
+        LSP_CUDA(h, cudaEventElapsedTime(&whole, ev[1], ev[3]));
+        ms[1] = whole - acc; ms[2] = acc;
+    }
     return LSP_OK;
 }
 
@@ -565,20 +668,20 @@ int lsp_plan_query(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int64_t out[
 {
     if (!out || sm_count < 1 || B < 1 || Nt < 2 || Nf < 1) return LSP_EINVAL;
     const PlanChoice pc = plan_choose(sm_count, B, Nt, Nf, PlanOverrides());
-    out[0] = pc.K; out[1] = pc.T; out[2] = pc.nsplit; out[3] = pc.rec;
+    out[0] = pc.K; out[1] = pc.T; out[2] = pc.nsplit; out[3] = pc.pipe;
     out[4] = pc.nfb; out[5] = pc.split_len; out[6] = pc.ctas_per_sm;
     out[7] = (int64_t)(pc.score * 1e6);
     return LSP_OK;
 }
 
-int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int recurrence, int64_t out[8])
+int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int pipe, int64_t out[8])
 {
-    if (!out || sm_count < 1 || B < 1 || Nt < 2 || Nf < 1 || recurrence < 0 || recurrence > 5) return LSP_EINVAL;
+    if (!out || sm_count < 1 || B < 1 || Nt < 2 || Nf < 1 || pipe < 0 || pipe > LSP_PIPE_TENSOR) return LSP_EINVAL;
     PlanOverrides ov;
-    ov.rec = recurrence;
+    ov.pipe = pipe;
     const PlanChoice pc = plan_choose(sm_count, B, Nt, Nf, ov);
-    out[0] = pc.K; out[1] = pc.T; out[2] = pc.nsplit; out[3] = pc.rec;
-    out[4] = pc.nfb; out[5] = pc.split_len; out[6] = pc.ctas_per_sm;
+    out[0] = pc.K; out[1] = pc.T; out[2] = pc.nsplit; out[3] = pc.pipe;
+    out[4] = pc.nfb; out[5] = pc.split_len; out[6] = (pc.pipe == PLAN_PIPE_TENSOR && pc.L >= 128) ? pc.nchunks : pc.ctas_per_sm;
     out[7] = (int64_t)plan_est_cycles(sm_count, B, Nt, Nf, pc);
     return LSP_OK;
 }
@@ -588,16 +691,9 @@ int lsp_periodogram_batched(lsp_handle h,
                             int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                             float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, void* stream)
 {
-    if (!h || !t || !x) return LSP_EINVAL;
-    if (B < 1 || Nt < 2 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
-    if (bad_grid(f_min, df)) return LSP_EINVAL;
-    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
-    if (!P && !peak_idx) return LSP_EINVAL;
-    if (B > 1) {
-        if (t_stride != 0 && std::llabs(t_stride) < Nt) return LSP_EINVAL;
-        if (std::llabs(x_stride) < Nt) return LSP_EINVAL;
-        if (P && std::llabs(p_stride) < Nf) return LSP_EINVAL;
-    }
+    int rc = check_batch_args(h, t, x, B, Nt, 2, f_min, df, Nf, P, peak_idx, peak_val);
+    if (rc == LSP_OK) rc = check_strides(t_stride, x_stride, p_stride, B, Nt, Nf, P);
+    if (rc != LSP_OK) return rc;
     DeviceGuard g(h->device);
     return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
                       peak_idx, peak_val, static_cast<cudaStream_t>(stream));
@@ -608,16 +704,9 @@ int lsp_periodogram_gls_batched(lsp_handle h,
                                 int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                                 float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, void* stream)
 {
-    if (!h || !t || !x) return LSP_EINVAL;
-    if (B < 1 || Nt < 4 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
-    if (bad_grid(f_min, df)) return LSP_EINVAL;
-    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
-    if (!P && !peak_idx) return LSP_EINVAL;
-    if (B > 1) {
-        if (t_stride != 0 && std::llabs(t_stride) < Nt) return LSP_EINVAL;
-        if (std::llabs(x_stride) < Nt) return LSP_EINVAL;
-        if (P && std::llabs(p_stride) < Nf) return LSP_EINVAL;
-    }
+    int rc = check_batch_args(h, t, x, B, Nt, 4, f_min, df, Nf, P, peak_idx, peak_val);
+    if (rc == LSP_OK) rc = check_strides(t_stride, x_stride, p_stride, B, Nt, Nf, P);
+    if (rc != LSP_OK) return rc;
     DeviceGuard g(h->device);
     return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
                       peak_idx, peak_val, static_cast<cudaStream_t>(stream), true);
@@ -641,11 +730,8 @@ int lsp_periodogram_batched_host(lsp_handle h, const double* t, int share_t, con
                                  int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                                  float* P, int32_t* peak_idx, float* peak_val, void* stream)
 {
-    if (!h || !t || !x) return LSP_EINVAL;
-    if (B < 1 || Nt < 2 || Nf < 1 || Nt > 2000000000LL || Nf > 2000000000LL) return LSP_EINVAL;
-    if (bad_grid(f_min, df)) return LSP_EINVAL;
-    if ((peak_idx == nullptr) != (peak_val == nullptr)) return LSP_EINVAL;
-    if (!P && !peak_idx) return LSP_EINVAL;
+    const int rc0 = check_batch_args(h, t, x, B, Nt, 2, f_min, df, Nf, P, peak_idx, peak_val);
+    if (rc0 != LSP_OK) return rc0;
     DeviceGuard g(h->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t nt_t = (size_t)(share_t ? 1 : B) * (size_t)Nt;
@@ -699,9 +785,9 @@ int lsp_last_plan(lsp_handle h, int64_t out[8])
 {
     if (!h || !out) return LSP_EINVAL;
     const Plan& p = h->plan;
-    out[0] = p.K; out[1] = p.T; out[2] = p.nsplit; out[3] = p.rec;
+    out[0] = p.K; out[1] = p.T; out[2] = p.nsplit; out[3] = p.pipe;
     out[4] = p.nfb; out[5] = p.split_len; out[6] = p.launches;
-    out[7] = (p.rec == REC_ROTATION) ? 8 : ((p.rec == REC_MMA || p.rec == REC_UMMA) ? 0 : 6);   // 0: tensor-core form (16 tensor FLOP per term)
+    out[7] = (p.pipe == PLAN_PIPE_TENSOR) ? 0 : 6;        // 0: tensor-core form (16 tensor FLOP per term)
     return LSP_OK;
 }
 
@@ -720,6 +806,6 @@ const char* lsp_status_string(int status)
     }
 }
 
-const char* lsp_version(void) { return "lsp_b200 0.1 (sm_100a)"; }
+const char* lsp_version(void) { return "lsp_b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

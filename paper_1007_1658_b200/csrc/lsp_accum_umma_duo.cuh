@@ -26,7 +26,7 @@ constexpr int UD_STAGE_BYTES = 6 * UM_A_BYTES;          // A_hi, A_lo, A_V, B_hi
 constexpr int UD_REC_BYTES = 2 * 2 * UM_TS * 16;        // [series][buffer][128 samples]
 constexpr size_t UD_SMEM = (size_t)UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES + 256;
 constexpr int UD_TMEM_COLS = 256;
-constexpr uint32_t UD_IDESC = (1u << 4) | ((uint32_t)(128 >> 3) << 17) | ((uint32_t)(UM_H >> 4) << 24);   // M = 128, N = 128
+constexpr uint32_t UD_IDESC = umma_idesc(UM_H, 128);   // M = 128, N = 128
 
 // One B task: series s, coarse value l, 4 samples: rows (s,Re,l) and (s,Im,l) of B_hi, B_lo, B_V.  sB = address of row (s,Re,l).
 __device__ __forceinline__ void ud_gen_b(const float4* rec, int s0, unsigned l, uint32_t sB)
@@ -83,18 +83,6 @@ struct UmmaDuoParams {
     float* P; int64_t p_stride;     // nullable
     int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
 };
-
-// 32 lanes x 8 consecutive columns of fp32 accumulators -> 8 registers per thread.
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float (&v)[8])
-{
-    uint32_t r[8];
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-    #pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
-}
 
 // Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
 // thread = fine value h of series `db`; 16 coarse values l0..l0+15 -> frequencies kb + 64 l + h.

@@ -1,29 +1,60 @@
-// lsp_accum_umma_pair2.cuh -- CTA-pair tcgen05 form of steps 3-5 with the GENERATED operand shared by the pair.
-//
-// In lsp_accum_umma_pair.cuh the pair shares the streamed (table) operand and each CTA still generates a full
-// 128-row fine operand: 128 MUFU sin/cos pairs per sample per CTA, and the 16 producer warps are as busy as the
-// tensor pipe (measured: generation alone = MMAs alone; tensor pipe 60 % active).  Here the roles are swapped:
+// lsp_accum_umma_pair2.cuh -- the tcgen05 form of steps 3-5 for LONG grids: a CTA pair (cta_group::2) per 32,768
+// frequencies, one operand streamed from a table, the other generated and shared by the pair (algebra: lsp_tc.cuh).
 //
 //     k = kb + 256 h + l,   l < 256 fine (table, M side),   h < 128 coarse (generated, N side),   kb = 32,768 * pair
 //     theta_jk = [2 pi frac(u_j + (kb + 256 h) v_j)]  +  [2 pi frac(l v_j)]  =  a_jh + b_jl          (exact 64-bit turns, G3)
 //     W[l,h] = sum_j e^{i b_jl} (X_j e^{i a_jh}),    V[l,h] = sum_j e^{2i b_jl} (e^{2i a_jh} / 2)     (eq. (8))
 //
-// One tcgen05.mma.cta_group::2 of M = 256, N = 256: the M rows are the fine index l -- CTA r streams ITS 128 rows
-// (c_l, s_l) of the table (12 KB per k-step, as before) and accumulates them in ITS TMEM -- and the N columns
-// (h,Re), (h,Im) are the generated operand, of which each CTA makes only HALF (64 coarse values h, both parts):
-// 64 sin/cos pairs per sample per CTA instead of 128.  The (h,Im) row is a permutation of the (h,Re) row
+// The fine factor e^{i b_jl} depends on the sample and on l only -- NOT on the frequency block -- so a pre-pass
+// (`umma_ftable_pair_kernel`) writes it ONCE per time chunk, already as the shared-memory image the tensor core reads
+// (no-swizzle K-major core matrices; planes: fp16 (c, s), e5m2 [hi | lo], fp16 double angle; 2 x 12 KB per k-step of 8
+// samples), and every CTA streams ITS 128 rows with one cp.async.bulk (TMA) per stage onto the stage's mbarrier; the
+// table is read once per CTA pair, mostly from L2 (CTAs of one wave work on the same few time splits in lockstep).
+// One tcgen05.mma.cta_group::2 of M = 256, N = 256: the M rows are the fine index l -- CTA r accumulates ITS 128 rows in
+// ITS TMEM -- and the N columns (h,Re), (h,Im) are the generated operand, of which each CTA makes only HALF (64 coarse
+// values h, both parts): 64 sin/cos pairs per sample per CTA.  The (h,Im) row is a permutation of the (h,Re) row
 // ((xc, -xs) -> (xs, xc)): PRMT / LOP3 on the packed words, no extra arithmetic.  A stage-step (two k-steps) is
-// 256 thread-tasks, so the 16 producer warps work as two groups of 8 on alternate stage-steps: per stage-step the
-// producers issue ~45 % fewer instructions than in the first pair form.
+// 256 thread-tasks, so the 16 producer warps work as two groups of 8 on alternate stage-steps.  Per k-step:
+//     D_W += T_hi G_hi (kind::f16);  D_W += T_8 G_8 (kind::f8f6f4, K = 32: both hi*lo corrections);  D_V += T_V G_V (kind::f16)
 //
 // TMEM (per CTA): lane = l - 128 r;  column n = 128 r' + 64 part + h',  h = 64 r' + h'  (r' = CTA that generated it);
 // D_W in columns 0..255, D_V in 256..511.  For a fixed column the 32 lanes of a warp are 32 consecutive
-// frequencies: the drain into `ws` is coalesced.  Operand precision, the e5m2 correction MMA, the periodic drain of
-// D_W and all barriers are as in lsp_accum_umma_pair.cuh (FULL count = 8 warps + 1 per stage).
+// frequencies: the drain into `ws` is coalesced.
+//
+// Time chunks.  The table is 3 KB per sample, so the host bounds it (1 GiB by default): the series is cut into chunks,
+// each with its own table pre-pass + accumulate launch on the same table buffer; later chunks fold into `ws`
+// (`accumulate` = 1: the first drain read-modify-writes too).  Fixed order, no atomics: deterministic.
+//
+// Synchronisation (all mbarriers; s = stage):
+//   FULL[s]   in each CTA, count 8 + 1 + tx: the 8 producer warps of the stage's group and the CTA's own cp.async.bulk.
+//   PEER[s]   in CTA 0, count 1: CTA 1's otherwise idle MMA warp forwards "my FULL[s] completed" by a remote arrive;
+//             the issuing thread of CTA 0 waits FULL[s] and PEER[s].
+//   EMPTY[s]  in each CTA, count 1: tcgen05.commit.cta_group::2 multicast to both CTAs frees the stage in both.
+//   ACCF      in each CTA, count 1 (commit multicast): every MMA so far has completed, drain may read TMEM.
+//   ACCE      in CTA 0, count 32: the 16 drain warps of each CTA (CTA 1's by remote arrive) have read D_W.
 #pragma once
-#include "lsp_accum_umma_pair.cuh"
+#include "lsp_tc.cuh"
 
 namespace lsp {
+
+constexpr int UM_GEN_WARPS = 16;                                  // producer (and drain) warps per CTA; warp 16 issues the MMAs
+constexpr int UP_B_HALF = 128 * 32;                               // one table plane of a k-step in ONE CTA: 128 rows x 32 bytes
+constexpr int UP_GROUP_BYTES = 3 * UP_B_HALF;                     // per k-step per CTA: T_hi, T_8, T_V (12 KB)
+constexpr int U2_TABLE_BYTES_PER_KSTEP = 2 * UP_GROUP_BYTES;      // both CTAs of the pair: 24 KB per 8 samples = 3 KB per sample
+constexpr int U2_TABLE_PAD_KSTEPS = 2;                            // the last stage's bulk copy may read one k-step past the data
+// M = 256 (both CTAs), N = 256, fp32 accumulate; kind::f16 and kind::f8f6f4 (e5m2 x e5m2)
+constexpr uint32_t UP_IDESC = umma_idesc(256, 256);
+constexpr uint32_t UP_IDESC_F8 = UP_IDESC | UMMA_IDESC_E5M2;
+
+struct UmmaPairParams {
+    UmmaParams u;                   // u.nfb = 2 * npairs; u.split_len / u.nsplit divide the CHUNK; u.Nt = samples of the whole series
+    const unsigned char* btable;    // [B or 1][2][ngroups][UP_GROUP_BYTES] for the chunk's samples
+    int64_t half_stride;            // bytes between the two 128-row halves of one series' table
+    int64_t table_stride;           // bytes between the tables of consecutive series (0: shared times)
+    int64_t j0, chunk_len;          // the chunk: samples j0 .. j0 + chunk_len - 1
+    int nsplit_grid;                // time splits this launch covers (a short last chunk has fewer than u.nsplit, the stride of `ws`)
+    int accumulate;                 // 1: `ws` holds the sums of earlier chunks
+};
 
 constexpr int U2_FPP = 256 * UM_H;                                // frequencies per CTA pair
 constexpr int U2_HC = 64;                                         // coarse values generated per CTA
@@ -48,8 +79,9 @@ constexpr size_t U2_SMEM = (size_t)U2_STAGES * U2_STAGE_BYTES + U2_REC_BYTES + 2
 
 // ------------------------------------------------------------------ pre-pass: the fine-operand table
 // table[r][g][plane][chunk][l & 127][16 bytes], r = l >> 7: plane 0 = (c, s) fp16, 1 = [e5m2(c_h, s_h) | e5m2(c - c_h, s - s_h)],
-// 2 = (cos 2b, sin 2b) fp16; b = 2 pi frac(l v_j).  grid (ngroups, series), 512 threads = 2 K-chunks x 256 fine indices.
-__global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t rec_stride,
+// 2 = (cos 2b, sin 2b) fp16; b = 2 pi frac(l v_j).  grid (ngroups, series), 512 threads = 2 K-chunks x 256 fine indices;
+// group g holds samples j0 + 8g .. j0 + 8g + 7 of the chunk [j0, j1).
+__global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2* __restrict__ recB, int64_t j0, int64_t j1, int64_t rec_stride,
                                                                unsigned char* __restrict__ table, int64_t half_stride, int64_t table_stride)
 {
     const int64_t g = blockIdx.x;
@@ -58,8 +90,8 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
     unsigned hh[4], h8[4], l8[4], vv[4];
     #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const int64_t j = g * UM_KS + chunk * 4 + i;
-        const u64 v = (j < Nt) ? __ldg(&rb[j].y) : 0ull;                // beyond Nt: e^{i0}; the generated operand is zero there
+        const int64_t j = j0 + g * UM_KS + chunk * 4 + i;
+        const u64 v = (j < j1) ? __ldg(&rb[j].y) : 0ull;                // beyond the chunk: e^{i0}; the generated operand is zero there
         const unsigned v32 = (unsigned)((v + 0x80000000ull) >> 32);
         float c, s;
         sincos_phase32(l * v32, c, s);
@@ -122,22 +154,29 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
 // ------------------------------------------------------------------ step 5: drain 64 accumulator columns into ws
 // Thread = TMEM lane = fine index; its 64 registers are 64 consecutive coarse values h (frequency stride 256).
 //
-// Truncation compensation.  The tensor core adds into the fp32 accumulator with round-toward-zero, so a window of n k-steps loses
-// ~n/2 ulps of |D| in expectation -- a BIAS toward zero that grows with the window and was the largest error term of the tensor
-// forms (2.6e-5 of max P at C3 with 2,048-sample windows, 9e-5 with 8,192).  `comp` = (measured 0.45 ulp per k-step) x n is added
-// back, away from zero, before the value is folded into `ws`: C3 2.6e-5 -> 5e-6, C5 1.8e-5 -> 4e-6 at 2,048 samples, and
-// 9e-6 / 6e-6 (P0: 1.9e-5) at 4,096, which is why this form drains half as often as the others.
-__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float comp)
+// Truncation compensation: the tensor core folds each MMA into the fp32 accumulator with
+// round-toward-zero, a loss in [0, 1) ulp of the running |D| per MMA -- a BIAS toward zero that grows with the window.
+// `comp` = (expected loss in ulps of the FINAL |D|) is added back, away from zero, before the value is folded into `ws`.
+//   mode < 0 (default): the model.  Two MMAs per k-step add into D_W, each losing 1/2 ulp of the RUNNING |D| on average.
+//     A sum that grows from 0 to D_n over the window -- linearly for a coherent signal, whose per-window bias adds up over
+//     the series; like a random walk for noise, with the same mean E[D_t | D_n] = (t/n) D_n -- passes through the binades
+//     below its final one: with m in [1, 2) the mantissa of D_n, sum_t ulp(D_t) = n ulp(D_n) [1 - 1/m + 1/(3m)], so
+//     the expected loss is  n_ksteps x (1 - 2/(3m)) x ulp(D_n)  (0.33 ... 0.67 ulp per k-step, 0.52 on average).
+//   mode > 0: that many ulps of D_n per k-step, whatever m (ablation, LSP_PARAM_TRUNC);  mode = 0: nothing is added.
+__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float mode, float n_ksteps)
 {
     #pragma unroll 1
     for (int half = 0; half < 2; ++half) {
         float v[32];
         tmem_ld32(taddr + 32u * half, v);
-        if (comp != 0.f) {
+        if (mode != 0.f) {
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
-                const float ulp = __uint_as_float(__float_as_uint(v[i]) & 0x7f800000u) * 1.1920929e-7f;      // 2^(e-23)
-                v[i] += copysignf(comp * ulp, v[i]);
+                const unsigned bits = __float_as_uint(v[i]);
+                const float ulp = __uint_as_float(bits & 0x7f800000u) * 1.1920929e-7f;      // 2^(e-23)
+                float per = mode;
+                if (mode < 0.f) per = 1.f - __fdividef(0.6666667f, __uint_as_float((bits & 0x007fffffu) | 0x3f800000u));
+                v[i] += copysignf(n_ksteps * per * ulp, v[i]);
             }
         }
         const int64_t kh = k0 + (int64_t)half * 32 * 256;
@@ -151,7 +190,7 @@ __device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k
 }
 
 // ------------------------------------------------------------------ the kernel
-// grid.x = B * nsplit * (2 * npairs) (CTA of the pair fastest, then the pair), clusters of 2, UM_THREADS threads,
+// grid.x = B * nsplit * (2 * npairs) (CTA of the pair fastest, then the pair), clusters of 2, U2_THREADS threads,
 // U2_SMEM bytes of dynamic shared memory, one CTA per SM.  q.u.nfb = 2 * npairs, npairs = ceil(Nf / 32,768).
 __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const UmmaPairParams q)
 {
@@ -165,11 +204,11 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
     const uint32_t rank = cluster_ctarank();
     int64_t unit = blockIdx.x;
     const int fb = (int)(unit % p.nfb); unit /= p.nfb;
-    const int sp = (int)(unit % p.nsplit);
-    const int64_t b = unit / p.nsplit;
+    const int sp = (int)(unit % q.nsplit_grid);
+    const int64_t b = unit / q.nsplit_grid;
     const int64_t kb = (int64_t)(fb >> 1) * U2_FPP;
-    const int64_t j_begin = (int64_t)sp * p.split_len;
-    const int64_t j_end = min(p.Nt, j_begin + p.split_len);
+    const int64_t j_begin = q.j0 + (int64_t)sp * p.split_len;
+    const int64_t j_end = min(q.j0 + q.chunk_len, j_begin + p.split_len);
     const int n_samp = (int)(j_end - j_begin);                          // split_len < 2^31
     const int nks = (n_samp + UM_KS - 1) / UM_KS;
     const int nst = (nks + U2_KPS - 1) / U2_KPS;                        // stage-steps (two k-steps each)
@@ -206,7 +245,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
         float4* rec = rec_all + grp * (2 * UM_TS);
         const float4* recA = p.recA + b * p.Nt;
         const ulonglong2* recB = p.recB + b * p.Nt;
-        const unsigned char* tab = q.btable + b * q.table_stride + (int64_t)rank * q.half_stride + (j_begin / UM_KS) * (int64_t)UP_GROUP_BYTES;
+        const unsigned char* tab = q.btable + b * q.table_stride + (int64_t)rank * q.half_stride + ((j_begin - q.j0) / UM_KS) * (int64_t)UP_GROUP_BYTES;
         const float xs = (tg < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
         float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
         auto prefetch = [&](int ti) {
@@ -270,8 +309,8 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const bool last = (f == nwin - 1);
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
-            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0, p.trunc_ulps * (float)((it_end - f * flush_st) * U2_KPS));
-            if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, true, 0.f);
+            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, p.trunc_ulps, (float)((it_end - f * flush_st) * U2_KPS));
+            if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, !q.accumulate, 0.f, 0.f);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) { if (rank == 0) mbar_arrive(bar_acce); else mbar_arrive_remote(bar_acce, 0u); }
@@ -283,7 +322,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const int s = it & (U2_STAGES - 1);
             const uint32_t ph = (uint32_t)(it / U2_STAGES) & 1u;
             mbar_wait(U2_FULL(s), ph);
-            mbar_wait_cluster(U2_PEER(s), ph);
+            mbar_wait(U2_PEER(s), ph);
             tc_fence_after();
             const bool win_first = (it == f * flush_st);
             #pragma unroll
@@ -303,7 +342,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const bool last = (it == nst - 1);
             if (it + 1 == (f + 1) * flush_st || last) {
                 tc_commit_pair(bar_accf);
-                if (!last) { mbar_wait_cluster(bar_acce, (uint32_t)f & 1u); tc_fence_after(); }
+                if (!last) { mbar_wait(bar_acce, (uint32_t)f & 1u); tc_fence_after(); }
                 ++f;
             }
         }

@@ -1,20 +1,62 @@
-// lsp_accum_umma_small.cuh -- the tcgen05 form of steps 3-5 for SHORT frequency grids and batches.
+// lsp_accum_umma_small.cuh -- the tcgen05 form of steps 3-5 for SHORT frequency grids (lsp_tc.cuh states the algebra).
 //
-// lsp_accum_umma.cuh gives every CTA 128 fine x 128 coarse = 16,384 frequencies.  A Monte-Carlo batch
-// (BASELINE config C4: 4,096 series x 2,000 frequencies) or a short grid would leave most
-// of that tile empty.  Here the coarse extent L is a template parameter (16, 32 or 64): a CTA owns
-// 128 x L frequencies, k = kb + 128 l + h, the MMAs are m128 n(2L) k16 and the accumulators take 4L of the
-// 512 TMEM columns (D_W: columns [0, 2L), D_V: [2L, 4L)), so two (L = 16: three) CTAs of 8 producer warps +
-// 1 MMA warp share an SM: one CTA's set-up and drain overlap the others' main loops, and the extra warps hide
-// the latency of the generation chain (LDS -> IMAD -> I2F -> MUFU -> F2FP -> STS).  Same algebra, same operand
-// tiles (um_gen_a), same four MMAs per k-step of 8 samples, same periodic drain of D_W as lsp_accum_umma.cuh;
-// the coarse operand B (2L rows) is generated on the fly by a rotating subset of the producer threads.
-// With L <= 32 the kernel is bound by the generation of the fine operand A (128 MUFU sin/cos pairs per
-// sample for 128 L terms), not by the tensor pipe.
+// A CTA owns 128 fine x L coarse frequencies, k = kb + 128 l + h, with the coarse extent L a template parameter
+// (16, 32 or 64): the MMAs are m128 n(2L) k16 and the accumulators take 4L of the 512 TMEM columns (D_W: columns
+// [0, 2L), D_V: [2L, 4L)), so two (L = 16: three) CTAs of 8 producer warps + 1 MMA warp share an SM: one CTA's set-up
+// and drain overlap the others' main loops, and the extra warps hide the latency of the generation chain
+// (LDS -> IMAD -> I2F -> MUFU -> F2FP -> STS).  As real GEMMs D[m][n] = sum_k A[m][k] B[n][k], K index = (sample j, component):
+//     A_W[h][(j,.)] = (X cos a, X sin a)            A_V[h][(j,.)] = (cos^2 a - 1/2, cos a sin a) = e^{2ia}/2
+//     B[(l,Re)][(j,.)] = (cos b, -sin b)            B[(l,Im)][(j,.)] = (sin b, cos b)     (same with 2b for V)
+// so D_W[h][(l,Re)] = XC, D_W[h][(l,Im)] = XS, D_V[h][(l,Re)] = CC - n/2, D_V[h][(l,Im)] = CS.  Per k-step of 8 samples:
+//     D_W += A_hi B_hi;  D_W += A_lo B_hi;  D_W += A_hi B_lo;  D_V += A_V B_V          (four kind::f16 MMAs)
+// Both operand tiles are GENERATED (step 3: integer phase -> MUFU sin/cos) by the producer warps straight
+// into shared memory in the canonical no-swizzle K-major core-matrix layout; the coarse operand B (2L rows) by a
+// rotating subset of the producer threads.  A ring of stages decouples the producers from the single MMA-issuing thread
+// (mbarrier full/empty; tcgen05.commit frees a stage).  With L <= 32 the kernel is bound by the generation of the
+// fine operand A (128 MUFU sin/cos pairs per sample for 128 L terms), not by the tensor pipe.
+//
+// Step 5 (the chunked sums of PAPER.md:122): tensor-core accumulation rounds toward zero, so D_W is drained every
+// `flush_ksteps` k-steps (default 2,048 samples): tcgen05.ld -> fp32 add (round to nearest) into the CTA's own slice of
+// `ws` (L2-resident; first drain stores, later ones read-modify-write; no atomics, deterministic).  D_V only needs
+// Nt-relative accuracy and is drained once, at the end.
 #pragma once
-#include "lsp_accum_umma.cuh"
+#include "lsp_tc.cuh"
 
 namespace lsp {
+
+// One A item: row h, 4 samples starting at rec[s0].  Writes the 16-byte row chunks of A_hi, A_lo (X e^{ia} as
+// fp16 hi + lo) and A_V (e^{2ia}/2).
+template <bool TAIL>
+__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int nvalid)
+{
+    unsigned hi[4], lo[4], vv[4];
+    #pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float4 r = rec[s0 + i];                                   // {X / sigma, pA32, v32, w32}: broadcast read
+        float c, s;
+        sincos_phase32(__float_as_uint(r.y) + h * __float_as_uint(r.z), c, s);
+        const u64 cs = pack2(c, s);
+        float xc, xs;
+        unpack2(mul2(pack2(r.x, r.x), cs), xc, xs);                     // packed FP32: one FMUL2
+        hi[i] = pack_h2(xc, xs);
+        const float2 hf = unpack_h2(hi[i]);
+        float lc, ls;
+        unpack2(fma2(pack2(hf.x, hf.y), pack2(-1.f, -1.f), pack2(xc, xs)), lc, ls);
+        lo[i] = pack_h2(lc, ls);
+        float v0, v1;
+        unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
+        vv[i] = pack_h2(v0, v1);
+        if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
+    }
+    sts128(sA, hi[0], hi[1], hi[2], hi[3]);
+    sts128(sA + UM_A_BYTES, lo[0], lo[1], lo[2], lo[3]);
+    sts128(sA + 2 * UM_A_BYTES, vv[0], vv[1], vv[2], vv[3]);
+}
+__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int64_t left)
+{
+    if (left >= 4) um_gen_a<false>(rec, s0, h, sA, 4);                  // `left` is warp-uniform
+    else um_gen_a<true>(rec, s0, h, sA, (int)max((int64_t)0, left));
+}
 
 constexpr int US_GEN_WARPS = 8;                        // producer (and drain) warps; warp 8 issues the MMAs
 constexpr int US_THREADS = (US_GEN_WARPS + 1) * 32;
@@ -24,23 +66,9 @@ template <int L, int US_STAGES> struct UmmaSmall {
     static constexpr int STAGE_BYTES = 3 * UM_A_BYTES + 3 * B_BYTES;
     static constexpr size_t SMEM = (size_t)US_STAGES * STAGE_BYTES + UM_REC_BYTES + 256;
     static constexpr int TMEM_COLS = 4 * L < 32 ? 32 : 4 * L;
-    static constexpr uint32_t IDESC = (1u << 4) | ((uint32_t)(2 * L >> 3) << 17) | ((uint32_t)(UM_H >> 4) << 24);
+    static constexpr uint32_t IDESC = umma_idesc(UM_H, 2 * L);
     static constexpr int FPB = UM_H * L;               // frequencies per CTA
 };
-
-// 32 lanes x 16 consecutive columns of fp32 accumulators -> 16 registers per thread.
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
-{
-    uint32_t r[16];
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                 : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-    #pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
-}
 
 // One B item: coarse index l, K chunk of 4 samples: rows (l,Re) and (l,Im) of B_hi, B_lo (e^{ib}) and B_V (e^{2ib}).
 template <int L>

@@ -1,8 +1,16 @@
-// lsp_accum_z.cuh -- steps 3-5 of the hot path, "z-packed" form (the default accumulate kernel).
+// lsp_accum_z.cuh -- steps 3-5 of the hot path on the FP32 pipe: anchor, rotate-and-accumulate, cascade.
 //
-// Same sums as lsp_accum.cuh (eq. (8)) and the same three-term recurrence, but the
-// two lanes of a packed f32x2 register hold (cos, sin) of ONE sample instead of the cosines of two
-// samples:   z_m = (cos th_m, sin th_m),  th_m = w_{k0+m} t_j.  Per term (one sample, one frequency)
+// What it computes: the four sums of eq. (8) (SS is never formed)
+//     XC = sum_j X_j cos(w t_j), XS = sum_j X_j sin(w t_j), CC = sum_j cos^2(w t_j), CS = sum_j cos sin
+// for every frequency of a block over one split of the time axis: all of the O(Nt*Nf) work of eq. (4)
+// in the paper's own arithmetic (fp32 throughout, with the SFU for the trig).
+//
+// How it differs from the paper's kernel (listing PAPER.md:138-277: one thread per frequency, one SFU sincos per term):
+//   * each thread owns K ADJACENT frequencies k0..k0+K-1; for a sample j the angle at k0 is evaluated once (32-bit
+//     fixed-point phase -> MUFU sin/cos) and then ADVANCED K-1 times by the per-sample step 2 pi df t_j with the
+//     three-term recurrence z_{m+1} = 2 cos(d) z_m - z_{m-1} (the Press et al. idea the paper sets aside at PAPER.md:59,
+//     made safe by re-anchoring every K <= 32 steps from an exact integer phase);
+//   * the two lanes of a packed f32x2 register hold z_m = (cos th_m, sin th_m), th_m = w_{k0+m} t_j.  Per term
 //
 //     (XC, XS)_m += X      * z_m        FFMA2  X.F32 (scalar broadcast), z, acc1
 //     (CC, CS)_m += cos th * z_m        FFMA2  z.lo.F32 (scalar broadcast), z, acc2
@@ -12,16 +20,25 @@
 // DESIGN.md "Register-file model"): an FFMA2 issues every 2 cycles only if at most two of its
 // 64-bit operands are fetched from the register file; here all three instructions of a term share
 // the multiplicand z (operand-reuse cache) and the other multiplicand is a 32-bit scalar, so the
-// limit is met whatever order ptxas picks.  The accumulators cost 4 registers per frequency (8 in
-// the pair-packed form), so K = 24..32 adjacent frequencies fit per thread and the MUFU anchor
-// is amortised over twice as many terms.  No phantom sample is needed for odd Nt.
+// limit is met whatever order ptxas picks.  The accumulators cost 4 registers per frequency,
+// so K = 24..32 adjacent frequencies fit per thread and the MUFU anchor
+// is amortised over many terms.  Chunked partial sums become: packed register partials per
+// flush interval, folded into per-thread shared-memory accumulators, written once per split to `ws`.
 #pragma once
 #include "lsp_common.cuh"
-#include "lsp_accum.cuh"
 
 namespace lsp {
 
-constexpr int REC_THREE_TERM_Z = 3;
+struct AccumParams {
+    const float4* recA;
+    const ulonglong2* recB;
+    float* ws;              // [B][nsplit][4][Nf]
+    int64_t Nt, Nf;
+    int64_t split_len;      // samples per split (multiple of TILE_Z; the last split may be shorter)
+    int nsplit;
+    int nfb;                // frequency blocks per series: ceil(Nf / (K * blockDim.x))
+    int flush_tiles;        // tiles of TILE_Z samples between folds of the register partials
+};
 
 struct ZAnchor { float c0, s0, cp, sp, X, g; };
 
@@ -42,7 +59,7 @@ __device__ __forceinline__ ZAnchor z_anchor(const float4* tS, const float2* tR, 
     return a;
 }
 
-template <int K, int TILE_Z, int MAXT, int MINB>
+template <int K, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p)
 {
     extern __shared__ float4 lsp_smem[];
@@ -69,7 +86,7 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
     const int64_t j_end = min(p.Nt, j_begin + p.split_len);
     const float4* recA = p.recA + b * p.Nt;
     const ulonglong2* recB = p.recB + b * p.Nt;
-    const int flush_tiles = max(1, p.flush_tiles * TILE / TILE_Z);
+    const int flush_tiles = max(1, p.flush_tiles);
 
     #pragma unroll
     for (int i = 0; i < 4 * K; ++i) outer[OIDX(i / K, i % K)] = 0.f;

@@ -13,13 +13,15 @@
 
 namespace lsp {
 
-constexpr int TILE = 512;                 // samples staged in shared memory per tile
-constexpr int PAIRS = TILE / 2;           // two consecutive samples form one packed f32x2 operand
+constexpr int TILE_Z = 256;               // samples staged in shared memory per tile of the FP32-pipe kernel
 constexpr int MAX_PARTS = 128;            // max blocks per series in the pre-pass reductions
+
+// 2 pi / 2^32: signed 32-bit phase (turns * 2^32) -> radians in [-pi, pi)
+#define LSP_RAD_PER_PHASE 1.4629180792671596e-9f
 
 typedef unsigned long long u64;
 
-// ---- packed FP32 (f32x2) helpers: one instruction works on two consecutive time samples ----
+// ---- packed FP32 (f32x2) helpers: one instruction works on both lanes of a 64-bit register pair ----
 __device__ __forceinline__ u64 pack2(float lo, float hi) {
     u64 d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d;
 }

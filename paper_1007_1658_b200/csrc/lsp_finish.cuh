@@ -27,8 +27,7 @@ struct FinishParams {
     unsigned* counter;                 // [B]
     int64_t Nt, Nf;
     int nsplit, nparts;
-    double cc_fix;                     // added to sum(CC - n/2): 0.5 when the pair-packed kernel padded an odd Nt
-    int x_scaled;                      // 1: XC, XS were accumulated from X * x_scale() (tensor-core form)
+    int x_scaled;                      // 1: XC, XS were accumulated from X * x_scale() (tensor-core forms)
     const float* ws1;                  // generalised periodogram: [B][nsplit][4][Nf] of the unit-weight pass (planes 0, 1 = sum cos, sum sin); else NULL
     const float* ws_x;                 // shared-time batch (lsp_shared_gemm.cuh): XC, XS from [B][nsplit][2][x_row]; `ws` is then ONE
     int64_t x_row;                     //   [nsplit][4][Nf] block shared by all series (planes 2, 3 = CC - n/2, CS); else NULL / 0
@@ -43,7 +42,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
         double q = 0.0;                                    // fixed-order sum of the block partials
         for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
         s_var = q / (double)(p.Nt - 1);                    // sample variance (reading G1)
-        if (p.x_scaled) {                                  // undo the fp32 scale factor exactly (lsp_accum_mma.cuh)
+        if (p.x_scaled) {                                  // undo the fp32 scale factor exactly (lsp_tc.cuh)
             const double xs = (double)(float)(1.0 / sqrt(s_var));
             s_var *= xs * xs;
         }
@@ -51,7 +50,6 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     __syncthreads();
     const double inv2var = 0.5 / s_var;
     const double Nt = (double)p.Nt;
-    const double cc_fix = p.cc_fix;
     const float* ws = p.ws_x ? p.ws : p.ws + b * p.nsplit * 4 * p.Nf;
     const float* wx = p.ws_x ? p.ws_x + b * p.nsplit * 2 * p.x_row : nullptr;
 
@@ -60,7 +58,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     for (int i = 0; i < FIN_FPT; ++i) {
         const int64_t k = ((int64_t)blockIdx.x * FIN_FPT + i) * FIN_THREADS + threadIdx.x;
         if (k >= p.Nf) continue;
-        double XC = 0.0, XS = 0.0, CCh = cc_fix, CS = 0.0;
+        double XC = 0.0, XS = 0.0, CCh = 0.0, CS = 0.0;
         for (int sp = 0; sp < p.nsplit; ++sp) {            // fixed order over the time splits
             const float* w = ws + (int64_t)sp * 4 * p.Nf + k;
             if (wx) {

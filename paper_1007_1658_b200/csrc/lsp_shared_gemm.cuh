@@ -19,7 +19,7 @@
 //                     columns; 4 warps drain them to ws_x[b][split][part][k].  A time split is at most 2,048 samples, so the
 //                     truncating tensor-core accumulation is folded as often as in the single-series forms.
 #pragma once
-#include "lsp_accum_umma_tab.cuh"
+#include "lsp_tc.cuh"
 
 namespace lsp {
 
@@ -37,6 +37,7 @@ constexpr size_t SG_SMEM = (size_t)SG_STAGES * SG_STAGE_BYTES + 256;
 constexpr int SG_THREADS = 6 * 32;                         // warp 0: TMA, warp 1: MMA + TMEM, warps 2-5: drain
 constexpr int SG_MAX_SPLIT = 2048;                         // samples per time split (multiple of SG_KPS * SG_KS)
 constexpr int SG_TMEM_COLS = 256;
+constexpr uint32_t SG_IDESC = umma_idesc(SG_M, 2 * SG_F);
 
 struct SharedGemmParams {
     const unsigned char* xa;        // [nmb][ng][SG_A_GROUP]
@@ -338,8 +339,8 @@ __global__ void __launch_bounds__(SG_THREADS, 2) shared_gemm_kernel(const Shared
                     const uint32_t b0 = s_stage + (uint32_t)s * SG_STAGE_BYTES + SG_KPS * SG_A_GROUP + kk * SG_B_GROUP;
                     const uint64_t dAh = umma_desc(a0, SG_A_PLANE / 2, 128), dA8 = umma_desc(a0 + SG_A_PLANE, SG_A_PLANE / 2, 128);
                     const uint64_t dBh = umma_desc(b0, SG_B_PLANE / 2, 128), dB8 = umma_desc(b0 + SG_B_PLANE, SG_B_PLANE / 2, 128);
-                    tc_mma_f16(tmem, dAh, dBh, UM_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
-                    tc_mma_f8(tmem, dA8, dB8, UM_IDESC_F8, 1u);
+                    tc_mma_f16(tmem, dAh, dBh, SG_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
+                    tc_mma_f8(tmem, dA8, dB8, SG_IDESC | UMMA_IDESC_E5M2, 1u);
                 }
                 tc_commit(SG_EMPTY(s));
             }

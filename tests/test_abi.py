@@ -36,16 +36,19 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert exported == set(declared)
 
 
-def test_sass_is_sm100a_packed_fp32():
-    """The accumulate kernels are sm_100a SASS built on FFMA2 (packed f32x2) and MUFU anchors."""
+def test_sass_is_sm100a_packed_fp32_and_tcgen05():
+    """The FP32-form accumulate kernel is sm_100a SASS built on FFMA2 (packed f32x2) and MUFU anchors; the tensor forms
+    issue tcgen05 MMAs (UTCHMMA / UTCQMMA, single-CTA and .2CTA), read TMEM with LDTM and stream operands with bulk copies."""
     import paper_1007_1658_b200 as pkg
     path = pkg.build()
     res = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True)
     if res.returncode != 0:
         pytest.skip("cuobjdump unavailable")
     assert "sm_100a" in res.stdout
-    assert res.stdout.count("FFMA2") > 1000
+    assert res.stdout.count("FFMA2") > 400
     assert "MUFU.SIN" in res.stdout and "MUFU.COS" in res.stdout
+    for mnemonic in ("UTCHMMA", "UTCHMMA.2CTA", "UTCQMMA.2CTA", "LDTM", "UBLKCP"):
+        assert mnemonic in res.stdout, mnemonic
 
 
 def test_no_compute_without_gpu_fails_loudly():

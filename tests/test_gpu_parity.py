@@ -31,216 +31,251 @@ def _check(P_gpu, P_ref, what=""):
     return err / np.max(P_ref)
 
 
-def _same_peak(P_gpu, P_ref):
-    """Reading G9: the arg-max must be bit-exact on seed-QUALIFIED inputs (top-two gap >= 1e-5 max P).  The ad-hoc
-    ragged-size inputs of this file are not qualified; on a near-tie below that gap either bin is a valid peak."""
+RELAXED = []        # (test, gap) of every arg-max comparison that had to take the near-tie branch; must stay empty (test_zz_...)
+QUAL_GAP = 2e-4     # ad-hoc inputs are seed-qualified to this top-two gap: twice the tolerance, so that a path within TOL cannot flip it
+
+
+def _same_peak(P_gpu, P_ref, what=""):
+    """Reading G9: the arg-max must be bit-exact.  Inputs of this file are seed-qualified (`_qualified`): the oracle's top-two gap is
+    >= 2e-4 max P, which a result within TOL cannot flip.  A near-tie below that gap (either bin a valid peak) is still accepted but
+    RECORDED, and test_zz_no_argmax_comparison_was_relaxed fails if any comparison needed it."""
     i_gpu, i_ref = int(np.argmax(P_gpu)), oracle.argmax(P_ref)
-    return i_gpu == i_ref or (P_ref[i_ref] - P_ref[i_gpu]) < 1e-5 * P_ref[i_ref]
+    if i_gpu == i_ref:
+        return True
+    gap = float(P_ref[i_ref] - P_ref[i_gpu]) / float(P_ref[i_ref])
+    if gap < 1e-5:
+        RELAXED.append((what, gap))
+        return True
+    return False
 
 
-def _run_single(h, w, **params):
+def _top_two_gap(P):
+    o = np.argsort(P)
+    return float(P[o[-1]] - P[o[-2]]) / float(P[o[-1]])
+
+
+def _qualified(make, seed, ref_fn=None, tries=50):
+    """Input-side seed qualification (reading G9) with the oracle only: bump the seed until the top-two gap of every series
+    is >= QUAL_GAP.  `make(seed)` -> Workload; returns (workload, oracle periodogram[s])."""
+    for s in range(seed, seed + tries):
+        w = make(s)
+        if ref_fn is not None:
+            ref = ref_fn(w)
+        elif w.B > 1:
+            ref = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)[0]
+        else:
+            ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+        gaps = [_top_two_gap(r) for r in (ref if ref.ndim == 2 else [ref])]
+        if w.Nf < 2 or min(gaps) >= QUAL_GAP:
+            return w, ref
+    raise AssertionError("no qualified seed in %d tries" % tries)
+
+
+PARAM_KEYS = ("K", "THREADS", "NSPLIT", "PIPE", "FLUSH", "TABLE_MB", "COARSE", "TRUNC", "SHARED")
+
+
+class _params:
+    """Set LSP_PARAM_* tunables on the handle for the duration of a with-block (name=value, lower case), then restore 0."""
+    def __init__(self, h, **kw):
+        import paper_1007_1658_b200 as pkg
+        self.h = h
+        self.kv = {getattr(pkg, "PARAM_" + k.upper()): v for k, v in kw.items() if v}
+        assert all(k.upper() in PARAM_KEYS for k in kw)
+
+    def __enter__(self):
+        for k, v in self.kv.items():
+            self.h.set_param(k, v)
+        return self.h
+
+    def __exit__(self, *exc):
+        for k in self.kv:
+            self.h.set_param(k, 0)
+
+
+def _run_single(h, w, gls=False, **params):
     import torch
-    from paper_1007_1658_b200 import (PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_RECURRENCE, PARAM_FLUSH, PARAM_BTABLE,
-                                      PARAM_COARSE, PARAM_CORR, PARAM_PAIR)
-    keys = {"K": PARAM_K, "threads": PARAM_THREADS, "nsplit": PARAM_NSPLIT,
-            "rec": PARAM_RECURRENCE, "flush": PARAM_FLUSH, "btable": PARAM_BTABLE, "coarse": PARAM_COARSE, "corr": PARAM_CORR, "pair": PARAM_PAIR}
-    for k, v in keys.items():
-        h.set_param(v, params.get(k, 0))
-    try:
+    with _params(h, **params):
         t, x = _dev(w)
-        P = h.periodogram(t, x, w.f_min, w.df, w.Nf)
+        P = h.periodogram(t, x, w.f_min, w.df, w.Nf, gls=gls)
         torch.cuda.synchronize()
         return P.cpu().numpy()
-    finally:
-        for v in keys.values():
-            h.set_param(v, 0)
+
+
+def _run_batched(h, w, shared_t=False, gls=False, want_P=True, **params):
+    import torch
+    with _params(h, **params):
+        t = torch.from_numpy(np.ascontiguousarray(w.t[0] if (shared_t and w.t.ndim == 2) else w.t)).cuda()
+        x = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
+        P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf, gls=gls, want_P=want_P)
+        torch.cuda.synchronize()
+        plan = h.last_plan()
+    return (P.cpu().numpy() if P is not None else None), pi.cpu().numpy(), pv.cpu().numpy(), plan
+
+
+FP32, TENSOR = 1, 2      # LSP_PIPE_*
 
 
 # ------------------------------------------------------------------ full-grid parity, C1 and C2
-def test_C1_full_grid(lsp):
+@pytest.mark.parametrize("pipe", [0, FP32, TENSOR])
+def test_C1_full_grid(lsp, pipe):
     pkg, h = lsp
     w = workloads.c1()
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w)
+    P = _run_single(h, w, pipe=pipe)
     _check(P, ref, "C1")
     assert int(np.argmax(P)) == oracle.argmax(ref)
     assert abs(int(np.argmax(P)) - w.expected_peak_bin) <= 1
 
 
-def test_C2_full_grid(lsp):
+@pytest.mark.parametrize("pipe", [0, FP32, TENSOR])
+def test_C2_full_grid(lsp, pipe):
     pkg, h = lsp
     w = workloads.c2()
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w)
+    P = _run_single(h, w, pipe=pipe)
     _check(P, ref, "C2")
     assert int(np.argmax(P)) == oracle.argmax(ref)
 
 
-# ------------------------------------------------------------------ every kernel variant, ragged sizes
-@pytest.mark.parametrize("rec", [1, 2, 3])
+# ------------------------------------------------------------------ FP32 form: every K, ragged sizes
 @pytest.mark.parametrize("K", [4, 8, 12, 16, 20, 24, 28, 32])
-def test_variants_ragged(lsp, K, rec):
+def test_fp32_form_variants_ragged(lsp, K):
     """Nt odd and not a multiple of the tile, Nf not a multiple of K*threads, several splits and tiles."""
     pkg, h = lsp
-    if K >= 28 and rec != 3:
-        pytest.skip("K = 28, 32 exist only in the z-packed kernel")
     w = workloads.c1(Nt=2731, Nf=1777, seed=1234 + K)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
     big = 96 if K >= 28 else 256                       # K >= 28 is compiled for <= 128 threads per CTA
     for threads, nsplit in ((32, 0), (128, 2), (big, 1)):
-        P = _run_single(h, w, K=K, rec=rec, threads=threads, nsplit=nsplit, flush=512)
-        _check(P, ref, "K=%d rec=%d T=%d" % (K, rec, threads))
+        P = _run_single(h, w, K=K, pipe=FP32, threads=threads, nsplit=nsplit, flush=512)
+        _check(P, ref, "K=%d T=%d" % (K, threads))
         assert int(np.argmax(P)) == oracle.argmax(ref)
         plan = h.last_plan()
-        assert plan["K"] == K and plan["recurrence"] == rec and plan["threads"] == threads
-        assert plan["lane_ops_per_term"] == (8 if rec == 1 else 6)
+        assert plan["K"] == K and plan["pipe"] == FP32 and plan["threads"] == threads
+        assert plan["lane_ops_per_term"] == 6
 
 
-TC_FORMS = [4, 5]     # 4: mma.sync m16n8k16, 5: tcgen05.mma m128n256k16 with TMEM accumulators
+# ------------------------------------------------------------------ tensor forms, ragged sizes
+RAGGED = [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 50011, 0, 0), (1025, 8193, 2, 0), (127, 40, 0, 0), (130, 16385, 1, 0),
+          (4099, 3001, 1, 16), (4099, 3001, 2, 1000), (8, 100, 1, 0), (137, 33000, 1, 0), (1024, 8192, 1, 0), (129, 1024, 0, 0)]
 
 
-@pytest.mark.parametrize("rec", TC_FORMS)
-@pytest.mark.parametrize("Nt,Nf,nsplit", [(2731, 1777, 0), (2731, 1777, 3), (5000, 20011, 0), (1024, 8192, 1),
-                                          (1025, 8193, 2), (127, 40, 0), (129, 1024, 0), (130, 16385, 1)])
-def test_tensor_core_form_ragged(lsp, Nt, Nf, nsplit, rec):
-    """The tensor-core forms (fp16 hi+lo, fp32 accumulate) of steps 3-5; ragged tiles, k-steps, blocks.
-    Nt >= ~100: V = sum e^{2i th} takes one fp16 pass, so |dP|/P ~ 4e-4 / sqrt(Nt)."""
-    pkg, h = lsp
-    w = workloads.c1(Nt=Nt, Nf=Nf, seed=4000 + Nt)
-    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=rec, nsplit=nsplit, coarse=128 if rec == 5 else 0)
-    _check(P, ref, "rec=%d Nt=%d Nf=%d" % (rec, Nt, Nf))
-    assert int(np.argmax(P)) == oracle.argmax(ref)
-    plan = h.last_plan()
-    assert plan["recurrence"] == rec and "mma" in plan["kernel"]
-
-
-@pytest.mark.parametrize("Nt,Nf,nsplit,flush", [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 50011, 0, 0), (1025, 8193, 2, 0),
-                                                (127, 40, 0, 0), (130, 16385, 1, 0), (4099, 3001, 1, 16), (4099, 3001, 2, 1000),
-                                                (8, 100, 1, 0), (137, 33000, 1, 0)])
-@pytest.mark.parametrize("corr", [1, 2, 3, 4])
-def test_umma_table_form_ragged(lsp, Nt, Nf, nsplit, flush, corr):
-    """rec = 5 with the coarse operand streamed from the pre-computed table (cp.async.bulk), two k-steps per stage:
-    odd k-step counts, ragged tiles and blocks, several drains.  corr = 1: the hi*lo correction products as two fp16
-    MMAs; corr = 2: as one e5m2 MMA of K = 32; corr = 3: the same on CTA pairs (cta_group::2, M = 256, each CTA
-    holding half of the coarse operand; odd block counts get one masked block); corr = 4 (the default form): CTA pairs that share
-    the GENERATED operand (k = kb + 256 h + l, 64 generated coarse values per CTA, fine table of 256 rows)."""
+@pytest.mark.parametrize("Nt,Nf,nsplit,flush", RAGGED)
+@pytest.mark.parametrize("table_mb", [0, 1])
+def test_pair_form_ragged(lsp, Nt, Nf, nsplit, flush, table_mb):
+    """The CTA-pair tcgen05 form (fine operand streamed from the table by cp.async.bulk, coarse operand generated and shared by
+    the pair; k = kb + 256 h + l): odd k-step counts, ragged tiles and blocks (odd block counts get one masked block), several
+    drains.  table_mb = 1: the table may take 1 MiB only, so every series longer than 256 samples runs in TIME CHUNKS
+    (table pre-pass + accumulate launch per chunk, later chunks fold into the workspace) -- same result."""
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=6000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    pair = {3: 2, 4: 3}.get(corr, 1)
-    corr = min(corr, 2)
-    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=2, coarse=128, corr=corr, pair=pair)
+    P = _run_single(h, w, pipe=TENSOR, nsplit=nsplit, flush=flush, coarse=128, table_mb=table_mb)
     if Nt >= 100:
-        _check(P, ref, "umma-tab Nt=%d Nf=%d" % (Nt, Nf))
-        assert _same_peak(P, ref)
+        _check(P, ref, "pair form Nt=%d Nf=%d" % (Nt, Nf))
+        assert _same_peak(P, ref, "pair form Nt=%d" % Nt)
     else:                                                  # tiny Nt: single fp16 pass of V limits |dP|/P to ~4e-4/sqrt(Nt)
         assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
     plan = h.last_plan()
-    assert plan["recurrence"] == 5 and "table" in plan["kernel"] and plan["launches"] == (4 if Nt <= 4096 else 5)   # one-block series: step 1 fused into the records kernel
-    assert ("e5m2corr" in plan["kernel"]) == (corr == 2)
-    assert ("cta_group2" in plan["kernel"]) == (pair >= 2) and ("pair2" in plan["kernel"]) == (pair == 3)
+    nchunks = 1 if not table_mb else -(-Nt // 256)
+    assert plan["pipe"] == TENSOR and "pair2" in plan["kernel"] and plan["K"] == 128
+    assert plan["launches"] == (2 if Nt <= 4096 else 3) + 2 * nchunks   # one-block series: step 1 fused into the records kernel
 
 
-@pytest.mark.parametrize("corr", [1, 2, 3, 4])
-def test_umma_table_form_noise_and_scale(lsp, corr):
-    """The table form on pure noise (max P ~ 8: the tightest absolute tolerance) and badly scaled x.  With the 8-bit
+def test_pair_form_time_chunks_are_bit_identical_run_to_run_and_close_to_unchunked(lsp):
+    """A chunked call is deterministic (fixed order of chunks, read-modify-write of one owner per workspace element) and differs
+    from the unchunked call only by fp32 rounding of where the partial sums are cut."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=20011, Nf=70001, seed=515)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    one = _run_single(h, w, pipe=TENSOR, coarse=128)
+    assert h.last_plan()["launches"] == 3 + 2
+    a = _run_single(h, w, pipe=TENSOR, coarse=128, table_mb=16)        # 16 MiB / 3 KB = 5,461 -> 4 chunks of 5,120 (last: 4,651)
+    assert h.last_plan()["launches"] == 3 + 2 * 4
+    b = _run_single(h, w, pipe=TENSOR, coarse=128, table_mb=16)
+    assert np.array_equal(a, b)
+    _check(one, ref, "unchunked"); _check(a, ref, "4 chunks")
+    assert np.max(np.abs(a - one)) <= 2e-5 * ref.max()
+    assert int(np.argmax(a)) == oracle.argmax(ref) == int(np.argmax(one))
+
+
+def test_pair_form_noise_and_scale(lsp):
+    """The pair form on pure noise (max P ~ 8: the tightest absolute tolerance) and badly scaled x.  With the 8-bit
     correction MMA the residual is ~2^-15 per product, measured 1.4e-5 ... 3.5e-5 of max P here."""
     pkg, h = lsp
-    wb = workloads.c4(B=4, Nt=3000, Nf=9000, seed=4242)
     for b, scale in enumerate((1.0, 1e-6, 1e6, 1.0)):
-        x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
-        w = workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
-        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-        P = _run_single(h, w, rec=5, btable=2, coarse=128, corr=min(corr, 2), pair={3: 2, 4: 3}.get(corr, 1))
-        _check(P, ref, "umma-tab corr=%d noise scale=%g" % (corr, scale))
-        assert _same_peak(P, ref)
+        def make(seed, b=b, scale=scale):
+            wb = workloads.c4(B=4, Nt=3000, Nf=9000, seed=seed)
+            x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
+            return workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
+        w, ref = _qualified(make, 4242)
+        P = _run_single(h, w, pipe=TENSOR, coarse=128)
+        print("pair form, noise, scale %g: max|dP|/max P = %.2e" % (scale, _check(P, ref, "pair form noise scale=%g" % scale)))
+        assert _same_peak(P, ref, "pair noise")
 
 
 @pytest.mark.parametrize("coarse", [16, 32, 64])
 @pytest.mark.parametrize("Nt,Nf,nsplit,flush", [(2731, 1777, 0, 0), (2731, 1777, 3, 0), (5000, 20011, 0, 0), (1025, 8193, 2, 0),
                                                 (127, 40, 0, 0), (130, 16385, 1, 0), (4099, 3001, 1, 16), (4099, 3001, 2, 1000),
                                                 (8, 100, 1, 0), (1000, 2000, 1, 0)])
-def test_umma_small_form_ragged(lsp, Nt, Nf, nsplit, flush, coarse):
-    """rec = 5 with a narrow coarse extent (128 x L frequencies per CTA, MMA N = 2L, two CTAs per SM):
+def test_small_form_ragged(lsp, Nt, Nf, nsplit, flush, coarse):
+    """The tcgen05 form with a narrow coarse extent (128 x L frequencies per CTA, MMA N = 2L, two or three CTAs per SM):
     ragged tiles, k-steps and frequency blocks, several drains, every L."""
     pkg, h = lsp
     w = workloads.c1(Nt=Nt, Nf=Nf, seed=7000 + Nt)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-    P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, coarse=coarse)
+    P = _run_single(h, w, pipe=TENSOR, nsplit=nsplit, flush=flush, coarse=coarse)
     if Nt >= 100:
-        _check(P, ref, "umma-small L=%d Nt=%d Nf=%d" % (coarse, Nt, Nf))
+        _check(P, ref, "small form L=%d Nt=%d Nf=%d" % (coarse, Nt, Nf))
         if Nt >= 512:                                      # below the automatic form's threshold (PLAN_TC_MIN_NT) only the tolerance is promised
-            assert _same_peak(P, ref)
+            assert _same_peak(P, ref, "small form")
     else:                                                  # tiny Nt: single fp16 pass of V limits |dP|/P to ~4e-4/sqrt(Nt)
         assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
     plan = h.last_plan()
-    assert plan["recurrence"] == 5 and plan["K"] == coarse and "small" in plan["kernel"]
+    assert plan["pipe"] == TENSOR and plan["K"] == coarse and "small" in plan["kernel"]
     assert plan["n_freq_blocks"] == -(-Nf // (128 * coarse))
 
 
 @pytest.mark.parametrize("coarse", [16, 32, 64])
-def test_umma_small_form_batched_noise(lsp, coarse):
-    """Batched pure noise (the tightest tolerance) through the narrow tcgen05 tiles, with per-series peaks."""
-    import torch
+def test_small_and_duo_forms_batched_noise(lsp, coarse):
+    """Batched pure noise (the tightest tolerance) through the narrow tcgen05 tiles (L = 16 on a batch: two series per CTA),
+    with per-series peaks."""
     pkg, h = lsp
-    w = workloads.c4(B=37, Nt=1000, Nf=2000, seed=4747)
-    Pref, iref, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
-    h.set_param(pkg.PARAM_RECURRENCE, 5); h.set_param(pkg.PARAM_COARSE, coarse)
-    try:
-        t, x = _dev(w)
-        P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
-        torch.cuda.synchronize()
-        assert h.last_plan()["K"] == coarse
-    finally:
-        h.set_param(pkg.PARAM_RECURRENCE, 0); h.set_param(pkg.PARAM_COARSE, 0)
+    w, Pref = _qualified(lambda s: workloads.c4(B=37, Nt=1000, Nf=2000, seed=s), 4747)
+    iref = np.array([oracle.argmax(Pref[b]) for b in range(w.B)])
+    P, pi, pv, plan = _run_batched(h, w, pipe=TENSOR, coarse=coarse)
+    assert plan["K"] == coarse and (("duo" in plan["kernel"]) == (coarse == 16))
     for b in range(w.B):
-        _check(P[b].cpu().numpy(), Pref[b], "umma-small L=%d series %d" % (coarse, b))
-    assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
+        _check(P[b], Pref[b], "L=%d series %d" % (coarse, b))
+    assert np.array_equal(pi, iref.astype(np.int32))
 
 
 @pytest.mark.parametrize("flush", [8, 64, 1000, 4096])
-def test_umma_drain_intervals(lsp, flush):
-    """rec = 5: D_W is drained from TMEM every `flush` samples (store first, then read-modify-write)."""
+@pytest.mark.parametrize("coarse", [64, 128])
+def test_drain_intervals(lsp, flush, coarse):
+    """Tensor forms: D_W is drained from TMEM every `flush` samples (store first, then read-modify-write)."""
     pkg, h = lsp
     w = workloads.c1(Nt=4099, Nf=3001, seed=5005)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
     for nsplit in (1, 2):
-        P = _run_single(h, w, rec=5, nsplit=nsplit, flush=flush, btable=1, coarse=128)
-        _check(P, ref, "umma flush=%d nsplit=%d" % (flush, nsplit))
+        P = _run_single(h, w, pipe=TENSOR, nsplit=nsplit, flush=flush, coarse=coarse)
+        _check(P, ref, "flush=%d nsplit=%d L=%d" % (flush, nsplit, coarse))
         assert int(np.argmax(P)) == oracle.argmax(ref)
 
 
-@pytest.mark.parametrize("rec", TC_FORMS)
-def test_tensor_core_form_noise_and_scale(lsp, rec):
-    """Pure noise (the tightest tolerance: max P ~ 10) and badly scaled x (1e-6 and 1e+6): the fp16 split must hold."""
+def test_tensor_form_batched_with_table(lsp):
+    """The CTA-pair form on a batch: one fine-operand table per series, or ONE table for all when the times are shared
+    (t_stride = 0); 40,000 frequencies = 2 pairs."""
     pkg, h = lsp
-    wb = workloads.c4(B=3, Nt=3000, Nf=9000, seed=4242)
-    for b, scale in enumerate((1.0, 1e-6, 1e6)):
-        x = (wb.x[b].astype(np.float64) * scale + 3.0 * scale).astype(np.float32)
-        w = workloads.Workload("noise", wb.t[b], x, wb.f_min, wb.df, wb.Nf)
-        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
-        P = _run_single(h, w, rec=rec)
-        _check(P, ref, "rec=%d noise scale=%g" % (rec, scale))
-        assert int(np.argmax(P)) == oracle.argmax(ref)
-
-
-@pytest.mark.parametrize("rec", TC_FORMS)
-def test_tensor_core_form_batched(lsp, rec):
-    import torch
-    pkg, h = lsp
-    w = workloads.c4(B=5, Nt=900, Nf=2100, seed=4343)
-    Pref, iref, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
-    h.set_param(pkg.PARAM_RECURRENCE, rec)
-    try:
-        t, x = _dev(w)
-        P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
-        torch.cuda.synchronize()
-    finally:
-        h.set_param(pkg.PARAM_RECURRENCE, 0)
-    for b in range(w.B):
-        _check(P[b].cpu().numpy(), Pref[b], "mma series %d" % b)
-    assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
+    w, Pref = _qualified(lambda s: workloads.c4(B=3, Nt=1500, Nf=40000, seed=s), 31337)
+    for shared in (False, True):
+        ref = Pref if not shared else oracle.periodogram_batched(w.t[0], w.x, w.f_min, w.df, w.Nf)[0]
+        P, pi, pv, plan = _run_batched(h, w, shared_t=shared, pipe=TENSOR, coarse=128, table_mb=(0 if shared else 4))
+        assert "pair2" in plan["kernel"]
+        for b in range(w.B):
+            _check(P[b], ref[b], "pair form batch, series %d" % b)
+            if not shared:
+                assert _same_peak(P[b], ref[b], "pair form batch")
+        assert np.array_equal(pi, P.argmax(axis=1).astype(np.int32))
 
 
 @pytest.mark.parametrize("Nt,Nf", [(2, 1), (3, 7), (511, 33), (512, 128), (513, 129), (1025, 4097)])
@@ -265,9 +300,61 @@ def test_f_zero_and_large_time_offset(lsp):
     w = workloads.c1(Nt=1500, Nf=900, seed=77)
     w0 = workloads.Workload("f0", w.t + 2455000.25, w.x, 0.0, w.df, w.Nf)
     ref = oracle.periodogram(w0.t, w0.x, w0.f_min, w0.df, w0.Nf)
-    P = _run_single(h, w0)
-    _check(P, ref, "f_min=0, t+2455000")
-    assert abs(P[0]) <= TOL * ref.max()
+    for pipe in (0, FP32):
+        P = _run_single(h, w0, pipe=pipe)
+        _check(P, ref, "f_min=0, t+2455000")
+        assert abs(P[0]) <= TOL * ref.max()
+
+
+# ------------------------------------------------------------------ reading G7 on the GPU: even sampling, f = 0 and the exact Nyquist bin
+def _even(Nt, seed, B=1):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    dt = 0.25
+    t = dt * np.arange(Nt, dtype=np.float64)
+    x = (0.8 * np.sin(2 * np.pi * 0.37 * t)[None, :] + rng.normal(0.0, 1.0, (B, Nt))).astype(np.float32)
+    f_ny = 1.0 / (2 * dt)
+    return t, x, f_ny
+
+
+@pytest.mark.parametrize("prm", [dict(pipe=FP32), dict(pipe=TENSOR, coarse=128), dict(pipe=TENSOR, coarse=16), dict(pipe=TENSOR, coarse=64)])
+def test_G7_even_sampling_zero_frequency_and_exact_nyquist(lsp, prm):
+    """Even sampling t_j = j dt on a grid that starts at f = 0 and ends EXACTLY at the Nyquist frequency 1/(2 dt): there
+    sin(w t_j) = 0 for every sample, SS = 0 and the second term of eq. (1) is 0/0 (reading G7: dropped, on both sides);
+    just below it Nt - R is small but not zero.  Through the FP32 form and every tensor form, against the oracle's values."""
+    pkg, h = lsp
+    Nt = 2048
+    t, x, f_ny = _even(Nt, 99)
+    Nf = 4097                                              # df = f_ny / 4096: bins 0 .. 4096, the last one exactly Nyquist
+    w = workloads.Workload("even", t, x[0], 0.0, f_ny / (Nf - 1), Nf)
+    assert w.f_min + (Nf - 1) * w.df == f_ny
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P = _run_single(h, w, **prm)
+    _check(P, ref, "even sampling %r" % (prm,))
+    bound = TOL * ref.max()
+    assert abs(P[0] - ref[0]) <= bound and abs(P[-1] - ref[-1]) <= bound and np.all(np.abs(P[-8:] - ref[-8:]) <= bound)
+    assert ref[-1] > 0.05                                  # the Nyquist bin is not trivially zero for this input
+    assert int(np.argmax(P)) == oracle.argmax(ref)
+
+
+def test_G7_even_sampling_batch_paths(lsp):
+    """The same grid through the batch kernels: two series per CTA (fused steps 6-7) and the shared-time GEMM (its
+    per-frequency constants 1/(Nt - R) carry the G7 branch)."""
+    pkg, h = lsp
+    Nt, B = 1024, 20
+    t, x, f_ny = _even(Nt, 100, B=B)
+    Nf = 2049
+    df = f_ny / (Nf - 1)
+    tb = np.broadcast_to(t, (B, Nt)).copy()
+    w = workloads.Workload("evenB", tb, x, 0.0, df, Nf, B=B)
+    Pref = oracle.periodogram_batched(t, x, 0.0, df, Nf)[0]
+    for shared_t, prm, tag in ((False, dict(pipe=TENSOR, coarse=16, nsplit=1), "duo"), (True, dict(shared=2), "shared_gemm"), (False, dict(pipe=FP32), "accum_z")):
+        P, pi, pv, plan = _run_batched(h, w, shared_t=shared_t, **prm)
+        assert tag in plan["kernel"]
+        for b in range(B):
+            _check(P[b], Pref[b], "%s series %d" % (tag, b))
+            bound = TOL * Pref[b].max()
+            assert abs(P[b, 0] - Pref[b, 0]) <= bound and abs(P[b, -1] - Pref[b, -1]) <= bound
+        assert np.array_equal(pi, P.argmax(axis=1).astype(np.int32))
 
 
 def test_unsorted_times_and_shift_invariance(lsp):
@@ -292,12 +379,96 @@ def test_affine_x_invariance_and_determinism(lsp):
     assert np.max(np.abs(a - c)) <= 1e-4 * a.max()
 
 
+# ------------------------------------------------------------------ adversarial inputs for the tensor forms' accumulation
+def _adv_check(h, w, ks, what, **prm):
+    """Run through the given plan; compare with the oracle on the index set ks; print the margin."""
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf, ks=ks)
+    P = _run_single(h, w, **prm)
+    assert np.all(np.isfinite(P))
+    rel = float(np.max(np.abs(P[ks].astype(np.float64) - ref)) / ref.max())
+    print("%s %r: max|dP|/max P = %.2e (%.1fx inside the tolerance); kernel %s" % (what, prm, rel, TOL / max(rel, 1e-30), h.last_plan()["kernel"]))
+    assert rel <= TOL, (what, prm, rel)
+    assert int(ks[oracle.argmax(ref)]) == int(np.argmax(P)), what
+    return rel
+
+
+@pytest.mark.parametrize("flush", [0, 4096, 8192])
+@pytest.mark.parametrize("trunc", [0, 1])
+def test_adversarial_coherent_sinusoid(lsp, flush, trunc):
+    """A noise-free sinusoid on its own grid frequency, Nt = 1e5: the accumulators grow LINEARLY for the whole of every drain
+    window and every window is biased the same way -- the worst case for the round-toward-zero accumulation of the tensor
+    cores; P_peak = (Nt - 1)/2, the largest possible value (pin P4).  Default plan (CTA-pair form).  trunc = 1 switches the
+    compensation off (ablation): at the default window the uncompensated error must ALSO be inside the tolerance -- the
+    compensation buys margin, the bound does not rest on it; at longer windows only the compensated form is required to pass."""
+    pkg, h = lsp
+    Nt, Nf = 100000, 70001
+    dt = 1.0 / 48.0
+    t = dt * np.arange(Nt, dtype=np.float64)
+    T = Nt * dt
+    k0 = 1523                                              # whole number of cycles: f0 = k0 / T is on the grid f_k = k / T
+    x = np.sin(2 * np.pi * (k0 / T) * t + 0.3).astype(np.float32)
+    w = workloads.Workload("coherent", t, x, 1.0 / T, 1.0 / T, Nf, expected_peak_bin=k0 - 1)
+    ks = np.unique(np.concatenate([np.arange(0, Nf, 64), np.arange(k0 - 1 - 200, k0 - 1 + 201), [Nf - 1]]))
+    if trunc == 1 and flush > 2048:
+        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf, ks=ks)
+        P = _run_single(h, w, flush=flush, trunc=trunc)
+        print("coherent sinusoid, NO compensation, window %d: max|dP|/max P = %.2e" % (flush, np.max(np.abs(P[ks] - ref)) / ref.max()))
+        return
+    rel = _adv_check(h, w, ks, "coherent sinusoid", flush=flush, trunc=trunc)
+    assert "pair2" in h.last_plan()["kernel"]
+    if flush == 0 and trunc == 0:
+        assert rel <= 3e-5                                 # the default configuration keeps a 3x margin here
+
+
+def test_adversarial_outlier(lsp):
+    """One sample 1e4 sigma away: after the 1/sigma scaling that sample is ~sqrt(Nt) and everything else ~1e-2 -- the fp16 hi+lo
+    split and the e5m2 cross terms see their widest dynamic range."""
+    pkg, h = lsp
+    w0 = workloads.c1(Nt=20000, Nf=40001, seed=4141)
+    x = w0.x.copy(); x[7777] += 1e4 * float(np.std(x))
+    w = workloads.Workload("outlier", w0.t, x, w0.f_min, w0.df, w0.Nf)
+    ks = np.unique(np.concatenate([np.arange(0, w.Nf, 16), [w.Nf - 1]]))
+    for prm in (dict(), dict(pipe=FP32), dict(pipe=TENSOR, coarse=64)):
+        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf, ks=ks)
+        P = _run_single(h, w, **prm)
+        rel = float(np.max(np.abs(P[ks] - ref)) / ref.max())
+        print("outlier %r: max|dP|/max P = %.2e; kernel %s" % (prm, rel, h.last_plan()["kernel"]))
+        assert rel <= TOL
+
+
+@pytest.mark.parametrize("Nt", [512, 513, 600])
+def test_adversarial_short_noise_at_the_tensor_threshold(lsp, Nt):
+    """Pure noise with Nt just above PLAN_TC_MIN_NT = 512, where the single fp16 pass of V = sum e^{2i theta} is coarsest
+    (|dP|/P ~ 4e-4 / sqrt(Nt)) and max P ~ 8 makes the absolute tolerance tightest.  Default plan."""
+    pkg, h = lsp
+    def make(seed):
+        wb = workloads.c4(B=1, Nt=Nt, Nf=3001, seed=seed)
+        return workloads.Workload("short-noise", wb.t[0], wb.x[0], wb.f_min, wb.df, wb.Nf)
+    w, ref = _qualified(make, 5100 + Nt)
+    rel = _adv_check(h, w, np.arange(w.Nf), "short noise Nt=%d" % Nt)
+    assert h.last_plan()["pipe"] == TENSOR
+
+
+def test_adversarial_huge_phase(lsp):
+    """f t up to 1e7 cycles (a 1e4-day span at 1,000 cycles/day, on Julian-date-sized times): the exact 64-bit fixed-point
+    phases (reading G3) against the oracle's libm reduction of 2 pi f t ~ 6e7 rad."""
+    pkg, h = lsp
+    rng = np.random.Generator(np.random.PCG64(6060))
+    Nt, Nf = 3000, 5001
+    t = 2455000.5 + np.sort(rng.uniform(0.0, 1e4, Nt))
+    f_inj = 999.4321
+    x = (np.sin(2 * np.pi * f_inj * (t - 2455000.5)) + rng.normal(0.0, 1.0, Nt)).astype(np.float32)
+    w = workloads.Workload("huge-phase", t, x, 999.0, 1.0 / (Nf - 1), Nf)
+    for prm in (dict(), dict(pipe=FP32), dict(pipe=TENSOR, coarse=128)):
+        _adv_check(h, w, np.arange(Nf), "f t ~ 1e7 cycles", **prm)
+
+
 # ------------------------------------------------------------------ batched path
 def test_batched_small_full_parity(lsp):
     import torch
     pkg, h = lsp
-    w = workloads.c4(B=24, Nt=777, Nf=1501, seed=4321)
-    Pref, iref, vref = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
+    w, Pref = _qualified(lambda s: workloads.c4(B=24, Nt=777, Nf=1501, seed=s), 4321)
+    iref = np.array([oracle.argmax(Pref[b]) for b in range(w.B)])
     t, x = _dev(w)
     P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
     torch.cuda.synchronize()
@@ -313,71 +484,39 @@ def test_batched_small_full_parity(lsp):
 
 
 def test_batched_shared_times(lsp):
-    import torch
     pkg, h = lsp
-    w = workloads.c4(B=6, Nt=600, Nf=700, seed=999)
-    t_shared = w.t[0].copy()
-    Pref, iref, _ = oracle.periodogram_batched(t_shared, w.x, w.f_min, w.df, w.Nf)
-    t = torch.from_numpy(t_shared).cuda()
-    x = torch.from_numpy(w.x).cuda()
-    P, pi, pv = h.periodogram_batched(t, x, w.f_min, w.df, w.Nf)
-    torch.cuda.synchronize()
+    def make(seed):
+        w = workloads.c4(B=6, Nt=600, Nf=700, seed=seed)
+        return workloads.Workload("c4-shared", np.broadcast_to(w.t[0], w.t.shape).copy(), w.x, w.f_min, w.df, w.Nf, B=w.B)
+    w, Pref = _qualified(make, 999)
+    P, pi, pv, plan = _run_batched(h, w, shared_t=True)
     for b in range(w.B):
-        _check(P[b].cpu().numpy(), Pref[b], "shared-t series %d" % b)
-    assert np.array_equal(pi.cpu().numpy(), iref.astype(np.int32))
-
-
-@pytest.mark.parametrize("shared", [False, True])
-@pytest.mark.parametrize("pair", [1, 2, 3])
-def test_batched_table_form(lsp, shared, pair):
-    """The tcgen05 table form on a batch: one coarse-operand table per series, or ONE table for all when the
-    times are shared (t_stride = 0); 3 frequency blocks (pairs: padded to 4, the last one masked)."""
-    import torch
-    pkg, h = lsp
-    w = workloads.c4(B=3, Nt=1500, Nf=40000, seed=31337)
-    tt = w.t[0].copy() if shared else w.t
-    Pref, iref, _ = oracle.periodogram_batched(tt, w.x, w.f_min, w.df, w.Nf)
-    keys = {pkg.PARAM_RECURRENCE: 5, pkg.PARAM_BTABLE: 2, pkg.PARAM_COARSE: 128, pkg.PARAM_PAIR: pair}
-    for k, v in keys.items():
-        h.set_param(k, v)
-    try:
-        P, pi, pv = h.periodogram_batched(torch.from_numpy(tt).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf)
-        torch.cuda.synchronize()
-        assert ("cta_group2" in h.last_plan()["kernel"]) == (pair >= 2)
-    finally:
-        for k in keys:
-            h.set_param(k, 0)
-    for b in range(w.B):
-        _check(P[b].cpu().numpy(), Pref[b], "table form, series %d" % b)
-        assert _same_peak(P[b].cpu().numpy(), Pref[b])
+        _check(P[b], Pref[b], "shared-t series %d" % b)
+    assert np.array_equal(pi, np.array([oracle.argmax(Pref[b]) for b in range(w.B)], dtype=np.int32))
 
 
 @pytest.mark.parametrize("B,Nt,Nf", [(20, 1500, 3000), (130, 700, 777), (5, 5000, 1001), (33, 2049, 130), (2, 17, 9)])
 def test_shared_time_gemm(lsp, B, Nt, Nf):
     """t_stride = 0 through the dense-contraction path (lsp_shared_gemm.cuh): ragged series /
     frequency / sample counts, one to three time splits, against the oracle series by series; and against the generic path."""
-    import torch
     pkg, h = lsp
-    w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=100 + B)
-    tt = w.t[0].copy()
-    Pref, iref, _ = oracle.periodogram_batched(tt, w.x, w.f_min, w.df, w.Nf)
+    def make(seed):
+        w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=seed)
+        return workloads.Workload("c4-shared", np.broadcast_to(w.t[0], w.t.shape).copy(), w.x, w.f_min, w.df, w.Nf, B=w.B)
+    w, Pref = _qualified(make, 100 + B)
     out = {}
     for shared in (1, 2):
-        h.set_param(pkg.PARAM_SHARED, shared)
-        try:
-            P, pi, pv = h.periodogram_batched(torch.from_numpy(tt).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf)
-            torch.cuda.synchronize()
-            assert ("shared_gemm" in h.last_plan()["kernel"]) == (shared == 2)
-        finally:
-            h.set_param(pkg.PARAM_SHARED, 0)
-        out[shared] = P.cpu().numpy()
+        P, pi, pv, plan = _run_batched(h, w, shared_t=True, shared=shared)
+        assert ("shared_gemm" in plan["kernel"]) == (shared == 2)
+        out[shared] = P
         if shared == 2:
-            assert np.array_equal(pv.cpu().numpy(), out[2].max(axis=1)) and np.array_equal(pi.cpu().numpy(), out[2].argmax(axis=1))
-    tol = TOL if Nt >= 100 else 1e-3                       # tiny Nt: fp16 V in the generic path (see test_umma_table_form_ragged)
+            assert np.array_equal(pv, P.max(axis=1)) and np.array_equal(pi, P.argmax(axis=1))
+    tol = TOL if Nt >= 100 else 1e-3                       # tiny Nt: fp16 V in the generic path (see test_pair_form_ragged)
     for b in range(B):
         for shared in (1, 2):
             assert np.max(np.abs(out[shared][b] - Pref[b])) <= tol * Pref[b].max(), "series %d shared=%d" % (b, shared)
-        assert _same_peak(out[2][b], Pref[b])
+        if Nt >= 100:
+            assert _same_peak(out[2][b], Pref[b], "shared gemm")
 
 
 @pytest.mark.parametrize("B,Nt,Nf,nsplit", [(5, 900, 2100, 0), (2, 1500, 2000, 0), (7, 3000, 5000, 2), (3, 600, 700, 0)])
@@ -386,102 +525,76 @@ def test_two_series_per_cta_form(lsp, B, Nt, Nf, nsplit, gls):
     """accum_umma_duo_kernel: two series x 64 fine x 32 coarse per CTA (the batch form of the 2,048-frequency tile);
     odd B (the last CTA's second series does not exist), several frequency blocks and time splits, and the unit-weight
     second pass of the generalised periodogram."""
-    import torch
     pkg, h = lsp
-    w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=300 + B)
+    fn = None
     if gls:
-        Pref = np.stack([oracle.periodogram_gls(w.t[b], w.x[b], w.f_min, w.df, w.Nf) for b in range(B)])
-    else:
-        Pref, _, _ = oracle.periodogram_batched(w.t, w.x, w.f_min, w.df, w.Nf)
-    keys = {pkg.PARAM_DUO: 2, pkg.PARAM_RECURRENCE: 5, pkg.PARAM_COARSE: 16, pkg.PARAM_NSPLIT: nsplit}
-    for k, v in keys.items():
-        h.set_param(k, v)
-    try:
-        P, pi, pv = h.periodogram_batched(torch.from_numpy(w.t).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf, gls=gls)
-        torch.cuda.synchronize()
-        assert "duo" in h.last_plan()["kernel"]
-    finally:
-        for k in keys:
-            h.set_param(k, 0)
-    P = P.cpu().numpy()
+        fn = lambda w: np.stack([oracle.periodogram_gls(w.t[b], w.x[b], w.f_min, w.df, w.Nf) for b in range(w.B)])
+    w, Pref = _qualified(lambda s: workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=s), 300 + B, ref_fn=fn)
+    P, pi, pv, plan = _run_batched(h, w, gls=gls, pipe=TENSOR, coarse=16, nsplit=nsplit)
+    assert "duo" in plan["kernel"]
     for b in range(B):
         _check(P[b], Pref[b], "duo series %d" % b)
-        assert _same_peak(P[b], Pref[b])
-    assert np.array_equal(pi.cpu().numpy(), P.argmax(axis=1).astype(np.int32))
+        assert _same_peak(P[b], Pref[b], "duo")
+    assert np.array_equal(pi, P.argmax(axis=1).astype(np.int32))
 
 
 @pytest.mark.parametrize("shared", [False, True])
 def test_batched_peaks_only(lsp, shared):
     """P = NULL: only the per-series peaks are wanted (fused steps 6-7 of the two-series kernel and of the shared-time GEMM)."""
-    import torch
     pkg, h = lsp
     w = workloads.c4(B=37, Nt=1000, Nf=2000, seed=808)
-    tt = torch.from_numpy(w.t[0].copy() if shared else w.t).cuda()
-    xx = torch.from_numpy(w.x).cuda()
-    h.set_param(pkg.PARAM_NSPLIT, 1)                       # one time split: the fused epilogues apply
-    try:
-        P, pi, pv = h.periodogram_batched(tt, xx, w.f_min, w.df, w.Nf)
-        name = h.last_plan()["kernel"]
-        assert "fused-finish" in name and (("shared_gemm" in name) == shared)
-        P0, pi0, pv0 = h.periodogram_batched(tt, xx, w.f_min, w.df, w.Nf, want_P=False)
-        torch.cuda.synchronize()
-    finally:
-        h.set_param(pkg.PARAM_NSPLIT, 0)
+    P, pi, pv, plan = _run_batched(h, w, shared_t=shared, nsplit=1)       # one time split: the fused epilogues apply
+    assert "fused-finish" in plan["kernel"] and (("shared_gemm" in plan["kernel"]) == shared)
+    P0, pi0, pv0, _ = _run_batched(h, w, shared_t=shared, nsplit=1, want_P=False)
     assert P0 is None
-    assert torch.equal(pi, pi0) and torch.equal(pv, pv0)
-    assert torch.equal(pi.cpu(), P.argmax(dim=1).to(torch.int32).cpu()) and torch.equal(pv.cpu(), P.max(dim=1).values.cpu())
+    assert np.array_equal(pi, pi0) and np.array_equal(pv, pv0)
+    assert np.array_equal(pi, P.argmax(axis=1).astype(np.int32)) and np.array_equal(pv, P.max(axis=1))
 
 
 def test_cuda_graph_capture_and_replay(lsp):
-    """The device-pointer entry points only enqueue on the caller's stream (no allocation once the workspace exists, no
-    synchronisation): a call can be captured into a CUDA graph and replayed; the replay is bit-identical to the eager call."""
+    """The device-pointer entry points only enqueue on the caller's stream (no allocation once the workspace exists -- lsp_reserve
+    sizes it --, no synchronisation): a call can be captured into a CUDA graph and replayed; the replay is bit-identical to the
+    eager call.  A fresh handle: the workspace comes from lsp_reserve alone."""
     import torch
-    pkg, h = lsp
+    pkg, _ = lsp
     w = workloads.c1()
     t, x = _dev(w)
     P = torch.empty(w.Nf, dtype=torch.float32, device="cuda")
-    for _ in range(2):
-        h.periodogram(t, x, w.f_min, w.df, w.Nf, out=P)             # sizes the workspace
-    torch.cuda.synchronize()
-    ref = P.clone()
-    g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
-    with torch.cuda.stream(s):
-        h.periodogram(t, x, w.f_min, w.df, w.Nf, out=P)
+    with pkg.Handle(0) as h:
+        h.reserve(1, w.Nt, w.Nf)
+        g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            torch.cuda.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                h.periodogram(t, x, w.f_min, w.df, w.Nf, out=P)       # first call of this handle: captured, not run
+        ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+        first = None
+        for _ in range(3):
+            P.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            first = P.clone() if first is None else first
+            assert torch.equal(P, first)
+        _check(P.cpu().numpy(), ref, "graph replay")
+        eager = h.periodogram(t, x, w.f_min, w.df, w.Nf)
         torch.cuda.synchronize()
-        with torch.cuda.graph(g, stream=s):
-            h.periodogram(t, x, w.f_min, w.df, w.Nf, out=P)
-    for _ in range(3):
-        P.zero_()
-        g.replay()
-        torch.cuda.synchronize()
-        assert torch.equal(P, ref)
-    _check(P.cpu().numpy(), oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf), "graph replay")
+        assert torch.equal(eager, first)
 
 
 @pytest.mark.parametrize("B,Nt,Nf,shared,prm", [
-    (2, 2, 1, True, {"SHARED": 2}), (3, 5, 3, True, {"SHARED": 2}), (2, 33, 129, True, {"SHARED": 2}), (129, 40, 5, True, {"SHARED": 2}),
-    (2, 2, 1, False, {"RECURRENCE": 5, "COARSE": 16}), (3, 9, 2049, False, {"RECURRENCE": 5, "COARSE": 16}),
-    (5, 130, 4097, False, {"RECURRENCE": 5, "COARSE": 16, "NSPLIT": 3})])
+    (2, 2, 1, True, {"shared": 2}), (3, 5, 3, True, {"shared": 2}), (2, 33, 129, True, {"shared": 2}), (129, 40, 5, True, {"shared": 2}),
+    (2, 2, 1, False, {"pipe": TENSOR, "coarse": 16}), (3, 9, 2049, False, {"pipe": TENSOR, "coarse": 16}),
+    (5, 130, 4097, False, {"pipe": TENSOR, "coarse": 16, "nsplit": 3})])
 def test_batch_paths_degenerate_sizes(lsp, B, Nt, Nf, shared, prm):
     """The two batch kernels forced onto degenerate sizes (Nt = 2, Nf = 1, one sample more than a tile, more series than a tile):
     finite, peaks consistent, and within tolerance (1e-3 where a forced tensor form keeps V in fp16 with Nt < 100)."""
-    import torch
     pkg, h = lsp
     w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=900 + Nt)
     tt = w.t[0].copy() if shared else w.t
     Pref, _, _ = oracle.periodogram_batched(tt, w.x, w.f_min, w.df, w.Nf)
-    for k, v in prm.items():
-        h.set_param(getattr(pkg, "PARAM_" + k), v)
-    try:
-        P, pi, pv = h.periodogram_batched(torch.from_numpy(tt).cuda(), torch.from_numpy(w.x).cuda(), w.f_min, w.df, w.Nf)
-        torch.cuda.synchronize()
-        name = h.last_plan()["kernel"]
-    finally:
-        for k in prm:
-            h.set_param(getattr(pkg, "PARAM_" + k), 0)
-    assert ("shared_gemm" in name) if shared else ("duo" in name)
-    P = P.cpu().numpy()
-    assert np.all(np.isfinite(P)) and np.array_equal(pi.cpu().numpy(), P.argmax(axis=1).astype(np.int32))
+    P, pi, pv, plan = _run_batched(h, w, shared_t=shared, **prm)
+    assert ("shared_gemm" in plan["kernel"]) if shared else ("duo" in plan["kernel"])
+    assert np.all(np.isfinite(P)) and np.array_equal(pi, P.argmax(axis=1).astype(np.int32))
     tol = TOL if (shared or Nt >= 100) else 1e-3
     for b in range(B):
         assert np.max(np.abs(P[b] - Pref[b])) <= tol * max(Pref[b].max(), 1e-30), "series %d" % b
@@ -509,23 +622,23 @@ def test_host_entry_points(lsp):
     P = torch.empty(w.Nf, dtype=torch.float32).pin_memory()
     h.periodogram_host(t, x, w.f_min, w.df, w.Nf, out=P)
     _check(P.numpy(), ref, "host single")
-    wb = workloads.c4(B=5, Nt=400, Nf=300, seed=82)
-    Pref, iref, _ = oracle.periodogram_batched(wb.t, wb.x, wb.f_min, wb.df, wb.Nf)
+    wb, Pref = _qualified(lambda s: workloads.c4(B=5, Nt=400, Nf=300, seed=s), 82)
     Pb = torch.empty((5, 300), dtype=torch.float32)
     pi = torch.empty(5, dtype=torch.int32); pv = torch.empty(5, dtype=torch.float32)
     h.periodogram_batched_host(torch.from_numpy(wb.t), torch.from_numpy(wb.x), wb.f_min, wb.df, wb.Nf,
                                P=Pb, peak_idx=pi, peak_val=pv)
     for b in range(5):
         _check(Pb[b].numpy(), Pref[b], "host batched %d" % b)
-    assert np.array_equal(pi.numpy(), iref.astype(np.int32))
+    assert np.array_equal(pi.numpy(), np.array([oracle.argmax(Pref[b]) for b in range(5)], dtype=np.int32))
 
 
-# ------------------------------------------------------------------ argument errors
-@pytest.mark.parametrize("rec,coarse", [(0, 0), (3, 0), (1, 0), (4, 0), (5, 128), (5, 32)])
-def test_generalised_periodogram(lsp, rec, coarse):
+# ------------------------------------------------------------------ generalised periodogram, false-alarm probability
+@pytest.mark.parametrize("prm", [dict(), dict(pipe=FP32), dict(pipe=TENSOR, coarse=128), dict(pipe=TENSOR, coarse=32),
+                                 dict(pipe=TENSOR, coarse=128, table_mb=2)])
+def test_generalised_periodogram(lsp, prm):
     """lsp_periodogram_gls (floating-mean fit) against the oracle's 3-parameter least squares, on
-    gappy sampling with a large offset where it differs visibly from eq. (1); every form of steps 3-5."""
-    import torch
+    gappy sampling with a large offset where it differs visibly from eq. (1); every form of steps 3-5 (the unit-weight
+    second pass reuses each chunk's table in the CTA-pair form)."""
     pkg, h = lsp
     rng = np.random.default_rng(2024)
     Nt, Nf = 3001, 4099
@@ -536,26 +649,18 @@ def test_generalised_periodogram(lsp, rec, coarse):
     ref = oracle.periodogram_gls(t, x, f_min, df, Nf)
     ls = oracle.periodogram(t, x, f_min, df, Nf)
     assert np.max(np.abs(ref - ls)) > 1e-2 * ref.max()      # the two periodograms really differ on this input
-    for key, val in ((pkg.PARAM_RECURRENCE, rec), (pkg.PARAM_COARSE, coarse)):
-        h.set_param(key, val)
-    try:
-        P = h.periodogram(torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), f_min, df, Nf, gls=True)
-        torch.cuda.synchronize()
-        plan = h.last_plan()
-    finally:
-        h.set_param(pkg.PARAM_RECURRENCE, 0); h.set_param(pkg.PARAM_COARSE, 0)
-    P = P.cpu().numpy()
-    _check(P, ref, "gls rec=%d" % rec)
-    assert _same_peak(P, ref)
-    if rec:
-        assert plan["recurrence"] == rec
+    assert _top_two_gap(ref) >= QUAL_GAP
+    w = workloads.Workload("gls", t, x, f_min, df, Nf)
+    P = _run_single(h, w, gls=True, **prm)
+    plan = h.last_plan()
+    _check(P, ref, "gls %r" % (prm,))
+    assert int(np.argmax(P)) == oracle.argmax(ref)
+    if prm.get("pipe"):
+        assert plan["pipe"] == prm["pipe"]
 
 
-@pytest.mark.parametrize("pair", [1, 2, 3])
-def test_generalised_periodogram_table_forms(lsp, pair):
-    """GLS through the table forms of the tcgen05 path (single CTA, CTA pair sharing the streamed operand, CTA pair sharing the
-    generated operand): the unit-weight second pass reuses the table and, in the default form, the truncation-compensated drain."""
-    import torch
+def test_generalised_periodogram_long_grid(lsp):
+    """GLS through the CTA-pair form on a grid of two pairs."""
     pkg, h = lsp
     rng = np.random.default_rng(77)
     Nt, Nf = 5003, 40001
@@ -563,35 +668,26 @@ def test_generalised_periodogram_table_forms(lsp, pair):
     x = (4.0 + 0.5 * np.sin(2 * np.pi * 0.0213 * t + 0.4) + 0.4 * np.sin(2 * np.pi * 2.3 * t) + rng.standard_normal(Nt)).astype(np.float32)
     f_min, df = 1.0 / 80.0, (6.0 - 1.0 / 80.0) / (Nf - 1)
     ref = oracle.periodogram_gls(t, x, f_min, df, Nf)
-    keys = {pkg.PARAM_RECURRENCE: 5, pkg.PARAM_BTABLE: 2, pkg.PARAM_COARSE: 128, pkg.PARAM_PAIR: pair}
-    for k, v in keys.items():
-        h.set_param(k, v)
-    try:
-        P = h.periodogram(torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), f_min, df, Nf, gls=True)
-        torch.cuda.synchronize()
-        name = h.last_plan()["kernel"]
-    finally:
-        for k in keys:
-            h.set_param(k, 0)
-    assert "table" in name and (("pair2" in name) == (pair == 3))
-    P = P.cpu().numpy()
-    _check(P, ref, "gls table form pair=%d" % pair)
-    assert _same_peak(P, ref)
+    assert _top_two_gap(ref) >= QUAL_GAP
+    P = _run_single(h, workloads.Workload("gls", t, x, f_min, df, Nf), gls=True, pipe=TENSOR, coarse=128)
+    assert "pair2" in h.last_plan()["kernel"]
+    _check(P, ref, "gls pair form")
+    assert int(np.argmax(P)) == oracle.argmax(ref)
 
 
 def test_generalised_periodogram_batched_and_reduction(lsp):
     """Batched GLS with per-series peaks; and on even sampling at Fourier frequencies GLS == eq. (1) (pin GP4) on the GPU."""
     import torch
     pkg, h = lsp
-    w = workloads.c4(B=9, Nt=800, Nf=1500, seed=515)
-    x = (w.x + 3.0).astype(np.float32)
-    P, pi, pv = h.periodogram_batched(torch.from_numpy(w.t).cuda(), torch.from_numpy(x).cuda(), w.f_min, w.df, w.Nf, gls=True)
-    torch.cuda.synchronize()
-    P = P.cpu().numpy()
+    def make(seed):
+        w = workloads.c4(B=9, Nt=800, Nf=1500, seed=seed)
+        return workloads.Workload("gls-batch", w.t, (w.x + 3.0).astype(np.float32), w.f_min, w.df, w.Nf, B=w.B)
+    fn = lambda w: np.stack([oracle.periodogram_gls(w.t[b], w.x[b], w.f_min, w.df, w.Nf) for b in range(w.B)])
+    w, Pref = _qualified(make, 515, ref_fn=fn)
+    P, pi, pv, plan = _run_batched(h, w, gls=True)
     for b in range(w.B):
-        ref = oracle.periodogram_gls(w.t[b], x[b], w.f_min, w.df, w.Nf)
-        _check(P[b], ref, "gls series %d" % b)
-        assert _same_peak(P[b], ref)
+        _check(P[b], Pref[b], "gls series %d" % b)
+        assert int(pi[b]) == oracle.argmax(Pref[b])
         assert int(pi[b]) == int(np.argmax(P[b])) and float(pv[b]) == float(P[b].max())
     N, dt = 1024, 0.25
     t = dt * np.arange(N)
@@ -707,5 +803,33 @@ def test_argument_errors(lsp):
     pi = torch.zeros(2, dtype=torch.int32, device="cuda")
     assert lib.lsp_periodogram_batched(H, t.data_ptr(), 5, x.data_ptr(), 5, 2, 5, 0.1, 0.1, 2,
                                        P.data_ptr(), 2, pi.data_ptr(), None, None) == pkg.LSP_EINVAL
+    # B beyond the grid limit of the pre-pass kernels is refused before anything is allocated or launched
+    assert lib.lsp_periodogram_batched(H, t.data_ptr(), 0, x.data_ptr(), 5, 65536, 5, 0.1, 0.1, 2,
+                                       None, 0, pi.data_ptr(), pi.data_ptr(), None) == pkg.LSP_EINVAL
+    for gone in (10, 12):                                 # tunables of kernel forms that no longer exist
+        assert lib.lsp_set_param(H, gone, 1) == pkg.LSP_EINVAL
+    assert lib.lsp_set_param(H, pkg.PARAM_PIPE, 3) == pkg.LSP_EINVAL
     torch.cuda.synchronize()
     assert pkg.status_string(pkg.LSP_EINVAL) == "invalid argument"
+
+
+def test_failed_growth_keeps_the_workspace(lsp):
+    """LSP_ENOMEM leaves the handle usable: lsp_reserve for a 2 TB problem fails, the next ordinary call runs on the workspace the
+    handle had (ensure() allocates the new buffer before it releases the old one)."""
+    pkg, _ = lsp
+    w = workloads.c1()
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    with pkg.Handle(0) as h:
+        a = _run_single(h, w)
+        with pytest.raises(pkg.LspError) as ei:
+            h.reserve(65535, 1000000, 1000)
+        assert ei.value.status == pkg.LSP_ENOMEM
+        b = _run_single(h, w)
+        assert np.array_equal(a, b)
+        _check(b, ref, "after ENOMEM")
+
+
+def test_zz_no_argmax_comparison_was_relaxed():
+    """Runs last in this file: every `_same_peak` above matched the oracle's index exactly (count of near-tie acceptances = 0)."""
+    print("arg-max comparisons that took the near-tie branch: %d %r" % (len(RELAXED), RELAXED))
+    assert not RELAXED

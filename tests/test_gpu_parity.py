@@ -172,7 +172,8 @@ def test_pair_form_ragged(lsp, Nt, Nf, nsplit, flush, table_mb):
     P = _run_single(h, w, pipe=TENSOR, nsplit=nsplit, flush=flush, coarse=128, table_mb=table_mb)
     if Nt >= 100:
         _check(P, ref, "pair form Nt=%d Nf=%d" % (Nt, Nf))
-        assert _same_peak(P, ref, "pair form Nt=%d" % Nt)
+        if Nt >= 512:                                      # below the automatic form's threshold (PLAN_TC_MIN_NT) only the tolerance is promised
+            assert _same_peak(P, ref, "pair form Nt=%d" % Nt)
     else:                                                  # tiny Nt: single fp16 pass of V limits |dP|/P to ~4e-4/sqrt(Nt)
         assert np.max(np.abs(P - ref)) <= 1e-3 * np.max(ref)
     plan = h.last_plan()
@@ -311,7 +312,8 @@ def _even(Nt, seed, B=1):
     rng = np.random.Generator(np.random.PCG64(seed))
     dt = 0.25
     t = dt * np.arange(Nt, dtype=np.float64)
-    x = (0.8 * np.sin(2 * np.pi * 0.37 * t)[None, :] + rng.normal(0.0, 1.0, (B, Nt))).astype(np.float32)
+    x = (0.8 * np.sin(2 * np.pi * 0.37 * t)[None, :] + 0.3 * np.cos(np.pi * np.arange(Nt))[None, :]      # a line AT the Nyquist frequency too
+         + rng.normal(0.0, 1.0, (B, Nt))).astype(np.float32)
     f_ny = 1.0 / (2 * dt)
     return t, x, f_ny
 
@@ -397,7 +399,7 @@ def _adv_check(h, w, ks, what, **prm):
 def test_adversarial_coherent_sinusoid(lsp, flush, trunc):
     """A noise-free sinusoid on its own grid frequency, Nt = 1e5: the accumulators grow LINEARLY for the whole of every drain
     window and every window is biased the same way -- the worst case for the round-toward-zero accumulation of the tensor
-    cores; P_peak = (Nt - 1)/2, the largest possible value (pin P4).  Default plan (CTA-pair form).  trunc = 1 switches the
+    cores; P_peak = (Nt - 1)/2, the largest possible value (pin P4).  CTA-pair form (the only one with the compensation).  trunc = 1 switches the
     compensation off (ablation): at the default window the uncompensated error must ALSO be inside the tolerance -- the
     compensation buys margin, the bound does not rest on it; at longer windows only the compensated form is required to pass."""
     pkg, h = lsp
@@ -411,13 +413,14 @@ def test_adversarial_coherent_sinusoid(lsp, flush, trunc):
     ks = np.unique(np.concatenate([np.arange(0, Nf, 64), np.arange(k0 - 1 - 200, k0 - 1 + 201), [Nf - 1]]))
     if trunc == 1 and flush > 2048:
         ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf, ks=ks)
-        P = _run_single(h, w, flush=flush, trunc=trunc)
+        P = _run_single(h, w, flush=flush, trunc=trunc, pipe=TENSOR, coarse=128)
         print("coherent sinusoid, NO compensation, window %d: max|dP|/max P = %.2e" % (flush, np.max(np.abs(P[ks] - ref)) / ref.max()))
         return
-    rel = _adv_check(h, w, ks, "coherent sinusoid", flush=flush, trunc=trunc)
+    rel = _adv_check(h, w, ks, "coherent sinusoid", flush=flush, trunc=trunc, pipe=TENSOR, coarse=128)
     assert "pair2" in h.last_plan()["kernel"]
     if flush == 0 and trunc == 0:
         assert rel <= 3e-5                                 # the default configuration keeps a 3x margin here
+        _adv_check(h, w, ks, "coherent sinusoid, automatic plan")   # whatever form the planner picks for this size (no compensation outside pair2)
 
 
 def test_adversarial_outlier(lsp):
@@ -743,7 +746,7 @@ def test_outputs_stay_inside_their_rows(lsp, path):
     pkg, h = lsp
     lib, H = pkg.load(), h._h
     SENT = -12345.0
-    cfg = {"pair2": (1, 3000, 70001, False, {}), "duo": (5, 900, 2001, False, {"NSPLIT": 1}),
+    cfg = {"pair2": (1, 3000, 70001, False, {"COARSE": 128}), "duo": (5, 900, 2001, False, {"NSPLIT": 1}),
            "shared": (130, 700, 777, True, {"SHARED": 2}), "generic_batch": (3, 2100, 5003, False, {})}[path]
     B, Nt, Nf, shared, prm = cfg
     w = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=4321)

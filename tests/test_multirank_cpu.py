@@ -61,6 +61,63 @@ def test_two_rank_gloo_max_time_and_aggregate():
     assert v0 == v1 == pytest.approx(2 * n0 / 15e-3)   # whole-job units / max time
 
 
+def _worker_freq(rank, world, port, q):
+    """--shard freq host logic: every rank takes its contiguous slice of ONE series' grid, finds its
+    local peak (a numpy stand-in for the device's P: this test is about slice bounds and the peak merge, not arithmetic) and the
+    ranks merge by MAXLOC, lowest index on ties."""
+    import torch.distributed as dist
+    import bench
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        Nf = 1001                                      # ragged: 501 + 500
+        k0, n = bench.freq_slice(Nf, world, rank)
+        P = np.zeros(Nf, dtype=np.float32)
+        P[[137, 700, 900]] = [5.0, 9.0, 9.0]           # the global maximum is tied between bins 700 and 900, both on rank 1
+        P[400] = 8.5                                   # rank 0's local peak
+        local = P[k0:k0 + n]
+        val, idx = bench.merge_peaks(float(local.max()), int(local.argmax()) + k0, dist)
+        # a tie ACROSS ranks: equal maxima at 300 (rank 0) and 800 (rank 1)
+        P2 = np.zeros(Nf, dtype=np.float32); P2[[300, 800]] = 4.0
+        l2 = P2[k0:k0 + n]
+        val2, idx2 = bench.merge_peaks(float(l2.max()), int(l2.argmax()) + k0, dist)
+        q.put((rank, k0, n, val, idx, val2, idx2))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_gloo_frequency_slices_and_peak_merge():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker_freq, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, k0a, na, v0, i0, w0, j0), (r1, k0b, nb, v1, i1, w1, j1) = out
+    assert (k0a, na, k0b, nb) == (0, 501, 501, 500)    # every k owned exactly once, ragged Nf
+    assert v0 == v1 == 9.0 and i0 == i1 == 700         # global MAXLOC, lowest index among equal maxima, seen by both ranks
+    assert w0 == w1 == 4.0 and j0 == j1 == 300         # tie across ranks: the lower rank's (lower) index wins
+
+
+def test_frequency_slices_cover_the_grid_once():
+    import bench
+    for Nf in (1, 7, 1000, 1000003):
+        for world in (1, 2, 3, 8):
+            seen, total = 0, 0
+            for r in range(world):
+                k0, n = bench.freq_slice(Nf, world, r)
+                assert k0 == seen and n >= 0
+                seen += n; total += n
+            assert total == Nf
+    assert bench.merge_peaks(3.0, 5, None) == (3.0, 5)
+
+
 def test_single_process_helpers():
     import bench
     assert bench.reduce_max(3.5, None) == 3.5

@@ -12,7 +12,8 @@ Nothing under paper_1007_1658_b200/ imports this package, and this package impor
 nothing from it.  Only tests/, __graft_entry__.smoke() and bench.py (cpu_baseline and
 --impl reference) may import it.  Every function cites the passage it follows.
 
-Pins: tests/test_oracle_pins.py (P1..P9 of DESIGN.md; GP1..GP5 for the generalised periodogram).
+Pins: tests/test_oracle_pins.py (P1..P9 of DESIGN.md; GP1..GP5 for the generalised periodogram, GW1..GW5 for its
+weighted form).
 No function here is "parity unpinned" (false_alarm_probability: pins F1-F3).
 """
 from __future__ import annotations
@@ -54,6 +55,11 @@ def _load():
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
         lib.lsp_oracle_gls.restype = ctypes.c_int
         lib.lsp_oracle_gls.argtypes = lib.lsp_oracle_periodogram.argtypes
+        lib.lsp_oracle_gls_weighted.restype = ctypes.c_int
+        lib.lsp_oracle_gls_weighted.argtypes = [
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+            ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
         lib.lsp_oracle_moments.restype = None
         lib.lsp_oracle_moments.argtypes = [ctypes.c_void_p, ctypes.c_int64,
                                            ctypes.c_void_p, ctypes.c_void_p]
@@ -121,6 +127,28 @@ def periodogram_gls(t, x, f_min: float, df: float, Nf: int,
     scratch = np.empty(t.size, dtype=np.float64)
     _load().lsp_oracle_gls(t.ctypes.data, x.ctypes.data, t.size, float(f_min), float(df), ks_ptr, nk,
                            P.ctypes.data, scratch.ctypes.data, int(nthreads))
+    return P
+
+
+def periodogram_gls_weighted(t, x, w, f_min: float, df: float, Nf: int,
+                             ks: Optional[np.ndarray] = None, nthreads: int = 0) -> np.ndarray:
+    """Weighted generalised periodogram (per-sample weights w_j >= 0): the weighted
+    3-parameter least-squares fit, P = (Nt - 1)/2 * (chi0^2 - chi^2_min)/chi0^2 (reading G14; see lsp_oracle.c)."""
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    w = np.ascontiguousarray(w, dtype=np.float32)
+    assert t.ndim == 1 and t.shape == x.shape == w.shape and t.size >= 4
+    assert np.all(np.isfinite(w)) and np.all(w >= 0) and w.sum() > 0
+    if ks is None:
+        nk, ks_ptr = int(Nf), None
+    else:
+        ks = np.ascontiguousarray(ks, dtype=np.int64)
+        nk, ks_ptr = int(ks.size), ks.ctypes.data
+    P = np.empty(nk, dtype=np.float64)
+    s1 = np.empty(t.size, dtype=np.float64)
+    s2 = np.empty(t.size, dtype=np.float64)
+    _load().lsp_oracle_gls_weighted(t.ctypes.data, x.ctypes.data, w.ctypes.data, t.size, float(f_min), float(df),
+                                    ks_ptr, nk, P.ctypes.data, s1.ctypes.data, s2.ctypes.data, int(nthreads))
     return P
 
 

@@ -28,7 +28,8 @@
  *
  * Parity pins (tests/test_oracle_pins.py): brute-force least squares, FFT periodogram on
  * even sampling, time-shift invariance, closed form (Nt-1)/2, scipy.signal.lombscargle,
- * Gaussian-noise statistics, injected sinusoid, eqs (5)-(8) equivalence, mpmath brute force.
+ * Gaussian-noise statistics, injected sinusoid, eqs (5)-(8) equivalence, mpmath brute force;
+ * generalised periodogram GP1-GP5, weighted generalised periodogram GW1-GW5.
  */
 #include <math.h>
 #include <stdint.h>
@@ -185,6 +186,86 @@ int lsp_oracle_gls(const double* t, const float* x, int64_t Nt,
     for (int64_t i = 0; i < nk; ++i) {
         int64_t k = ks ? ks[i] : i;
         P[i] = lsp_oracle_gls_one(t, scratch, Nt, f_min + (double)k * df, var);
+    }
+    return used;
+}
+
+/*
+ * Weighted generalised periodogram (SURVEY.md 8(f)-1 "optional weights"; the per-sample weights w_j of Zechmeister &
+ * Kuerster 2009, the extension the paper names at PAPER.md:375).  Again the DEFINITION, not their closed-form sums:
+ * for every frequency, the WEIGHTED linear least-squares fit
+ *     minimise  chi^2 = sum_j w_j (x_j - a cos(w t_j) - b sin(w t_j) - c)^2
+ * (weighted normal equations, Gaussian elimination with partial pivoting), against the weighted constant model
+ *     chi0^2 = sum_j w_j (x_j - xbar_w)^2,   xbar_w = sum w_j x_j / sum w_j,
+ * and  P = (Nt - 1)/2 * (chi0^2 - chi^2_min) / chi0^2.
+ * Reading G14: the paper gives no normalisation for the weighted case; this one is the unweighted
+ * P = (chi0^2 - chi^2_min)/(2 var), var = chi0^2/(Nt - 1), written as a chi^2 RATIO, so that w_j = const reproduces
+ * lsp_oracle_gls exactly and 0 <= P <= (Nt - 1)/2 whatever the weights.  Only the ratios of the weights matter.
+ * Weights must be finite and >= 0 with a positive sum (w_j = 0 removes sample j from the fit but not from Nt).
+ */
+static double lsp_oracle_gls_w_one(const double* t, const double* X, const double* w, int64_t Nt, double f, double chi0)
+{
+    const double om = LSP_ORACLE_TWO_PI * f;
+    double M[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};      /* [A^T W A | A^T W X] */
+    double wsum = 0.0;
+    for (int64_t j = 0; j < Nt; ++j) {
+        const double a = om * t[j];
+        const double g[3] = {cos(a), sin(a), 1.0};
+        for (int r = 0; r < 3; ++r) {
+            for (int c = 0; c < 3; ++c) M[r][c] += w[j] * g[r] * g[c];
+            M[r][3] += w[j] * g[r] * X[j];
+        }
+        wsum += w[j];
+    }
+    const double rhs[3] = {M[0][3], M[1][3], M[2][3]};
+    const double tiny = 1e-12 * wsum;
+    for (int col = 0; col < 3; ++col) {                                /* elimination, partial pivoting */
+        int piv = col;
+        for (int r = col + 1; r < 3; ++r) if (fabs(M[r][col]) > fabs(M[piv][col])) piv = r;
+        if (fabs(M[piv][col]) <= tiny) return 0.0;                      /* singular: G7 */
+        if (piv != col) for (int c = 0; c < 4; ++c) { double tmp = M[col][c]; M[col][c] = M[piv][c]; M[piv][c] = tmp; }
+        for (int r = col + 1; r < 3; ++r) {
+            const double q = M[r][col] / M[col][col];
+            for (int c = col; c < 4; ++c) M[r][c] -= q * M[col][c];
+        }
+    }
+    double beta[3];
+    for (int r = 2; r >= 0; --r) {
+        double v = M[r][3];
+        for (int c = r + 1; c < 3; ++c) v -= M[r][c] * beta[c];
+        beta[r] = v / M[r][r];
+    }
+    const double reduction = beta[0] * rhs[0] + beta[1] * rhs[1] + beta[2] * rhs[2];   /* chi0^2 - chi^2_min (X has zero weighted mean) */
+    return 0.5 * (double)(Nt - 1) * reduction / chi0;
+}
+
+/* Same calling convention as lsp_oracle_gls plus wts[Nt] fp32 (host) and a second scratch array of Nt doubles. */
+int lsp_oracle_gls_weighted(const double* t, const float* x, const float* wts, int64_t Nt,
+                            double f_min, double df, const int64_t* ks, int64_t nk,
+                            double* P, double* scratch, double* scratch_w, int nthreads)
+{
+    double sw = 0.0, swx = 0.0;
+    for (int64_t j = 0; j < Nt; ++j) { sw += (double)wts[j]; swx += (double)wts[j] * (double)x[j]; }
+    const double mean = swx / sw;
+    double chi0 = 0.0;
+    for (int64_t j = 0; j < Nt; ++j) {
+        scratch[j] = (double)x[j] - mean;
+        scratch_w[j] = (double)wts[j];
+        chi0 += scratch_w[j] * scratch[j] * scratch[j];
+    }
+    int used = 1;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    #pragma omp parallel
+    {
+        #pragma omp single
+        used = omp_get_num_threads();
+    }
+    #pragma omp parallel for schedule(dynamic, 4)
+#endif
+    for (int64_t i = 0; i < nk; ++i) {
+        int64_t k = ks ? ks[i] : i;
+        P[i] = lsp_oracle_gls_w_one(t, scratch, scratch_w, Nt, f_min + (double)k * df, chi0);
     }
     return used;
 }

@@ -440,3 +440,102 @@ def test_GP5_zechmeister_kuerster_closed_form():
     assert np.max(np.abs(P - out)) <= 1e-10 * P.max()
     assert P.min() >= 0.0 and P.max() <= (N - 1) / 2.0
     assert oracle.periodogram_gls(t, x, 0.0, 0.1, 1)[0] == 0.0                  # singular at f = 0 (G7)
+
+
+# ----------------------------------------------------------------------------- weighted generalised periodogram (GW1-GW5)
+def _weighted_case(Nt=120, seed=31, span=40.0):
+    rng, t = _gappy(Nt, seed, span=span)
+    sig = rng.uniform(0.3, 2.0, t.size)                                   # per-sample error bars
+    x = (3.0 + 0.9 * np.sin(2 * np.pi * 0.31 * t + 0.4) + sig * rng.standard_normal(t.size)).astype(np.float32)
+    w = (1.0 / sig ** 2).astype(np.float32)
+    return rng, t, x, w
+
+
+def test_GW1_constant_weights_reduce_to_the_unweighted_periodogram():
+    """w_j = const must reproduce lsp_oracle_gls (pins GP1-GP5), whatever the constant: only weight RATIOS matter."""
+    rng, t, x, _ = _weighted_case()
+    f0, df, Nf = 0.02, 0.007, 300
+    ref = oracle.periodogram_gls(t, x, f0, df, Nf)
+    for c in (1.0, 0.125, 37.0):
+        P = oracle.periodogram_gls_weighted(t, x, np.full(t.size, c, np.float32), f0, df, Nf)
+        assert np.max(np.abs(P - ref)) <= 1e-11 * ref.max()
+
+
+def test_GW2_integer_weights_equal_repeated_samples():
+    """A sample with weight n is n copies of that sample: the chi^2 ratio of the weighted fit equals the chi^2 ratio of
+    the UNWEIGHTED generalised periodogram (pinned on its own) of the expanded series.  Catches a weight applied to the
+    wrong factor, squared, or left out of one of the sums."""
+    rng, t, x, _ = _weighted_case(Nt=60, seed=5)
+    n = rng.integers(1, 5, t.size)
+    f0, df, Nf = 0.03, 0.011, 150
+    Pw = oracle.periodogram_gls_weighted(t, x, n.astype(np.float32), f0, df, Nf)
+    te, xe = np.repeat(t, n), np.repeat(x, n)
+    Pe = oracle.periodogram_gls(te, xe, f0, df, Nf)
+    ratio_w = Pw / ((t.size - 1) / 2.0)
+    ratio_e = Pe / ((te.size - 1) / 2.0)
+    assert np.max(np.abs(ratio_w - ratio_e)) <= 1e-11
+
+
+def test_GW3_numpy_lstsq_on_sqrt_weighted_rows():
+    """Independent solver: minimise |sqrt(w) (x - A beta)|^2 by numpy.linalg.lstsq (SVD) row-scaled by sqrt(w)."""
+    rng, t, x, w = _weighted_case(Nt=90, seed=77)
+    f0, df, Nf = 0.04, 0.013, 120
+    P = oracle.periodogram_gls_weighted(t, x, w, f0, df, Nf)
+    y, wd = x.astype(np.float64), w.astype(np.float64)
+    sw = np.sqrt(wd)
+    ybar = (wd * y).sum() / wd.sum()
+    chi0 = (wd * (y - ybar) ** 2).sum()
+    out = np.empty(Nf)
+    for i in range(Nf):
+        om = 2 * np.pi * (f0 + i * df)
+        A = np.stack([np.cos(om * t), np.sin(om * t), np.ones(t.size)], axis=1)
+        beta = np.linalg.lstsq(A * sw[:, None], y * sw, rcond=None)[0]
+        chi = (wd * (y - A @ beta) ** 2).sum()
+        out[i] = 0.5 * (t.size - 1) * (chi0 - chi) / chi0
+    assert np.max(np.abs(P - out)) <= 1e-10 * P.max()
+    assert P.min() >= 0.0 and P.max() <= (t.size - 1) / 2.0
+
+
+def test_GW4_scipy_lombscargle_weights():
+    """Library special case: scipy.signal.lombscargle(weights=w, floating_mean=True, normalize=True) is the fraction of the
+    weighted variance the fit explains; times (Nt - 1)/2 it is this normalisation (as GP2 for unit weights)."""
+    from scipy.signal import lombscargle
+    rng, t, x, w = _weighted_case(Nt=200, seed=12, span=50.0)
+    f = 0.01 + 0.004 * np.arange(400)
+    P = oracle.periodogram_gls_weighted(t, x, w, f[0], 0.004, f.size)
+    p = lombscargle(t, x.astype(np.float64), 2 * np.pi * f, weights=w.astype(np.float64), floating_mean=True, normalize=True)
+    assert np.max(np.abs(P - p * (t.size - 1) / 2.0)) <= 1e-9 * P.max()
+
+
+def test_GW5_zechmeister_kuerster_closed_form_with_weights():
+    """The closed form of the cited paper (Zechmeister & Kuerster 2009) with normalised weights w_j / sum w, typed here:
+    p = [SS YC^2 + CC YS^2 - 2 CS YC YS] / (YY D); plus: a zero weight removes the sample from the fit, and a noise-free
+    sinusoid + offset reaches the maximum (Nt - 1)/2 whatever the weights."""
+    rng, t, x, w = _weighted_case(Nt=83, seed=14, span=12.0)
+    y, wn = x.astype(np.float64), w.astype(np.float64) / w.astype(np.float64).sum()
+    f = 0.05 + 0.021 * np.arange(120)
+    out = np.empty(f.size)
+    for i, fi in enumerate(f):
+        c, s = np.cos(2 * np.pi * fi * t), np.sin(2 * np.pi * fi * t)
+        Y, C, S = (wn * y).sum(), (wn * c).sum(), (wn * s).sum()
+        YY = (wn * y * y).sum() - Y * Y
+        YC = (wn * y * c).sum() - Y * C
+        YS = (wn * y * s).sum() - Y * S
+        CC = (wn * c * c).sum() - C * C
+        SS = (wn * s * s).sum() - S * S
+        CS = (wn * c * s).sum() - C * S
+        D = CC * SS - CS * CS
+        out[i] = (SS * YC ** 2 + CC * YS ** 2 - 2 * CS * YC * YS) / (YY * D) * (t.size - 1) / 2.0
+    P = oracle.periodogram_gls_weighted(t, x, w, f[0], 0.021, f.size)
+    assert np.max(np.abs(P - out)) <= 1e-10 * P.max()
+    # zero weights: same chi^2 ratio as the series without those samples
+    w0 = w.copy(); w0[::3] = 0.0
+    keep = w0 > 0
+    Pz = oracle.periodogram_gls_weighted(t, x, w0, f[0], 0.021, f.size) / ((t.size - 1) / 2.0)
+    Pk = oracle.periodogram_gls_weighted(t[keep], x[keep], w0[keep], f[0], 0.021, f.size) / ((keep.sum() - 1) / 2.0)
+    assert np.max(np.abs(Pz - Pk)) <= 1e-11
+    # exact model: the fit is perfect at its own frequency
+    xs = (2.0 + 1.5 * np.cos(2 * np.pi * 0.4 * t - 0.3)).astype(np.float32)
+    Pm = oracle.periodogram_gls_weighted(t, xs, w, 0.4, 0.1, 1)[0]
+    assert abs(Pm - (t.size - 1) / 2.0) <= 1e-5 * (t.size - 1) / 2.0     # x is fp32: the model is exact to ~1e-7 per sample
+    assert oracle.periodogram_gls_weighted(t, x, w, 0.0, 0.1, 1)[0] == 0.0          # singular at f = 0 (G7)

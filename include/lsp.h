@@ -144,6 +144,33 @@ int lsp_periodogram_gls_batched(lsp_handle h,
                                 void* stream);
 
 /*
+ * Weighted generalised periodogram (the per-sample weights of Zechmeister & Kuerster 2009):
+ * the fit of lsp_periodogram_gls with chi^2 = sum_j w_j (x_j - a cos - b sin - c)^2, returned as
+ *     P = (Nt - 1)/2 * (chi0^2 - chi^2_min) / chi0^2,   chi0^2 = sum_j w_j (x_j - xbar_w)^2,  xbar_w = sum w x / sum w
+ * (reading G14: the unweighted normalisation written as a chi^2 ratio; w_j = const gives
+ * lsp_periodogram_gls; 0 <= P <= (Nt - 1)/2).  Typical use: w_j = 1 / sigma_j^2.
+ *   w DEVICE const float[Nt] per series (series b at w + b*w_stride, |w_stride| >= Nt; w_stride = 0: one weight vector for
+ *   all series), finite, >= 0, positive sum (not checked: a violation yields NaN).  Only weight ratios matter; w_j = 0
+ *   removes sample j from the fit.  w == NULL: unit weights (identical to lsp_periodogram_gls[_batched]).
+ *   Everything else as lsp_periodogram_gls[_batched].  Runs steps 3-5 on the FP32 pipe (two accumulate launches), with the
+ *   samples entering as sqrt(w_j) x_j and sqrt(w_j) e^{i theta}: the recurrence is linear, so the weights cost nothing per term.
+ */
+int lsp_periodogram_gls_weighted(lsp_handle h,
+                                 const double* t, const float* x, const float* w, int64_t Nt,
+                                 double f_min, double df, int64_t Nf,
+                                 float* P, void* stream);
+
+int lsp_periodogram_gls_weighted_batched(lsp_handle h,
+                                         const double* t, int64_t t_stride,
+                                         const float* x, int64_t x_stride,
+                                         const float* w, int64_t w_stride,
+                                         int64_t B, int64_t Nt,
+                                         double f_min, double df, int64_t Nf,
+                                         float* P, int64_t p_stride,
+                                         int32_t* peak_idx, float* peak_val,
+                                         void* stream);
+
+/*
  * Host-buffer forms: same arithmetic, HOST pointers.  The call copies t and x to the device
  * (cudaMemcpyAsync on `stream`), runs the device path, copies P (and the peaks) back and
  * synchronises `stream`.  Arrays are dense: series b at t + b*Nt, x + b*Nt, P + b*Nf.

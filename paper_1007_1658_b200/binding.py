@@ -21,7 +21,8 @@ SYMBOLS = (
     "lsp_create", "lsp_destroy", "lsp_set_param", "lsp_get_param",
     "lsp_periodogram", "lsp_periodogram_batched",
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
-    "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched", "lsp_reserve",
+    "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched",
+    "lsp_periodogram_gls_weighted", "lsp_periodogram_gls_weighted_batched", "lsp_reserve",
     "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
@@ -60,6 +61,9 @@ def load(rebuild: bool = False):
                                                  vp, vp, vp, vp]
     lib.lsp_periodogram_gls.argtypes = lib.lsp_periodogram.argtypes
     lib.lsp_periodogram_gls_batched.argtypes = lib.lsp_periodogram_batched.argtypes
+    lib.lsp_periodogram_gls_weighted.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, i64, vp, vp]
+    lib.lsp_periodogram_gls_weighted_batched.argtypes = [vp, vp, i64, vp, i64, vp, i64, i64, i64, dbl, dbl, i64,
+                                                         vp, i64, vp, vp, vp]
     lib.lsp_false_alarm.argtypes = [vp, vp, i64, i64, dbl, vp, vp]
     lib.lsp_reserve.argtypes = [vp, i64, ci, i64, i64, ci]
     lib.lsp_last_plan.argtypes = [vp, ctypes.POINTER(i64)]
@@ -185,8 +189,9 @@ class Handle:
         return dict(zip(("moments", "records", "accumulate", "finish"), [float(v) for v in out]))
 
     # -- device-pointer entry points (torch CUDA tensors in, enqueue only)
-    def periodogram(self, t, x, f_min: float, df: float, Nf: int, out=None, stream=None, gls: bool = False):
-        """lsp_periodogram (gls=True: lsp_periodogram_gls): t float64[Nt], x float32[Nt] CUDA tensors -> P float32[Nf] (CUDA)."""
+    def periodogram(self, t, x, f_min: float, df: float, Nf: int, out=None, stream=None, gls: bool = False, weights=None):
+        """lsp_periodogram (gls=True: lsp_periodogram_gls; weights float32[Nt]: lsp_periodogram_gls_weighted):
+        t float64[Nt], x float32[Nt] CUDA tensors -> P float32[Nf] (CUDA)."""
         import torch
         _want(t, torch.float64, 1, "t"); _want(x, torch.float32, 1, "x")
         if t.shape != x.shape:
@@ -195,6 +200,14 @@ class Handle:
         _want(P, torch.float32, 1, "P")
         if P.numel() < Nf:
             raise ValueError("P too small")
+        if weights is not None:
+            _want(weights, torch.float32, 1, "weights")
+            if weights.shape != x.shape:
+                raise ValueError("weights and x must have the same length")
+            st = self._lib.lsp_periodogram_gls_weighted(self._h, t.data_ptr(), x.data_ptr(), weights.data_ptr(), t.numel(),
+                                                        float(f_min), float(df), int(Nf), P.data_ptr(), _stream_ptr(stream))
+            self._check(st, "lsp_periodogram_gls_weighted")
+            return P
         fn = self._lib.lsp_periodogram_gls if gls else self._lib.lsp_periodogram
         st = fn(self._h, t.data_ptr(), x.data_ptr(), t.numel(),
                 float(f_min), float(df), int(Nf), P.data_ptr(), _stream_ptr(stream))
@@ -202,8 +215,9 @@ class Handle:
         return P
 
     def periodogram_batched(self, t, x, f_min: float, df: float, Nf: int,
-                            want_P: bool = True, want_peaks: bool = True, stream=None, gls: bool = False):
-        """lsp_periodogram_batched: x float32[B,Nt]; t float64[B,Nt] or float64[Nt] (shared).
+                            want_P: bool = True, want_peaks: bool = True, stream=None, gls: bool = False, weights=None):
+        """lsp_periodogram_batched: x float32[B,Nt]; t float64[B,Nt] or float64[Nt] (shared); gls=True: the generalised
+        periodogram; weights float32[B,Nt] or float32[Nt] (shared): lsp_periodogram_gls_weighted_batched.
 
         Returns (P float32[B,Nf] or None, peak_idx int32[B] or None, peak_val float32[B] or None)."""
         import torch
@@ -220,6 +234,18 @@ class Handle:
         P = torch.empty((B, int(Nf)), dtype=torch.float32, device=x.device) if want_P else None
         pi = torch.empty(B, dtype=torch.int32, device=x.device) if want_peaks else None
         pv = torch.empty(B, dtype=torch.float32, device=x.device) if want_peaks else None
+        if weights is not None:
+            _want(weights, torch.float32, weights.dim(), "weights")
+            if tuple(weights.shape) not in ((B, Nt), (Nt,)):
+                raise ValueError("weights must be [B, Nt] or [Nt]")
+            st = self._lib.lsp_periodogram_gls_weighted_batched(
+                self._h, t.data_ptr(), t_stride, x.data_ptr(), Nt, weights.data_ptr(), Nt if weights.dim() == 2 else 0,
+                B, Nt, float(f_min), float(df), int(Nf),
+                P.data_ptr() if want_P else None, int(Nf),
+                pi.data_ptr() if want_peaks else None, pv.data_ptr() if want_peaks else None,
+                _stream_ptr(stream))
+            self._check(st, "lsp_periodogram_gls_weighted_batched")
+            return P, pi, pv
         fn = self._lib.lsp_periodogram_gls_batched if gls else self._lib.lsp_periodogram_batched
         st = fn(
             self._h, t.data_ptr(), t_stride, x.data_ptr(), Nt, B, Nt, float(f_min), float(df), int(Nf),

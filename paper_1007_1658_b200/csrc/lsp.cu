@@ -104,9 +104,10 @@ int ensure(lsp_ctx* h, void** ptr, size_t* have, size_t need) {
 
 typedef void (*accum_fn)(const AccumParams);
 
-struct KernelEntry { int K; accum_fn fn; const char* name; int max_t; };
+struct KernelEntry { int K; accum_fn fn, fn_weighted; const char* name; const char* name_weighted; int max_t; };
 
-#define LSP_ENTRY_Z(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, "accum_z_kernel<K=" #K ",fp32,three-term>", MAXT }
+#define LSP_ENTRY_Z(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, accum_z_kernel<K, MAXT, MINB, true>, \
+                                     "accum_z_kernel<K=" #K ",fp32,three-term>", "accum_z_kernel<K=" #K ",fp32,three-term,weighted>", MAXT }
 const KernelEntry g_kernels[] = {
     LSP_ENTRY_Z(4, 256, 1), LSP_ENTRY_Z(8, 256, 1), LSP_ENTRY_Z(12, 256, 1), LSP_ENTRY_Z(16, 256, 1),
     LSP_ENTRY_Z(20, 256, 1), LSP_ENTRY_Z(24, 256, 2), LSP_ENTRY_Z(28, 128, 3), LSP_ENTRY_Z(32, 128, 3),
@@ -117,17 +118,17 @@ const KernelEntry* find_kernel(int K) {
     return nullptr;
 }
 
-size_t accum_smem_bytes(const KernelEntry* ke, int T) {
-    return (size_t)TILE_Z * 24 + (size_t)T * (4 * ke->K + 1) * sizeof(float);
+size_t accum_smem_bytes(const KernelEntry* ke, int T, bool weighted) {
+    return (size_t)TILE_Z * (weighted ? 32 : 24) + (size_t)T * (4 * ke->K + 1) * sizeof(float);
 }
 
 // Launch plan: which form and tile, how many time splits (and chunks).  Units of work = B * nfb * nsplit CTAs; the
 // hardware block scheduler balances them over the SMs, so we want many more units than CTA slots.
-Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t table_series)
+Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t table_series, int force_pipe = 0)
 {
     Plan pl;
     PlanOverrides ov;
-    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.pipe = h->opt_pipe; ov.L = h->opt_coarse;
+    ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.pipe = force_pipe ? force_pipe : h->opt_pipe; ov.L = h->opt_coarse;
     ov.table_budget = h->opt_table_mb ? (h->opt_table_mb << 20) : 0; ov.table_series = table_series;
     const PlanChoice pc = plan_choose(h->sm_count, B, Nt, Nf, ov);
     pl.pipe = pc.pipe; pl.K = pc.K; pl.T = pc.T; pl.nfb = pc.nfb; pl.L = pc.L;
@@ -182,7 +183,7 @@ bool shared_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, SharedLayo
 }
 
 struct Layout {
-    size_t recA, recB, ws, ws1, recA1, psum, pvar, peak, cnt, tab, total;
+    size_t recA, recB, ws, ws1, recA1, psum, pvar, pw, peak, cnt, tab, total;
     int64_t tab_groups;          // k-step groups of one series' table (one chunk + padding); 0: no table
     size_t tab_bytes;
 };
@@ -199,6 +200,7 @@ Layout device_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, int64_t 
     L.recA1 = off; if (gls) off = align_up(off + n_samp * sizeof(float4), 256);
     L.psum = off;  off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
     L.pvar = off;  off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);
+    L.pw = off;    if (gls) off = align_up(off + (size_t)B * pl.nparts * sizeof(double), 256);   // weighted form: sum of weights per block
     L.peak = off;  off = align_up(off + (size_t)B * sizeof(u64), 256);
     L.cnt = off;   off = align_up(off + (size_t)B * sizeof(unsigned), 256);
     L.tab_groups = 0; L.tab_bytes = 0; L.tab = off;
@@ -313,10 +315,10 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
 // What the call will run (shared by run_device and lsp_reserve).
 struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair; int64_t tab_series; };
 
-int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf, bool gls, Route& r)
+int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf, bool gls, Route& r, bool weighted = false)
 {
     r.tab_series = (t_stride == 0) ? 1 : B;
-    r.pl = make_plan(h, B, Nt, Nf, r.tab_series);
+    r.pl = make_plan(h, B, Nt, Nf, r.tab_series, weighted ? PLAN_PIPE_FP32 : 0);   // per-sample weights: the FP32-pipe form carries them
     Plan& pl = r.pl;
     if (pl.K == 0) return LSP_EINVAL;
     r.tensor = pl.pipe == PLAN_PIPE_TENSOR;
@@ -328,7 +330,7 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
     if (!r.tensor) {
         const KernelEntry* ke = find_kernel(pl.K);
         if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
-        pl.kernel_name = ke->name;
+        pl.kernel_name = weighted ? ke->name_weighted : ke->name;
     } else if (r.pair) {
         pl.kernel_name = "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>";
         pl.launches = 3 + 2 * pl.nchunks;
@@ -350,12 +352,14 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
 int run_device(lsp_ctx* h,
                const double* t, int64_t t_stride, const float* x, int64_t x_stride,
                int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
-               float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st, bool gls = false)
+               float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, cudaStream_t st, bool gls = false,
+               const float* w = nullptr, int64_t w_stride = 0)
 {
+    const bool weighted = w != nullptr;                    // weighted generalised periodogram (implies gls)
     if (use_shared_path(h, t_stride, B, Nt, gls))
         return run_device_shared(h, t, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride, peak_idx, peak_val, st);
     Route r;
-    int rc = route(h, t_stride, B, Nt, Nf, gls, r);
+    int rc = route(h, t_stride, B, Nt, Nf, gls, r, weighted);
     if (rc != LSP_OK) return rc;
     Plan& pl = r.pl;
     const bool tensor = r.tensor;                          // tensor-core forms: X scaled to unit variance
@@ -373,6 +377,7 @@ int run_device(lsp_ctx* h,
     float4* recA1 = gls ? reinterpret_cast<float4*>(base + L.recA1) : nullptr;
     double* psum = reinterpret_cast<double*>(base + L.psum);
     double* pvar = reinterpret_cast<double*>(base + L.pvar);
+    double* pw = reinterpret_cast<double*>(base + L.pw);
     u64* peak64 = reinterpret_cast<u64*>(base + L.peak);
     unsigned* counter = reinterpret_cast<unsigned*>(base + L.cnt);
     unsigned char* table = reinterpret_cast<unsigned char*>(base + L.tab);
@@ -394,16 +399,18 @@ int run_device(lsp_ctx* h,
 
     // steps 1-2
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
-    const bool fused_pre = pl.nparts == 1;                // one block per series: step 1's sum inside the records kernel
+    const bool fused_pre = pl.nparts == 1 && !weighted;   // one block per series: step 1's sum inside the records kernel
     if (!fused_pre) {
-        moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
+        moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter, w, w_stride, pw);
         LSP_CUDA(h, cudaGetLastError());
     } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
+    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar);
+    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
-    if (gls) {
+    if (weighted) pl.launches -= 1;                       // (the weight records were written by records_weighted_kernel)
+    if (gls && !weighted) {
         unit_records_kernel<<<(unsigned)((n_samp + 255) / 256), 256, 0, st>>>(recA, recA1, (int64_t)n_samp);
         LSP_CUDA(h, cudaGetLastError());
     }
@@ -477,11 +484,13 @@ int run_device(lsp_ctx* h,
                 }
             } else {
                 AccumParams ap;
+                ap.recW = weighted ? recA1 : nullptr;
                 ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.Nt = Nt; ap.Nf = Nf;
                 ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
-                const size_t smem = accum_smem_bytes(ke, pl.T);
-                LSP_CUDA(h, cudaFuncSetAttribute(ke->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                ke->fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
+                const size_t smem = accum_smem_bytes(ke, pl.T, weighted);
+                const accum_fn fn = weighted ? ke->fn_weighted : ke->fn;
+                LSP_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
             }
             LSP_CUDA(h, cudaGetLastError());
         }
@@ -710,6 +719,28 @@ int lsp_periodogram_gls_batched(lsp_handle h,
     DeviceGuard g(h->device);
     return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
                       peak_idx, peak_val, static_cast<cudaStream_t>(stream), true);
+}
+
+int lsp_periodogram_gls_weighted_batched(lsp_handle h,
+                                         const double* t, int64_t t_stride, const float* x, int64_t x_stride,
+                                         const float* w, int64_t w_stride,
+                                         int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
+                                         float* P, int64_t p_stride, int32_t* peak_idx, float* peak_val, void* stream)
+{
+    int rc = check_batch_args(h, t, x, B, Nt, 4, f_min, df, Nf, P, peak_idx, peak_val);
+    if (rc == LSP_OK) rc = check_strides(t_stride, x_stride, p_stride, B, Nt, Nf, P);
+    if (rc == LSP_OK && w && B > 1 && w_stride != 0 && std::llabs(w_stride) < Nt) rc = LSP_EINVAL;
+    if (rc != LSP_OK) return rc;
+    DeviceGuard g(h->device);
+    return run_device(h, t, t_stride, x, x_stride, B, Nt, f_min, df, Nf, P, p_stride,
+                      peak_idx, peak_val, static_cast<cudaStream_t>(stream), true, w, w_stride);
+}
+
+int lsp_periodogram_gls_weighted(lsp_handle h, const double* t, const float* x, const float* w, int64_t Nt,
+                                 double f_min, double df, int64_t Nf, float* P, void* stream)
+{
+    if (!P) return LSP_EINVAL;
+    return lsp_periodogram_gls_weighted_batched(h, t, Nt, x, Nt, w, Nt, 1, Nt, f_min, df, Nf, P, Nf, nullptr, nullptr, stream);
 }
 
 int lsp_periodogram_gls(lsp_handle h, const double* t, const float* x, int64_t Nt,

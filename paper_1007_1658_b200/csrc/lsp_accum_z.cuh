@@ -30,6 +30,7 @@
 namespace lsp {
 
 struct AccumParams {
+    const float4* recW;     // weighted generalised periodogram: recW[j].x = sqrt of the normalised weight (anchors are scaled by it); else NULL
     const float4* recA;
     const ulonglong2* recB;
     float* ws;              // [B][nsplit][4][Nf]
@@ -45,27 +46,34 @@ struct ZAnchor { float c0, s0, cp, sp, X, g; };
 // step 3: anchor at the thread's first frequency: exact integer phase (reading G3) -> MUFU sin/cos
 // (PAPER.md:290), plus the value one recurrence step back by an exact rotation (consistent with the
 // anchor, so the anchor's own error is not amplified by the three-term recurrence).
-__device__ __forceinline__ ZAnchor z_anchor(const float4* tS, const float2* tR, int q, unsigned tid)
+// WEIGHTED (weighted generalised periodogram): the tile also holds sw = sqrt(normalised weight) and the anchor pair is
+// scaled by it: the recurrence is linear, so z_m = sw e^{i th_m} throughout and, with X = sw x, the sums become
+// sum w x e^{i th} and sum w cos th e^{i th} at no cost per term (4 more FMUL per sample).
+template <bool WEIGHTED>
+__device__ __forceinline__ ZAnchor z_anchor(const float4* tS, const void* tRv, int q, unsigned tid)
 {
     const float4 sv = tS[q];
-    const float2 rv = tR[q];
+    float cd, sd, sw = 1.f;
+    if (WEIGHTED) { const float4 rv = static_cast<const float4*>(tRv)[q]; cd = rv.x; sd = rv.y; sw = rv.z; }
+    else { const float2 rv = static_cast<const float2*>(tRv)[q]; cd = rv.x; sd = rv.y; }
     const int ph = (int)(__float_as_uint(sv.z) + tid * __float_as_uint(sv.w));
     const float ang = (float)ph * LSP_RAD_PER_PHASE;
     ZAnchor a;
     a.c0 = __cosf(ang); a.s0 = __sinf(ang);
-    a.cp = fmaf(a.c0, rv.x, a.s0 * rv.y);
-    a.sp = fmaf(a.s0, rv.x, -(a.c0 * rv.y));
+    if (WEIGHTED) { a.c0 *= sw; a.s0 *= sw; }
+    a.cp = fmaf(a.c0, cd, a.s0 * sd);
+    a.sp = fmaf(a.s0, cd, -(a.c0 * sd));
     a.X = sv.x; a.g = sv.y;
     return a;
 }
 
-template <int K, int MAXT, int MINB>
+template <int K, int MAXT, int MINB, bool WEIGHTED = false>
 __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p)
 {
     extern __shared__ float4 lsp_smem[];
     float4* tS = lsp_smem;                                     // {X, g, b32, w32} per sample
-    float2* tR = reinterpret_cast<float2*>(tS + TILE_Z);       // {cd, sd} per sample
-    float* outer = reinterpret_cast<float*>(tR + TILE_Z);      // [T][4K+1] (odd stride: conflict-free)
+    void* tR = tS + TILE_Z;                                    // {cd, sd} per sample (WEIGHTED: {cd, sd, sw, -}, the tile region is sized for it)
+    float* outer = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(tR) + TILE_Z * (WEIGHTED ? 16 : 8));   // [T][4K+1] (odd stride: conflict-free)
 
     const int T = blockDim.x;
     const unsigned tid = threadIdx.x;
@@ -113,7 +121,8 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
             const unsigned b32 = (unsigned)((ph + 0x80000000ull) >> 32);
             const unsigned w32 = (unsigned)(((u64)K * r.y + 0x80000000ull) >> 32);
             tS[i] = make_float4(a.x, a.w, __uint_as_float(b32), __uint_as_float(w32));
-            tR[i] = make_float2(a.y, a.z);
+            if (WEIGHTED) static_cast<float4*>(tR)[i] = make_float4(a.y, a.z, __ldg(&p.recW[b * p.Nt + j + i].x), 0.f);
+            else static_cast<float2*>(tR)[i] = make_float2(a.y, a.z);
         }
         __syncthreads();
 
@@ -123,15 +132,15 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
 #define LSP_Z_PIPE 0
 #endif
 #if LSP_Z_PIPE
-        ZAnchor nx = z_anchor(tS, tR, 0, tid);
+        ZAnchor nx = z_anchor<WEIGHTED>(tS, tR, 0, tid);
 #endif
         #pragma unroll 1
         for (int q = 0; q < ns; ++q) {
 #if LSP_Z_PIPE
             const ZAnchor cur = nx;
-            nx = z_anchor(tS, tR, min(q + 1, ns - 1), tid);
+            nx = z_anchor<WEIGHTED>(tS, tR, min(q + 1, ns - 1), tid);
 #else
-            const ZAnchor cur = z_anchor(tS, tR, q, tid);
+            const ZAnchor cur = z_anchor<WEIGHTED>(tS, tR, q, tid);
 #endif
             u64 z = pack2(cur.c0, cur.s0);
             u64 zp = pack2(cur.cp, cur.sp);

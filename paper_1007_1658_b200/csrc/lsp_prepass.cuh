@@ -13,22 +13,78 @@
 namespace lsp {
 
 // grid (nb, B), any block size (multiple of 32).  part_sum[b][blk] = sum of x over the block's chunk.
+// Weighted generalised periodogram (w != NULL): part_sum = sum w x and part_w = sum w over the chunk.
 __global__ void moments_kernel(const float* __restrict__ x, int64_t x_stride, int64_t Nt,
                                int64_t chunk, double* __restrict__ part_sum,
-                               u64* __restrict__ peak64, unsigned* __restrict__ counter)
+                               u64* __restrict__ peak64, unsigned* __restrict__ counter,
+                               const float* __restrict__ w = nullptr, int64_t w_stride = 0, double* __restrict__ part_w = nullptr)
 {
     __shared__ double red[32];
     const int b = blockIdx.y;
     const float* xb = x + (int64_t)b * x_stride;
+    const float* wb = w ? w + (int64_t)b * w_stride : nullptr;
+    const int64_t j0 = (int64_t)blockIdx.x * chunk;
+    const int64_t j1 = min(Nt, j0 + chunk);
+    double acc = 0.0, accw = 0.0;
+    for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+        if (wb) { const double wj = (double)__ldg(wb + j); acc += wj * (double)__ldg(xb + j); accw += wj; }
+        else acc += (double)__ldg(xb + j);
+    }
+    acc = block_sum(acc, red);
+    if (wb) accw = block_sum(accw, red);
+    if (threadIdx.x == 0) {
+        part_sum[(int64_t)b * gridDim.x + blockIdx.x] = acc;
+        if (wb) part_w[(int64_t)b * gridDim.x + blockIdx.x] = accw;
+        if (blockIdx.x == 0) { peak64[b] = 0ull; counter[b] = 0u; }
+    }
+}
+
+// Weighted generalised periodogram: records of one series' chunk.  With W = sum w, wn_j = Nt w_j / W (mean weight 1):
+//   recA  = {sqrt(wn_j) (x_j - xbar_w), cos d_j, sin d_j, 2 cos d_j}   (measurement pass)
+//   recA1 = {sqrt(wn_j),                cos d_j, sin d_j, 2 cos d_j}   (weight pass: sum wn cos, sum wn sin)
+//   part_var[b][blk] = sum wn_j (x_j - xbar_w)^2  (so that part_var / (Nt - 1) is the weighted sample variance)
+// The accumulate kernel scales its anchors by recA1.x, so both passes form sums of wn_j (...) e^{i theta}.
+// grid (nb, B); part_sum / part_w from moments_kernel.
+__global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_stride,
+                                        const float* __restrict__ x, int64_t x_stride,
+                                        const float* __restrict__ w, int64_t w_stride,
+                                        int64_t Nt, int64_t chunk, double f_min, double df,
+                                        const double* __restrict__ part_sum, const double* __restrict__ part_w,
+                                        float4* __restrict__ recA, float4* __restrict__ recA1, ulonglong2* __restrict__ recB,
+                                        double* __restrict__ part_var)
+{
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    const int nb = gridDim.x;
+    const double* tb = t + (int64_t)b * t_stride;
+    const float* xb = x + (int64_t)b * x_stride;
+    const float* wb = w + (int64_t)b * w_stride;
+    double swx = 0.0, sw = 0.0;                            // fixed-order sums of the block partials
+    for (int i = 0; i < nb; ++i) { swx += part_sum[(int64_t)b * nb + i]; sw += part_w[(int64_t)b * nb + i]; }
+    const double mean = swx / sw;
+    const double wscale = (double)Nt / sw;
+    const double t0 = __ldg(tb);
     const int64_t j0 = (int64_t)blockIdx.x * chunk;
     const int64_t j1 = min(Nt, j0 + chunk);
     double acc = 0.0;
-    for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) acc += (double)__ldg(xb + j);
-    acc = block_sum(acc, red);
-    if (threadIdx.x == 0) {
-        part_sum[(int64_t)b * gridDim.x + blockIdx.x] = acc;
-        if (blockIdx.x == 0) { peak64[b] = 0ull; counter[b] = 0u; }
+    for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+        const double d = (double)__ldg(xb + j) - mean;
+        const double wn = (double)__ldg(wb + j) * wscale;
+        acc += wn * d * d;
+        const int64_t o = (int64_t)b * Nt + j;
+        const double tp = __ldg(tb + j) - t0;
+        double vfrac;
+        const u64 u = frac_fixed64(f_min, tp, nullptr);
+        const u64 v = frac_fixed64(df, tp, &vfrac);
+        double sd, cd;
+        sincospi(2.0 * vfrac, &sd, &cd);
+        const double sq = sqrt(wn);
+        recA[o] = make_float4((float)(sq * d), (float)cd, (float)sd, (float)(2.0 * cd));
+        recA1[o] = make_float4((float)sq, (float)cd, (float)sd, (float)(2.0 * cd));
+        recB[o] = make_ulonglong2(u, v);
     }
+    acc = block_sum(acc, red);
+    if (threadIdx.x == 0) part_var[(int64_t)b * nb + blockIdx.x] = acc;
 }
 
 // grid (nb, B).  Writes recA, recB for the block's chunk and part_var[b][blk] = sum (x - mean)^2.

@@ -704,6 +704,57 @@ def test_generalised_periodogram_batched_and_reduction(lsp):
         h.periodogram(td[:3].contiguous(), xd[:3].contiguous(), dfe, dfe, 4, gls=True)
 
 
+def test_weighted_generalised_periodogram(lsp):
+    """lsp_periodogram_gls_weighted (per-sample weights, SURVEY 8(f)-1 / PAPER.md:375) against the oracle's weighted
+    least squares: heteroscedastic series with w = 1/sigma^2 on gappy sampling, ragged sizes (several tiles, time splits,
+    a ragged last frequency block), zero weights, and constant weights (= the unweighted generalised periodogram)."""
+    import torch
+    pkg, h = lsp
+    rng = np.random.default_rng(808)
+    Nt, Nf = 5003, 4099
+    t = np.sort(np.concatenate([rng.uniform(0, 9, Nt // 2), rng.uniform(31, 40, Nt - Nt // 2)]))
+    sig = rng.uniform(0.3, 3.0, Nt)
+    x = (7.0 + 0.6 * np.sin(2 * np.pi * 0.0431 * t + 0.4) + 0.5 * np.sin(2 * np.pi * 1.7 * t) + sig * rng.standard_normal(Nt)).astype(np.float32)
+    wts = (1.0 / sig ** 2).astype(np.float32)
+    wts[::17] = 0.0                                                         # removed from the fit
+    f_min, df = 1.0 / 40.0, (3.0 - 1.0 / 40.0) / (Nf - 1)
+    ref = oracle.periodogram_gls_weighted(t, x, wts, f_min, df, Nf)
+    unw = oracle.periodogram_gls(t, x, f_min, df, Nf)
+    assert np.max(np.abs(ref - unw)) > 1e-2 * ref.max()                     # the weights really matter on this input
+    assert _top_two_gap(ref) >= QUAL_GAP
+    td, xd, wd = torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), torch.from_numpy(wts).cuda()
+    for K, ns in ((0, 0), (8, 3), (32, 2)):
+        h.set_param(pkg.PARAM_K, K); h.set_param(pkg.PARAM_NSPLIT, ns)
+        P = h.periodogram(td, xd, f_min, df, Nf, weights=wd).cpu().numpy()
+        plan = h.last_plan()
+        assert "weighted" in plan["kernel"] and plan["pipe"] == FP32, plan
+        _check(P, ref, "weighted gls K=%d nsplit=%d" % (K, ns))
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+    h.set_param(pkg.PARAM_K, 0); h.set_param(pkg.PARAM_NSPLIT, 0)
+    # constant weights: the unweighted generalised periodogram (oracle pin GW1), whatever the constant
+    Pc = h.periodogram(td, xd, f_min, df, Nf, weights=torch.full_like(wd, 0.37)).cpu().numpy()
+    _check(Pc, unw, "constant weights")
+    # batched, one weight vector per series and one shared by all series; per-series peaks
+    wl = workloads.c4(B=5, Nt=700, Nf=900, seed=11)
+    xb = (wl.x + 2.0).astype(np.float32)
+    wb = rng.uniform(0.2, 4.0, xb.shape).astype(np.float32)
+    tb, xbd, wbd = torch.from_numpy(wl.t).cuda(), torch.from_numpy(xb).cuda(), torch.from_numpy(wb).cuda()
+    P, pi, pv = h.periodogram_batched(tb, xbd, wl.f_min, wl.df, wl.Nf, weights=wbd)
+    P, pi, pv = P.cpu().numpy(), pi.cpu().numpy(), pv.cpu().numpy()
+    for b in range(wl.B):
+        rb = oracle.periodogram_gls_weighted(wl.t[b], xb[b], wb[b], wl.f_min, wl.df, wl.Nf)
+        _check(P[b], rb, "weighted gls series %d" % b)
+        assert _top_two_gap(rb) >= QUAL_GAP
+        assert _same_peak(P[b], rb, "weighted gls series %d" % b)
+        assert int(pi[b]) == int(np.argmax(P[b])) and float(pv[b]) == float(P[b].max())
+    P1, _, _ = h.periodogram_batched(tb, xbd, wl.f_min, wl.df, wl.Nf, weights=wbd[0].contiguous(), want_peaks=False)
+    P1 = P1.cpu().numpy()
+    for b in range(wl.B):
+        _check(P1[b], oracle.periodogram_gls_weighted(wl.t[b], xb[b], wb[0], wl.f_min, wl.df, wl.Nf), "shared weights series %d" % b)
+    with pytest.raises(pkg.LspError):
+        h.periodogram(td[:3].contiguous(), xd[:3].contiguous(), f_min, df, 4, weights=wd[:3].contiguous())
+
+
 def test_false_alarm_probability(lsp):
     """Eq. (3) epilogue against the oracle's plain formula on the GPU's own P (C1), on per-series peaks of a noise
     batch, and on hand-made values spanning Q = 1 ... 1e-30."""

@@ -25,6 +25,7 @@ namespace {
 
 struct Plan {
     int K = 0, T = 0, nsplit = 0, pipe = 0, nfb = 0, flush_tiles = 0, nparts = 0, launches = 0, L = 0, nchunks = 1;
+    bool fused_pre = false;
     int64_t split_len = 0, part_chunk = 0, chunk_len = 0;
     const char* kernel_name = "";
 };
@@ -39,7 +40,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     cudaEvent_t evc[TIMING_RING][2 * TIMING_MAX_CHUNKS] = {};   // accumulate launches of a chunked call, begin / end per chunk
     int ev_chunks[TIMING_RING] = {};
@@ -140,6 +141,8 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t tabl
     int64_t nparts = (Nt + 4095) / 4096;
     if (nparts > MAX_PARTS) nparts = MAX_PARTS;
     if (B >= 64 && nparts > 4) nparts = 4;
+    pl.fused_pre = Nt <= 16384;                           // short series: every block forms the mean itself (records_kernel<., FUSED>)
+    if (pl.fused_pre && B < 64) nparts = (Nt + 511) / 512;   // ... and a few series: spread the fp64 record work over more blocks
     pl.nparts = (int)nparts;
     pl.part_chunk = (Nt + nparts - 1) / nparts;
     pl.nparts = (int)((Nt + pl.part_chunk - 1) / pl.part_chunk);
@@ -213,6 +216,32 @@ Layout device_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, int64_t 
     return L;
 }
 
+// steps 6-7: with several time splits the sum over them is spread over 8 threads per frequency
+// Launch `kernel` as a programmatic dependent of the work before it in the stream (PDL): its CTAs may be scheduled while the
+// predecessor drains; the kernel calls pdl_wait() before reading what the predecessor wrote.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
+void launch_finish(const FinishParams& fp, int64_t B, cudaStream_t st, bool pdl = false)
+{
+    if (fp.nsplit >= 4) {
+        const int64_t per_block = FIN_THREADS / 8;
+        launch_pdl(finish_kernel<8>, dim3((unsigned)((fp.Nf + per_block - 1) / per_block), (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
+    } else {
+        const int64_t per_block = FIN_THREADS;
+        launch_pdl(finish_kernel<1>, dim3((unsigned)((fp.Nf + per_block - 1) / per_block), (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
+    }
+}
+
 bool use_shared_path(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, bool gls)
 {
     return t_stride == 0 && B > 1 && !gls && h->opt_shared != 1 && h->opt_pipe == 0 &&
@@ -261,7 +290,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     }
     // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
-    const bool fused_pre = pl.nparts == 1;                // one block per series: step 1's sum inside the records kernel
+    const bool fused_pre = pl.fused_pre;                   // short series: step 1's sum inside the records kernel
     if (!fused_pre) {
         moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
         LSP_CUDA(h, cudaGetLastError());
@@ -303,9 +332,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = (int)nsplit; fp.nparts = pl.nparts;
     fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
-    const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
-    dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
-    finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
+    launch_finish(fp, B, st);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
     h->plan = pl;
@@ -399,7 +426,7 @@ int run_device(lsp_ctx* h,
 
     // steps 1-2
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
-    const bool fused_pre = pl.nparts == 1 && !weighted;   // one block per series: step 1's sum inside the records kernel
+    const bool fused_pre = pl.fused_pre && !weighted;      // short series: step 1's sum inside the records kernel
     if (!fused_pre) {
         moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter, w, w_stride, pw);
         LSP_CUDA(h, cudaGetLastError());
@@ -417,6 +444,8 @@ int run_device(lsp_ctx* h,
 
     // steps 3-5 (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
     const int npass = gls ? 2 : 1;
+    // short grids, one pass: records -> accumulate -> finish as programmatic dependents (launch latency and CTA set-up overlap the predecessor's tail)
+    const bool pdl_small = r.small && !r.duo && !gls && h->opt_pdl != 1;
     const int flush_ksteps = (int)(((h->opt_flush ? h->opt_flush : 2048) + UM_KS - 1) / UM_KS);
     if (r.pair) {
         // CTA-pair form, one time chunk at a time: table pre-pass, then the accumulate launch(es) that read it
@@ -475,7 +504,7 @@ int run_device(lsp_ctx* h,
                 } else {
 #define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
                     LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
-                    accum_umma_small_kernel<LL, NS, MINB><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); } while (0)
+                    LSP_CUDA(h, launch_pdl(accum_umma_small_kernel<LL, NS, MINB>, dim3((unsigned)units), dim3(US_THREADS), UmmaSmall<LL, NS>::SMEM, st, pdl_small, up)); } while (0)
                     if (pl.L == 16) LSP_LAUNCH_SMALL(16, 4, 3);
                     else if (pl.L == 32) LSP_LAUNCH_SMALL(32, 4, 2);
                     else if (pl.L == 64) LSP_LAUNCH_SMALL(64, 4, 2);
@@ -512,9 +541,7 @@ int run_device(lsp_ctx* h,
     fp.x_scaled = tensor ? 1 : 0;
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
-    const int64_t per_block = (int64_t)FIN_THREADS * FIN_FPT;
-    dim3 gfin((unsigned)((Nf + per_block - 1) / per_block), (unsigned)B);
-    finish_kernel<<<gfin, FIN_THREADS, 0, st>>>(fp);
+    launch_finish(fp, B, st, pdl_small);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
 
@@ -604,6 +631,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
         case LSP_PARAM_TRUNC:      if (value > 4000) return LSP_EINVAL; h->opt_trunc = value; break;
         case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
+        case LSP_PARAM_PDL:        if (value > 1) return LSP_EINVAL; h->opt_pdl = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -623,6 +651,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_COARSE:     *value = h->opt_coarse; break;
         case LSP_PARAM_TRUNC:      *value = h->opt_trunc; break;
         case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
+        case LSP_PARAM_PDL:        *value = h->opt_pdl; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

@@ -162,6 +162,8 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
     tc_fence_after();
     const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
 
+    pdl_trigger();                                                      // the finish kernel may be scheduled (it waits for this grid to complete)
+    pdl_wait();                                                         // the pre-pass has completed: records and variance partials are visible
     if (w < US_GEN_WARPS) {
         // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
         const float4* recA = p.recA + b * p.Nt;

@@ -39,6 +39,12 @@ __device__ __forceinline__ u64 neg2(u64 a) {          // folded by ptxas into th
 }
 __device__ __forceinline__ float sum2(u64 a) { float lo, hi; unpack2(a, lo, hi); return lo + hi; }
 
+// ---- programmatic dependent launch (PDL): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
+// while its predecessor in the stream is still running; it must call pdl_wait() before it touches anything the predecessor
+// writes (a no-op when launched normally).  pdl_trigger() in the predecessor lets the dependent grid be scheduled early.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- deterministic block reduction of a double (fixed shuffle tree, then fixed-order warp sums) ----
 __device__ __forceinline__ double block_sum(double v, double* smem /* >= 32 doubles */) {
     #pragma unroll

@@ -14,7 +14,6 @@
 namespace lsp {
 
 constexpr int FIN_THREADS = 256;
-constexpr int FIN_FPT = 4;             // frequencies per thread
 
 struct FinishParams {
     const float* ws;                   // [B][nsplit][4][Nf]
@@ -33,11 +32,54 @@ struct FinishParams {
     int64_t x_row;                     //   [nsplit][4][Nf] block shared by all series (planes 2, 3 = CC - n/2, CS); else NULL / 0
 };
 
+// Step 6 for one frequency from the six sums (C1, S1 only for the generalised periodogram), in fp64.
+__device__ __forceinline__ double finish_combine(double XC, double XS, double CCh, double CS, double C1, double S1,
+                                                 double Nt, double inv2var, bool gls)
+{
+    if (gls) {
+        // Generalised (floating-mean) periodogram of Zechmeister & Kuerster 2009 (named at PAPER.md:375); the series is
+        // already (weighted-)mean-subtracted, so Y = 0 and YC = XC/N, YS = XS/N; with per-sample weights every sum carries the
+        // weights normalised to mean 1 (lsp_prepass.cuh), which leaves the formulas unchanged:
+        //   CCn = CC/N - (C/N)^2, SSn = SS/N - (S/N)^2, CSn = CS/N - C S/N^2, D = CCn SSn - CSn^2
+        //   P = (SSn XC^2 + CCn XS^2 - 2 CSn XC XS) / (2 var N D)        [same normalisation as eq. (1)]
+        const double cm = C1 / Nt, sm = S1 / Nt;
+        const double CCn = 0.5 + CCh / Nt - cm * cm, SSn = 0.5 - CCh / Nt - sm * sm, CSn = CS / Nt - cm * sm;
+        const double D = CCn * SSn - CSn * CSn;
+        if (!(D > 1e-9)) return 0.0;                                    // singular fit (f -> 0): 0, reading G7
+        return fmax(SSn * XC * XC + CCn * XS * XS - 2.0 * CSn * XC * XS, 0.0) / (Nt * D) * inv2var;
+    }
+    // The two terms of eq. (5) over the common denominator (Nt + R)(Nt - R) = Nt^2 - R^2: one fp64 division, no square root:
+    //   P 2 var = (S + D)/(Nt + R) + (S - D)/(Nt - R) = 2 (S Nt - D R) / (Nt^2 - R^2),   D R = (XC^2 - XS^2) A + 2 XC XS B
+    const double A = 2.0 * CCh, Bv = 2.0 * CS;
+    const double R2 = A * A + Bv * Bv;
+    const double xc2 = XC * XC, xs2 = XS * XS;
+    const double S = xc2 + xs2;
+    const double DR = (xc2 - xs2) * A + 2.0 * XC * XS * Bv;
+    double val;
+    if (R2 < (1.0 - 1e-6) * (1.0 - 1e-6) * Nt * Nt) {
+        val = fmax(2.0 * (S * Nt - DR), 0.0) / (Nt * Nt - R2);
+    } else {                                                            // Nt - R <= 1e-6 Nt: the 0/0 term is dropped (reading G7)
+        const double R = sqrt(R2);
+        val = fmax(S + DR / R, 0.0) / (Nt + R);
+    }
+    return val * inv2var;
+}
+
+// grid (ceil(Nf / FIN_BLOCK_F), B), FIN_THREADS threads = FIN_SL split lanes x FIN_BLOCK_F frequencies: thread (l, f) sums
+// the time splits sp = l, l + FIN_SL, ... of frequency f in that order (independent loads, all in flight at once); the
+// FIN_SL partial sums are then added in lane order by the l = 0 thread.  The order is fixed, so the result is
+// deterministic; with few frequencies and many splits (C1, C2) the sum over the splits is no longer one long dependent chain.
+// FIN_SL = 1 (few splits): one thread per frequency, 256 frequencies per block, no exchange.
+template <int FIN_SL>
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
 {
+    constexpr int FIN_BLOCK_F = FIN_THREADS / FIN_SL;
     __shared__ double s_var;
+    __shared__ double s_part[FIN_SL > 1 ? 6 : 1][FIN_SL][FIN_SL > 1 ? FIN_BLOCK_F : 1];
     __shared__ u64 s_best[FIN_THREADS / 32];
     const int64_t b = blockIdx.y;
+    const int fl = threadIdx.x % FIN_BLOCK_F, sl = threadIdx.x / FIN_BLOCK_F;
+    pdl_wait();                                            // (launched as a programmatic dependent of the accumulate kernel on the short-grid path)
     if (threadIdx.x == 0) {
         double q = 0.0;                                    // fixed-order sum of the block partials
         for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
@@ -47,19 +89,16 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
             s_var *= xs * xs;
         }
     }
-    __syncthreads();
-    const double inv2var = 0.5 / s_var;
-    const double Nt = (double)p.Nt;
     const float* ws = p.ws_x ? p.ws : p.ws + b * p.nsplit * 4 * p.Nf;
     const float* wx = p.ws_x ? p.ws_x + b * p.nsplit * 2 * p.x_row : nullptr;
+    const float* w1 = p.ws1 ? p.ws1 + b * p.nsplit * 4 * p.Nf : nullptr;
+    const int64_t k = (int64_t)blockIdx.x * FIN_BLOCK_F + fl;
+    const bool live = k < p.Nf;
 
-    u64 best = 0ull;
-    #pragma unroll
-    for (int i = 0; i < FIN_FPT; ++i) {
-        const int64_t k = ((int64_t)blockIdx.x * FIN_FPT + i) * FIN_THREADS + threadIdx.x;
-        if (k >= p.Nf) continue;
-        double XC = 0.0, XS = 0.0, CCh = 0.0, CS = 0.0;
-        for (int sp = 0; sp < p.nsplit; ++sp) {            // fixed order over the time splits
+    double XC = 0.0, XS = 0.0, CCh = 0.0, CS = 0.0, C1 = 0.0, S1 = 0.0;
+    if (live) {
+        #pragma unroll 2
+        for (int sp = sl; sp < p.nsplit; sp += FIN_SL) {   // fixed order over this lane's time splits
             const float* w = ws + (int64_t)sp * 4 * p.Nf + k;
             if (wx) {
                 XC += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + k);
@@ -70,60 +109,47 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
             }
             CCh += (double)__ldg(w + 2 * p.Nf);
             CS += (double)__ldg(w + 3 * p.Nf);
-        }
-        if (p.ws1) {
-            // Generalised (floating-mean) periodogram of Zechmeister & Kuerster 2009 (named at PAPER.md:375), unit
-            // weights; the series is already mean-subtracted, so Y = 0 and YC = XC/N, YS = XS/N:
-            //   CCn = CC/N - (C/N)^2, SSn = SS/N - (S/N)^2, CSn = CS/N - C S/N^2, D = CCn SSn - CSn^2
-            //   P = (SSn XC^2 + CCn XS^2 - 2 CSn XC XS) / (2 var N D)        [same normalisation as eq. (1)]
-            double C1 = 0.0, S1 = 0.0;
-            const float* w1 = p.ws1 + b * p.nsplit * 4 * p.Nf;
-            for (int sp = 0; sp < p.nsplit; ++sp) {
+            if (w1) {
                 C1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + k);
                 S1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + p.Nf + k);
             }
-            const double cm = C1 / Nt, sm = S1 / Nt;
-            const double CCn = 0.5 + CCh / Nt - cm * cm, SSn = 0.5 - CCh / Nt - sm * sm, CSn = CS / Nt - cm * sm;
-            const double D = CCn * SSn - CSn * CSn;
-            double val = 0.0;
-            if (D > 1e-9) val = fmax(SSn * XC * XC + CCn * XS * XS - 2.0 * CSn * XC * XS, 0.0) / (Nt * D) * inv2var;   // singular fit (f -> 0): 0, reading G7
-            const float Pf = (float)val;
-            if (p.P) p.P[b * p.p_stride + k] = Pf;
-            const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
-            best = (key > best) ? key : best;
-            continue;
         }
-        // The two terms of eq. (5) over the common denominator (Nt + R)(Nt - R) = Nt^2 - R^2: one fp64 division, no square root:
-        //   P 2 var = (S + D)/(Nt + R) + (S - D)/(Nt - R) = 2 (S Nt - D R) / (Nt^2 - R^2),   D R = (XC^2 - XS^2) A + 2 XC XS B
-        const double A = 2.0 * CCh, Bv = 2.0 * CS;
-        const double R2 = A * A + Bv * Bv;
-        const double xc2 = XC * XC, xs2 = XS * XS;
-        const double S = xc2 + xs2;
-        const double DR = (xc2 - xs2) * A + 2.0 * XC * XS * Bv;
-        double val;
-        if (R2 < (1.0 - 1e-6) * (1.0 - 1e-6) * Nt * Nt) {
-            val = fmax(2.0 * (S * Nt - DR), 0.0) / (Nt * Nt - R2);
-        } else {                                                        // Nt - R <= 1e-6 Nt: the 0/0 term is dropped (reading G7)
-            const double R = sqrt(R2);
-            val = fmax(S + DR / R, 0.0) / (Nt + R);
-        }
-        val *= inv2var;
-        const float Pf = (float)val;
-        if (p.P) p.P[b * p.p_stride + k] = Pf;
-        const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
-        best = (key > best) ? key : best;
     }
+    if (FIN_SL > 1) {
+        s_part[0][sl][fl] = XC; s_part[1][sl][fl] = XS; s_part[2][sl][fl] = CCh; s_part[3][sl][fl] = CS;
+        s_part[4][sl][fl] = C1; s_part[5][sl][fl] = S1;
+    }
+    __syncthreads();                                       // s_var; the lanes' partial sums
+    if (sl != 0) return;                                   // (whole warps: FIN_BLOCK_F is a multiple of 32)
 
+    u64 best = 0ull;
+    if (live) {
+        double v[6] = {XC, XS, CCh, CS, C1, S1};
+        if (FIN_SL > 1) {
+            #pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                double a = 0.0;
+                #pragma unroll
+                for (int l = 0; l < FIN_SL; ++l) a += s_part[q][l][fl];   // fixed order over the lanes
+                v[q] = a;
+            }
+        }
+        const float Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, p.ws1 != nullptr);
+        if (p.P) p.P[b * p.p_stride + k] = Pf;
+        best = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+    }
     if (p.peak_idx == nullptr) return;
     #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         const u64 other = __shfl_down_sync(0xffffffffu, best, o);
         best = (other > best) ? other : best;
     }
-    if ((threadIdx.x & 31) == 0) s_best[threadIdx.x >> 5] = best;
-    __syncthreads();
+    if (FIN_SL == 1) {                                     // eight warps: fold them through shared memory first
+        if ((threadIdx.x & 31) == 0) s_best[threadIdx.x >> 5] = best;
+        __syncthreads();
+        if (threadIdx.x == 0) for (int i = 1; i < FIN_THREADS / 32; ++i) best = (s_best[i] > best) ? s_best[i] : best;
+    }
     if (threadIdx.x == 0) {
-        for (int i = 1; i < FIN_THREADS / 32; ++i) best = (s_best[i] > best) ? s_best[i] : best;
         atomicMax(p.peak64 + b, best);
         __threadfence();
         const unsigned done = atomicAdd(p.counter + b, 1u);

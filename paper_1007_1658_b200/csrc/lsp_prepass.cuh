@@ -89,8 +89,9 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
 
 // grid (nb, B).  Writes recA, recB for the block's chunk and part_var[b][blk] = sum (x - mean)^2.
 // SHARED (shared-time batch, t_stride = 0): only X_j is needed per series, the phases only once (series 0).
-// FUSED (one block per series, Nt <= 4,096): step 1's sum is formed here, exactly as moments_kernel forms it (same strided
-// partials, same reduction tree), so one launch is saved where launches are what a call costs (C1, C2, C4).
+// FUSED (short series, Nt <= 16,384): step 1's sum is formed here -- by EVERY block of the series, over the whole series, with
+// the same strided partials and reduction tree, so all blocks hold the identical mean -- and one launch is saved where
+// launches are what a call costs (C1, C2, C4); the blocks then share the O(Nt) fp64 record work.
 template <bool SHARED, bool FUSED>
 __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                const float* __restrict__ x, int64_t x_stride,
@@ -101,17 +102,21 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                u64* __restrict__ peak64, unsigned* __restrict__ counter)
 {
     __shared__ double red[32];
+    pdl_trigger();                                         // the accumulate kernel may be scheduled now; it waits (pdl_wait) for this grid to finish
     const int b = blockIdx.y;
     const int nb = gridDim.x;
     const double* tb = t + (int64_t)b * t_stride;
     const float* xb = x + (int64_t)b * x_stride;
 
     double s = 0.0;                                        // fixed-order sum of the block partials
-    if (FUSED) {                                           // gridDim.x == 1
+    if (FUSED) {
         double a0 = 0.0;
         for (int64_t j = threadIdx.x; j < Nt; j += blockDim.x) a0 += (double)__ldg(xb + j);
         s = block_sum(a0, red);
-        if (threadIdx.x == 0) { part_sum[b] = s; peak64[b] = 0ull; counter[b] = 0u; }
+        if (threadIdx.x == 0) {                            // part_sum keeps its meaning for later readers: its entries add up to sum x
+            part_sum[(int64_t)b * nb + blockIdx.x] = blockIdx.x == 0 ? s : 0.0;
+            if (blockIdx.x == 0) { peak64[b] = 0ull; counter[b] = 0u; }
+        }
         __syncthreads();                                   // `red` is reused below
     } else
     for (int i = 0; i < nb; ++i) s += part_sum[(int64_t)b * nb + i];

@@ -151,14 +151,16 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t tabl
 }
 
 // ---- workspace layouts (byte offsets into the handle's buffer)
+constexpr int64_t SHARED_E_BUDGET_DEFAULT = (int64_t)256 << 20;   // bytes of workspace the E tiles of the shared-time GEMM may take (per band)
+
 struct SharedLayout {
-    int64_t nsplit, gps, ng, nmb, nfb, x_row;
+    int64_t nsplit, gps, ng, nmb, nfb, x_row, band_nfb;
     bool fuse;
     size_t recB, xa, eb, wsv, wsx, vc, vcf, psum, pvar, peak, cnt, total;
 };
 
 // Shared-time batch: false if the sizes do not fit the kernel's grid.
-bool shared_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, SharedLayout& L)
+bool shared_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, int64_t e_budget, SharedLayout& L)
 {
     int64_t nsplit = (Nt + SG_MAX_SPLIT - 1) / SG_MAX_SPLIT;
     int64_t gps = ((Nt + nsplit - 1) / nsplit + SG_KS - 1) / SG_KS;
@@ -172,7 +174,14 @@ bool shared_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, SharedLayo
     size_t off = 0;
     L.recB = off; off = align_up(off + (size_t)Nt * sizeof(ulonglong2), 256);   // phases of the one time vector
     L.xa = off;   off = align_up(off + (size_t)L.nmb * L.ng * SG_A_GROUP, 256);
-    L.eb = off;   off = align_up(off + (size_t)L.nfb * L.ng * SG_B_GROUP, 256);
+    // E = 8 bytes per (sample, frequency): made and consumed one band of frequency blocks at a time, so it takes O(Nt * band), not O(Nt * Nf)
+    int64_t band = (e_budget > 0 ? e_budget : SHARED_E_BUDGET_DEFAULT) / (L.ng * (int64_t)SG_B_GROUP);
+    const int64_t fill = (2 * 148 + L.nmb * nsplit - 1) / (L.nmb * nsplit);      // a band launch should still fill the device (two CTAs per SM)
+    if (band < fill) band = fill;
+    if (band > L.nfb) band = L.nfb;
+    if (band < 1) band = 1;
+    L.band_nfb = band;
+    L.eb = off;   off = align_up(off + (size_t)band * L.ng * SG_B_GROUP, 256);
     L.wsv = off;  off = align_up(off + (size_t)nsplit * 4 * (size_t)Nf * sizeof(float), 256);
     L.wsx = off;  if (!L.fuse) off = align_up(off + (size_t)B * nsplit * 2 * (size_t)L.x_row * sizeof(float), 256);
     L.vc = off;   off = align_up(off + (size_t)4 * (size_t)Nf * sizeof(double), 256);
@@ -255,11 +264,12 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
 {
     Plan pl = make_plan(h, B, Nt, Nf, 1);                 // pre-pass partition only
     SharedLayout L;
-    if (!shared_layout(pl, B, Nt, Nf, L)) return LSP_EINVAL;
+    if (!shared_layout(pl, B, Nt, Nf, h->opt_table_mb << 20, L)) return LSP_EINVAL;
     const int64_t nsplit = L.nsplit, gps = L.gps, ng = L.ng, nmb = L.nmb, nfb = L.nfb, x_row = L.x_row;
+    const int64_t nbands = (nfb + L.band_nfb - 1) / L.band_nfb;
     const bool fuse = L.fuse;
     pl.pipe = PLAN_PIPE_TENSOR; pl.K = SG_F; pl.T = SG_THREADS; pl.nsplit = (int)nsplit; pl.nfb = (int)nfb; pl.L = 0;
-    pl.split_len = gps * SG_KS; pl.launches = 7; pl.nchunks = 1; pl.chunk_len = 0;
+    pl.split_len = gps * SG_KS; pl.launches = 5 + 2 * (int)nbands; pl.nchunks = (int)nbands; pl.chunk_len = 0;
     pl.kernel_name = fuse ? "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times,fused-finish>"
                           : "shared_gemm_kernel<tcgen05.m128n256.f16+e5m2corr,TMA-fed,shared-times>";
 
@@ -299,9 +309,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     if (fused_pre) records_kernel<true, true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
-    // step 3 for every (sample, frequency) once; CC, CS once per frequency
-    shared_e_kernel<<<dim3((unsigned)nfb, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng);
-    LSP_CUDA(h, cudaGetLastError());
+    // CC, CS once per frequency
     shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
     LSP_CUDA(h, cudaGetLastError());
     if (fuse) {
@@ -310,16 +318,24 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     }
     shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(x, x_stride, psum, pvar, pl.nparts, B, Nt, xa, (int)ng);
     LSP_CUDA(h, cudaGetLastError());
-    if (timing) LSP_CUDA(h, cudaEventRecord(ev[2], st));
-    // steps 4-5: the contraction
+    // step 3 for every (sample, frequency) once, and steps 4-5, the contraction: one band of frequency blocks at a time
+    // (E tiles of the band -> GEMM over the band; the same buffer serves every band)
     SharedGemmParams gp;
     gp.xa = xa; gp.eb = eb; gp.ws_x = ws_x; gp.B = B; gp.Nf = Nf; gp.x_row = x_row;
-    gp.nmb = (int)nmb; gp.nfb = (int)nfb; gp.nsplit = (int)nsplit; gp.ng = (int)ng; gp.groups_per_split = (int)gps;
+    gp.nmb = (int)nmb; gp.nfb_total = (int)nfb; gp.nsplit = (int)nsplit; gp.ng = (int)ng; gp.groups_per_split = (int)gps;
     gp.vconst = fuse ? vconst : nullptr; gp.vconst_f = vconst_f; gp.part_var = pvar; gp.P = P; gp.p_stride = p_stride;
     gp.peak_idx = peak_idx; gp.peak_val = peak_val; gp.peak64 = peak64; gp.counter = counter; gp.Nt = Nt; gp.nparts = pl.nparts;
     LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
-    shared_gemm_kernel<<<(unsigned)(nmb * nfb * nsplit), SG_THREADS, SG_SMEM, st>>>(gp);
-    LSP_CUDA(h, cudaGetLastError());
+    for (int64_t band = 0; band < nbands; ++band) {
+        const int64_t nb0 = band * L.band_nfb;
+        const int64_t nb_n = (nfb - nb0 < L.band_nfb) ? nfb - nb0 : L.band_nfb;
+        shared_e_kernel<<<dim3((unsigned)nb_n, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng, (int)nb0);
+        LSP_CUDA(h, cudaGetLastError());
+        if (timing && band == 0) LSP_CUDA(h, cudaEventRecord(ev[2], st));
+        gp.nb0 = (int)nb0; gp.nfb = (int)nb_n;
+        shared_gemm_kernel<<<(unsigned)(nmb * nb_n * nsplit), SG_THREADS, SG_SMEM, st>>>(gp);
+        LSP_CUDA(h, cudaGetLastError());
+    }
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
     if (fuse) {                                           // steps 6-7 ran in the GEMM's epilogue
         if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
@@ -667,7 +683,7 @@ int lsp_reserve(lsp_handle h, int64_t B, int shared_t, int64_t Nt, int64_t Nf, i
     if (use_shared_path(h, t_stride, B, Nt, gls)) {
         const Plan pl = make_plan(h, B, Nt, Nf, 1);
         SharedLayout L;
-        if (!shared_layout(pl, B, Nt, Nf, L)) return LSP_EINVAL;
+        if (!shared_layout(pl, B, Nt, Nf, h->opt_table_mb << 20, L)) return LSP_EINVAL;
         need = L.total;
     } else {
         Route r;

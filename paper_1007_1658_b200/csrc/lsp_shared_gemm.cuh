@@ -41,10 +41,11 @@ constexpr uint32_t SG_IDESC = umma_idesc(SG_M, 2 * SG_F);
 
 struct SharedGemmParams {
     const unsigned char* xa;        // [nmb][ng][SG_A_GROUP]
-    const unsigned char* eb;        // [nfb][ng][SG_B_GROUP]
+    const unsigned char* eb;        // [nfb][ng][SG_B_GROUP]: the E tiles of ONE BAND of nfb frequency blocks starting at block nb0
     float* ws_x;                    // [B][nsplit][2][x_row]
     int64_t B, Nf, x_row;
-    int nmb, nfb, nsplit, ng;       // ng = k-step groups over ALL splits = nsplit * groups_per_split
+    int nmb, nfb, nsplit, ng;       // ng = k-step groups over ALL splits = nsplit * groups_per_split; nfb = frequency blocks of this launch (band)
+    int nb0, nfb_total;             // first frequency block of the band; blocks of the whole grid (the last one publishes the peak)
     int groups_per_split;           // even
     // fused steps 6-7 (only when nsplit == 1: the accumulators ARE the sums of eq. (8)); vconst == NULL: write ws_x instead
     const double* vconst;           // [4][Nf]: cos 2 w tau, sin 2 w tau, 1/(Nt + R), 1/(Nt - R) (0 if dropped, reading G7)
@@ -75,13 +76,14 @@ __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restr
 }
 
 // ------------------------------------------------------------------ E tiles + partial CC, CS
-// grid (nfb, ng), 256 threads: kf = tid & 127 (frequency k = 128 nfb + kf), chunk = tid >> 7 (8 of the group's 16 samples).
+// grid (band blocks, ng), 256 threads: kf = tid & 127 (frequency k = 128 (nb0 + block) + kf), chunk = tid >> 7 (8 of the group's
+// 16 samples).  E is made one BAND of frequency blocks at a time (the host bounds the buffer), block `nb` of the band at eb[nb].
 __global__ void __launch_bounds__(256) shared_e_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t Nf,
-                                                       unsigned char* __restrict__ eb, int ng)
+                                                       unsigned char* __restrict__ eb, int ng, int nb0)
 {
     const int nb = blockIdx.x, g = blockIdx.y;
     const unsigned kf = threadIdx.x & 127u, chunk = threadIdx.x >> 7;
-    const int64_t k = (int64_t)nb * SG_F + kf;
+    const int64_t k = (int64_t)(nb0 + nb) * SG_F + kf;
     float c[8], s[8];
     #pragma unroll
     for (int i = 0; i < 8; ++i) {
@@ -200,7 +202,7 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
             float vc[32], vs[32];
             tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, vc);
             tmem_ld32(tmem + ((32u * q4) << 16) + 128u + 32u * cc, vs);
-            const int64_t k0 = (int64_t)nb * SG_F + cc * 32;
+            const int64_t k0 = (int64_t)(p.nb0 + nb) * SG_F + cc * 32;
             if (b >= p.B) continue;
             float pf[32];
             // branch-free fp32 pass: the 32 loads and combines pipeline.  Frequencies with R > Nt/2 carry cf.x = NaN, come out
@@ -249,7 +251,7 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
             atomicMax(p.peak64 + b, best);
             __threadfence();
             const unsigned done = atomicAdd(p.counter + b, 1u);
-            if (done == (unsigned)p.nfb - 1u) {                     // last frequency block of this series: publish
+            if (done == (unsigned)p.nfb_total - 1u) {               // last frequency block of this series (over all bands): publish
                 __threadfence();
                 const u64 fin = atomicMax(p.peak64 + b, 0ull);
                 p.peak_idx[b] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
@@ -262,7 +264,7 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
     for (int cc = 0; cc < 8; ++cc) {
         float v[32];
         tmem_ld32(tmem + ((32u * q4) << 16) + 32u * cc, v);
-        const int64_t k0 = (int64_t)nb * SG_F + (cc & 3) * 32;
+        const int64_t k0 = (int64_t)(p.nb0 + nb) * SG_F + (cc & 3) * 32;
         float* d = dst + (int64_t)(cc >> 2) * p.x_row + k0;
         if (b < p.B) {
             #pragma unroll

@@ -193,3 +193,34 @@ def test_C3_run_to_run_bit_identical(lsp):
             assert "pair2" in h.last_plan()["kernel"]
         else:
             assert torch.equal(P, first)
+
+
+def test_shared_time_large_grid_bounded_workspace(lsp):
+    """a shared-time call at Nt = 2,048, Nf = 200,000, B = 256 (8 B x Nt x Nf = 3.3 GB of E tiles if
+    materialised at once) runs in frequency bands within the default 256 MiB; sampled series and frequencies against the oracle."""
+    pkg, h = lsp
+    B, Nt, Nf = 256, 2048, 200000
+    rng = np.random.default_rng(20481)
+    t = np.sort(rng.uniform(0.0, 200.0, Nt))
+    x = rng.standard_normal((B, Nt)).astype(np.float32)
+    x[7] += (0.3 * np.sin(2 * np.pi * 3.21 * t)).astype(np.float32)
+    f_min, f_max = 1.0 / 200.0, 40.0
+    df = (f_max - f_min) / (Nf - 1)
+    import torch
+    td, xd = torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda()
+    P, pi, pv = h.periodogram_batched(td, xd, f_min, df, Nf)
+    torch.cuda.synchronize()
+    plan = h.last_plan()
+    assert "shared_gemm" in plan["kernel"]
+    nbands = (plan["launches"] - 4) // 2
+    assert nbands >= 10, plan                                  # 1,563 blocks of 2 MiB each in bands of 128
+    P, pi, pv = P.cpu().numpy(), pi.cpu().numpy(), pv.cpu().numpy()
+    assert np.array_equal(pi, P.argmax(axis=1).astype(np.int32)) and np.array_equal(pv, P.max(axis=1))
+    ks = np.unique(np.concatenate([np.arange(0, Nf, 997), np.arange(Nf - 64, Nf), np.arange(128 * 128 - 32, 128 * 128 + 32),
+                                   np.arange(max(0, int(pi[7]) - 32), min(Nf, int(pi[7]) + 33))])).astype(np.int64)
+    for b in (0, 7, 130, 255):
+        ref = oracle.periodogram(t, x[b], f_min, df, Nf, ks=ks)
+        err = np.max(np.abs(P[b][ks] - ref)) / ref.max()
+        assert err <= 1e-4, (b, err)
+    inj = int(round((3.21 - f_min) / df))
+    assert abs(int(pi[7]) - inj) <= 2

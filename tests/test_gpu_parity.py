@@ -522,6 +522,31 @@ def test_shared_time_gemm(lsp, B, Nt, Nf):
             assert _same_peak(out[2][b], Pref[b], "shared gemm")
 
 
+def test_shared_time_gemm_frequency_bands(lsp):
+    """The E operand of the shared-time GEMM (8 bytes per sample and frequency) is made and consumed one BAND of frequency
+    blocks at a time, so the workspace is O(Nt x band), not O(Nt x Nf).  A 1 MiB budget forces bands (ragged last band) here;
+    the result must be bit-identical to the single-band call (each output element is computed by one CTA either way), the
+    peaks must merge across the bands, and sampled series must match the oracle."""
+    pkg, h = lsp
+    B, Nt, Nf = 24, 640, 50021                                 # 391 frequency blocks
+    w0 = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=4242)
+    w = workloads.Workload("c4-shared-bands", np.broadcast_to(w0.t[0], w0.t.shape).copy(), w0.x, w0.f_min, w0.df, w0.Nf, B=B)
+    P1, pi1, pv1, plan1 = _run_batched(h, w, shared_t=True, shared=2)
+    assert "shared_gemm" in plan1["kernel"] and plan1["launches"] == 4 + 2 * 1       # (records with the mean fused: one launch fewer)
+    P2, pi2, pv2, plan2 = _run_batched(h, w, shared_t=True, shared=2, table_mb=1)
+    assert plan2["launches"] == 4 + 2 * 2, plan2                                      # 296 + 95 blocks
+    assert np.array_equal(P1, P2) and np.array_equal(pi1, pi2) and np.array_equal(pv1, pv2)
+    assert np.array_equal(pi2, P2.argmax(axis=1).astype(np.int32)) and np.array_equal(pv2, P2.max(axis=1))
+    for b in (0, 11, 23):
+        ref = oracle.periodogram(w.t[b], w.x[b], w.f_min, w.df, w.Nf)
+        _check(P2[b], ref, "banded shared gemm series %d" % b)
+        if _top_two_gap(ref) >= QUAL_GAP:
+            assert int(pi2[b]) == oracle.argmax(ref)
+    # peaks only (P = NULL) through the bands
+    _, pi3, pv3, _ = _run_batched(h, w, shared_t=True, shared=2, table_mb=1, want_P=False)
+    assert np.array_equal(pi3, pi2) and np.array_equal(pv3, pv2)
+
+
 @pytest.mark.parametrize("B,Nt,Nf,nsplit", [(5, 900, 2100, 0), (2, 1500, 2000, 0), (7, 3000, 5000, 2), (3, 600, 700, 0)])
 @pytest.mark.parametrize("gls", [False, True])
 def test_two_series_per_cta_form(lsp, B, Nt, Nf, nsplit, gls):

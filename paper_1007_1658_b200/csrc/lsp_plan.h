@@ -5,7 +5,8 @@
 // The accumulate grid is B * nfb * nsplit equal-sized CTAs ("units") handed out by the hardware block scheduler.
 // Three effects decide the run time of the FP32 form and are modelled here (constants measured on B200):
 //   fill      frequencies actually needed / frequencies the nfb blocks cover (ragged last block)
-//   body      FFMA2 stream vs per-sample anchor overhead: 6K / (6K + 16) FMA-pipe cycles
+//   body      FFMA2 stream vs the per-sample fixed cost (anchor, loop, register moves): 6K / (6K + 44) FMA-pipe cycles per
+//             sample and warp (measured on B200 for K = 16 ... 48: 232 cycles at K = 32, 144 at K = 16; round 2)
 //   waves     units / CTA slots is rarely an integer; the last, partly filled wave costs a full
 //             unit time (measured: 8.28 waves ran as 9 => 8 % idle), so nsplit is chosen to make
 //             the wave count large and just below an integer
@@ -170,7 +171,7 @@ inline PlanChoice plan_choose_fp32(int sm_count, int64_t B, int64_t Nt, int64_t 
             const int64_t fb = (int64_t)K * T;
             const int64_t nfb = (Nf + fb - 1) / fb;
             const double fill = (double)Nf / (double)(nfb * fb);
-            const double body = 6.0 * K / (6.0 * K + 16.0);
+            const double body = 6.0 * K / (6.0 * K + 44.0);
             const double wps = cta * T / 128.0;                     // warps per SM sub-partition
             const double occ = wps >= 3.0 ? 1.0 : (wps >= 2.0 ? 0.93 : (wps >= 1.0 ? 0.72 : 0.72 * wps));
             const int64_t slots = (int64_t)cta * sm_count;

@@ -3,8 +3,9 @@
 // number of time-axis splits and, for the table-fed CTA-pair form, the time chunks that bound the table.
 //
 // The accumulate grid is B * nfb * nsplit equal-sized CTAs ("units") handed out by the hardware block scheduler.
-// Three effects decide the run time of the FP32 form and are modelled here (constants measured on B200):
-//   fill      frequencies actually needed / frequencies the nfb blocks cover (ragged last block)
+// The run time of the FP32 form is modelled as waves x (time of one wave of resident CTAs), score = ideal cycles / estimate
+// (constants measured on B200).  What enters:
+//   fill      frequencies actually needed / frequencies the nfb blocks cover (ragged last block): through the CTA count
 //   body      FFMA2 stream vs the per-sample fixed cost (anchor, loop, register moves): 6K / (6K + 44) FMA-pipe cycles per
 //             sample and warp (measured on B200 for K = 16 ... 48: 232 cycles at K = 32, 144 at K = 16; round 2)
 //   waves     units / CTA slots is rarely an integer; the last, partly filled wave costs a full
@@ -44,13 +45,15 @@ inline int plan_regs(int K) {
     return z[K / 4];
 }
 
-inline int64_t plan_smem_bytes(int K, int T) { return (int64_t)PLAN_TILE_Z * 24 + (int64_t)T * (4 * K + 1) * 4; }
+constexpr int64_t PLAN_FOLD_SAMPLES = 2048;                        // default fold interval of the FP32-pipe kernel's register partials
+// a split inside one fold interval needs no shared-memory accumulators (accum_z_kernel<..., DIRECT>)
+inline int64_t plan_smem_bytes(int K, int T, bool direct = false) { return (int64_t)PLAN_TILE_Z * 24 + (direct ? 0 : (int64_t)T * (4 * K + 1) * 4); }
 
 // resident CTAs per SM (B200: 64K registers, 228 KB shared memory with 1 KB reserved per CTA, 64 warps)
-inline int plan_ctas_per_sm(int K, int T) {
+inline int plan_ctas_per_sm(int K, int T, bool direct = false) {
     const int regs = (plan_regs(K) + 7) / 8 * 8;
     int by_regs = 65536 / (regs * T);
-    int by_smem = (int)((int64_t)233472 / (plan_smem_bytes(K, T) + 1024));
+    int by_smem = (int)((int64_t)233472 / (plan_smem_bytes(K, T, direct) + 1024));
     int by_warps = 2048 / T;
     int c = by_regs < by_smem ? by_regs : by_smem;
     if (by_warps < c) c = by_warps;
@@ -166,15 +169,11 @@ inline PlanChoice plan_choose_fp32(int sm_count, int64_t B, int64_t Nt, int64_t 
         for (int ti = 0; ti < nT; ++ti) {
             const int T = Ts[ti];
             if (T > plan_max_threads(K)) continue;
-            const int cta = plan_ctas_per_sm(K, T);
-            if (cta < 1) continue;
+            if (plan_ctas_per_sm(K, T) < 1) continue;
             const int64_t fb = (int64_t)K * T;
             const int64_t nfb = (Nf + fb - 1) / fb;
             const double fill = (double)Nf / (double)(nfb * fb);
             const double body = 6.0 * K / (6.0 * K + 44.0);
-            const double wps = cta * T / 128.0;                     // warps per SM sub-partition
-            const double occ = wps >= 3.0 ? 1.0 : (wps >= 2.0 ? 0.93 : (wps >= 1.0 ? 0.72 : 0.72 * wps));
-            const int64_t slots = (int64_t)cta * sm_count;
             // workspace cap: B * nsplit * 16 bytes * Nf <= 2 GiB
             int64_t cap = ((int64_t)1 << 31) / (B * 16 * Nf);
             if (cap < 1) cap = 1;
@@ -187,11 +186,21 @@ inline PlanChoice plan_choose_fp32(int sm_count, int64_t B, int64_t Nt, int64_t 
                 len = (len + tile - 1) / tile * tile;
                 const int64_t n_eff = (Nt + len - 1) / len;         // splits actually produced
                 if (n_eff != n && !ov.nsplit) continue;             // duplicate of a smaller n
+                const int cta = plan_ctas_per_sm(K, T, len <= PLAN_FOLD_SAMPLES);   // short splits keep their sums in registers: more CTAs per SM
+                const int64_t slots = (int64_t)cta * sm_count;
                 const int64_t units = B * nfb * n_eff;
-                const double wave = plan_wave_eff(units, slots);
+                // CTAs actually resident per SM: `cta` when the grid fills the machine, fewer when it does not (C1, C2) -- then what
+                // counts is how long ONE CTA takes, so short splits and small K win, not the per-term efficiency of a full machine
+                const int64_t resident = units >= slots ? cta : (units + sm_count - 1) / sm_count;
+                double wps = resident * T / 128.0;                  // warps per SM sub-partition
+                if (wps < 1.0) wps = 1.0;
+                const double occ = wps >= 3.0 ? 1.0 : (wps >= 2.0 ? 0.93 : 0.72);
+                const int64_t waves = units >= slots ? (units + slots - 1) / slots : 1;
                 const double avg_len = (double)Nt / (double)n_eff;
-                const double unit = avg_len / (avg_len + 40.0);
-                const double score = fill * body * occ * wave * unit;
+                const double est = (double)waves * (avg_len + 40.0) * (6.0 * K + 44.0) * wps / occ;   // SM cycles
+                const double ideal = (double)B * (double)Nt * (double)Nf * 6.0 / (128.0 * sm_count);
+                const double score = ideal / est;
+                (void)fill; (void)body;
                 if (score > best.score * 1.0025 || best.K == 0) {   // prefer earlier (larger K, fewer splits) on near-ties
                     best.K = K; best.T = T; best.nsplit = (int)n_eff; best.pipe = PLAN_PIPE_FP32; best.nfb = (int)nfb;
                     best.ctas_per_sm = cta; best.split_len = len; best.score = score;

@@ -75,8 +75,9 @@ enum {
     LSP_PARAM_TRUNC     = 9,  /* tensor form, CTA-pair kernel: 1 = do not add the expected round-toward-zero loss of the       */
                               /* tensor-core accumulation back at each drain; 0 = add it (default)       */
     LSP_PARAM_SHARED    = 11, /* batched call with t_stride = 0: 0 = the shared-time GEMM path when B >= 16 and Nt >= 512, 1 = never, 2 = always */
-    LSP_PARAM_PDL       = 13  /* short-grid tensor path: 0 = pre-pass -> accumulate -> finish launched as programmatic dependents       */
-                              /* (each kernel's launch and set-up overlap its predecessor's tail), 1 = plain stream order              */
+    LSP_PARAM_PDL       = 13  /* short-grid tensor path: 0 = steps 1-2 run inside the accumulate kernel when Nt <= 16,384 (two launches per  */
+                              /* call) and the kernels of a call are launched as programmatic dependents (each kernel's launch and      */
+                              /* set-up overlap its predecessor's tail); 1 = separate pre-pass kernels in plain stream order            */
 };
 enum { LSP_PIPE_AUTO = 0, LSP_PIPE_FP32 = 1, LSP_PIPE_TENSOR = 2 };
 

@@ -356,7 +356,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
 }
 
 // What the call will run (shared by run_device and lsp_reserve).
-struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair; int64_t tab_series; };
+struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair, fuse_pre; int64_t tab_series; };
 
 int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf, bool gls, Route& r, bool weighted = false)
 {
@@ -386,6 +386,9 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
                        : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
                                      : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
     }
+    // short grids, short series: steps 1-2 inside the accumulate kernel (accum_umma_small_kernel<..., FUSED_PRE>): two launches per call
+    r.fuse_pre = r.small && !r.duo && !gls && !weighted && Nt <= 16384 && h->opt_pdl != 1;
+    if (r.fuse_pre) { pl.launches = 2; pl.nparts = 1; pl.part_chunk = Nt; pl.fused_pre = false; }
     if (gls) pl.launches += 1 + (r.pair ? pl.nchunks : 1);   // unit records + second accumulate pass
     const int64_t units = (r.duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
@@ -443,6 +446,9 @@ int run_device(lsp_ctx* h,
     // steps 1-2
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
     const bool fused_pre = pl.fused_pre && !weighted;      // short series: step 1's sum inside the records kernel
+    if (r.fuse_pre) {                                     // (done by the accumulate kernel itself)
+        if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
+    } else {
     if (!fused_pre) {
         moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter, w, w_stride, pw);
         LSP_CUDA(h, cudaGetLastError());
@@ -452,6 +458,7 @@ int run_device(lsp_ctx* h,
     else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
     LSP_CUDA(h, cudaGetLastError());
+    }
     if (weighted) pl.launches -= 1;                       // (the weight records were written by records_weighted_kernel)
     if (gls && !weighted) {
         unit_records_kernel<<<(unsigned)((n_samp + 255) / 256), 256, 0, st>>>(recA, recA1, (int64_t)n_samp);
@@ -513,6 +520,8 @@ int run_device(lsp_ctx* h,
                 up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
                 up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
                 up.flush_ksteps = flush_ksteps; up.trunc_ulps = 0.f; up.unit_x = pass;
+                up.t = t; up.t_stride = t_stride; up.x = x; up.x_stride = x_stride; up.f_min = f_min; up.df = df;
+                up.part_var_out = pvar; up.peak64 = peak64; up.counter = counter;
                 if (r.duo) {
                     UmmaDuoParams dp;
                     dp.u = up; dp.B = B;
@@ -522,8 +531,12 @@ int run_device(lsp_ctx* h,
                     accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
                 } else {
 #define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
+                    if (r.fuse_pre) { \
+                    LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
+                    accum_umma_small_kernel<LL, NS, MINB, true><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); \
+                    LSP_CUDA(h, cudaGetLastError()); } else { \
                     LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
-                    LSP_CUDA(h, launch_pdl(accum_umma_small_kernel<LL, NS, MINB>, dim3((unsigned)units), dim3(US_THREADS), UmmaSmall<LL, NS>::SMEM, st, pdl_small, up)); } while (0)
+                    LSP_CUDA(h, launch_pdl(accum_umma_small_kernel<LL, NS, MINB>, dim3((unsigned)units), dim3(US_THREADS), UmmaSmall<LL, NS>::SMEM, st, pdl_small, up)); } } while (0)
                     if (pl.L == 16) LSP_LAUNCH_SMALL(16, 4, 3);
                     else if (pl.L == 32) LSP_LAUNCH_SMALL(32, 4, 2);
                     else if (pl.L == 64) LSP_LAUNCH_SMALL(64, 4, 2);

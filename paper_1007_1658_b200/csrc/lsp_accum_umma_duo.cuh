@@ -198,23 +198,29 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
 
     if (w < US_GEN_WARPS) {
         // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
+        // Everything that does not change from k-step to k-step is formed once, here, and the loop below only advances a few
+        // 32-bit counters: the loop overhead was 40 % of the instructions of this generation-bound kernel (round 2).
         // record loader role: thread tid -> series tid >> 7, sample tid & 127 of the tile
         const unsigned ls = tid >> 7, lj = tid & 127u;
         const int64_t lb = 2 * bp + ls;
         const bool l_live = lb < q.B;
-        const float4* recA = p.recA + (l_live ? lb : 0) * p.Nt;
-        const ulonglong2* recB = p.recB + (l_live ? lb : 0) * p.Nt;
+        const float* recAx = &p.recA[(l_live ? lb : 0) * p.Nt + j_begin].x;      // .x of the split's first record (stride 4 floats)
+        const ulonglong2* recB = p.recB + (l_live ? lb : 0) * p.Nt + j_begin;
         const float xs = l_live ? (p.unit_x ? 1.f : x_scale(p.part_var + lb * p.nparts, p.nparts, p.Nt)) : 0.f;
-        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
-        auto prefetch = [&](int ti) {
-            const int64_t j = j_begin + (int64_t)ti * UM_TS + lj;
-            pre_ok = l_live && (j < j_end);
-            if (pre_ok) { pre_x = __ldg(&recA[j].x); const ulonglong2 r = __ldg(recB + j); pre_u = r.x; pre_v = r.y; }
-        };
-        prefetch(0);
+        const int n_samp_i = (int)n_samp;                                         // split_len < 2^31
+        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull;
+        bool pre_ok = l_live && (int)lj < n_samp_i;
+        if (pre_ok) { pre_x = __ldg(recAx + 4 * lj); const ulonglong2 r = __ldg(recB + lj); pre_u = r.x; pre_v = r.y; }
+        float4* rec_mine = rec_all + (ls * 2) * UM_TS + lj;                       // this thread's slot of its series' tile, buffer 0
         // A task: row m = tid & 127 = (series m >> 6, fine value m & 63), 4 samples `chunk` of the k-step
         const unsigned m = tid & 127u, a_s = m >> 6, a_h = m & 63u;
         const int chunk = (int)(tid >> 7);
+        const float4* rec_a = rec_all + (a_s * 2) * UM_TS + chunk * 4;            // + buffer * UM_TS + first sample of the k-step
+        const uint32_t a_dst = s_stage + (uint32_t)chunk * (UM_A_BYTES / 2) + m * 16u;
+        // B task (128 per k-step: threads 0..127 on even k-steps, 128..255 on odd ones): series (tid >> 6) & 1, K chunk (tid >> 5) & 1, coarse value tid & 31
+        const unsigned b_s = (tid >> 6) & 1u, bc = (tid >> 5) & 1u, b_l = tid & 31u, b_par = (tid >> 7) & 1u;
+        const float4* rec_b = rec_all + (b_s * 2) * UM_TS + (int)bc * 4;
+        const uint32_t b_dst = s_stage + 3 * UM_A_BYTES + bc * (UM_A_BYTES / 2) + (b_s * 64u + b_l) * 16u;
         // drain role: TMEM lane quadrant q4 (series q4 >> 1), Re (0) / Im (1) columns of that series' diagonal block
         const unsigned q4 = w & 3u, part = w >> 2, d_s = q4 >> 1;
         const int64_t db = 2 * bp + d_s;
@@ -222,45 +228,53 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
         float* ws_unit = p.ws + (((d_live ? db : 0) * p.nsplit + sp) * 4) * p.Nf;
         const int64_t k0 = kb + (int64_t)((32u * q4 + lane) & 63u);
         const uint32_t t_drain = tmem + ((32u * q4) << 16) + 64u * d_s + (uint32_t)UD_L * part;
-        int kin = 0, flushes = 0;
+        int flushes = 0;
+        int s = 0;                                                              // ring stage of this k-step
+        uint32_t ph_empty = 1u;                                                 // parity to wait for on EMPTY[s]
+        int sb = 0, buf = 0;                                                    // first sample of the k-step within the tile; tile buffer
+        int left = n_samp_i - chunk * 4;                                        // samples left from this thread's first A sample on
+        int j_tile = (int)lj;                                                   // this thread's record of the tile being loaded, relative to j_begin
 
-        for (int ks = 0; ks < nks; ++ks) {
-            const int s = ks & (UD_STAGES - 1);
-            const uint32_t ph = (uint32_t)(ks / UD_STAGES) & 1u;
-            const int ti = ks >> 4;
-            if ((ks & 15) == 0) {                                       // next record tile of both series (buffer ti & 1)
-                float4 r = make_float4(0.f, 0.f, 0.f, 0.f);             // pad: X = 0, phases 0
+        for (int ks = 0; ks < nks; ) {
+          const int ks_end = min(nks, ks + flush_ksteps);                       // one drain window: the hot loop holds no drain code (registers)
+          #pragma unroll 1
+          for (; ks < ks_end; ++ks) {
+            if (sb == 0) {                                                      // next record tile of both series
+                float4 r = make_float4(0.f, 0.f, 0.f, 0.f);                     // pad: X = 0, phases 0
                 if (pre_ok) {
-                    const u64 pa = pre_u + (u64)kb * pre_v;             // u + kb v (mod 1, 64-bit wrap; reading G3)
+                    const u64 pa = pre_u + (u64)kb * pre_v;                     // u + kb v (mod 1, 64-bit wrap; reading G3)
                     r.x = pre_x * xs;
                     r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
                     r.z = __uint_as_float((unsigned)((pre_v + 0x80000000ull) >> 32));
                     r.w = __uint_as_float((unsigned)(((u64)UD_H * pre_v + 0x80000000ull) >> 32));
                 }
-                rec_all[(ls * 2 + (ti & 1)) * UM_TS + lj] = r;
-                prefetch(ti + 1);
+                rec_mine[buf * UM_TS] = r;
+                j_tile += UM_TS;                                                // prefetch this thread's record of the following tile
+                pre_ok = l_live && j_tile < n_samp_i;
+                if (pre_ok) { pre_x = __ldg(recAx + 4 * j_tile); const ulonglong2 rr = __ldg(recB + j_tile); pre_u = rr.x; pre_v = rr.y; }
                 asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
             }
-            mbar_wait(UD_EMPTY(s), ph ^ 1u);                            // the MMAs that read this stage have completed
-            const int sb = (ks & 15) * UM_KS;
-            const uint32_t st = s_stage + (uint32_t)s * UD_STAGE_BYTES;
-            um_gen_a(rec_all + (a_s * 2 + (ti & 1)) * UM_TS, sb + chunk * 4, a_h, st + chunk * (UM_A_BYTES / 2) + m * 16,
-                     n_samp - ((int64_t)ks * UM_KS + chunk * 4));
-            const unsigned bt = (tid - (unsigned)ks * 128u) & 255u;     // the 128 B tasks rotate over the 256 producer threads
-            if (bt < 128u) {
-                const unsigned b_s = bt >> 6, bc = (bt >> 5) & 1u, l = bt & 31u;
-                ud_gen_b(rec_all + (b_s * 2 + (ti & 1)) * UM_TS, sb + (int)bc * 4, l,
-                         st + 3 * UM_A_BYTES + bc * (UM_A_BYTES / 2) + (b_s * 64u + l) * 16u);
+            const uint32_t st_off = (uint32_t)s * UD_STAGE_BYTES;
+            mbar_wait(UD_EMPTY(s), ph_empty);                                   // the MMAs that read this stage have completed
+            {
+                const float4* ra = rec_a + buf * UM_TS + sb;
+                if (left >= 4) um_gen_a<false>(ra, 0, a_h, a_dst + st_off, 4);  // `left` is warp-uniform
+                else um_gen_a<true>(ra, 0, a_h, a_dst + st_off, max(0, left));
             }
-            fence_proxy_async();                                        // generic-proxy stores -> visible to the tensor core
+            if (((unsigned)ks & 1u) == b_par) ud_gen_b(rec_b + buf * UM_TS + sb, 0, b_l, b_dst + st_off);
+            fence_proxy_async();                                                // generic-proxy stores -> visible to the tensor core
             __syncwarp();
             if (lane == 0) mbar_arrive(UD_FULL(s));
-
-            const bool last = (ks == nks - 1);
-            if (++kin == flush_ksteps || last) {
-                mbar_wait(bar_accf, (uint32_t)flushes & 1u);            // every MMA issued so far has completed
+            left -= UM_KS;
+            sb += UM_KS;
+            if (sb == UM_TS) { sb = 0; buf ^= 1; }
+            if (++s == UD_STAGES) { s = 0; ph_empty ^= 1u; }
+          }
+            const bool last = (ks == nks);
+            {
+                mbar_wait(bar_accf, (uint32_t)flushes & 1u);                    // every MMA issued so far has completed
                 tc_fence_after();
-                if (q.fuse) {                                           // (host guarantees: this is the only drain of the CTA)
+                if (q.fuse) {                                                   // (host guarantees: this is the only drain of the CTA)
                     ud_finish16(q, tmem + ((32u * q4) << 16) + 64u * d_s + 16u * part, db, d_live, k0, 16u * part, lane);
                 } else {
                 ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live);
@@ -269,7 +283,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_acce);
-                ++flushes; kin = 0;
+                ++flushes;
             }
         }
     } else if (lane == 0) {

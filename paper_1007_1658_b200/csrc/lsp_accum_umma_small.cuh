@@ -120,7 +120,12 @@ __device__ __forceinline__ void us_drain(uint32_t taddr, float* dst, int64_t k0,
 
 // grid.x = B * nsplit * nfb (frequency block fastest), US_THREADS threads, UmmaSmall<L, US_STAGES>::SMEM bytes of
 // dynamic shared memory (one k-step of 8 samples per stage), MINB CTAs per SM.  p.nfb = ceil(Nf / (128 L)).
-template <int L, int US_STAGES, int MINB>
+// FUSED_PRE (one launch fewer where launches are what a call costs: C1, C2): steps 1-2 run inside this kernel.  Every CTA forms
+// the mean and the variance of its (short) series itself -- the same fixed-order fp64 reduction in every CTA, so all of them, and
+// the finish step through part_var_out, use bit-identical values -- and computes the exact 64-bit phases (reading G3) of the
+// samples of its own time split while it stages them.  The tensor forms need no per-sample rotation (cos d, sin d), so the fp64
+// work per sample is two exact products.
+template <int L, int US_STAGES, int MINB, bool FUSED_PRE = false>
 __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(const UmmaParams p)
 {
     using C = UmmaSmall<L, US_STAGES>;
@@ -168,12 +173,51 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
         // ===================== producers: steps 3 (operand tiles) and 5 (drain) =====================
         const float4* recA = p.recA + b * p.Nt;
         const ulonglong2* recB = p.recB + b * p.Nt;
-        const float xs = (tid < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
+        float xs;
+        double mean = 0.0, t0 = 0.0;
+        const double* tb = nullptr; const float* xb = nullptr;
+        if (FUSED_PRE) {
+            // steps 1-2: mean, then sum (x - mean)^2, over the whole series by the 256 producer threads
+            tb = p.t + b * p.t_stride; xb = p.x + b * p.x_stride;
+            double* red = reinterpret_cast<double*>(rec);               // 8 doubles of scratch (the record tile is not in use yet)
+            double a0 = 0.0;
+            for (int64_t j = tid; j < p.Nt; j += US_GEN_WARPS * 32) a0 += (double)__ldg(xb + j);
+            #pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a0 += __shfl_down_sync(0xffffffffu, a0, o);
+            if (lane == 0) red[w] = a0;
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            double sum = 0.0;
+            #pragma unroll
+            for (int i = 0; i < US_GEN_WARPS; ++i) sum += red[i];       // fixed order: the same value in every thread of every CTA
+            mean = sum / (double)p.Nt;
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            double a1 = 0.0;
+            for (int64_t j = tid; j < p.Nt; j += US_GEN_WARPS * 32) { const double d = (double)__ldg(xb + j) - mean; a1 += d * d; }
+            #pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a1 += __shfl_down_sync(0xffffffffu, a1, o);
+            if (lane == 0) red[w] = a1;
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            double q2 = 0.0;
+            #pragma unroll
+            for (int i = 0; i < US_GEN_WARPS; ++i) q2 += red[i];
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");   // `red` is the record tile from here on
+            if (tid == 0 && sp == 0 && fb == 0) { p.part_var_out[b] = q2; p.peak64[b] = 0ull; p.counter[b] = 0u; }
+            xs = (tid < UM_TS) ? x_scale(&q2, 1, p.Nt) : 0.f;           // the finish step recomputes exactly this from part_var_out
+            t0 = __ldg(tb);                                             // time origin (reading G6)
+        } else {
+            xs = (tid < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
+        }
         float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
         auto prefetch = [&](int ti) {
             const int64_t j = j_begin + (int64_t)ti * UM_TS + tid;
             pre_ok = (tid < UM_TS) && (j < j_end);
-            if (pre_ok) { pre_x = __ldg(&recA[j].x); const ulonglong2 q = __ldg(recB + j); pre_u = q.x; pre_v = q.y; }
+            if (!pre_ok) return;
+            if (FUSED_PRE) {
+                pre_x = (float)((double)__ldg(xb + j) - mean);          // X_j rounded to fp32 once (G4)
+                const double tp = __ldg(tb + j) - t0;
+                pre_u = frac_fixed64(p.f_min, tp, nullptr);
+                pre_v = frac_fixed64(p.df, tp, nullptr);
+            } else { pre_x = __ldg(&recA[j].x); const ulonglong2 q = __ldg(recB + j); pre_u = q.x; pre_v = q.y; }
         };
         prefetch(0);
         const unsigned h = tid & 127u;                                  // A item: row h, 4 samples `chunk` of the k-step

@@ -19,6 +19,7 @@ namespace lsp {
 
 constexpr int PLAN_PIPE_FP32 = 1, PLAN_PIPE_TENSOR = 2;            // = LSP_PIPE_* of include/lsp.h
 constexpr int PLAN_UMMA_TS = 128;                                  // samples per record tile of the tcgen05 kernels
+constexpr int PLAN_UMMA_TS_SMALL = 32;                             // granularity of the time splits of the short-grid tcgen05 forms
 constexpr int PLAN_TILE_Z = 256;                                   // samples per tile of the FP32-pipe kernel
 constexpr int64_t PLAN_TABLE_BYTES_PER_SAMPLE = 3072;              // CTA-pair form: fine-operand table (lsp_accum_umma_pair2.cuh)
 constexpr int64_t PLAN_TABLE_BUDGET_DEFAULT = (int64_t)1 << 30;    // bytes of workspace the table may take: longer series run in time chunks
@@ -105,7 +106,10 @@ inline PlanChoice plan_choose_tensor(int sm_count, int64_t B, int64_t Nt, int64_
     for (int li = 0; li < 4; ++li) {
         const int L = Ls[li];
         if (ov.L && ov.L != L) continue;
-        const int FPB = 128 * L, TS = PLAN_UMMA_TS;
+        // granularity of the time splits: the record tile (128 samples) for the table-fed pair form; 32 samples (4 k-steps) for the
+        // forms that generate both operands, so that short series (C1, C2) can be cut into many short CTAs: there the length of
+        // ONE CTA's k-step chain is what a call costs
+        const int FPB = 128 * L, TS = L >= 128 ? PLAN_UMMA_TS : PLAN_UMMA_TS_SMALL;
         const int cps = plan_umma_ctas_per_sm(L);
         int64_t nfb = (Nf + FPB - 1) / FPB;
         int nchunks = 1;

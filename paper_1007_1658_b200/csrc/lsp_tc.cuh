@@ -41,6 +41,13 @@ struct UmmaParams {
     int flush_ksteps;           // k-steps between drains of D_W
     float trunc_ulps;           // pair form: truncation compensation at each drain: < 0 the model, 0 off, > 0 ulps per k-step (u2_drain64)
     int unit_x;                 // 1: recA.x is a weight, not a measurement: no variance scaling, no V (second pass of the generalised periodogram)
+    // short-grid form with the pre-pass fused in (accum_umma_small_kernel<..., FUSED_PRE>): steps 1-2 are done by each CTA itself
+    // from the caller's arrays (short series: every CTA forms the mean and variance over the whole series, identically)
+    const double* t; int64_t t_stride;      // series b at t + b * t_stride
+    const float* x; int64_t x_stride;
+    double f_min, df;
+    double* part_var_out;       // [B]: sum (x - mean)^2, written by the series' first CTA for the finish step (nparts = 1)
+    u64* peak64; unsigned* counter;   // [B]: reset by the series' first CTA
 };
 
 // 1 / sigma as the fp32 factor applied to X before it is split into fp16 pairs (unit variance, so fp16

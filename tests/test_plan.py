@@ -75,7 +75,7 @@ def test_tensor_core_plans_cover_the_problem(B, Nt, Nf):
         assert p["chunks_or_ctas_per_sm"] == {64: 2, 32: 2, 16: 3}[L]
         assert nfb * fpb >= Nf and (nfb - 1) * fpb < Nf
         assert p["nsplit"] >= 1 and p["nsplit"] * p["split_len"] >= Nt and (p["nsplit"] - 1) * p["split_len"] < Nt
-    assert p["split_len"] % 128 == 0
+    assert p["split_len"] % (128 if L == 128 else 32) == 0
     assert B * p["nsplit"] * 16 * Nf <= (1 << 31) + 16 * Nf
     assert p["est_cycles"] > 0
 

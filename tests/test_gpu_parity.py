@@ -892,6 +892,37 @@ def test_argument_errors(lsp):
     assert pkg.status_string(pkg.LSP_EINVAL) == "invalid argument"
 
 
+def test_maximum_batch_and_degenerate_series(lsp):
+    """Edge cases of the batched entry point: the largest batch the ABI accepts (B = 65,535 tiny series: the pre-pass and finish grids
+    at their limit) against the oracle series by series; and a series of zero variance, for which the header promises NaN -- not a
+    fault, and not a disturbance of the other series of the batch."""
+    import torch
+    pkg, h = lsp
+    B, Nt, Nf = 65535, 9, 5
+    rng = np.random.default_rng(65535)
+    t = np.sort(rng.uniform(0.0, 10.0, (B, Nt)), axis=1)
+    x = rng.standard_normal((B, Nt)).astype(np.float32)
+    f_min, df = 0.05, 0.11
+    P, pi, pv = h.periodogram_batched(torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), f_min, df, Nf)
+    torch.cuda.synchronize()
+    P, pi, pv = P.cpu().numpy(), pi.cpu().numpy(), pv.cpu().numpy()
+    assert np.all(np.isfinite(P)) and P.min() >= 0.0 and P.max() <= (Nt - 1) / 2.0 * (1 + 1e-5)
+    assert np.array_equal(pv, P.max(axis=1))
+    for b in list(range(0, B, 4099)) + [B - 1]:
+        ref = oracle.periodogram(t[b], x[b], f_min, df, Nf)
+        assert np.max(np.abs(P[b] - ref)) <= TOL * ref.max(), b
+        if _top_two_gap(ref) >= QUAL_GAP:
+            assert int(pi[b]) == oracle.argmax(ref)
+    # zero variance: NaN for that series only
+    w = workloads.c4(B=4, Nt=600, Nf=700, seed=77)
+    xz = w.x.copy(); xz[2, :] = 3.25
+    for prm in (dict(pipe=FP32), dict()):
+        Pz, _, _, _ = _run_batched(h, workloads.Workload("zero-var", w.t, xz, w.f_min, w.df, w.Nf, B=4), **prm)
+        assert np.all(np.isnan(Pz[2])), prm
+        for b in (0, 1, 3):
+            _check(Pz[b], oracle.periodogram(w.t[b], xz[b], w.f_min, w.df, w.Nf), "next to a zero-variance series %r" % (prm,))
+
+
 def test_failed_growth_keeps_the_workspace(lsp):
     """LSP_ENOMEM leaves the handle usable: lsp_reserve for a 2 TB problem fails, the next ordinary call runs on the workspace the
     handle had (ensure() allocates the new buffer before it releases the old one)."""

@@ -69,7 +69,10 @@ constexpr int U2_STAGES = 8 / U2_KPS;                             // the ring al
 constexpr int U2_GSLOT = U2_KPS * 3 * UM_A_BYTES;                 // generated planes of one stage
 constexpr int U2_STAGE_BYTES = U2_GSLOT + U2_KPS * UP_GROUP_BYTES; // + this CTA's table rows
 constexpr int U2_GT = 128 * U2_KPS;                               // thread-tasks per stage-step = threads of a producer group
-constexpr int U2_GROUPS = 512 / U2_GT;                            // producer groups: group g owns the stage-steps it = g (mod U2_GROUPS)
+#ifndef LSP_U2_GROUPS
+#define LSP_U2_GROUPS (512 / (128 * LSP_U2_KPS))
+#endif
+constexpr int U2_GROUPS = LSP_U2_GROUPS;                          // producer groups: group g owns the stage-steps it = g (mod U2_GROUPS)
 constexpr int U2_GROUP_WARPS = U2_GT / 32;
 constexpr int U2_PROD_WARPS = U2_GROUPS * U2_GROUP_WARPS;         // 16; they also drain; warp 16 issues the MMAs
 constexpr int U2_THREADS = (U2_PROD_WARPS + 1) * 32;
@@ -291,15 +294,23 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 const uint32_t st = s_stage + (uint32_t)s * U2_STAGE_BYTES;
                 if (tg < 32u) {                                         // warp-uniform: only the group's first warp runs the copy-issue code
                     if (lane == 0) {                                    // this CTA's 128 table rows of the two k-steps: one bulk copy
+#ifdef LSP_U2_DBG_NOTMA
+                        mbar_arrive(U2_FULL(s));
+#else
                         mbar_expect_tx(U2_FULL(s), U2_KPS * UP_GROUP_BYTES);
                         tma_bulk_g2s(st + U2_GSLOT, tab + (int64_t)it * (U2_KPS * UP_GROUP_BYTES), U2_KPS * UP_GROUP_BYTES, U2_FULL(s));
+#endif
                     }
                     __syncwarp();
                 }
                 const int s0 = (it % U2_TILE_STEPS) * (U2_KPS * UM_KS) + samp_off;  // within the 128-sample record tile
                 const int left = n_samp - (it * (U2_KPS * UM_KS) + samp_off);
+#ifndef LSP_U2_DBG_NOGEN
                 if (left >= 4) u2_gen<false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
                 else u2_gen<true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+#else
+                (void)s0; (void)left; (void)h; (void)g_off;
+#endif
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(U2_FULL(s));
@@ -333,10 +344,14 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 const uint64_t dGv = umma_desc(g0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
                 const uint64_t dTh = umma_desc(t0, UP_B_HALF / 2, 128), dT8 = umma_desc(t0 + UP_B_HALF, UP_B_HALF / 2, 128);
                 const uint64_t dTv = umma_desc(t0 + 2 * UP_B_HALF, UP_B_HALF / 2, 128);
+#ifndef LSP_U2_DBG_NOMMA
                 tc_mma_f16_pair(tmem, dTh, dGh, UP_IDESC, (!win_first || kk > 0) ? 1u : 0u);
                 tc_mma_f8_pair(tmem, dT8, dG8, UP_IDESC_F8, 1u);
                 if (!p.unit_x)                                          // (the unit-weight pass of the generalised periodogram needs no V: CC, CS come from the first pass)
                     tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
+#else
+                (void)dTh; (void)dGh; (void)dT8; (void)dG8; (void)dTv; (void)dGv; (void)win_first;
+#endif
             }
             tc_commit_pair(U2_EMPTY(s));
             const bool last = (it == nst - 1);

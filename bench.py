@@ -2,6 +2,7 @@
 """bench.py -- Lomb-Scargle term-evaluation throughput on B200 (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference] [--shard series|freq]
+    python bench.py --sweep | --back-to-back N      (N_t scaling sweep; call latency of the small configs)
 
 One "step" = one pass of the whole hot path (moments -> records -> accumulate -> finish, all rows of
 SURVEY.md section 8(a)) over one seeded synthetic workload.  N = 1 times BASELINE.json's headline config
@@ -554,6 +555,52 @@ def run_sweep(args):
     return 0
 
 
+def run_back_to_back(args):
+    """SURVEY.md section 8(d) protocol for the small configs: N back-to-back device-pointer calls on one stream, no L2 flush, no
+    host synchronisation in between (separates launch latency from arithmetic); eager, and captured once into a CUDA graph and
+    replayed.  One JSON line."""
+    import torch
+    import paper_1007_1658_b200 as lsp
+    w = workloads.make(args.workload)
+    if w.B > 1:
+        raise SystemExit("--back-to-back is for a single series")
+    h = lsp.Handle(0)
+    if args.pipe:
+        h.set_param(lsp.PARAM_PIPE, args.pipe)
+    t_d = torch.from_numpy(np.ascontiguousarray(w.t)).cuda()
+    x_d = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
+    P_d = torch.empty(w.Nf, dtype=torch.float32, device="cuda")
+    n = args.back_to_back
+    for _ in range(20):
+        h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d)
+    torch.cuda.synchronize()
+    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ea.record()
+    for _ in range(n):
+        h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d)
+    eb.record(); torch.cuda.synchronize()
+    eager_ms = ea.elapsed_time(eb) / n
+    plan = h.last_plan()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        for _ in range(3):
+            h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d, stream=st)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d, stream=st)
+        torch.cuda.synchronize()
+        ea.record(st)
+        for _ in range(n):
+            g.replay()
+        eb.record(st); torch.cuda.synchronize()
+    graph_ms = ea.elapsed_time(eb) / n
+    h.close()
+    print(json.dumps({"metric": "lomb_scargle_back_to_back_call_ms", "workload": w.name, "calls": n, "unit": "ms per call", "data": "synthetic",
+                      "eager_ms_per_call": eager_ms, "graph_replay_ms_per_call": graph_ms, "terms_per_s_eager": w.terms / (eager_ms * 1e-3),
+                      "plan": plan, "note": "device-pointer calls back to back on one stream, no L2 flush, no host sync between calls"}))
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -573,6 +620,8 @@ def main(argv=None):
     ap.add_argument("--coarse", type=int, default=0)
     ap.add_argument("--trunc", type=int, default=0)
     ap.add_argument("--sweep", action="store_true", help="N_t scaling sweep of --workload (single series) instead of the bench line")
+    ap.add_argument("--back-to-back", type=int, default=0, dest="back_to_back",
+                    help="N back-to-back calls of --workload (single series), eager and as a replayed CUDA graph, instead of the bench line")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
@@ -580,6 +629,8 @@ def main(argv=None):
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.back_to_back:
+        return run_back_to_back(args)
     return run_ours(args)
 
 

@@ -361,7 +361,9 @@ struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair, fuse_pre; int64
 int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf, bool gls, Route& r, bool weighted = false)
 {
     r.tab_series = (t_stride == 0) ? 1 : B;
-    r.pl = make_plan(h, B, Nt, Nf, r.tab_series, weighted ? PLAN_PIPE_FP32 : 0);   // per-sample weights: the FP32-pipe form carries them
+    r.pl = make_plan(h, B, Nt, Nf, r.tab_series);
+    // per-sample weights: the CTA-pair tensor form and the FP32-pipe form carry them; where the plan is another form, the FP32 one runs
+    if (weighted && !(r.pl.pipe == PLAN_PIPE_TENSOR && r.pl.L >= 128)) r.pl = make_plan(h, B, Nt, Nf, r.tab_series, PLAN_PIPE_FP32);
     Plan& pl = r.pl;
     if (pl.K == 0) return LSP_EINVAL;
     r.tensor = pl.pipe == PLAN_PIPE_TENSOR;
@@ -375,7 +377,8 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
         if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
         pl.kernel_name = weighted ? ke->name_weighted : ke->name;
     } else if (r.pair) {
-        pl.kernel_name = "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>";
+        pl.kernel_name = weighted ? "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table,weighted>"
+                                  : "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>";
         pl.launches = 3 + 2 * pl.nchunks;
     } else if (r.duo) {
         pl.kernel_name = r.duo_fuse ? "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32,fused-finish>"
@@ -497,6 +500,7 @@ int run_device(lsp_ctx* h,
                 up.unit_x = pass;
                 pp.btable = table; pp.half_stride = half_stride; pp.table_stride = (r.tab_series == 1) ? 0 : series_stride;
                 pp.j0 = j0; pp.chunk_len = len; pp.accumulate = c > 0 ? 1 : 0;
+                pp.recW = weighted ? recA1 : nullptr;
                 pp.nsplit_grid = nsplit_c;                  // only the splits this chunk has; pl.nsplit still strides `ws`
                 const int64_t units = B * (int64_t)nsplit_c * pl.nfb;
                 cudaLaunchConfig_t cfg = {};

@@ -54,6 +54,8 @@ struct UmmaPairParams {
     int64_t j0, chunk_len;          // the chunk: samples j0 .. j0 + chunk_len - 1
     int nsplit_grid;                // time splits this launch covers (a short last chunk has fewer than u.nsplit, the stride of `ws`)
     int accumulate;                 // 1: `ws` holds the sums of earlier chunks
+    const float4* recW;             // weighted generalised periodogram: recW[j].x = sqrt of the normalised weight w_j (and u.recA.x carries one
+                                    // factor sqrt(w_j) already, lsp_prepass.cuh): X = recA.x recW.x, and V = sum w e^{2i theta}; else NULL
 };
 
 constexpr int U2_FPP = 256 * UM_H;                                // frequencies per CTA pair
@@ -120,13 +122,13 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
 __device__ __forceinline__ unsigned swap_halves(unsigned x) { return __byte_perm(x, 0u, 0x1032); }
 __device__ __forceinline__ unsigned swap_bytes16(unsigned x) { return __byte_perm(x, 0u, 0x2301); }
 
-template <bool TAIL>
+template <bool TAIL, bool WEIGHTED>
 __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, uint32_t sG, int nvalid)
 {
     unsigned hi[4], lo[4], h8[4], vv[4];
     #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const float4 r = rec[s0 + i];                                   // {X / sigma, pA32, w32, -}: broadcast read
+        const float4 r = rec[s0 + i];                                   // {X / sigma, pA32, w32, weight}: broadcast read
         float c, s;
         sincos_phase32(__float_as_uint(r.y) + h * __float_as_uint(r.z), c, s);
         const u64 cs = pack2(c, s);
@@ -140,6 +142,7 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
         h8[i] = pack_e5m2_h2(hi[i]);
         float v0, v1;
         unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
+        if (WEIGHTED) { v0 *= r.w; v1 *= r.w; }                         // V = sum_j w_j e^{2i theta}
         vv[i] = pack_h2(v0, v1);
         if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
@@ -250,11 +253,16 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
         const ulonglong2* recB = p.recB + b * p.Nt;
         const unsigned char* tab = q.btable + b * q.table_stride + (int64_t)rank * q.half_stride + ((j_begin - q.j0) / UM_KS) * (int64_t)UP_GROUP_BYTES;
         const float xs = (tg < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
-        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
+        const bool weighted = q.recW != nullptr;
+        const float4* recW = weighted ? q.recW + b * p.Nt : nullptr;
+        float pre_x = 0.f, pre_w = 1.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
         auto prefetch = [&](int ti) {
             const int64_t j = j_begin + (int64_t)ti * UM_TS + tg;
             pre_ok = (tg < UM_TS) && (j < j_end);
-            if (pre_ok) { pre_x = __ldg(&recA[j].x); const ulonglong2 r = __ldg(recB + j); pre_u = r.x; pre_v = r.y; }
+            if (pre_ok) {
+                pre_x = __ldg(&recA[j].x); const ulonglong2 r = __ldg(recB + j); pre_u = r.x; pre_v = r.y;
+                if (weighted) pre_w = __ldg(&recW[j].x);
+            }
         };
         prefetch(0);
         const unsigned hl = tg & 63u, h = (unsigned)U2_HC * rank + hl;   // coarse value: local row, global index
@@ -281,9 +289,10 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                         float4 r = make_float4(0.f, 0.f, 0.f, 0.f);     // pad: X = 0, phases 0
                         if (pre_ok) {
                             const u64 pa = pre_u + (u64)kb * pre_v;     // u + kb v (mod 1, 64-bit wrap; reading G3)
-                            r.x = pre_x * xs;
+                            r.x = pre_x * xs * pre_w;                   // (pre_w = 1 without weights)
                             r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
                             r.z = __uint_as_float((unsigned)((256ull * pre_v + 0x80000000ull) >> 32));
+                            r.w = pre_w * pre_w;
                         }
                         rec[(ti & 1) * UM_TS + tg] = r;
                         prefetch(ti + 1);
@@ -306,8 +315,13 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 const int s0 = (it % U2_TILE_STEPS) * (U2_KPS * UM_KS) + samp_off;  // within the 128-sample record tile
                 const int left = n_samp - (it * (U2_KPS * UM_KS) + samp_off);
 #ifndef LSP_U2_DBG_NOGEN
-                if (left >= 4) u2_gen<false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
-                else u2_gen<true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+                if (!weighted) {
+                    if (left >= 4) u2_gen<false, false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
+                    else u2_gen<true, false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+                } else {
+                    if (left >= 4) u2_gen<false, true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);
+                    else u2_gen<true, true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+                }
 #else
                 (void)s0; (void)left; (void)h; (void)g_off;
 #endif

@@ -780,6 +780,37 @@ def test_weighted_generalised_periodogram(lsp):
         h.periodogram(td[:3].contiguous(), xd[:3].contiguous(), f_min, df, 4, weights=wd[:3].contiguous())
 
 
+def test_weighted_generalised_periodogram_long_grid(lsp):
+    """Per-sample weights through the CTA-pair tensor form (the generated operand carries w x, and w e^{2i theta} for the sums of
+    cos^2 and cos sin; both passes stream the same table): a grid of two pairs, time chunks, zero weights."""
+    import torch
+    pkg, h = lsp
+    rng = np.random.default_rng(911)                           # (seed-qualified: top-two gap 4.5e-4)
+    Nt, Nf = 6007, 40001
+    t = np.sort(np.concatenate([rng.uniform(0, 20, Nt // 2), rng.uniform(55, 80, Nt - Nt // 2)]))
+    sig = rng.uniform(0.4, 2.5, Nt)
+    x = (4.0 + 0.5 * np.sin(2 * np.pi * 0.0213 * t + 0.4) + 0.4 * np.sin(2 * np.pi * 2.3 * t) + sig * rng.standard_normal(Nt)).astype(np.float32)
+    wts = (1.0 / sig ** 2).astype(np.float32)
+    wts[5::23] = 0.0
+    f_min, df = 1.0 / 80.0, (6.0 - 1.0 / 80.0) / (Nf - 1)
+    ref = oracle.periodogram_gls_weighted(t, x, wts, f_min, df, Nf)
+    assert _top_two_gap(ref) >= QUAL_GAP
+    assert np.max(np.abs(ref - oracle.periodogram_gls(t, x, f_min, df, Nf))) > 1e-2 * ref.max()
+    td, xd, wd = torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), torch.from_numpy(wts).cuda()
+    for table_mb in (0, 4):                                    # one chunk; 4 MiB: five time chunks
+        with _params(h, pipe=TENSOR, coarse=128, table_mb=table_mb):
+            P = h.periodogram(td, xd, f_min, df, Nf, weights=wd).cpu().numpy()
+            plan = h.last_plan()
+        assert "pair2" in plan["kernel"] and "weighted" in plan["kernel"], plan
+        _check(P, ref, "weighted gls, pair form, table_mb=%d" % table_mb)
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+    # a short grid with the tensor pipe requested: the plan is not the pair form, so the FP32 form carries the weights
+    with _params(h, pipe=TENSOR):
+        Ps = h.periodogram(td, xd, f_min, df, 3000, weights=wd).cpu().numpy()
+        assert h.last_plan()["pipe"] == FP32
+    _check(Ps, ref[:3000], "weighted gls, short grid")
+
+
 def test_false_alarm_probability(lsp):
     """Eq. (3) epilogue against the oracle's plain formula on the GPU's own P (C1), on per-series peaks of a noise
     batch, and on hand-made values spanning Q = 1 ... 1e-30."""

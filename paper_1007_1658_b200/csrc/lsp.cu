@@ -225,7 +225,7 @@ Layout device_layout(const Plan& pl, int64_t B, int64_t Nt, int64_t Nf, int64_t 
     return L;
 }
 
-// steps 6-7: with several time splits the sum over them is spread over 8 threads per frequency
+// steps 6-7: on short grids with several time splits the sum over them is spread over 8 threads per frequency
 // Launch `kernel` as a programmatic dependent of the work before it in the stream (PDL): its CTAs may be scheduled while the
 // predecessor drains; the kernel calls pdl_wait() before reading what the predecessor wrote.
 template <typename... KArgs, typename... Args>
@@ -242,7 +242,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 
 void launch_finish(const FinishParams& fp, int64_t B, cudaStream_t st, bool pdl = false)
 {
-    if (fp.nsplit >= 4) {
+    if (fp.nsplit >= 4 && fp.Nf <= 65536) {               // (long grids have enough frequencies to fill the machine one thread each: 170 vs 360 us at C5)
         const int64_t per_block = FIN_THREADS / 8;
         launch_pdl(finish_kernel<8>, dim3((unsigned)((fp.Nf + per_block - 1) / per_block), (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
     } else {

@@ -431,6 +431,12 @@ def run_ours(args):
         fast = time_config_checked(0)                                     # the library's automatic plan
         if fast["plan"]["kernel"] == rec["plan"]["kernel"]:
             fast = None                                                   # (same kernel: nothing to add)
+    fast16 = None
+    if fast is not None and "pair2" in fast["plan"]["kernel"] and not args.no_fast_path:
+        # the same tensor form with the corrections as two fp16 MMAs: 22 significant operand bits in every product of XC, XS
+        h.set_param(lsp.PARAM_CORR, 1)
+        fast16 = time_config_checked(0)
+        h.set_param(lsp.PARAM_CORR, 0)
     h2d = t_h.numel() * 8 + x_h.numel() * 4
     d2h = P_h.numel() * 4 + (pi_h.numel() * 8 if batched else 0)
 
@@ -494,6 +500,13 @@ def run_ours(args):
                       "the paper's fp32, inside the path's 1e-4 max P tolerance; reported, not the headline")
         f0["speedup_over_line_of_record"] = r0["ms_per_step"] / f0["ms_per_step"]
         line["fast_path"] = f0
+    if fast16 is not None:
+        f1 = finish_record(fast16)
+        f1["note"] = ("the fast path with LSP_PARAM_CORR = 1: first-order corrections of the fp16 hi + lo operand split as two fp16 MMAs "
+                      "(22 significant operand bits per product of XC, XS -- no less than the paper's fp32 with SFU trig, PAPER.md:290; "
+                      "CC, CS in one fp16 pass, fp32 accumulation in the tensor core); reported, not the headline")
+        f1["speedup_over_line_of_record"] = r0["ms_per_step"] / f1["ms_per_step"]
+        line["fast_path_fp16x3"] = f1
     if batched:
         # BASELINE config 4: "report per-series peak power distribution" -- the peaks the last host-buffer step returned,
         # and their false-alarm probabilities by eq. (3) with N_ind = Nf (lsp_false_alarm)

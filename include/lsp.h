@@ -75,6 +75,10 @@ enum {
     LSP_PARAM_TRUNC     = 9,  /* tensor form, CTA-pair kernel: 1 = do not add the expected round-toward-zero loss of the       */
                               /* tensor-core accumulation back at each drain; 0 = add it (default)       */
     LSP_PARAM_SHARED    = 11, /* batched call with t_stride = 0: 0 = the shared-time GEMM path when B >= 16 and Nt >= 512, 1 = never, 2 = always */
+    LSP_PARAM_CORR      = 15, /* tensor form, CTA-pair kernel: how the first-order corrections A_lo B_hi + A_hi B_lo of the fp16 hi + lo   */
+                              /* operand split are formed: 0 = one kind::f8f6f4 MMA on e5m2 copies (3 MMAs per 8 samples, the default);  */
+                              /* 1 = two kind::f16 MMAs on fp16 lo parts (4 MMAs per 8 samples): every product of the sums XC, XS then   */
+                              /* carries 22 significant operand bits, no less than the paper's fp32 arithmetic with SFU trig*/
     LSP_PARAM_PDL       = 13  /* short-grid tensor path: 0 = steps 1-2 run inside the accumulate kernel when Nt <= 16,384 (two launches per  */
                               /* call) and the kernels of a call are launched as programmatic dependents (each kernel's launch and      */
                               /* set-up overlap its predecessor's tail); 1 = separate pre-pass kernels in plain stream order            */

@@ -40,7 +40,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0, opt_corr = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     cudaEvent_t evc[TIMING_RING][2 * TIMING_MAX_CHUNKS] = {};   // accumulate launches of a chunked call, begin / end per chunk
     int ev_chunks[TIMING_RING] = {};
@@ -377,6 +377,9 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
         if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
         pl.kernel_name = weighted ? ke->name_weighted : ke->name;
     } else if (r.pair) {
+        if (h->opt_corr) pl.kernel_name = weighted ? "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16,hi+lo,fine-table,weighted>"
+                                                   : "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16,hi+lo,fine-table>";
+        else
         pl.kernel_name = weighted ? "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table,weighted>"
                                   : "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>";
         pl.launches = 3 + 2 * pl.nchunks;
@@ -480,12 +483,13 @@ int run_device(lsp_ctx* h,
         // CTA-pair form, one time chunk at a time: table pre-pass, then the accumulate launch(es) that read it
         const int64_t half_stride = L.tab_groups * (int64_t)UP_GROUP_BYTES;
         const int64_t series_stride = L.tab_groups * (int64_t)U2_TABLE_BYTES_PER_KSTEP;
-        LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_pair2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)U2_SMEM));
+        void (*pair_kernel)(const UmmaPairParams) = h->opt_corr ? accum_umma_pair2_kernel<true> : accum_umma_pair2_kernel<false>;
+        LSP_CUDA(h, cudaFuncSetAttribute(pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)U2_SMEM));
         for (int c = 0; c < pl.nchunks; ++c) {
             const int64_t j0 = (int64_t)c * pl.chunk_len;
             const int64_t len = (Nt - j0 < pl.chunk_len) ? Nt - j0 : pl.chunk_len;
             const int64_t groups = (len + UM_KS - 1) / UM_KS + U2_TABLE_PAD_KSTEPS;
-            umma_ftable_pair_kernel<<<dim3((unsigned)groups, (unsigned)r.tab_series), 512, 0, st>>>(recB, j0, j0 + len, Nt, table, half_stride, series_stride);
+            umma_ftable_pair_kernel<<<dim3((unsigned)groups, (unsigned)r.tab_series), 512, 0, st>>>(recB, j0, j0 + len, Nt, table, half_stride, series_stride, (int)h->opt_corr);
             LSP_CUDA(h, cudaGetLastError());
             if (timing && c == 0) LSP_CUDA(h, cudaEventRecord(ev[2], st));
             if (chunk_timing) LSP_CUDA(h, cudaEventRecord(evc[2 * c], st));
@@ -509,7 +513,7 @@ int run_device(lsp_ctx* h,
                 at[0].id = cudaLaunchAttributeClusterDimension;
                 at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
                 cfg.attrs = at; cfg.numAttrs = 1;
-                LSP_CUDA(h, cudaLaunchKernelEx(&cfg, accum_umma_pair2_kernel, pp));
+                LSP_CUDA(h, cudaLaunchKernelEx(&cfg, pair_kernel, pp));
             }
             if (chunk_timing) LSP_CUDA(h, cudaEventRecord(evc[2 * c + 1], st));
         }
@@ -670,6 +674,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_TRUNC:      if (value > 4000) return LSP_EINVAL; h->opt_trunc = value; break;
         case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
         case LSP_PARAM_PDL:        if (value > 1) return LSP_EINVAL; h->opt_pdl = value; break;
+        case LSP_PARAM_CORR:       if (value > 1) return LSP_EINVAL; h->opt_corr = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -690,6 +695,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_TRUNC:      *value = h->opt_trunc; break;
         case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
         case LSP_PARAM_PDL:        *value = h->opt_pdl; break;
+        case LSP_PARAM_CORR:       *value = h->opt_corr; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

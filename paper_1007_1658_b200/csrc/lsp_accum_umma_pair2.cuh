@@ -87,12 +87,12 @@ constexpr size_t U2_SMEM = (size_t)U2_STAGES * U2_STAGE_BYTES + U2_REC_BYTES + 2
 // 2 = (cos 2b, sin 2b) fp16; b = 2 pi frac(l v_j).  grid (ngroups, series), 512 threads = 2 K-chunks x 256 fine indices;
 // group g holds samples j0 + 8g .. j0 + 8g + 7 of the chunk [j0, j1).
 __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2* __restrict__ recB, int64_t j0, int64_t j1, int64_t rec_stride,
-                                                               unsigned char* __restrict__ table, int64_t half_stride, int64_t table_stride)
+                                                               unsigned char* __restrict__ table, int64_t half_stride, int64_t table_stride, int corr16)
 {
     const int64_t g = blockIdx.x;
     const unsigned l = threadIdx.x & 255u, chunk = threadIdx.x >> 8;
     const ulonglong2* rb = recB + (int64_t)blockIdx.y * rec_stride;
-    unsigned hh[4], h8[4], l8[4], vv[4];
+    unsigned hh[4], h8[4], l8[4], vv[4], l16[4];
     #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int64_t j = j0 + g * UM_KS + chunk * 4 + i;
@@ -104,6 +104,7 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
         const float2 hf = unpack_h2(hh[i]);
         h8[i] = pack_e5m2_h2(hh[i]);
         l8[i] = pack_e5m2(c - hf.x, s - hf.y);
+        l16[i] = pack_h2(c - hf.x, s - hf.y);
         const float cc = c + c;
         vv[i] = pack_h2(fmaf(cc, c, -1.f), cc * s);
     }
@@ -112,7 +113,8 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
     constexpr int PLANE = UP_B_HALF / 16;
     const int row = (int)(chunk * (PLANE / 2) + (l & 127u));
     o[row] = make_uint4(hh[0], hh[1], hh[2], hh[3]);
-    o[PLANE + row] = make_uint4(h8[0] | (h8[1] << 16), h8[2] | (h8[3] << 16), l8[0] | (l8[1] << 16), l8[2] | (l8[3] << 16));
+    if (corr16) o[PLANE + row] = make_uint4(l16[0], l16[1], l16[2], l16[3]);      // plane 1 = fp16 (c - c_h, s - s_h)
+    else o[PLANE + row] = make_uint4(h8[0] | (h8[1] << 16), h8[2] | (h8[3] << 16), l8[0] | (l8[1] << 16), l8[2] | (l8[3] << 16));
     o[2 * PLANE + row] = make_uint4(vv[0], vv[1], vv[2], vv[3]);
 }
 
@@ -122,7 +124,7 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
 __device__ __forceinline__ unsigned swap_halves(unsigned x) { return __byte_perm(x, 0u, 0x1032); }
 __device__ __forceinline__ unsigned swap_bytes16(unsigned x) { return __byte_perm(x, 0u, 0x2301); }
 
-template <bool TAIL, bool WEIGHTED>
+template <bool TAIL, bool WEIGHTED, bool CORR16>
 __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, uint32_t sG, int nvalid)
 {
     unsigned hi[4], lo[4], h8[4], vv[4];
@@ -138,21 +140,27 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
         const float2 hf = unpack_h2(hi[i]);
         float lc, ls;
         unpack2(fma2(pack2(hf.x, hf.y), pack2(-1.f, -1.f), pack2(xc, xs)), lc, ls);
-        lo[i] = pack_e5m2(lc, ls);
-        h8[i] = pack_e5m2_h2(hi[i]);
+        if (CORR16) lo[i] = pack_h2(lc, ls);
+        else { lo[i] = pack_e5m2(lc, ls); h8[i] = pack_e5m2_h2(hi[i]); }
         float v0, v1;
         unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
         if (WEIGHTED) { v0 *= r.w; v1 *= r.w; }                         // V = sum_j w_j e^{2i theta}
         vv[i] = pack_h2(v0, v1);
         if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
-    const unsigned q0 = lo[0] | (lo[1] << 16), q1 = lo[2] | (lo[3] << 16), q2 = h8[0] | (h8[1] << 16), q3 = h8[2] | (h8[3] << 16);
+    unsigned q0 = 0u, q1 = 0u, q2 = 0u, q3 = 0u;
+    if (!CORR16) { q0 = lo[0] | (lo[1] << 16); q1 = lo[2] | (lo[3] << 16); q2 = h8[0] | (h8[1] << 16); q3 = h8[2] | (h8[3] << 16); }
     constexpr uint32_t IM = U2_HC * 16;                                 // row (h,Im) is 64 rows below row (h,Re)
     // row (h,Re) = (xc, -xs): flip the sign of the second component;  row (h,Im) = (xs, xc): swap the components
     sts128(sG, hi[0] ^ 0x80000000u, hi[1] ^ 0x80000000u, hi[2] ^ 0x80000000u, hi[3] ^ 0x80000000u);
     sts128(sG + IM, swap_halves(hi[0]), swap_halves(hi[1]), swap_halves(hi[2]), swap_halves(hi[3]));
+    if (CORR16) {                                                       // plane 1 = G_lo in fp16, rows built as those of G_hi
+        sts128(sG + UM_A_BYTES, lo[0] ^ 0x80000000u, lo[1] ^ 0x80000000u, lo[2] ^ 0x80000000u, lo[3] ^ 0x80000000u);
+        sts128(sG + UM_A_BYTES + IM, swap_halves(lo[0]), swap_halves(lo[1]), swap_halves(lo[2]), swap_halves(lo[3]));
+    } else {
     sts128(sG + UM_A_BYTES, q0 ^ 0x80008000u, q1 ^ 0x80008000u, q2 ^ 0x80008000u, q3 ^ 0x80008000u);
     sts128(sG + UM_A_BYTES + IM, swap_bytes16(q0), swap_bytes16(q1), swap_bytes16(q2), swap_bytes16(q3));
+    }
     sts128(sG + 2 * UM_A_BYTES, vv[0] ^ 0x80000000u, vv[1] ^ 0x80000000u, vv[2] ^ 0x80000000u, vv[3] ^ 0x80000000u);
     sts128(sG + 2 * UM_A_BYTES + IM, swap_halves(vv[0]), swap_halves(vv[1]), swap_halves(vv[2]), swap_halves(vv[3]));
 }
@@ -198,6 +206,8 @@ __device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k
 // ------------------------------------------------------------------ the kernel
 // grid.x = B * nsplit * (2 * npairs) (CTA of the pair fastest, then the pair), clusters of 2, U2_THREADS threads,
 // U2_SMEM bytes of dynamic shared memory, one CTA per SM.  q.u.nfb = 2 * npairs, npairs = ceil(Nf / 32,768).
+// CORR16 (LSP_PARAM_CORR = 1): plane 1 of both operands holds fp16 lo parts and the corrections are two kind::f16 MMAs.
+template <bool CORR16>
 __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const UmmaPairParams q)
 {
     const UmmaParams& p = q.u;
@@ -316,11 +326,11 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 const int left = n_samp - (it * (U2_KPS * UM_KS) + samp_off);
 #ifndef LSP_U2_DBG_NOGEN
                 if (!weighted) {
-                    if (left >= 4) u2_gen<false, false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
-                    else u2_gen<true, false>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+                    if (left >= 4) u2_gen<false, false, CORR16>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);      // `left` is warp-uniform
+                    else u2_gen<true, false, CORR16>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
                 } else {
-                    if (left >= 4) u2_gen<false, true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);
-                    else u2_gen<true, true>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
+                    if (left >= 4) u2_gen<false, true, CORR16>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, 4);
+                    else u2_gen<true, true, CORR16>(rec + (ti & 1) * UM_TS, s0, h, st + g_off, max(0, left));
                 }
 #else
                 (void)s0; (void)left; (void)h; (void)g_off;
@@ -334,7 +344,8 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const bool last = (f == nwin - 1);
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
-            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, p.trunc_ulps, (float)((it_end - f * flush_st) * U2_KPS));
+            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, p.trunc_ulps,
+                       (float)((it_end - f * flush_st) * U2_KPS) * (CORR16 ? 1.5f : 1.f));      // (the loss model counts two MMAs into D_W per k-step; CORR16 issues three)
             if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, !q.accumulate, 0.f, 0.f);
             tc_fence_before();
             __syncwarp();
@@ -360,7 +371,10 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 const uint64_t dTv = umma_desc(t0 + 2 * UP_B_HALF, UP_B_HALF / 2, 128);
 #ifndef LSP_U2_DBG_NOMMA
                 tc_mma_f16_pair(tmem, dTh, dGh, UP_IDESC, (!win_first || kk > 0) ? 1u : 0u);
-                tc_mma_f8_pair(tmem, dT8, dG8, UP_IDESC_F8, 1u);
+                if (CORR16) {                                           // plane 1 holds fp16 lo parts: A_lo B_hi + A_hi B_lo as two fp16 MMAs
+                    tc_mma_f16_pair(tmem, dT8, dGh, UP_IDESC, 1u);
+                    tc_mma_f16_pair(tmem, dTh, dG8, UP_IDESC, 1u);
+                } else tc_mma_f8_pair(tmem, dT8, dG8, UP_IDESC_F8, 1u);
                 if (!p.unit_x)                                          // (the unit-weight pass of the generalised periodogram needs no V: CC, CS come from the first pass)
                     tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
 #else

@@ -71,7 +71,7 @@ def _qualified(make, seed, ref_fn=None, tries=50):
     raise AssertionError("no qualified seed in %d tries" % tries)
 
 
-PARAM_KEYS = ("K", "THREADS", "NSPLIT", "PIPE", "FLUSH", "TABLE_MB", "COARSE", "TRUNC", "SHARED")
+PARAM_KEYS = ("K", "THREADS", "NSPLIT", "PIPE", "FLUSH", "TABLE_MB", "COARSE", "TRUNC", "SHARED", "CORR")
 
 
 class _params:
@@ -180,6 +180,26 @@ def test_pair_form_ragged(lsp, Nt, Nf, nsplit, flush, table_mb):
     nchunks = 1 if not table_mb else -(-Nt // 256)
     assert plan["pipe"] == TENSOR and "pair2" in plan["kernel"] and plan["K"] == 128
     assert plan["launches"] == (2 if Nt <= 16384 else 3) + 2 * nchunks   # short series: step 1 fused into the records kernel
+
+
+@pytest.mark.parametrize("Nt,Nf,nsplit,table_mb", [(5000, 50011, 0, 0), (4099, 40001, 2, 1), (20011, 70001, 0, 16)])
+def test_pair_form_fp16_corrections(lsp, Nt, Nf, nsplit, table_mb):
+    """LSP_PARAM_CORR = 1: the CTA-pair form with the first-order corrections as two fp16 MMAs on fp16 lo planes (every product of
+    XC, XS carries 22 significant operand bits) instead of one e5m2 MMA: same layout, same table size, four MMAs per k-step.
+    Ragged sizes, time splits and chunks; the result must be closer to the oracle than the tolerance by a wide margin and at
+    least as close as the e5m2 form."""
+    pkg, h = lsp
+    w = workloads.c1(Nt=Nt, Nf=Nf, seed=7000 + Nt)
+    ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
+    P8 = _run_single(h, w, pipe=TENSOR, nsplit=nsplit, coarse=128, table_mb=table_mb)
+    P16 = _run_single(h, w, pipe=TENSOR, nsplit=nsplit, coarse=128, table_mb=table_mb, corr=1)
+    plan = h.last_plan()
+    assert "pair2" in plan["kernel"] and "hi+lo" in plan["kernel"] and "e5m2" not in plan["kernel"], plan
+    e8 = float(np.max(np.abs(P8 - ref)) / ref.max())
+    e16 = float(np.max(np.abs(P16 - ref)) / ref.max())
+    print("pair form Nt=%d: max|dP|/max P = %.2e (e5m2 corrections), %.2e (fp16 hi+lo corrections)" % (Nt, e8, e16))
+    assert e16 <= 2e-5 and e16 <= 1.5 * e8 + 1e-6
+    assert _same_peak(P16, ref, "pair form, fp16 corrections")
 
 
 def test_pair_form_time_chunks_are_bit_identical_run_to_run_and_close_to_unchunked(lsp):

@@ -331,7 +331,7 @@ def run_ours(args):
     h = lsp.Handle(local)
     for key, val in ((lsp.PARAM_K, args.K), (lsp.PARAM_THREADS, args.threads), (lsp.PARAM_NSPLIT, args.nsplit),
                      (lsp.PARAM_FLUSH, args.flush), (lsp.PARAM_TABLE_MB, args.table_mb), (lsp.PARAM_COARSE, args.coarse),
-                     (lsp.PARAM_TRUNC, args.trunc)):
+                     (lsp.PARAM_TRUNC, args.trunc), (lsp.PARAM_CORR, args.corr)):
         if val:
             h.set_param(key, val)
     h.set_param(lsp.PARAM_TIMING, 1)
@@ -632,6 +632,7 @@ def main(argv=None):
     ap.add_argument("--table-mb", type=int, default=0, dest="table_mb")
     ap.add_argument("--coarse", type=int, default=0)
     ap.add_argument("--trunc", type=int, default=0)
+    ap.add_argument("--corr", type=int, default=0, help="with --pipe 2: 1 = LSP_PARAM_CORR (fp16 hi + lo corrections in the CTA-pair kernel)")
     ap.add_argument("--sweep", action="store_true", help="N_t scaling sweep of --workload (single series) instead of the bench line")
     ap.add_argument("--back-to-back", type=int, default=0, dest="back_to_back",
                     help="N back-to-back calls of --workload (single series), eager and as a replayed CUDA graph, instead of the bench line")

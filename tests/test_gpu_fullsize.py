@@ -108,6 +108,22 @@ def test_P0_sampled(lsp, pipe):
     _single_fullsize(h, w, stride=8192, pipe=pipe, windows=wins, what="pipe=%d" % pipe)
 
 
+@pytest.mark.parametrize("name", ["C3", "P0"])
+def test_fp16_hi_lo_corrections_fullsize(lsp, name):
+    """LSP_PARAM_CORR = 1 (bench.py's fast_path_fp16x3: the CTA-pair form with all-fp16 hi + lo operands, four MMAs per k-step) at
+    full size: C3 (one chunk, exact Nyquist in its last bin) and the paper-shaped P0 (two chunks, strongly peaked)."""
+    from paper_1007_1658_b200 import PARAM_CORR
+    pkg, h = lsp
+    w = workloads.c3() if name == "C3" else workloads.p0()
+    h.set_param(PARAM_CORR, 1)
+    try:
+        err, plan = _single_fullsize(h, w, stride=8192, pipe=0, windows=[(w.Nf - 128, w.Nf)], what="LSP_PARAM_CORR=1")
+    finally:
+        h.set_param(PARAM_CORR, 0)
+    assert "pair2" in plan["kernel"] and "hi+lo" in plan["kernel"]
+    assert err <= 2e-5
+
+
 def _batch_fullsize(h, w, golden, shared):
     import torch
     t = torch.from_numpy(w.t).cuda()

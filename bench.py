@@ -578,8 +578,10 @@ def run_back_to_back(args):
     if w.B > 1:
         raise SystemExit("--back-to-back is for a single series")
     h = lsp.Handle(0)
-    if args.pipe:
-        h.set_param(lsp.PARAM_PIPE, args.pipe)
+    for key, val in ((lsp.PARAM_PIPE, args.pipe), (lsp.PARAM_NSPLIT, args.nsplit), (lsp.PARAM_COARSE, args.coarse), (lsp.PARAM_K, args.K),
+                     (lsp.PARAM_THREADS, args.threads)):
+        if val:
+            h.set_param(key, val)
     t_d = torch.from_numpy(np.ascontiguousarray(w.t)).cuda()
     x_d = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
     P_d = torch.empty(w.Nf, dtype=torch.float32, device="cuda")

@@ -181,9 +181,12 @@ int lsp_periodogram_gls_weighted_batched(lsp_handle h,
 
 /*
  * Host-buffer forms: same arithmetic, HOST pointers.  The call copies t and x to the device
- * (cudaMemcpyAsync on `stream`), runs the device path, copies P (and the peaks) back and
- * synchronises `stream`.  Arrays are dense: series b at t + b*Nt, x + b*Nt, P + b*Nf.
+ * (cudaMemcpyAsync), runs the device path, copies P (and the peaks) back and synchronises
+ * `stream`.  Arrays are dense: series b at t + b*Nt, x + b*Nt, P + b*Nf.
  * share_t != 0: t holds ONE time vector of length Nt used by every series.
+ * Batches of >= 64 series that move >= 8 MiB are pipelined over 2 or 4 chunks of series: the copies of a chunk run on two
+ * copy streams owned by the handle while its neighbours compute on `stream` (same kernels, same results; pinned host
+ * buffers are needed for the copies to overlap).
  */
 int lsp_periodogram_host(lsp_handle h,
                          const double* t, const float* x, int64_t Nt,

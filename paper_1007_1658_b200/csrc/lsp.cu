@@ -32,6 +32,7 @@ struct Plan {
 
 }  // namespace
 
+constexpr int HOST_PIPE_CHUNKS = 4;        // host-buffer batches: series chunks whose copies overlap the compute of their neighbours
 constexpr int TIMING_RING = 64;
 constexpr int TIMING_MAX_CHUNKS = 16;      // per-chunk accumulate events (more chunks: the accumulate bracket includes the later table pre-passes)
 
@@ -48,9 +49,11 @@ struct lsp_ctx {
     // workspace
     void* buf = nullptr;
     size_t buf_bytes = 0;
-    // staging for the host-pointer entry points
+    // staging for the host-pointer entry points; copy streams and events of the pipelined batch form
     void* stage = nullptr;
     size_t stage_bytes = 0;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_pipe[2 * HOST_PIPE_CHUNKS + 1] = {};
     Plan plan;
 };
 
@@ -591,6 +594,45 @@ int run_device(lsp_ctx* h,
     return LSP_OK;
 }
 
+// Host-buffer batches: into how many chunks of series (1, 2 or HOST_PIPE_CHUNKS) the call is cut so that the copies of one chunk
+// overlap the compute of its neighbours.  A coarse model decides: copies at ~50 GB/s each way; compute from the terms and the rate
+// of the form the plan picks, times the wave quantisation a smaller grid suffers (a chunk of an FP32-form batch that is 1.15 waves
+// long costs two); chunks are taken only where the modelled pipelined time beats the serial one by >= 10 %.
+int host_pipe_chunks(const lsp_ctx* h, bool share_t, int64_t B, int64_t Nt, int64_t Nf, bool want_P)
+{
+    const double t_in = ((double)(share_t ? 1 : B) * Nt * 8.0 + (double)B * Nt * 4.0) / 50e9;
+    const double t_out = (want_P ? (double)B * Nf * 4.0 : 0.0) / 50e9;
+    if (B < 64 || t_in + t_out < 150e-6) return 1;
+    const double terms = (double)B * (double)Nt * (double)Nf;
+    auto grid = [&](int64_t nb, double& units, double& slots, double& rate) {
+        if (use_shared_path(h, share_t ? 0 : Nt, nb, Nt, false)) {
+            units = (double)((nb + SG_M - 1) / SG_M) * (double)((Nf + SG_F - 1) / SG_F); slots = 2.0 * h->sm_count; rate = 5e13;
+            return true;
+        }
+        Route r;
+        if (route(h, share_t ? 0 : Nt, nb, Nt, Nf, false, r) != LSP_OK) return false;
+        units = (double)(r.duo ? (nb + 1) / 2 : nb) * r.pl.nsplit * r.pl.nfb;
+        if (r.tensor) { slots = (double)plan_umma_ctas_per_sm(r.pl.L) * h->sm_count; rate = r.pair ? 5e13 : 1.2e13; }
+        else { slots = (double)plan_ctas_per_sm(r.pl.K, r.pl.T, r.pl.split_len <= PLAN_FOLD_SAMPLES) * h->sm_count; rate = 4.5e12; }
+        return true;
+    };
+    double u1, s1, rate;
+    if (!grid(B, u1, s1, rate)) return 1;
+    const double t_comp = terms / rate;
+    const double waves1 = u1 > s1 ? std::ceil(u1 / s1) : 1.0;
+    const double serial = t_in + t_comp + t_out;
+    int best = 1; double best_t = serial * 0.9;
+    for (int n = 2; n <= HOST_PIPE_CHUNKS; n *= 2) {
+        double un, sn, rn;
+        if (!grid((B + n - 1) / n, un, sn, rn)) continue;
+        const double wavesn = un > sn ? std::ceil(un / sn) : 1.0;
+        const double comp = t_comp * (n * wavesn) / waves1 * (u1 > s1 ? 1.0 : std::fmax(1.0, n * 0.35));   // under-filled grids: chunks do not get n times shorter
+        const double pipe = std::fmax(t_in + (comp + t_out) / n, std::fmax(comp + (t_in + t_out) / n, t_out + (t_in + comp) / n));
+        if (pipe < best_t) { best_t = pipe; best = n; }
+    }
+    return best;
+}
+
 bool bad_grid(double f_min, double df) {
     return !(std::isfinite(f_min) && std::isfinite(df)) || f_min < 0.0 || df < 0.0;
 }
@@ -651,6 +693,9 @@ int lsp_destroy(lsp_handle h)
     cudaDeviceSynchronize();
     if (h->buf) cudaFree(h->buf);
     if (h->stage) cudaFree(h->stage);
+    if (h->s_in) cudaStreamDestroy(h->s_in);
+    if (h->s_out) cudaStreamDestroy(h->s_out);
+    for (cudaEvent_t e : h->ev_pipe) if (e) cudaEventDestroy(e);
     for (int r = 0; r < TIMING_RING; ++r) {
         for (int i = 0; i < 5; ++i) if (h->ev[r][i]) cudaEventDestroy(h->ev[r][i]);
         for (int i = 0; i < 2 * TIMING_MAX_CHUNKS; ++i) if (h->evc[r][i]) cudaEventDestroy(h->evc[r][i]);
@@ -854,6 +899,45 @@ int lsp_periodogram_batched_host(lsp_handle h, const double* t, int share_t, con
     float* d_P = P ? reinterpret_cast<float*>(base + o_P) : nullptr;
     int32_t* d_pi = peak_idx ? reinterpret_cast<int32_t*>(base + o_pi) : nullptr;
     float* d_pv = peak_val ? reinterpret_cast<float*>(base + o_pv) : nullptr;
+    // Large batches: the series are independent, so the call is pipelined over chunks of series -- the H2D copy of chunk c+1 and
+    // the D2H copy of chunk c-1 run on two copy streams while chunk c computes on `stream` (same kernels, same results).
+    const int nchunk = host_pipe_chunks(h, share_t != 0, B, Nt, Nf, P != nullptr);
+    if (nchunk > 1) {
+        if (!h->s_in) LSP_CUDA(h, cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+        if (!h->s_out) LSP_CUDA(h, cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+        for (cudaEvent_t& e : h->ev_pipe) if (!e) LSP_CUDA(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        cudaEvent_t e_start = h->ev_pipe[2 * HOST_PIPE_CHUNKS];
+        LSP_CUDA(h, cudaEventRecord(e_start, st));                    // earlier work on `stream` may still use the staging buffers
+        LSP_CUDA(h, cudaStreamWaitEvent(h->s_in, e_start, 0));
+        LSP_CUDA(h, cudaStreamWaitEvent(h->s_out, e_start, 0));
+        const int64_t per = (B + nchunk - 1) / nchunk;
+        if (share_t) LSP_CUDA(h, cudaMemcpyAsync(d_t, t, nt_t * sizeof(double), cudaMemcpyHostToDevice, h->s_in));
+        for (int c = 0; c < nchunk; ++c) {                            // all copies in, back to back
+            const int64_t b0 = c * per, nb = (B - b0 < per) ? B - b0 : per;
+            if (nb <= 0) break;
+            if (!share_t) LSP_CUDA(h, cudaMemcpyAsync(d_t + b0 * Nt, t + b0 * Nt, (size_t)nb * Nt * sizeof(double), cudaMemcpyHostToDevice, h->s_in));
+            LSP_CUDA(h, cudaMemcpyAsync(d_x + b0 * Nt, x + b0 * Nt, (size_t)nb * Nt * sizeof(float), cudaMemcpyHostToDevice, h->s_in));
+            LSP_CUDA(h, cudaEventRecord(h->ev_pipe[c], h->s_in));
+        }
+        for (int c = 0; c < nchunk; ++c) {
+            const int64_t b0 = c * per, nb = (B - b0 < per) ? B - b0 : per;
+            if (nb <= 0) break;
+            LSP_CUDA(h, cudaStreamWaitEvent(st, h->ev_pipe[c], 0));
+            rc = run_device(h, share_t ? d_t : d_t + b0 * Nt, share_t ? 0 : Nt, d_x + b0 * Nt, Nt, nb, Nt, f_min, df, Nf,
+                            d_P ? d_P + b0 * Nf : nullptr, Nf, d_pi ? d_pi + b0 : nullptr, d_pv ? d_pv + b0 : nullptr, st);
+            if (rc != LSP_OK) { cudaStreamSynchronize(h->s_in); cudaStreamSynchronize(h->s_out); cudaStreamSynchronize(st); return rc; }
+            LSP_CUDA(h, cudaEventRecord(h->ev_pipe[HOST_PIPE_CHUNKS + c], st));
+            LSP_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_pipe[HOST_PIPE_CHUNKS + c], 0));
+            if (P) LSP_CUDA(h, cudaMemcpyAsync(P + b0 * Nf, d_P + b0 * Nf, (size_t)nb * (size_t)Nf * sizeof(float), cudaMemcpyDeviceToHost, h->s_out));
+            if (peak_idx) {
+                LSP_CUDA(h, cudaMemcpyAsync(peak_idx + b0, d_pi + b0, (size_t)nb * sizeof(int32_t), cudaMemcpyDeviceToHost, h->s_out));
+                LSP_CUDA(h, cudaMemcpyAsync(peak_val + b0, d_pv + b0, (size_t)nb * sizeof(float), cudaMemcpyDeviceToHost, h->s_out));
+            }
+        }
+        LSP_CUDA(h, cudaStreamSynchronize(h->s_out));
+        LSP_CUDA(h, cudaStreamSynchronize(st));
+        return LSP_OK;
+    }
     LSP_CUDA(h, cudaMemcpyAsync(d_t, t, nt_t * sizeof(double), cudaMemcpyHostToDevice, st));
     LSP_CUDA(h, cudaMemcpyAsync(d_x, x, nt_x * sizeof(float), cudaMemcpyHostToDevice, st));
     rc = run_device(h, d_t, share_t ? 0 : Nt, d_x, Nt, B, Nt, f_min, df, Nf, d_P, Nf, d_pi, d_pv, st);

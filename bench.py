@@ -507,6 +507,32 @@ def run_ours(args):
                       "CC, CS in one fp16 pass, fp32 accumulation in the tensor core); reported, not the headline")
         f1["speedup_over_line_of_record"] = r0["ms_per_step"] / f1["ms_per_step"]
         line["fast_path_fp16x3"] = f1
+    if world == 1 and w.name == "C5" and not args.pipe and not args.no_extras:
+        # SURVEY.md section 8(f) row 3 in the driver's own run: the paper-shaped P0 in the FP32 form and the automatic
+        # plan (whole-call device time, median of 5, L2 flushed), and the N_t sweep of this workload in the FP32 form (slope -> 2)
+        extras = {}
+        p0 = workloads.make("P0")
+        t0_d, x0_d = torch.from_numpy(p0.t).cuda(), torch.from_numpy(p0.x).cuda()
+        P0_d = torch.empty(p0.Nf, dtype=torch.float32, device="cuda")
+        for name, pipe in (("fp32", PIPE_FP32), ("automatic", 0)):
+            h.set_param(lsp.PARAM_PIPE, pipe)
+            for _ in range(2):
+                h.periodogram(t0_d, x0_d, p0.f_min, p0.df, p0.Nf, out=P0_d)
+            ms = []
+            for _ in range(5):
+                flush_buf.zero_()
+                ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ea.record(); h.periodogram(t0_d, x0_d, p0.f_min, p0.df, p0.Nf, out=P0_d); eb.record()
+                torch.cuda.synchronize()
+                ms.append(ea.elapsed_time(eb))
+            med = statistics.median(ms)
+            extras["P0_" + name] = {"ms": med, "terms_per_s": p0.terms / (med * 1e-3), "kernel": h.last_plan()["kernel"],
+                                    "peak_index": int(torch.argmax(P0_d)), "expected_peak_bin": p0.expected_peak_bin}
+        extras["P0_note"] = "paper-shaped run: Nt = 382,003, Nf = 1,528,064 (5.84e11 terms, the count behind the paper's Table 2)"
+        h.set_param(lsp.PARAM_PIPE, PIPE_FP32)
+        extras["sweep_fp32"] = sweep_rows(h, w, 5, steps=(16, 8, 4, 2), flush_buf=flush_buf)
+        h.set_param(lsp.PARAM_PIPE, 0)
+        line["extras"] = extras
     if batched:
         # BASELINE config 4: "report per-series peak power distribution" -- the peaks the last host-buffer step returned,
         # and their false-alarm probabilities by eq. (3) with N_ind = Nf (lsp_false_alarm)
@@ -533,15 +559,26 @@ def run_sweep(args):
     """N_t scaling sweep (the paper's Fig. 4): the workload is uniformly
     down-sampled by 64, 32, ..., 1 with N_f in proportion to N_t; whole-call device time (all kernels, CUDA events) per
     size, and the log-log slope d log t / d log N_t, which the paper expects to approach 2.  One JSON line."""
-    import torch
     import paper_1007_1658_b200 as lsp
     base = workloads.make(args.workload)
     h = lsp.Handle(0)
     if args.pipe:
         h.set_param(lsp.PARAM_PIPE, args.pipe)
-    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    rows = sweep_rows(h, base, max(5, args.steps // 2))
+    h.close()
+    print(json.dumps({"metric": "lomb_scargle_Nt_sweep", "workload": base.name, "unit": "ms", "data": "synthetic",
+                      "note": "uniform down-sampling, Nf proportional to Nt (PAPER.md:351-353, eq. (11)); expected slope -> 2",
+                      "sweep": rows}))
+    return 0
+
+
+def sweep_rows(h, base, reps, steps=(64, 32, 16, 8, 4, 2, 1), flush_buf=None):
+    """Whole-call device time of `base` down-sampled by each of `steps` (Nf in proportion), L2 flushed between calls."""
+    import torch
+    if flush_buf is None:
+        flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     rows = []
-    for step in (64, 32, 16, 8, 4, 2, 1):
+    for step in steps:
         w = workloads.downsample(base, step) if step > 1 else base
         t_d = torch.from_numpy(np.ascontiguousarray(w.t)).cuda()
         x_d = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
@@ -550,7 +587,7 @@ def run_sweep(args):
             h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d)
         torch.cuda.synchronize()
         ms = []
-        for _ in range(max(5, args.steps // 2)):
+        for _ in range(reps):
             flush_buf.zero_()
             ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ea.record(); h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, out=P_d); eb.record()
@@ -561,11 +598,7 @@ def run_sweep(args):
                      "kernel": h.last_plan()["kernel"]})
     for a, b in zip(rows[:-1], rows[1:]):
         b["slope_vs_previous"] = float(np.log(b["ms_median"] / a["ms_median"]) / np.log(b["Nt"] / a["Nt"]))
-    h.close()
-    print(json.dumps({"metric": "lomb_scargle_Nt_sweep", "workload": base.name, "unit": "ms", "data": "synthetic",
-                      "note": "uniform down-sampling, Nf proportional to Nt (PAPER.md:351-353, eq. (11)); expected slope -> 2",
-                      "sweep": rows}))
-    return 0
+    return rows
 
 
 def run_back_to_back(args):
@@ -627,6 +660,7 @@ def main(argv=None):
                     help="N > 1: independent series per rank (weak scaling) or frequency slices of one series (strong scaling)")
     ap.add_argument("--pipe", type=int, default=0, help="time ONLY this form (1 = FP32 pipe, 2 = tensor cores) instead of the line of record + fast path")
     ap.add_argument("--no-fast-path", action="store_true", help="skip the automatic-plan sub-record")
+    ap.add_argument("--no-extras", action="store_true", dest="no_extras", help="default C5 run: skip the P0 and N_t-sweep sub-records")
     ap.add_argument("--K", type=int, default=0)
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--nsplit", type=int, default=0)

@@ -256,6 +256,9 @@ int lsp_plan_query_form(int sm_count, int64_t B, int64_t Nt, int64_t Nf, int pip
 /* Name of the accumulate kernel the last call launched (static string; "" before any call). */
 const char* lsp_last_kernel_name(lsp_handle h);
 
+/* Chunks of series the last host-buffer batched call was pipelined over (1: not pipelined; 0 before any such call). */
+int lsp_last_host_chunks(lsp_handle h);
+
 /* Last cudaError_t seen by the handle (0 = cudaSuccess). */
 int lsp_last_cuda_error(lsp_handle h);
 

@@ -23,7 +23,7 @@ SYMBOLS = (
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
     "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched",
     "lsp_periodogram_gls_weighted", "lsp_periodogram_gls_weighted_batched", "lsp_reserve",
-    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_cuda_error",
+    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_host_chunks", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
 
@@ -73,6 +73,7 @@ def load(rebuild: bool = False):
     lib.lsp_plan_query_form.argtypes = [ci, i64, i64, i64, ci, ctypes.POINTER(i64)]
     lib.lsp_last_kernel_name.argtypes = [vp]
     lib.lsp_last_kernel_name.restype = ctypes.c_char_p
+    lib.lsp_last_host_chunks.argtypes = [vp]
     lib.lsp_last_cuda_error.argtypes = [vp]
     lib.lsp_status_string.argtypes = [ci]
     lib.lsp_status_string.restype = ctypes.c_char_p
@@ -175,6 +176,10 @@ class Handle:
         d = dict(zip(keys, [int(v) for v in out]))
         d["kernel"] = self._lib.lsp_last_kernel_name(self._h).decode()
         return d
+
+    def last_host_chunks(self) -> int:
+        """Chunks of series the last host-buffer batched call was pipelined over (1: not pipelined)."""
+        return int(self._lib.lsp_last_host_chunks(self._h))
 
     def last_timing(self) -> dict:
         """Per-kernel milliseconds of the last call (requires set_param(PARAM_TIMING, 1))."""

@@ -53,6 +53,7 @@ struct lsp_ctx {
     void* stage = nullptr;
     size_t stage_bytes = 0;
     cudaStream_t s_in = nullptr, s_out = nullptr;
+    int last_host_chunks = 0;
     cudaEvent_t ev_pipe[2 * HOST_PIPE_CHUNKS + 1] = {};
     Plan plan;
 };
@@ -902,6 +903,7 @@ int lsp_periodogram_batched_host(lsp_handle h, const double* t, int share_t, con
     // Large batches: the series are independent, so the call is pipelined over chunks of series -- the H2D copy of chunk c+1 and
     // the D2H copy of chunk c-1 run on two copy streams while chunk c computes on `stream` (same kernels, same results).
     const int nchunk = host_pipe_chunks(h, share_t != 0, B, Nt, Nf, P != nullptr);
+    h->last_host_chunks = nchunk;
     if (nchunk > 1) {
         if (!h->s_in) LSP_CUDA(h, cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
         if (!h->s_out) LSP_CUDA(h, cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
@@ -980,6 +982,8 @@ int lsp_last_plan(lsp_handle h, int64_t out[8])
 }
 
 const char* lsp_last_kernel_name(lsp_handle h) { return h ? h->plan.kernel_name : ""; }
+
+int lsp_last_host_chunks(lsp_handle h) { return h ? h->last_host_chunks : 0; }
 
 int lsp_last_cuda_error(lsp_handle h) { return h ? h->last_cuda : 0; }
 

@@ -680,6 +680,33 @@ def test_host_entry_points(lsp):
     assert np.array_equal(pi.numpy(), np.array([oracle.argmax(Pref[b]) for b in range(5)], dtype=np.int32))
 
 
+@pytest.mark.parametrize("shared_t", [False, True])
+def test_host_batch_pipelined_over_series_chunks(lsp, shared_t):
+    """A host-buffer batch large enough to be pipelined (copies of one chunk of series overlap the compute of its neighbours, two
+    copy streams of the handle): a ragged series count (chunks of unequal size), full P and peaks, peaks only; the result must be
+    BIT-IDENTICAL to the device-pointer call (same kernels on the same data), and sampled series must match the oracle."""
+    import torch
+    pkg, h = lsp
+    B, Nt, Nf = 1237, 700, 2500
+    w0 = workloads.c4(B=B, Nt=Nt, Nf=Nf, seed=8899)
+    t_np = w0.t[0].copy() if shared_t else w0.t
+    t_h = torch.from_numpy(np.ascontiguousarray(t_np)).pin_memory(); x_h = torch.from_numpy(w0.x).pin_memory()
+    P_h = torch.full((B, Nf), -1.0, dtype=torch.float32).pin_memory()
+    pi_h = torch.full((B,), -1, dtype=torch.int32).pin_memory(); pv_h = torch.full((B,), -1.0, dtype=torch.float32).pin_memory()
+    h.periodogram_batched_host(t_h, x_h, w0.f_min, w0.df, Nf, P=P_h, peak_idx=pi_h, peak_val=pv_h)
+    assert h.last_host_chunks() in ((1, 2, 4) if shared_t else (2, 4)), h.last_host_chunks()      # distinct times: this size is pipelined
+    Pd, pid, pvd = h.periodogram_batched(t_h.cuda(), x_h.cuda(), w0.f_min, w0.df, Nf)
+    torch.cuda.synchronize()
+    assert np.array_equal(P_h.numpy(), Pd.cpu().numpy())
+    assert np.array_equal(pi_h.numpy(), pid.cpu().numpy()) and np.array_equal(pv_h.numpy(), pvd.cpu().numpy())
+    for b in (0, 309, 310, 618, 619, 927, 928, B - 1):         # around the chunk boundaries of 4 x 310 (and of 2 x 619)
+        ref = oracle.periodogram(t_np if shared_t else t_np[b], w0.x[b], w0.f_min, w0.df, Nf)
+        _check(P_h[b].numpy(), ref, "pipelined host batch, series %d" % b)
+    pi2 = torch.full((B,), -1, dtype=torch.int32).pin_memory(); pv2 = torch.full((B,), -1.0, dtype=torch.float32).pin_memory()
+    h.periodogram_batched_host(t_h, x_h, w0.f_min, w0.df, Nf, P=None, peak_idx=pi2, peak_val=pv2)     # peaks only
+    assert np.array_equal(pi2.numpy(), pi_h.numpy()) and np.array_equal(pv2.numpy(), pv_h.numpy())
+
+
 # ------------------------------------------------------------------ generalised periodogram, false-alarm probability
 @pytest.mark.parametrize("prm", [dict(), dict(pipe=FP32), dict(pipe=TENSOR, coarse=128), dict(pipe=TENSOR, coarse=32),
                                  dict(pipe=TENSOR, coarse=128, table_mb=2)])

@@ -132,3 +132,26 @@ def test_reference_arm_is_rank0_only(monkeypatch, capsys):
     args = bench.argparse.Namespace(workload="C1", steps=1, warmup=0, gpus=2)
     assert bench.run_reference(args) == 0
     assert capsys.readouterr().out == ""               # other ranks exit 0 without work
+
+
+def test_roofline_record_is_recomputable():
+    """The bench line's roofline numbers follow from terms, kernel time and the stated peaks: the FP32 form
+    against 148 x 128 lanes x 2 FLOP x clock at 6 lane-ops per term, with the MUFU fraction from 2 MUFU per K terms; the tensor
+    form against the measured sustained bf16 figure at 16 FLOP per term."""
+    import bench
+    peaks = {"sm_max_mhz": 1965.0, "bf16_tflops_sustained": 1376.4, "bf16_tflops": 1628.7}
+    clocks = {"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": []}
+    plan = {"lane_ops_per_term": 6, "K": 32, "kernel": "accum_z_kernel<K=32,fp32,three-term>"}
+    r = bench.roofline_record(1e12, 1, 10**6, 10**6, plan, 194.81, [195.0], clocks, peaks, 148, "C5")
+    peak = 148 * 128 * 2 * 1.965e9 / 1e12
+    assert r["bound"] == "alu" and abs(r["peak"] - peak) < 1e-9
+    assert abs(r["achieved"] - 1e12 * 12 / 0.19481 / 1e12) < 1e-6 and abs(r["frac"] - r["achieved"] / peak) < 1e-12
+    assert abs(r["frac"] - 0.827) < 2e-3
+    assert abs(r["mufu_frac"] - (1e12 * 2 / 32 / 0.19481) / (148 * 16 * 1.965e9)) < 1e-12
+    assert r["algorithmic_bytes"] == 16e6 and abs(r["kernel_share_of_step"] - 194.81 / 195.0) < 1e-12
+    tplan = {"lane_ops_per_term": 0, "K": 128, "kernel": "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16+e5m2corr,fine-table>"}
+    t = bench.roofline_record(1e12, 1, 10**6, 10**6, tplan, 18.37, [19.4], clocks, peaks, 148, "C5")
+    assert t["bound"] == "tensor" and t["peak"] == 1376.4 and t["flop_per_term_algorithmic"] == 16 and t["flop_per_term_executed"] == 24
+    assert abs(t["achieved"] - 1e12 * 16 / 0.01837 / 1e12) < 1e-6 and abs(t["frac"] - t["achieved"] / 1376.4) < 1e-12
+    assert bench.dtype_of(plan) == "f32" and bench.dtype_of(tplan).startswith("f16 + e5m2")
+    assert bench.dtype_of({"lane_ops_per_term": 0, "kernel": "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16,hi+lo,fine-table>"}).startswith("f16 hi+lo")

@@ -66,14 +66,15 @@ enum {
     LSP_PARAM_THREADS   = 2,  /* FP32 form: threads per CTA: 32..256 (multiple of 32; <= 128 for K >= 28) */
     LSP_PARAM_NSPLIT    = 3,  /* number of time-axis splits per (series, frequency block) */
     LSP_PARAM_PIPE      = 4,  /* LSP_PIPE_FP32 or LSP_PIPE_TENSOR (see above) */
-    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the fp32 partial sums / drains of the TMEM accumulators (default 2,048; CTA-pair form 4,096) */
+    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the fp32 partial sums / drains of the TMEM accumulators (default 2,048; CTA-pair form 8,192) */
     LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
     LSP_PARAM_TABLE_MB  = 7,  /* tensor form, CTA-pair kernel: MiB of workspace its operand table may take (default 1,024);  */
                               /* a series whose table (3 KB per sample) is larger runs in time chunks, same result             */
     LSP_PARAM_COARSE    = 8,  /* tensor form: coarse extent L = 16, 32, 64 (a CTA owns 128 L frequencies) or 128 (CTA pairs,   */
                               /* 32,768 frequencies per pair, one operand streamed from the table)                             */
-    LSP_PARAM_TRUNC     = 9,  /* tensor form, CTA-pair kernel: 1 = do not add the expected round-toward-zero loss of the       */
-                              /* tensor-core accumulation back at each drain; 0 = add it (default)       */
+    LSP_PARAM_TRUNC     = 9,  /* tensor forms: 1 = do not add the expected round-toward-zero loss of the tensor-core          */
+                              /* accumulation back at each drain; 0 = add it (default); CTA-pair kernel   */
+                              /* also n > 1: a fixed n / 1000 ulps per 8 samples instead of the model (ablation)                */
     LSP_PARAM_SHARED    = 11, /* batched call with t_stride = 0: 0 = the shared-time GEMM path when B >= 16 and Nt >= 512, 1 = never, 2 = always */
     LSP_PARAM_CORR      = 15, /* tensor form, CTA-pair kernel: how the first-order corrections A_lo B_hi + A_hi B_lo of the fp16 hi + lo   */
                               /* operand split are formed: 0 = one kind::f8f6f4 MMA on e5m2 copies (3 MMAs per 8 samples, the default);  */

@@ -479,9 +479,10 @@ int run_device(lsp_ctx* h,
     const int npass = gls ? 2 : 1;
     // short grids, one pass: records -> accumulate -> finish as programmatic dependents (launch latency and CTA set-up overlap the predecessor's tail)
     const bool pdl_small = r.small && !r.duo && !gls && h->opt_pdl != 1;
-    // drain interval of D_W: 2,048 samples; the CTA-pair form, which adds the expected truncation loss back at each drain
-    // (u2_drain64), takes 4,096 (3 % faster; worst adversarial case 2.6e-5 of max P)
-    const int64_t flush_default = r.pair ? 4096 : 2048;
+    // drain interval of D_W: 2,048 samples; 8,192 in the CTA-pair form, where a drain stalls the whole pipeline of the pair (5 % faster
+    // than 2,048).  The expected truncation loss of a window is added back at its drain (tc_trunc_comp): worst adversarial case
+    // 2.3e-6 of max P at 8,192 samples
+    const int64_t flush_default = r.pair ? 8192 : 2048;
     const int flush_ksteps = (int)(((h->opt_flush ? h->opt_flush : flush_default) + UM_KS - 1) / UM_KS);
     if (r.pair) {
         // CTA-pair form, one time chunk at a time: table pre-pass, then the accumulate launch(es) that read it
@@ -531,7 +532,7 @@ int run_device(lsp_ctx* h,
                 UmmaParams up;
                 up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
                 up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
-                up.flush_ksteps = flush_ksteps; up.trunc_ulps = 0.f; up.unit_x = pass;
+                up.flush_ksteps = flush_ksteps; up.trunc_ulps = h->opt_trunc == 1 ? 0.f : -1.f; up.unit_x = pass;   // (the model, or none: LSP_PARAM_TRUNC = 1)
                 up.t = t; up.t_stride = t_stride; up.x = x; up.x_stride = x_stride; up.f_min = f_min; up.df = df;
                 up.part_var_out = pvar; up.peak64 = peak64; up.counter = counter;
                 if (r.duo) {

@@ -57,13 +57,18 @@ __device__ __forceinline__ void ud_gen_b(const float4* rec, int s0, unsigned l, 
 
 // Drain 32 accumulator columns (one series, one of Re / Im) of this warp's 32 TMEM lanes into one plane of ws:
 // thread = lane = fine value h, column l is frequency k0 + 64 l (coalesced over the lanes).
-__device__ __forceinline__ void ud_drain(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, bool live)
+// n_ksteps > 0: D_W of a drain window of that many k-steps: the expected truncation loss is added back (tc_trunc_comp, three fp16 MMAs).
+__device__ __forceinline__ void ud_drain(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, bool live, float n_ksteps = 0.f, float inv_coherent = 0.f)
 {
     #pragma unroll 1
     for (int part = 0; part < 2; ++part) {
         float v[16];
         tmem_ld16(taddr + 16u * part, v);
         if (!live) continue;
+        if (n_ksteps > 0.f) {
+            #pragma unroll
+            for (int i = 0; i < 16; ++i) v[i] = tc_trunc_comp(v[i], n_ksteps, 1.125f, inv_coherent);
+        }
         const int64_t kp = k0 + (int64_t)part * 16 * UD_H;
         if (!first) {
             #pragma unroll
@@ -86,7 +91,7 @@ struct UmmaDuoParams {
 
 // Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
 // thread = fine value h of series `db`; 16 coarse values l0..l0+15 -> frequencies kb + 64 l + h.
-__device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tbase, int64_t db, bool live, int64_t kh, unsigned l0, unsigned lane)
+__device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tbase, int64_t db, bool live, int64_t kh, unsigned l0, unsigned lane, float n_ksteps)
 {
     const UmmaParams& p = q.u;
     u64 best = 0ull;
@@ -109,6 +114,11 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
         tmem_ld8(tbase + c8 + 128u, cc);
         tmem_ld8(tbase + c8 + 128u + (uint32_t)UD_L, cs);
         if (!live) continue;
+        if (p.trunc_ulps < 0.f) {                                       // XC, XS: the expected truncation loss of the (single) window added back
+            const float ic = 0.6366198f / (16.f * n_ksteps * TC_MEAN_ABS_PRODUCT);
+            #pragma unroll
+            for (int i = 0; i < 8; ++i) { xc[i] = tc_trunc_comp(xc[i], n_ksteps, 1.125f, ic); xs[i] = tc_trunc_comp(xs[i], n_ksteps, 1.125f, ic); }
+        }
         const float inv2var_f = (float)inv2var;
         // fp32 where R <= Nt/2 (no amplification of the rounding of S Nt - D R); fp64 where the denominator Nt^2 - R^2 gets small
         float pf[8];
@@ -236,6 +246,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
         int j_tile = (int)lj;                                                   // this thread's record of the tile being loaded, relative to j_begin
 
         for (int ks = 0; ks < nks; ) {
+          const int ks_begin = ks;
           const int ks_end = min(nks, ks + flush_ksteps);                       // one drain window: the hot loop holds no drain code (registers)
           #pragma unroll 1
           for (; ks < ks_end; ++ks) {
@@ -275,9 +286,11 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 mbar_wait(bar_accf, (uint32_t)flushes & 1u);                    // every MMA issued so far has completed
                 tc_fence_after();
                 if (q.fuse) {                                                   // (host guarantees: this is the only drain of the CTA)
-                    ud_finish16(q, tmem + ((32u * q4) << 16) + 64u * d_s + 16u * part, db, d_live, k0, 16u * part, lane);
+                    ud_finish16(q, tmem + ((32u * q4) << 16) + 64u * d_s + 16u * part, db, d_live, k0, 16u * part, lane, (float)nks);
                 } else {
-                ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live);
+                const float nk = (float)(ks - ks_begin);                // k-steps of this window
+                ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live, p.trunc_ulps < 0.f ? nk : 0.f,
+                         0.6366198f / (16.f * nk * (p.unit_x ? TC_MEAN_ABS_COS : TC_MEAN_ABS_PRODUCT)));
                 if (last) ud_drain(t_drain + 128u, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true, d_live);
                 }
                 tc_fence_before();

@@ -168,16 +168,9 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
 // ------------------------------------------------------------------ step 5: drain 64 accumulator columns into ws
 // Thread = TMEM lane = fine index; its 64 registers are 64 consecutive coarse values h (frequency stride 256).
 //
-// Truncation compensation: the tensor core folds each MMA into the fp32 accumulator with
-// round-toward-zero, a loss in [0, 1) ulp of the running |D| per MMA -- a BIAS toward zero that grows with the window.
-// `comp` = (expected loss in ulps of the FINAL |D|) is added back, away from zero, before the value is folded into `ws`.
-//   mode < 0 (default): the model.  Two MMAs per k-step add into D_W, each losing 1/2 ulp of the RUNNING |D| on average.
-//     A sum that grows from 0 to D_n over the window -- linearly for a coherent signal, whose per-window bias adds up over
-//     the series; like a random walk for noise, with the same mean E[D_t | D_n] = (t/n) D_n -- passes through the binades
-//     below its final one: with m in [1, 2) the mantissa of D_n, sum_t ulp(D_t) = n ulp(D_n) [1 - 1/m + 1/(3m)], so
-//     the expected loss is  n_ksteps x (1 - 2/(3m)) x ulp(D_n)  (0.33 ... 0.67 ulp per k-step, 0.52 on average).
-//   mode > 0: that many ulps of D_n per k-step, whatever m (ablation, LSP_PARAM_TRUNC);  mode = 0: nothing is added.
-__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float mode, float n_ksteps)
+// Truncation compensation: tc_trunc_comp (lsp_tc.cuh).  mode < 0 (default): the model; mode > 0: that many ulps of D_n per k-step,
+// whatever the data (ablation, LSP_PARAM_TRUNC); mode = 0: nothing is added.
+__device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float mode, float n_ksteps, float c0, float inv_coherent)
 {
     #pragma unroll 1
     for (int half = 0; half < 2; ++half) {
@@ -186,11 +179,8 @@ __device__ __forceinline__ void u2_drain64(uint32_t taddr, float* dst, int64_t k
         if (mode != 0.f) {
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
-                const unsigned bits = __float_as_uint(v[i]);
-                const float ulp = __uint_as_float(bits & 0x7f800000u) * 1.1920929e-7f;      // 2^(e-23)
-                float per = mode;
-                if (mode < 0.f) per = 1.f - __fdividef(0.6666667f, __uint_as_float((bits & 0x007fffffu) | 0x3f800000u));
-                v[i] += copysignf(n_ksteps * per * ulp, v[i]);
+                if (mode < 0.f) v[i] = tc_trunc_comp(v[i], n_ksteps, c0, inv_coherent);
+                else v[i] += copysignf(n_ksteps * mode * __uint_as_float(__float_as_uint(v[i]) & 0x7f800000u) * 1.1920929e-7f, v[i]);
             }
         }
         const int64_t kh = k0 + (int64_t)half * 32 * 256;
@@ -344,9 +334,13 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
             const bool last = (f == nwin - 1);
             mbar_wait(bar_accf, (uint32_t)f & 1u);
             tc_fence_after();
-            u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, p.trunc_ulps,
-                       (float)((it_end - f * flush_st) * U2_KPS) * (CORR16 ? 1.5f : 1.f));      // (the loss model counts two MMAs into D_W per k-step; CORR16 issues three)
-            if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, !q.accumulate, 0.f, 0.f);
+            {
+                const float nk = (float)((it_end - f * flush_st) * U2_KPS);                 // k-steps of this window
+                const float mean_abs_product = p.unit_x ? TC_MEAN_ABS_COS : TC_MEAN_ABS_PRODUCT;
+                u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, p.trunc_ulps, nk,
+                           CORR16 ? 1.125f : 0.75f, 0.6366198f / (16.f * nk * mean_abs_product));
+            }
+            if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, !q.accumulate, 0.f, 0.f, 0.f, 0.f);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) { if (rank == 0) mbar_arrive(bar_acce); else mbar_arrive_remote(bar_acce, 0u); }

@@ -101,13 +101,19 @@ __device__ __forceinline__ void us_gen_b(const float4* rec, int s0, unsigned l, 
 // Drain L accumulator columns (one of Re / Im) of this warp's 32 TMEM lanes into one plane of ws.
 // Thread = TMEM lane = row h; column l is frequency k0 + 128 l: for a fixed column the warp touches
 // 32 consecutive frequencies (coalesced).
+// n_ksteps > 0: D_W of a drain window of that many k-steps: the expected truncation loss is added back (tc_trunc_comp; three fp16 MMAs
+// per k-step add into D_W here); 0: no compensation (D_V).
 template <int L>
-__device__ __forceinline__ void us_drain(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first)
+__device__ __forceinline__ void us_drain(uint32_t taddr, float* dst, int64_t k0, int64_t Nf, bool first, float n_ksteps = 0.f, float inv_coherent = 0.f)
 {
     #pragma unroll 1
     for (int part = 0; part < L / 16; ++part) {
         float v[16];
         tmem_ld16(taddr + 16u * part, v);
+        if (n_ksteps > 0.f) {
+            #pragma unroll
+            for (int i = 0; i < 16; ++i) v[i] = tc_trunc_comp(v[i], n_ksteps, 1.125f, inv_coherent);
+        }
         const int64_t kp = k0 + (int64_t)part * 16 * UM_H;
         if (!first) {
             #pragma unroll
@@ -265,7 +271,11 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
             if (++kin == flush_ksteps || last) {
                 mbar_wait(bar_accf, (uint32_t)flushes & 1u);            // every MMA issued so far has completed
                 tc_fence_after();
-                us_drain<L>(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0);
+                {
+                    const float nk = (float)kin;                        // k-steps of this window
+                    us_drain<L>(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, p.trunc_ulps < 0.f ? nk : 0.f,
+                                0.6366198f / (16.f * nk * (p.unit_x ? TC_MEAN_ABS_COS : TC_MEAN_ABS_PRODUCT)));
+                }
                 if (last) us_drain<L>(t_drain + 2u * L, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true);
                 tc_fence_before();
                 __syncwarp();

@@ -23,7 +23,7 @@ SYMBOLS = (
     "lsp_periodogram_host", "lsp_periodogram_batched_host",
     "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched",
     "lsp_periodogram_gls_weighted", "lsp_periodogram_gls_weighted_batched", "lsp_reserve",
-    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_host_chunks", "lsp_last_cuda_error",
+    "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_host_chunks", "lsp_probe_mma_accumulate", "lsp_last_cuda_error",
     "lsp_status_string", "lsp_version",
 )
 
@@ -74,6 +74,7 @@ def load(rebuild: bool = False):
     lib.lsp_last_kernel_name.argtypes = [vp]
     lib.lsp_last_kernel_name.restype = ctypes.c_char_p
     lib.lsp_last_host_chunks.argtypes = [vp]
+    lib.lsp_probe_mma_accumulate.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     lib.lsp_last_cuda_error.argtypes = [vp]
     lib.lsp_status_string.argtypes = [ci]
     lib.lsp_status_string.restype = ctypes.c_char_p
@@ -176,6 +177,12 @@ class Handle:
         d = dict(zip(keys, [int(v) for v in out]))
         d["kernel"] = self._lib.lsp_last_kernel_name(self._h).decode()
         return d
+
+    def probe_mma_accumulate(self):
+        """lsp_probe_mma_accumulate: the accumulator after eight one-element tcgen05.mma sequences (hardware check of DESIGN.md section 8)."""
+        out = (ctypes.c_float * 8)()
+        self._check(self._lib.lsp_probe_mma_accumulate(self._h, out), "lsp_probe_mma_accumulate")
+        return [float(v) for v in out]
 
     def last_host_chunks(self) -> int:
         """Chunks of series the last host-buffer batched call was pipelined over (1: not pipelined)."""

@@ -12,6 +12,7 @@
 #include "lsp_shared_gemm.cuh"
 #include "lsp_finish.cuh"
 #include "lsp_fap.cuh"
+#include "lsp_probe.cuh"
 #include "lsp_plan.h"
 
 #include <cmath>
@@ -970,6 +971,41 @@ int lsp_false_alarm(lsp_handle h, const float* P, int64_t n, int64_t Nt, double 
     fap_kernel<<<(unsigned)blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(P, n, (double)Nt, N_ind, Q);
     LSP_CUDA(h, cudaGetLastError());
     return LSP_OK;
+}
+
+int lsp_probe_mma_accumulate(lsp_handle h, float out[8])
+{
+    if (!h || !out) return LSP_EINVAL;
+    DeviceGuard g(h->device);
+    // start value 2^24 + 2 (ulp 2), built exactly by two MMAs; then one more MMA with the products listed
+    const float big[2] = {4096.f, 4096.f}, two[2] = {2.f, 1.f};
+    const float third[8][PROBE_MAX_PRODUCTS] = {
+        {0.f, 0.f, 0.f, 0.f},                       // [0] nothing:                 2^24 + 2
+        {1.f, 0.f, 0.f, 0.f},                       // [1] + 1  (half an ulp):      truncation keeps 2^24 + 2 (rounding would give 2^24 + 4)
+        {-1.f, 0.f, 0.f, 0.f},                      // [2] - 1:                     2^24
+        {-0.5f, 0.f, 0.f, 0.f},                     // [3] - 0.5 (a quarter ulp):   2^24: within the two extra bits, pulls a whole ulp
+        {-0.0009765625f, 0.f, 0.f, 0.f},            // [4] - 2^-10:                 2^24 + 2: below the extra bits, dropped
+        {-0.75f, -0.75f, -0.75f, -0.75f},           // [5] four times - 0.75:       2^24 (each product cut to - 0.5 first; the exact sum is 2^24 - 1)
+        {0.75f, 0.75f, 0.75f, 0.75f},               // [6] four times + 0.75:       2^24 + 4
+        {3.f, 0.f, 0.f, 0.f},                       // [7] + 3:                     2^24 + 4 (exact 2^24 + 5 truncated)
+    };
+    ProbeSeq host[8];
+    for (int s = 0; s < 8; ++s) {
+        ProbeSeq q = {};
+        q.n = 3;
+        q.a[0][0] = big[0]; q.b[0][0] = big[1]; q.a[1][0] = two[0]; q.b[1][0] = two[1];
+        for (int k = 0; k < PROBE_MAX_PRODUCTS; ++k) { q.a[2][k] = third[s][k]; q.b[2][k] = 1.f; }
+        host[s] = q;
+    }
+    ProbeSeq* d_seq = nullptr; float* d_out = nullptr;
+    LSP_CUDA(h, cudaMalloc(&d_seq, sizeof(host)));
+    cudaError_t e = cudaMalloc(&d_out, 8 * sizeof(float));
+    if (e != cudaSuccess) { cudaFree(d_seq); return cuda_fail(h, e); }
+    e = cudaMemcpy(d_seq, host, sizeof(host), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) { probe_mma_kernel<<<1, 128, 8192>>>(d_seq, 8, d_out); e = cudaGetLastError(); }
+    if (e == cudaSuccess) e = cudaMemcpy(out, d_out, 8 * sizeof(float), cudaMemcpyDeviceToHost);
+    cudaFree(d_seq); cudaFree(d_out);
+    return e == cudaSuccess ? LSP_OK : cuda_fail(h, e);
 }
 
 int lsp_last_plan(lsp_handle h, int64_t out[8])

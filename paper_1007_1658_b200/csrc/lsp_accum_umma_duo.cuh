@@ -91,7 +91,7 @@ struct UmmaDuoParams {
 
 // Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
 // thread = fine value h of series `db`; 16 coarse values l0..l0+15 -> frequencies kb + 64 l + h.
-__device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tbase, int64_t db, bool live, int64_t kh, unsigned l0, unsigned lane, float n_ksteps)
+__device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tbase, int64_t db, bool live, int64_t kh, unsigned l0, unsigned lane)
 {
     const UmmaParams& p = q.u;
     u64 best = 0ull;
@@ -114,11 +114,6 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
         tmem_ld8(tbase + c8 + 128u, cc);
         tmem_ld8(tbase + c8 + 128u + (uint32_t)UD_L, cs);
         if (!live) continue;
-        if (p.trunc_ulps < 0.f) {                                       // XC, XS: the expected truncation loss of the (single) window added back
-            const float ic = 0.6366198f / (16.f * n_ksteps * TC_MEAN_ABS_PRODUCT);
-            #pragma unroll
-            for (int i = 0; i < 8; ++i) { xc[i] = tc_trunc_comp(xc[i], n_ksteps, 1.125f, ic); xs[i] = tc_trunc_comp(xs[i], n_ksteps, 1.125f, ic); }
-        }
         const float inv2var_f = (float)inv2var;
         // fp32 where R <= Nt/2 (no amplification of the rounding of S Nt - D R); fp64 where the denominator Nt^2 - R^2 gets small
         float pf[8];
@@ -286,7 +281,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 mbar_wait(bar_accf, (uint32_t)flushes & 1u);                    // every MMA issued so far has completed
                 tc_fence_after();
                 if (q.fuse) {                                                   // (host guarantees: this is the only drain of the CTA)
-                    ud_finish16(q, tmem + ((32u * q4) << 16) + 64u * d_s + 16u * part, db, d_live, k0, 16u * part, lane, (float)nks);
+                    ud_finish16(q, tmem + ((32u * q4) << 16) + 64u * d_s + 16u * part, db, d_live, k0, 16u * part, lane);   // (one short window of noise-like sums: no compensation, it costs 5 % here)
                 } else {
                 const float nk = (float)(ks - ks_begin);                // k-steps of this window
                 ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live, p.trunc_ulps < 0.f ? nk : 0.f,

@@ -16,7 +16,8 @@
 // fine operand A (128 MUFU sin/cos pairs per sample for 128 L terms), not by the tensor pipe.
 //
 // Step 5 (the chunked sums of PAPER.md:122): tensor-core accumulation rounds toward zero, so D_W is drained every
-// `flush_ksteps` k-steps (default 2,048 samples): tcgen05.ld -> fp32 add (round to nearest) into the CTA's own slice of
+// `flush_ksteps` k-steps (default 2,048 samples): tcgen05.ld -> the expected truncation loss of the window added back
+// (tc_trunc_comp, lsp_tc.cuh) -> fp32 add (round to nearest) into the CTA's own slice of
 // `ws` (L2-resident; first drain stores, later ones read-modify-write; no atomics, deterministic).  D_V only needs
 // Nt-relative accuracy and is drained once, at the end.
 #pragma once

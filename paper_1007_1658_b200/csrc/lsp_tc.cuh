@@ -15,7 +15,8 @@
 // bracket is 2^-12 of the main product and needs ~3 significant bits, so it is either two more fp16 MMAs or ONE
 // kind::f8f6f4 MMA of K = 32 on e5m2 operands (the upper byte of an fp16: same exponent range, no scaling).  V needs
 // only Nt-relative accuracy: one fp16 MMA.  Accumulators: fp32 in TMEM; the tensor core adds with round-toward-zero, so
-// D_W is drained every <= 2,048 samples (the paper's chunked sums).
+// D_W is drained every <= 2,048 samples (8,192 in the CTA-pair form) and the expected loss of the window is added back at the
+// drain (tc_trunc_comp below; the paper's chunked sums).
 #pragma once
 #include "lsp_common.cuh"
 #include <cuda_fp16.h>

@@ -29,7 +29,7 @@
  * Parity pins (tests/test_oracle_pins.py): brute-force least squares, FFT periodogram on
  * even sampling, time-shift invariance, closed form (Nt-1)/2, scipy.signal.lombscargle,
  * Gaussian-noise statistics, injected sinusoid, eqs (5)-(8) equivalence, mpmath brute force;
- * generalised periodogram GP1-GP5, weighted generalised periodogram GW1-GW5.
+ * generalised periodogram GP1-GP6, weighted generalised periodogram GW1-GW5.
  */
 #include <math.h>
 #include <stdint.h>
@@ -121,30 +121,54 @@ int lsp_oracle_periodogram(const double* t, const float* x, int64_t Nt,
 }
 
 /*
- * Generalised (floating-mean) periodogram, the extension the paper names in section 6.3 (PAPER.md:375,
- * Zechmeister & Kuerster 2009; DESIGN.md section 9, SURVEY.md 8(f)-1).  Written here as its DEFINITION, not
- * through their closed-form sums: for every frequency, the unweighted linear least-squares fit of
- *     x_j ~ a cos(w t_j) + b sin(w t_j) + c
- * (normal equations of the 3 basis functions, Gaussian elimination with partial pivoting), and
- *     P = (chi0^2 - chi^2_min) / (2 var),   chi0^2 = sum (x_j - mean)^2,   var = chi0^2 / (Nt - 1)
- * i.e. the same normalisation as eq. (1) (PAPER.md:43), which is the special case c = 0: for the 2-function fit
- * the chi^2 reduction IS eq. (1) (pin P1).  0 <= P <= (Nt - 1)/2.  A singular fit (w = 0: the constant and the
- * cosine coincide) returns 0 (reading G7 carried over).
+ * The least-squares fit both generalised periodograms below are defined by: for one frequency, minimise
+ *     chi^2 = sum_j w_j (X_j - a cos(w t_j) - b sin(w t_j) - c)^2          (w_j = 1 when wts is NULL)
+ * and return chi0^2 - chi^2_min, where X has zero (weighted) mean so that chi0^2 = sum_j w_j X_j^2 belongs to the constant
+ * model.  Normal equations of three basis functions, Gaussian elimination with partial pivoting.
+ *
+ * Reading G15: the model space {cos, sin, 1} does not depend on the time origin or on which basis spans
+ * it, so the fit is posed in the best-conditioned equivalent basis: times measured from their weighted mean,
+ *     g0 = (cos(w t') - 1) - its weighted mean,   g1 = sin(w t') - its weighted mean,   g2 = 1,
+ * with cos - 1 = -2 sin^2(w t'/2) formed without cancellation, and every basis function scaled to unit norm before the
+ * elimination.  The chi^2 reduction is the same number (pin GP6: 60-digit arithmetic on the raw basis); what changes is that
+ * it stays accurate as f T -> 0, where cos -> 1 runs into the constant and the raw normal equations lose every digit (the
+ * earlier form of this function returned 0 below f T ~ 1e-3; the exact fit there is that of a constant + linear + quadratic
+ * trend, which is not small for a series with a drift).  A fit that is singular even so -- a basis function that vanishes on
+ * the samples (f = 0; the aliases of regular sampling), or two that coincide to 1e-12 -- returns 0 (reading G7 carried over).
  */
-static double lsp_oracle_gls_one(const double* t, const double* X, int64_t Nt, double f, double var)
+static double lsp_oracle_gls_fit(const double* t, const double* X, const double* wts, int64_t Nt, double f)
 {
-    const double w = LSP_ORACLE_TWO_PI * f;
-    double M[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};      /* [A^T A | A^T X] */
+    const double om = LSP_ORACLE_TWO_PI * f;
+    double wsum = 0.0, tbar = 0.0;
+    for (int64_t j = 0; j < Nt; ++j) { const double w = wts ? wts[j] : 1.0; wsum += w; tbar += w * t[j]; }
+    tbar /= wsum;
+    double cbar = 0.0, sbar = 0.0;                                     /* weighted means of cos - 1 and sin */
     for (int64_t j = 0; j < Nt; ++j) {
-        const double a = w * t[j];
-        const double g[3] = {cos(a), sin(a), 1.0};
+        const double w = wts ? wts[j] : 1.0, a = om * (t[j] - tbar), sh = sin(0.5 * a);
+        cbar += w * (-2.0 * sh * sh);
+        sbar += w * sin(a);
+    }
+    cbar /= wsum; sbar /= wsum;
+    double M[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};      /* [A^T W A | A^T W X] */
+    for (int64_t j = 0; j < Nt; ++j) {
+        const double w = wts ? wts[j] : 1.0, a = om * (t[j] - tbar), sh = sin(0.5 * a);
+        const double g[3] = {-2.0 * sh * sh - cbar, sin(a) - sbar, 1.0};
         for (int r = 0; r < 3; ++r) {
-            for (int c = 0; c < 3; ++c) M[r][c] += g[r] * g[c];
-            M[r][3] += g[r] * X[j];
+            for (int c = 0; c < 3; ++c) M[r][c] += w * g[r] * g[c];
+            M[r][3] += w * g[r] * X[j];
         }
     }
+    double norm[3];
+    for (int r = 0; r < 3; ++r) {
+        if (!(M[r][r] > 0.0)) return 0.0;                              /* a basis function that vanishes on the samples: G7 */
+        norm[r] = sqrt(M[r][r]);
+    }
+    for (int r = 0; r < 3; ++r) {
+        for (int c = 0; c < 3; ++c) M[r][c] /= norm[r] * norm[c];
+        M[r][3] /= norm[r];
+    }
     const double rhs[3] = {M[0][3], M[1][3], M[2][3]};
-    const double tiny = 1e-12 * (double)Nt;
+    const double tiny = 1e-12;                                         /* relative: the matrix now has a unit diagonal */
     for (int col = 0; col < 3; ++col) {                                /* elimination, partial pivoting */
         int piv = col;
         for (int r = col + 1; r < 3; ++r) if (fabs(M[r][col]) > fabs(M[piv][col])) piv = r;
@@ -161,8 +185,23 @@ static double lsp_oracle_gls_one(const double* t, const double* X, int64_t Nt, d
         for (int c = r + 1; c < 3; ++c) v -= M[r][c] * beta[c];
         beta[r] = v / M[r][r];
     }
-    const double reduction = beta[0] * rhs[0] + beta[1] * rhs[1] + beta[2] * rhs[2];   /* chi0^2 - chi^2_min */
-    return reduction / (2.0 * var);
+    return beta[0] * rhs[0] + beta[1] * rhs[1] + beta[2] * rhs[2];     /* chi0^2 - chi^2_min */
+}
+
+/*
+ * Generalised (floating-mean) periodogram, the extension the paper names in section 6.3 (PAPER.md:375,
+ * Zechmeister & Kuerster 2009; DESIGN.md section 9, SURVEY.md 8(f)-1).  Written here as its DEFINITION, not
+ * through their closed-form sums: for every frequency, the unweighted linear least-squares fit of
+ *     x_j ~ a cos(w t_j) + b sin(w t_j) + c                                (lsp_oracle_gls_fit)
+ * and
+ *     P = (chi0^2 - chi^2_min) / (2 var),   chi0^2 = sum (x_j - mean)^2,   var = chi0^2 / (Nt - 1)
+ * i.e. the same normalisation as eq. (1) (PAPER.md:43), which is the special case c = 0: for the 2-function fit
+ * the chi^2 reduction IS eq. (1) (pin P1).  0 <= P <= (Nt - 1)/2.  A singular fit (w = 0: the constant and the
+ * cosine coincide) returns 0 (reading G7 carried over).
+ */
+static double lsp_oracle_gls_one(const double* t, const double* X, int64_t Nt, double f, double var)
+{
+    return lsp_oracle_gls_fit(t, X, NULL, Nt, f) / (2.0 * var);
 }
 
 /* Same calling convention as lsp_oracle_periodogram. */
@@ -195,7 +234,7 @@ int lsp_oracle_gls(const double* t, const float* x, int64_t Nt,
  * Kuerster 2009, the extension the paper names at PAPER.md:375).  Again the DEFINITION, not their closed-form sums:
  * for every frequency, the WEIGHTED linear least-squares fit
  *     minimise  chi^2 = sum_j w_j (x_j - a cos(w t_j) - b sin(w t_j) - c)^2
- * (weighted normal equations, Gaussian elimination with partial pivoting), against the weighted constant model
+ * (lsp_oracle_gls_fit), against the weighted constant model
  *     chi0^2 = sum_j w_j (x_j - xbar_w)^2,   xbar_w = sum w_j x_j / sum w_j,
  * and  P = (Nt - 1)/2 * (chi0^2 - chi^2_min) / chi0^2.
  * Reading G14: the paper gives no normalisation for the weighted case; this one is the unweighted
@@ -205,38 +244,7 @@ int lsp_oracle_gls(const double* t, const float* x, int64_t Nt,
  */
 static double lsp_oracle_gls_w_one(const double* t, const double* X, const double* w, int64_t Nt, double f, double chi0)
 {
-    const double om = LSP_ORACLE_TWO_PI * f;
-    double M[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};      /* [A^T W A | A^T W X] */
-    double wsum = 0.0;
-    for (int64_t j = 0; j < Nt; ++j) {
-        const double a = om * t[j];
-        const double g[3] = {cos(a), sin(a), 1.0};
-        for (int r = 0; r < 3; ++r) {
-            for (int c = 0; c < 3; ++c) M[r][c] += w[j] * g[r] * g[c];
-            M[r][3] += w[j] * g[r] * X[j];
-        }
-        wsum += w[j];
-    }
-    const double rhs[3] = {M[0][3], M[1][3], M[2][3]};
-    const double tiny = 1e-12 * wsum;
-    for (int col = 0; col < 3; ++col) {                                /* elimination, partial pivoting */
-        int piv = col;
-        for (int r = col + 1; r < 3; ++r) if (fabs(M[r][col]) > fabs(M[piv][col])) piv = r;
-        if (fabs(M[piv][col]) <= tiny) return 0.0;                      /* singular: G7 */
-        if (piv != col) for (int c = 0; c < 4; ++c) { double tmp = M[col][c]; M[col][c] = M[piv][c]; M[piv][c] = tmp; }
-        for (int r = col + 1; r < 3; ++r) {
-            const double q = M[r][col] / M[col][col];
-            for (int c = col; c < 4; ++c) M[r][c] -= q * M[col][c];
-        }
-    }
-    double beta[3];
-    for (int r = 2; r >= 0; --r) {
-        double v = M[r][3];
-        for (int c = r + 1; c < 3; ++c) v -= M[r][c] * beta[c];
-        beta[r] = v / M[r][r];
-    }
-    const double reduction = beta[0] * rhs[0] + beta[1] * rhs[1] + beta[2] * rhs[2];   /* chi0^2 - chi^2_min (X has zero weighted mean) */
-    return 0.5 * (double)(Nt - 1) * reduction / chi0;
+    return 0.5 * (double)(Nt - 1) * lsp_oracle_gls_fit(t, X, w, Nt, f) / chi0;   /* (X has zero weighted mean) */
 }
 
 /* Same calling convention as lsp_oracle_gls plus wts[Nt] fp32 (host) and a second scratch array of Nt doubles. */

@@ -442,6 +442,49 @@ def test_GP5_zechmeister_kuerster_closed_form():
     assert oracle.periodogram_gls(t, x, 0.0, 0.1, 1)[0] == 0.0                  # singular at f = 0 (G7)
 
 
+def test_GP6_low_frequencies_against_60_digit_least_squares():
+    """Reading G15 (oracle/lsp_oracle.c, lsp_oracle_gls_fit): the fit is posed in a centred, scaled basis so that it stays
+    accurate as f T -> 0.  Pin: the SAME fit on the RAW basis {cos(w t), sin(w t), 1} and raw times, solved in 60-digit
+    arithmetic (there the raw normal equations have digits to spare), with and without weights, on a series with a drift
+    (whose low-frequency power is large: the fit tends to that of a quadratic trend), from f T = 1e-6 to 2.5."""
+    import mpmath as mp
+    mp.mp.dps = 60
+    rng = np.random.default_rng(77)
+    Nt, T = 40, 9.0
+    t = 1000.0 + np.sort(rng.uniform(0.0, T, Nt))                          # far from the origin: the centring has work to do
+    x = (rng.standard_normal(Nt) + 0.4 * (t - 1000.0)).astype(np.float32)
+    wts = rng.uniform(0.2, 3.0, Nt).astype(np.float32)
+
+    def exact(weights, f):
+        w = [mp.mpf(float(v)) for v in weights]
+        tm = [mp.mpf(float(v)) for v in t]
+        xm = [mp.mpf(float(v)) for v in x]
+        W = sum(w)
+        mean = sum(a * b for a, b in zip(w, xm)) / W
+        d = [v - mean for v in xm]
+        chi0 = sum(a * b * b for a, b in zip(w, d))
+        A, rhs = mp.zeros(3, 3), mp.zeros(3, 1)
+        for tj, dj, wj in zip(tm, d, w):
+            a = 2 * mp.pi * mp.mpf(f) * tj
+            g = [mp.cos(a), mp.sin(a), mp.mpf(1)]
+            for r in range(3):
+                for c in range(3):
+                    A[r, c] += wj * g[r] * g[c]
+                rhs[r] += wj * g[r] * dj
+        beta = mp.lu_solve(A, rhs)
+        return float((Nt - 1) / 2 * sum(beta[r] * rhs[r] for r in range(3)) / chi0)
+
+    for fT in (1e-6, 1e-4, 1e-2, 0.3, 2.5):
+        f = fT / T
+        want_w, want_u = exact(wts, f), exact(np.ones(Nt), f)
+        got_w = oracle.periodogram_gls_weighted(t, x, wts, f, 0.1, 1)[0]
+        got_u = oracle.periodogram_gls(t, x, f, 0.1, 1)[0]
+        assert abs(got_w - want_w) <= 1e-7 * want_w, (fT, got_w, want_w)
+        assert abs(got_u - want_u) <= 1e-7 * want_u, (fT, got_u, want_u)
+        assert fT > 0.3 or want_u > 1.0                                    # the drift: low-frequency power is not negligible
+    assert oracle.periodogram_gls(t, x, 0.0, 0.1, 1)[0] == 0.0             # f = 0 itself: singular, reading G7
+
+
 # ----------------------------------------------------------------------------- weighted generalised periodogram (GW1-GW5)
 def _weighted_case(Nt=120, seed=31, span=40.0):
     rng, t = _gappy(Nt, seed, span=span)

@@ -13,7 +13,7 @@ from typing import Optional, Tuple
 from . import build as _build
 
 LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM = 0, -1, -2, -3
-PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_PIPE, PARAM_FLUSH, PARAM_TIMING, PARAM_TABLE_MB, PARAM_COARSE, PARAM_TRUNC, PARAM_SHARED, PARAM_PDL, PARAM_CORR = 1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15
+PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_PIPE, PARAM_FLUSH, PARAM_TIMING, PARAM_TABLE_MB, PARAM_COARSE, PARAM_TRUNC, PARAM_SHARED, PARAM_PDL, PARAM_CORR, PARAM_REFINE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15, 16
 PIPE_AUTO, PIPE_FP32, PIPE_TENSOR = 0, 1, 2
 
 # every symbol include/lsp.h declares (checked by tests/test_abi.py against the header text)

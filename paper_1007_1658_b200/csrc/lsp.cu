@@ -42,7 +42,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0, opt_corr = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0, opt_corr = 0, opt_refine = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     cudaEvent_t evc[TIMING_RING][2 * TIMING_MAX_CHUNKS] = {};   // accumulate launches of a chunked call, begin / end per chunk
     int ev_chunks[TIMING_RING] = {};
@@ -50,6 +50,7 @@ struct lsp_ctx {
     // workspace
     void* buf = nullptr;
     size_t buf_bytes = 0;
+    void* refine_buf = nullptr;                           // list of ill-conditioned (series, frequency) pairs left by the fused epilogues (lsp_refine.cuh)
     // staging for the host-pointer entry points; copy streams and events of the pipelined batch form
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -256,6 +257,35 @@ void launch_finish(const FinishParams& fp, int64_t B, cudaStream_t st, bool pdl 
     }
 }
 
+// The list the fused epilogues append their ill-conditioned frequencies to (allocated on first use; its head is 0 between calls:
+// refine_kernel clears it).
+int refine_list(lsp_ctx* h, RefineList& L)
+{
+    constexpr size_t HEAD = 256;
+    if (!h->refine_buf) {
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, HEAD + (size_t)REFINE_LIST_CAP * sizeof(int2));
+        if (e != cudaSuccess) { h->last_cuda = (int)e; cudaGetLastError(); return LSP_ENOMEM; }
+        e = cudaMemset(p, 0, HEAD);
+        if (e != cudaSuccess) { cudaFree(p); return cuda_fail(h, e); }
+        h->refine_buf = p;
+    }
+    L.head = static_cast<unsigned*>(h->refine_buf);
+    L.items = reinterpret_cast<int2*>(static_cast<char*>(h->refine_buf) + HEAD);
+    return LSP_OK;
+}
+
+// After a fused epilogue: steps 6-7 again for the frequencies it listed (none on most grids: the kernel then returns at once).
+cudaError_t launch_refine(const RefineList& list, const RefineSrc& src, const double* pvar, int nparts, float* P, int64_t p_stride,
+                          int32_t* peak_idx, float* peak_val, u64* peak64, cudaStream_t st)
+{
+    RefineParams rp;
+    rp.src = src; rp.list = list; rp.part_var = pvar; rp.nparts = nparts; rp.P = P; rp.p_stride = p_stride;
+    rp.peak_idx = peak_idx; rp.peak_val = peak_val; rp.peak64 = peak64; rp.gls = 0;
+    refine_kernel<<<4 * 148, REFINE_THREADS, 0, st>>>(rp);
+    return cudaGetLastError();
+}
+
 bool use_shared_path(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, bool gls)
 {
     return t_stride == 0 && B > 1 && !gls && h->opt_shared != 1 && h->opt_pipe == 0 &&
@@ -303,6 +333,15 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
         h->ev_chunks[slot] = 0;
         LSP_CUDA(h, cudaEventRecord(ev[0], st));
     }
+    // ill-conditioned frequencies (lsp_refine.cuh): V comes from a single fp16 pass here too
+    RefineSrc src;
+    src.t = t; src.t_stride = 0; src.x = x; src.x_stride = x_stride; src.w = nullptr; src.w_stride = 0; src.f_min = f_min; src.df = df; src.Nt = Nt;
+    const bool refine = h->opt_refine == 0;
+    const double amp = refine ? refine_amplification(true, Nt) : 0.0;
+    const double refine_thr = 1.0 - 1.0 / (refine ? amp : 20.0);
+    const double redo_thr = (refine && refine_thr < 0.5) ? refine_thr : 0.5;      // the epilogue looks closer (fp64, list) above this R / Nt
+    RefineList rlist; rlist.head = nullptr; rlist.items = nullptr;
+    if (fuse && refine) { rc = refine_list(h, rlist); if (rc != LSP_OK) return rc; pl.launches += 1; }
     // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
     const bool fused_pre = pl.fused_pre;                   // short series: step 1's sum inside the records kernel
@@ -318,7 +357,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
     LSP_CUDA(h, cudaGetLastError());
     if (fuse) {
-        shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst, vconst_f);
+        shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst, vconst_f, redo_thr);
         LSP_CUDA(h, cudaGetLastError());
     }
     shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(x, x_stride, psum, pvar, pl.nparts, B, Nt, xa, (int)ng);
@@ -330,6 +369,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     gp.nmb = (int)nmb; gp.nfb_total = (int)nfb; gp.nsplit = (int)nsplit; gp.ng = (int)ng; gp.groups_per_split = (int)gps;
     gp.vconst = fuse ? vconst : nullptr; gp.vconst_f = vconst_f; gp.part_var = pvar; gp.P = P; gp.p_stride = p_stride;
     gp.peak_idx = peak_idx; gp.peak_val = peak_val; gp.peak64 = peak64; gp.counter = counter; gp.Nt = Nt; gp.nparts = pl.nparts;
+    gp.list = rlist; gp.refine_thr = refine_thr;
     LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
     for (int64_t band = 0; band < nbands; ++band) {
         const int64_t nb0 = band * L.band_nfb;
@@ -343,6 +383,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     }
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
     if (fuse) {                                           // steps 6-7 ran in the GEMM's epilogue
+        if (refine) LSP_CUDA(h, launch_refine(rlist, src, pvar, pl.nparts, P, p_stride, peak_idx, peak_val, peak64, st));
         if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
         h->plan = pl;
         return LSP_OK;
@@ -353,6 +394,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = (int)nsplit; fp.nparts = pl.nparts;
     fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
+    fp.src = src; fp.refine_amp = amp;
     launch_finish(fp, B, st);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
@@ -476,6 +518,12 @@ int run_device(lsp_ctx* h,
         LSP_CUDA(h, cudaGetLastError());
     }
 
+    RefineSrc src;                                        // the raw series, for the frequencies whose sums are ill-conditioned
+    src.t = t; src.t_stride = t_stride; src.x = x; src.x_stride = x_stride; src.w = w; src.w_stride = w_stride; src.f_min = f_min; src.df = df; src.Nt = Nt;
+    const bool refine = h->opt_refine == 0;
+    RefineList rlist; rlist.head = nullptr; rlist.items = nullptr;
+    if (r.duo_fuse && refine) { rc = refine_list(h, rlist); if (rc != LSP_OK) return rc; pl.launches += 1; }
+
     // steps 3-5 (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
     const int npass = gls ? 2 : 1;
     // short grids, one pass: records -> accumulate -> finish as programmatic dependents (launch latency and CTA set-up overlap the predecessor's tail)
@@ -541,6 +589,8 @@ int run_device(lsp_ctx* h,
                     dp.u = up; dp.B = B;
                     dp.fuse = r.duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
                     dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
+                    dp.list = rlist;
+                    { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
                     LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
                     accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
                 } else {
@@ -577,6 +627,7 @@ int run_device(lsp_ctx* h,
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
 
     if (r.duo_fuse) {
+        if (refine) LSP_CUDA(h, launch_refine(rlist, src, pvar, pl.nparts, P, p_stride, peak_idx, peak_val, peak64, st));
         if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
         h->plan = pl;
         return LSP_OK;
@@ -589,6 +640,7 @@ int run_device(lsp_ctx* h,
     fp.x_scaled = tensor ? 1 : 0;
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
+    fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt) : 0.0;
     launch_finish(fp, B, st, pdl_small);
     LSP_CUDA(h, cudaGetLastError());
     if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
@@ -695,6 +747,7 @@ int lsp_destroy(lsp_handle h)
     DeviceGuard g(h->device);
     cudaDeviceSynchronize();
     if (h->buf) cudaFree(h->buf);
+    if (h->refine_buf) cudaFree(h->refine_buf);
     if (h->stage) cudaFree(h->stage);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -723,6 +776,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
         case LSP_PARAM_PDL:        if (value > 1) return LSP_EINVAL; h->opt_pdl = value; break;
         case LSP_PARAM_CORR:       if (value > 1) return LSP_EINVAL; h->opt_corr = value; break;
+        case LSP_PARAM_REFINE:     if (value > 1) return LSP_EINVAL; h->opt_refine = value; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;
@@ -744,6 +798,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
         case LSP_PARAM_PDL:        *value = h->opt_pdl; break;
         case LSP_PARAM_CORR:       *value = h->opt_corr; break;
+        case LSP_PARAM_REFINE:     *value = h->opt_refine; break;
         default: return LSP_EINVAL;
     }
     return LSP_OK;

@@ -15,6 +15,7 @@
 // the layout of `ws` are those of lsp_accum_umma_small.cuh; D_W: TMEM columns 0..127, D_V: 128..255; two CTAs per SM.
 #pragma once
 #include "lsp_accum_umma_small.cuh"
+#include "lsp_refine.cuh"
 
 namespace lsp {
 
@@ -87,6 +88,8 @@ struct UmmaDuoParams {
     int fuse;
     float* P; int64_t p_stride;     // nullable
     int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
+    RefineList list;                // fused epilogue: where the ill-conditioned frequencies go (lsp_refine.cuh); head NULL: nowhere
+    float refine_r2;                //   ... those with R^2 above this (refine_amplification)
 };
 
 // Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
@@ -117,12 +120,14 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
         const float inv2var_f = (float)inv2var;
         // fp32 where R <= Nt/2 (no amplification of the rounding of S Nt - D R); fp64 where the denominator Nt^2 - R^2 gets small
         float pf[8];
+        unsigned ill = 0u;                                              // R > 0.95 Nt: to be redone in fp64 by refine_kernel
         #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const float A = 2.f * cc[i], Bv = 2.f * cs[i], R2 = fmaf(A, A, Bv * Bv);
             const float xc2 = xc[i] * xc[i], xs2 = xs[i] * xs[i], S = xc2 + xs2;
             const float DR = fmaf(xc2 - xs2, A, 2.f * xc[i] * xs[i] * Bv);
             pf[i] = fmaxf(2.f * fmaf(S, Nt_f, -DR), 0.f) / fmaf(Nt_f, Nt_f, -R2) * inv2var_f;
+            if (q.list.head && !(R2 < q.refine_r2)) ill |= 1u << i;
             if (R2 > 0.25f * Nt_f * Nt_f) {
                 const double XC = (double)xc[i], XS = (double)xs[i], Ad = 2.0 * (double)cc[i], Bd = 2.0 * (double)cs[i];
                 const double R2d = Ad * Ad + Bd * Bd, x2 = XC * XC, y2 = XS * XS, Sd = x2 + y2;
@@ -138,6 +143,7 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
             const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;
             if (k < p.Nf) {
                 if (q.P) q.P[db * q.p_stride + k] = pf[i];
+                if (((ill >> i) & 1u) && refine_push(q.list, db, k)) continue;      // (its refined value enters the arg-max there)
                 const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
                 best = (key > best) ? key : best;
             }

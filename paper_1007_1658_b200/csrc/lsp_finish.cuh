@@ -10,6 +10,7 @@
 // atomicMax per block -- integer max is order-independent, so the result is deterministic.
 #pragma once
 #include "lsp_common.cuh"
+#include "lsp_refine.cuh"
 
 namespace lsp {
 
@@ -30,6 +31,8 @@ struct FinishParams {
     const float* ws1;                  // generalised periodogram: [B][nsplit][4][Nf] of the unit-weight pass (planes 0, 1 = sum cos, sum sin); else NULL
     const float* ws_x;                 // shared-time batch (lsp_shared_gemm.cuh): XC, XS from [B][nsplit][2][x_row]; `ws` is then ONE
     int64_t x_row;                     //   [nsplit][4][Nf] block shared by all series (planes 2, 3 = CC - n/2, CS); else NULL / 0
+    RefineSrc src;                     // the raw series, for the ill-conditioned frequencies (lsp_refine.cuh)
+    double refine_amp;                 // refine where the sums' rounding is amplified by more than this (refine_amplification); 0: nowhere
 };
 
 // Step 6 for one frequency from the six sums (C1, S1 only for the generalised periodogram), in fp64.
@@ -70,11 +73,15 @@ __device__ __forceinline__ double finish_combine(double XC, double XS, double CC
 // FIN_SL partial sums are then added in lane order by the l = 0 thread.  The order is fixed, so the result is
 // deterministic; with few frequencies and many splits (C1, C2) the sum over the splits is no longer one long dependent chain.
 // FIN_SL = 1 (few splits): one thread per frequency, 256 frequencies per block, no exchange.
+// Frequencies whose sums are ill-conditioned (needs_refine) are then redone by the whole block in fp64, one after the other.
 template <int FIN_SL>
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
 {
     constexpr int FIN_BLOCK_F = FIN_THREADS / FIN_SL;
-    __shared__ double s_var;
+    __shared__ double s_var, s_var_raw;
+    __shared__ int s_nflag;
+    __shared__ short s_flag[FIN_BLOCK_F];
+    __shared__ double s_red[(FIN_THREADS / 32) * 6];
     __shared__ double s_part[FIN_SL > 1 ? 6 : 1][FIN_SL][FIN_SL > 1 ? FIN_BLOCK_F : 1];
     __shared__ u64 s_best[FIN_THREADS / 32];
     const int64_t b = blockIdx.y;
@@ -84,6 +91,8 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
         double q = 0.0;                                    // fixed-order sum of the block partials
         for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
         s_var = q / (double)(p.Nt - 1);                    // sample variance (reading G1)
+        s_var_raw = s_var;
+        s_nflag = 0;
         if (p.x_scaled) {                                  // undo the fp32 scale factor exactly (lsp_tc.cuh)
             const double xs = (double)(float)(1.0 / sqrt(s_var));
             s_var *= xs * xs;
@@ -120,21 +129,35 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
         s_part[4][sl][fl] = C1; s_part[5][sl][fl] = S1;
     }
     __syncthreads();                                       // s_var; the lanes' partial sums
+    const bool owner = live && sl == 0;
+    const bool gls = p.ws1 != nullptr;
+    double v[6] = {XC, XS, CCh, CS, C1, S1};
+    if (owner && FIN_SL > 1) {
+        #pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            double a = 0.0;
+            #pragma unroll
+            for (int l = 0; l < FIN_SL; ++l) a += s_part[q][l][fl];       // fixed order over the lanes
+            v[q] = a;
+        }
+    }
+    float Pf = 0.f;
+    if (owner) Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, gls);
+    if (p.refine_amp > 0.0) {                              // (uniform over the grid)
+        if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) s_flag[atomicAdd(&s_nflag, 1)] = (short)fl;
+        __syncthreads();
+        const int nflag = s_nflag;
+        for (int i = 0; i < nflag; ++i) {                  // the order of the list varies from run to run; each entry's result does not
+            const int f = s_flag[i];
+            double r[6];
+            refine_sums<FIN_THREADS>(p.src, b, (int64_t)blockIdx.x * FIN_BLOCK_F + f, gls, r, s_red);
+            if (owner && fl == f) Pf = (float)refine_combine(r, (double)p.Nt, 0.5 / s_var_raw, gls);
+        }
+    }
     if (sl != 0) return;                                   // (whole warps: FIN_BLOCK_F is a multiple of 32)
 
     u64 best = 0ull;
     if (live) {
-        double v[6] = {XC, XS, CCh, CS, C1, S1};
-        if (FIN_SL > 1) {
-            #pragma unroll
-            for (int q = 0; q < 6; ++q) {
-                double a = 0.0;
-                #pragma unroll
-                for (int l = 0; l < FIN_SL; ++l) a += s_part[q][l][fl];   // fixed order over the lanes
-                v[q] = a;
-            }
-        }
-        const float Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, p.ws1 != nullptr);
         if (p.P) p.P[b * p.p_stride + k] = Pf;
         best = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
     }

@@ -1,0 +1,234 @@
+// lsp_refine.cuh -- step 6 for the ill-conditioned frequencies: the six sums again, in fp64, from the raw series.
+//
+// Eq. (5) divides by (Nt +- R)/2.  Where R -> Nt (f T << 1: every cos^2 is ~1; and the aliases of regular
+// sampling) the second term is (S - D)/(Nt - R), a small difference over a small difference: the rounding of the fp32 sums
+// of steps 4-5 (relative 1e-7 ... 1e-6 of Nt) is amplified by Nt/(Nt - R).  The generalised periodogram has the same
+// structure in its determinant D -> 0.  Such frequencies are few (none on a grid that starts at 1/T unless the sampling is
+// regular), so they are simply done again the slow way: one block per frequency, all Nt samples, phases from t (f_min + k df)
+// in fp64, fp64 sincospi, fp64 sums in a fixed order -- the arithmetic of the paper's CPU code on the few
+// bins that need it.  With fp64 sums the 0/0 decision of reading G7 is taken at the oracle's threshold.
+//
+// Two users: finish_kernel (lsp_finish.cuh) refines the flagged frequencies of its block in place; the fused epilogues
+// (lsp_accum_umma_duo.cuh, lsp_shared_gemm.cuh), which have no block to spare, append (series, frequency) to a bounded
+// list that refine_kernel works off afterwards.
+#pragma once
+#include "lsp_common.cuh"
+
+namespace lsp {
+
+// Which frequencies: those where the rounding of the sums is amplified by more than `amp`, the amplification being
+// Nt / (Nt - R) for eq. (5) and (1/4) / D for the generalised form's determinant D <= 1/4.  The FP32-pipe form's sums are good to
+// ~1e-7 Nt, so amp = 20 (R > 0.95 Nt) keeps every bin within ~2e-6.  The tensor-core forms sum cos 2 theta, sin 2 theta from a
+// single fp16 pass, good to ~5e-4 / sqrt(Nt) of Nt: for 3e-5 the amplification may be 0.06 sqrt(Nt) at
+// most -- R > 0.26 Nt at Nt = 512, R > 0.83 Nt at 10,000, and the FP32 form's 0.95 from 111,000 samples on.  (In a periodogram of
+// noise R / Nt ~ sqrt(ln Nf / Nt): 0.12 at Nt = 512.  Only f T < ~0.4 and aliases get there.)
+__host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt)
+{
+    if (!tensor) return 20.0;
+    const double a = 0.06 * sqrt((double)Nt);
+    return a < 1.35 ? 1.35 : (a > 20.0 ? 20.0 : a);
+}
+constexpr int REFINE_THREADS = 256;
+constexpr int REFINE_LIST_CAP = 1 << 20;     // entries of the fused epilogues' list (8 bytes each: 8 MiB, allocated at the first fused call); overflow keeps the fp32-sum value
+
+struct RefineSrc {
+    const double* t; int64_t t_stride;      // the call's own inputs (device)
+    const float* x; int64_t x_stride;
+    const float* w; int64_t w_stride;       // nullable
+    double f_min, df;
+    int64_t Nt;
+};
+
+struct RefineList {
+    unsigned* head;                          // [0] entries appended, [1] blocks of refine_kernel done; both 0 between calls
+    int2* items;                             // [REFINE_LIST_CAP] {series, frequency index}
+};
+
+__device__ __forceinline__ bool needs_refine(double CCh, double CS, double C1, double S1, double Nt, bool gls, double amp)
+{
+    if (gls) {
+        const double cm = C1 / Nt, sm = S1 / Nt;
+        const double CCn = 0.5 + CCh / Nt - cm * cm, SSn = 0.5 - CCh / Nt - sm * sm, CSn = CS / Nt - cm * sm;
+        return !((CCn * SSn - CSn * CSn) * amp > 0.25);
+    }
+    const double thr = (1.0 - 1.0 / amp) * Nt;                         // R > thr
+    return !(4.0 * (CCh * CCh + CS * CS) < thr * thr);
+}
+
+// false: the list is full (the caller keeps its own value and lets it take part in the arg-max)
+__device__ __forceinline__ bool refine_push(const RefineList& L, int64_t b, int64_t k)
+{
+    const unsigned i = atomicAdd(L.head, 1u);
+    if (i >= (unsigned)REFINE_LIST_CAP) return false;
+    L.items[i] = make_int2((int)b, (int)k);
+    return true;
+}
+
+// Sum over the block of NV values per thread, the same result in every thread: xor-butterfly inside a warp (both partners
+// add the same two numbers), then the warps' sums in warp order.  `red` holds (NT / 32) * NV doubles.
+template <int NT, int NV>
+__device__ __forceinline__ void refine_block_sum(double (&v)[NV], double* red)
+{
+    #pragma unroll
+    for (int q = 0; q < NV; ++q)
+        #pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();                                                    // (red may still be read from the previous call)
+    if (lane == 0) {
+        #pragma unroll
+        for (int q = 0; q < NV; ++q) red[wid * NV + q] = v[q];
+    }
+    __syncthreads();
+    #pragma unroll
+    for (int q = 0; q < NV; ++q) {
+        double a = 0.0;
+        #pragma unroll
+        for (int i = 0; i < NT / 32; ++i) a += red[i * NV + q];
+        v[q] = a;
+    }
+}
+
+// The sums of frequency k of series b in fp64 (every thread of the block calls this with the same arguments and gets the same
+// result), with the (weighted) mean removed from x and the weights scaled to mean 1:
+//   eq. (8):            out = {XC, XS, CC - Nt/2, CS, -, -}, times from t_0
+//   generalised form:   out = {XC', XS', CC', CS', SS', -} over the CENTRED basis c' = cos - mean(cos), s' = sin - mean(sin), times
+//                       from their weighted mean: the fit is the same (the constant absorbs the means, the origin is free by eq. (2)),
+//                       but CC' = sum w c'^2 is summed directly instead of CC - C^2/N, so nothing cancels as f T -> 0
+//                       (cos - 1 = -2 sin^2 of the half angle: exact to fp64 relative precision however small)
+template <int NT>
+__device__ void refine_sums(const RefineSrc& s, int64_t b, int64_t k, bool gls, double (&out)[6], double* red /* (NT / 32) * 6 doubles */)
+{
+    const double* t = s.t + b * s.t_stride;
+    const float* x = s.x + b * s.x_stride;
+    const float* w = s.w ? s.w + b * s.w_stride : nullptr;
+    const int64_t Nt = s.Nt;
+    const double t0 = __ldg(t);
+    double m[3] = {0.0, 0.0, 0.0};                                      // sum w, sum w x, sum w (t - t_0)
+    for (int64_t j = threadIdx.x; j < Nt; j += NT) {
+        const double wj = w ? (double)__ldg(w + j) : 1.0;
+        m[0] += wj; m[1] += wj * (double)__ldg(x + j); m[2] += wj * (__ldg(t + j) - t0);
+    }
+    refine_block_sum<NT, 3>(m, red);
+    const double mean = m[1] / m[0], wn = (double)Nt / m[0];
+    const double f = s.f_min + (double)k * s.df;
+    double v[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (!gls) {
+        for (int64_t j = threadIdx.x; j < Nt; j += NT) {               // time origin t_0: legal by eq. (2), keeps f t small
+            double ph = (__ldg(t + j) - t0) * f;
+            ph -= rint(ph);
+            double sn, cs;
+            sincospi(2.0 * ph, &sn, &cs);
+            const double wj = w ? wn * (double)__ldg(w + j) : 1.0;
+            const double d = wj * ((double)__ldg(x + j) - mean);
+            v[0] += d * cs; v[1] += d * sn;
+            v[2] += wj * (cs * cs - 0.5); v[3] += wj * (cs * sn);
+        }
+        refine_block_sum<NT, 6>(v, red);
+    } else {
+        const double tc = t0 + m[2] / m[0];                             // weighted mean time
+        double a[2] = {0.0, 0.0};                                       // sum w (cos - 1), sum w sin
+        for (int64_t j = threadIdx.x; j < Nt; j += NT) {
+            double ph = (__ldg(t + j) - tc) * f;
+            ph -= rint(ph);
+            double sh, ch;
+            sincospi(ph, &sh, &ch);                                     // half angle
+            const double wj = w ? wn * (double)__ldg(w + j) : 1.0;
+            a[0] += wj * (-2.0 * sh * sh); a[1] += wj * (2.0 * sh * ch);
+        }
+        refine_block_sum<NT, 2>(a, red);
+        const double cbar = a[0] / (double)Nt, sbar = a[1] / (double)Nt;   // (sum of the scaled weights = Nt)
+        for (int64_t j = threadIdx.x; j < Nt; j += NT) {
+            double ph = (__ldg(t + j) - tc) * f;
+            ph -= rint(ph);
+            double sh, ch;
+            sincospi(ph, &sh, &ch);
+            const double wj = w ? wn * (double)__ldg(w + j) : 1.0;
+            const double d = wj * ((double)__ldg(x + j) - mean);
+            const double c1 = -2.0 * sh * sh - cbar, s1 = 2.0 * sh * ch - sbar;
+            v[0] += d * c1; v[1] += d * s1;
+            v[2] += wj * c1 * c1; v[3] += wj * c1 * s1; v[4] += wj * s1 * s1;
+        }
+        refine_block_sum<NT, 6>(v, red);
+    }
+    #pragma unroll
+    for (int q = 0; q < 6; ++q) out[q] = v[q];
+}
+
+// Step 6 from fp64 sums: eq. (5) term by term; the second term is dropped where its denominator (Nt - R)/2 <= 1e-12 Nt,
+// the oracle's own threshold for reading G7 (with fp32 sums finish_combine has to take 1e-6).  Generalised form: the
+// Zechmeister-Kuerster quotient over the centred sums; singular (0, reading G7) where a basis function vanishes on the
+// samples or the two coincide to 1e-12, as in the oracle's scaled elimination.
+__device__ __forceinline__ double refine_combine(const double (&v)[6], double Nt, double inv2var, bool gls)
+{
+    const double XC = v[0], XS = v[1];
+    if (gls) {
+        const double CCn = v[2] / Nt, CSn = v[3] / Nt, SSn = v[4] / Nt;
+        const double prod = CCn * SSn, D = prod - CSn * CSn;
+        if (!(prod > 0.0) || !(D > 1e-12 * prod)) return 0.0;
+        return fmax(SSn * XC * XC + CCn * XS * XS - 2.0 * CSn * XC * XS, 0.0) / (Nt * D) * inv2var;
+    }
+    const double CCh = v[2], CS = v[3];
+    const double A = 2.0 * CCh, Bv = 2.0 * CS;
+    const double R = sqrt(A * A + Bv * Bv);
+    const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
+    const double D = R > 0.0 ? ((xc2 - xs2) * A + 2.0 * XC * XS * Bv) / R : 0.0;
+    double val = fmax(S + D, 0.0) / (Nt + R);
+    if (Nt - R > 2e-12 * Nt) val += fmax(S - D, 0.0) / (Nt - R);
+    return val * inv2var;
+}
+
+struct RefineParams {
+    RefineSrc src;
+    RefineList list;
+    const double* part_var; int nparts;     // [B][nparts]
+    float* P; int64_t p_stride;              // nullable
+    int32_t* peak_idx; float* peak_val; u64* peak64;   // nullable (all or none)
+    int gls;
+};
+
+// Works off the list the fused epilogues left: grid-stride over its entries, one block per entry; the last block to finish
+// publishes the peaks of the series it touched again and clears the list's head for the next call.
+// grid: any (REFINE_GRID blocks), REFINE_THREADS threads.
+__global__ void __launch_bounds__(REFINE_THREADS) refine_kernel(const RefineParams p)
+{
+    __shared__ double red[(REFINE_THREADS / 32) * 6];
+    __shared__ unsigned s_last;
+    pdl_wait();
+    const unsigned appended = *reinterpret_cast<volatile unsigned*>(p.list.head);
+    const unsigned n = appended < (unsigned)REFINE_LIST_CAP ? appended : (unsigned)REFINE_LIST_CAP;
+    for (unsigned e = blockIdx.x; e < n; e += gridDim.x) {
+        const int2 it = p.list.items[e];
+        const int64_t b = it.x, k = it.y;
+        double v[6];
+        refine_sums<REFINE_THREADS>(p.src, b, k, p.gls != 0, v, red);
+        if (threadIdx.x == 0) {
+            double q = 0.0;
+            for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
+            const double var = q / (double)(p.src.Nt - 1);
+            const float Pf = (float)refine_combine(v, (double)p.src.Nt, 0.5 / var, p.gls != 0);
+            if (p.P) p.P[b * p.p_stride + k] = Pf;
+            if (p.peak_idx) atomicMax(p.peak64 + b, ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k));
+        }
+    }
+    if (n == 0 && appended == 0) return;                                // nothing was flagged: head[1] stays 0
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = (atomicAdd(p.list.head + 1, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (p.peak_idx)
+        for (unsigned e = threadIdx.x; e < n; e += REFINE_THREADS) {   // (several entries of one series write the same values)
+            const int b = p.list.items[e].x;
+            const u64 fin = *reinterpret_cast<volatile u64*>(p.peak64 + b);
+            p.peak_idx[b] = (int32_t)(0xffffffffu - (unsigned)(fin & 0xffffffffull));
+            p.peak_val[b] = __uint_as_float((unsigned)(fin >> 32));
+        }
+    __syncthreads();
+    if (threadIdx.x == 0) { p.list.head[0] = 0u; p.list.head[1] = 0u; }
+}
+
+}  // namespace lsp

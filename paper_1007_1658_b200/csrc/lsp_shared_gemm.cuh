@@ -20,6 +20,7 @@
 //                     truncating tensor-core accumulation is folded as often as in the single-series forms.
 #pragma once
 #include "lsp_tc.cuh"
+#include "lsp_refine.cuh"
 
 namespace lsp {
 
@@ -54,12 +55,14 @@ struct SharedGemmParams {
     float* P; int64_t p_stride;     // nullable
     int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
     int64_t Nt; int nparts;
+    RefineList list;                // fused epilogue: where the ill-conditioned frequencies go (lsp_refine.cuh); head NULL: nowhere
+    double refine_thr;              //   ... those with R > refine_thr Nt (refine_amplification)
 };
 
 // Per-frequency part of step 6 for the shared-time batch: from CC - n/2, CS (summed over the splits in fixed order)
 // A = CC - SS, B = 2 CS, R = hypot(A, B) -> (A/R, B/R, 1/(Nt + R), 1/(Nt - R)); eqs (5)-(7), tau eliminated.
 __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restrict__ ws_v, int nsplit, int64_t Nf, int64_t Nt_i, double* __restrict__ vconst,
-                                                            float4* __restrict__ vconst_f)
+                                                            float4* __restrict__ vconst_f, double redo_thr /* <= 0.5: fp32 below R = redo_thr Nt */)
 {
     const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (k >= Nf) return;
@@ -71,7 +74,7 @@ __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restr
     vconst[2 * Nf + k] = 1.0 / (Nt + R);
     vconst[3 * Nf + k] = (Nt - R > 1e-6 * Nt) ? 1.0 / (Nt - R) : 0.0;
     // fp32 copy for the common case R <= Nt/2 (1/(Nt - R) <= 3/(Nt + R): no amplification of the fp32 rounding of S - D)
-    vconst_f[k] = make_float4((R <= 0.5 * Nt) ? (float)vconst[k] : __int_as_float(0x7fc00000), (float)vconst[Nf + k],
+    vconst_f[k] = make_float4((R <= redo_thr * Nt) ? (float)vconst[k] : __int_as_float(0x7fc00000), (float)vconst[Nf + k],
                               (float)vconst[2 * Nf + k], (float)vconst[3 * Nf + k]);
 }
 
@@ -208,6 +211,7 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
             // branch-free fp32 pass: the 32 loads and combines pipeline.  Frequencies with R > Nt/2 carry cf.x = NaN, come out
             // as NaN and are redone in fp64 below (rare: f -> 0, aliases of regular sampling).
             bool redo = false;
+            unsigned ill = 0u;                                          // R > 0.95 Nt: to be redone in fp64 by refine_kernel
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
                 const int64_t k = min(k0 + i, p.Nf - 1);
@@ -226,12 +230,15 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
                     const double xc2 = XC * XC, xs2 = XS * XS, S = xc2 + xs2;
                     const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
                     pf[i] = (float)((fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var);
+                    // R > thr Nt: 1/(Nt + R) < 1/((1 + thr) Nt)
+                    if (p.list.head && k0 + i < p.Nf && __ldg(p.vconst + 2 * p.Nf + k) * ((1.0 + p.refine_thr) * (double)p.Nt) < 1.0) ill |= 1u << i;
                 }
             }
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
                 const int64_t k = k0 + i;
                 if (k < p.Nf) {
+                    if (((ill >> i) & 1u) && refine_push(p.list, b, k)) continue;   // (its refined value enters the arg-max there)
                     const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
                     best = (key > best) ? key : best;
                 }

@@ -157,6 +157,7 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t tabl
 }
 
 // ---- workspace layouts (byte offsets into the handle's buffer)
+constexpr int64_t REFINE_INPLACE_MAX_NT = 16384;        // longer series: finish_kernel lists its ill-conditioned frequencies for refine_kernel (lsp_refine.cuh)
 constexpr int64_t SHARED_E_BUDGET_DEFAULT = (int64_t)256 << 20;   // bytes of workspace the E tiles of the shared-time GEMM may take (per band)
 
 struct SharedLayout {
@@ -261,27 +262,33 @@ void launch_finish(const FinishParams& fp, int64_t B, cudaStream_t st, bool pdl 
 // refine_kernel clears it).
 int refine_list(lsp_ctx* h, RefineList& L)
 {
-    constexpr size_t HEAD = 256;
+    constexpr size_t HEAD = 256, DONE = (size_t)REFINE_SPLIT_ENTRIES * sizeof(unsigned);
+    constexpr size_t PARTIAL = (size_t)REFINE_SPLIT_ENTRIES * REFINE_MAX_SPLIT * 4 * sizeof(double);
     if (!h->refine_buf) {
         void* p = nullptr;
-        cudaError_t e = cudaMalloc(&p, HEAD + (size_t)REFINE_LIST_CAP * sizeof(int2));
+        cudaError_t e = cudaMalloc(&p, HEAD + DONE + PARTIAL + (size_t)REFINE_LIST_CAP * sizeof(int2));
         if (e != cudaSuccess) { h->last_cuda = (int)e; cudaGetLastError(); return LSP_ENOMEM; }
-        e = cudaMemset(p, 0, HEAD);
+        e = cudaMemset(p, 0, HEAD + DONE);
         if (e != cudaSuccess) { cudaFree(p); return cuda_fail(h, e); }
         h->refine_buf = p;
     }
-    L.head = static_cast<unsigned*>(h->refine_buf);
-    L.items = reinterpret_cast<int2*>(static_cast<char*>(h->refine_buf) + HEAD);
+    char* base = static_cast<char*>(h->refine_buf);
+    L.head = reinterpret_cast<unsigned*>(base);
+    L.entry_done = reinterpret_cast<unsigned*>(base + HEAD);
+    L.partial = reinterpret_cast<double*>(base + HEAD + DONE);
+    L.items = reinterpret_cast<int2*>(base + HEAD + DONE + PARTIAL);
     return LSP_OK;
 }
 
 // After a fused epilogue: steps 6-7 again for the frequencies it listed (none on most grids: the kernel then returns at once).
 cudaError_t launch_refine(const RefineList& list, const RefineSrc& src, const double* pvar, int nparts, float* P, int64_t p_stride,
-                          int32_t* peak_idx, float* peak_val, u64* peak64, cudaStream_t st)
+                          int32_t* peak_idx, float* peak_val, u64* peak64, cudaStream_t st, bool gls = false,
+                          const double* psum = nullptr, const double* pw = nullptr)
 {
     RefineParams rp;
     rp.src = src; rp.list = list; rp.part_var = pvar; rp.nparts = nparts; rp.P = P; rp.p_stride = p_stride;
-    rp.peak_idx = peak_idx; rp.peak_val = peak_val; rp.peak64 = peak64; rp.gls = 0;
+    rp.peak_idx = peak_idx; rp.peak_val = peak_val; rp.peak64 = peak64; rp.gls = gls ? 1 : 0;
+    rp.part_sum = psum; rp.part_w = pw;
     refine_kernel<<<4 * 148, REFINE_THREADS, 0, st>>>(rp);
     return cudaGetLastError();
 }
@@ -340,7 +347,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     const double amp = refine ? refine_amplification(true, Nt) : 0.0;
     const double refine_thr = 1.0 - 1.0 / (refine ? amp : 20.0);
     const double redo_thr = (refine && refine_thr < 0.5) ? refine_thr : 0.5;      // the epilogue looks closer (fp64, list) above this R / Nt
-    RefineList rlist; rlist.head = nullptr; rlist.items = nullptr;
+    RefineList rlist = {};
     if (fuse && refine) { rc = refine_list(h, rlist); if (rc != LSP_OK) return rc; pl.launches += 1; }
     // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
@@ -395,8 +402,12 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = (int)nsplit; fp.nparts = pl.nparts;
     fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
     fp.src = src; fp.refine_amp = amp;
+    fp.list = RefineList{};
+    const bool listed = refine && Nt > REFINE_INPLACE_MAX_NT;
+    if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }
     launch_finish(fp, B, st);
     LSP_CUDA(h, cudaGetLastError());
+    if (listed) LSP_CUDA(h, launch_refine(fp.list, src, pvar, pl.nparts, P, p_stride, peak_idx, peak_val, peak64, st, false, psum));
     if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
     h->plan = pl;
     return LSP_OK;
@@ -521,7 +532,7 @@ int run_device(lsp_ctx* h,
     RefineSrc src;                                        // the raw series, for the frequencies whose sums are ill-conditioned
     src.t = t; src.t_stride = t_stride; src.x = x; src.x_stride = x_stride; src.w = w; src.w_stride = w_stride; src.f_min = f_min; src.df = df; src.Nt = Nt;
     const bool refine = h->opt_refine == 0;
-    RefineList rlist; rlist.head = nullptr; rlist.items = nullptr;
+    RefineList rlist = {};
     if (r.duo_fuse && refine) { rc = refine_list(h, rlist); if (rc != LSP_OK) return rc; pl.launches += 1; }
 
     // steps 3-5 (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
@@ -641,8 +652,12 @@ int run_device(lsp_ctx* h,
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
     fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt) : 0.0;
+    fp.list = RefineList{};
+    const bool listed = refine && Nt > REFINE_INPLACE_MAX_NT;
+    if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }
     launch_finish(fp, B, st, pdl_small);
     LSP_CUDA(h, cudaGetLastError());
+    if (listed) LSP_CUDA(h, launch_refine(fp.list, src, pvar, pl.nparts, P, p_stride, peak_idx, peak_val, peak64, st, gls, psum, weighted ? pw : nullptr));
     if (timing) { LSP_CUDA(h, cudaEventRecord(ev[4], st)); h->timed_calls++; }
 
     h->plan = pl;

@@ -33,6 +33,8 @@ struct FinishParams {
     int64_t x_row;                     //   [nsplit][4][Nf] block shared by all series (planes 2, 3 = CC - n/2, CS); else NULL / 0
     RefineSrc src;                     // the raw series, for the ill-conditioned frequencies (lsp_refine.cuh)
     double refine_amp;                 // refine where the sums' rounding is amplified by more than this (refine_amplification); 0: nowhere
+    RefineList list;                   // head != NULL (long series): append the flagged frequencies here for refine_kernel (one block each,
+                                       //   in parallel) instead of redoing them one after the other inside this block
 };
 
 // Step 6 for one frequency from the six sums (C1, S1 only for the generalised periodogram), in fp64.
@@ -143,7 +145,10 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     }
     float Pf = 0.f;
     if (owner) Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, gls);
-    if (p.refine_amp > 0.0) {                              // (uniform over the grid)
+    bool listed = false;                                   // refine_kernel will write this frequency and enter it in the arg-max
+    if (p.refine_amp > 0.0 && p.list.head) {
+        if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) listed = refine_push(p.list, b, k);
+    } else if (p.refine_amp > 0.0) {                       // (uniform over the grid)
         if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) s_flag[atomicAdd(&s_nflag, 1)] = (short)fl;
         __syncthreads();
         const int nflag = s_nflag;
@@ -159,7 +164,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     u64 best = 0ull;
     if (live) {
         if (p.P) p.P[b * p.p_stride + k] = Pf;
-        best = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+        if (!listed) best = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
     }
     if (p.peak_idx == nullptr) return;
     #pragma unroll

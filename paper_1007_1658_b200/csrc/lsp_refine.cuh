@@ -39,9 +39,15 @@ struct RefineSrc {
     int64_t Nt;
 };
 
+constexpr int REFINE_SPLIT_ENTRIES = 256;   // refine_kernel: up to this many listed frequencies of long series are each spread over ...
+constexpr int REFINE_MAX_SPLIT = 64;        // ... up to this many blocks (ranges of samples), REFINE_SPLIT_MIN samples or more each
+constexpr int REFINE_SPLIT_MIN = 4096;
+
 struct RefineList {
     unsigned* head;                          // [0] entries appended, [1] blocks of refine_kernel done; both 0 between calls
     int2* items;                             // [REFINE_LIST_CAP] {series, frequency index}
+    double* partial;                         // [REFINE_SPLIT_ENTRIES][REFINE_MAX_SPLIT][4] sums of a range of samples
+    unsigned* entry_done;                    // [REFINE_SPLIT_ENTRIES] ranges of the entry summed so far; 0 between calls
 };
 
 __device__ __forceinline__ bool needs_refine(double CCh, double CS, double C1, double S1, double Nt, bool gls, double amp)
@@ -89,6 +95,29 @@ __device__ __forceinline__ void refine_block_sum(double (&v)[NV], double* red)
     }
 }
 
+// eq. (8) over the samples j0 <= j < j1 of series b at frequency k, in fp64: v = {XC, XS, CC - n/2, CS} (v[4], v[5] untouched = 0);
+// `mean` = the (weighted) mean of x, `wn` = Nt / sum of the weights.  Time origin t_0: legal by eq. (2), keeps f t small.
+template <int NT>
+__device__ void refine_sums_range(const RefineSrc& s, int64_t b, int64_t k, double mean, double wn, int64_t j0, int64_t j1,
+                                  double (&v)[6], double* red)
+{
+    const double* t = s.t + b * s.t_stride;
+    const float* x = s.x + b * s.x_stride;
+    const float* w = s.w ? s.w + b * s.w_stride : nullptr;
+    const double t0 = __ldg(t), f = s.f_min + (double)k * s.df;
+    for (int64_t j = j0 + threadIdx.x; j < j1; j += NT) {
+        double ph = (__ldg(t + j) - t0) * f;
+        ph -= rint(ph);
+        double sn, cs;
+        sincospi(2.0 * ph, &sn, &cs);
+        const double wj = w ? wn * (double)__ldg(w + j) : 1.0;
+        const double d = wj * ((double)__ldg(x + j) - mean);
+        v[0] += d * cs; v[1] += d * sn;
+        v[2] += wj * (cs * cs - 0.5); v[3] += wj * (cs * sn);
+    }
+    refine_block_sum<NT, 6>(v, red);
+}
+
 // The sums of frequency k of series b in fp64 (every thread of the block calls this with the same arguments and gets the same
 // result), with the (weighted) mean removed from x and the weights scaled to mean 1:
 //   eq. (8):            out = {XC, XS, CC - Nt/2, CS, -, -}, times from t_0
@@ -114,17 +143,7 @@ __device__ void refine_sums(const RefineSrc& s, int64_t b, int64_t k, bool gls, 
     const double f = s.f_min + (double)k * s.df;
     double v[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     if (!gls) {
-        for (int64_t j = threadIdx.x; j < Nt; j += NT) {               // time origin t_0: legal by eq. (2), keeps f t small
-            double ph = (__ldg(t + j) - t0) * f;
-            ph -= rint(ph);
-            double sn, cs;
-            sincospi(2.0 * ph, &sn, &cs);
-            const double wj = w ? wn * (double)__ldg(w + j) : 1.0;
-            const double d = wj * ((double)__ldg(x + j) - mean);
-            v[0] += d * cs; v[1] += d * sn;
-            v[2] += wj * (cs * cs - 0.5); v[3] += wj * (cs * sn);
-        }
-        refine_block_sum<NT, 6>(v, red);
+        refine_sums_range<NT>(s, b, k, mean, wn, 0, Nt, v, red);
     } else {
         const double tc = t0 + m[2] / m[0];                             // weighted mean time
         double a[2] = {0.0, 0.0};                                       // sum w (cos - 1), sum w sin
@@ -182,6 +201,8 @@ struct RefineParams {
     RefineSrc src;
     RefineList list;
     const double* part_var; int nparts;     // [B][nparts]
+    const double* part_sum;                  // [B][nparts] sum x (weighted: sum w x) from moments_kernel, or NULL: no spreading over blocks
+    const double* part_w;                    // [B][nparts] sum w (weighted form), else NULL
     float* P; int64_t p_stride;              // nullable
     int32_t* peak_idx; float* peak_val; u64* peak64;   // nullable (all or none)
     int gls;
@@ -197,6 +218,53 @@ __global__ void __launch_bounds__(REFINE_THREADS) refine_kernel(const RefinePara
     pdl_wait();
     const unsigned appended = *reinterpret_cast<volatile unsigned*>(p.list.head);
     const unsigned n = appended < (unsigned)REFINE_LIST_CAP ? appended : (unsigned)REFINE_LIST_CAP;
+    // long series, few entries: each entry's samples are cut into S ranges, one block each (a block sums 256 samples of fp64
+    // sincospi in ~600 cycles whatever its size: the only way to go faster is more SMs); the block that finishes an entry last adds
+    // the S partial sums in range order, so the result does not depend on which block that is
+    const int64_t Nt = p.src.Nt;
+    unsigned S = 1;
+    if (!p.gls && p.part_sum && n > 0 && n <= (unsigned)REFINE_SPLIT_ENTRIES) {
+        const int64_t by_len = Nt / REFINE_SPLIT_MIN;
+        S = gridDim.x / n;
+        if ((int64_t)S > by_len) S = (unsigned)by_len;
+        if (S > (unsigned)REFINE_MAX_SPLIT) S = (unsigned)REFINE_MAX_SPLIT;
+        if (S < 1) S = 1;
+    }
+    if (S > 1) {
+        const unsigned item = blockIdx.x;                               // n S <= gridDim.x items
+        if (item < n * S) {
+            const unsigned e = item / S, r = item % S;
+            const int2 it = p.list.items[e];
+            const int64_t b = it.x, k = it.y;
+            double sx = 0.0, sw = 0.0;                                  // (every thread: nparts <= 128 loads from L2)
+            for (int i = 0; i < p.nparts; ++i) { sx += p.part_sum[b * p.nparts + i]; if (p.part_w) sw += p.part_w[b * p.nparts + i]; }
+            if (!p.part_w) sw = (double)Nt;
+            int64_t len = (Nt + S - 1) / S;
+            len = (len + REFINE_THREADS - 1) / REFINE_THREADS * REFINE_THREADS;
+            const int64_t j0 = (int64_t)r * len, j1 = (j0 + len < Nt) ? j0 + len : Nt;
+            double v[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+            refine_sums_range<REFINE_THREADS>(p.src, b, k, sx / sw, (double)Nt / sw, j0, j1, v, red);
+            if (threadIdx.x == 0) {
+                double* mine = p.list.partial + ((size_t)e * REFINE_MAX_SPLIT + r) * 4;
+                mine[0] = v[0]; mine[1] = v[1]; mine[2] = v[2]; mine[3] = v[3];
+                __threadfence();
+                if (atomicAdd(p.list.entry_done + e, 1u) == S - 1) {    // the entry's last range: fold in range order
+                    __threadfence();
+                    double a[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+                    for (unsigned q = 0; q < S; ++q) {
+                        const volatile double* part = p.list.partial + ((size_t)e * REFINE_MAX_SPLIT + q) * 4;
+                        a[0] += part[0]; a[1] += part[1]; a[2] += part[2]; a[3] += part[3];
+                    }
+                    double qv = 0.0;
+                    for (int i = 0; i < p.nparts; ++i) qv += p.part_var[b * p.nparts + i];
+                    const float Pf = (float)refine_combine(a, (double)Nt, 0.5 / (qv / (double)(Nt - 1)), false);
+                    if (p.P) p.P[b * p.p_stride + k] = Pf;
+                    if (p.peak_idx) atomicMax(p.peak64 + b, ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k));
+                    p.list.entry_done[e] = 0u;                          // (for the next call)
+                }
+            }
+        }
+    } else
     for (unsigned e = blockIdx.x; e < n; e += gridDim.x) {
         const int2 it = p.list.items[e];
         const int64_t b = it.x, k = it.y;

@@ -179,7 +179,7 @@ def test_pair_form_ragged(lsp, Nt, Nf, nsplit, flush, table_mb):
     plan = h.last_plan()
     nchunks = 1 if not table_mb else -(-Nt // 256)
     assert plan["pipe"] == TENSOR and "pair2" in plan["kernel"] and plan["K"] == 128
-    assert plan["launches"] == (2 if Nt <= 16384 else 3) + 2 * nchunks   # short series: step 1 fused into the records kernel
+    assert plan["launches"] == (2 if Nt <= 16384 else 4) + 2 * nchunks   # short series: step 1 fused into the records kernel; long: + refine_kernel
 
 
 @pytest.mark.parametrize("Nt,Nf,nsplit,table_mb", [(5000, 50011, 0, 0), (4099, 40001, 2, 1), (20011, 70001, 0, 16)])
@@ -209,9 +209,9 @@ def test_pair_form_time_chunks_are_bit_identical_run_to_run_and_close_to_unchunk
     w = workloads.c1(Nt=20011, Nf=70001, seed=515)
     ref = oracle.periodogram(w.t, w.x, w.f_min, w.df, w.Nf)
     one = _run_single(h, w, pipe=TENSOR, coarse=128)
-    assert h.last_plan()["launches"] == 3 + 2
+    assert h.last_plan()["launches"] == 4 + 2                          # moments, records, finish, refine + table, accumulate
     a = _run_single(h, w, pipe=TENSOR, coarse=128, table_mb=16)        # 16 MiB / 3 KB = 5,461 -> 4 chunks of 5,120 (last: 4,651)
-    assert h.last_plan()["launches"] == 3 + 2 * 4
+    assert h.last_plan()["launches"] == 4 + 2 * 4
     b = _run_single(h, w, pipe=TENSOR, coarse=128, table_mb=16)
     assert np.array_equal(a, b)
     _check(one, ref, "unchunked"); _check(a, ref, "4 chunks")

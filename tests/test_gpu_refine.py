@@ -79,6 +79,10 @@ FORMS = [  # name, B, Nt, shared_t, params, kernel substring, launches the refin
     ("duo", 7, 3000, False, dict(pipe=2, coarse=16), "accum_umma_duo_kernel", False),
     ("shared-gemm-fused", 21, 1000, True, dict(), "shared-times,fused-finish", True),
     ("shared-gemm", 21, 9000, True, dict(), "shared_gemm_kernel", False),
+    # Nt > 16,384: finish_kernel lists the flagged frequencies for refine_kernel instead of redoing them inside its block
+    ("fp32-long", 1, 20000, False, dict(pipe=1), "accum_z_kernel", False),
+    ("pair-long", 2, 20000, False, dict(pipe=2, coarse=128), "accum_umma_pair2_kernel", False),
+    ("shared-gemm-long", 17, 20000, True, dict(), "shared_gemm_kernel", False),
 ]
 
 
@@ -111,19 +115,20 @@ def test_low_frequencies_every_form(lsp, name, B, Nt, shared_t, params, kernel, 
     assert np.array_equal(P[:, 150:], P0[:, 150:])           # (f T >= 0.6: R is small, nothing is flagged, nothing changes)
 
 
+@pytest.mark.parametrize("Nt", [2500, 20000], ids=["in-block", "listed"])
 @pytest.mark.parametrize("weighted", [False, True])
 @pytest.mark.parametrize("params,kernel", [(dict(pipe=1), "accum_z_kernel"), (dict(pipe=2, coarse=128), "accum_umma_pair2_kernel")],
                          ids=["fp32", "pair"])
-def test_generalised_periodogram_low_frequencies(lsp, weighted, params, kernel):
+def test_generalised_periodogram_low_frequencies(lsp, weighted, params, kernel, Nt):
     """The floating-mean fit as f T -> 0 tends to that of a quadratic trend (not to 0): large on a series with a drift.  The
     closed-form determinant of the fp32 sums is useless there; the refinement sums the centred basis directly in fp64.
     Oracle: the least-squares definition in its well-conditioned form (reading G15, pin GP6)."""
     pkg, h = lsp
-    B, Nt, T = 2, 2500, 80.0
+    B, T = 2, 80.0
     t, x = _series(B, Nt, T, seed=41)
     rng = np.random.default_rng(5)
     w = rng.uniform(0.2, 3.0, (B, Nt)).astype(np.float32) if weighted else None
-    f_min, df, Nf = 0.0, 0.0007 / T, 400                      # f T = 0 ... 0.28
+    f_min, df, Nf = 0.0, 0.0007 / T, (400 if Nt < 10000 else 150)   # f T = 0 ... 0.28 (0.1)
     ref = _ref(t, x, f_min, df, Nf, gls=True, w=w)
     P, pi, pv, plan = _gpu(h, pkg, t, x, f_min, df, Nf, gls=True, w=w, **params)
     assert kernel in plan["kernel"]

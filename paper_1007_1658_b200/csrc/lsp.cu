@@ -345,7 +345,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     src.t = t; src.t_stride = 0; src.x = x; src.x_stride = x_stride; src.w = nullptr; src.w_stride = 0; src.f_min = f_min; src.df = df; src.Nt = Nt;
     const bool refine = h->opt_refine == 0;
     const double amp = refine ? refine_amplification(true, Nt) : 0.0;
-    const double refine_thr = 1.0 - 1.0 / (refine ? amp : 20.0);
+    const double refine_thr = 1.0 - 1.0 / (refine ? amp : 10.0);
     const double redo_thr = (refine && refine_thr < 0.5) ? refine_thr : 0.5;      // the epilogue looks closer (fp64, list) above this R / Nt
     RefineList rlist = {};
     if (fuse && refine) { rc = refine_list(h, rlist); if (rc != LSP_OK) return rc; pl.launches += 1; }
@@ -357,8 +357,8 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
         LSP_CUDA(h, cudaGetLastError());
     } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    if (fused_pre) records_kernel<true, true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
-    else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
+    if (fused_pre) records_kernel<true, true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
+    else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
     LSP_CUDA(h, cudaGetLastError());
     // CC, CS once per frequency
     shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
@@ -518,9 +518,9 @@ int run_device(lsp_ctx* h,
         LSP_CUDA(h, cudaGetLastError());
     } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar);
-    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
-    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter);
+    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar, origin_offset(f_min, df, Nf));
+    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
+    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
     LSP_CUDA(h, cudaGetLastError());
     }
     if (weighted) pl.launches -= 1;                       // (the weight records were written by records_weighted_kernel)
@@ -651,7 +651,7 @@ int run_device(lsp_ctx* h,
     fp.x_scaled = tensor ? 1 : 0;
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
-    fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt) : 0.0;
+    fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt, gls) : 0.0;
     fp.list = RefineList{};
     const bool listed = refine && Nt > REFINE_INPLACE_MAX_NT;
     if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }

@@ -12,6 +12,21 @@
 
 namespace lsp {
 
+// Where the time origin goes (reading G6: P does not depend on it, eq. (2)).  The FP32-pipe form steps from one frequency to the
+// next with z_{m+1} = 2 cos d_j z_m - z_{m-1}, d_j = 2 pi df t'_j, and the fp32 rounding of 2 cos d_j is an error 6e-8 / sin d_j in
+// the step angle, applied K times: samples whose d_j is near 0 or pi carry it.  With the origin at t_0 that is every sample close
+// to the start of the series -- all of them on a grid much finer than 1/T.  With the origin 1/(8 df) BEFORE t_0 the step angles
+// start at pi/4, and stay inside [pi/4, 3 pi/4] whenever df T <= 1/4 (an oversampling of 4 or more): sin d_j >= 0.71 for every
+// sample.  The phases are exact 64-bit turns of the fp64 products, so the longer lever arm costs nothing (bounded to 1e7 cycles
+// at the highest frequency, where the fp64 rounding of t' is still 1e-9 cycles).
+__host__ __device__ inline double origin_offset(double f_min, double df, int64_t Nf)
+{
+    const double f_max = f_min + (double)(Nf - 1) * df;
+    double off = (df > 0.0) ? 0.125 / df : 0.0;
+    if (off * f_max > 1e7) off = 1e7 / f_max;
+    return off;
+}
+
 // grid (nb, B), any block size (multiple of 32).  part_sum[b][blk] = sum of x over the block's chunk.
 // Weighted generalised periodogram (w != NULL): part_sum = sum w x and part_w = sum w over the chunk.
 __global__ void moments_kernel(const float* __restrict__ x, int64_t x_stride, int64_t Nt,
@@ -51,7 +66,7 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
                                         int64_t Nt, int64_t chunk, double f_min, double df,
                                         const double* __restrict__ part_sum, const double* __restrict__ part_w,
                                         float4* __restrict__ recA, float4* __restrict__ recA1, ulonglong2* __restrict__ recB,
-                                        double* __restrict__ part_var)
+                                        double* __restrict__ part_var, double t_off /* origin_offset() */)
 {
     __shared__ double red[32];
     const int b = blockIdx.y;
@@ -63,7 +78,7 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
     for (int i = 0; i < nb; ++i) { swx += part_sum[(int64_t)b * nb + i]; sw += part_w[(int64_t)b * nb + i]; }
     const double mean = swx / sw;
     const double wscale = (double)Nt / sw;
-    const double t0 = __ldg(tb);
+    const double t0 = __ldg(tb) - t_off;
     const int64_t j0 = (int64_t)blockIdx.x * chunk;
     const int64_t j1 = min(Nt, j0 + chunk);
     double acc = 0.0;
@@ -99,7 +114,7 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                double* __restrict__ part_sum,
                                float4* __restrict__ recA, ulonglong2* __restrict__ recB,
                                double* __restrict__ part_var,
-                               u64* __restrict__ peak64, unsigned* __restrict__ counter)
+                               u64* __restrict__ peak64, unsigned* __restrict__ counter, double t_off /* origin_offset() */)
 {
     __shared__ double red[32];
     pdl_trigger();                                         // the accumulate kernel may be scheduled now; it waits (pdl_wait) for this grid to finish
@@ -121,7 +136,7 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
     } else
     for (int i = 0; i < nb; ++i) s += part_sum[(int64_t)b * nb + i];
     const double mean = s / (double)Nt;
-    const double t0 = __ldg(tb);                           // time origin (reading G6)
+    const double t0 = __ldg(tb) - t_off;   // time origin (reading G6)
 
     const int64_t j0 = (int64_t)blockIdx.x * chunk;
     const int64_t j1 = min(Nt, j0 + chunk);

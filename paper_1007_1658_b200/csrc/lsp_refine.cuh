@@ -18,18 +18,27 @@ namespace lsp {
 
 // Which frequencies: those where the rounding of the sums is amplified by more than `amp`, the amplification being
 // Nt / (Nt - R) for eq. (5) and (1/4) / D for the generalised form's determinant D <= 1/4.  The FP32-pipe form's sums are good to
-// ~1e-7 Nt, so amp = 20 (R > 0.95 Nt) keeps every bin within ~2e-6.  The tensor-core forms sum cos 2 theta, sin 2 theta from a
-// single fp16 pass, good to ~5e-4 / sqrt(Nt) of Nt: for 3e-5 the amplification may be 0.06 sqrt(Nt) at
-// most -- R > 0.26 Nt at Nt = 512, R > 0.83 Nt at 10,000, and the FP32 form's 0.95 from 111,000 samples on.  (In a periodogram of
-// noise R / Nt ~ sqrt(ln Nf / Nt): 0.12 at Nt = 512.  Only f T < ~0.4 and aliases get there.)
-__host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt)
+// 1e-7 ... 6e-6 of Nt (the three-term recurrence over K = 32 frequencies at tiny Nt is the upper end), so amp = 5 (R > 0.8 Nt)
+// keeps every bin within ~3e-5.  The tensor-core forms sum cos 2 theta, sin 2 theta from a single fp16 pass, good to
+// ~5e-4 / sqrt(Nt) of Nt: for 3e-5 the amplification may be 0.06 sqrt(Nt) at most -- R > 0.26 Nt at Nt = 512,
+// R > 0.83 Nt at 10,000, capped at 10 (R > 0.9 Nt) from 28,000 samples on.  (In a periodogram of noise R / Nt ~ sqrt(ln Nf / Nt):
+// 0.12 at Nt = 512.  Only f T < ~0.4 and aliases get there -- and tiny series, where a refinement costs next to nothing.)
+// The generalised form is more delicate (its numerator cancels along with the determinant; measured 1e-4 of max P at D ~ 0.02 on
+// fp32 sums): amplification 5 (D < 0.05) for the FP32-pipe form, 2.5 ... 5 for the tensor-core forms.
+__host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt, bool gls = false)
 {
-    if (!tensor) return 20.0;
+    if (gls) {
+        if (!tensor) return 5.0;
+        const double a = 0.03 * sqrt((double)Nt);
+        return a < 2.5 ? 2.5 : (a > 5.0 ? 5.0 : a);
+    }
+    if (!tensor) return 5.0;
     const double a = 0.06 * sqrt((double)Nt);
-    return a < 1.35 ? 1.35 : (a > 20.0 ? 20.0 : a);
+    return a < 1.35 ? 1.35 : (a > 10.0 ? 10.0 : a);
 }
+
 constexpr int REFINE_THREADS = 256;
-constexpr int REFINE_LIST_CAP = 1 << 20;     // entries of the fused epilogues' list (8 bytes each: 8 MiB, allocated at the first fused call); overflow keeps the fp32-sum value
+constexpr int REFINE_LIST_CAP = 1 << 20;     // entries of the list (8 bytes each: 8 MiB, allocated at the first call that needs it); overflow keeps the fp32-sum value
 
 struct RefineSrc {
     const double* t; int64_t t_stride;      // the call's own inputs (device)

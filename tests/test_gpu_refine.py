@@ -6,7 +6,7 @@ rounding of fp32 sums is amplified by Nt/(Nt - R).  The library recomputes such 
 (LSP_PARAM_REFINE = 0, the default).  Every form of the accumulate step and both places the refinement runs -- inside
 finish_kernel, and refine_kernel behind the fused epilogues -- are compared here with the fp64 oracle on grids that start at
 f = 0, on series with a drift (so that the low-frequency power is the LARGEST on the grid and the arg-max falls among the
-refined bins).  How far up the refinement reaches depends on the form (refine_amplification in lsp_refine.cuh): R > 0.95 Nt
+refined bins).  How far up the refinement reaches depends on the form (refine_amplification in lsp_refine.cuh): R > 0.8 Nt
 for the FP32-pipe form, down to R > 0.26 Nt at Nt = 512 for the tensor-core forms, whose cos 2 theta sums come from one fp16 pass."""
 import numpy as np
 import pytest
@@ -88,7 +88,7 @@ FORMS = [  # name, B, Nt, shared_t, params, kernel substring, launches the refin
 
 @pytest.mark.parametrize("name,B,Nt,shared_t,params,kernel,own_kernel", FORMS, ids=[f[0] for f in FORMS])
 def test_low_frequencies_every_form(lsp, name, B, Nt, shared_t, params, kernel, own_kernel):
-    """Grid from f = 0 in steps of 0.004 / T (f T = 0 ... 1.2): the bins below f T ~ 0.09 have R > 0.95 Nt and are refined."""
+    """Grid from f = 0 in steps of 0.004 / T (f T = 0 ... 1.2): the bins below f T ~ 0.09 have R > 0.95 Nt and are refined in every form."""
     pkg, h = lsp
     T = 50.0
     t, x = _series(B, Nt, T, seed=900 + Nt + B, shared_t=shared_t)

@@ -1,0 +1,91 @@
+"""Randomised sweep of the C ABI against the oracle: every entry point, form, split, stride and grid placement the library
+accepts, on small seeded problems -- the test that found the ill-conditioned low-frequency bins (tests/test_gpu_refine.py).
+
+Each case draws B, Nt, Nf, the form (automatic / FP32 pipe / tensor cores), the number of time splits, the coarse extent, shared or
+per-series times, classical / generalised / weighted, and where the grid starts (f = 0, 1/T, or in between), runs the batched or
+single-series call, and compares every frequency of every series with the fp64 oracle: max |dP| <= 1e-4 max P (north_star), the
+returned peak = the arg-max of the returned P (lowest index).  What is left out, and why:
+  * Nt < 8: an exact or nearly exact fit; P sits at (Nt - 1)/2 with infinitely narrow notches where fp32 and fp64 sums land on
+    different sides (reading G7);
+  * tensor-core forms forced below Nt = 512 are held to 5e-3 only (the automatic plan never picks them there: DESIGN.md section 8);
+  * a series whose largest oracle power on the drawn grid is below 0.5 (a one- or two-bin grid on pure noise) has no scale to
+    measure 1e-4 against and is compared at 1e-4 of the noise level 1 instead.
+"""
+import numpy as np
+import pytest
+
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _case(rng):
+    B = int(rng.choice([1, 1, 1, 2, 3, 7, 17, 40]))
+    Nt = int(rng.choice([8, 9, 12, 31, 127, 128, 129, 255, 256, 257, 511, 512, 513, 700, 1000, 2047, 2048, 2049, 3001, 4097, 9000, 17000]))
+    Nf = int(rng.choice([1, 2, 7, 31, 128, 129, 255, 1000, 2047, 2048, 2049, 4096, 4097, 8193, 33000, 70001]))
+    if B * Nt * Nf > 4e8:
+        Nf = max(1, int(4e8 / (B * Nt)))
+    pipe = int(rng.choice([0, 0, 1, 2]))
+    shared = bool(rng.integers(0, 2)) and B > 1
+    gls = bool(rng.integers(0, 4) == 0)
+    weighted = gls and bool(rng.integers(0, 2))
+    span = float(rng.choice([10.0, 100.0, 1000.0]))
+    t = np.sort(rng.uniform(0, span, (1 if shared else B, Nt)), axis=1)
+    x = (rng.standard_normal((B, Nt)) + 0.5 * np.sin(2 * np.pi * 0.37 * (t if not shared else t[0]))).astype(np.float32)
+    f_min = float(rng.choice([0.0, 1.0 / span, 0.013]))
+    f_max = float(rng.choice([1.0, 5.0, 20.0]))
+    df = (f_max - f_min) / max(1, Nf - 1) if Nf > 1 else 0.1
+    w = rng.uniform(0.2, 3.0, (B, Nt)).astype(np.float32) if weighted else None
+    nsplit = int(rng.choice([0, 0, 0, 2, 3]))
+    coarse = int(rng.choice([0, 0, 0, 16, 32, 64, 128])) if pipe == 2 else 0
+    return dict(B=B, Nt=Nt, Nf=Nf, pipe=pipe, shared=shared, gls=gls, weighted=weighted, span=span, t=t, x=x, f_min=f_min, df=df, w=w,
+                nsplit=nsplit, coarse=coarse)
+
+
+@pytest.mark.parametrize("seed", [101, 102, 103, 104])
+def test_random_calls_match_the_oracle(lsp, seed):
+    import torch
+    pkg, h = lsp
+    rng = np.random.default_rng(seed)
+    worst_overall, forms = 0.0, set()
+    for case in range(100):
+        c = _case(rng)
+        B, Nt, Nf, t, x, w = c["B"], c["Nt"], c["Nf"], c["t"], c["x"], c["w"]
+        desc = "seed %d case %d: %r" % (seed, case, {k: v for k, v in c.items() if k not in ("t", "x", "w")})
+        for key, val in ((pkg.PARAM_PIPE, c["pipe"]), (pkg.PARAM_NSPLIT, c["nsplit"]), (pkg.PARAM_COARSE, c["coarse"])):
+            h.set_param(key, val)
+        try:
+            td = torch.from_numpy(np.ascontiguousarray(t[0] if c["shared"] else t)).cuda()
+            xd = torch.from_numpy(x).cuda()
+            if B == 1:
+                P = h.periodogram(td.reshape(-1), xd.reshape(-1), c["f_min"], c["df"], Nf, gls=c["gls"],
+                                  weights=(torch.from_numpy(w[0]).cuda() if w is not None else None))
+                P, pi, pv = P.cpu().numpy()[None, :], None, None
+            else:
+                P, pi, pv = h.periodogram_batched(td, xd, c["f_min"], c["df"], Nf, gls=c["gls"],
+                                                  weights=(torch.from_numpy(w).cuda() if w is not None else None))
+                P, pi, pv = P.cpu().numpy(), pi.cpu().numpy(), pv.cpu().numpy()
+            torch.cuda.synchronize()
+            plan = h.last_plan()
+        finally:
+            for key in (pkg.PARAM_PIPE, pkg.PARAM_NSPLIT, pkg.PARAM_COARSE):
+                h.set_param(key, 0)
+        forms.add(plan["kernel"].split("<")[0] + ("/fused" if "fused-finish" in plan["kernel"] else ""))
+        tol = 1e-4 if (Nt >= 512 or plan["pipe"] == 1) else 5e-3
+        assert np.all(np.isfinite(P)), desc
+        for b in range(B):
+            tb = t[0] if c["shared"] else t[b]
+            if w is not None:
+                ref = oracle.periodogram_gls_weighted(tb, x[b], w[b], c["f_min"], c["df"], Nf)
+            elif c["gls"]:
+                ref = oracle.periodogram_gls(tb, x[b], c["f_min"], c["df"], Nf)
+            else:
+                ref = oracle.periodogram(tb, x[b], c["f_min"], c["df"], Nf)
+            scale = max(float(ref.max()), 1.0 if ref.max() < 0.5 else 0.0)
+            err = float(np.max(np.abs(P[b] - ref))) / scale
+            worst_overall = max(worst_overall, err if tol == 1e-4 else 0.0)
+            assert err <= tol, "%s series %d (%s): %.2e" % (desc, b, plan["kernel"], err)
+            if pi is not None:
+                assert int(pi[b]) == int(np.argmax(P[b])) and float(pv[b]) == float(P[b].max()), desc
+    print("seed %d: worst error at the 1e-4 tolerance %.2e; forms run: %s" % (seed, worst_overall, sorted(forms)))
+    assert len(forms) >= 5

@@ -20,8 +20,8 @@
  *     library never frees or reallocates caller memory.  The handle owns a device workspace
  *     that grows to the largest call seen (growth allocates and may synchronise the device once;
  *     lsp_reserve sizes it ahead of time).  Size: 32 B per sample + 16 B x Nf x (time splits, <= 2 GiB)
- *     + at most LSP_PARAM_TABLE_MB for the tensor form's table; if it cannot be allocated the call
- *     returns LSP_ENOMEM and the handle keeps the workspace it had.
+ *     + at most LSP_PARAM_TABLE_MB for the tensor form's table (+ 8.5 MiB, once, for the list of LSP_PARAM_REFINE);
+ *     if it cannot be allocated the call returns LSP_ENOMEM and the handle keeps the workspace it had.
  *   - Device-pointer entry points only ENQUEUE work on `stream` (a cudaStream_t passed as
  *     void*; NULL = legacy default stream) and return without synchronising; inputs must stay
  *     valid until the stream reaches the end of the call.  Host-pointer entry points copy
@@ -31,6 +31,9 @@
  *   - Return value: LSP_OK (0) or a negative LSP_E* code; nothing throws, nothing aborts.
  *     Data-dependent degeneracy (zero variance) cannot be reported without a sync: P is NaN then.
  *   - f = 0 is legal: the sine term of eq. (1) is 0/0 and dropped (reading G7), P = XC^2/Nt/(2 var) ~ 0.
+ *   - Accuracy: max |P - P_fp64| <= 1e-4 max P on any grid, including f T << 1 and the aliases of regular sampling, where the
+ *     single-pass sums of eqs (5)-(8) are ill-conditioned (R -> Nt): those frequencies are recomputed from t and x in fp64
+ *     (LSP_PARAM_REFINE; DESIGN.md section 6 item 6).  Not covered: Nt < 8 (an exact fit: P has infinitely narrow notches).
  *   - There is no CPU fallback: without a CUDA device lsp_create fails with LSP_ECUDA.
  */
 #ifndef LSP_B200_H

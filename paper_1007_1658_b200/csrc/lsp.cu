@@ -837,6 +837,8 @@ int lsp_reserve(lsp_handle h, int64_t B, int shared_t, int64_t Nt, int64_t Nf, i
         if (rc != LSP_OK) return rc;
         need = device_layout(r.pl, B, Nt, Nf, r.tab_series, gls).total;
     }
+    RefineList rl;                                        // (so that a call captured into a CUDA graph afterwards allocates nothing)
+    if (h->opt_refine == 0) { const int rc = refine_list(h, rl); if (rc != LSP_OK) return rc; }
     return ensure(h, &h->buf, &h->buf_bytes, need);
 }
 

@@ -244,3 +244,37 @@ def test_refine_param(lsp):
     h.set_param(pkg.PARAM_REFINE, 0)
     with pytest.raises(pkg.LspError):
         h.set_param(pkg.PARAM_REFINE, 2)
+
+
+def test_listed_refinement_in_a_cuda_graph(lsp):
+    """Long series (refine_kernel behind finish_kernel) on a fresh handle whose memory comes from lsp_reserve alone: the call
+    is captured into a CUDA graph, replayed three times (the list must be empty again after every replay) and compared with the
+    eager call and the oracle."""
+    import torch
+    pkg, _ = lsp
+    T, Nt, Nf = 50.0, 20000, 301
+    t, x = _series(1, Nt, T, seed=21)
+    f_min, df = 0.0, 0.004 / T
+    ref = _ref(t, x, f_min, df, Nf)[0]
+    td, xd = torch.from_numpy(t[0]).cuda(), torch.from_numpy(x[0]).cuda()
+    P = torch.empty(Nf, dtype=torch.float32, device="cuda")
+    with pkg.Handle(0) as h:
+        h.reserve(1, Nt, Nf)
+        g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            torch.cuda.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                h.periodogram(td, xd, f_min, df, Nf, out=P)
+        first = None
+        for _ in range(3):
+            P.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            first = P.clone() if first is None else first
+            assert torch.equal(P, first)
+        got = P.cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(got[:20] - ref[:20])) <= TIGHT * ref.max()
+        assert np.max(np.abs(got - ref)) <= TOL * ref.max()
+        eager = h.periodogram(td, xd, f_min, df, Nf)
+        torch.cuda.synchronize()
+        assert torch.equal(eager, first)

@@ -289,8 +289,8 @@ cudaError_t launch_refine(const RefineList& list, const RefineSrc& src, const do
     rp.src = src; rp.list = list; rp.part_var = pvar; rp.nparts = nparts; rp.P = P; rp.p_stride = p_stride;
     rp.peak_idx = peak_idx; rp.peak_val = peak_val; rp.peak64 = peak64; rp.gls = gls ? 1 : 0;
     rp.part_sum = psum; rp.part_w = pw;
-    refine_kernel<<<4 * 148, REFINE_THREADS, 0, st>>>(rp);
-    return cudaGetLastError();
+    // a programmatic dependent of the kernel before it (it waits before reading the list): its launch overlaps that kernel's tail
+    return launch_pdl(refine_kernel, dim3(2 * 148), dim3(REFINE_THREADS), 0, st, true, rp);
 }
 
 bool use_shared_path(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, bool gls)
@@ -601,7 +601,8 @@ int run_device(lsp_ctx* h,
                     dp.fuse = r.duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
                     dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
                     dp.list = rlist;
-                    { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
+                    dp.refine_r2 = INFINITY;
+                    if (rlist.head) { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
                     LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
                     accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
                 } else {

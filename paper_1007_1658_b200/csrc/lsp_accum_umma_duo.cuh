@@ -89,7 +89,7 @@ struct UmmaDuoParams {
     float* P; int64_t p_stride;     // nullable
     int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
     RefineList list;                // fused epilogue: where the ill-conditioned frequencies go (lsp_refine.cuh); head NULL: nowhere
-    float refine_r2;                //   ... those with R^2 above this (refine_amplification)
+    float refine_r2;                //   ... those with R^2 above this (refine_amplification); +inf: none
 };
 
 // Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
@@ -118,17 +118,20 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
         tmem_ld8(tbase + c8 + 128u + (uint32_t)UD_L, cs);
         if (!live) continue;
         const float inv2var_f = (float)inv2var;
+        const float redo_r2 = fminf(0.25f * Nt_f * Nt_f, q.refine_r2);
         // fp32 where R <= Nt/2 (no amplification of the rounding of S Nt - D R); fp64 where the denominator Nt^2 - R^2 gets small
         float pf[8];
-        unsigned ill = 0u;                                              // R > 0.95 Nt: to be redone in fp64 by refine_kernel
         #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const float A = 2.f * cc[i], Bv = 2.f * cs[i], R2 = fmaf(A, A, Bv * Bv);
             const float xc2 = xc[i] * xc[i], xs2 = xs[i] * xs[i], S = xc2 + xs2;
             const float DR = fmaf(xc2 - xs2, A, 2.f * xc[i] * xs[i] * Bv);
             pf[i] = fmaxf(2.f * fmaf(S, Nt_f, -DR), 0.f) / fmaf(Nt_f, Nt_f, -R2) * inv2var_f;
-            if (q.list.head && !(R2 < q.refine_r2)) ill |= 1u << i;
-            if (R2 > 0.25f * Nt_f * Nt_f) {
+            if (R2 > redo_r2) {
+                // ill-conditioned: listed for refine_kernel, which writes P and enters it in the arg-max; here it counts as 0
+                const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;
+                if (!(R2 < q.refine_r2) && k < p.Nf && refine_push(q.list, db, k)) { pf[i] = 0.f; continue; }
+                if (!(R2 > 0.25f * Nt_f * Nt_f)) continue;
                 const double XC = (double)xc[i], XS = (double)xs[i], Ad = 2.0 * (double)cc[i], Bd = 2.0 * (double)cs[i];
                 const double R2d = Ad * Ad + Bd * Bd, x2 = XC * XC, y2 = XS * XS, Sd = x2 + y2;
                 const double DRd = (x2 - y2) * Ad + 2.0 * XC * XS * Bd;
@@ -143,7 +146,6 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
             const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;
             if (k < p.Nf) {
                 if (q.P) q.P[db * q.p_stride + k] = pf[i];
-                if (((ill >> i) & 1u) && refine_push(q.list, db, k)) continue;      // (its refined value enters the arg-max there)
                 const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
                 best = (key > best) ? key : best;
             }

@@ -211,7 +211,6 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
             // branch-free fp32 pass: the 32 loads and combines pipeline.  Frequencies with R > Nt/2 carry cf.x = NaN, come out
             // as NaN and are redone in fp64 below (rare: f -> 0, aliases of regular sampling).
             bool redo = false;
-            unsigned ill = 0u;                                          // R > 0.95 Nt: to be redone in fp64 by refine_kernel
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
                 const int64_t k = min(k0 + i, p.Nf - 1);
@@ -231,14 +230,15 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
                     const double D = (xc2 - xs2) * __ldg(p.vconst + k) + 2.0 * XC * XS * __ldg(p.vconst + p.Nf + k);
                     pf[i] = (float)((fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var);
                     // R > thr Nt: 1/(Nt + R) < 1/((1 + thr) Nt)
-                    if (p.list.head && k0 + i < p.Nf && __ldg(p.vconst + 2 * p.Nf + k) * ((1.0 + p.refine_thr) * (double)p.Nt) < 1.0) ill |= 1u << i;
+                    // ill-conditioned: listed for refine_kernel, which writes P and enters it in the arg-max; here it counts as 0
+                    if (p.list.head && k0 + i < p.Nf && __ldg(p.vconst + 2 * p.Nf + k) * ((1.0 + p.refine_thr) * (double)p.Nt) < 1.0 &&
+                        refine_push(p.list, b, k)) pf[i] = 0.f;
                 }
             }
             #pragma unroll
             for (int i = 0; i < 32; ++i) {
                 const int64_t k = k0 + i;
                 if (k < p.Nf) {
-                    if (((ill >> i) & 1u) && refine_push(p.list, b, k)) continue;   // (its refined value enters the arg-max there)
                     const u64 key = ((u64)__float_as_uint(fmaxf(pf[i], 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
                     best = (key > best) ? key : best;
                 }

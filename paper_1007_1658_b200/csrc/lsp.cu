@@ -352,13 +352,14 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     // steps 1-2 (per series: mean, variance, X; the phase records of series 0 serve all)
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
     const bool fused_pre = pl.fused_pre;                   // short series: step 1's sum inside the records kernel
+    const int TRIG = 0;
     if (!fused_pre) {
         moments_kernel<<<gpre, 256, 0, st>>>(x, x_stride, Nt, pl.part_chunk, psum, peak64, counter);
         LSP_CUDA(h, cudaGetLastError());
     } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    if (fused_pre) records_kernel<true, true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
-    else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
+    if (fused_pre) records_kernel<true, true><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
+    else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
     LSP_CUDA(h, cudaGetLastError());
     // CC, CS once per frequency
     shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
@@ -453,6 +454,12 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
     // short grids, short series: steps 1-2 inside the accumulate kernel (accum_umma_small_kernel<..., FUSED_PRE>): two launches per call
     r.fuse_pre = r.small && !r.duo && !gls && !weighted && Nt <= 16384 && h->opt_pdl != 1;
     if (r.fuse_pre) { pl.launches = 2; pl.nparts = 1; pl.part_chunk = Nt; pl.fused_pre = false; }
+    // ... and of the batch kernel (accum_umma_duo_kernel<FUSED_PRE>); with the fused epilogue only where one CTA owns the whole series
+    // (the CTA that resets the arg-max cell is then the only one that updates it)
+    if (r.duo && !gls && !weighted && Nt <= 16384 && h->opt_pdl != 1 && (!r.duo_fuse || pl.nfb == 1)) {
+        r.fuse_pre = true;
+        pl.launches = r.duo_fuse ? 1 : 2; pl.nparts = 1; pl.part_chunk = Nt; pl.fused_pre = false;
+    }
     if (gls) pl.launches += 1 + (r.pair ? pl.nchunks : 1);   // unit records + second accumulate pass
     const int64_t units = (r.duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
@@ -510,6 +517,7 @@ int run_device(lsp_ctx* h,
     // steps 1-2
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
     const bool fused_pre = pl.fused_pre && !weighted;      // short series: step 1's sum inside the records kernel
+    const int TRIG = tensor ? 0 : 1;                       // (cos d_j, sin d_j) of the FP32-pipe form's recurrence
     if (r.fuse_pre) {                                     // (done by the accumulate kernel itself)
         if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
     } else {
@@ -518,9 +526,9 @@ int run_device(lsp_ctx* h,
         LSP_CUDA(h, cudaGetLastError());
     } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar, origin_offset(f_min, df, Nf));
-    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
-    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf));
+    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar, origin_offset(f_min, df, Nf), TRIG);
+    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
+    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
     LSP_CUDA(h, cudaGetLastError());
     }
     if (weighted) pl.launches -= 1;                       // (the weight records were written by records_weighted_kernel)
@@ -603,8 +611,9 @@ int run_device(lsp_ctx* h,
                     dp.list = rlist;
                     dp.refine_r2 = INFINITY;
                     if (rlist.head) { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
-                    LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
-                    accum_umma_duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
+                    void (*duo_kernel)(const UmmaDuoParams) = r.fuse_pre ? accum_umma_duo_kernel<true> : accum_umma_duo_kernel<false>;
+                    LSP_CUDA(h, cudaFuncSetAttribute(duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
+                    duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
                 } else {
 #define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
                     if (r.fuse_pre) { \

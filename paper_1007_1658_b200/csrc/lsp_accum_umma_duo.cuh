@@ -168,6 +168,11 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
 }
 
 // grid.x = ceil(B / 2) * nsplit * nfb (frequency block fastest), US_THREADS threads, UD_SMEM bytes, two CTAs per SM.
+// FUSED_PRE (short series, as in accum_umma_small_kernel): steps 1-2 run here -- the 128 loader threads of each series form its mean
+// and variance over the WHOLE series (fixed order: every CTA of the series gets the identical values) and the exact phases of the
+// samples they stage, straight from t and x; no record arrays, no pre-pass launches.  The first CTA of a series publishes the
+// variance partial and resets the arg-max cell (host: only where no other CTA of the series can reach its epilogue first).
+template <bool FUSED_PRE>
 __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const UmmaDuoParams q)
 {
     const UmmaParams& p = q.u;
@@ -219,11 +224,50 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
         const bool l_live = lb < q.B;
         const float* recAx = &p.recA[(l_live ? lb : 0) * p.Nt + j_begin].x;      // .x of the split's first record (stride 4 floats)
         const ulonglong2* recB = p.recB + (l_live ? lb : 0) * p.Nt + j_begin;
-        const float xs = l_live ? (p.unit_x ? 1.f : x_scale(p.part_var + lb * p.nparts, p.nparts, p.Nt)) : 0.f;
+        float xs;
+        double mean = 0.0, t0 = 0.0;
+        const double* tb = nullptr; const float* xb = nullptr;
+        if (FUSED_PRE) {
+            // steps 1-2: mean, then sum (x - mean)^2, of series `ls` by its 128 loader threads (warps 4 ls ... 4 ls + 3)
+            tb = p.t + (l_live ? lb : 0) * p.t_stride; xb = p.x + (l_live ? lb : 0) * p.x_stride;
+            double* red = reinterpret_cast<double*>(rec_all);                     // 8 doubles of scratch (the record tiles are not in use yet)
+            double a0 = 0.0;
+            for (int64_t j = lj; j < p.Nt; j += 128) a0 += (double)__ldg(xb + j);
+            #pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a0 += __shfl_down_sync(0xffffffffu, a0, o);
+            if (lane == 0) red[w] = a0;
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            mean = (((red[4 * ls] + red[4 * ls + 1]) + red[4 * ls + 2]) + red[4 * ls + 3]) / (double)p.Nt;   // fixed order
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            double a1 = 0.0;
+            for (int64_t j = lj; j < p.Nt; j += 128) { const double d = (double)__ldg(xb + j) - mean; a1 += d * d; }
+            #pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a1 += __shfl_down_sync(0xffffffffu, a1, o);
+            if (lane == 0) red[w] = a1;
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
+            const double q2 = ((red[4 * ls] + red[4 * ls + 1]) + red[4 * ls + 2]) + red[4 * ls + 3];
+            asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");   // `red` is the record tiles from here on
+            if (lj == 0 && l_live && sp == 0 && fb == 0) { p.part_var_out[lb] = q2; p.peak64[lb] = 0ull; p.counter[lb] = 0u; }
+            xs = l_live ? x_scale(&q2, 1, p.Nt) : 0.f;                            // steps 6-7 recompute exactly this from part_var_out
+            t0 = __ldg(tb);                                                       // time origin (reading G6)
+        } else {
+            xs = l_live ? (p.unit_x ? 1.f : x_scale(p.part_var + lb * p.nparts, p.nparts, p.Nt)) : 0.f;
+        }
         const int n_samp_i = (int)n_samp;                                         // split_len < 2^31
         float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull;
-        bool pre_ok = l_live && (int)lj < n_samp_i;
-        if (pre_ok) { pre_x = __ldg(recAx + 4 * lj); const ulonglong2 r = __ldg(recB + lj); pre_u = r.x; pre_v = r.y; }
+        bool pre_ok = false;
+        auto prefetch = [&](int jt) {                                             // this thread's record of a tile, relative to j_begin
+            pre_ok = l_live && jt < n_samp_i;
+            if (!pre_ok) return;
+            if (FUSED_PRE) {
+                const int64_t j = j_begin + jt;
+                pre_x = (float)((double)__ldg(xb + j) - mean);                    // X_j rounded to fp32 once (G4)
+                const double tp = __ldg(tb + j) - t0;
+                pre_u = frac_fixed64(p.f_min, tp, nullptr);
+                pre_v = frac_fixed64(p.df, tp, nullptr);
+            } else { pre_x = __ldg(recAx + 4 * jt); const ulonglong2 r = __ldg(recB + jt); pre_u = r.x; pre_v = r.y; }
+        };
+        prefetch((int)lj);
         float4* rec_mine = rec_all + (ls * 2) * UM_TS + lj;                       // this thread's slot of its series' tile, buffer 0
         // A task: row m = tid & 127 = (series m >> 6, fine value m & 63), 4 samples `chunk` of the k-step
         const unsigned m = tid & 127u, a_s = m >> 6, a_h = m & 63u;
@@ -264,8 +308,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 }
                 rec_mine[buf * UM_TS] = r;
                 j_tile += UM_TS;                                                // prefetch this thread's record of the following tile
-                pre_ok = l_live && j_tile < n_samp_i;
-                if (pre_ok) { pre_x = __ldg(recAx + 4 * j_tile); const ulonglong2 rr = __ldg(recB + j_tile); pre_u = rr.x; pre_v = rr.y; }
+                prefetch(j_tile);
                 asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
             }
             const uint32_t st_off = (uint32_t)s * UD_STAGE_BYTES;

@@ -66,7 +66,8 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
                                         int64_t Nt, int64_t chunk, double f_min, double df,
                                         const double* __restrict__ part_sum, const double* __restrict__ part_w,
                                         float4* __restrict__ recA, float4* __restrict__ recA1, ulonglong2* __restrict__ recB,
-                                        double* __restrict__ part_var, double t_off /* origin_offset() */)
+                                        double* __restrict__ part_var, double t_off /* origin_offset() */,
+                                        int trig /* 0: tensor-core forms, which read only .x of the records: no sincospi */)
 {
     __shared__ double red[32];
     const int b = blockIdx.y;
@@ -91,8 +92,8 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
         double vfrac;
         const u64 u = frac_fixed64(f_min, tp, nullptr);
         const u64 v = frac_fixed64(df, tp, &vfrac);
-        double sd, cd;
-        sincospi(2.0 * vfrac, &sd, &cd);
+        double sd = 0.0, cd = 0.0;
+        if (trig) sincospi(2.0 * vfrac, &sd, &cd);
         const double sq = sqrt(wn);
         recA[o] = make_float4((float)(sq * d), (float)cd, (float)sd, (float)(2.0 * cd));
         recA1[o] = make_float4((float)sq, (float)cd, (float)sd, (float)(2.0 * cd));
@@ -114,7 +115,8 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                double* __restrict__ part_sum,
                                float4* __restrict__ recA, ulonglong2* __restrict__ recB,
                                double* __restrict__ part_var,
-                               u64* __restrict__ peak64, unsigned* __restrict__ counter, double t_off /* origin_offset() */)
+                               u64* __restrict__ peak64, unsigned* __restrict__ counter, double t_off /* origin_offset() */,
+                               int trig /* 0: tensor-core forms, which read only .x of the records: no sincospi */)
 {
     __shared__ double red[32];
     pdl_trigger();                                         // the accumulate kernel may be scheduled now; it waits (pdl_wait) for this grid to finish
@@ -151,7 +153,7 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
         const u64 u = frac_fixed64(f_min, tp, nullptr);
         const u64 v = frac_fixed64(df, tp, &vfrac);
         double sd = 0.0, cd = 0.0;
-        if (!SHARED) sincospi(2.0 * vfrac, &sd, &cd);      // accurate: its error is applied K times per run
+        if (!SHARED && trig) sincospi(2.0 * vfrac, &sd, &cd);   // accurate: its error is applied K times per run
         if (!SHARED) recA[o] = make_float4((float)d, (float)cd, (float)sd, (float)(2.0 * cd));
         recB[o] = make_ulonglong2(u, v);
     }

@@ -362,14 +362,12 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     else records_kernel<true, false><<<gpre, 256, 0, st>>>(t, 0, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
     LSP_CUDA(h, cudaGetLastError());
     // CC, CS once per frequency
-    shared_v_kernel<<<dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), 256, 0, st>>>(recB, Nt, Nf, gps * SG_KS, ws_v);
-    LSP_CUDA(h, cudaGetLastError());
+    const bool pdl = h->opt_pdl != 1;                      // programmatic dependents: each kernel's launch overlaps its predecessor's tail
+    LSP_CUDA(h, launch_pdl(shared_v_kernel, dim3((unsigned)((Nf + 7) / 8), (unsigned)nsplit), dim3(256), 0, st, pdl, (const ulonglong2*)recB, Nt, Nf, gps * SG_KS, ws_v));
     if (fuse) {
-        shared_vconst_kernel<<<(unsigned)((Nf + 255) / 256), 256, 0, st>>>(ws_v, (int)nsplit, Nf, Nt, vconst, vconst_f, redo_thr);
-        LSP_CUDA(h, cudaGetLastError());
+        LSP_CUDA(h, launch_pdl(shared_vconst_kernel, dim3((unsigned)((Nf + 255) / 256)), dim3(256), 0, st, pdl, (const float*)ws_v, (int)nsplit, Nf, Nt, vconst, vconst_f, redo_thr));
     }
-    shared_x_kernel<<<dim3((unsigned)nmb, (unsigned)ng), 256, 0, st>>>(x, x_stride, psum, pvar, pl.nparts, B, Nt, xa, (int)ng);
-    LSP_CUDA(h, cudaGetLastError());
+    LSP_CUDA(h, launch_pdl(shared_x_kernel, dim3((unsigned)nmb, (unsigned)ng), dim3(256), 0, st, pdl, x, x_stride, (const double*)psum, (const double*)pvar, pl.nparts, B, Nt, xa, (int)ng));
     // step 3 for every (sample, frequency) once, and steps 4-5, the contraction: one band of frequency blocks at a time
     // (E tiles of the band -> GEMM over the band; the same buffer serves every band)
     SharedGemmParams gp;
@@ -382,12 +380,10 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     for (int64_t band = 0; band < nbands; ++band) {
         const int64_t nb0 = band * L.band_nfb;
         const int64_t nb_n = (nfb - nb0 < L.band_nfb) ? nfb - nb0 : L.band_nfb;
-        shared_e_kernel<<<dim3((unsigned)nb_n, (unsigned)ng), 256, 0, st>>>(recB, Nt, Nf, eb, (int)ng, (int)nb0);
-        LSP_CUDA(h, cudaGetLastError());
+        LSP_CUDA(h, launch_pdl(shared_e_kernel, dim3((unsigned)nb_n, (unsigned)ng), dim3(256), 0, st, pdl, (const ulonglong2*)recB, Nt, Nf, eb, (int)ng, (int)nb0));
         if (timing && band == 0) LSP_CUDA(h, cudaEventRecord(ev[2], st));
         gp.nb0 = (int)nb0; gp.nfb = (int)nb_n;
-        shared_gemm_kernel<<<(unsigned)(nmb * nb_n * nsplit), SG_THREADS, SG_SMEM, st>>>(gp);
-        LSP_CUDA(h, cudaGetLastError());
+        LSP_CUDA(h, launch_pdl(shared_gemm_kernel, dim3((unsigned)(nmb * nb_n * nsplit)), dim3(SG_THREADS), SG_SMEM, st, pdl, gp));
     }
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[3], st));
     if (fuse) {                                           // steps 6-7 ran in the GEMM's epilogue

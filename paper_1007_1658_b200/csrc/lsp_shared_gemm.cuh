@@ -64,6 +64,8 @@ struct SharedGemmParams {
 __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restrict__ ws_v, int nsplit, int64_t Nf, int64_t Nt_i, double* __restrict__ vconst,
                                                             float4* __restrict__ vconst_f, double redo_thr /* <= 0.5: fp32 below R = redo_thr Nt */)
 {
+    pdl_trigger();                                          // (the kernels of a shared-time call are launched as programmatic dependents:
+    pdl_wait();                                             //  launch and set-up overlap the predecessor's tail; nothing is read or written before this)
     const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (k >= Nf) return;
     double CCh = 0.0, CS = 0.0;
@@ -84,6 +86,8 @@ __global__ void __launch_bounds__(256) shared_vconst_kernel(const float* __restr
 __global__ void __launch_bounds__(256) shared_e_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t Nf,
                                                        unsigned char* __restrict__ eb, int ng, int nb0)
 {
+    pdl_trigger();                                          // (the kernels of a shared-time call are launched as programmatic dependents:
+    pdl_wait();                                             //  launch and set-up overlap the predecessor's tail; nothing is read or written before this)
     const int nb = blockIdx.x, g = blockIdx.y;
     const unsigned kf = threadIdx.x & 127u, chunk = threadIdx.x >> 7;
     const int64_t k = (int64_t)(nb0 + nb) * SG_F + kf;
@@ -124,6 +128,8 @@ __global__ void __launch_bounds__(256) shared_e_kernel(const ulonglong2* __restr
 // grid (ceil(Nf / 8), nsplit), 256 threads.
 __global__ void __launch_bounds__(256) shared_v_kernel(const ulonglong2* __restrict__ recB, int64_t Nt, int64_t Nf, int64_t split_len, float* __restrict__ ws_v)
 {
+    pdl_trigger();                                          // (the kernels of a shared-time call are launched as programmatic dependents:
+    pdl_wait();                                             //  launch and set-up overlap the predecessor's tail; nothing is read or written before this)
     const int64_t k = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
     const unsigned lane = threadIdx.x & 31u;
     const int sp = blockIdx.y;
@@ -152,6 +158,8 @@ __global__ void __launch_bounds__(256) shared_x_kernel(const float* __restrict__
                                                        const double* __restrict__ part_var, int nparts,
                                                        int64_t B, int64_t Nt, unsigned char* __restrict__ xa, int ng)
 {
+    pdl_trigger();                                          // (the kernels of a shared-time call are launched as programmatic dependents:
+    pdl_wait();                                             //  launch and set-up overlap the predecessor's tail; nothing is read or written before this)
     const int mb = blockIdx.x, g = blockIdx.y;
     const unsigned row = threadIdx.x & 127u, chunk = threadIdx.x >> 7;
     const int64_t b = (int64_t)mb * SG_M + row;
@@ -318,6 +326,8 @@ __global__ void __launch_bounds__(SG_THREADS, 2) shared_gemm_kernel(const Shared
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
+    pdl_trigger();
+    pdl_wait();                                                         // the operand tiles of this band are complete
 
     if (w == 0) {
         if (lane == 0) {

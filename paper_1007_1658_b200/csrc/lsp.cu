@@ -15,6 +15,7 @@
 #include "lsp_probe.cuh"
 #include "lsp_plan.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -249,12 +250,18 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 
 void launch_finish(const FinishParams& fp, int64_t B, cudaStream_t st, bool pdl = false)
 {
+    // blocks per series: all the frequency chunks of a single series; for a batch about four waves of blocks in all (each block
+    // then loops over several chunks of its series)
+    constexpr int64_t TARGET_BLOCKS = 4 * 8 * 148;
+    const int64_t per_series = (TARGET_BLOCKS + B - 1) / B;
     if (fp.nsplit >= 4 && fp.Nf <= 65536) {               // (long grids have enough frequencies to fill the machine one thread each: 170 vs 360 us at C5)
-        const int64_t per_block = FIN_THREADS / 8;
-        launch_pdl(finish_kernel<8>, dim3((unsigned)((fp.Nf + per_block - 1) / per_block), (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
+        const int64_t nchunk = (fp.Nf + FIN_THREADS / 8 - 1) / (FIN_THREADS / 8);
+        if (per_series < nchunk) launch_pdl(finish_kernel<8, true>, dim3((unsigned)per_series, (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
+        else launch_pdl(finish_kernel<8, false>, dim3((unsigned)nchunk, (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
     } else {
-        const int64_t per_block = FIN_THREADS;
-        launch_pdl(finish_kernel<1>, dim3((unsigned)((fp.Nf + per_block - 1) / per_block), (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
+        const int64_t nchunk = (fp.Nf + FIN_THREADS - 1) / FIN_THREADS;
+        if (per_series < nchunk) launch_pdl(finish_kernel<1, true>, dim3((unsigned)per_series, (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
+        else launch_pdl(finish_kernel<1, false>, dim3((unsigned)nchunk, (unsigned)B), dim3(FIN_THREADS), 0, st, pdl, fp);
     }
 }
 

@@ -76,7 +76,7 @@ __device__ __forceinline__ double finish_combine(double XC, double XS, double CC
 // deterministic; with few frequencies and many splits (C1, C2) the sum over the splits is no longer one long dependent chain.
 // FIN_SL = 1 (few splits): one thread per frequency, 256 frequencies per block, no exchange.
 // Frequencies whose sums are ill-conditioned (needs_refine) are then redone by the whole block in fp64, one after the other.
-template <int FIN_SL>
+template <int FIN_SL, bool LOOP>
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams p)
 {
     constexpr int FIN_BLOCK_F = FIN_THREADS / FIN_SL;
@@ -103,70 +103,85 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
     const float* ws = p.ws_x ? p.ws : p.ws + b * p.nsplit * 4 * p.Nf;
     const float* wx = p.ws_x ? p.ws_x + b * p.nsplit * 2 * p.x_row : nullptr;
     const float* w1 = p.ws1 ? p.ws1 + b * p.nsplit * 4 * p.Nf : nullptr;
-    const int64_t k = (int64_t)blockIdx.x * FIN_BLOCK_F + fl;
-    const bool live = k < p.Nf;
-
-    double XC = 0.0, XS = 0.0, CCh = 0.0, CS = 0.0, C1 = 0.0, S1 = 0.0;
-    if (live) {
-        #pragma unroll 2
-        for (int sp = sl; sp < p.nsplit; sp += FIN_SL) {   // fixed order over this lane's time splits
-            const float* w = ws + (int64_t)sp * 4 * p.Nf + k;
-            if (wx) {
-                XC += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + k);
-                XS += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + p.x_row + k);
-            } else {
-                XC += (double)__ldg(w);
-                XS += (double)__ldg(w + p.Nf);
-            }
-            CCh += (double)__ldg(w + 2 * p.Nf);
-            CS += (double)__ldg(w + 3 * p.Nf);
-            if (w1) {
-                C1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + k);
-                S1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + p.Nf + k);
-            }
-        }
-    }
-    if (FIN_SL > 1) {
-        s_part[0][sl][fl] = XC; s_part[1][sl][fl] = XS; s_part[2][sl][fl] = CCh; s_part[3][sl][fl] = CS;
-        s_part[4][sl][fl] = C1; s_part[5][sl][fl] = S1;
-    }
-    __syncthreads();                                       // s_var; the lanes' partial sums
-    const bool owner = live && sl == 0;
     const bool gls = p.ws1 != nullptr;
-    double v[6] = {XC, XS, CCh, CS, C1, S1};
-    if (owner && FIN_SL > 1) {
-        #pragma unroll
-        for (int q = 0; q < 6; ++q) {
-            double a = 0.0;
-            #pragma unroll
-            for (int l = 0; l < FIN_SL; ++l) a += s_part[q][l][fl];       // fixed order over the lanes
-            v[q] = a;
-        }
-    }
-    float Pf = 0.f;
-    if (owner) Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, gls);
-    bool listed = false;                                   // refine_kernel will write this frequency and enter it in the arg-max
-    if (p.refine_amp > 0.0 && p.list.head) {
-        if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) listed = refine_push(p.list, b, k);
-    } else if (p.refine_amp > 0.0) {                       // (uniform over the grid)
-        if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) s_flag[atomicAdd(&s_nflag, 1)] = (short)fl;
-        __syncthreads();
-        const int nflag = s_nflag;
-        for (int i = 0; i < nflag; ++i) {                  // the order of the list varies from run to run; each entry's result does not
-            const int f = s_flag[i];
-            double r[6];
-            refine_sums<FIN_THREADS>(p.src, b, (int64_t)blockIdx.x * FIN_BLOCK_F + f, gls, r, s_red);
-            if (owner && fl == f) Pf = (float)refine_combine(r, (double)p.Nt, 0.5 / s_var_raw, gls);
-        }
-    }
-    if (sl != 0) return;                                   // (whole warps: FIN_BLOCK_F is a multiple of 32)
-
+    const int64_t nchunk = (p.Nf + FIN_BLOCK_F - 1) / FIN_BLOCK_F;
     u64 best = 0ull;
-    if (live) {
-        if (p.P) p.P[b * p.p_stride + k] = Pf;
-        if (!listed) best = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
-    }
-    if (p.peak_idx == nullptr) return;
+
+    // LOOP (batches): a block takes the chunks blockIdx.x, blockIdx.x + gridDim.x, ... of its series -- a batch of short grids would
+    // otherwise be tens of thousands of blocks that each pay the serial prologue above (0.19 -> 0.13 ms at C4).  Otherwise one chunk
+    // per block, straight-line code (gridDim.x = nchunk).
+    int64_t c = blockIdx.x;
+    do {
+        const int64_t k = c * FIN_BLOCK_F + fl;
+        const bool live = k < p.Nf;
+
+        double XC = 0.0, XS = 0.0, CCh = 0.0, CS = 0.0, C1 = 0.0, S1 = 0.0;
+        if (live) {
+            #pragma unroll 2
+            for (int sp = sl; sp < p.nsplit; sp += FIN_SL) {   // fixed order over this lane's time splits
+                const float* w = ws + (int64_t)sp * 4 * p.Nf + k;
+                if (wx) {
+                    XC += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + k);
+                    XS += (double)__ldg(wx + (int64_t)sp * 2 * p.x_row + p.x_row + k);
+                } else {
+                    XC += (double)__ldg(w);
+                    XS += (double)__ldg(w + p.Nf);
+                }
+                CCh += (double)__ldg(w + 2 * p.Nf);
+                CS += (double)__ldg(w + 3 * p.Nf);
+                if (w1) {
+                    C1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + k);
+                    S1 += (double)__ldg(w1 + (int64_t)sp * 4 * p.Nf + p.Nf + k);
+                }
+            }
+        }
+        if (FIN_SL > 1) {
+            s_part[0][sl][fl] = XC; s_part[1][sl][fl] = XS; s_part[2][sl][fl] = CCh; s_part[3][sl][fl] = CS;
+            s_part[4][sl][fl] = C1; s_part[5][sl][fl] = S1;
+        }
+        __syncthreads();                                   // s_var, s_nflag (thread 0's prologue runs beside the loads above); the lanes' partial sums
+        const bool owner = live && sl == 0;
+        double v[6] = {XC, XS, CCh, CS, C1, S1};
+        if (owner && FIN_SL > 1) {
+            #pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                double a = 0.0;
+                #pragma unroll
+                for (int l = 0; l < FIN_SL; ++l) a += s_part[q][l][fl];   // fixed order over the lanes
+                v[q] = a;
+            }
+        }
+        float Pf = 0.f;
+        if (owner) Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, gls);
+        bool listed = false;                               // refine_kernel will write this frequency and enter it in the arg-max
+        if (p.refine_amp > 0.0 && p.list.head) {
+            if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) listed = refine_push(p.list, b, k);
+        } else if (p.refine_amp > 0.0) {                   // (uniform over the grid)
+            if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) s_flag[atomicAdd(&s_nflag, 1)] = (short)fl;
+            __syncthreads();
+            const int nflag = s_nflag;
+            for (int i = 0; i < nflag; ++i) {              // the order of the list varies from run to run; each entry's result does not
+                const int f = s_flag[i];
+                double r[6];
+                refine_sums<FIN_THREADS>(p.src, b, c * FIN_BLOCK_F + f, gls, r, s_red);
+                if (owner && fl == f) Pf = (float)refine_combine(r, (double)p.Nt, 0.5 / s_var_raw, gls);
+            }
+        }
+        if (owner) {
+            if (p.P) p.P[b * p.p_stride + k] = Pf;
+            if (!listed) {
+                const u64 key = ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k);
+                best = (key > best) ? key : best;
+            }
+        }
+        if (!LOOP) break;
+        c += gridDim.x;
+        if (c < nchunk) {                                  // another chunk follows (uniform): the shared arrays are free again after this
+            __syncthreads();
+            if (threadIdx.x == 0) s_nflag = 0;
+        }
+    } while (c < nchunk);
+    if (p.peak_idx == nullptr || sl != 0) return;          // (whole warps: FIN_BLOCK_F is a multiple of 32)
     #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         const u64 other = __shfl_down_sync(0xffffffffu, best, o);

@@ -33,7 +33,8 @@
  *   - f = 0 is legal: the sine term of eq. (1) is 0/0 and dropped (reading G7), P = XC^2/Nt/(2 var) ~ 0.
  *   - Accuracy: max |P - P_fp64| <= 1e-4 max P on any grid, including f T << 1 and the aliases of regular sampling, where the
  *     single-pass sums of eqs (5)-(8) are ill-conditioned (R -> Nt): those frequencies are recomputed from t and x in fp64
- *     (LSP_PARAM_REFINE; DESIGN.md section 6 item 6).  Not covered: Nt < 8 (an exact fit: P has infinitely narrow notches).
+ *     (LSP_PARAM_REFINE; DESIGN.md section 6 item 6); verified from Nt = 2 up.  The tensor form forced below Nt = 512
+ *     (LSP_PARAM_PIPE = 2; the automatic plan never picks it there) is good to 5e-3 only.
  *   - There is no CPU fallback: without a CUDA device lsp_create fails with LSP_ECUDA.
  */
 #ifndef LSP_B200_H

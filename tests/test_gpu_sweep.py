@@ -4,9 +4,8 @@ accepts, on small seeded problems -- the test that found the ill-conditioned low
 Each case draws B, Nt, Nf, the form (automatic / FP32 pipe / tensor cores), the number of time splits, the coarse extent, shared or
 per-series times, classical / generalised / weighted, and where the grid starts (f = 0, 1/T, or in between), runs the batched or
 single-series call, and compares every frequency of every series with the fp64 oracle: max |dP| <= 1e-4 max P (north_star), the
-returned peak = the arg-max of the returned P (lowest index).  What is left out, and why:
-  * Nt < 8: an exact or nearly exact fit; P sits at (Nt - 1)/2 with infinitely narrow notches where fp32 and fp64 sums land on
-    different sides (reading G7);
+returned peak = the arg-max of the returned P (lowest index).  Series as short as Nt = 2 are in (an exact fit: P sits at (Nt - 1)/2
+with narrow notches; the fp64 refinement takes the 0/0 decisions of reading G7 at the oracle's own threshold).  What is held to less:
   * tensor-core forms forced below Nt = 512 are held to 5e-3 only (the automatic plan never picks them there: DESIGN.md section 8);
   * a series whose largest oracle power on the drawn grid is below 0.5 (a one- or two-bin grid on pure noise) has no scale to
     measure 1e-4 against and is compared at 1e-4 of the noise level 1 instead.
@@ -21,13 +20,13 @@ pytestmark = pytest.mark.gpu
 
 def _case(rng):
     B = int(rng.choice([1, 1, 1, 2, 3, 7, 17, 40]))
-    Nt = int(rng.choice([8, 9, 12, 31, 127, 128, 129, 255, 256, 257, 511, 512, 513, 700, 1000, 2047, 2048, 2049, 3001, 4097, 9000, 17000]))
+    Nt = int(rng.choice([2, 3, 5, 8, 9, 12, 31, 127, 128, 129, 255, 256, 257, 511, 512, 513, 700, 1000, 2047, 2048, 2049, 3001, 4097, 9000, 17000]))
     Nf = int(rng.choice([1, 2, 7, 31, 128, 129, 255, 1000, 2047, 2048, 2049, 4096, 4097, 8193, 33000, 70001]))
     if B * Nt * Nf > 4e8:
         Nf = max(1, int(4e8 / (B * Nt)))
     pipe = int(rng.choice([0, 0, 1, 2]))
     shared = bool(rng.integers(0, 2)) and B > 1
-    gls = bool(rng.integers(0, 4) == 0)
+    gls = bool(rng.integers(0, 4) == 0) and Nt >= 4
     weighted = gls and bool(rng.integers(0, 2))
     span = float(rng.choice([10.0, 100.0, 1000.0]))
     t = np.sort(rng.uniform(0, span, (1 if shared else B, Nt)), axis=1)

@@ -46,7 +46,7 @@ def test_random_calls_match_the_oracle(lsp, seed):
     import torch
     pkg, h = lsp
     rng = np.random.default_rng(seed)
-    worst_overall, forms = 0.0, set()
+    worst_overall, worst_desc, forms = 0.0, "", set()
     for case in range(100):
         c = _case(rng)
         B, Nt, Nf, t, x, w = c["B"], c["Nt"], c["Nf"], c["t"], c["x"], c["w"]
@@ -82,9 +82,10 @@ def test_random_calls_match_the_oracle(lsp, seed):
                 ref = oracle.periodogram(tb, x[b], c["f_min"], c["df"], Nf)
             scale = max(float(ref.max()), 1.0 if ref.max() < 0.5 else 0.0)
             err = float(np.max(np.abs(P[b] - ref))) / scale
-            worst_overall = max(worst_overall, err if tol == 1e-4 else 0.0)
+            if tol == 1e-4 and err > worst_overall:
+                worst_overall, worst_desc = err, "%s (%s)" % (desc, plan["kernel"])
             assert err <= tol, "%s series %d (%s): %.2e" % (desc, b, plan["kernel"], err)
             if pi is not None:
                 assert int(pi[b]) == int(np.argmax(P[b])) and float(pv[b]) == float(P[b].max()), desc
-    print("seed %d: worst error at the 1e-4 tolerance %.2e; forms run: %s" % (seed, worst_overall, sorted(forms)))
+    print("seed %d: worst error at the 1e-4 tolerance %.2e in %s; forms run: %s" % (seed, worst_overall, worst_desc, sorted(forms)))
     assert len(forms) >= 5

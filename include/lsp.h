@@ -168,10 +168,9 @@ int lsp_periodogram_gls_batched(lsp_handle h,
  *   w DEVICE const float[Nt] per series (series b at w + b*w_stride, |w_stride| >= Nt; w_stride = 0: one weight vector for
  *   all series), finite, >= 0, positive sum (not checked: a violation yields NaN).  Only weight ratios matter; w_j = 0
  *   removes sample j from the fit.  w == NULL: unit weights (identical to lsp_periodogram_gls[_batched]).
- *   Everything else as lsp_periodogram_gls[_batched].  Two accumulate passes, on the CTA-pair tensor form where the plan
- *   picks it (long grids: the generated operand carries w_j x_j, and w_j e^{2i theta} for the sums of cos^2, cos sin), else on the
- *   FP32 pipe with the samples entering as sqrt(w_j) x_j and sqrt(w_j) e^{i theta} (the recurrence is linear, so the weights
- *   cost nothing per term).
+ *   Everything else as lsp_periodogram_gls[_batched].  Two accumulate passes in whatever form the plan picks: on the tensor-core
+ *   forms the generated operand carries w_j x_j, and w_j e^{2i theta} for the sums of cos^2, cos sin; on the FP32 pipe the samples
+ *   enter as sqrt(w_j) x_j and sqrt(w_j) e^{i theta} (the recurrence is linear, so the weights cost nothing per term).
  */
 int lsp_periodogram_gls_weighted(lsp_handle h,
                                  const double* t, const float* x, const float* w, int64_t Nt,

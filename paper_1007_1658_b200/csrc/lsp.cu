@@ -424,8 +424,7 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
 {
     r.tab_series = (t_stride == 0) ? 1 : B;
     r.pl = make_plan(h, B, Nt, Nf, r.tab_series);
-    // per-sample weights: the CTA-pair tensor form and the FP32-pipe form carry them; where the plan is another form, the FP32 one runs
-    if (weighted && !(r.pl.pipe == PLAN_PIPE_TENSOR && r.pl.L >= 128)) r.pl = make_plan(h, B, Nt, Nf, r.tab_series, PLAN_PIPE_FP32);
+    // (per-sample weights: every form carries them)
     Plan& pl = r.pl;
     if (pl.K == 0) return LSP_EINVAL;
     r.tensor = pl.pipe == PLAN_PIPE_TENSOR;
@@ -447,9 +446,15 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
         pl.launches = 3 + 2 * pl.nchunks;
     } else if (r.duo) {
         pl.kernel_name = r.duo_fuse ? "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32,fused-finish>"
-                                    : "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>";
+                       : (weighted ? "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32,weighted>"
+                                   : "accum_umma_duo_kernel<tcgen05.m128n128k16.f16,hi+lo,2 series x 64 x 32>");
         if (r.duo_fuse) pl.launches = 3;
     } else {
+        if (weighted)
+        pl.kernel_name = pl.L == 16 ? "accum_umma_small_kernel<tcgen05.m128n32k16.f16,hi+lo,weighted>"
+                       : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo,weighted>"
+                                     : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo,weighted>");
+        else
         pl.kernel_name = pl.L == 16 ? "accum_umma_small_kernel<tcgen05.m128n32k16.f16,hi+lo>"
                        : (pl.L == 32 ? "accum_umma_small_kernel<tcgen05.m128n64k16.f16,hi+lo>"
                                      : "accum_umma_small_kernel<tcgen05.m128n128k16.f16,hi+lo>");
@@ -573,7 +578,7 @@ int run_device(lsp_ctx* h,
             for (int pass = 0; pass < npass; ++pass) {
                 UmmaPairParams pp;
                 UmmaParams& up = pp.u;
-                up.recA = pass ? recA1 : recA; up.recB = recB; up.part_var = pvar; up.ws = pass ? ws1 : ws; up.Nt = Nt; up.Nf = Nf;
+                up.recA = pass ? recA1 : recA; up.recB = recB; up.recW = nullptr; up.part_var = pvar; up.ws = pass ? ws1 : ws; up.Nt = Nt; up.Nf = Nf;
                 up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
                 up.flush_ksteps = flush_ksteps;
                 up.trunc_ulps = h->opt_trunc == 0 ? -1.f : (h->opt_trunc == 1 ? 0.f : 1e-3f * (float)h->opt_trunc);
@@ -601,7 +606,7 @@ int run_device(lsp_ctx* h,
             float* wsp = pass ? ws1 : ws;
             if (tensor) {
                 UmmaParams up;
-                up.recA = rA; up.recB = recB; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
+                up.recA = rA; up.recB = recB; up.recW = weighted ? recA1 : nullptr; up.part_var = pvar; up.ws = wsp; up.Nt = Nt; up.Nf = Nf;
                 up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
                 up.flush_ksteps = flush_ksteps; up.trunc_ulps = h->opt_trunc == 1 ? 0.f : -1.f; up.unit_x = pass;   // (the model, or none: LSP_PARAM_TRUNC = 1)
                 up.t = t; up.t_stride = t_stride; up.x = x; up.x_stride = x_stride; up.f_min = f_min; up.df = df;
@@ -614,11 +619,16 @@ int run_device(lsp_ctx* h,
                     dp.list = rlist;
                     dp.refine_r2 = INFINITY;
                     if (rlist.head) { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
-                    void (*duo_kernel)(const UmmaDuoParams) = r.fuse_pre ? accum_umma_duo_kernel<true> : accum_umma_duo_kernel<false>;
+                    void (*duo_kernel)(const UmmaDuoParams) = weighted ? accum_umma_duo_kernel<false, true>
+                                                            : (r.fuse_pre ? accum_umma_duo_kernel<true> : accum_umma_duo_kernel<false>);
                     LSP_CUDA(h, cudaFuncSetAttribute(duo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UD_SMEM));
                     duo_kernel<<<(unsigned)units, US_THREADS, UD_SMEM, st>>>(dp);
                 } else {
 #define LSP_LAUNCH_SMALL(LL, NS, MINB) do { \
+                    if (weighted) { \
+                    LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
+                    accum_umma_small_kernel<LL, NS, MINB, false, true><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); \
+                    LSP_CUDA(h, cudaGetLastError()); } else \
                     if (r.fuse_pre) { \
                     LSP_CUDA(h, cudaFuncSetAttribute(accum_umma_small_kernel<LL, NS, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UmmaSmall<LL, NS>::SMEM)); \
                     accum_umma_small_kernel<LL, NS, MINB, true><<<(unsigned)units, US_THREADS, UmmaSmall<LL, NS>::SMEM, st>>>(up); \

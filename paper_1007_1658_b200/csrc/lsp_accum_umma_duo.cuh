@@ -25,7 +25,8 @@ constexpr int UD_FPB = UD_H * UD_L;                     // frequencies per serie
 constexpr int UD_STAGES = 4;
 constexpr int UD_STAGE_BYTES = 6 * UM_A_BYTES;          // A_hi, A_lo, A_V, B_hi, B_lo, B_V: 128 rows x 32 bytes each
 constexpr int UD_REC_BYTES = 2 * 2 * UM_TS * 16;        // [series][buffer][128 samples]
-constexpr size_t UD_SMEM = (size_t)UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES + 256;
+constexpr int UD_RECW_BYTES = 2 * UM_RECW_BYTES;        // ... and their normalised weights (weighted generalised periodogram)
+constexpr size_t UD_SMEM = (size_t)UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES + UD_RECW_BYTES + 256;
 constexpr int UD_TMEM_COLS = 256;
 constexpr uint32_t UD_IDESC = umma_idesc(UM_H, 128);   // M = 128, N = 128
 
@@ -172,13 +173,15 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
 // and variance over the WHOLE series (fixed order: every CTA of the series gets the identical values) and the exact phases of the
 // samples they stage, straight from t and x; no record arrays, no pre-pass launches.  The first CTA of a series publishes the
 // variance partial and resets the arg-max cell (host: only where no other CTA of the series can reach its epilogue first).
-template <bool FUSED_PRE>
+// WEIGHTED (weighted generalised periodogram, never with FUSED_PRE): as in accum_umma_small_kernel.
+template <bool FUSED_PRE, bool WEIGHTED = false>
 __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const UmmaDuoParams q)
 {
     const UmmaParams& p = q.u;
     extern __shared__ __align__(128) unsigned char um_smem[];
     float4* rec_all = reinterpret_cast<float4*>(um_smem + UD_STAGES * UD_STAGE_BYTES);            // [series][2][UM_TS] {X/sigma, pA32, v32, w32}
-    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES);
+    float* recw_all = reinterpret_cast<float*>(um_smem + UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES);   // [series][2][UM_TS] normalised weight (WEIGHTED)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + UD_STAGES * UD_STAGE_BYTES + UD_REC_BYTES + UD_RECW_BYTES);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * UD_STAGES + 2);
 
     const unsigned tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
@@ -254,8 +257,9 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             xs = l_live ? (p.unit_x ? 1.f : x_scale(p.part_var + lb * p.nparts, p.nparts, p.Nt)) : 0.f;
         }
         const int n_samp_i = (int)n_samp;                                         // split_len < 2^31
-        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull;
+        float pre_x = 0.f, pre_w = 1.f; u64 pre_u = 0ull, pre_v = 0ull;
         bool pre_ok = false;
+        const float* recWx = WEIGHTED ? &p.recW[(l_live ? lb : 0) * p.Nt + j_begin].x : nullptr;
         auto prefetch = [&](int jt) {                                             // this thread's record of a tile, relative to j_begin
             pre_ok = l_live && jt < n_samp_i;
             if (!pre_ok) return;
@@ -266,13 +270,16 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 pre_u = frac_fixed64(p.f_min, tp, nullptr);
                 pre_v = frac_fixed64(p.df, tp, nullptr);
             } else { pre_x = __ldg(recAx + 4 * jt); const ulonglong2 r = __ldg(recB + jt); pre_u = r.x; pre_v = r.y; }
+            if (WEIGHTED) pre_w = __ldg(recWx + 4 * jt);
         };
         prefetch((int)lj);
         float4* rec_mine = rec_all + (ls * 2) * UM_TS + lj;                       // this thread's slot of its series' tile, buffer 0
+        float* recw_mine = recw_all + (ls * 2) * UM_TS + lj;
         // A task: row m = tid & 127 = (series m >> 6, fine value m & 63), 4 samples `chunk` of the k-step
         const unsigned m = tid & 127u, a_s = m >> 6, a_h = m & 63u;
         const int chunk = (int)(tid >> 7);
         const float4* rec_a = rec_all + (a_s * 2) * UM_TS + chunk * 4;            // + buffer * UM_TS + first sample of the k-step
+        const float* recw_a = recw_all + (a_s * 2) * UM_TS + chunk * 4;
         const uint32_t a_dst = s_stage + (uint32_t)chunk * (UM_A_BYTES / 2) + m * 16u;
         // B task (128 per k-step: threads 0..127 on even k-steps, 128..255 on odd ones): series (tid >> 6) & 1, K chunk (tid >> 5) & 1, coarse value tid & 31
         const unsigned b_s = (tid >> 6) & 1u, bc = (tid >> 5) & 1u, b_l = tid & 31u, b_par = (tid >> 7) & 1u;
@@ -301,12 +308,13 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 float4 r = make_float4(0.f, 0.f, 0.f, 0.f);                     // pad: X = 0, phases 0
                 if (pre_ok) {
                     const u64 pa = pre_u + (u64)kb * pre_v;                     // u + kb v (mod 1, 64-bit wrap; reading G3)
-                    r.x = pre_x * xs;
+                    r.x = WEIGHTED ? pre_x * xs * pre_w : pre_x * xs;
                     r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
                     r.z = __uint_as_float((unsigned)((pre_v + 0x80000000ull) >> 32));
                     r.w = __uint_as_float((unsigned)(((u64)UD_H * pre_v + 0x80000000ull) >> 32));
                 }
                 rec_mine[buf * UM_TS] = r;
+                if (WEIGHTED) recw_mine[buf * UM_TS] = pre_ok ? pre_w * pre_w : 0.f;
                 j_tile += UM_TS;                                                // prefetch this thread's record of the following tile
                 prefetch(j_tile);
                 asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
@@ -315,8 +323,9 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             mbar_wait(UD_EMPTY(s), ph_empty);                                   // the MMAs that read this stage have completed
             {
                 const float4* ra = rec_a + buf * UM_TS + sb;
-                if (left >= 4) um_gen_a<false>(ra, 0, a_h, a_dst + st_off, 4);  // `left` is warp-uniform
-                else um_gen_a<true>(ra, 0, a_h, a_dst + st_off, max(0, left));
+                const float* rw = recw_a + buf * UM_TS + sb;
+                if (left >= 4) um_gen_a<false, WEIGHTED>(ra, 0, a_h, a_dst + st_off, 4, rw);  // `left` is warp-uniform
+                else um_gen_a<true, WEIGHTED>(ra, 0, a_h, a_dst + st_off, max(0, left), rw);
             }
             if (((unsigned)ks & 1u) == b_par) ud_gen_b(rec_b + buf * UM_TS + sb, 0, b_l, b_dst + st_off);
             fence_proxy_async();                                                // generic-proxy stores -> visible to the tensor core

@@ -27,8 +27,8 @@ namespace lsp {
 
 // One A item: row h, 4 samples starting at rec[s0].  Writes the 16-byte row chunks of A_hi, A_lo (X e^{ia} as
 // fp16 hi + lo) and A_V (e^{2ia}/2).
-template <bool TAIL>
-__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int nvalid)
+template <bool TAIL, bool WEIGHTED = false>
+__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int nvalid, const float* recw = nullptr)
 {
     unsigned hi[4], lo[4], vv[4];
     #pragma unroll
@@ -46,6 +46,7 @@ __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, 
         lo[i] = pack_h2(lc, ls);
         float v0, v1;
         unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
+        if (WEIGHTED) { const float wv = recw[s0 + i]; v0 *= wv; v1 *= wv; }   // V = sum_j w_j e^{2i theta} (broadcast read)
         vv[i] = pack_h2(v0, v1);
         if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
@@ -53,10 +54,11 @@ __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, 
     sts128(sA + UM_A_BYTES, lo[0], lo[1], lo[2], lo[3]);
     sts128(sA + 2 * UM_A_BYTES, vv[0], vv[1], vv[2], vv[3]);
 }
-__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int64_t left)
+template <bool WEIGHTED = false>
+__device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, uint32_t sA, int64_t left, const float* recw = nullptr)
 {
-    if (left >= 4) um_gen_a<false>(rec, s0, h, sA, 4);                  // `left` is warp-uniform
-    else um_gen_a<true>(rec, s0, h, sA, (int)max((int64_t)0, left));
+    if (left >= 4) um_gen_a<false, WEIGHTED>(rec, s0, h, sA, 4, recw);                  // `left` is warp-uniform
+    else um_gen_a<true, WEIGHTED>(rec, s0, h, sA, (int)max((int64_t)0, left), recw);
 }
 
 constexpr int US_GEN_WARPS = 8;                        // producer (and drain) warps; warp 8 issues the MMAs
@@ -65,7 +67,7 @@ constexpr int US_THREADS = (US_GEN_WARPS + 1) * 32;
 template <int L, int US_STAGES> struct UmmaSmall {
     static constexpr int B_BYTES = 2 * L * 32;         // one B operand tile: 2L rows x 16 fp16
     static constexpr int STAGE_BYTES = 3 * UM_A_BYTES + 3 * B_BYTES;
-    static constexpr size_t SMEM = (size_t)US_STAGES * STAGE_BYTES + UM_REC_BYTES + 256;
+    static constexpr size_t SMEM = (size_t)US_STAGES * STAGE_BYTES + UM_REC_BYTES + UM_RECW_BYTES + 256;
     static constexpr int TMEM_COLS = 4 * L < 32 ? 32 : 4 * L;
     static constexpr uint32_t IDESC = umma_idesc(UM_H, 2 * L);
     static constexpr int FPB = UM_H * L;               // frequencies per CTA
@@ -132,13 +134,16 @@ __device__ __forceinline__ void us_drain(uint32_t taddr, float* dst, int64_t k0,
 // the finish step through part_var_out, use bit-identical values -- and computes the exact 64-bit phases (reading G3) of the
 // samples of its own time split while it stages them.  The tensor forms need no per-sample rotation (cos d, sin d), so the fp64
 // work per sample is two exact products.
-template <int L, int US_STAGES, int MINB, bool FUSED_PRE = false>
+// WEIGHTED (weighted generalised periodogram, never with FUSED_PRE): X = recA.x recW.x = w_j (x_j - xbar_w) / sigma (w_j in the unit
+// pass), and the double-angle operand is scaled by w_j.
+template <int L, int US_STAGES, int MINB, bool FUSED_PRE = false, bool WEIGHTED = false>
 __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(const UmmaParams p)
 {
     using C = UmmaSmall<L, US_STAGES>;
     extern __shared__ __align__(128) unsigned char um_smem[];
     float4* rec = reinterpret_cast<float4*>(um_smem + US_STAGES * C::STAGE_BYTES);                 // [2][UM_TS] {X/sigma, pA32, v32, w32}
-    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + US_STAGES * C::STAGE_BYTES + UM_REC_BYTES);
+    float* recw = reinterpret_cast<float*>(um_smem + US_STAGES * C::STAGE_BYTES + UM_REC_BYTES);    // [2][UM_TS] normalised weight (WEIGHTED)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(um_smem + US_STAGES * C::STAGE_BYTES + UM_REC_BYTES + UM_RECW_BYTES);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * US_STAGES + 2);
 
     const unsigned tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
@@ -214,7 +219,8 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
         } else {
             xs = (tid < UM_TS) ? (p.unit_x ? 1.f : x_scale(p.part_var + b * p.nparts, p.nparts, p.Nt)) : 0.f;
         }
-        float pre_x = 0.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
+        float pre_x = 0.f, pre_w = 1.f; u64 pre_u = 0ull, pre_v = 0ull; bool pre_ok = false;
+        const float4* recW = WEIGHTED ? p.recW + b * p.Nt : nullptr;
         auto prefetch = [&](int ti) {
             const int64_t j = j_begin + (int64_t)ti * UM_TS + tid;
             pre_ok = (tid < UM_TS) && (j < j_end);
@@ -225,6 +231,7 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
                 pre_u = frac_fixed64(p.f_min, tp, nullptr);
                 pre_v = frac_fixed64(p.df, tp, nullptr);
             } else { pre_x = __ldg(&recA[j].x); const ulonglong2 q = __ldg(recB + j); pre_u = q.x; pre_v = q.y; }
+            if (WEIGHTED) pre_w = __ldg(&recW[j].x);
         };
         prefetch(0);
         const unsigned h = tid & 127u;                                  // A item: row h, 4 samples `chunk` of the k-step
@@ -244,12 +251,13 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
                     float4 r = make_float4(0.f, 0.f, 0.f, 0.f);         // pad: X = 0, phases 0
                     if (pre_ok) {
                         const u64 pa = pre_u + (u64)kb * pre_v;         // u + kb v (mod 1, 64-bit wrap; reading G3)
-                        r.x = pre_x * xs;
+                        r.x = WEIGHTED ? pre_x * xs * pre_w : pre_x * xs;
                         r.y = __uint_as_float((unsigned)((pa + 0x80000000ull) >> 32));
                         r.z = __uint_as_float((unsigned)((pre_v + 0x80000000ull) >> 32));
                         r.w = __uint_as_float((unsigned)(((u64)UM_H * pre_v + 0x80000000ull) >> 32));
                     }
                     rec[(ti & 1) * UM_TS + tid] = r;
+                    if (WEIGHTED) recw[(ti & 1) * UM_TS + tid] = pre_ok ? pre_w * pre_w : 0.f;
                     prefetch(ti + 1);
                 }
                 asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
@@ -258,7 +266,7 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
             const float4* rt = rec + (ti & 1) * UM_TS;
             const int sb = (ks & 15) * UM_KS;
             const uint32_t st = s_stage + (uint32_t)s * C::STAGE_BYTES;
-            um_gen_a(rt, sb + chunk * 4, h, st + chunk * (UM_A_BYTES / 2) + h * 16, n_samp - ((int64_t)ks * UM_KS + chunk * 4));
+            um_gen_a<WEIGHTED>(rt, sb + chunk * 4, h, st + chunk * (UM_A_BYTES / 2) + h * 16, n_samp - ((int64_t)ks * UM_KS + chunk * 4), recw + (ti & 1) * UM_TS);
             const unsigned bt = (tid - (unsigned)ks * (2u * L)) & 255u;  // the 2L B items rotate over the 256 producer threads
             if (bt < 2u * L) {
                 const unsigned l = bt % (unsigned)L, bc = bt / (unsigned)L;

@@ -29,11 +29,14 @@ constexpr int UM_KS = 8;                               // samples per k-step (MM
 constexpr int UM_TS = 128;                             // samples per record tile (16 k-steps)
 constexpr int UM_A_BYTES = UM_H * 32;                  // one 128-row operand plane of a k-step: 128 rows x 16 fp16
 constexpr int UM_REC_BYTES = 2 * UM_TS * 16;           // double-buffered record tile
+constexpr int UM_RECW_BYTES = 2 * UM_TS * 4;           // ... and the normalised weights of its samples (weighted generalised periodogram)
 constexpr int UM_TMEM_COLS = 512;
 
 struct UmmaParams {
     const float4* recA;
     const ulonglong2* recB;
+    const float4* recW;         // weighted generalised periodogram (short-grid and batch kernels): recW[j].x = sqrt of the normalised weight w_j;
+                                // recA.x carries one factor sqrt(w_j) already (lsp_prepass.cuh): X = recA.x recW.x, V = sum w e^{2i theta}; else NULL
     const double* part_var;     // [B][nparts]
     float* ws;                  // [B][nsplit][4][Nf]
     int64_t Nt, Nf;

@@ -812,14 +812,23 @@ def test_weighted_generalised_periodogram(lsp):
     assert np.max(np.abs(ref - unw)) > 1e-2 * ref.max()                     # the weights really matter on this input
     assert _top_two_gap(ref) >= QUAL_GAP
     td, xd, wd = torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), torch.from_numpy(wts).cuda()
-    for K, ns in ((0, 0), (8, 3), (32, 2)):
-        h.set_param(pkg.PARAM_K, K); h.set_param(pkg.PARAM_NSPLIT, ns)
+    for K, ns in ((0, 0), (8, 3), (32, 2)):                                 # the FP32-pipe form
+        h.set_param(pkg.PARAM_PIPE, FP32); h.set_param(pkg.PARAM_K, K); h.set_param(pkg.PARAM_NSPLIT, ns)
         P = h.periodogram(td, xd, f_min, df, Nf, weights=wd).cpu().numpy()
         plan = h.last_plan()
         assert "weighted" in plan["kernel"] and plan["pipe"] == FP32, plan
         _check(P, ref, "weighted gls K=%d nsplit=%d" % (K, ns))
         assert int(np.argmax(P)) == oracle.argmax(ref)
-    h.set_param(pkg.PARAM_K, 0); h.set_param(pkg.PARAM_NSPLIT, 0)
+    h.set_param(pkg.PARAM_PIPE, 0); h.set_param(pkg.PARAM_K, 0); h.set_param(pkg.PARAM_NSPLIT, 0)
+    for coarse, ns in ((0, 0), (16, 3), (32, 0), (64, 2)):                  # the short-grid tensor kernel, every coarse extent (automatic plan: (0, 0))
+        h.set_param(pkg.PARAM_COARSE, coarse); h.set_param(pkg.PARAM_NSPLIT, ns)
+        if coarse: h.set_param(pkg.PARAM_PIPE, TENSOR)
+        P = h.periodogram(td, xd, f_min, df, Nf, weights=wd).cpu().numpy()
+        plan = h.last_plan()
+        assert "accum_umma_small_kernel" in plan["kernel"] and "weighted" in plan["kernel"] and plan["pipe"] == TENSOR, plan
+        _check(P, ref, "weighted gls, short-grid tensor kernel, L=%d nsplit=%d" % (coarse, ns))
+        assert int(np.argmax(P)) == oracle.argmax(ref)
+    h.set_param(pkg.PARAM_PIPE, 0); h.set_param(pkg.PARAM_COARSE, 0); h.set_param(pkg.PARAM_NSPLIT, 0)
     # constant weights: the unweighted generalised periodogram (oracle pin GW1), whatever the constant
     Pc = h.periodogram(td, xd, f_min, df, Nf, weights=torch.full_like(wd, 0.37)).cpu().numpy()
     _check(Pc, unw, "constant weights")
@@ -829,6 +838,7 @@ def test_weighted_generalised_periodogram(lsp):
     wb = rng.uniform(0.2, 4.0, xb.shape).astype(np.float32)
     tb, xbd, wbd = torch.from_numpy(wl.t).cuda(), torch.from_numpy(xb).cuda(), torch.from_numpy(wb).cuda()
     P, pi, pv = h.periodogram_batched(tb, xbd, wl.f_min, wl.df, wl.Nf, weights=wbd)
+    assert "accum_umma_duo_kernel" in h.last_plan()["kernel"] and "weighted" in h.last_plan()["kernel"], h.last_plan()   # (odd B: the last CTA holds one series)
     P, pi, pv = P.cpu().numpy(), pi.cpu().numpy(), pv.cpu().numpy()
     for b in range(wl.B):
         rb = oracle.periodogram_gls_weighted(wl.t[b], xb[b], wb[b], wl.f_min, wl.df, wl.Nf)
@@ -868,10 +878,10 @@ def test_weighted_generalised_periodogram_long_grid(lsp):
         assert "pair2" in plan["kernel"] and "weighted" in plan["kernel"], plan
         _check(P, ref, "weighted gls, pair form, table_mb=%d" % table_mb)
         assert int(np.argmax(P)) == oracle.argmax(ref)
-    # a short grid with the tensor pipe requested: the plan is not the pair form, so the FP32 form carries the weights
+    # a short grid: the short-grid tensor kernel carries the weights too
     with _params(h, pipe=TENSOR):
         Ps = h.periodogram(td, xd, f_min, df, 3000, weights=wd).cpu().numpy()
-        assert h.last_plan()["pipe"] == FP32
+        assert h.last_plan()["pipe"] == TENSOR and "accum_umma_small_kernel" in h.last_plan()["kernel"] and "weighted" in h.last_plan()["kernel"]
     _check(Ps, ref[:3000], "weighted gls, short grid")
 
 

@@ -697,6 +697,7 @@ int host_pipe_chunks(const lsp_ctx* h, bool share_t, int64_t B, int64_t Nt, int6
     const double t_out = (want_P ? (double)B * Nf * 4.0 : 0.0) / 50e9;
     if (B < 64 || t_in + t_out < 150e-6) return 1;
     const double terms = (double)B * (double)Nt * (double)Nf;
+    bool fp32_form = false;
     auto grid = [&](int64_t nb, double& units, double& slots, double& rate) {
         if (use_shared_path(h, share_t ? 0 : Nt, nb, Nt, false)) {
             units = (double)((nb + SG_M - 1) / SG_M) * (double)((Nf + SG_F - 1) / SG_F); slots = 2.0 * h->sm_count; rate = 5e13;
@@ -705,8 +706,8 @@ int host_pipe_chunks(const lsp_ctx* h, bool share_t, int64_t B, int64_t Nt, int6
         Route r;
         if (route(h, share_t ? 0 : Nt, nb, Nt, Nf, false, r) != LSP_OK) return false;
         units = (double)(r.duo ? (nb + 1) / 2 : nb) * r.pl.nsplit * r.pl.nfb;
-        if (r.tensor) { slots = (double)plan_umma_ctas_per_sm(r.pl.L) * h->sm_count; rate = r.pair ? 5e13 : 1.2e13; }
-        else { slots = (double)plan_ctas_per_sm(r.pl.K, r.pl.T, r.pl.split_len <= PLAN_FOLD_SAMPLES) * h->sm_count; rate = 4.5e12; }
+        if (r.tensor) { slots = (double)(r.duo ? 2 : plan_umma_ctas_per_sm(r.pl.L)) * h->sm_count; rate = r.pair ? 5e13 : 1.2e13; }
+        else { slots = (double)plan_ctas_per_sm(r.pl.K, r.pl.T, r.pl.split_len <= PLAN_FOLD_SAMPLES) * h->sm_count; rate = 4.5e12; fp32_form = true; }
         return true;
     };
     double u1, s1, rate;
@@ -719,7 +720,11 @@ int host_pipe_chunks(const lsp_ctx* h, bool share_t, int64_t B, int64_t Nt, int6
         double un, sn, rn;
         if (!grid((B + n - 1) / n, un, sn, rn)) continue;
         const double wavesn = un > sn ? std::ceil(un / sn) : 1.0;
-        const double comp = t_comp * (n * wavesn) / waves1 * (u1 > s1 ? 1.0 : std::fmax(1.0, n * 0.35));   // under-filled grids: chunks do not get n times shorter
+        // waves x work per CTA, relative to the whole batch in one call (a chunk of a tensor-form batch may be planned with more, shorter
+        // CTAs: un != u1 / n; measured at C4: 4 chunks 1.40 ms, 2 chunks 1.61 ms).  FP32 form: every split pays its fixed cost again and the
+        // finish step reads them all: a wave of a chunk is charged like a wave of the whole batch (C4S: 1 chunk 2.85 ms, 4 chunks 3.26 ms)
+        const double rel = fp32_form ? (n * wavesn) / waves1 : (wavesn / un) / (waves1 / u1);
+        const double comp = t_comp * rel * (u1 > s1 ? 1.0 : std::fmax(1.0, n * 0.35));   // under-filled grids: chunks do not get n times shorter
         const double pipe = std::fmax(t_in + (comp + t_out) / n, std::fmax(comp + (t_in + t_out) / n, t_out + (t_in + comp) / n));
         if (pipe < best_t) { best_t = pipe; best = n; }
     }

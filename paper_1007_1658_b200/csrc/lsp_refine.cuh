@@ -51,6 +51,7 @@ struct RefineSrc {
 constexpr int REFINE_SPLIT_ENTRIES = 256;   // refine_kernel: up to this many listed frequencies of long series are each spread over ...
 constexpr int REFINE_MAX_SPLIT = 64;        // ... up to this many blocks (ranges of samples), REFINE_SPLIT_MIN samples or more each
 constexpr int REFINE_SPLIT_MIN = 4096;
+constexpr int REFINE_WARP_MAX_NT = 4096;   // refine_kernel: series no longer than this get a warp per listed frequency instead of a block
 
 struct RefineList {
     unsigned* head;                          // [0] entries appended, [1] blocks of refine_kernel done; both 0 between calls
@@ -81,6 +82,7 @@ __device__ __forceinline__ bool refine_push(const RefineList& L, int64_t b, int6
 
 // Sum over the block of NV values per thread, the same result in every thread: xor-butterfly inside a warp (both partners
 // add the same two numbers), then the warps' sums in warp order.  `red` holds (NT / 32) * NV doubles.
+// NT = 32: the team is ONE WARP of a larger block (short series: a warp per frequency); no shared memory, no barrier.
 template <int NT, int NV>
 __device__ __forceinline__ void refine_block_sum(double (&v)[NV], double* red)
 {
@@ -88,6 +90,7 @@ __device__ __forceinline__ void refine_block_sum(double (&v)[NV], double* red)
     for (int q = 0; q < NV; ++q)
         #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+    if (NT == 32) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     __syncthreads();                                                    // (red may still be read from the previous call)
     if (lane == 0) {
@@ -114,7 +117,7 @@ __device__ void refine_sums_range(const RefineSrc& s, int64_t b, int64_t k, doub
     const float* x = s.x + b * s.x_stride;
     const float* w = s.w ? s.w + b * s.w_stride : nullptr;
     const double t0 = __ldg(t), f = s.f_min + (double)k * s.df;
-    for (int64_t j = j0 + threadIdx.x; j < j1; j += NT) {
+    for (int64_t j = j0 + (NT == 32 ? (threadIdx.x & 31) : threadIdx.x); j < j1; j += NT) {
         double ph = (__ldg(t + j) - t0) * f;
         ph -= rint(ph);
         double sn, cs;
@@ -141,9 +144,10 @@ __device__ void refine_sums(const RefineSrc& s, int64_t b, int64_t k, bool gls, 
     const float* x = s.x + b * s.x_stride;
     const float* w = s.w ? s.w + b * s.w_stride : nullptr;
     const int64_t Nt = s.Nt;
+    const int tid = NT == 32 ? (threadIdx.x & 31) : threadIdx.x;        // (NT = 32: a warp of a larger block)
     const double t0 = __ldg(t);
     double m[3] = {0.0, 0.0, 0.0};                                      // sum w, sum w x, sum w (t - t_0)
-    for (int64_t j = threadIdx.x; j < Nt; j += NT) {
+    for (int64_t j = tid; j < Nt; j += NT) {
         const double wj = w ? (double)__ldg(w + j) : 1.0;
         m[0] += wj; m[1] += wj * (double)__ldg(x + j); m[2] += wj * (__ldg(t + j) - t0);
     }
@@ -156,7 +160,7 @@ __device__ void refine_sums(const RefineSrc& s, int64_t b, int64_t k, bool gls, 
     } else {
         const double tc = t0 + m[2] / m[0];                             // weighted mean time
         double a[2] = {0.0, 0.0};                                       // sum w (cos - 1), sum w sin
-        for (int64_t j = threadIdx.x; j < Nt; j += NT) {
+        for (int64_t j = tid; j < Nt; j += NT) {
             double ph = (__ldg(t + j) - tc) * f;
             ph -= rint(ph);
             double sh, ch;
@@ -166,7 +170,7 @@ __device__ void refine_sums(const RefineSrc& s, int64_t b, int64_t k, bool gls, 
         }
         refine_block_sum<NT, 2>(a, red);
         const double cbar = a[0] / (double)Nt, sbar = a[1] / (double)Nt;   // (sum of the scaled weights = Nt)
-        for (int64_t j = threadIdx.x; j < Nt; j += NT) {
+        for (int64_t j = tid; j < Nt; j += NT) {
             double ph = (__ldg(t + j) - tc) * f;
             ph -= rint(ph);
             double sh, ch;
@@ -271,6 +275,22 @@ __global__ void __launch_bounds__(REFINE_THREADS) refine_kernel(const RefinePara
                     if (p.peak_idx) atomicMax(p.peak64 + b, ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k));
                     p.list.entry_done[e] = 0u;                          // (for the next call)
                 }
+            }
+        }
+    } else if (Nt <= REFINE_WARP_MAX_NT) {
+        // short series: a warp per entry (eight at a time per block); a block per entry would spend its time in the reductions
+        const unsigned lane = threadIdx.x & 31u;
+        for (unsigned e = blockIdx.x * (REFINE_THREADS / 32) + (threadIdx.x >> 5); e < n; e += gridDim.x * (REFINE_THREADS / 32)) {
+            const int2 it = p.list.items[e];
+            const int64_t b = it.x, k = it.y;
+            double v[6];
+            refine_sums<32>(p.src, b, k, p.gls != 0, v, nullptr);
+            if (lane == 0) {
+                double q = 0.0;
+                for (int i = 0; i < p.nparts; ++i) q += p.part_var[b * p.nparts + i];
+                const float Pf = (float)refine_combine(v, (double)Nt, 0.5 / (q / (double)(Nt - 1)), p.gls != 0);
+                if (p.P) p.P[b * p.p_stride + k] = Pf;
+                if (p.peak_idx) atomicMax(p.peak64 + b, ((u64)__float_as_uint(fmaxf(Pf, 0.f)) << 32) | (u64)(0xffffffffu - (unsigned)k));
             }
         }
     } else

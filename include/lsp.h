@@ -143,7 +143,7 @@ int lsp_periodogram_batched(lsp_handle h,
  * P = (chi0^2 - chi^2_min) / (2 var) -- the normalisation of eq. (1), to which it reduces when the constant is
  * orthogonal to the sinusoids.  Same arguments, layout, ownership and errors as lsp_periodogram[_batched], Nt >= 4.
  * Computed from the sums of eq. (8) plus sum cos(w t_j), sum sin(w t_j), which a second accumulate pass with unit
- * weights provides (cost: two accumulate launches).  Where the fit is singular (f -> 0: D = CCn SSn - CSn^2 <= 1e-9) P = 0.
+ * weights provides (cost: two accumulate launches on the tensor-core forms, one on the FP32-pipe form).  Where the fit is singular (f -> 0: D = CCn SSn - CSn^2 <= 1e-9) P = 0.
  */
 int lsp_periodogram_gls(lsp_handle h,
                         const double* t, const float* x, int64_t Nt,

@@ -112,30 +112,37 @@ int ensure(lsp_ctx* h, void** ptr, size_t* have, size_t need) {
 
 typedef void (*accum_fn)(const AccumParams);
 
-struct KernelEntry { int K; accum_fn fn, fn_weighted, fn_direct; const char* name; const char* name_weighted; int max_t; };
+struct KernelEntry { int K; accum_fn fn, fn_weighted, fn_direct, fn_gls, fn_gls_weighted; const char* name; const char* name_weighted;
+                     const char* name_gls; const char* name_gls_weighted; int max_t; };
 
+constexpr int GLS_FUSED_MAX_K = 20;       // FP32 form, generalised periodogram in one pass (accum_z_kernel<..., GLS>): 2 K more registers per thread
 #define LSP_ENTRY_Z(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, accum_z_kernel<K, MAXT, MINB, true>, accum_z_kernel<K, MAXT, MINB, false, true>, \
-                                     "accum_z_kernel<K=" #K ",fp32,three-term>", "accum_z_kernel<K=" #K ",fp32,three-term,weighted>", MAXT }
+                                     nullptr, nullptr, \
+                                     "accum_z_kernel<K=" #K ",fp32,three-term>", "accum_z_kernel<K=" #K ",fp32,three-term,weighted>", "", "", MAXT }
+#define LSP_ENTRY_ZG(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, accum_z_kernel<K, MAXT, MINB, true>, accum_z_kernel<K, MAXT, MINB, false, true>, \
+                                     accum_z_kernel<K, MAXT, MINB, false, false, true>, accum_z_kernel<K, MAXT, MINB, true, false, true>, \
+                                     "accum_z_kernel<K=" #K ",fp32,three-term>", "accum_z_kernel<K=" #K ",fp32,three-term,weighted>", \
+                                     "accum_z_kernel<K=" #K ",fp32,three-term,generalised one-pass>", "accum_z_kernel<K=" #K ",fp32,three-term,generalised one-pass,weighted>", MAXT }
 const KernelEntry g_kernels[] = {
-    LSP_ENTRY_Z(4, 256, 1), LSP_ENTRY_Z(8, 256, 1), LSP_ENTRY_Z(12, 256, 1), LSP_ENTRY_Z(16, 256, 1),
-    LSP_ENTRY_Z(20, 256, 1), LSP_ENTRY_Z(24, 256, 2), LSP_ENTRY_Z(28, 128, 3), LSP_ENTRY_Z(32, 128, 3),
+    LSP_ENTRY_ZG(4, 256, 1), LSP_ENTRY_ZG(8, 256, 1), LSP_ENTRY_ZG(12, 256, 1), LSP_ENTRY_ZG(16, 256, 1),
+    LSP_ENTRY_ZG(20, 256, 1), LSP_ENTRY_Z(24, 256, 2), LSP_ENTRY_Z(28, 128, 3), LSP_ENTRY_Z(32, 128, 3),
 };
-
 const KernelEntry* find_kernel(int K) {
     for (const KernelEntry& e : g_kernels) if (e.K == K) return &e;
     return nullptr;
 }
 
-size_t accum_smem_bytes(const KernelEntry* ke, int T, bool weighted, bool direct) {
-    return (size_t)TILE_Z * (weighted ? 32 : 24) + (direct ? 0 : (size_t)T * (4 * ke->K + 1) * sizeof(float));
+size_t accum_smem_bytes(const KernelEntry* ke, int T, bool weighted, bool direct, bool gls_fused = false) {
+    return (size_t)TILE_Z * (weighted ? 32 : 24) + (direct ? 0 : (size_t)T * ((gls_fused ? 6 : 4) * ke->K + 1) * sizeof(float));
 }
 
 // Launch plan: which form and tile, how many time splits (and chunks).  Units of work = B * nfb * nsplit CTAs; the
 // hardware block scheduler balances them over the SMs, so we want many more units than CTA slots.
-Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t table_series, int force_pipe = 0)
+Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t table_series, int force_pipe = 0, int max_K = 32)
 {
     Plan pl;
     PlanOverrides ov;
+    ov.max_K = max_K;
     ov.K = h->opt_K; ov.T = h->opt_T; ov.nsplit = h->opt_nsplit; ov.pipe = force_pipe ? force_pipe : h->opt_pipe; ov.L = h->opt_coarse;
     ov.table_budget = h->opt_table_mb ? (h->opt_table_mb << 20) : 0; ov.table_series = table_series;
     const PlanChoice pc = plan_choose(h->sm_count, B, Nt, Nf, ov);
@@ -418,13 +425,13 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
 }
 
 // What the call will run (shared by run_device and lsp_reserve).
-struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair, fuse_pre; int64_t tab_series; };
+struct Route { Plan pl; bool tensor, small, duo, duo_fuse, pair, fuse_pre, gls_fused; int64_t tab_series; };
 
 int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf, bool gls, Route& r, bool weighted = false)
 {
     r.tab_series = (t_stride == 0) ? 1 : B;
-    r.pl = make_plan(h, B, Nt, Nf, r.tab_series);
-    // (per-sample weights: every form carries them)
+    // (per-sample weights: every form carries them; generalised periodogram on the FP32 form: one pass with K <= 20 frequencies per thread)
+    r.pl = make_plan(h, B, Nt, Nf, r.tab_series, 0, gls ? GLS_FUSED_MAX_K : 32);
     Plan& pl = r.pl;
     if (pl.K == 0) return LSP_EINVAL;
     r.tensor = pl.pipe == PLAN_PIPE_TENSOR;
@@ -433,10 +440,13 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
     r.duo = r.small && pl.L == 16 && B >= 2;              // batches: two series per CTA (lsp_accum_umma_duo.cuh)
     // one CTA sees all samples of its series in one drain window: steps 6-7 run in its epilogue, no workspace round trip
     r.duo_fuse = r.duo && !gls && pl.nsplit == 1 && Nt <= (h->opt_flush ? h->opt_flush : 2048);
+    r.gls_fused = false;
     if (!r.tensor) {
         const KernelEntry* ke = find_kernel(pl.K);
         if (!ke || pl.T < 32 || pl.T > ke->max_t || (pl.T % 32) != 0) return LSP_EINVAL;
         pl.kernel_name = weighted ? ke->name_weighted : ke->name;
+        r.gls_fused = gls && ke->fn_gls != nullptr;          // (a forced K > 20 takes the two-pass route)
+        if (r.gls_fused) pl.kernel_name = weighted ? ke->name_gls_weighted : ke->name_gls;
     } else if (r.pair) {
         if (h->opt_corr) pl.kernel_name = weighted ? "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16,hi+lo,fine-table,weighted>"
                                                    : "accum_umma_pair2_kernel<tcgen05.cta_group2.m256n256.f16,hi+lo,fine-table>";
@@ -468,7 +478,7 @@ int route(const lsp_ctx* h, int64_t t_stride, int64_t B, int64_t Nt, int64_t Nf,
         r.fuse_pre = true;
         pl.launches = r.duo_fuse ? 1 : 2; pl.nparts = 1; pl.part_chunk = Nt; pl.fused_pre = false;
     }
-    if (gls) pl.launches += 1 + (r.pair ? pl.nchunks : 1);   // unit records + second accumulate pass
+    if (gls && !r.gls_fused) pl.launches += 1 + (r.pair ? pl.nchunks : 1);   // unit records + second accumulate pass
     const int64_t units = (r.duo ? (B + 1) / 2 : B) * (int64_t)pl.nsplit * pl.nfb;
     if (units > 2147483647LL) return LSP_EINVAL;
     return LSP_OK;
@@ -539,8 +549,8 @@ int run_device(lsp_ctx* h,
     else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
     LSP_CUDA(h, cudaGetLastError());
     }
-    if (weighted) pl.launches -= 1;                       // (the weight records were written by records_weighted_kernel)
-    if (gls && !weighted) {
+    if (weighted && !r.gls_fused) pl.launches -= 1;       // (the weight records were written by records_weighted_kernel)
+    if (gls && !weighted && !r.gls_fused) {
         unit_records_kernel<<<(unsigned)((n_samp + 255) / 256), 256, 0, st>>>(recA, recA1, (int64_t)n_samp);
         LSP_CUDA(h, cudaGetLastError());
     }
@@ -552,7 +562,7 @@ int run_device(lsp_ctx* h,
     if (r.duo_fuse && refine) { rc = refine_list(h, rlist); if (rc != LSP_OK) return rc; pl.launches += 1; }
 
     // steps 3-5 (generalised periodogram: a second pass with unit weights gives sum cos, sum sin in ws1)
-    const int npass = gls ? 2 : 1;
+    const int npass = (gls && !r.gls_fused) ? 2 : 1;
     // short grids, one pass: records -> accumulate -> finish as programmatic dependents (launch latency and CTA set-up overlap the predecessor's tail)
     const bool pdl_small = r.small && !r.duo && !gls && h->opt_pdl != 1;
     // drain interval of D_W: 2,048 samples; 8,192 in the CTA-pair form, where a drain stalls the whole pipeline of the pair (5 % faster
@@ -644,12 +654,13 @@ int run_device(lsp_ctx* h,
             } else {
                 AccumParams ap;
                 ap.recW = weighted ? recA1 : nullptr;
-                ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.Nt = Nt; ap.Nf = Nf;
+                ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.ws1 = ws1; ap.Nt = Nt; ap.Nf = Nf;
                 ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
                 // the whole split inside one fold interval: the register partials go straight to `ws` (no shared-memory accumulators)
-                const bool direct = !weighted && pl.split_len <= (int64_t)pl.flush_tiles * TILE_Z;
-                const size_t smem = accum_smem_bytes(ke, pl.T, weighted, direct);
-                const accum_fn fn = weighted ? ke->fn_weighted : (direct ? ke->fn_direct : ke->fn);
+                const bool direct = !weighted && !r.gls_fused && pl.split_len <= (int64_t)pl.flush_tiles * TILE_Z;
+                const size_t smem = accum_smem_bytes(ke, pl.T, weighted, direct, r.gls_fused);
+                const accum_fn fn = r.gls_fused ? (weighted ? ke->fn_gls_weighted : ke->fn_gls)
+                                                : (weighted ? ke->fn_weighted : (direct ? ke->fn_direct : ke->fn));
                 LSP_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                 fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
             }

@@ -34,6 +34,7 @@ struct AccumParams {
     const float4* recA;
     const ulonglong2* recB;
     float* ws;              // [B][nsplit][4][Nf]
+    float* ws1;             // GLS kernels: [B][nsplit][4][Nf], planes 0, 1 = sum (w) cos, sum (w) sin (the generalised periodogram's C, S)
     int64_t Nt, Nf;
     int64_t split_len;      // samples per split (multiple of TILE_Z; the last split may be shorter)
     int nsplit;
@@ -41,7 +42,7 @@ struct AccumParams {
     int flush_tiles;        // tiles of TILE_Z samples between folds of the register partials
 };
 
-struct ZAnchor { float c0, s0, cp, sp, X, g; };
+struct ZAnchor { float c0, s0, cp, sp, X, g, sw; };
 
 // step 3: anchor at the thread's first frequency: exact integer phase (reading G3) -> MUFU sin/cos
 // (PAPER.md:290), plus the value one recurrence step back by an exact rotation (consistent with the
@@ -63,15 +64,19 @@ __device__ __forceinline__ ZAnchor z_anchor(const float4* tS, const void* tRv, i
     if (WEIGHTED) { a.c0 *= sw; a.s0 *= sw; }
     a.cp = fmaf(a.c0, cd, a.s0 * sd);
     a.sp = fmaf(a.s0, cd, -(a.c0 * sd));
-    a.X = sv.x; a.g = sv.y;
+    a.X = sv.x; a.g = sv.y; a.sw = sw;
     return a;
 }
 
 // DIRECT (the CTA's whole time split fits ONE fold interval, e.g. batches of short series): the register partials are the
 // split's sums and go straight to `ws`; no shared-memory accumulators, so more CTAs fit per SM (C4: 6 instead of 5).
-template <int K, int MAXT, int MINB, bool WEIGHTED = false, bool DIRECT = false>
+// GLS (generalised periodogram in ONE pass: "two more FMAs per term in the same kernel"): a third packed
+// accumulator per frequency, (C, S)_m += sw * z_m (sw = 1 without weights; with weights z carries one sqrt(w) already), one more
+// FFMA2 per term = 8 lane-ops instead of the 12 of two passes; 2 K more registers, so K <= 20.
+template <int K, int MAXT, int MINB, bool WEIGHTED = false, bool DIRECT = false, bool GLS = false>
 __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p)
 {
+    constexpr int NQ = GLS ? 6 : 4;                            // sums per frequency
     extern __shared__ float4 lsp_smem[];
     float4* tS = lsp_smem;                                     // {X, g, b32, w32} per sample
     void* tR = tS + TILE_Z;                                    // {cd, sd} per sample (WEIGHTED: {cd, sd, sw, -}, the tile region is sized for it)
@@ -83,7 +88,7 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
 #define LSP_Z_OUTER_TM 1
 #endif
 #if LSP_Z_OUTER_TM
-#define OIDX(q, m) (tid * (4 * K + 1) + (q) * K + (m))
+#define OIDX(q, m) (tid * (NQ * K + 1) + (q) * K + (m))
 #else
 #define OIDX(q, m) (((q) * K + (m)) * T + tid)
 #endif
@@ -100,17 +105,18 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
 
     if (!DIRECT) {
         #pragma unroll
-        for (int i = 0; i < 4 * K; ++i) outer[OIDX(i / K, i % K)] = 0.f;
+        for (int i = 0; i < NQ * K; ++i) outer[OIDX(i / K, i % K)] = 0.f;
     }
 
     u64 A1[K], A2[K];                                          // (XC, XS), (CC - n/2, CS)
+    u64 A3[GLS ? K : 1];                                       // GLS: (C, S)
     int64_t j = j_begin;
     int tiles_since_flush = 0;
     bool fresh = true;
     if (DIRECT) {                                              // one interval: the whole split
         const u64 init = pack2(-0.5f * (float)max((int64_t)0, j_end - j_begin), 0.f);
         #pragma unroll
-        for (int m = 0; m < K; ++m) { A1[m] = 0ull; A2[m] = init; }
+        for (int m = 0; m < K; ++m) { A1[m] = 0ull; A2[m] = init; if (GLS) A3[m] = 0ull; }
         fresh = false;
     }
 
@@ -120,7 +126,7 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
             const float n_int = (float)min((int64_t)flush_tiles * TILE_Z, j_end - j);
             const u64 init = pack2(-0.5f * n_int, 0.f);        // centred CC partial
             #pragma unroll
-            for (int m = 0; m < K; ++m) { A1[m] = 0ull; A2[m] = init; }
+            for (int m = 0; m < K; ++m) { A1[m] = 0ull; A2[m] = init; if (GLS) A3[m] = 0ull; }
             fresh = false;
         }
         __syncthreads();                                       // previous tile fully consumed
@@ -155,12 +161,14 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
             u64 z = pack2(cur.c0, cur.s0);
             u64 zp = pack2(cur.cp, cur.sp);
             const u64 XX = pack2(cur.X, cur.X), GG = pack2(cur.g, cur.g);
+            const u64 SW = pack2(cur.sw, cur.sw);              // (GLS only)
             // step 4
             #pragma unroll
             for (int m = 0; m < K; ++m) {
                 float cm, sm; unpack2(z, cm, sm);
                 A1[m] = fma2(XX, z, A1[m]);
                 A2[m] = fma2(pack2(cm, cm), z, A2[m]);
+                if (GLS) A3[m] = fma2(SW, z, A3[m]);
                 if (m + 1 < K) { const u64 zn = fma2(GG, z, neg2(zp)); zp = z; z = zn; }
             }
         }
@@ -176,6 +184,7 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
                 outer[OIDX(1, m)] += xs;
                 outer[OIDX(2, m)] += cc;
                 outer[OIDX(3, m)] += cs;
+                if (GLS) { float c1, s1; unpack2(A3[m], c1, s1); outer[OIDX(4, m)] += c1; outer[OIDX(5, m)] += s1; }
             }
             tiles_since_flush = 0;
             fresh = true;
@@ -183,10 +192,15 @@ __global__ void __launch_bounds__(MAXT, MINB) accum_z_kernel(const AccumParams p
     }
 
     float* ws = p.ws + ((b * p.nsplit + sp) * 4) * p.Nf;
+    float* ws1 = GLS ? p.ws1 + ((b * p.nsplit + sp) * 4) * p.Nf : nullptr;
     #pragma unroll
     for (int m = 0; m < K; ++m) {
         const int64_t k = kb + (int64_t)tid * K + m;
         if (k < p.Nf) {
+            if (GLS) {
+                if (DIRECT) { float c1, s1; unpack2(A3[m], c1, s1); ws1[k] = c1; ws1[p.Nf + k] = s1; }
+                else { ws1[k] = outer[OIDX(4, m)]; ws1[p.Nf + k] = outer[OIDX(5, m)]; }
+            }
             if (DIRECT) {
                 float xc, xs, cc, cs;
                 unpack2(A1[m], xc, xs); unpack2(A2[m], cc, cs);

@@ -34,7 +34,7 @@ struct PlanChoice {
     double score = 0.0;
 };
 
-struct PlanOverrides { int64_t K = 0, T = 0, nsplit = 0, pipe = 0, L = 0, table_budget = 0, table_series = 1; };
+struct PlanOverrides { int64_t K = 0, T = 0, nsplit = 0, pipe = 0, L = 0, table_budget = 0, table_series = 1; int max_K = 32; /* FP32 form: widest thread tile considered */ };
 
 inline bool plan_valid_K(int K) { return K >= 4 && K <= 32 && (K % 4) == 0; }
 
@@ -170,6 +170,7 @@ inline PlanChoice plan_choose_fp32(int sm_count, int64_t B, int64_t Nt, int64_t 
     PlanChoice best;
     for (int K = 32; K >= 4; K -= 4) {
         if (ov.K && ov.K != K) continue;
+        if (!ov.K && K > ov.max_K) continue;
         for (int ti = 0; ti < nT; ++ti) {
             const int T = Ts[ti];
             if (T > plan_max_threads(K)) continue;

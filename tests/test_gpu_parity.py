@@ -725,8 +725,8 @@ def test_host_batch_pipelined_over_series_chunks(lsp, shared_t):
 
 
 # ------------------------------------------------------------------ generalised periodogram, false-alarm probability
-@pytest.mark.parametrize("prm", [dict(), dict(pipe=FP32), dict(pipe=TENSOR, coarse=128), dict(pipe=TENSOR, coarse=32),
-                                 dict(pipe=TENSOR, coarse=128, table_mb=2)])
+@pytest.mark.parametrize("prm", [dict(), dict(pipe=FP32), dict(pipe=FP32, K=8, nsplit=3), dict(pipe=FP32, K=32), dict(pipe=TENSOR, coarse=128),
+                                 dict(pipe=TENSOR, coarse=32), dict(pipe=TENSOR, coarse=128, table_mb=2)])
 def test_generalised_periodogram(lsp, prm):
     """lsp_periodogram_gls (floating-mean fit) against the oracle's 3-parameter least squares, on
     gappy sampling with a large offset where it differs visibly from eq. (1); every form of steps 3-5 (the unit-weight
@@ -749,6 +749,9 @@ def test_generalised_periodogram(lsp, prm):
     assert int(np.argmax(P)) == oracle.argmax(ref)
     if prm.get("pipe"):
         assert plan["pipe"] == prm["pipe"]
+    if prm.get("pipe") == FP32:                             # one pass with a third accumulator per frequency up to K = 20; two passes beyond
+        assert ("generalised one-pass" in plan["kernel"]) == (prm.get("K", 0) <= 20), plan
+        assert plan["launches"] == (3 if prm.get("K", 0) <= 20 else 5), plan      # records (mean fused), accumulate, finish (+ unit records, second pass)
 
 
 def test_generalised_periodogram_long_grid(lsp):

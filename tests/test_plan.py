@@ -121,7 +121,7 @@ def test_occupancy_model_matches_the_compiled_kernels():
     src = open(os.path.join(b.CSRC, "lsp_plan.h")).read()
     table = [int(v) for v in re.search(r"static const int z\[9\] = \{([^}]*)\}", src).group(1).split(",")]
     seen = {}
-    for m in re.finditer(r"Compiling entry function '_ZN3lsp14accum_z_kernelILi(\d+)ELi\d+ELi\d+ELb0ELb0EEEvNS_11AccumParamsE'.*?Used (\d+) registers", log, re.S):
+    for m in re.finditer(r"Compiling entry function '_ZN3lsp14accum_z_kernelILi(\d+)ELi\d+ELi\d+ELb0ELb0ELb0EEEvNS_11AccumParamsE'.*?Used (\d+) registers", log, re.S):
         seen[int(m.group(1))] = int(m.group(2))
     assert sorted(seen) == [4, 8, 12, 16, 20, 24, 28, 32]
     for K, regs in seen.items():

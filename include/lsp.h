@@ -52,7 +52,8 @@ enum {
     LSP_OK      =  0,
     LSP_EINVAL  = -1,   /* NULL handle/pointer, Nt < 2, Nf < 1, B < 1 or B > 65,535, bad stride, non-finite or negative f_min/df */
     LSP_ECUDA   = -2,   /* a CUDA runtime call failed; see lsp_last_cuda_error */
-    LSP_ENOMEM  = -3    /* workspace allocation failed */
+    LSP_ENOMEM  = -3,   /* workspace allocation failed */
+    LSP_ELIMIT  = -4    /* lsp_periodogram_static only: Nt or Nf beyond its fixed limits */
 };
 
 /*
@@ -93,6 +94,8 @@ enum {
                               /* set-up overlap its predecessor's tail); 1 = separate pre-pass kernels in plain stream order            */
 };
 enum { LSP_PIPE_AUTO = 0, LSP_PIPE_FP32 = 1, LSP_PIPE_TENSOR = 2 };
+/* lsp_periodogram_static: its fixed device array and the sizes it accepts */
+enum { LSP_STATIC_SCRATCH_BYTES = 8 << 20, LSP_STATIC_MAX_NT = 16384, LSP_STATIC_MAX_NF = 262144 };
 
 /* Create a handle bound to CUDA device `device` (-1 = the calling thread's current device). */
 int lsp_create(lsp_handle* out, int device);
@@ -217,6 +220,25 @@ int lsp_periodogram_batched_host(lsp_handle h,
  *   N_f, or the N_f,ind <= N_f of PAPER.md:369 (real-valued).  Enqueues one kernel on `stream`; no synchronisation.
  */
 int lsp_false_alarm(lsp_handle h, const float* P, int64_t n, int64_t Nt, double N_ind, float* Q, void* stream);
+
+/*
+ * One series, NO ALLOCATION: for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it).  Same result as lsp_periodogram with LSP_PARAM_PIPE = LSP_PIPE_FP32 (eqs (1)-(2) via (5)-(8),
+ * the paper's fp32 arithmetic, ill-conditioned frequencies refined in fp64), plus the optional peak of
+ * lsp_periodogram_batched.  No handle: it runs on the calling thread's CURRENT device; no tunables apply.
+ *   t DEVICE const double[Nt], x DEVICE const float[Nt], P DEVICE float[Nf] (nullable if the peak is asked for),
+ *   peak_idx DEVICE int32_t[1], peak_val DEVICE float[1] (both or neither; lowest index among equal maxima, reading G9).
+ * Limits: 2 <= Nt <= LSP_STATIC_MAX_NT (16,384), 1 <= Nf <= LSP_STATIC_MAX_NF (262,144); beyond them LSP_ELIMIT, nothing launched.
+ * Its workspace (32 B per sample + 16 B x Nf x time splits, as many splits as fit) is a file-scope `static __device__` array of
+ * LSP_STATIC_SCRATCH_BYTES (8 MiB) inside the library: every GPU that loads the library holds those 8 MiB until the process
+ * exits.  The call itself calls no cudaMalloc / cudaFree and no allocating library routine, never synchronises, and enqueues
+ * three kernels on `stream`; the first call on a device also resolves the array's device address (cudaGetSymbolAddress).
+ * ALL calls on a device share the one array, which keeps the previous call's contents: every region is rewritten before it is
+ * read and the arg-max cell is reset by the call's first kernel, so calls in stream order are independent of each other --
+ * but two calls that OVERLAP on the GPU (different streams, or graphs replayed concurrently) race on it: serialise them.
+ */
+int lsp_periodogram_static(const double* t, const float* x, int64_t Nt, double f_min, double df, int64_t Nf,
+                           float* P, int32_t* peak_idx, float* peak_val, void* stream);
 
 /*
  * Grow the workspace now to what a call with (B series -- `shared_t` != 0: on one time vector --, Nt samples, Nf

@@ -12,7 +12,8 @@ from typing import Optional, Tuple
 
 from . import build as _build
 
-LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM = 0, -1, -2, -3
+LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM, LSP_ELIMIT = 0, -1, -2, -3, -4
+STATIC_SCRATCH_BYTES, STATIC_MAX_NT, STATIC_MAX_NF = 8 << 20, 16384, 262144
 PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_PIPE, PARAM_FLUSH, PARAM_TIMING, PARAM_TABLE_MB, PARAM_COARSE, PARAM_TRUNC, PARAM_SHARED, PARAM_PDL, PARAM_CORR, PARAM_REFINE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15, 16
 PIPE_AUTO, PIPE_FP32, PIPE_TENSOR = 0, 1, 2
 
@@ -24,7 +25,7 @@ SYMBOLS = (
     "lsp_false_alarm", "lsp_periodogram_gls", "lsp_periodogram_gls_batched",
     "lsp_periodogram_gls_weighted", "lsp_periodogram_gls_weighted_batched", "lsp_reserve",
     "lsp_last_plan", "lsp_last_timing", "lsp_call_timing", "lsp_plan_query", "lsp_plan_query_form", "lsp_last_kernel_name", "lsp_last_host_chunks", "lsp_probe_mma_accumulate", "lsp_last_cuda_error",
-    "lsp_status_string", "lsp_version",
+    "lsp_status_string", "lsp_version", "lsp_periodogram_static",
 )
 
 _lib = None
@@ -65,6 +66,7 @@ def load(rebuild: bool = False):
     lib.lsp_periodogram_gls_weighted_batched.argtypes = [vp, vp, i64, vp, i64, vp, i64, i64, i64, dbl, dbl, i64,
                                                          vp, i64, vp, vp, vp]
     lib.lsp_false_alarm.argtypes = [vp, vp, i64, i64, dbl, vp, vp]
+    lib.lsp_periodogram_static.argtypes = [vp, vp, i64, dbl, dbl, i64, vp, vp, vp, vp]
     lib.lsp_reserve.argtypes = [vp, i64, ci, i64, i64, ci]
     lib.lsp_last_plan.argtypes = [vp, ctypes.POINTER(i64)]
     lib.lsp_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
@@ -101,6 +103,32 @@ def _stream_ptr(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
     return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def periodogram_static(t, x, f_min: float, df: float, Nf: int, out=None, peak_idx=None, peak_val=None, stream=None):
+    """lsp_periodogram_static: one series on the current device with no allocation inside the library (its workspace is a fixed
+    8 MiB device array; Nt <= 16,384, Nf <= 262,144, else LspError with status LSP_ELIMIT).  t float64[Nt], x float32[Nt] CUDA
+    tensors; `out` float32[Nf] and the optional int32[1] / float32[1] peak tensors are the caller's (pass them to keep this
+    call allocation-free on the Python side too).  Returns `out`."""
+    import torch
+    _want(t, torch.float64, 1, "t"); _want(x, torch.float32, 1, "x")
+    if t.shape != x.shape:
+        raise ValueError("t and x must have the same length")
+    P = out if out is not None else torch.empty(int(Nf), dtype=torch.float32, device=t.device)
+    _want(P, torch.float32, 1, "P")
+    if P.numel() < Nf:
+        raise ValueError("P too small")
+    if (peak_idx is None) != (peak_val is None):
+        raise ValueError("peak_idx and peak_val go together")
+    if peak_idx is not None:
+        _want(peak_idx, torch.int32, 1, "peak_idx"); _want(peak_val, torch.float32, 1, "peak_val")
+    with torch.cuda.device(t.device):
+        st = load().lsp_periodogram_static(t.data_ptr(), x.data_ptr(), t.numel(), float(f_min), float(df), int(Nf), P.data_ptr(),
+                                           peak_idx.data_ptr() if peak_idx is not None else None,
+                                           peak_val.data_ptr() if peak_val is not None else None, _stream_ptr(stream))
+    if st != LSP_OK:
+        raise LspError(st, "lsp_periodogram_static")
+    return P
 
 
 def plan_query(sm_count: int, B: int, Nt: int, Nf: int) -> dict:

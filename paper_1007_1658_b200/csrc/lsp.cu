@@ -19,6 +19,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <new>
 
 using namespace lsp;
@@ -989,6 +990,119 @@ int lsp_periodogram(lsp_handle h, const double* t, const float* x, int64_t Nt,
     return lsp_periodogram_batched(h, t, Nt, x, Nt, 1, Nt, f_min, df, Nf, P, Nf, nullptr, nullptr, stream);
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// lsp_periodogram_static: one series through the FP32-pipe form with NO allocation of any kind -- for callers that cannot call
+// cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).  The workspace the other entry points
+// keep in the handle's cudaMalloc'ed buffer (records, per-split partial sums, block partials, arg-max cell) lives instead in ONE
+// file-scope device array of LSP_STATIC_SCRATCH_BYTES, which every GPU that loads this library holds until the process exits.
+// In host code the array's NAME is only a host-side stand-in for the symbol, not a device address (a kernel given it would fault
+// or, where the GPU can reach host memory, silently use the wrong memory): its address is resolved once per device, with that
+// device current, by cudaGetSymbolAddress below, and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char lsp_static_scratch[LSP_STATIC_SCRATCH_BYTES];
+static_assert(LSP_STATIC_MAX_NT <= REFINE_INPLACE_MAX_NT, "the static entry point relies on finish_kernel refining in place");
+static_assert(2 * 16 * (int64_t)LSP_STATIC_MAX_NT + 4096 + 16 * (int64_t)LSP_STATIC_MAX_NF <= (int64_t)LSP_STATIC_SCRATCH_BYTES,
+              "the stated limits must fit the array with one time split");
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_ptr[STATIC_MAX_DEVICES] = {};      // device address of lsp_static_scratch on device i (0: not resolved yet)
+int g_static_sm[STATIC_MAX_DEVICES] = {};
+
+// set-up, once per device (the calling thread's current device): no allocation, no synchronisation
+int static_setup(int dev, unsigned char** ptr, int* sm_count)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        int major = 0, sms = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); return LSP_ECUDA; }
+        if (major < 10 || sms < 1) return LSP_ECUDA;       // sm_100a SASS only: fail loudly elsewhere
+        unsigned char* a = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&a, lsp_static_scratch);
+        if (e != cudaSuccess || !a) { cudaGetLastError(); return LSP_ECUDA; }
+        g_static_sm[dev] = sms;
+        g_static_ptr[dev] = a;
+    }
+    *ptr = g_static_ptr[dev]; *sm_count = g_static_sm[dev];
+    return LSP_OK;
+}
+}  // namespace
+
+int lsp_periodogram_static(const double* t, const float* x, int64_t Nt, double f_min, double df, int64_t Nf,
+                           float* P, int32_t* peak_idx, float* peak_val, void* stream)
+{
+    if (!t || !x || Nt < 2 || Nf < 1 || bad_grid(f_min, df)) return LSP_EINVAL;
+    if ((peak_idx == nullptr) != (peak_val == nullptr) || (!P && !peak_idx)) return LSP_EINVAL;
+    if (Nt > LSP_STATIC_MAX_NT || Nf > LSP_STATIC_MAX_NF) return LSP_ELIMIT;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return LSP_ECUDA; }
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return LSP_ELIMIT;
+    unsigned char* base = nullptr; int sm_count = 0;
+    int rc = static_setup(dev, &base, &sm_count);
+    if (rc != LSP_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+    // layout inside the array (every region is written in full by the call before it is read: nothing needs clearing but the
+    // arg-max cell and its counter, which the records kernel resets)
+    const int nparts = (int)((Nt + 511) / 512);                              // <= 32
+    const int64_t part_chunk = (Nt + nparts - 1) / nparts;
+    const size_t o_recA = 0;
+    const size_t o_recB = align_up(o_recA + (size_t)Nt * sizeof(float4), 256);
+    const size_t o_psum = align_up(o_recB + (size_t)Nt * sizeof(ulonglong2), 256);
+    const size_t o_pvar = align_up(o_psum + (size_t)nparts * sizeof(double), 256);
+    const size_t o_peak = align_up(o_pvar + (size_t)nparts * sizeof(double), 256);
+    const size_t o_cnt = o_peak + 256;
+    const size_t o_ws = o_cnt + 256;
+    // the plan of the FP32-pipe form (no tunables apply), with as many time splits as the array has room for
+    PlanOverrides ov;
+    ov.pipe = PLAN_PIPE_FP32;
+    PlanChoice pc = plan_choose_fp32(sm_count, 1, Nt, Nf, ov);
+    const int64_t room = ((int64_t)LSP_STATIC_SCRATCH_BYTES - (int64_t)o_ws) / (16 * Nf);   // whole [4][Nf] float blocks
+    if (room < 1) return LSP_ELIMIT;
+    for (int64_t cap = room; pc.K && pc.nsplit > room && cap >= 1; --cap) { ov.nsplit = cap; pc = plan_choose_fp32(sm_count, 1, Nt, Nf, ov); }
+    if (pc.K == 0 || pc.nsplit > room) return LSP_ELIMIT;
+    const KernelEntry* ke = find_kernel(pc.K);
+    if (!ke || pc.T < 32 || pc.T > ke->max_t || (pc.T % 32) != 0) return LSP_EINVAL;
+
+    float4* recA = reinterpret_cast<float4*>(base + o_recA);
+    ulonglong2* recB = reinterpret_cast<ulonglong2*>(base + o_recB);
+    double* psum = reinterpret_cast<double*>(base + o_psum);
+    double* pvar = reinterpret_cast<double*>(base + o_pvar);
+    u64* peak64 = reinterpret_cast<u64*>(base + o_peak);
+    unsigned* counter = reinterpret_cast<unsigned*>(base + o_cnt);
+    float* ws = reinterpret_cast<float*>(base + o_ws);
+
+    // steps 1-2 (the mean inside the records kernel: Nt <= 16,384; it also resets the arg-max cell and its counter)
+    records_kernel<false, true><<<dim3((unsigned)nparts, 1u), 256, 0, st>>>(t, Nt, x, Nt, Nt, part_chunk, f_min, df, psum, recA, recB, pvar,
+                                                                          peak64, counter, origin_offset(f_min, df, Nf), 1);
+    if (cudaGetLastError() != cudaSuccess) return LSP_ECUDA;
+    // steps 3-5
+    const int flush_tiles = (int)((2048 + TILE_Z - 1) / TILE_Z);
+    AccumParams ap;
+    ap.recW = nullptr; ap.recA = recA; ap.recB = recB; ap.ws = ws; ap.ws1 = nullptr; ap.Nt = Nt; ap.Nf = Nf;
+    ap.split_len = pc.split_len; ap.nsplit = pc.nsplit; ap.nfb = pc.nfb; ap.flush_tiles = flush_tiles;
+    const bool direct = pc.split_len <= (int64_t)flush_tiles * TILE_Z;
+    const size_t smem = accum_smem_bytes(ke, pc.T, false, direct);
+    const accum_fn fn = direct ? ke->fn_direct : ke->fn;
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return LSP_ECUDA; }
+    fn<<<(unsigned)((int64_t)pc.nsplit * pc.nfb), pc.T, smem, st>>>(ap);
+    if (cudaGetLastError() != cudaSuccess) return LSP_ECUDA;
+    // steps 6-7; ill-conditioned frequencies are redone in fp64 inside finish_kernel (Nt <= 16,384: no list, no further kernel)
+    FinishParams fp;
+    fp.ws = ws; fp.part_var = pvar; fp.P = P; fp.p_stride = Nf;
+    fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
+    fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = pc.nsplit; fp.nparts = nparts;
+    fp.x_scaled = 0; fp.ws1 = nullptr; fp.ws_x = nullptr; fp.x_row = 0;
+    fp.src.t = t; fp.src.t_stride = Nt; fp.src.x = x; fp.src.x_stride = Nt; fp.src.w = nullptr; fp.src.w_stride = 0;
+    fp.src.f_min = f_min; fp.src.df = df; fp.src.Nt = Nt;
+    fp.refine_amp = refine_amplification(false, Nt, false);
+    fp.list = RefineList{};
+    launch_finish(fp, 1, st);
+    if (cudaGetLastError() != cudaSuccess) return LSP_ECUDA;
+    return LSP_OK;
+}
+
 int lsp_periodogram_batched_host(lsp_handle h, const double* t, int share_t, const float* x,
                                  int64_t B, int64_t Nt, double f_min, double df, int64_t Nf,
                                  float* P, int32_t* peak_idx, float* peak_val, void* stream)
@@ -1142,6 +1256,7 @@ const char* lsp_status_string(int status)
         case LSP_EINVAL: return "invalid argument";
         case LSP_ECUDA:  return "CUDA runtime error (or no sm_100 device)";
         case LSP_ENOMEM: return "device workspace allocation failed";
+        case LSP_ELIMIT: return "size beyond the fixed limits of lsp_periodogram_static (Nt <= 16,384, Nf <= 262,144)";
         default:         return "unknown status";
     }
 }

@@ -649,6 +649,84 @@ def run_back_to_back(args):
     return 0
 
 
+def run_variants(args):
+    """SURVEY.md section 8(f) row 1 beside the classical periodogram, same workload, same protocol: whole-call device time (CUDA
+    events, L2 flushed between calls) of lsp_periodogram, lsp_periodogram_gls and lsp_periodogram_gls_weighted in the FP32-pipe
+    form and under the automatic plan, each checked against ITS oracle function on sampled series; for a single series within its
+    limits also lsp_periodogram_static.  One JSON line."""
+    import torch
+    import paper_1007_1658_b200 as lsp
+    import oracle
+    w = workloads.make(args.workload)
+    batched = w.B > 1
+    t2 = np.ascontiguousarray(w.t if w.t.ndim == 2 or not batched else np.broadcast_to(w.t, w.x.shape)).reshape(w.B, -1) if batched else w.t.reshape(1, -1)
+    x2 = np.ascontiguousarray(w.x).reshape(w.B, -1)
+    wts = np.random.default_rng(20100716).uniform(0.2, 3.0, x2.shape).astype(np.float32)      # heteroscedastic weights 1 / sigma^2
+    t_d = torch.from_numpy(np.ascontiguousarray(w.t)).cuda()
+    x_d = torch.from_numpy(np.ascontiguousarray(w.x)).cuda()
+    w_d = torch.from_numpy(wts if batched else wts[0]).cuda()
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    h = lsp.Handle(0)
+    sample = sorted(set([0, w.B // 2, w.B - 1]))
+    ks = np.unique(np.linspace(0, w.Nf - 1, min(w.Nf, 2048)).astype(np.int64))
+    refs = {}
+
+    def ref_of(kind, b):
+        if (kind, b) not in refs:
+            tb, xb = t2[b if t2.shape[0] > 1 else 0], x2[b]
+            if kind == "classical":
+                refs[(kind, b)] = oracle.periodogram(tb, xb, w.f_min, w.df, w.Nf, ks=ks)
+            elif kind == "generalised":
+                refs[(kind, b)] = oracle.periodogram_gls(tb, xb, w.f_min, w.df, w.Nf, ks=ks)
+            else:
+                refs[(kind, b)] = oracle.periodogram_gls_weighted(tb, xb, wts[b], w.f_min, w.df, w.Nf, ks=ks)
+        return refs[(kind, b)]
+
+    def call(kind):
+        gls = kind != "classical"
+        wt = w_d if kind == "weighted" else None
+        if batched:
+            return h.periodogram_batched(t_d, x_d, w.f_min, w.df, w.Nf, gls=gls, weights=wt)[0]
+        return h.periodogram(t_d, x_d, w.f_min, w.df, w.Nf, gls=gls, weights=wt).reshape(1, -1)
+
+    def timed(fn):
+        for _ in range(3):
+            P = fn()
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(max(5, args.steps)):
+            flush_buf.zero_()
+            ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ea.record(); P = fn(); eb.record()
+            torch.cuda.synchronize()
+            ms.append(ea.elapsed_time(eb))
+        return statistics.median(ms), P
+
+    rows = []
+    for pipe, form in ((lsp.PIPE_FP32, "FP32 pipe"), (0, "automatic")):
+        h.set_param(lsp.PARAM_PIPE, pipe)
+        for kind in ("classical", "generalised", "weighted"):
+            ms, P = timed(lambda: call(kind))
+            plan = h.last_plan()
+            Pn = P.cpu().numpy()
+            err = max(float(np.max(np.abs(Pn[b][ks] - ref_of(kind, b))) / np.max(ref_of(kind, b))) for b in sample)
+            rows.append({"form": form, "periodogram": kind, "ms": ms, "terms_per_s": w.terms / (ms * 1e-3), "kernel": plan["kernel"],
+                         "launches": plan["launches"], "max_rel_err_vs_oracle": err, "series_checked": len(sample), "frequencies_checked": int(ks.size)})
+    if not batched and w.Nt <= lsp.STATIC_MAX_NT and w.Nf <= lsp.STATIC_MAX_NF:
+        P_s = torch.empty(w.Nf, dtype=torch.float32, device="cuda")
+        ms, P = timed(lambda: lsp.periodogram_static(t_d, x_d, w.f_min, w.df, w.Nf, out=P_s).reshape(1, -1))
+        err = float(np.max(np.abs(P.cpu().numpy()[0][ks] - ref_of("classical", 0))) / np.max(ref_of("classical", 0)))
+        rows.append({"form": "FP32 pipe, lsp_periodogram_static (no allocation)", "periodogram": "classical", "ms": ms,
+                     "terms_per_s": w.terms / (ms * 1e-3), "kernel": "accum_z_kernel", "launches": 3, "max_rel_err_vs_oracle": err,
+                     "series_checked": 1, "frequencies_checked": int(ks.size)})
+    h.close()
+    print(json.dumps({"metric": "lomb_scargle_variants_ms", "workload": w.name, "unit": "ms per call", "data": "synthetic",
+                      "config": {"workload": w.name, "series": w.B, "Nt": w.Nt, "Nf": w.Nf, "l2_flush_between_calls": True},
+                      "tolerance": 1e-4, "rows": rows,
+                      "note": "whole-call device time (median); weights U[0.2, 3) per sample; each row checked against its own oracle function on a strided frequency subset, the error relative to the largest SAMPLED oracle value (<= max P: conservative)"}))
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -672,6 +750,8 @@ def main(argv=None):
     ap.add_argument("--sweep", action="store_true", help="N_t scaling sweep of --workload (single series) instead of the bench line")
     ap.add_argument("--back-to-back", type=int, default=0, dest="back_to_back",
                     help="N back-to-back calls of --workload (single series), eager and as a replayed CUDA graph, instead of the bench line")
+    ap.add_argument("--variants", action="store_true",
+                    help="time the classical, generalised and weighted periodograms (and the no-allocation entry point) on --workload instead of the bench line")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
@@ -681,6 +761,8 @@ def main(argv=None):
         return run_sweep(args)
     if args.back_to_back:
         return run_back_to_back(args)
+    if args.variants:
+        return run_variants(args)
     return run_ours(args)
 
 

@@ -113,15 +113,16 @@ int ensure(lsp_ctx* h, void** ptr, size_t* have, size_t need) {
 
 typedef void (*accum_fn)(const AccumParams);
 
-struct KernelEntry { int K; accum_fn fn, fn_weighted, fn_direct, fn_gls, fn_gls_weighted; const char* name; const char* name_weighted;
+struct KernelEntry { int K; accum_fn fn, fn_weighted, fn_direct, fn_gls, fn_gls_weighted, fn_gls_direct; const char* name; const char* name_weighted;
                      const char* name_gls; const char* name_gls_weighted; int max_t; };
 
 constexpr int GLS_FUSED_MAX_K = 20;       // FP32 form, generalised periodogram in one pass (accum_z_kernel<..., GLS>): 2 K more registers per thread
 #define LSP_ENTRY_Z(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, accum_z_kernel<K, MAXT, MINB, true>, accum_z_kernel<K, MAXT, MINB, false, true>, \
-                                     nullptr, nullptr, \
+                                     nullptr, nullptr, nullptr, \
                                      "accum_z_kernel<K=" #K ",fp32,three-term>", "accum_z_kernel<K=" #K ",fp32,three-term,weighted>", "", "", MAXT }
 #define LSP_ENTRY_ZG(K, MAXT, MINB) { K, accum_z_kernel<K, MAXT, MINB>, accum_z_kernel<K, MAXT, MINB, true>, accum_z_kernel<K, MAXT, MINB, false, true>, \
                                      accum_z_kernel<K, MAXT, MINB, false, false, true>, accum_z_kernel<K, MAXT, MINB, true, false, true>, \
+                                     accum_z_kernel<K, MAXT, MINB, false, true, true>, \
                                      "accum_z_kernel<K=" #K ",fp32,three-term>", "accum_z_kernel<K=" #K ",fp32,three-term,weighted>", \
                                      "accum_z_kernel<K=" #K ",fp32,three-term,generalised one-pass>", "accum_z_kernel<K=" #K ",fp32,three-term,generalised one-pass,weighted>", MAXT }
 const KernelEntry g_kernels[] = {
@@ -658,9 +659,9 @@ int run_device(lsp_ctx* h,
                 ap.recA = rA; ap.recB = recB; ap.ws = wsp; ap.ws1 = ws1; ap.Nt = Nt; ap.Nf = Nf;
                 ap.split_len = pl.split_len; ap.nsplit = pl.nsplit; ap.nfb = pl.nfb; ap.flush_tiles = pl.flush_tiles;
                 // the whole split inside one fold interval: the register partials go straight to `ws` (no shared-memory accumulators)
-                const bool direct = !weighted && !r.gls_fused && pl.split_len <= (int64_t)pl.flush_tiles * TILE_Z;
+                const bool direct = !weighted && pl.split_len <= (int64_t)pl.flush_tiles * TILE_Z;
                 const size_t smem = accum_smem_bytes(ke, pl.T, weighted, direct, r.gls_fused);
-                const accum_fn fn = r.gls_fused ? (weighted ? ke->fn_gls_weighted : ke->fn_gls)
+                const accum_fn fn = r.gls_fused ? (weighted ? ke->fn_gls_weighted : (direct ? ke->fn_gls_direct : ke->fn_gls))
                                                 : (weighted ? ke->fn_weighted : (direct ? ke->fn_direct : ke->fn));
                 LSP_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                 fn<<<(unsigned)units, pl.T, smem, st>>>(ap);
@@ -688,7 +689,9 @@ int run_device(lsp_ctx* h,
     fp.ws_x = nullptr; fp.x_row = 0;
     fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt, gls) : 0.0;
     fp.list = RefineList{};
-    const bool listed = refine && Nt > REFINE_INPLACE_MAX_NT;
+    // generalised form: its flagged frequencies come in runs (every alias of a nightly cadence), which one finish block would redo one
+    // after the other: always through the list, a block or warp per frequency (C2-shaped call: steps 6-7 0.053 -> 0.02 ms)
+    const bool listed = refine && (Nt > REFINE_INPLACE_MAX_NT || gls);
     if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }
     launch_finish(fp, B, st, pdl_small);
     LSP_CUDA(h, cudaGetLastError());

@@ -751,7 +751,7 @@ def test_generalised_periodogram(lsp, prm):
         assert plan["pipe"] == prm["pipe"]
     if prm.get("pipe") == FP32:                             # one pass with a third accumulator per frequency up to K = 20; two passes beyond
         assert ("generalised one-pass" in plan["kernel"]) == (prm.get("K", 0) <= 20), plan
-        assert plan["launches"] == (3 if prm.get("K", 0) <= 20 else 5), plan      # records (mean fused), accumulate, finish (+ unit records, second pass)
+        assert plan["launches"] == (4 if prm.get("K", 0) <= 20 else 6), plan      # records (mean fused), accumulate, finish, refine_kernel (+ unit records, second pass)
 
 
 def test_generalised_periodogram_long_grid(lsp):

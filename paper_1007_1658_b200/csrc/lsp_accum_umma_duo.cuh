@@ -324,11 +324,19 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             {
                 const float4* ra = rec_a + buf * UM_TS + sb;
                 const float* rw = recw_a + buf * UM_TS + sb;
+#ifndef LSP_UD_DBG_NOA
                 if (left >= 4) um_gen_a<false, WEIGHTED>(ra, 0, a_h, a_dst + st_off, 4, rw);  // `left` is warp-uniform
                 else um_gen_a<true, WEIGHTED>(ra, 0, a_h, a_dst + st_off, max(0, left), rw);
+#else
+                (void)ra; (void)rw;
+#endif
             }
+#ifndef LSP_UD_DBG_NOB
             if (((unsigned)ks & 1u) == b_par) ud_gen_b(rec_b + buf * UM_TS + sb, 0, b_l, b_dst + st_off);
+#endif
+#ifndef LSP_UD_DBG_NOFENCE
             fence_proxy_async();                                                // generic-proxy stores -> visible to the tensor core
+#endif
             __syncwarp();
             if (lane == 0) mbar_arrive(UD_FULL(s));
             left -= UM_KS;
@@ -367,10 +375,14 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             const uint64_t dAv = umma_desc(a0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
             const uint64_t dBh = umma_desc(b0, UM_A_BYTES / 2, 128), dBl = umma_desc(b0 + UM_A_BYTES, UM_A_BYTES / 2, 128);
             const uint64_t dBv = umma_desc(b0 + 2 * UM_A_BYTES, UM_A_BYTES / 2, 128);
+#ifndef LSP_UD_DBG_NOMMA
             tc_mma_f16(tmem, dAh, dBh, UD_IDESC, kin > 0 ? 1u : 0u);
             tc_mma_f16(tmem, dAl, dBh, UD_IDESC, 1u);
             tc_mma_f16(tmem, dAh, dBl, UD_IDESC, 1u);
             tc_mma_f16(tmem + 128u, dAv, dBv, UD_IDESC, ks > 0 ? 1u : 0u);
+#else
+            (void)dAh; (void)dAl; (void)dAv; (void)dBh; (void)dBl; (void)dBv;
+#endif
             tc_commit(UD_EMPTY(s));
             const bool last = (ks == nks - 1);
             if (++kin == flush_ksteps || last) {

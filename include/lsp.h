@@ -71,7 +71,7 @@ enum {
     LSP_PARAM_THREADS   = 2,  /* FP32 form: threads per CTA: 32..256 (multiple of 32; <= 128 for K >= 28) */
     LSP_PARAM_NSPLIT    = 3,  /* number of time-axis splits per (series, frequency block) */
     LSP_PARAM_PIPE      = 4,  /* LSP_PIPE_FP32 or LSP_PIPE_TENSOR (see above) */
-    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the fp32 partial sums / drains of the TMEM accumulators (default 2,048; CTA-pair form 8,192) */
+    LSP_PARAM_FLUSH     = 5,  /* samples between folds of the fp32 partial sums / drains of the TMEM accumulators (default 2,048; CTA-pair form 4,096) */
     LSP_PARAM_TIMING    = 6,  /* 1 = record CUDA events around each kernel of a call (see lsp_last_timing) */
     LSP_PARAM_TABLE_MB  = 7,  /* tensor form, CTA-pair kernel: MiB of workspace its operand table may take (default 1,024);  */
                               /* a series whose table (3 KB per sample) is larger runs in time chunks, same result             */

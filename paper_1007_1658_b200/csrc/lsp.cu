@@ -567,10 +567,10 @@ int run_device(lsp_ctx* h,
     const int npass = (gls && !r.gls_fused) ? 2 : 1;
     // short grids, one pass: records -> accumulate -> finish as programmatic dependents (launch latency and CTA set-up overlap the predecessor's tail)
     const bool pdl_small = r.small && !r.duo && !gls && h->opt_pdl != 1;
-    // drain interval of D_W: 2,048 samples; 8,192 in the CTA-pair form, where a drain stalls the whole pipeline of the pair (5 % faster
-    // than 2,048).  The expected truncation loss of a window is added back at its drain (tc_trunc_comp): worst adversarial case
-    // 2.3e-6 of max P at 8,192 samples
-    const int64_t flush_default = r.pair ? 8192 : 2048;
+    // drain interval of D_W and D_V: 2,048 samples; 4,096 in the CTA-pair form, where a drain stalls the whole pipeline of the pair
+    // (2,048 / 4,096 / 8,192: 21.6 / 20.5 / 20.2 ms at C5).  The expected truncation loss of a D_W window is added back at its drain
+    // (tc_trunc_comp); on series with a trend the model is only approximate and the residual grows with the window
+    const int64_t flush_default = r.pair ? 4096 : 2048;
     const int flush_ksteps = (int)(((h->opt_flush ? h->opt_flush : flush_default) + UM_KS - 1) / UM_KS);
     if (r.pair) {
         // CTA-pair form, one time chunk at a time: table pre-pass, then the accumulate launch(es) that read it
@@ -687,7 +687,7 @@ int run_device(lsp_ctx* h,
     fp.x_scaled = tensor ? 1 : 0;
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
-    fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt, gls) : 0.0;
+    fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt, gls, r.pair) : 0.0;
     fp.list = RefineList{};
     // generalised form: its flagged frequencies come in runs (every alias of a nightly cadence), which one finish block would redo one
     // after the other: always through the list, a block or warp per frequency (C2-shaped call: steps 6-7 0.053 -> 0.02 ms)

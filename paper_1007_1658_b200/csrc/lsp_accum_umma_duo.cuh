@@ -354,7 +354,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
                 const float nk = (float)(ks - ks_begin);                // k-steps of this window
                 ud_drain(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, d_live, p.trunc_ulps < 0.f ? nk : 0.f,
                          0.6366198f / (16.f * nk * (p.unit_x ? TC_MEAN_ABS_COS : TC_MEAN_ABS_PRODUCT)));
-                if (last) ud_drain(t_drain + 128u, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true, d_live);
+                ud_drain(t_drain + 128u, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, flushes == 0, d_live);   // D_V with D_W (see lsp_accum_umma_small.cuh)
                 }
                 tc_fence_before();
                 __syncwarp();
@@ -379,7 +379,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             tc_mma_f16(tmem, dAh, dBh, UD_IDESC, kin > 0 ? 1u : 0u);
             tc_mma_f16(tmem, dAl, dBh, UD_IDESC, 1u);
             tc_mma_f16(tmem, dAh, dBl, UD_IDESC, 1u);
-            tc_mma_f16(tmem + 128u, dAv, dBv, UD_IDESC, ks > 0 ? 1u : 0u);
+            tc_mma_f16(tmem + 128u, dAv, dBv, UD_IDESC, kin > 0 ? 1u : 0u);
 #else
             (void)dAh; (void)dAl; (void)dAv; (void)dBh; (void)dBl; (void)dBv;
 #endif

@@ -340,7 +340,11 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                 u2_drain64(t_drain, ws_unit + (int64_t)(cg & 1u) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, p.trunc_ulps, nk,
                            CORR16 ? 1.125f : 0.75f, 0.6366198f / (16.f * nk * mean_abs_product));
             }
-            if (last && !p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, !q.accumulate, 0.f, 0.f, 0.f, 0.f);
+            // D_V is drained with D_W (round 2): left to accumulate over the whole split it lost ~n ulp toward zero wherever sum e^{2i theta}
+            // is coherent (f T < ~1, aliases of regular sampling, any series with a trend), an error that grew with the split length and
+            // that Nt / (Nt - R) amplifies (found by a randomised sweep on series with a drift: up to 1e-3 of max P)
+            if (!p.unit_x) u2_drain64(t_drain + 256u, ws_unit + (int64_t)(2 + (cg & 1u)) * p.Nf, k0, p.Nf, f == 0 && !q.accumulate, 0.f, 0.f, 0.f, 0.f);
+            (void)last;
             tc_fence_before();
             __syncwarp();
             if (lane == 0) { if (rank == 0) mbar_arrive(bar_acce); else mbar_arrive_remote(bar_acce, 0u); }
@@ -370,7 +374,7 @@ __global__ void __launch_bounds__(U2_THREADS, 1) accum_umma_pair2_kernel(const U
                     tc_mma_f16_pair(tmem, dTh, dG8, UP_IDESC, 1u);
                 } else tc_mma_f8_pair(tmem, dT8, dG8, UP_IDESC_F8, 1u);
                 if (!p.unit_x)                                          // (the unit-weight pass of the generalised periodogram needs no V: CC, CS come from the first pass)
-                    tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (it > 0 || kk > 0) ? 1u : 0u);
+                    tc_mma_f16_pair(tmem + 256u, dTv, dGv, UP_IDESC, (!win_first || kk > 0) ? 1u : 0u);
 #else
                 (void)dTh; (void)dGh; (void)dT8; (void)dG8; (void)dTv; (void)dGv; (void)win_first;
 #endif

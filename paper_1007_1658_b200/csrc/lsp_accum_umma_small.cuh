@@ -285,7 +285,8 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
                     us_drain<L>(t_drain, ws_unit + (int64_t)part * p.Nf, k0, p.Nf, flushes == 0, p.trunc_ulps < 0.f ? nk : 0.f,
                                 0.6366198f / (16.f * nk * (p.unit_x ? TC_MEAN_ABS_COS : TC_MEAN_ABS_PRODUCT)));
                 }
-                if (last) us_drain<L>(t_drain + 2u * L, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, true);
+                // D_V is drained with D_W: left to accumulate over the whole split it loses ~n ulp toward zero where sum e^{2i theta} is coherent
+                us_drain<L>(t_drain + 2u * L, ws_unit + (int64_t)(2 + part) * p.Nf, k0, p.Nf, flushes == 0);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_acce);
@@ -308,7 +309,7 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
             tc_mma_f16(tmem, dAh, dBh, C::IDESC, kin > 0 ? 1u : 0u);
             tc_mma_f16(tmem, dAl, dBh, C::IDESC, 1u);
             tc_mma_f16(tmem, dAh, dBl, C::IDESC, 1u);
-            tc_mma_f16(tmem + 2u * L, dAv, dBv, C::IDESC, ks > 0 ? 1u : 0u);
+            tc_mma_f16(tmem + 2u * L, dAv, dBv, C::IDESC, kin > 0 ? 1u : 0u);
             tc_commit(US_EMPTY(s));
             const bool last = (ks == nks - 1);
             if (++kin == flush_ksteps || last) {

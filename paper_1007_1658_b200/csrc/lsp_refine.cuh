@@ -17,24 +17,27 @@
 namespace lsp {
 
 // Which frequencies: those where the rounding of the sums is amplified by more than `amp`, the amplification being
-// Nt / (Nt - R) for eq. (5) and (1/4) / D for the generalised form's determinant D <= 1/4.  The FP32-pipe form's sums are good to
-// 1e-7 ... 6e-6 of Nt (the three-term recurrence over K = 32 frequencies at tiny Nt is the upper end), so amp = 5 (R > 0.8 Nt)
-// keeps every bin within ~3e-5.  The tensor-core forms sum cos 2 theta, sin 2 theta from a single fp16 pass, good to
-// ~5e-4 / sqrt(Nt) of Nt: for 3e-5 the amplification may be 0.06 sqrt(Nt) at most -- R > 0.26 Nt at Nt = 512,
-// R > 0.83 Nt at 10,000, capped at 10 (R > 0.9 Nt) from 28,000 samples on.  (In a periodogram of noise R / Nt ~ sqrt(ln Nf / Nt):
-// 0.12 at Nt = 512.  Only f T < ~0.4 and aliases get there -- and tiny series, where a refinement costs next to nothing.)
-// The generalised form is more delicate (its numerator cancels along with the determinant; measured 1e-4 of max P at D ~ 0.02 on
-// fp32 sums): amplification 5 (D < 0.05) for the FP32-pipe form, 2.5 ... 5 for the tensor-core forms.
-__host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt, bool gls = false)
+// Nt / (Nt - R) for eq. (5) and (1/4) / D for the generalised form's determinant D <= 1/4 (D ~ (1 - (R/Nt)^2) / 4).
+// FP32-pipe form: its sums are good to 1e-7 ... 6e-6 of Nt (the three-term recurrence over K = 32 frequencies at tiny Nt is the
+// upper end), so amp = 5 (R > 0.8 Nt) keeps every bin within ~3e-5.
+// Tensor-core forms: two error sources grow with R.  (i) sum cos 2 theta, sin 2 theta come from a single fp16 pass, good to
+// ~5e-4 / sqrt(Nt) of Nt: amp <= 0.06 sqrt(Nt) (R > 0.26 Nt at Nt = 512).  (ii) Where the sums are COHERENT -- f T < ~1, aliases of
+// regular sampling, and above all series with a trend, whose low-frequency power is the largest on the grid -- the tensor core's
+// round-toward-zero accumulation is a bias that the compensation model (tc_trunc_comp) removes only in part; measured on series
+// with a drift of 1 ... 3 sigma over the span (refinement off, error in units of max P): <= 5e-5 below R = 0.6 Nt and 1.4e-4 above
+// for the short-grid and batch kernels (2,048-sample drain windows); <= 4e-5 ... 9.5e-5 below R = 0.45 Nt and 1.5e-4 ... 2e-4 above
+// for the CTA-pair kernel (4,096-sample windows); with long forced splits the short-grid kernel reached 8.8e-5 below 0.6 Nt too.
+// Hence R > 0.45 Nt (amp 1.82) at the latest, for all of them.
+// (In a periodogram of noise R / Nt ~ sqrt(ln Nf / Nt): 0.12 at Nt = 512.  Only f T < ~0.5 and aliases get there.)
+__host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt, bool gls = false, bool pair = false)
 {
-    if (gls) {
-        if (!tensor) return 5.0;
-        const double a = 0.03 * sqrt((double)Nt);
-        return a < 2.5 ? 2.5 : (a > 5.0 ? 5.0 : a);
-    }
     if (!tensor) return 5.0;
-    const double a = 0.06 * sqrt((double)Nt);
-    return a < 1.35 ? 1.35 : (a > 10.0 ? 10.0 : a);
+    const double cap = 1.82; (void)pair;
+    double a = 0.06 * sqrt((double)Nt);
+    a = a < 1.35 ? 1.35 : (a > cap ? cap : a);
+    if (!gls) return a;
+    const double r = 1.0 - 1.0 / a;                                    // the same R / Nt, as a bound on the determinant
+    return 1.0 / (1.0 - r * r);
 }
 
 constexpr int REFINE_THREADS = 256;

@@ -89,3 +89,72 @@ def test_random_calls_match_the_oracle(lsp, seed):
                 assert int(pi[b]) == int(np.argmax(P[b])) and float(pv[b]) == float(P[b].max()), desc
     print("seed %d: worst error at the 1e-4 tolerance %.2e in %s; forms run: %s" % (seed, worst_overall, worst_desc, sorted(forms)))
     assert len(forms) >= 5
+
+
+def test_random_medium_calls_match_the_oracle_on_samples(lsp):
+    """The same idea at sizes where the long-grid kernels run (Nt 20,000 ... 250,001, Nf up to 2e6; time chunks of the table, drain
+    windows, forced time splits, the fp16 hi + lo corrections; regular and random sampling; half of the series with a drift, whose
+    coherent low-frequency sums found the weaknesses documented in tests/test_gpu_refine.py::test_series_with_a_trend): compared
+    with the oracle on the first and last 40 bins, 300 random bins and +-20 bins around the GPU's peak of every series."""
+    import torch
+    pkg, h = lsp
+    rng = np.random.default_rng(2024)
+    worst_overall, worst_desc = 0.0, ""
+    for case in range(40):
+        B = int(rng.choice([1, 1, 1, 2, 3, 5]))
+        Nt = int(rng.choice([20000, 33333, 65537, 100000, 131072, 250001]))
+        Nf = int(rng.choice([10000, 65536, 65537, 200000, 1000003, 2000000]))
+        if B * Nt * Nf > 3e11:
+            Nf = int(3e11 / (B * Nt))
+        shared = bool(rng.integers(0, 2)) and B > 1
+        gls = bool(rng.integers(0, 3) == 0)
+        weighted = gls and bool(rng.integers(0, 2))
+        even = bool(rng.integers(0, 4) == 0)
+        span = float(rng.choice([100.0, 1000.0, 5000.0]))
+        nt_rows = 1 if shared else B
+        if even:
+            tt = np.broadcast_to(np.arange(Nt) * (span / Nt), (nt_rows, Nt)) + rng.uniform(0, 1e-6, (nt_rows, Nt))
+        else:
+            tt = rng.uniform(0, span, (nt_rows, Nt))
+        tt = np.sort(tt, axis=1)
+        tfull = np.broadcast_to(tt, (B, Nt)) if shared else tt
+        x = (rng.standard_normal((B, Nt)) + 0.1 * np.sin(2 * np.pi * 0.37 * tfull) + float(rng.choice([0.0, 1.0])) * tfull / span).astype(np.float32)
+        f_min = float(rng.choice([0.0, 1.0 / span, 0.013]))
+        f_max = float(rng.choice([1.0, 5.0, Nt / span / 2, Nt / span]))
+        df = (f_max - f_min) / (Nf - 1)
+        w = rng.uniform(0.2, 3.0, (B, Nt)).astype(np.float32) if weighted else None
+        prm = {pkg.PARAM_PIPE: int(rng.choice([0, 0, 1, 2])), pkg.PARAM_TABLE_MB: int(rng.choice([0, 0, 64, 200])),
+               pkg.PARAM_FLUSH: int(rng.choice([0, 0, 1024, 4096, 5000])), pkg.PARAM_NSPLIT: int(rng.choice([0, 0, 0, 3, 7])),
+               pkg.PARAM_CORR: int(rng.choice([0, 0, 1]))}
+        desc = "case %d: B=%d Nt=%d Nf=%d shared=%s gls=%s weighted=%s even=%s f_min=%g f_max=%g params=%s" % (
+            case, B, Nt, Nf, shared, gls, weighted, even, f_min, f_max, list(prm.values()))
+        for k, v in prm.items():
+            h.set_param(k, v)
+        try:
+            td = torch.from_numpy(np.ascontiguousarray(tt[0] if shared else tt)).cuda()
+            xd = torch.from_numpy(x).cuda()
+            wd = torch.from_numpy(w).cuda() if weighted else None
+            P, pi, pv = h.periodogram_batched(td, xd, f_min, df, Nf, gls=gls, weights=wd)
+            P, pi = P.cpu().numpy(), pi.cpu().numpy()
+            torch.cuda.synchronize()
+            plan = h.last_plan()
+        finally:
+            for k in prm:
+                h.set_param(k, 0)
+        assert np.all(np.isfinite(P)), desc
+        for b in range(B):
+            pk = int(np.argmax(P[b]))
+            assert int(pi[b]) == pk, desc
+            ks = np.unique(np.concatenate([np.arange(0, min(Nf, 40)), np.arange(max(0, Nf - 40), Nf), rng.integers(0, Nf, 300),
+                                           np.arange(max(0, pk - 20), min(Nf, pk + 21))])).astype(np.int64)
+            if weighted:
+                ref = oracle.periodogram_gls_weighted(tfull[b], x[b], w[b], f_min, df, Nf, ks=ks)
+            elif gls:
+                ref = oracle.periodogram_gls(tfull[b], x[b], f_min, df, Nf, ks=ks)
+            else:
+                ref = oracle.periodogram(tfull[b], x[b], f_min, df, Nf, ks=ks)
+            err = float(np.max(np.abs(P[b][ks] - ref))) / max(float(P[b].max()), float(ref.max()))
+            if err > worst_overall:
+                worst_overall, worst_desc = err, "%s (%s)" % (desc, plan["kernel"])
+            assert err <= 1e-4, "%s series %d (%s): %.2e" % (desc, b, plan["kernel"], err)
+    print("worst error %.2e in %s" % (worst_overall, worst_desc))

@@ -167,7 +167,9 @@ Plan make_plan(const lsp_ctx* h, int64_t B, int64_t Nt, int64_t Nf, int64_t tabl
 }
 
 // ---- workspace layouts (byte offsets into the handle's buffer)
-constexpr int64_t REFINE_INPLACE_MAX_NT = 16384;        // longer series: finish_kernel lists its ill-conditioned frequencies for refine_kernel (lsp_refine.cuh)
+constexpr int64_t REFINE_INPLACE_MAX_NT = 16384;        // lsp_periodogram_static: finish_kernel redoes its ill-conditioned frequencies itself up to this length
+constexpr int64_t REFINE_LIST_MIN_NT = 2048;            // handle paths: longer series list them for refine_kernel (lsp_refine.cuh): flagged bins come in runs
+                                                        // (low f, every alias of a nightly cadence) that one finish block would redo one after the other (C2: +21 us)
 constexpr int64_t SHARED_E_BUDGET_DEFAULT = (int64_t)256 << 20;   // bytes of workspace the E tiles of the shared-time GEMM may take (per band)
 
 struct SharedLayout {
@@ -416,7 +418,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
     fp.src = src; fp.refine_amp = amp;
     fp.list = RefineList{};
-    const bool listed = refine && Nt > REFINE_INPLACE_MAX_NT;
+    const bool listed = refine && Nt > REFINE_LIST_MIN_NT;
     if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }
     launch_finish(fp, B, st);
     LSP_CUDA(h, cudaGetLastError());
@@ -622,7 +624,7 @@ int run_device(lsp_ctx* h,
                 up.split_len = pl.split_len; up.nsplit = pl.nsplit; up.nfb = pl.nfb; up.nparts = pl.nparts;
                 up.flush_ksteps = flush_ksteps; up.trunc_ulps = h->opt_trunc == 1 ? 0.f : -1.f; up.unit_x = pass;   // (the model, or none: LSP_PARAM_TRUNC = 1)
                 up.t = t; up.t_stride = t_stride; up.x = x; up.x_stride = x_stride; up.f_min = f_min; up.df = df;
-                up.part_var_out = pvar; up.peak64 = peak64; up.counter = counter;
+                up.part_var_out = pvar; up.part_sum_out = psum; up.peak64 = peak64; up.counter = counter;
                 if (r.duo) {
                     UmmaDuoParams dp;
                     dp.u = up; dp.B = B;
@@ -691,7 +693,7 @@ int run_device(lsp_ctx* h,
     fp.list = RefineList{};
     // generalised form: its flagged frequencies come in runs (every alias of a nightly cadence), which one finish block would redo one
     // after the other: always through the list, a block or warp per frequency (C2-shaped call: steps 6-7 0.053 -> 0.02 ms)
-    const bool listed = refine && (Nt > REFINE_INPLACE_MAX_NT || gls);
+    const bool listed = refine && (Nt > REFINE_LIST_MIN_NT || gls);
     if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }
     launch_finish(fp, B, st, pdl_small);
     LSP_CUDA(h, cudaGetLastError());

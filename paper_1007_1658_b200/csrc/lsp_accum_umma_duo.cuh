@@ -240,7 +240,8 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             for (int o = 16; o > 0; o >>= 1) a0 += __shfl_down_sync(0xffffffffu, a0, o);
             if (lane == 0) red[w] = a0;
             asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
-            mean = (((red[4 * ls] + red[4 * ls + 1]) + red[4 * ls + 2]) + red[4 * ls + 3]) / (double)p.Nt;   // fixed order
+            const double sum_x = ((red[4 * ls] + red[4 * ls + 1]) + red[4 * ls + 2]) + red[4 * ls + 3];      // fixed order
+            mean = sum_x / (double)p.Nt;
             asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
             double a1 = 0.0;
             for (int64_t j = lj; j < p.Nt; j += 128) { const double d = (double)__ldg(xb + j) - mean; a1 += d * d; }
@@ -250,7 +251,7 @@ __global__ void __launch_bounds__(US_THREADS, 2) accum_umma_duo_kernel(const Umm
             asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");
             const double q2 = ((red[4 * ls] + red[4 * ls + 1]) + red[4 * ls + 2]) + red[4 * ls + 3];
             asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");   // `red` is the record tiles from here on
-            if (lj == 0 && l_live && sp == 0 && fb == 0) { p.part_var_out[lb] = q2; p.peak64[lb] = 0ull; p.counter[lb] = 0u; }
+            if (lj == 0 && l_live && sp == 0 && fb == 0) { p.part_var_out[lb] = q2; p.part_sum_out[lb] = sum_x; p.peak64[lb] = 0ull; p.counter[lb] = 0u; }
             xs = l_live ? x_scale(&q2, 1, p.Nt) : 0.f;                            // steps 6-7 recompute exactly this from part_var_out
             t0 = __ldg(tb);                                                       // time origin (reading G6)
         } else {

@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(US_THREADS, MINB) accum_umma_small_kernel(cons
             #pragma unroll
             for (int i = 0; i < US_GEN_WARPS; ++i) q2 += red[i];
             asm volatile("bar.sync 1, %0;" :: "n"(US_GEN_WARPS * 32) : "memory");   // `red` is the record tile from here on
-            if (tid == 0 && sp == 0 && fb == 0) { p.part_var_out[b] = q2; p.peak64[b] = 0ull; p.counter[b] = 0u; }
+            if (tid == 0 && sp == 0 && fb == 0) { p.part_var_out[b] = q2; p.part_sum_out[b] = sum; p.peak64[b] = 0ull; p.counter[b] = 0u; }
             xs = (tid < UM_TS) ? x_scale(&q2, 1, p.Nt) : 0.f;           // the finish step recomputes exactly this from part_var_out
             t0 = __ldg(tb);                                             // time origin (reading G6)
         } else {

@@ -53,7 +53,7 @@ struct RefineSrc {
 
 constexpr int REFINE_SPLIT_ENTRIES = 256;   // refine_kernel: up to this many listed frequencies of long series are each spread over ...
 constexpr int REFINE_MAX_SPLIT = 64;        // ... up to this many blocks (ranges of samples), REFINE_SPLIT_MIN samples or more each
-constexpr int REFINE_SPLIT_MIN = 4096;
+constexpr int REFINE_SPLIT_MIN = 1024;      // (fp64 sincospi is slow on this part: 1,000 samples per block take ~1 us)
 constexpr int REFINE_WARP_MAX_NT = 4096;   // refine_kernel: series no longer than this get a warp per listed frequency instead of a block
 
 struct RefineList {

@@ -51,6 +51,7 @@ struct UmmaParams {
     const float* x; int64_t x_stride;
     double f_min, df;
     double* part_var_out;       // [B]: sum (x - mean)^2, written by the series' first CTA for the finish step (nparts = 1)
+    double* part_sum_out;       // [B]: sum x, likewise (refine_kernel takes the mean from it)
     u64* peak64; unsigned* counter;   // [B]: reset by the series' first CTA
 };
 

@@ -179,7 +179,7 @@ def test_pair_form_ragged(lsp, Nt, Nf, nsplit, flush, table_mb):
     plan = h.last_plan()
     nchunks = 1 if not table_mb else -(-Nt // 256)
     assert plan["pipe"] == TENSOR and "pair2" in plan["kernel"] and plan["K"] == 128
-    assert plan["launches"] == (2 if Nt <= 16384 else 4) + 2 * nchunks   # short series: step 1 fused into the records kernel; long: + refine_kernel
+    assert plan["launches"] == (2 if Nt <= 2048 else (3 if Nt <= 16384 else 4)) + 2 * nchunks   # records (step 1 fused in up to 16,384 samples), finish; > 2,048 samples: + refine_kernel
 
 
 @pytest.mark.parametrize("Nt,Nf,nsplit,table_mb", [(5000, 50011, 0, 0), (4099, 40001, 2, 1), (20011, 70001, 0, 16)])

@@ -85,10 +85,11 @@ enum {
                               /* operand split are formed: 0 = one kind::f8f6f4 MMA on e5m2 copies (3 MMAs per 8 samples, the default);  */
                               /* 1 = two kind::f16 MMAs on fp16 lo parts (4 MMAs per 8 samples): every product of the sums XC, XS then   */
                               /* carries 22 significant operand bits, no less than the paper's fp32 arithmetic with SFU trig*/
-    LSP_PARAM_REFINE    = 16, /* 0 = frequencies whose sums are ill-conditioned (R > 0.8 Nt in eq. (5), less on the tensor forms at small */
-                              /* Nt: f T << 1 and the aliases of regular sampling; generalised form: determinant < 1/20) are recomputed */
-                              /* from the raw series in fp64 (default; none on a grid that starts at 1/T over irregular times);         */
-                              /* 1 = keep the value of the fp32 sums there (poor below f T ~ 0.05 on the tensor forms)                  */
+    LSP_PARAM_REFINE    = 16, /* 0 = frequencies whose sums are ill-conditioned (R > 0.8 Nt in eq. (5) on the FP32-pipe form, R > 0.45 Nt  */
+                              /* on the tensor-core forms, less below 1,000 samples: f T << 1 and the aliases of regular sampling; the     */
+                              /* generalised form by its determinant) are recomputed from the raw series in fp64 (default; none on a grid  */
+                              /* that starts at 1/T over irregular times); 1 = keep the value of the fp32 sums there (poor below           */
+                              /* f T ~ 0.5 on the tensor forms)                                                                           */
     LSP_PARAM_PDL       = 13  /* short-grid tensor path: 0 = steps 1-2 run inside the accumulate kernel when Nt <= 16,384 (two launches per  */
                               /* call) and the kernels of a call are launched as programmatic dependents (each kernel's launch and      */
                               /* set-up overlap its predecessor's tail); 1 = separate pre-pass kernels in plain stream order            */

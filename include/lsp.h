@@ -87,9 +87,10 @@ enum {
                               /* carries 22 significant operand bits, no less than the paper's fp32 arithmetic with SFU trig*/
     LSP_PARAM_REFINE    = 16, /* 0 = frequencies whose sums are ill-conditioned (R > 0.8 Nt in eq. (5) on the FP32-pipe form, R > 0.45 Nt  */
                               /* on the tensor-core forms, less below 1,000 samples: f T << 1 and the aliases of regular sampling; the     */
-                              /* generalised form by its determinant) are recomputed from the raw series in fp64 (default; none on a grid  */
-                              /* that starts at 1/T over irregular times); 1 = keep the value of the fp32 sums there (poor below           */
-                              /* f T ~ 0.5 on the tensor forms)                                                                           */
+                              /* generalised form by its determinant) are recomputed from the raw series in fp64, and on the tensor-core  */
+                              /* forms also the frequencies of strong lines (P > 0.0118 Nt, i.e. 2.4 % of the largest possible power)      */
+                              /* (default; none on a grid that starts at 1/T over irregular times of noise); 1 = keep the value of the      */
+                              /* fp32 sums there (poor below f T ~ 0.5 on the tensor forms)                                               */
     LSP_PARAM_PDL       = 13  /* short-grid tensor path: 0 = steps 1-2 run inside the accumulate kernel when Nt <= 16,384 (two launches per  */
                               /* call) and the kernels of a call are launched as programmatic dependents (each kernel's launch and      */
                               /* set-up overlap its predecessor's tail); 1 = separate pre-pass kernels in plain stream order            */

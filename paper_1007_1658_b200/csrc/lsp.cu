@@ -394,6 +394,8 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     gp.vconst = fuse ? vconst : nullptr; gp.vconst_f = vconst_f; gp.part_var = pvar; gp.P = P; gp.p_stride = p_stride;
     gp.peak_idx = peak_idx; gp.peak_val = peak_val; gp.peak64 = peak64; gp.counter = counter; gp.Nt = Nt; gp.nparts = pl.nparts;
     gp.list = rlist; gp.refine_thr = refine_thr;
+    const float refine_pow = refine ? refine_power(true, Nt, gps * SG_KS) : INFINITY;     // a time split is one accumulation window here
+    gp.refine_pow = refine_pow;
     LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
     for (int64_t band = 0; band < nbands; ++band) {
         const int64_t nb0 = band * L.band_nfb;
@@ -416,7 +418,7 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     fp.peak_idx = peak_idx; fp.peak_val = peak_val; fp.peak64 = peak64; fp.counter = counter;
     fp.Nt = Nt; fp.Nf = Nf; fp.nsplit = (int)nsplit; fp.nparts = pl.nparts;
     fp.x_scaled = 1; fp.ws1 = nullptr; fp.ws_x = ws_x; fp.x_row = x_row;
-    fp.src = src; fp.refine_amp = amp;
+    fp.src = src; fp.refine_amp = amp; fp.refine_pow = refine_pow;
     fp.list = RefineList{};
     const bool listed = refine && Nt > REFINE_LIST_MIN_NT;
     if (listed) { rc = refine_list(h, fp.list); if (rc != LSP_OK) return rc; pl.launches += 1; }
@@ -574,6 +576,9 @@ int run_device(lsp_ctx* h,
     // (tc_trunc_comp); on series with a trend the model is only approximate and the residual grows with the window
     const int64_t flush_default = r.pair ? 4096 : 2048;
     const int flush_ksteps = (int)(((h->opt_flush ? h->opt_flush : flush_default) + UM_KS - 1) / UM_KS);
+    // strong lines on the tensor forms are refined as well (refine_power, lsp_refine.cuh); the window is the drain window or the time split
+    const int64_t window = ((int64_t)flush_ksteps * UM_KS < pl.split_len) ? (int64_t)flush_ksteps * UM_KS : pl.split_len;
+    const float refine_pow = refine ? refine_power(tensor, Nt, window) : INFINITY;
     if (r.pair) {
         // CTA-pair form, one time chunk at a time: table pre-pass, then the accumulate launch(es) that read it
         const int64_t half_stride = L.tab_groups * (int64_t)UP_GROUP_BYTES;
@@ -631,7 +636,7 @@ int run_device(lsp_ctx* h,
                     dp.fuse = r.duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
                     dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
                     dp.list = rlist;
-                    dp.refine_r2 = INFINITY;
+                    dp.refine_r2 = INFINITY; dp.refine_pow = rlist.head ? refine_pow : INFINITY;
                     if (rlist.head) { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
                     void (*duo_kernel)(const UmmaDuoParams) = weighted ? accum_umma_duo_kernel<false, true>
                                                             : (r.fuse_pre ? accum_umma_duo_kernel<true> : accum_umma_duo_kernel<false>);
@@ -690,6 +695,7 @@ int run_device(lsp_ctx* h,
     fp.ws1 = ws1;
     fp.ws_x = nullptr; fp.x_row = 0;
     fp.src = src; fp.refine_amp = refine ? refine_amplification(tensor, Nt, gls, r.pair) : 0.0;
+    fp.refine_pow = refine_pow;
     fp.list = RefineList{};
     // generalised form: its flagged frequencies come in runs (every alias of a nightly cadence), which one finish block would redo one
     // after the other: always through the list, a block or warp per frequency (C2-shaped call: steps 6-7 0.053 -> 0.02 ms)
@@ -1101,7 +1107,7 @@ int lsp_periodogram_static(const double* t, const float* x, int64_t Nt, double f
     fp.x_scaled = 0; fp.ws1 = nullptr; fp.ws_x = nullptr; fp.x_row = 0;
     fp.src.t = t; fp.src.t_stride = Nt; fp.src.x = x; fp.src.x_stride = Nt; fp.src.w = nullptr; fp.src.w_stride = 0;
     fp.src.f_min = f_min; fp.src.df = df; fp.src.Nt = Nt;
-    fp.refine_amp = refine_amplification(false, Nt, false);
+    fp.refine_amp = refine_amplification(false, Nt, false); fp.refine_pow = INFINITY;
     fp.list = RefineList{};
     launch_finish(fp, 1, st);
     if (cudaGetLastError() != cudaSuccess) return LSP_ECUDA;

@@ -33,6 +33,7 @@ struct FinishParams {
     int64_t x_row;                     //   [nsplit][4][Nf] block shared by all series (planes 2, 3 = CC - n/2, CS); else NULL / 0
     RefineSrc src;                     // the raw series, for the ill-conditioned frequencies (lsp_refine.cuh)
     double refine_amp;                 // refine where the sums' rounding is amplified by more than this (refine_amplification); 0: nowhere
+    float refine_pow;                  // ... and where P exceeds this (refine_power: strong lines on the tensor forms); INFINITY: nowhere
     RefineList list;                   // head != NULL (long series): append the flagged frequencies here for refine_kernel (one block each,
                                        //   in parallel) instead of redoing them one after the other inside this block
 };
@@ -155,9 +156,9 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(const FinishParams 
         if (owner) Pf = (float)finish_combine(v[0], v[1], v[2], v[3], v[4], v[5], (double)p.Nt, 0.5 / s_var, gls);
         bool listed = false;                               // refine_kernel will write this frequency and enter it in the arg-max
         if (p.refine_amp > 0.0 && p.list.head) {
-            if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) listed = refine_push(p.list, b, k);
+            if (owner && (needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp) || Pf > p.refine_pow)) listed = refine_push(p.list, b, k);
         } else if (p.refine_amp > 0.0) {                   // (uniform over the grid)
-            if (owner && needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp)) s_flag[atomicAdd(&s_nflag, 1)] = (short)fl;
+            if (owner && (needs_refine(v[2], v[3], v[4], v[5], (double)p.Nt, gls, p.refine_amp) || Pf > p.refine_pow)) s_flag[atomicAdd(&s_nflag, 1)] = (short)fl;
             __syncthreads();
             const int nflag = s_nflag;
             for (int i = 0; i < nflag; ++i) {              // the order of the list varies from run to run; each entry's result does not

@@ -40,6 +40,27 @@ __host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt, 
     return 1.0 / (1.0 - r * r);
 }
 
+// Tensor-core forms, strong lines: frequencies whose power exceeds refine_power() are refined as well.  Where the sums of a drain
+// window are coherent AND the phases move slowly across it (time-sorted samples, f T (window / Nt) < ~1: a trend, a period comparable
+// to the span), the products of an MMA come in two families, X cos a cos b and -X sin a sin b, whose signs are fixed over the window:
+// the tensor core's per-product truncation then cancels between them or adds up, which the compensation model (tc_trunc_comp: sign
+// excess from the window sum alone) cannot tell; and D_V, which has no compensation, loses in some windows and not in others.
+// Measured (Nt = 1e5, drifts of 1 ... 100 sigma over the span, slow sinusoids and parabolas of 3 ... 30 sigma; refinement by R only):
+// the error is a fraction of P_k ITSELF that saturates with the strength of the line -- CTA-pair kernel, 4,096-sample windows: 1.43e-4
+// (1.58e-4 with fp16 lo planes), 7.7e-5 where the line holds 4 % of Nt, i.e. eps(P) ~ 1.43e-4 min(1, 2.8 sqrt(P / Nt)); 2,048-sample
+// windows: 1.0e-4; short-grid kernel <= 5e-5, batch kernel <= 1.2e-5 at any strength.  Bins that are not refined are to stay within
+// 4e-5 of THEIR OWN power (max P is at least that): P_k > 0.0118 Nt is refined -- with it the CTA-pair kernel measures <= 1e-5 of
+// max P on all of those inputs.  Windows below 1,024 samples (32-sample splits of the short-grid kernel: C1, C2; short series) lose
+// less: the threshold rises with (1,024 / window)^2 and soon passes (Nt - 1)/2, the largest power there is.  On noise next to nothing
+// qualifies (P ~ Exp(1) against 0.0118 Nt: ~30 of C4's 8e6 bins, none from Nt = 2,048 on); a line of 20 % of the largest possible
+// power (C3) has its main lobe refined: tens of bins.  The FP32-pipe form has no such term (INFINITY).
+__host__ __device__ inline float refine_power(bool tensor, int64_t Nt, int64_t window_samples)
+{
+    if (!tensor || window_samples <= 0) return INFINITY;
+    const double s = window_samples >= 1024 ? 1.0 : 1024.0 / (double)window_samples;
+    return (float)(0.0118 * (double)Nt * s * s);
+}
+
 constexpr int REFINE_THREADS = 256;
 constexpr int REFINE_LIST_CAP = 1 << 20;     // entries of the list (8 bytes each: 8 MiB, allocated at the first call that needs it); overflow keeps the fp32-sum value
 

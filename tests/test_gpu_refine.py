@@ -112,7 +112,11 @@ def test_low_frequencies_every_form(lsp, name, B, Nt, shared_t, params, kernel, 
     assert e_off > 10 * e_on, (e_on, e_off)
     if "accum_z" not in plan["kernel"]:
         assert e_off > TOL
-    assert np.array_equal(P[:, 150:], P0[:, 150:])           # (f T >= 0.6: R is small, nothing is flagged, nothing changes)
+    # f T >= 0.6: R is small; only the strong bins of the tensor forms are flagged there (P > 0.0118 Nt or more: refine_power,
+    # lsp_refine.cuh), nothing else changes
+    weak = (P0[:, 150:] <= 0.0118 * Nt) if "accum_z" not in plan["kernel"] else np.ones_like(P0[:, 150:], dtype=bool)
+    assert np.array_equal(P[:, 150:][weak], P0[:, 150:][weak])
+    assert np.max(np.abs(P[:, 150:] - P0[:, 150:])) <= TOL * ref.max()
 
 
 @pytest.mark.parametrize("Nt", [2500, 20000], ids=["in-block", "listed"])
@@ -321,3 +325,40 @@ def test_series_with_a_trend(lsp, name, B, Nt, Nf, span, f_max, shared_t, params
         assert int(pi[b]) == int(np.argmax(P[b]))
     print("%s: max |dP| / max P = %.2e" % (name, worst))
     assert worst <= TOL
+
+
+STRONG_FORMS = [  # name, Nt, Nf, span, f_max, params, kernel substring
+    ("pair", 100000, 1000003, 100.0, 1.0, dict(), "accum_umma_pair2_kernel"),
+    ("pair-fp16x3", 100000, 1000003, 100.0, 1.0, dict(corr=1), "accum_umma_pair2_kernel"),
+    ("small-20k", 20000, 20000, 100.0, 0.1, dict(), "accum_umma_small_kernel"),
+]
+
+
+@pytest.mark.parametrize("kind,a", [("drift", 3.0), ("drift", 100.0), ("sine", 30.0), ("parabola", 10.0), ("drift", 0.5)],
+                         ids=["drift-3-sigma", "drift-100-sigma", "slow-sine-30-sigma", "parabola-10-sigma", "drift-half-sigma"])
+@pytest.mark.parametrize("name,Nt,Nf,span,f_max,params,kernel", STRONG_FORMS, ids=[f[0] for f in STRONG_FORMS])
+def test_strong_slow_signals(lsp, name, Nt, Nf, span, f_max, params, kernel, kind, a):
+    """Signals that are strong AND slow (a drift of many sigma, a sinusoid of 1.3 cycles over the span, a parabola; time-sorted samples):
+    every drain window of the tensor forms then sums products whose signs are fixed over the window, the case the truncation
+    compensation cannot model from the window sum alone.  Before bins with P > 0.0118 Nt were refined (refine_power, lsp_refine.cuh)
+    the CTA-pair kernel was off by 1.1e-4 ... 1.6e-4 of max P on these inputs (an error proportional to P_k itself, so the largest bins
+    carried it); now every form stays within half the tolerance.  The half-sigma drift is just below the threshold (nothing refined for
+    its power): the CTA-pair kernel measures 6.7e-5 ... 7.1e-5 there, the short-grid kernel 4.7e-5 (inside the tolerance; DESIGN.md
+    section 8)."""
+    pkg, h = lsp
+    rng = np.random.default_rng(1100 + Nt % 977 + 1)
+    tt = np.sort(rng.uniform(0.0, span, Nt))
+    sig = {"drift": a * tt / span, "sine": a * np.sin(2 * np.pi * (1.3 / span) * tt + 0.4), "parabola": a * (tt / span - 0.5) ** 2}[kind]
+    x = (rng.standard_normal(Nt) + sig).astype(np.float32)[None, :]
+    f_min, df = 0.0, f_max / (Nf - 1)
+    P, pi, pv, plan = _gpu(h, pkg, tt[None, :], x, f_min, df, Nf, **params)
+    assert kernel in plan["kernel"], plan
+    fT = np.arange(Nf) * df * span
+    low = np.where(fT < 6.0)[0]
+    ks = np.unique(np.concatenate([low[::max(1, len(low) // 500)], rng.integers(0, Nf, 100), [int(pi[0])]])).astype(np.int64)
+    ref = oracle.periodogram(tt, x[0], f_min, df, Nf, ks=ks)
+    top = max(float(ref.max()), float(P[0].max()))
+    worst = float(np.max(np.abs(P[0][ks] - ref))) / top
+    print("%s, %s %g sigma: max P = %.4g (%.1f %% of (Nt - 1)/2), max |dP| / max P = %.2e" % (name, kind, a, top, 200.0 * top / (Nt - 1), worst))
+    assert int(pi[0]) == int(np.argmax(P[0])) and float(pv[0]) == float(P[0].max())
+    assert worst <= (0.5 * TOL if a >= 1.0 else TOL)

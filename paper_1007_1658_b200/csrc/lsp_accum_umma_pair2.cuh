@@ -86,6 +86,20 @@ constexpr size_t U2_SMEM = (size_t)U2_STAGES * U2_STAGE_BYTES + U2_REC_BYTES + 2
 // table[r][g][plane][chunk][l & 127][16 bytes], r = l >> 7: plane 0 = (c, s) fp16, 1 = [e5m2(c_h, s_h) | e5m2(c - c_h, s - s_h)],
 // 2 = (cos 2b, sin 2b) fp16; b = 2 pi frac(l v_j).  grid (ngroups, series), 512 threads = 2 K-chunks x 256 fine indices;
 // group g holds samples j0 + 8g .. j0 + 8g + 7 of the chunk [j0, j1).
+__device__ __forceinline__ unsigned u2_hash(unsigned x)
+{
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+// two fp32 -> packed fp16 pair, each rounded stochastically: r supplies 13 random bits per value (below the 10 mantissa bits fp16 keeps of
+// the 23), then round toward zero.  (fp16 subnormals, |x| < 6.1e-5, are cut with a coarser step than 13 bits: an error below 6e-8, no matter.)
+__device__ __forceinline__ unsigned pack_h2_sr(float lo, float hi, unsigned r)
+{
+    const float a = __uint_as_float(__float_as_uint(lo) + (r & 0x1fffu));
+    const float b = __uint_as_float(__float_as_uint(hi) + ((r >> 13) & 0x1fffu));
+    const __half2 h = __floats2half2_rn(__uint_as_float(__float_as_uint(a) & 0xffffe000u), __uint_as_float(__float_as_uint(b) & 0xffffe000u));
+    return *reinterpret_cast<const unsigned*>(&h);
+}
 __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2* __restrict__ recB, int64_t j0, int64_t j1, int64_t rec_stride,
                                                                unsigned char* __restrict__ table, int64_t half_stride, int64_t table_stride, int corr16)
 {
@@ -106,7 +120,13 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
         l8[i] = pack_e5m2(c - hf.x, s - hf.y);
         l16[i] = pack_h2(c - hf.x, s - hf.y);
         const float cc = c + c;
-        vv[i] = pack_h2(fmaf(cc, c, -1.f), cc * s);
+        // e^{2ib} to fp16 by STOCHASTIC rounding (13 pseudo-random bits under the fp16 mantissa, then truncation).  D_V has one fp16 pass, and
+        // where b hardly moves over the series (l df T << 1: the low frequencies) round-to-nearest makes the SAME error in every sample --
+        // cos 2b within one or two fp16 steps of 1 -- which sums coherently: |dV| = 2.8e-5 Nt at f T = 0.54 on the probe of DESIGN.md section 8,
+        // i.e. 5e-5 ... 7e-5 of P_k on ANY series.  Unbiased rounding makes the errors independent: 5e-7 Nt there.  Deterministic (a hash of
+        // the sample and fine index).
+        const unsigned rb = u2_hash((unsigned)(j0 + g * UM_KS + chunk * 4 + i) * 256u + l);
+        vv[i] = pack_h2_sr(fmaf(cc, c, -1.f), cc * s, rb);
     }
     unsigned char* base = table + (int64_t)blockIdx.y * table_stride + (int64_t)(l >> 7) * half_stride + g * (int64_t)UP_GROUP_BYTES;
     uint4* o = reinterpret_cast<uint4*>(base);

@@ -343,8 +343,9 @@ def test_strong_slow_signals(lsp, name, Nt, Nf, span, f_max, params, kernel, kin
     compensation cannot model from the window sum alone.  Before bins with P > 0.0118 Nt were refined (refine_power, lsp_refine.cuh)
     the CTA-pair kernel was off by 1.1e-4 ... 1.6e-4 of max P on these inputs (an error proportional to P_k itself, so the largest bins
     carried it); now every form stays within half the tolerance.  The half-sigma drift is just below the threshold (nothing refined for
-    its power): the CTA-pair kernel measures 6.7e-5 ... 7.1e-5 there, the short-grid kernel 4.7e-5 (inside the tolerance; DESIGN.md
-    section 8)."""
+    its power): there the CTA-pair kernel measured 6.7e-5 ... 7.1e-5 -- an error of sum e^{2i theta}, not of the data: round-to-nearest
+    of the fine operand's fp16 (cos 2b, sin 2b) makes the same error in every sample where b hardly moves -- until the table was
+    rounded stochastically (umma_ftable_pair_kernel): 2.5e-5 ... 3.3e-5."""
     pkg, h = lsp
     rng = np.random.default_rng(1100 + Nt % 977 + 1)
     tt = np.sort(rng.uniform(0.0, span, Nt))
@@ -361,4 +362,4 @@ def test_strong_slow_signals(lsp, name, Nt, Nf, span, f_max, params, kernel, kin
     worst = float(np.max(np.abs(P[0][ks] - ref))) / top
     print("%s, %s %g sigma: max P = %.4g (%.1f %% of (Nt - 1)/2), max |dP| / max P = %.2e" % (name, kind, a, top, 200.0 * top / (Nt - 1), worst))
     assert int(pi[0]) == int(np.argmax(P[0])) and float(pv[0]) == float(P[0].max())
-    assert worst <= (0.5 * TOL if a >= 1.0 else TOL)
+    assert worst <= 0.5 * TOL

@@ -91,15 +91,6 @@ __device__ __forceinline__ unsigned u2_hash(unsigned x)
     x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
     return x;
 }
-// two fp32 -> packed fp16 pair, each rounded stochastically: r supplies 13 random bits per value (below the 10 mantissa bits fp16 keeps of
-// the 23), then round toward zero.  (fp16 subnormals, |x| < 6.1e-5, are cut with a coarser step than 13 bits: an error below 6e-8, no matter.)
-__device__ __forceinline__ unsigned pack_h2_sr(float lo, float hi, unsigned r)
-{
-    const float a = __uint_as_float(__float_as_uint(lo) + (r & 0x1fffu));
-    const float b = __uint_as_float(__float_as_uint(hi) + ((r >> 13) & 0x1fffu));
-    const __half2 h = __floats2half2_rn(__uint_as_float(__float_as_uint(a) & 0xffffe000u), __uint_as_float(__float_as_uint(b) & 0xffffe000u));
-    return *reinterpret_cast<const unsigned*>(&h);
-}
 __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2* __restrict__ recB, int64_t j0, int64_t j1, int64_t rec_stride,
                                                                unsigned char* __restrict__ table, int64_t half_stride, int64_t table_stride, int corr16)
 {
@@ -126,7 +117,7 @@ __global__ void __launch_bounds__(512) umma_ftable_pair_kernel(const ulonglong2*
         // i.e. 5e-5 ... 7e-5 of P_k on ANY series.  Unbiased rounding makes the errors independent: 5e-7 Nt there.  Deterministic (a hash of
         // the sample and fine index).
         const unsigned rb = u2_hash((unsigned)(j0 + g * UM_KS + chunk * 4 + i) * 256u + l);
-        vv[i] = pack_h2_sr(fmaf(cc, c, -1.f), cc * s, rb);
+        vv[i] = pack_h2_sr(fmaf(cc, c, -1.f), cc * s, rb & 0x1fffu);
     }
     unsigned char* base = table + (int64_t)blockIdx.y * table_stride + (int64_t)(l >> 7) * half_stride + g * (int64_t)UP_GROUP_BYTES;
     uint4* o = reinterpret_cast<uint4*>(base);
@@ -165,7 +156,7 @@ __device__ __forceinline__ void u2_gen(const float4* rec, int s0, unsigned h, ui
         float v0, v1;
         unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
         if (WEIGHTED) { v0 *= r.w; v1 *= r.w; }                         // V = sum_j w_j e^{2i theta}
-        vv[i] = pack_h2(v0, v1);
+        vv[i] = pack_h2(v0, v1);                                        // (rounded stochastically like the table's plane: measured no gain, +1 %)
         if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
     unsigned q0 = 0u, q1 = 0u, q2 = 0u, q3 = 0u;

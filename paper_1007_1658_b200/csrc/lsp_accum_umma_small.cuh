@@ -47,7 +47,8 @@ __device__ __forceinline__ void um_gen_a(const float4* rec, int s0, unsigned h, 
         float v0, v1;
         unpack2(fma2(pack2(c, c), cs, pack2(-0.5f, 0.f)), v0, v1);      // (cos^2 a - 1/2, cos a sin a) = e^{2ia} / 2
         if (WEIGHTED) { const float wv = recw[s0 + i]; v0 *= wv; v1 *= wv; }   // V = sum_j w_j e^{2i theta} (broadcast read)
-        vv[i] = pack_h2(v0, v1);
+        // stochastic rounding; the random bits are the low mantissa bits of X cos a (X is data: they are noise)
+        vv[i] = pack_h2_sr(v0, v1, __float_as_uint(xc) & 0x1fffu);
         if (TAIL && i >= nvalid) vv[i] = 0u;                            // pads (X = 0) must not count in V either
     }
     sts128(sA, hi[0], hi[1], hi[2], hi[3]);

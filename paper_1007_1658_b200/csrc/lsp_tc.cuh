@@ -71,6 +71,15 @@ __device__ __forceinline__ unsigned pack_h2(float lo, float hi)
     const __half2 h = __floats2half2_rn(lo, hi);
     return *reinterpret_cast<const unsigned*>(&h);
 }
+// Two fp32 -> packed fp16 pair rounded STOCHASTICALLY: the 13 bits `r` (< 2^13) go under the 10 mantissa bits fp16 keeps of fp32's 23, then
+// round toward zero.  Unbiased: the rounding errors of an operand that hardly changes from sample to sample (e^{2ia} at low frequencies)
+// no longer add up coherently in the one-pass sum D_V.  (fp16 subnormals are cut more coarsely than 13 bits: < 6e-8.)
+__device__ __forceinline__ unsigned pack_h2_sr(float lo, float hi, unsigned r)
+{
+    unsigned d;
+    asm("cvt.rz.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(__uint_as_float(__float_as_uint(hi) + r)), "f"(__uint_as_float(__float_as_uint(lo) + r)));
+    return d;
+}
 __device__ __forceinline__ float2 unpack_h2(unsigned v)
 {
     return __half22float2(*reinterpret_cast<const __half2*>(&v));

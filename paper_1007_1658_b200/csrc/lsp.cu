@@ -395,7 +395,6 @@ int run_device_shared(lsp_ctx* h, const double* t, const float* x, int64_t x_str
     gp.peak_idx = peak_idx; gp.peak_val = peak_val; gp.peak64 = peak64; gp.counter = counter; gp.Nt = Nt; gp.nparts = pl.nparts;
     gp.list = rlist; gp.refine_thr = refine_thr;
     const float refine_pow = refine ? refine_power(true, Nt, gps * SG_KS) : INFINITY;     // a time split is one accumulation window here
-    gp.refine_pow = refine_pow;
     LSP_CUDA(h, cudaFuncSetAttribute(shared_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SG_SMEM));
     for (int64_t band = 0; band < nbands; ++band) {
         const int64_t nb0 = band * L.band_nfb;
@@ -636,7 +635,7 @@ int run_device(lsp_ctx* h,
                     dp.fuse = r.duo_fuse ? 1 : 0; dp.P = P; dp.p_stride = p_stride;
                     dp.peak_idx = peak_idx; dp.peak_val = peak_val; dp.peak64 = peak64; dp.counter = counter;
                     dp.list = rlist;
-                    dp.refine_r2 = INFINITY; dp.refine_pow = rlist.head ? refine_pow : INFINITY;
+                    dp.refine_r2 = INFINITY;
                     if (rlist.head) { const double thr = (1.0 - 1.0 / refine_amplification(true, Nt)) * (double)Nt; dp.refine_r2 = (float)(thr * thr); }
                     void (*duo_kernel)(const UmmaDuoParams) = weighted ? accum_umma_duo_kernel<false, true>
                                                             : (r.fuse_pre ? accum_umma_duo_kernel<true> : accum_umma_duo_kernel<false>);

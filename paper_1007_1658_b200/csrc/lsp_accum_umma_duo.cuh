@@ -91,7 +91,6 @@ struct UmmaDuoParams {
     int32_t* peak_idx; float* peak_val; u64* peak64; unsigned* counter;   // nullable (all or none)
     RefineList list;                // fused epilogue: where the ill-conditioned frequencies go (lsp_refine.cuh); head NULL: nowhere
     float refine_r2;                //   ... those with R^2 above this (refine_amplification); +inf: none
-    float refine_pow;               //   ... and those with P above this (refine_power); +inf: none
 };
 
 // Steps 6-7 in the epilogue (same arithmetic as finish_kernel, eqs (5)-(7) PAPER.md:61-70 over the common denominator):
@@ -129,10 +128,6 @@ __device__ __forceinline__ void ud_finish16(const UmmaDuoParams& q, uint32_t tba
             const float xc2 = xc[i] * xc[i], xs2 = xs[i] * xs[i], S = xc2 + xs2;
             const float DR = fmaf(xc2 - xs2, A, 2.f * xc[i] * xs[i] * Bv);
             pf[i] = fmaxf(2.f * fmaf(S, Nt_f, -DR), 0.f) / fmaf(Nt_f, Nt_f, -R2) * inv2var_f;
-            if (pf[i] > q.refine_pow) {                                 // a strong line (refine_power): listed like the ill-conditioned ones
-                const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;
-                if (k < p.Nf && refine_push(q.list, db, k)) { pf[i] = 0.f; continue; }
-            }
             if (R2 > redo_r2) {
                 // ill-conditioned: listed for refine_kernel, which writes P and enters it in the arg-max; here it counts as 0
                 const int64_t k = kh + (int64_t)(l0 + c8 + i) * UD_H;

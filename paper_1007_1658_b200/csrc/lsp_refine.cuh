@@ -53,7 +53,10 @@ __host__ __device__ inline double refine_amplification(bool tensor, int64_t Nt, 
 // max P on all of those inputs.  Windows below 1,024 samples (32-sample splits of the short-grid kernel: C1, C2; short series) lose
 // less: the threshold rises with (1,024 / window)^2 and soon passes (Nt - 1)/2, the largest power there is.  On noise next to nothing
 // qualifies (P ~ Exp(1) against 0.0118 Nt: ~30 of C4's 8e6 bins, none from Nt = 2,048 on); a line of 20 % of the largest possible
-// power (C3) has its main lobe refined: tens of bins.  The FP32-pipe form has no such term (INFINITY).
+// power (C3) has its main lobe refined: tens of bins.  The FP32-pipe form has no such term (INFINITY).  Applied by finish_kernel (the
+// CTA-pair and short-grid kernels, batches with time splits); the fused epilogues of the batch kernel and of the shared-time GEMM do not
+// test for it: those kernels measure <= 1.2e-5 and <= 1.5e-5 on the same inputs at any strength (one window of <= 2,048 samples per
+// series there), and the test inside the epilogue's pipelined loop cost the shared-time GEMM half its speed at C4S.
 __host__ __device__ inline float refine_power(bool tensor, int64_t Nt, int64_t window_samples)
 {
     if (!tensor || window_samples <= 0) return INFINITY;

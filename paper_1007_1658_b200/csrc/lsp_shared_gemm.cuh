@@ -57,7 +57,6 @@ struct SharedGemmParams {
     int64_t Nt; int nparts;
     RefineList list;                // fused epilogue: where the ill-conditioned frequencies go (lsp_refine.cuh); head NULL: nowhere
     double refine_thr;              //   ... those with R > refine_thr Nt (refine_amplification)
-    float refine_pow;               //   ... and those with P above this (refine_power); +inf: none
 };
 
 // Per-frequency part of step 6 for the shared-time batch: from CC - n/2, CS (summed over the splits in fixed order)
@@ -228,8 +227,6 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
                 const float D = fmaf(xc2 - xs2, cf.x, 2.f * vc[i] * vs[i] * cf.y);
                 pf[i] = fmaf(fmaxf(S + D, 0.f), cf.z, fmaxf(S - D, 0.f) * cf.w) * inv2var_f;
                 redo |= (cf.x != cf.x);
-                // a strong line (refine_power): listed like the ill-conditioned frequencies; here it counts as 0
-                if (pf[i] > p.refine_pow && p.list.head && k0 + i < p.Nf && refine_push(p.list, b, k)) pf[i] = 0.f;     // (NaN compares false)
             }
             if (redo) {                                                 // warp-uniform (cf depends on k only)
                 #pragma unroll
@@ -242,7 +239,7 @@ __device__ __forceinline__ void sg_drain(const SharedGemmParams& p, uint32_t tme
                     pf[i] = (float)((fmax(S + D, 0.0) * __ldg(p.vconst + 2 * p.Nf + k) + fmax(S - D, 0.0) * __ldg(p.vconst + 3 * p.Nf + k)) * inv2var);
                     // R > thr Nt: 1/(Nt + R) < 1/((1 + thr) Nt)
                     // ill-conditioned: listed for refine_kernel, which writes P and enters it in the arg-max; here it counts as 0
-                    if (p.list.head && k0 + i < p.Nf && (__ldg(p.vconst + 2 * p.Nf + k) * ((1.0 + p.refine_thr) * (double)p.Nt) < 1.0 || pf[i] > p.refine_pow) &&
+                    if (p.list.head && k0 + i < p.Nf && __ldg(p.vconst + 2 * p.Nf + k) * ((1.0 + p.refine_thr) * (double)p.Nt) < 1.0 &&
                         refine_push(p.list, b, k)) pf[i] = 0.f;
                 }
             }

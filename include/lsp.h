@@ -91,6 +91,10 @@ enum {
                               /* forms also the frequencies of strong lines (P > 0.0118 Nt, i.e. 2.4 % of the largest possible power)      */
                               /* (default; none on a grid that starts at 1/T over irregular times of noise); 1 = keep the value of the      */
                               /* fp32 sums there (poor below f T ~ 0.5 on the tensor forms)                                               */
+    LSP_PARAM_ORDER     = 17, /* tensor-core forms: 0 = the per-sample records are laid out in a golden-ratio stride order, so that every      */
+                              /* accumulation window holds samples from all over the time span (a strong trend or slow signal, inside the   */
+                              /* grid or below it, then no longer makes the tensor core's truncating accumulator swing: DESIGN.md section   */
+                              /* 8) (default); 1 = in the order given                                                                      */
     LSP_PARAM_PDL       = 13  /* short-grid tensor path: 0 = steps 1-2 run inside the accumulate kernel when Nt <= 16,384 (two launches per  */
                               /* call) and the kernels of a call are launched as programmatic dependents (each kernel's launch and      */
                               /* set-up overlap its predecessor's tail); 1 = separate pre-pass kernels in plain stream order            */

@@ -14,7 +14,7 @@ from . import build as _build
 
 LSP_OK, LSP_EINVAL, LSP_ECUDA, LSP_ENOMEM, LSP_ELIMIT = 0, -1, -2, -3, -4
 STATIC_SCRATCH_BYTES, STATIC_MAX_NT, STATIC_MAX_NF = 8 << 20, 16384, 262144
-PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_PIPE, PARAM_FLUSH, PARAM_TIMING, PARAM_TABLE_MB, PARAM_COARSE, PARAM_TRUNC, PARAM_SHARED, PARAM_PDL, PARAM_CORR, PARAM_REFINE = 1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15, 16
+PARAM_K, PARAM_THREADS, PARAM_NSPLIT, PARAM_PIPE, PARAM_FLUSH, PARAM_TIMING, PARAM_TABLE_MB, PARAM_COARSE, PARAM_TRUNC, PARAM_SHARED, PARAM_PDL, PARAM_CORR, PARAM_REFINE, PARAM_ORDER = 1, 2, 3, 4, 5, 6, 7, 8, 9, 11, 13, 15, 16, 17
 PIPE_AUTO, PIPE_FP32, PIPE_TENSOR = 0, 1, 2
 
 # every symbol include/lsp.h declares (checked by tests/test_abi.py against the header text)

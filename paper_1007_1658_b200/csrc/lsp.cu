@@ -44,7 +44,7 @@ struct lsp_ctx {
     int sm_count = 148;
     int last_cuda = 0;
     // tunables (0 = automatic)
-    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0, opt_corr = 0, opt_refine = 0;
+    int64_t opt_K = 0, opt_T = 0, opt_nsplit = 0, opt_pipe = 0, opt_flush = 0, opt_timing = 0, opt_table_mb = 0, opt_coarse = 0, opt_trunc = 0, opt_shared = 0, opt_pdl = 0, opt_corr = 0, opt_refine = 0, opt_order = 0;
     cudaEvent_t ev[TIMING_RING][5] = {};                  // ring of per-call event sets (LSP_PARAM_TIMING)
     cudaEvent_t evc[TIMING_RING][2 * TIMING_MAX_CHUNKS] = {};   // accumulate launches of a chunked call, begin / end per chunk
     int ev_chunks[TIMING_RING] = {};
@@ -541,6 +541,7 @@ int run_device(lsp_ctx* h,
     dim3 gpre((unsigned)pl.nparts, (unsigned)B);
     const bool fused_pre = pl.fused_pre && !weighted;      // short series: step 1's sum inside the records kernel
     const int TRIG = tensor ? 0 : 1;                       // (cos d_j, sin d_j) of the FP32-pipe form's recurrence
+    const int64_t order_stride = (tensor && h->opt_order != 1) ? record_order_stride(Nt) : 1;   // tensor forms: samples in a golden-ratio stride order (lsp_prepass.cuh)
     if (r.fuse_pre) {                                     // (done by the accumulate kernel itself)
         if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
     } else {
@@ -549,9 +550,9 @@ int run_device(lsp_ctx* h,
         LSP_CUDA(h, cudaGetLastError());
     } else pl.launches -= 1;
     if (timing) LSP_CUDA(h, cudaEventRecord(ev[1], st));
-    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar, origin_offset(f_min, df, Nf), TRIG);
-    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
-    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG);
+    if (weighted) records_weighted_kernel<<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, w, w_stride, Nt, pl.part_chunk, f_min, df, psum, pw, recA, recA1, recB, pvar, origin_offset(f_min, df, Nf), TRIG, order_stride);
+    else if (fused_pre) records_kernel<false, true><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG, order_stride);
+    else records_kernel<false, false><<<gpre, 256, 0, st>>>(t, t_stride, x, x_stride, Nt, pl.part_chunk, f_min, df, psum, recA, recB, pvar, peak64, counter, origin_offset(f_min, df, Nf), TRIG, order_stride);
     LSP_CUDA(h, cudaGetLastError());
     }
     if (weighted && !r.gls_fused) pl.launches -= 1;       // (the weight records were written by records_weighted_kernel)
@@ -838,6 +839,7 @@ int lsp_set_param(lsp_handle h, int key, int64_t value)
         case LSP_PARAM_TABLE_MB:   if (value > (1 << 20)) return LSP_EINVAL; h->opt_table_mb = value; break;
         case LSP_PARAM_COARSE:     if (value && value != 16 && value != 32 && value != 64 && value != 128) return LSP_EINVAL; h->opt_coarse = value; break;
         case LSP_PARAM_TRUNC:      if (value > 4000) return LSP_EINVAL; h->opt_trunc = value; break;
+        case LSP_PARAM_ORDER:      if (value > 1) return LSP_EINVAL; h->opt_order = value; break;
         case LSP_PARAM_SHARED:     if (value > 2) return LSP_EINVAL; h->opt_shared = value; break;
         case LSP_PARAM_PDL:        if (value > 1) return LSP_EINVAL; h->opt_pdl = value; break;
         case LSP_PARAM_CORR:       if (value > 1) return LSP_EINVAL; h->opt_corr = value; break;
@@ -860,6 +862,7 @@ int lsp_get_param(lsp_handle h, int key, int64_t* value)
         case LSP_PARAM_TABLE_MB:   *value = h->opt_table_mb; break;
         case LSP_PARAM_COARSE:     *value = h->opt_coarse; break;
         case LSP_PARAM_TRUNC:      *value = h->opt_trunc; break;
+        case LSP_PARAM_ORDER:      *value = h->opt_order; break;
         case LSP_PARAM_SHARED:     *value = h->opt_shared; break;
         case LSP_PARAM_PDL:        *value = h->opt_pdl; break;
         case LSP_PARAM_CORR:       *value = h->opt_corr; break;

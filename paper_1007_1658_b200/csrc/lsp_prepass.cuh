@@ -54,6 +54,25 @@ __global__ void moments_kernel(const float* __restrict__ x, int64_t x_stride, in
     }
 }
 
+// Record order of the tensor-core forms.  The sums of eq. (8) do not care in which order the samples are added, the tensor core's
+// round-toward-zero accumulator does: with time-sorted samples a strong slow component of the series (a trend, a period of the order of the
+// span -- inside the frequency grid or not) makes the running accumulator of a drain window swing far from the window's final value, and
+// the truncation loss, which goes with the ulp of the RUNNING value, is not what tc_trunc_comp reads off the final one: 1.1e-4 ... 2e-4 of
+// max P on the CTA-pair kernel for a 20-sigma sinusoid of 1.7 cycles per span below the grid (Nt = 250,001; FP32 form 1.1e-5).  So the
+// records are written in a golden-ratio stride order: record i = (j S) mod Nt holds sample j, S ~ 0.618 Nt coprime to Nt -- every run of
+// consecutive records, hence every drain window and every MMA, then holds samples from all over the span (three-distance theorem: gaps of
+// ~Nt / run), the slow component enters each window with both signs and the accumulator does a random walk.  Costs one scattered 32-byte
+// write per sample in the pre-pass.
+__host__ inline int64_t record_order_stride(int64_t Nt)
+{
+    if (Nt < 64) return 1;
+    int64_t s = (int64_t)(0.6180339887498949 * (double)Nt);
+    for (;; ++s) {
+        int64_t a = s, b = Nt;
+        while (b) { const int64_t c = a % b; a = b; b = c; }
+        if (a == 1) return s;
+    }
+}
 // Weighted generalised periodogram: records of one series' chunk.  With W = sum w, wn_j = Nt w_j / W (mean weight 1):
 //   recA  = {sqrt(wn_j) (x_j - xbar_w), cos d_j, sin d_j, 2 cos d_j}   (measurement pass)
 //   recA1 = {sqrt(wn_j),                cos d_j, sin d_j, 2 cos d_j}   (weight pass: sum wn cos, sum wn sin)
@@ -67,7 +86,8 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
                                         const double* __restrict__ part_sum, const double* __restrict__ part_w,
                                         float4* __restrict__ recA, float4* __restrict__ recA1, ulonglong2* __restrict__ recB,
                                         double* __restrict__ part_var, double t_off /* origin_offset() */,
-                                        int trig /* 0: tensor-core forms, which read only .x of the records: no sincospi */)
+                                        int trig /* 0: tensor-core forms, which read only .x of the records: no sincospi */,
+                                        int64_t order_stride = 1 /* record_order_stride() */)
 {
     __shared__ double red[32];
     const int b = blockIdx.y;
@@ -87,7 +107,7 @@ __global__ void records_weighted_kernel(const double* __restrict__ t, int64_t t_
         const double d = (double)__ldg(xb + j) - mean;
         const double wn = (double)__ldg(wb + j) * wscale;
         acc += wn * d * d;
-        const int64_t o = (int64_t)b * Nt + j;
+        const int64_t o = (int64_t)b * Nt + (order_stride == 1 ? j : (int64_t)(((u64)j * (u64)order_stride) % (u64)Nt));
         const double tp = __ldg(tb + j) - t0;
         double vfrac;
         const u64 u = frac_fixed64(f_min, tp, nullptr);
@@ -116,7 +136,8 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
                                float4* __restrict__ recA, ulonglong2* __restrict__ recB,
                                double* __restrict__ part_var,
                                u64* __restrict__ peak64, unsigned* __restrict__ counter, double t_off /* origin_offset() */,
-                               int trig /* 0: tensor-core forms, which read only .x of the records: no sincospi */)
+                               int trig /* 0: tensor-core forms, which read only .x of the records: no sincospi */,
+                               int64_t order_stride = 1 /* record i = (j order_stride) mod Nt holds sample j (record_order_stride()) */)
 {
     __shared__ double red[32];
     pdl_trigger();                                         // the accumulate kernel may be scheduled now; it waits (pdl_wait) for this grid to finish
@@ -146,7 +167,7 @@ __global__ void records_kernel(const double* __restrict__ t, int64_t t_stride,
     for (int64_t j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         const double d = (double)__ldg(xb + j) - mean;
         acc += d * d;
-        const int64_t o = (int64_t)b * Nt + j;
+        const int64_t o = (int64_t)b * Nt + (order_stride == 1 ? j : (int64_t)(((u64)j * (u64)order_stride) % (u64)Nt));
         if (SHARED && b != 0) continue;                     // shared-time batch: only the variance is needed per series
         const double tp = __ldg(tb + j) - t0;
         double vfrac;

@@ -363,3 +363,32 @@ def test_strong_slow_signals(lsp, name, Nt, Nf, span, f_max, params, kernel, kin
     print("%s, %s %g sigma: max P = %.4g (%.1f %% of (Nt - 1)/2), max |dP| / max P = %.2e" % (name, kind, a, top, 200.0 * top / (Nt - 1), worst))
     assert int(pi[0]) == int(np.argmax(P[0])) and float(pv[0]) == float(P[0].max())
     assert worst <= 0.5 * TOL
+
+
+@pytest.mark.parametrize("params", [dict(), dict(corr=1)], ids=["pair", "pair-fp16x3"])
+@pytest.mark.parametrize("kind,a", [("sine", 20.0), ("drift", 30.0)], ids=["slow-sine-20-sigma", "drift-30-sigma"])
+def test_strong_slow_signal_below_the_grid(lsp, params, kind, a):
+    """A strong slow component whose frequency the grid does NOT contain (f_min T = 65; the signal has 1.7 cycles per span, or is a drift):
+    no bin holds its power, so nothing is refined for it, but every bin sees it inside each accumulation window.  With time-sorted
+    samples the tensor core's running accumulator swings with it far from the window's final value and the truncation loss is not what
+    the compensation reads off that value: 1.1e-4 ... 2.0e-4 of max P on the CTA-pair kernel (found by a randomised sweep with strong
+    signals).  The records are therefore laid out in a golden-ratio stride order (record_order_stride, lsp_prepass.cuh; LSP_PARAM_ORDER):
+    every window holds samples from all over the span.  Both orders are measured here."""
+    pkg, h = lsp
+    Nt, Nf, span, f_min, f_max = 250001, 239999, 5000.0, 0.013, 5.0
+    rng = np.random.default_rng(7)
+    tt = np.sort(rng.uniform(0.0, span, Nt))
+    sig = a * np.sin(2 * np.pi * 1.7 / span * tt + 1.0) if kind == "sine" else a * tt / span
+    x = (rng.standard_normal(Nt) + sig).astype(np.float32)[None, :]
+    df = (f_max - f_min) / (Nf - 1)
+    ks = np.unique(np.concatenate([np.arange(40), rng.integers(0, Nf, 400), np.arange(Nf - 20, Nf)])).astype(np.int64)
+    ref = oracle.periodogram(tt, x[0], f_min, df, Nf, ks=ks)
+    err = {}
+    for order in (0, 1):
+        P, pi, pv, plan = _gpu(h, pkg, tt[None, :], x, f_min, df, Nf, order=order, **params)
+        assert "accum_umma_pair2_kernel" in plan["kernel"], plan
+        err[order] = float(np.max(np.abs(P[0][ks] - ref))) / max(float(ref.max()), float(P[0].max()))
+        assert int(pi[0]) == int(np.argmax(P[0]))
+    print("%s %g sigma, %s: max |dP| / max P = %.2e in stride order, %.2e in the order given" % (kind, a, params, err[0], err[1]))
+    assert err[0] <= 0.5 * TOL
+    assert err[1] > 2.0 * err[0]

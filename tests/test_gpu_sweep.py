@@ -91,14 +91,19 @@ def test_random_calls_match_the_oracle(lsp, seed):
     assert len(forms) >= 5
 
 
-def test_random_medium_calls_match_the_oracle_on_samples(lsp):
+@pytest.mark.parametrize("strong", [False, True], ids=["one-sigma-drift", "strong-slow-signals"])
+def test_random_medium_calls_match_the_oracle_on_samples(lsp, strong):
     """The same idea at sizes where the long-grid kernels run (Nt 20,000 ... 250,001, Nf up to 2e6; time chunks of the table, drain
     windows, forced time splits, the fp16 hi + lo corrections; regular and random sampling; half of the series with a drift, whose
     coherent low-frequency sums found the weaknesses documented in tests/test_gpu_refine.py::test_series_with_a_trend): compared
-    with the oracle on the first and last 40 bins, 300 random bins and +-20 bins around the GPU's peak of every series."""
+    with the oracle on the first and last 40 bins, 300 random bins and +-20 bins around the GPU's peak of every series.
+    `strong`: drifts up to 30 sigma, slow sinusoids (0.3 ... 6 cycles per span) up to 20 sigma and parabolas instead -- most of them BELOW
+    the grid; this mix found that time-sorted samples let the tensor core's accumulator swing with a strong slow component (8 of 600
+    calls at 1.0e-4 ... 4.2e-4 of max P before the records were laid out in stride order: test_gpu_refine.py::
+    test_strong_slow_signal_below_the_grid)."""
     import torch
     pkg, h = lsp
-    rng = np.random.default_rng(2024)
+    rng = np.random.default_rng(2025 if strong else 2024)
     worst_overall, worst_desc = 0.0, ""
     for case in range(40):
         B = int(rng.choice([1, 1, 1, 2, 3, 5]))
@@ -118,7 +123,12 @@ def test_random_medium_calls_match_the_oracle_on_samples(lsp):
             tt = rng.uniform(0, span, (nt_rows, Nt))
         tt = np.sort(tt, axis=1)
         tfull = np.broadcast_to(tt, (B, Nt)) if shared else tt
-        x = (rng.standard_normal((B, Nt)) + 0.1 * np.sin(2 * np.pi * 0.37 * tfull) + float(rng.choice([0.0, 1.0])) * tfull / span).astype(np.float32)
+        if strong:
+            x = (rng.standard_normal((B, Nt)) + 0.1 * np.sin(2 * np.pi * 0.37 * tfull) + float(rng.choice([0.0, 0.5, 1.0, 3.0, 30.0])) * tfull / span
+                 + float(rng.choice([0.0, 0.0, 2.0, 20.0])) * np.sin(2 * np.pi * rng.uniform(0.3, 6.0) / span * tfull + 1.0)
+                 + float(rng.choice([0.0, 0.0, 0.0, 5.0])) * (tfull / span - 0.4) ** 2).astype(np.float32)
+        else:
+            x = (rng.standard_normal((B, Nt)) + 0.1 * np.sin(2 * np.pi * 0.37 * tfull) + float(rng.choice([0.0, 1.0])) * tfull / span).astype(np.float32)
         f_min = float(rng.choice([0.0, 1.0 / span, 0.013]))
         f_max = float(rng.choice([1.0, 5.0, Nt / span / 2, Nt / span]))
         df = (f_max - f_min) / (Nf - 1)
